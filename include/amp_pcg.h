@@ -1,0 +1,175 @@
+/* ===========================================================================================
+ * amp_pcg.h — C ABI of the B200-native AMP-PCG iteration loop.
+ *
+ * Method: Guo, de Sturler, Warburton, "An adaptive mixed-precision and dynamically scaled
+ * preconditioned conjugate gradient algorithm", arXiv 2505.04155 (PAPER.md in this task):
+ *   problem statement  SPD  A x = b, preconditioner M, x0, relative-residual tol, maxit
+ *   PCG                Algorithm 3.1
+ *   dynamic scaling    Algorithm 3.2, Theorem 3.2
+ *   AMP-PCG(u0)        Algorithm 4.1
+ *   precision selector eq. (4.1)
+ *   indicators eta_k   eq. (4.9)+(4.10) "delay", eq. (4.11) "linear"
+ *   defaults           d=10, C=1, ell=5, tau_zs=1e-4, tau_zh=1e-6
+ *
+ * Every step of the loop (SpMV, Jacobi apply + scaling + cast + (r,z), p update, x/r update +
+ * ||r|| + precision bookkeeping) runs in hand-written sm_100a CUDA kernels inside this
+ * library; convergence, precision switches and breakdown are decided from device-side scalars
+ * and the loop is one CUDA-graph launch (WHILE conditional node) or one persistent
+ * cooperative kernel, so the host is not synchronised until the solve has ended.
+ * There is no CPU fallback: every entry point fails with AMP_ERR_CUDA if no device is usable.
+ *
+ * Pointer convention: unless a parameter is marked HOST, every pointer is a DEVICE pointer
+ * (e.g. torch-allocated), 16-byte aligned, valid on the device current at amp_pcg_create().
+ * All functions are thread-compatible (one handle = one thread at a time), not thread-safe.
+ * =========================================================================================== */
+#ifndef AMP_PCG_H_
+#define AMP_PCG_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct amp_pcg amp_pcg_t; /* opaque solver handle */
+
+/* preconditioner M: the paper uses M = I for its small examples and Jacobi for
+ * the timed GPU example */
+enum { AMP_PRECOND_NONE = 0, AMP_PRECOND_JACOBI = 1 };
+/* storage / working precisions u_z, u_r */
+enum { AMP_FP64 = 0, AMP_FP32 = 1, AMP_FP16 = 2 };
+/* indicator used by the u_r switch */
+enum { AMP_ETA_DELAY = 0 /* (4.9)+(4.10) */, AMP_ETA_LINEAR = 1 /* (4.11) */, AMP_ETA_NEVER = 2 /* u_r stays FP64 */ };
+/* scaling factor omega_k of Algorithm 3.2 ("other scaling factors can be used") */
+enum {
+  AMP_SCALE_NORM2 = 0, /* omega = 1/||r_k||                 (Algorithm 4.1 line 4) — default */
+  AMP_SCALE_RMS = 1,   /* omega = sqrt(n)/||r_k||            */
+  AMP_SCALE_POW2 = 2,  /* omega = 2^round(log2(1/||r_k||))   (exact scaling) */
+  AMP_SCALE_NONE = 3   /* omega = 1                          (diagnostic: naive low precision) */
+};
+/* how the iteration loop is driven (execution choice; does not change the arithmetic) */
+enum {
+  AMP_LOOP_AUTO = 0,       /* persistent kernel when the problem fits its limits, else graph */
+  AMP_LOOP_STREAM = 1,     /* plain stream launches in batches; host polls a device flag between batches */
+  AMP_LOOP_GRAPH = 2,      /* one CUDA graph launch: WHILE conditional node around the 4 kernels */
+  AMP_LOOP_PERSISTENT = 3  /* one cooperative kernel, grid barriers between the phases */
+};
+
+/* return / status codes */
+enum {
+  AMP_OK = 0,             /* converged: ||r_k|| <= stop_safety * tol * ||b||  (Alg 4.1 line 18) */
+  AMP_MAXIT = 1,          /* maxit reached; x holds the last iterate, stats are valid */
+  AMP_ERR_INVALID = -1,   /* invalid argument (see each function) */
+  AMP_ERR_BREAKDOWN = -2, /* gamma <= 0, rho <= 0 or a non-finite scalar: A not SPD, or FP16 overflow */
+  AMP_ERR_CUDA = -3,      /* CUDA error or no usable device; see amp_pcg_last_error() */
+  AMP_ERR_NOMEM = -4      /* device allocation failed */
+};
+
+/* Policy of one solve.  A NULL policy means AMP-PCG(FP64) with the paper's defaults and
+ * the delay indicator.  Use amp_policy_default() to fill a struct and then edit fields. */
+typedef struct {
+  int32_t amp;        /* 0: PCG(FP64), Algorithm 3.1 exactly (no scaling, no switching); 1: Algorithm 4.1 */
+  int32_t u0;         /* AMP_FP64 -> AMP-PCG(FP64): z,p start FP64 and step down by (4.1);
+                         AMP_FP16 -> AMP-PCG(FP16): z,p in FP16 throughout */
+  int32_t eta_rule;   /* AMP_ETA_* */
+  int32_t d;          /* delay of (4.9), default 10 (1 <= d <= 64) */
+  int32_t ell;        /* window of (4.11), default 5 (1 <= ell <= 64) */
+  int32_t scale_mode; /* AMP_SCALE_* */
+  int32_t no_stop;    /* 1: ignore the stopping test, run maxit iterations (attainable-accuracy runs) */
+  int32_t x0_zero;    /* 1: caller promises x0 = 0; x is zero-filled and r0 = b without a mat-vec */
+  int32_t true_residual; /* 1: after the loop compute ||b - A x||/||b|| in FP64 (one extra FP64 SpMV, not in solve_ms) */
+  int32_t loop_mode;  /* AMP_LOOP_* */
+  double C;           /* constant of Assumption 4.1, default 1 */
+  double tau_zs;      /* u_z: FP64 -> FP32 when ||r_k||/||b|| < tau_zs, default 1e-4 (5.1) */
+  double tau_zh;      /* u_z: FP32 -> FP16 when ||r_k||/||b|| < tau_zh, default 1e-6 (5.1); 0 = never FP16 */
+  double eps32;       /* unit roundoff of FP32 in eta_k; 0 means 2^-24 */
+  double eta_safety;  /* switch u_r when eta_k <= eta_safety * tol * ||b||; 0 means 1 (paper, (4.10)) */
+  double stop_safety; /* stop when ||r_k|| <= stop_safety * tol * ||b||; 0 means 1 (paper). eta_safety = theta,
+                         stop_safety = 1 - theta enforces (3.10): ||zeta|| + ||r|| <= tol ||b|| */
+} amp_policy_t;
+
+/* Result of one solve. */
+typedef struct {
+  int32_t status;           /* same value amp_pcg_solve returns */
+  int32_t iters;            /* iterations performed (k+1 of the last executed loop index) */
+  int32_t it_ur32;          /* iteration index k at which u_r became FP32, -1 if never */
+  int32_t it_uz32;          /* iteration index k at which u_z became FP32 (or lower), -1 if never */
+  int32_t it_uz16;          /* iteration index k at which u_z became FP16, -1 if never */
+  int32_t loop_mode;        /* AMP_LOOP_* actually used */
+  double bnorm;             /* ||b||_2 */
+  double relres_updated;    /* ||r_m|| / ||b|| of the recursively updated residual */
+  double relres_true;       /* ||b - A x_m|| / ||b|| in FP64 if policy.true_residual, else -1 */
+  double solve_ms;          /* device time of setup + loop (CUDA events on the solve stream) */
+  double algorithmic_bytes; /* compulsory bytes moved by the loop: sum over iterations of the per-row byte
+                               model of DESIGN.md section 5 for the precisions in use at each iteration */
+  uint64_t fp16_subnormal;  /* FP16 stores of z,p that were subnormal / flushed to 0 / overflowed; */
+  uint64_t fp16_flushed;    /* filled only when the library is built with -DAMP_COUNT_FP16, else 0 */
+  uint64_t fp16_inf;
+} amp_stats_t;
+
+/* Fill *p with the paper's defaults: amp=1, u0=FP64, eta_rule=DELAY, d=10, ell=5, C=1,
+ * tau=(1e-4,1e-6), eps32=2^-24, safeties 1, scale NORM2, x0_zero=0, true_residual=0, loop AUTO. */
+void amp_policy_default(amp_policy_t *p);
+
+/* Build a solver for the SPD matrix A given in CSR (CSR per BASELINE.json).
+ *   n, nnz      rows (= columns) and stored entries; 0 < n, 0 <= nnz < 2^31
+ *   rowptr      int32[n+1], rowptr[0] = 0, non-decreasing, rowptr[n] = nnz
+ *   colidx      int32[nnz], 0 <= colidx < n (any order within a row; duplicates are summed by the mat-vec)
+ *   vals        float64[nnz]
+ *   precond     AMP_PRECOND_NONE (M = I) or AMP_PRECOND_JACOBI (M = diag(A); every row needs a
+ *               stored, positive diagonal entry)
+ * rowptr/colidx/vals are BORROWED: they must stay valid and unchanged until amp_pcg_destroy().
+ * The handle owns everything derived (FP32 value copy, 1/diag in FP64 and FP32, row tiles,
+ * work vectors in FP64/FP32/FP16, device state, captured graph).  Symmetry is not verified.
+ * Returns NULL on failure; amp_pcg_last_error() says why (invalid structure, CUDA, memory). */
+amp_pcg_t *amp_pcg_create(int64_t n, int64_t nnz, const int32_t *rowptr, const int32_t *colidx,
+                          const double *vals, int precond);
+
+/* Solve A x = b to ||r_k|| <= tol ||b|| (Algorithm 3.1 or 4.1 by policy).
+ *   b        float64[n], read-only
+ *   x        float64[n], in: initial guess x0, out: x_m (FP64 always)
+ *   tol      > 0 relative residual tolerance;  maxit >= 1 (<= 2^24)
+ *   policy   HOST pointer or NULL;  stats  HOST pointer or NULL
+ * ||b|| = 0 gives x = 0, status AMP_OK, 0 iterations.  If x0 already satisfies the stopping test,
+ * 0 iterations are made.  Returns the status (also in stats->status).  The call synchronises the
+ * stream once, after the loop has ended, to read the result scalars. */
+int amp_pcg_solve(amp_pcg_t *h, const double *b, double *x, double tol, int32_t maxit,
+                  const amp_policy_t *policy, amp_stats_t *stats);
+
+/* Same as amp_pcg_solve but b and x are HOST buffers (pinned memory recommended): b and x0 are
+ * copied to the device, the solve runs, x is copied back; all three inside the call. */
+int amp_pcg_solve_host(amp_pcg_t *h, const double *b_host, double *x_host, double tol, int32_t maxit,
+                       const amp_policy_t *policy, amp_stats_t *stats);
+
+/* q = A p with the loop's own SpMV kernel (step a4, Alg 4.1 line 11).
+ *   mat_prec  AMP_FP64 (original values, FP64 accumulation) or AMP_FP32 (FP32 value copy, FP32 arithmetic)
+ *   vec_prec  storage type of p: AMP_FP64 double[n], AMP_FP32 float[n], AMP_FP16 __half[n rounded up to 8]
+ *   q         mat_prec type: double[n] or float[n]
+ * Returns AMP_OK, AMP_ERR_INVALID or AMP_ERR_CUDA.  Asynchronous on the handle's stream. */
+int amp_spmv(amp_pcg_t *h, int mat_prec, int vec_prec, const void *p, void *q);
+
+/* Copy the residual-norm history ||r_t||, t = 0..iters of the last solve into HOST out[0..count);
+ * returns the number of values written (<= iters+1), or a negative error code. */
+int32_t amp_pcg_residual_history(amp_pcg_t *h, double *out_host, int32_t count);
+
+/* Run all work of this handle on the given cudaStream_t (NULL = legacy default stream). */
+int amp_pcg_set_stream(amp_pcg_t *h, void *cuda_stream);
+
+/* Number of kernel launches (graph launches count their kernel nodes once per loop iteration)
+ * made by the last solve / spmv call of this handle: bench.py's gpu_launches. */
+int64_t amp_pcg_last_launch_count(const amp_pcg_t *h);
+
+/* Release the handle and everything it owns (not the borrowed CSR arrays). NULL is ignored. */
+void amp_pcg_destroy(amp_pcg_t *h);
+
+/* Thread-local message of the last failure in this library ("" if none). */
+const char *amp_pcg_last_error(void);
+
+/* Per-row algorithmic bytes of one iteration for m = nnz/n and the given (u_z, u_r): the byte
+ * model of DESIGN.md section 5 (4-pass accounting, every vector read/written once per pass). */
+double amp_pcg_bytes_per_row(double m, int uz, int ur);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* AMP_PCG_H_ */

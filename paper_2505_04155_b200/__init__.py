@@ -1,0 +1,22 @@
+"""B200-native AMP-PCG iteration loop (arXiv 2505.04155) — thin Python binding over the C ABI.
+
+Everything numerical runs inside ``libamp_pcg.so`` (hand-written sm_100a CUDA, see
+``csrc/`` and ``include/amp_pcg.h``).  This module only marshals arguments: torch tensors
+provide device memory and the current stream.  There is no CPU fallback — if the CUDA library
+or a GPU is missing, calls raise.
+"""
+from .binding import (  # noqa: F401
+    AmpPcg,
+    Policy,
+    Stats,
+    AmpPcgError,
+    bytes_per_row,
+    load_library,
+    library_path,
+    FP64, FP32, FP16,
+    ETA_DELAY, ETA_LINEAR, ETA_NEVER,
+    SCALE_NORM2, SCALE_RMS, SCALE_POW2, SCALE_NONE,
+    LOOP_AUTO, LOOP_STREAM, LOOP_GRAPH, LOOP_PERSISTENT,
+    PRECOND_NONE, PRECOND_JACOBI,
+    EXPORTED_SYMBOLS,
+)

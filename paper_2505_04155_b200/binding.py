@@ -1,0 +1,232 @@
+"""ctypes binding of include/amp_pcg.h — argument marshalling only.
+
+The names mirror the C ABI: ``AmpPcg(rowptr, colidx, vals, precond)`` = ``amp_pcg_create``,
+``.solve`` = ``amp_pcg_solve``, ``.solve_host`` = ``amp_pcg_solve_host``, ``.spmv`` =
+``amp_spmv``, ``.close`` = ``amp_pcg_destroy``.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional
+
+import numpy as np
+
+FP64, FP32, FP16 = 0, 1, 2
+ETA_DELAY, ETA_LINEAR, ETA_NEVER = 0, 1, 2
+SCALE_NORM2, SCALE_RMS, SCALE_POW2, SCALE_NONE = 0, 1, 2, 3
+LOOP_AUTO, LOOP_STREAM, LOOP_GRAPH, LOOP_PERSISTENT = 0, 1, 2, 3
+PRECOND_NONE, PRECOND_JACOBI = 0, 1
+
+EXPORTED_SYMBOLS = (
+    "amp_policy_default", "amp_pcg_create", "amp_pcg_solve", "amp_pcg_solve_host", "amp_spmv",
+    "amp_pcg_residual_history", "amp_pcg_set_stream", "amp_pcg_last_launch_count", "amp_pcg_destroy",
+    "amp_pcg_last_error", "amp_pcg_bytes_per_row",
+)
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+
+
+class AmpPcgError(RuntimeError):
+    pass
+
+
+class Policy(C.Structure):
+    """amp_policy_t (include/amp_pcg.h)."""
+
+    _fields_ = [
+        ("amp", C.c_int32), ("u0", C.c_int32), ("eta_rule", C.c_int32), ("d", C.c_int32), ("ell", C.c_int32),
+        ("scale_mode", C.c_int32), ("no_stop", C.c_int32), ("x0_zero", C.c_int32), ("true_residual", C.c_int32),
+        ("loop_mode", C.c_int32),
+        ("C", C.c_double), ("tau_zs", C.c_double), ("tau_zh", C.c_double), ("eps32", C.c_double),
+        ("eta_safety", C.c_double), ("stop_safety", C.c_double),
+    ]
+
+    @classmethod
+    def default(cls, **overrides) -> "Policy":
+        p = cls()
+        load_library().amp_policy_default(C.byref(p))
+        for k, v in overrides.items():
+            if not hasattr(p, k):
+                raise AttributeError(k)
+            setattr(p, k, v)
+        return p
+
+
+class Stats(C.Structure):
+    """amp_stats_t (include/amp_pcg.h)."""
+
+    _fields_ = [
+        ("status", C.c_int32), ("iters", C.c_int32), ("it_ur32", C.c_int32), ("it_uz32", C.c_int32),
+        ("it_uz16", C.c_int32), ("loop_mode", C.c_int32),
+        ("bnorm", C.c_double), ("relres_updated", C.c_double), ("relres_true", C.c_double),
+        ("solve_ms", C.c_double), ("algorithmic_bytes", C.c_double),
+        ("fp16_subnormal", C.c_uint64), ("fp16_flushed", C.c_uint64), ("fp16_inf", C.c_uint64),
+    ]
+
+    def asdict(self):
+        return {k: getattr(self, k) for k, _ in self._fields_}
+
+
+_lib = None
+
+
+def library_path() -> str:
+    return os.path.join(_HERE, "libamp_pcg.so")
+
+
+def load_library():
+    """dlopen the in-tree CUDA library (no build here: see build.py / __graft_entry__.build)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = library_path()
+    if not os.path.exists(path):
+        raise AmpPcgError(f"{path} is missing: build it with `python -m paper_2505_04155_b200.build` "
+                          "(there is no CPU fallback)")
+    L = C.CDLL(path)
+    vp, i32, i64, dbl = C.c_void_p, C.c_int32, C.c_int64, C.c_double
+    L.amp_policy_default.restype = None
+    L.amp_policy_default.argtypes = [C.POINTER(Policy)]
+    L.amp_pcg_create.restype = vp
+    L.amp_pcg_create.argtypes = [i64, i64, vp, vp, vp, C.c_int]
+    L.amp_pcg_solve.restype = C.c_int
+    L.amp_pcg_solve.argtypes = [vp, vp, vp, dbl, i32, C.POINTER(Policy), C.POINTER(Stats)]
+    L.amp_pcg_solve_host.restype = C.c_int
+    L.amp_pcg_solve_host.argtypes = [vp, vp, vp, dbl, i32, C.POINTER(Policy), C.POINTER(Stats)]
+    L.amp_spmv.restype = C.c_int
+    L.amp_spmv.argtypes = [vp, C.c_int, C.c_int, vp, vp]
+    L.amp_pcg_residual_history.restype = i32
+    L.amp_pcg_residual_history.argtypes = [vp, vp, i32]
+    L.amp_pcg_set_stream.restype = C.c_int
+    L.amp_pcg_set_stream.argtypes = [vp, vp]
+    L.amp_pcg_last_launch_count.restype = i64
+    L.amp_pcg_last_launch_count.argtypes = [vp]
+    L.amp_pcg_destroy.restype = None
+    L.amp_pcg_destroy.argtypes = [vp]
+    L.amp_pcg_last_error.restype = C.c_char_p
+    L.amp_pcg_last_error.argtypes = []
+    L.amp_pcg_bytes_per_row.restype = dbl
+    L.amp_pcg_bytes_per_row.argtypes = [dbl, C.c_int, C.c_int]
+    _lib = L
+    return L
+
+
+def bytes_per_row(m: float, uz: int, ur: int) -> float:
+    return float(load_library().amp_pcg_bytes_per_row(float(m), int(uz), int(ur)))
+
+
+def _last_error() -> str:
+    return load_library().amp_pcg_last_error().decode("utf-8", "replace")
+
+
+class AmpPcg:
+    """One SPD matrix in CSR on the current CUDA device (amp_pcg_create ... amp_pcg_destroy).
+
+    ``rowptr`` (int32[n+1]), ``colidx`` (int32[nnz]) and ``vals`` (float64[nnz]) are CUDA torch
+    tensors; they are borrowed by the library, so this object keeps references to them.
+    """
+
+    def __init__(self, rowptr, colidx, vals, precond: int = PRECOND_JACOBI):
+        import torch
+
+        if not (rowptr.is_cuda and colidx.is_cuda and vals.is_cuda):
+            raise AmpPcgError("AmpPcg needs CUDA tensors (there is no CPU fallback)")
+        if rowptr.dtype != torch.int32 or colidx.dtype != torch.int32 or vals.dtype != torch.float64:
+            raise AmpPcgError("rowptr/colidx must be int32 and vals float64")
+        self._keep = (rowptr.contiguous(), colidx.contiguous(), vals.contiguous())
+        self.n = int(rowptr.numel() - 1)
+        self.nnz = int(colidx.numel())
+        self.device = vals.device
+        self._torch = torch
+        L = load_library()
+        with torch.cuda.device(self.device):
+            self._h = L.amp_pcg_create(self.n, self.nnz, self._keep[0].data_ptr(), self._keep[1].data_ptr(),
+                                       self._keep[2].data_ptr(), int(precond))
+        if not self._h:
+            raise AmpPcgError(_last_error())
+
+    # -- helpers --------------------------------------------------------------------------
+    def _sync_stream(self):
+        s = self._torch.cuda.current_stream(self.device).cuda_stream
+        load_library().amp_pcg_set_stream(self._h, C.c_void_p(s))
+
+    def _check(self, rc: int, allow=(0, 1, -2)):
+        if rc not in allow:
+            raise AmpPcgError(f"amp_pcg error {rc}: {_last_error()}")
+
+    # -- C ABI ----------------------------------------------------------------------------
+    def solve(self, b, x, tol: float, maxit: int, policy: Optional[Policy] = None) -> Stats:
+        """amp_pcg_solve: b, x float64 CUDA tensors of length n; x is x0 on entry, x_m on exit."""
+        torch = self._torch
+        if b.dtype != torch.float64 or x.dtype != torch.float64 or not b.is_cuda or not x.is_cuda:
+            raise AmpPcgError("b and x must be float64 CUDA tensors")
+        if b.numel() != self.n or x.numel() != self.n or not b.is_contiguous() or not x.is_contiguous():
+            raise AmpPcgError("b and x must be contiguous with n elements")
+        st = Stats()
+        with torch.cuda.device(self.device):
+            self._sync_stream()
+            rc = load_library().amp_pcg_solve(self._h, b.data_ptr(), x.data_ptr(), float(tol), int(maxit),
+                                              C.byref(policy) if policy is not None else None, C.byref(st))
+        self._check(rc)
+        self._last_iters = int(st.iters)
+        return st
+
+    def solve_host(self, b_host, x_host, tol: float, maxit: int, policy: Optional[Policy] = None) -> Stats:
+        """amp_pcg_solve_host: b, x are HOST float64 buffers (pinned torch tensors or numpy arrays)."""
+        st = Stats()
+        bp = b_host.data_ptr() if hasattr(b_host, "data_ptr") else b_host.ctypes.data
+        xp = x_host.data_ptr() if hasattr(x_host, "data_ptr") else x_host.ctypes.data
+        with self._torch.cuda.device(self.device):
+            self._sync_stream()
+            rc = load_library().amp_pcg_solve_host(self._h, bp, xp, float(tol), int(maxit),
+                                                   C.byref(policy) if policy is not None else None, C.byref(st))
+        self._check(rc)
+        self._last_iters = int(st.iters)
+        return st
+
+    def spmv(self, p, mat_prec: int = FP64, out=None):
+        """amp_spmv: q = A p.  p: float64/float32/float16 CUDA tensor (float16: length padded to 8)."""
+        torch = self._torch
+        vec_prec = {torch.float64: FP64, torch.float32: FP32, torch.float16: FP16}[p.dtype]
+        if p.numel() < self.n or not p.is_contiguous():
+            raise AmpPcgError("p must be contiguous with at least n elements")
+        qdt = torch.float64 if mat_prec == FP64 else torch.float32
+        q = out if out is not None else torch.empty(self.n, dtype=qdt, device=self.device)
+        if q.dtype != qdt or q.numel() < self.n:
+            raise AmpPcgError("out has the wrong dtype/size")
+        with torch.cuda.device(self.device):
+            self._sync_stream()
+            rc = load_library().amp_spmv(self._h, int(mat_prec), vec_prec, p.data_ptr(), q.data_ptr())
+        self._check(rc, allow=(0,))
+        return q
+
+    def residual_history(self) -> np.ndarray:
+        """amp_pcg_residual_history: ||r_t||, t = 0..iters of the last solve (host numpy array)."""
+        buf = np.empty(self._last_iters + 1, dtype=np.float64)
+        m = load_library().amp_pcg_residual_history(self._h, buf.ctypes.data, buf.size)
+        if m < 0:
+            raise AmpPcgError(_last_error())
+        return buf[:m]
+
+    _last_iters = -1
+
+    def last_launch_count(self) -> int:
+        return int(load_library().amp_pcg_last_launch_count(self._h))
+
+    def close(self):
+        if getattr(self, "_h", None):
+            load_library().amp_pcg_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()

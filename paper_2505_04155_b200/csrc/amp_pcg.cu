@@ -1,0 +1,451 @@
+// amp_pcg.cu — host side of the C ABI declared in include/amp_pcg.h: handle management,
+// validation, the solve drivers (stream batches / CUDA-graph WHILE loop / persistent kernel)
+// and result read-back.  All arithmetic of the method runs in the kernels of kernels.cuh.
+#include "../../include/amp_pcg.h"
+
+#include <algorithm>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "kernels.cuh"
+#include "persistent.cuh"
+
+using namespace amp;
+
+static thread_local std::string g_last_error;
+
+static void set_error(const char* fmt, ...) {
+  char buf[512];
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(buf, sizeof(buf), fmt, ap);
+  va_end(ap);
+  g_last_error = buf;
+}
+
+#define CU_TRY(call, onfail)                                                                  \
+  do {                                                                                        \
+    cudaError_t e_ = (call);                                                                  \
+    if (e_ != cudaSuccess) {                                                                  \
+      set_error("%s failed: %s (%s:%d)", #call, cudaGetErrorString(e_), __FILE__, __LINE__);   \
+      onfail;                                                                                 \
+    }                                                                                         \
+  } while (0)
+
+struct amp_pcg {
+  int64_t n = 0, nnz = 0, npad = 0;
+  int precond = 0, device = 0, num_sms = 0;
+  cudaStream_t stream = nullptr;
+  Ctx ctx{};
+  std::vector<void*> owned;     // device allocations released in destroy
+  DevState* h_state = nullptr;  // pinned staging for the state block
+  int* h_flag = nullptr;        // pinned: done flag polled by the stream loop
+  double* hist = nullptr;
+  int64_t hist_cap = 0;
+  int vec_grid = 1, spmv_grid = 1, persist_grid = 0, persist_ok = 0;
+  // graph loop
+  cudaGraph_t graph = nullptr;
+  cudaGraphExec_t graph_exec = nullptr;
+  cudaGraphConditionalHandle cond{};
+  // host-buffer staging for amp_pcg_solve_host
+  double* d_b_stage = nullptr;
+  double* d_x_stage = nullptr;
+  cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+  int64_t launches = 0;
+  int32_t last_iters = -1;
+  double m_avg = 0.0;
+};
+
+template <class T> static T* dev_alloc(amp_pcg* h, size_t count, bool zero) {
+  void* p = nullptr;
+  cudaError_t e = cudaMalloc(&p, std::max<size_t>(count, 1) * sizeof(T));
+  if (e != cudaSuccess) {
+    set_error("cudaMalloc of %zu bytes failed: %s", count * sizeof(T), cudaGetErrorString(e));
+    cudaGetLastError();
+    return nullptr;
+  }
+  h->owned.push_back(p);
+  if (zero && cudaMemsetAsync(p, 0, std::max<size_t>(count, 1) * sizeof(T), h->stream) != cudaSuccess) return nullptr;
+  return static_cast<T*>(p);
+}
+
+extern "C" const char* amp_pcg_last_error(void) { return g_last_error.c_str(); }
+
+extern "C" void amp_policy_default(amp_policy_t* p) {
+  if (!p) return;
+  std::memset(p, 0, sizeof(*p));
+  p->amp = 1; p->u0 = AMP_FP64; p->eta_rule = AMP_ETA_DELAY; p->d = 10; p->ell = 5;
+  p->scale_mode = AMP_SCALE_NORM2; p->loop_mode = AMP_LOOP_AUTO;
+  p->C = 1.0; p->tau_zs = 1e-4; p->tau_zh = 1e-6; p->eps32 = std::ldexp(1.0, -24);
+  p->eta_safety = 1.0; p->stop_safety = 1.0;
+}
+
+extern "C" double amp_pcg_bytes_per_row(double m, int uz, int ur) {
+  const double sA = (ur == AMP_FP64) ? 8.0 : 4.0, sr = sA;
+  const double sz = (uz == AMP_FP64) ? 8.0 : (uz == AMP_FP32 ? 4.0 : 2.0);
+  const double sd = (uz == AMP_FP64) ? 8.0 : 4.0;          // 1/diag copy read by the z kernel
+  const double k_spmv = m * (sA + 4.0) + 4.0 + sz + sr;    // values+indices, rowptr, p, q
+  const double k_z = sr + sd + sz;                         // r, 1/diag -> z
+  const double k_p = 3.0 * sz;                             // z, p -> p
+  const double k_xr = 16.0 + sz + sr + 2.0 * sr;           // x (r/w FP64), p, q, r (r/w)
+  return k_spmv + k_z + k_p + k_xr;
+}
+
+extern "C" void amp_pcg_destroy(amp_pcg_t* h) {
+  if (!h) return;
+  cudaSetDevice(h->device);
+  cudaStreamSynchronize(h->stream);
+  if (h->graph_exec) cudaGraphExecDestroy(h->graph_exec);
+  if (h->graph) cudaGraphDestroy(h->graph);
+  for (void* p : h->owned) cudaFree(p);
+  if (h->hist) cudaFree(h->hist);
+  if (h->h_state) cudaFreeHost(h->h_state);
+  if (h->h_flag) cudaFreeHost(h->h_flag);
+  if (h->ev0) cudaEventDestroy(h->ev0);
+  if (h->ev1) cudaEventDestroy(h->ev1);
+  delete h;
+}
+
+static bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+extern "C" amp_pcg_t* amp_pcg_create(int64_t n, int64_t nnz, const int32_t* rowptr, const int32_t* colidx,
+                                     const double* vals, int precond) {
+  g_last_error.clear();
+  if (n <= 0 || n > (int64_t)0x7fffffff - 64 || nnz < 0 || nnz > (int64_t)0x7fffffff - 64) {
+    set_error("amp_pcg_create: n and nnz must satisfy 0 < n, 0 <= nnz < 2^31 (got n=%lld nnz=%lld)", (long long)n, (long long)nnz);
+    return nullptr;
+  }
+  if (!rowptr || (nnz > 0 && (!colidx || !vals)) || (precond != AMP_PRECOND_NONE && precond != AMP_PRECOND_JACOBI)) {
+    set_error("amp_pcg_create: null pointer or unknown preconditioner %d", precond);
+    return nullptr;
+  }
+  if (!aligned16(rowptr) || !aligned16(colidx) || !aligned16(vals)) {
+    set_error("amp_pcg_create: rowptr, colidx and vals must be 16-byte aligned device pointers");
+    return nullptr;
+  }
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+    cudaGetLastError();
+    set_error("amp_pcg_create: no usable CUDA device (this library has no CPU fallback)");
+    return nullptr;
+  }
+  amp_pcg* h = new amp_pcg();
+  CU_TRY(cudaGetDevice(&h->device), { delete h; return nullptr; });
+  cudaDeviceProp prop;
+  CU_TRY(cudaGetDeviceProperties(&prop, h->device), { delete h; return nullptr; });
+  h->num_sms = prop.multiProcessorCount;
+  h->n = n; h->nnz = nnz; h->npad = (n + 7) & ~(int64_t)7; h->precond = precond;
+  h->m_avg = (double)nnz / (double)n;
+  Ctx& c = h->ctx;
+  c.n = n; c.npad = h->npad; c.nnz = nnz;
+  c.rowptr = rowptr; c.colidx = colidx; c.vals64 = vals;
+
+#define ALLOC(dst, T, count)                                            \
+  do {                                                                  \
+    dst = dev_alloc<T>(h, (count), true);                               \
+    if (!dst) { amp_pcg_destroy(h); return nullptr; }                   \
+  } while (0)
+  const size_t np = (size_t)h->npad;
+  double* dinv64; float* dinv32; float* vals32; int* flags; int32_t* tile_row;
+  ALLOC(dinv64, double, np); ALLOC(dinv32, float, np);
+  ALLOC(vals32, float, (size_t)nnz + 8);
+  ALLOC(c.r64, double, np); ALLOC(c.r32, float, np);
+  ALLOC(c.q64, double, np); ALLOC(c.q32, float, np);
+  ALLOC(c.z64, double, np); ALLOC(c.z32, float, np); ALLOC(c.z16, __half, np);
+  ALLOC(c.p64, double, np); ALLOC(c.p32, float, np); ALLOC(c.p16, __half, np);
+  ALLOC(c.partials, double, (size_t)4 * kMaxGrid);
+  ALLOC(c.st, DevState, 1);
+  ALLOC(flags, int, 1);
+  ALLOC(h->d_b_stage, double, np);
+  ALLOC(h->d_x_stage, double, np);
+  c.dinv64 = dinv64; c.dinv32 = dinv32; c.vals32 = vals32;
+  CU_TRY(cudaMallocHost(&h->h_state, sizeof(DevState)), { amp_pcg_destroy(h); return nullptr; });
+  CU_TRY(cudaMallocHost(&h->h_flag, 64), { amp_pcg_destroy(h); return nullptr; });
+  CU_TRY(cudaEventCreate(&h->ev0), { amp_pcg_destroy(h); return nullptr; });
+  CU_TRY(cudaEventCreate(&h->ev1), { amp_pcg_destroy(h); return nullptr; });
+
+  // structure check + 1/diag, FP32 value copy
+  const int vgrid = (int)std::min<int64_t>((n + 255) / 256, (int64_t)h->num_sms * 16);
+  k_validate_dinv<<<vgrid, 256, 0, h->stream>>>(n, nnz, rowptr, colidx, vals, precond == AMP_PRECOND_JACOBI, dinv64,
+                                                dinv32, flags);
+  if (nnz > 0) {
+    const int cgrid = (int)std::min<int64_t>((nnz + 255) / 256, (int64_t)h->num_sms * 16);
+    k_to_fp32<<<cgrid, 256, 0, h->stream>>>(nnz, vals, vals32);
+  }
+  std::vector<int32_t> rp((size_t)n + 1);
+  int hflags = 0;
+  CU_TRY(cudaMemcpyAsync(&hflags, flags, sizeof(int), cudaMemcpyDeviceToHost, h->stream), { amp_pcg_destroy(h); return nullptr; });
+  CU_TRY(cudaMemcpyAsync(rp.data(), rowptr, sizeof(int32_t) * ((size_t)n + 1), cudaMemcpyDeviceToHost, h->stream),
+         { amp_pcg_destroy(h); return nullptr; });
+  CU_TRY(cudaStreamSynchronize(h->stream), { amp_pcg_destroy(h); return nullptr; });
+  if (hflags) {
+    set_error("amp_pcg_create: invalid matrix:%s%s%s%s", (hflags & 1) ? " rowptr not monotone or rowptr[n] != nnz;" : "",
+              (hflags & 2) ? " column index out of range;" : "", (hflags & 4) ? " missing diagonal entry (Jacobi);" : "",
+              (hflags & 8) ? " non-positive diagonal entry (Jacobi);" : "");
+    amp_pcg_destroy(h);
+    return nullptr;
+  }
+
+  // row tiles of the SpMV: <= kTileRows rows and <= kTileNnz entries; a longer row stands alone
+  std::vector<int32_t> tiles;
+  tiles.push_back(0);
+  int64_t r = 0;
+  while (r < n) {
+    int64_t r1 = r + 1;
+    if (rp[r1] - rp[r] <= kTileNnz) {
+      while (r1 < n && r1 - r < kTileRows && rp[r1 + 1] - rp[r] <= kTileNnz) ++r1;
+    }
+    tiles.push_back((int32_t)r1);
+    r = r1;
+  }
+  c.ntiles = (int32_t)tiles.size() - 1;
+  ALLOC(tile_row, int32_t, tiles.size());
+  CU_TRY(cudaMemcpyAsync(tile_row, tiles.data(), sizeof(int32_t) * tiles.size(), cudaMemcpyHostToDevice, h->stream),
+         { amp_pcg_destroy(h); return nullptr; });
+  CU_TRY(cudaStreamSynchronize(h->stream), { amp_pcg_destroy(h); return nullptr; });
+  c.tile_row = tile_row;
+  int L = 1;  // lanes per row: about 4 entries per lane
+  while (L < 32 && L * 4 < h->m_avg) L <<= 1;
+  c.lanes_per_row = L;
+
+  // launch geometry: whole multiples of the SM count
+  CU_TRY(cudaFuncSetAttribute(k_spmv, cudaFuncAttributeMaxDynamicSharedMemorySize, kSpmvSmemBytes), { amp_pcg_destroy(h); return nullptr; });
+  int occ_spmv = 1, occ_vec = 1;
+  CU_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_spmv, k_spmv, kSpmvThreads, kSpmvSmemBytes), { amp_pcg_destroy(h); return nullptr; });
+  CU_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_vec, k_xr, kVecThreads, 0), { amp_pcg_destroy(h); return nullptr; });
+  occ_spmv = std::max(occ_spmv, 1); occ_vec = std::max(occ_vec, 1);
+  h->spmv_grid = (int)std::min<int64_t>({(int64_t)c.ntiles, (int64_t)h->num_sms * occ_spmv, (int64_t)kMaxGrid});
+  const int64_t vec_blocks = ((h->npad / 2) + (int64_t)kVecThreads * kVecUnroll - 1) / ((int64_t)kVecThreads * kVecUnroll);
+  h->vec_grid = (int)std::min<int64_t>({std::max<int64_t>(vec_blocks, 1), (int64_t)h->num_sms * occ_vec, (int64_t)kMaxGrid});
+  persistent_configure(h->num_sms, &h->persist_grid, &h->persist_ok);
+#undef ALLOC
+  return h;
+}
+
+extern "C" int amp_pcg_set_stream(amp_pcg_t* h, void* cuda_stream) {
+  if (!h) return AMP_ERR_INVALID;
+  h->stream = static_cast<cudaStream_t>(cuda_stream);
+  return AMP_OK;
+}
+
+extern "C" int64_t amp_pcg_last_launch_count(const amp_pcg_t* h) { return h ? h->launches : 0; }
+
+// ------------------------------------------------------------------ SpMV entry --------------
+template <int UR, class PT>
+static void launch_spmv_any(amp_pcg* h, const void* p, void* q) {
+  static bool attr_done = false;
+  if (!attr_done) {
+    cudaFuncSetAttribute(k_spmv_any<UR, PT>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSpmvSmemBytes);
+    attr_done = true;
+  }
+  k_spmv_any<UR, PT><<<h->spmv_grid, kSpmvThreads, kSpmvSmemBytes, h->stream>>>(
+      h->ctx, static_cast<const PT*>(p), static_cast<typename Store<UR>::T*>(q));
+}
+
+static int spmv_dispatch(amp_pcg* h, int mat_prec, int vec_prec, const void* p, void* q) {
+  if (mat_prec == AMP_FP64) {
+    if (vec_prec == AMP_FP64) launch_spmv_any<P64, double>(h, p, q);
+    else if (vec_prec == AMP_FP32) launch_spmv_any<P64, float>(h, p, q);
+    else if (vec_prec == AMP_FP16) launch_spmv_any<P64, __half>(h, p, q);
+    else return AMP_ERR_INVALID;
+  } else if (mat_prec == AMP_FP32) {
+    if (vec_prec == AMP_FP64) launch_spmv_any<P32, double>(h, p, q);
+    else if (vec_prec == AMP_FP32) launch_spmv_any<P32, float>(h, p, q);
+    else if (vec_prec == AMP_FP16) launch_spmv_any<P32, __half>(h, p, q);
+    else return AMP_ERR_INVALID;
+  } else {
+    return AMP_ERR_INVALID;
+  }
+  h->launches += 1;
+  return AMP_OK;
+}
+
+extern "C" int amp_spmv(amp_pcg_t* h, int mat_prec, int vec_prec, const void* p, void* q) {
+  g_last_error.clear();
+  if (!h || !p || !q) { set_error("amp_spmv: null argument"); return AMP_ERR_INVALID; }
+  CU_TRY(cudaSetDevice(h->device), return AMP_ERR_CUDA);
+  h->launches = 0;
+  const int rc = spmv_dispatch(h, mat_prec, vec_prec, p, q);
+  if (rc != AMP_OK) { set_error("amp_spmv: mat_prec must be FP64/FP32 and vec_prec FP64/FP32/FP16"); return rc; }
+  CU_TRY(cudaGetLastError(), return AMP_ERR_CUDA);
+  return AMP_OK;
+}
+
+// ------------------------------------------------------------------ graph loop --------------
+static void launch_iteration(amp_pcg* h, const Ctx& c, cudaStream_t s) {
+  k_z<<<h->vec_grid, kVecThreads, 0, s>>>(c);
+  k_p<<<h->vec_grid, kVecThreads, 0, s>>>(c);
+  k_spmv<<<h->spmv_grid, kSpmvThreads, kSpmvSmemBytes, s>>>(c);
+  k_xr<<<h->vec_grid, kVecThreads, 0, s>>>(c);
+}
+
+// One graph = one WHILE conditional node whose body is the four loop kernels; the condition is
+// written from the device by epi_delta / epi_gamma, so a whole solve is a single launch.
+static int build_graph(amp_pcg* h) {
+  if (h->graph_exec) return AMP_OK;
+  CU_TRY(cudaGraphCreate(&h->graph, 0), return AMP_ERR_CUDA);
+  CU_TRY(cudaGraphConditionalHandleCreate(&h->cond, h->graph, 1, cudaGraphCondAssignDefault), return AMP_ERR_CUDA);
+  cudaGraphNodeParams np = {};
+  np.type = cudaGraphNodeTypeConditional;
+  np.conditional.handle = h->cond;
+  np.conditional.type = cudaGraphCondTypeWhile;
+  np.conditional.size = 1;
+  cudaGraphNode_t node;
+  CU_TRY(cudaGraphAddNode(&node, h->graph, nullptr, 0, &np), return AMP_ERR_CUDA);
+  cudaGraph_t body = np.conditional.phGraph_out[0];
+  cudaStream_t cap;
+  CU_TRY(cudaStreamCreateWithFlags(&cap, cudaStreamNonBlocking), return AMP_ERR_CUDA);
+  Ctx c = h->ctx;
+  c.cond = h->cond;
+  c.use_cond = 1;
+  cudaError_t e = cudaStreamBeginCaptureToGraph(cap, body, nullptr, nullptr, 0, cudaStreamCaptureModeRelaxed);
+  if (e == cudaSuccess) {
+    launch_iteration(h, c, cap);
+    e = cudaStreamEndCapture(cap, nullptr);
+  }
+  cudaStreamDestroy(cap);
+  if (e != cudaSuccess) { set_error("graph capture failed: %s", cudaGetErrorString(e)); return AMP_ERR_CUDA; }
+  CU_TRY(cudaGraphInstantiate(&h->graph_exec, h->graph, 0), return AMP_ERR_CUDA);
+  return AMP_OK;
+}
+
+// ------------------------------------------------------------------ solve -------------------
+static int solve_impl(amp_pcg* h, const double* b, double* x, double tol, int32_t maxit, const amp_policy_t* policy,
+                      amp_stats_t* stats) {
+  g_last_error.clear();
+  if (!h || !b || !x) { set_error("amp_pcg_solve: null argument"); return AMP_ERR_INVALID; }
+  amp_policy_t pol;
+  if (policy) pol = *policy; else amp_policy_default(&pol);
+  if (pol.eps32 == 0.0) pol.eps32 = std::ldexp(1.0, -24);
+  if (pol.eta_safety == 0.0) pol.eta_safety = 1.0;
+  if (pol.stop_safety == 0.0) pol.stop_safety = 1.0;
+  if (pol.C == 0.0 && !policy) pol.C = 1.0;
+  if (!(tol > 0.0) || maxit < 1 || maxit > (1 << 24) || !aligned16(b) || !aligned16(x) || pol.u0 < 0 || pol.u0 > 2 ||
+      pol.eta_rule < 0 || pol.eta_rule > 2 || pol.scale_mode < 0 || pol.scale_mode > 3 || pol.d < 1 || pol.d > kMaxWindow ||
+      pol.ell < 1 || pol.ell > kMaxWindow || pol.loop_mode < 0 || pol.loop_mode > 3 || !(pol.tau_zs >= 0.0) ||
+      !(pol.tau_zh >= 0.0) || !(pol.eps32 > 0.0) || !(pol.eta_safety > 0.0) || !(pol.stop_safety > 0.0)) {
+    set_error("amp_pcg_solve: invalid tol/maxit/policy or misaligned b/x");
+    return AMP_ERR_INVALID;
+  }
+  CU_TRY(cudaSetDevice(h->device), return AMP_ERR_CUDA);
+  cudaStream_t st = h->stream;
+  if ((int64_t)maxit + 2 > h->hist_cap) {
+    if (h->hist) cudaFree(h->hist);
+    h->hist = nullptr;
+    h->hist_cap = 0;
+    CU_TRY(cudaMalloc(&h->hist, sizeof(double) * ((size_t)maxit + 2)), return AMP_ERR_NOMEM);
+    h->hist_cap = (int64_t)maxit + 2;
+  }
+  int mode = pol.loop_mode;
+  if (mode == AMP_LOOP_AUTO) mode = (h->persist_ok && persistent_fits(h->ctx)) ? AMP_LOOP_PERSISTENT : AMP_LOOP_GRAPH;
+  if (mode == AMP_LOOP_PERSISTENT && !(h->persist_ok && persistent_fits(h->ctx))) {
+    set_error("amp_pcg_solve: persistent loop not available for this problem/device");
+    return AMP_ERR_INVALID;
+  }
+  if (mode == AMP_LOOP_GRAPH) { const int rc = build_graph(h); if (rc != AMP_OK) return rc; }
+
+  DevState* hs = h->h_state;
+  std::memset(hs, 0, sizeof(DevState));
+  hs->b = b; hs->x = x; hs->hist = h->hist;
+  hs->tol = tol; hs->tau_zs = pol.tau_zs; hs->tau_zh = pol.tau_zh; hs->eps32 = pol.eps32; hs->C = pol.C;
+  hs->eta_safety = pol.eta_safety; hs->stop_safety = pol.stop_safety;
+  hs->amp = pol.amp ? 1 : 0; hs->u0 = pol.u0; hs->eta_rule = pol.eta_rule; hs->d = pol.d; hs->ell = pol.ell;
+  hs->scale_mode = pol.scale_mode; hs->no_stop = pol.no_stop ? 1 : 0; hs->maxit = maxit;
+  hs->status = AMP_MAXIT; hs->it_ur32 = hs->it_uz32 = hs->it_uz16 = -1;
+  hs->relres_true = -1.0;
+  h->launches = 0;
+
+  CU_TRY(cudaEventRecord(h->ev0, st), return AMP_ERR_CUDA);
+  CU_TRY(cudaMemcpyAsync(h->ctx.st, hs, sizeof(DevState), cudaMemcpyHostToDevice, st), return AMP_ERR_CUDA);
+  // a0: r0 = b - A x0 (FP64), ||b||, delta_0
+  if (!pol.x0_zero) { spmv_dispatch(h, AMP_FP64, AMP_FP64, x, h->ctx.q64); }
+  k_setup<<<h->vec_grid, kVecThreads, 0, st>>>(h->ctx, pol.x0_zero ? 1 : 0);
+  h->launches += 1;
+
+  if (mode == AMP_LOOP_GRAPH) {
+    CU_TRY(cudaGraphLaunch(h->graph_exec, st), return AMP_ERR_CUDA);
+  } else if (mode == AMP_LOOP_PERSISTENT) {
+    const int rc = persistent_launch(h->ctx, h->persist_grid, st);
+    if (rc != 0) { set_error("persistent kernel launch failed: %s", cudaGetErrorString((cudaError_t)rc)); return AMP_ERR_CUDA; }
+  } else {
+    const int batch = 32;
+    int done_iters = 0;
+    while (done_iters < maxit) {
+      const int nb = std::min(batch, maxit - done_iters);
+      for (int i = 0; i < nb; ++i) launch_iteration(h, h->ctx, st);
+      done_iters += nb;
+      CU_TRY(cudaMemcpyAsync(h->h_flag, &h->ctx.st->done, sizeof(int), cudaMemcpyDeviceToHost, st), return AMP_ERR_CUDA);
+      CU_TRY(cudaStreamSynchronize(st), return AMP_ERR_CUDA);
+      if (*h->h_flag) break;
+    }
+  }
+  CU_TRY(cudaEventRecord(h->ev1, st), return AMP_ERR_CUDA);
+  if (pol.true_residual) spmv_dispatch(h, AMP_FP64, AMP_FP64, x, h->ctx.q64);
+  k_finalize<<<h->vec_grid, kVecThreads, 0, st>>>(h->ctx, pol.true_residual ? 1 : 0);
+  h->launches += 1;
+  CU_TRY(cudaMemcpyAsync(hs, h->ctx.st, sizeof(DevState), cudaMemcpyDeviceToHost, st), return AMP_ERR_CUDA);
+  CU_TRY(cudaStreamSynchronize(st), return AMP_ERR_CUDA);
+  CU_TRY(cudaGetLastError(), return AMP_ERR_CUDA);
+  float ms = 0.f;
+  cudaEventElapsedTime(&ms, h->ev0, h->ev1);
+
+  const int iters = hs->k;
+  h->last_iters = iters;
+  h->launches += (mode == AMP_LOOP_PERSISTENT) ? 1 : (int64_t)4 * iters;
+  if (stats) {
+    std::memset(stats, 0, sizeof(*stats));
+    stats->status = hs->status; stats->iters = iters;
+    stats->it_ur32 = hs->it_ur32; stats->it_uz32 = hs->it_uz32; stats->it_uz16 = hs->it_uz16;
+    stats->loop_mode = mode;
+    stats->bnorm = hs->bnorm;
+    stats->relres_updated = (hs->bnorm > 0.0) ? hs->delta / hs->bnorm : 0.0;
+    stats->relres_true = hs->relres_true;
+    stats->solve_ms = ms;
+    double bytes = 0.0;
+    for (int k = 0; k < iters; ++k) {
+      const int ur = (hs->it_ur32 >= 0 && k >= hs->it_ur32) ? AMP_FP32 : AMP_FP64;
+      int uz = hs->amp ? hs->u0 : AMP_FP64;
+      if (hs->it_uz32 >= 0 && k >= hs->it_uz32) uz = std::max(uz, (int)AMP_FP32);
+      if (hs->it_uz16 >= 0 && k >= hs->it_uz16) uz = AMP_FP16;
+      bytes += amp_pcg_bytes_per_row(h->m_avg, uz, ur);
+    }
+    stats->algorithmic_bytes = bytes * (double)h->n;
+    stats->fp16_subnormal = hs->fp16_subnormal; stats->fp16_flushed = hs->fp16_flushed; stats->fp16_inf = hs->fp16_inf;
+  }
+  return hs->status;
+}
+
+extern "C" int amp_pcg_solve(amp_pcg_t* h, const double* b, double* x, double tol, int32_t maxit,
+                             const amp_policy_t* policy, amp_stats_t* stats) {
+  return solve_impl(h, b, x, tol, maxit, policy, stats);
+}
+
+extern "C" int amp_pcg_solve_host(amp_pcg_t* h, const double* b_host, double* x_host, double tol, int32_t maxit,
+                                  const amp_policy_t* policy, amp_stats_t* stats) {
+  g_last_error.clear();
+  if (!h || !b_host || !x_host) { set_error("amp_pcg_solve_host: null argument"); return AMP_ERR_INVALID; }
+  CU_TRY(cudaSetDevice(h->device), return AMP_ERR_CUDA);
+  const size_t bytes = sizeof(double) * (size_t)h->n;
+  CU_TRY(cudaMemcpyAsync(h->d_b_stage, b_host, bytes, cudaMemcpyHostToDevice, h->stream), return AMP_ERR_CUDA);
+  if (!(policy && policy->x0_zero))
+    CU_TRY(cudaMemcpyAsync(h->d_x_stage, x_host, bytes, cudaMemcpyHostToDevice, h->stream), return AMP_ERR_CUDA);
+  const int rc = solve_impl(h, h->d_b_stage, h->d_x_stage, tol, maxit, policy, stats);
+  if (rc < 0 && rc != AMP_ERR_BREAKDOWN) return rc;
+  CU_TRY(cudaMemcpyAsync(x_host, h->d_x_stage, bytes, cudaMemcpyDeviceToHost, h->stream), return AMP_ERR_CUDA);
+  CU_TRY(cudaStreamSynchronize(h->stream), return AMP_ERR_CUDA);
+  return rc;
+}
+
+extern "C" int32_t amp_pcg_residual_history(amp_pcg_t* h, double* out_host, int32_t count) {
+  if (!h || !out_host || count < 0) return AMP_ERR_INVALID;
+  if (h->last_iters < 0 || !h->hist) return 0;
+  const int32_t m = std::min<int32_t>(count, h->last_iters + 1);
+  if (m == 0) return 0;
+  CU_TRY(cudaMemcpyAsync(out_host, h->hist, sizeof(double) * (size_t)m, cudaMemcpyDeviceToHost, h->stream), return AMP_ERR_CUDA);
+  CU_TRY(cudaStreamSynchronize(h->stream), return AMP_ERR_CUDA);
+  return m;
+}

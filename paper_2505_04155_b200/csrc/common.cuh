@@ -1,0 +1,173 @@
+// common.cuh — device state, kernel context and small device helpers of the AMP-PCG loop.
+//
+// Notation follows Algorithm 4.1 of arXiv 2505.04155: r, z, p, q, x,
+// rho = r^T z, beta, gamma = q^T p, alpha, delta = ||r||, omega = scaling factor,
+// u_r = precision of r, q and of the matrix copy, u_z = precision of z, p.
+#pragma once
+#include <cuda_fp16.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace amp {
+
+constexpr int P64 = 0, P32 = 1, P16 = 2;       // precision codes (= AMP_FP64/32/16 of the C ABI)
+constexpr int kVecThreads = 256;               // block size of the vector kernels
+constexpr int kVecUnroll = 4;                  // independent 2-element chunks in flight per thread
+constexpr int kSpmvThreads = 256;              // block size of the SpMV kernel
+constexpr int kTileNnz = 4096;                 // stored entries staged per SpMV tile
+constexpr int kTileRows = 1024;                // max rows per SpMV tile
+constexpr int kMaxGrid = 4096;                 // capacity of each partial-sum array
+constexpr int kMaxWindow = 64;                 // max d / ell of the indicators
+
+// Scalars of one solve, resident in device memory.  The host writes the policy part before the
+// loop and reads the whole block once after it; inside the loop only kernels touch it.
+struct DevState {
+  // ---- per-solve inputs (host-written) ----
+  const double* b;
+  double* x;
+  double* hist;            // ||r_t||, t = 0..maxit
+  double tol, tau_zs, tau_zh, eps32, C, eta_safety, stop_safety;
+  int32_t amp, u0, eta_rule, d, ell, scale_mode, no_stop, maxit;
+  // ---- loop scalars (device-written) ----
+  double bnorm, delta, omega, rho, rho_prev, beta, gamma, alpha, relres_true;
+  int32_t k, done, status, zero_x;
+  int32_t ur, uz;          // precisions selected for iteration k by (4.1)
+  int32_t r_store, p_store;  // precisions r and p are currently stored in
+  int32_t it_ur32, it_uz32, it_uz16, pad0;
+  unsigned int counter[4];  // last-block tickets of the three reductions (+ setup)
+  unsigned long long fp16_subnormal, fp16_flushed, fp16_inf;
+  // ---- grid barrier of the persistent kernel ----
+  unsigned int bar_count, bar_gen;
+};
+
+// Handle-lifetime constants, passed to every kernel by value.
+struct Ctx {
+  DevState* st;
+  int64_t n;       // rows
+  int64_t npad;    // n rounded up to a multiple of 8: length of the library-owned vectors (zero padded)
+  int64_t nnz;
+  const int32_t* rowptr;
+  const int32_t* colidx;
+  const double* vals64;   // borrowed FP64 values
+  const float* vals32;    // owned FP32-rounded copy (u_r = FP32 phase)
+  const double* dinv64;   // 1/a_ii in FP64 (1 for M = I), used while u_z = FP64
+  const float* dinv32;    // RN32(1/a_ii), used when u_z < FP64 (reading R6)
+  double* r64; float* r32;
+  double* q64; float* q32;
+  double* z64; float* z32; __half* z16;
+  double* p64; float* p32; __half* p16;
+  double* partials;       // [4][kMaxGrid] per-block partial sums
+  const int32_t* tile_row;  // [ntiles+1] first row of each SpMV tile
+  int32_t ntiles;
+  int32_t lanes_per_row;  // lanes cooperating on one row in the SpMV row reduction (power of 2)
+  cudaGraphConditionalHandle cond;  // WHILE-node handle (graph loop only)
+  int32_t use_cond;
+};
+
+// ------------------------------------------------------------------ typed storage access ----
+template <int P> struct Store;
+template <> struct Store<P64> { using T = double; };
+template <> struct Store<P32> { using T = float; };
+template <> struct Store<P16> { using T = __half; };
+
+template <int P> __device__ __forceinline__ typename Store<P>::T* rvec(const Ctx& c);
+template <> __device__ __forceinline__ double* rvec<P64>(const Ctx& c) { return c.r64; }
+template <> __device__ __forceinline__ float* rvec<P32>(const Ctx& c) { return c.r32; }
+template <int P> __device__ __forceinline__ typename Store<P>::T* qvec(const Ctx& c);
+template <> __device__ __forceinline__ double* qvec<P64>(const Ctx& c) { return c.q64; }
+template <> __device__ __forceinline__ float* qvec<P32>(const Ctx& c) { return c.q32; }
+template <int P> __device__ __forceinline__ typename Store<P>::T* zvec(const Ctx& c);
+template <> __device__ __forceinline__ double* zvec<P64>(const Ctx& c) { return c.z64; }
+template <> __device__ __forceinline__ float* zvec<P32>(const Ctx& c) { return c.z32; }
+template <> __device__ __forceinline__ __half* zvec<P16>(const Ctx& c) { return c.z16; }
+template <int P> __device__ __forceinline__ typename Store<P>::T* pvec(const Ctx& c);
+template <> __device__ __forceinline__ double* pvec<P64>(const Ctx& c) { return c.p64; }
+template <> __device__ __forceinline__ float* pvec<P32>(const Ctx& c) { return c.p32; }
+template <> __device__ __forceinline__ __half* pvec<P16>(const Ctx& c) { return c.p16; }
+
+// one IEEE round-to-nearest-even of an FP64 value to the storage precision, returned as FP64
+template <int P> __device__ __forceinline__ double round_to(double v);
+template <> __device__ __forceinline__ double round_to<P64>(double v) { return v; }
+template <> __device__ __forceinline__ double round_to<P32>(double v) { return (double)__double2float_rn(v); }
+template <> __device__ __forceinline__ double round_to<P16>(double v) { return (double)__half2float(__double2half(v)); }
+
+// load / store of 2 consecutive elements (element index 2*pair), values exchanged as FP64.
+// Stored values convert to FP64 exactly; stores round once (RN-even, direct from the double).
+__device__ __forceinline__ void load2(const double* a, int64_t pair, double& v0, double& v1) {
+  const double2 t = reinterpret_cast<const double2*>(a)[pair];
+  v0 = t.x; v1 = t.y;
+}
+__device__ __forceinline__ void load2(const float* a, int64_t pair, double& v0, double& v1) {
+  const float2 t = reinterpret_cast<const float2*>(a)[pair];
+  v0 = (double)t.x; v1 = (double)t.y;
+}
+__device__ __forceinline__ void load2(const __half* a, int64_t pair, double& v0, double& v1) {
+  const float2 t = __half22float2(reinterpret_cast<const __half2*>(a)[pair]);
+  v0 = (double)t.x; v1 = (double)t.y;
+}
+__device__ __forceinline__ void store2(double* a, int64_t pair, double v0, double v1) {
+  reinterpret_cast<double2*>(a)[pair] = make_double2(v0, v1);
+}
+__device__ __forceinline__ void store2(float* a, int64_t pair, double v0, double v1) {
+  reinterpret_cast<float2*>(a)[pair] = make_float2(__double2float_rn(v0), __double2float_rn(v1));
+}
+__device__ __forceinline__ void store2(__half* a, int64_t pair, double v0, double v1) {
+  reinterpret_cast<__half2*>(a)[pair] = __halves2half2(__double2half(v0), __double2half(v1));
+}
+
+// gather of one element of p as the SpMV working type.  COH = false: read-only path (p is not
+// written by the running kernel); COH = true: plain coherent load.
+template <bool COH, class T> __device__ __forceinline__ T ldp(const T* p, int j) { return COH ? p[j] : __ldg(p + j); }
+template <bool COH> __device__ __forceinline__ double gather64(const double* p, int j) { return ldp<COH>(p, j); }
+template <bool COH> __device__ __forceinline__ double gather64(const float* p, int j) { return (double)ldp<COH>(p, j); }
+template <bool COH> __device__ __forceinline__ double gather64(const __half* p, int j) { return (double)__half2float(ldp<COH>(p, j)); }
+template <bool COH> __device__ __forceinline__ float gather32(const double* p, int j) { return __double2float_rn(ldp<COH>(p, j)); }
+template <bool COH> __device__ __forceinline__ float gather32(const float* p, int j) { return ldp<COH>(p, j); }
+template <bool COH> __device__ __forceinline__ float gather32(const __half* p, int j) { return __half2float(ldp<COH>(p, j)); }
+
+// ------------------------------------------------------------------ reductions --------------
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+
+// Sum over the block; the result is valid in warp 0.  Fixed tree => deterministic.
+template <int NT> __device__ __forceinline__ double block_sum(double v, double* sm /* [32] */) {
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  v = warp_sum(v);
+  __syncthreads();
+  if (lane == 0) sm[w] = v;
+  __syncthreads();
+  double t = (threadIdx.x < NT / 32) ? sm[threadIdx.x] : 0.0;
+  if (w == 0) t = warp_sum(t);
+  return t;
+}
+
+// Single-pass deterministic grid reduction: every block publishes its partial sum, the block
+// that takes the last ticket adds the partials in index order and runs epi(total) on thread 0.
+template <int NT, class Epi>
+__device__ __forceinline__ void grid_reduce(double v, double* partials, unsigned int* counter, int bid, int nb,
+                                            double* sm, Epi epi) {
+  __shared__ int s_last;
+  const double bs = block_sum<NT>(v, sm);
+  if (threadIdx.x == 0) {
+    __stcg(partials + bid, bs);
+    __threadfence();
+    const unsigned int t = atomicAdd(counter, 1u);
+    s_last = (t == (unsigned int)nb - 1u);
+  }
+  __syncthreads();
+  if (s_last) {
+    __threadfence();
+    double s = 0.0;
+    for (int i = threadIdx.x; i < nb; i += NT) s += __ldcg(partials + i);
+    const double tot = block_sum<NT>(s, sm);
+    if (threadIdx.x == 0) {
+      *counter = 0u;
+      epi(tot);
+    }
+  }
+}
+
+}  // namespace amp

@@ -1,0 +1,213 @@
+// kernels.cuh — __global__ entry points: the four loop kernels (precision dispatched at run
+// time from the device state, so one static CUDA graph serves every precision phase), the
+// set-up / finalisation kernels, the stand-alone SpMV and the one-off kernels of create().
+#pragma once
+#include "phases.cuh"
+
+namespace amp {
+
+constexpr int kSpmvSmemBytes = (int)(sizeof(double) * kTileNnz + sizeof(int) * (kTileRows + 4));
+
+// ------------------------------------------------------------------ precision dispatch ------
+// The precisions in use are device-side scalars (they change inside the loop without the host
+// knowing), so every loop kernel branches on them once, uniformly, and runs the templated body.
+__device__ __forceinline__ double dispatch_z(const Ctx& c, int rs, int ur, int uz, double omega, int bid, int nb) {
+  if (rs == P64 && ur == P64) {
+    if (uz == P64) return phase_z<P64, P64, P64>(c, omega, bid, nb);
+    if (uz == P32) return phase_z<P64, P64, P32>(c, omega, bid, nb);
+    return phase_z<P64, P64, P16>(c, omega, bid, nb);
+  }
+  if (rs == P64 && ur == P32) {
+    if (uz == P64) return phase_z<P64, P32, P64>(c, omega, bid, nb);
+    if (uz == P32) return phase_z<P64, P32, P32>(c, omega, bid, nb);
+    return phase_z<P64, P32, P16>(c, omega, bid, nb);
+  }
+  if (uz == P64) return phase_z<P32, P32, P64>(c, omega, bid, nb);
+  if (uz == P32) return phase_z<P32, P32, P32>(c, omega, bid, nb);
+  return phase_z<P32, P32, P16>(c, omega, bid, nb);
+}
+
+__device__ __forceinline__ void dispatch_p(const Ctx& c, int ps, int uz, double beta, bool first, int bid, int nb) {
+  if (uz == P64) phase_p<P64, P64>(c, beta, first, bid, nb);
+  else if (uz == P32) {
+    if (ps == P64) phase_p<P64, P32>(c, beta, first, bid, nb);
+    else phase_p<P32, P32>(c, beta, first, bid, nb);
+  } else {
+    if (ps == P64) phase_p<P64, P16>(c, beta, first, bid, nb);
+    else if (ps == P32) phase_p<P32, P16>(c, beta, first, bid, nb);
+    else phase_p<P16, P16>(c, beta, first, bid, nb);
+  }
+}
+
+template <bool COH>
+__device__ __forceinline__ double dispatch_spmv(const Ctx& c, int ur, int uz, int bid, int nb, unsigned char* smem,
+                                                double* red) {
+  if (ur == P64) {
+    if (uz == P64) return phase_spmv<P64, COH>(c, c.p64, c.q64, bid, nb, smem, red);
+    if (uz == P32) return phase_spmv<P64, COH>(c, c.p32, c.q64, bid, nb, smem, red);
+    return phase_spmv<P64, COH>(c, c.p16, c.q64, bid, nb, smem, red);
+  }
+  if (uz == P64) return phase_spmv<P32, COH>(c, c.p64, c.q32, bid, nb, smem, red);
+  if (uz == P32) return phase_spmv<P32, COH>(c, c.p32, c.q32, bid, nb, smem, red);
+  return phase_spmv<P32, COH>(c, c.p16, c.q32, bid, nb, smem, red);
+}
+
+__device__ __forceinline__ double dispatch_xr(const Ctx& c, int ur, int uz, double alpha, double* x, int bid, int nb) {
+  if (ur == P64) {
+    if (uz == P64) return phase_xr<P64, P64>(c, alpha, x, bid, nb);
+    if (uz == P32) return phase_xr<P64, P32>(c, alpha, x, bid, nb);
+    return phase_xr<P64, P16>(c, alpha, x, bid, nb);
+  }
+  if (uz == P64) return phase_xr<P32, P64>(c, alpha, x, bid, nb);
+  if (uz == P32) return phase_xr<P32, P32>(c, alpha, x, bid, nb);
+  return phase_xr<P32, P16>(c, alpha, x, bid, nb);
+}
+
+// ------------------------------------------------------------------ loop kernels ------------
+__global__ void __launch_bounds__(kVecThreads) k_z(const Ctx c) {
+  __shared__ double red[32];
+  DevState* s = c.st;
+  if (s->done) return;
+  const int bid = blockIdx.x, nb = gridDim.x;
+  const double v = dispatch_z(c, s->r_store, s->ur, s->uz, s->omega, bid, nb);
+  grid_reduce<kVecThreads>(v, c.partials + 0 * kMaxGrid, &s->counter[0], bid, nb, red,
+                           [&](double tot) { epi_rho(c, tot); });
+}
+
+__global__ void __launch_bounds__(kVecThreads) k_p(const Ctx c) {
+  const DevState* s = c.st;
+  if (s->done) return;
+  dispatch_p(c, s->p_store, s->uz, s->beta, s->k == 0, blockIdx.x, gridDim.x);
+}
+
+__global__ void __launch_bounds__(kSpmvThreads) k_spmv(const Ctx c) {
+  extern __shared__ __align__(16) unsigned char smem[];
+  __shared__ double red[32];
+  DevState* s = c.st;
+  if (s->done) return;
+  const int bid = blockIdx.x, nb = gridDim.x;
+  const double v = dispatch_spmv<false>(c, s->ur, s->uz, bid, nb, smem, red);
+  grid_reduce<kSpmvThreads>(v, c.partials + 1 * kMaxGrid, &s->counter[1], bid, nb, red,
+                            [&](double tot) { epi_gamma(c, tot); });
+}
+
+__global__ void __launch_bounds__(kVecThreads) k_xr(const Ctx c) {
+  __shared__ double red[32];
+  DevState* s = c.st;
+  if (s->done) {  // nothing to do (converged at set-up, or breakdown): make sure the WHILE node stops
+    if (blockIdx.x == 0 && threadIdx.x == 0) set_loop_cond(c, 0);
+    return;
+  }
+  const int bid = blockIdx.x, nb = gridDim.x;
+  const double v = dispatch_xr(c, s->ur, s->uz, s->alpha, s->x, bid, nb);
+  grid_reduce<kVecThreads>(v, c.partials + 2 * kMaxGrid, &s->counter[2], bid, nb, red,
+                           [&](double tot) { epi_delta(c, tot); });
+}
+
+// ------------------------------------------------------------------ stand-alone SpMV --------
+template <int UR, class PT>
+__global__ void __launch_bounds__(kSpmvThreads) k_spmv_any(const Ctx c, const PT* p, typename Store<UR>::T* q) {
+  extern __shared__ __align__(16) unsigned char smem[];
+  __shared__ double red[32];
+  (void)phase_spmv<UR, false>(c, p, q, blockIdx.x, gridDim.x, smem, red);
+}
+
+// ------------------------------------------------------------------ set-up / finalise -------
+// step a0 (Alg 4.1 line 1): r0 = b - A x0 in FP64 (q64 holds A x0; for x0 = 0: r0 = b, x = 0),
+// ||b||, delta_0 = ||r0||, then the selector for k = 0.
+__global__ void __launch_bounds__(kVecThreads) k_setup(const Ctx c, int x0_zero) {
+  __shared__ double red[32];
+  __shared__ int s_last;
+  DevState* s = c.st;
+  const double* __restrict__ b = s->b;
+  double* __restrict__ x = s->x;
+  double bb = 0.0, rr = 0.0;
+  const int64_t stride = (int64_t)gridDim.x * kVecThreads;
+  for (int64_t i = (int64_t)blockIdx.x * kVecThreads + threadIdx.x; i < c.n; i += stride) {
+    const double bi = b[i];
+    double ri;
+    if (x0_zero) { ri = bi; x[i] = 0.0; }
+    else ri = bi - c.q64[i];
+    c.r64[i] = ri;
+    bb = fma(bi, bi, bb);
+    rr = fma(ri, ri, rr);
+  }
+  const double b1 = block_sum<kVecThreads>(bb, red);
+  const double b2 = block_sum<kVecThreads>(rr, red);
+  double* part = c.partials + 3 * kMaxGrid;
+  if (threadIdx.x == 0) {
+    __stcg(part + 2 * blockIdx.x, b1);
+    __stcg(part + 2 * blockIdx.x + 1, b2);
+    __threadfence();
+    s_last = (atomicAdd(&s->counter[3], 1u) == gridDim.x - 1);
+  }
+  __syncthreads();
+  if (s_last) {
+    __threadfence();
+    double s1 = 0.0, s2 = 0.0;
+    for (int i = threadIdx.x; i < (int)gridDim.x; i += kVecThreads) {
+      s1 += __ldcg(part + 2 * i);
+      s2 += __ldcg(part + 2 * i + 1);
+    }
+    const double t1 = block_sum<kVecThreads>(s1, red);
+    const double t2 = block_sum<kVecThreads>(s2, red);
+    if (threadIdx.x == 0) {
+      s->counter[3] = 0u;
+      epi_setup(c, t1, t2);
+    }
+  }
+}
+
+// after the loop: x = 0 if b = 0; optional true residual ||b - A x|| / ||b|| (q64 holds A x)
+__global__ void __launch_bounds__(kVecThreads) k_finalize(const Ctx c, int true_residual) {
+  __shared__ double red[32];
+  DevState* s = c.st;
+  const int64_t stride = (int64_t)gridDim.x * kVecThreads;
+  if (s->zero_x) {
+    for (int64_t i = (int64_t)blockIdx.x * kVecThreads + threadIdx.x; i < c.n; i += stride) s->x[i] = 0.0;
+  }
+  if (!true_residual) return;
+  double rr = 0.0;
+  if (!s->zero_x) {
+    for (int64_t i = (int64_t)blockIdx.x * kVecThreads + threadIdx.x; i < c.n; i += stride) {
+      const double t = s->b[i] - c.q64[i];
+      rr = fma(t, t, rr);
+    }
+  }
+  grid_reduce<kVecThreads>(rr, c.partials + 3 * kMaxGrid, &s->counter[3], blockIdx.x, gridDim.x, red,
+                           [&](double tot) { s->relres_true = (s->bnorm > 0.0) ? sqrt(tot) / s->bnorm : 0.0; });
+}
+
+// ------------------------------------------------------------------ create() kernels --------
+// flags: bit0 rowptr not monotone / out of range, bit1 column out of range,
+//        bit2 missing diagonal, bit3 non-positive or non-finite diagonal
+__global__ void k_validate_dinv(int64_t n, int64_t nnz, const int32_t* rowptr, const int32_t* colidx,
+                                const double* vals, int jacobi, double* dinv64, float* dinv32, int* flags) {
+  const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+  int f = 0;
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
+    const int64_t a = rowptr[i], b = rowptr[i + 1];
+    if (i == 0 && a != 0) f |= 1;
+    if (i == n - 1 && b != nnz) f |= 1;
+    if (a < 0 || b < a || b > nnz) { f |= 1; continue; }
+    double d = 1.0;
+    bool found = !jacobi;
+    for (int64_t e = a; e < b; ++e) {
+      const int j = colidx[e];
+      if (j < 0 || j >= n) { f |= 2; continue; }
+      if (jacobi && j == i) { d = vals[e]; found = true; }
+    }
+    if (!found) { f |= 4; d = 1.0; }
+    else if (!(d > 0.0) || isinf(d)) { f |= 8; d = 1.0; }
+    dinv64[i] = 1.0 / d;
+    dinv32[i] = __double2float_rn(1.0 / d);
+  }
+  if (f) atomicOr(flags, f);
+}
+
+__global__ void k_to_fp32(int64_t n, const double* __restrict__ a, float* __restrict__ o) {
+  const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) o[i] = __double2float_rn(a[i]);
+}
+
+}  // namespace amp

@@ -1,0 +1,381 @@
+// phases.cuh — the steps of one AMP-PCG iteration (Algorithm 4.1) as device
+// functions over a (block id, block count) work decomposition, so that the same code runs as
+// four stand-alone kernels (stream / CUDA-graph loop) or inside the persistent kernel.
+//
+//   phase_z    a2: y = omega r, z = M^-1 y (fused), one rounding to u_z; rho = r^T z
+//   phase_p    a3: p = z + beta p, one rounding to u_z
+//   phase_spmv a4: q = A p in u_r (CSR, tile-staged), gamma = q^T p
+//   phase_xr   a5: x += alpha p (FP64), r -= alpha q (u_r), delta = ||r||
+// and the scalar epilogues (one thread, after each grid reduction):
+//   epi_rho    beta = rho_k / rho_{k-1}                       (Alg 4.1 lines 6-9)
+//   epi_gamma  alpha = rho / gamma, breakdown test             (lines 13-14)
+//   epi_delta  stop test, eta_k and the selector (4.1) for the next iteration (lines 3, 17-20)
+#pragma once
+#include <math_constants.h>
+
+#include "common.cuh"
+
+namespace amp {
+
+// ------------------------------------------------------------------ scalar epilogues --------
+__device__ __forceinline__ void set_loop_cond(const Ctx& c, int keep_going) {
+  if (c.use_cond) cudaGraphSetConditional(c.cond, keep_going ? 1u : 0u);
+}
+
+__device__ __forceinline__ int lower_prec(int a, int b) { return a > b ? a : b; }
+
+// eta_k (4.9)/(4.11) and (u_z,k, u_r,k) = precisionSelector (4.1) for iteration k = s->k, then
+// omega_k.  Readings R2 (norms with negative index are ||r_0||), R3 (eta vs tol*||b||, <=) and
+// R5 (both switches latched) of DESIGN.md.  hist[t] = ||r_t||.
+__device__ __noinline__ void select_precisions(DevState* s, int64_t n) {
+  const int k = s->k;
+  const double delta = s->delta;
+  if (!s->amp) {
+    s->omega = 1.0;
+    return;
+  }
+  const double* hist = s->hist;
+  if (s->ur == P64 && s->eta_rule != 2) {
+    double eta = CUDART_INF;
+    const double C = s->C, e32 = s->eps32;
+    if (s->eta_rule == 0) {  // (4.9)
+      eta = 0.0;
+      for (int t = k - s->d; t <= k; ++t) {
+        const double hm1 = hist[(t - 1) > 0 ? (t - 1) : 0], h0 = hist[t > 0 ? t : 0];
+        eta += e32 * ((3.0 + C) * hm1 + (2.0 + C) * h0);
+      }
+    } else {  // (4.11)
+      const int l = s->ell;
+      if (k >= l && hist[k] < hist[k - l]) {
+        const double rate = pow(hist[k] / hist[k - l], 1.0 / (double)l);
+        eta = e32 * (5.0 + 2.0 * C) * hist[k - 1] / (1.0 - rate);
+      }
+    }
+    if (eta <= s->eta_safety * s->tol * s->bnorm) {  // (4.10)
+      s->ur = P32;
+      s->it_ur32 = k;
+    }
+  }
+  const double nu = delta / s->bnorm;  // nu_k
+  int want = s->u0;
+  if (nu < s->tau_zs) want = lower_prec(s->u0, nu >= s->tau_zh ? P32 : P16);
+  if (want > s->uz) {
+    s->uz = want;
+    if (want >= P32 && s->it_uz32 < 0) s->it_uz32 = k;
+    if (want == P16 && s->it_uz16 < 0) s->it_uz16 = k;
+  }
+  double om = 1.0;  // omega_k: Alg 4.1 line 4, or the alternatives allowed by PAPER.md:34, :223
+  if (s->scale_mode == 0) om = 1.0 / delta;
+  else if (s->scale_mode == 1) om = sqrt((double)n) / delta;
+  else if (s->scale_mode == 2) om = ldexp(1.0, (int)rint(log2(1.0 / delta)));
+  s->omega = om;
+}
+
+// after the setup reduction: ||b||, delta_0 = ||r_0||, edge cases, selector for k = 0
+__device__ __noinline__ void epi_setup(const Ctx& c, double bb, double rr) {
+  DevState* s = c.st;
+  s->bnorm = sqrt(bb);
+  s->delta = sqrt(rr);
+  s->hist[0] = s->delta;
+  s->k = 0;
+  s->r_store = P64;
+  s->ur = P64;
+  s->uz = s->amp ? s->u0 : P64;
+  s->p_store = s->uz;
+  s->rho_prev = 0.0;
+  s->beta = 0.0;
+  if (bb == 0.0) {  // b = 0: x = 0 (reading R13)
+    s->done = 1; s->status = 0; s->zero_x = 1; s->delta = 0.0;
+  } else if (!(s->delta == s->delta) || isinf(s->delta) || isinf(s->bnorm)) {
+    s->done = 1; s->status = -2;
+  } else if (s->delta <= s->stop_safety * s->tol * s->bnorm && !s->no_stop) {
+    s->done = 1; s->status = 0;  // x0 already satisfies the stopping test
+  } else {
+    select_precisions(s, c.n);
+  }
+}
+
+__device__ __forceinline__ void epi_rho(const Ctx& c, double rho) {
+  DevState* s = c.st;
+  s->rho = rho;
+  s->beta = (s->k > 0) ? rho / s->rho_prev : 0.0;  // Alg 4.1 lines 7-9
+}
+
+__device__ __forceinline__ void epi_gamma(const Ctx& c, double gamma) {
+  DevState* s = c.st;
+  s->gamma = gamma;
+  const double rho = s->rho;
+  if (!(gamma > 0.0) || !(rho > 0.0) || isinf(gamma) || isinf(rho)) {  // breakdown (reading R13)
+    s->status = -2;
+    s->done = 1;
+    set_loop_cond(c, 0);
+  } else {
+    s->alpha = rho / gamma;  // line 14
+  }
+}
+
+__device__ __noinline__ void epi_delta(const Ctx& c, double rr) {
+  DevState* s = c.st;
+  const double delta = sqrt(rr);  // line 17
+  const int k1 = s->k + 1;
+  s->delta = delta;
+  s->hist[k1] = delta;
+  s->rho_prev = s->rho;
+  s->k = k1;
+  s->r_store = s->ur;
+  s->p_store = s->uz;
+  if (!(delta == delta) || isinf(delta)) {
+    s->status = -2; s->done = 1;
+  } else if (delta <= s->stop_safety * s->tol * s->bnorm && !s->no_stop) {  // line 18
+    s->status = 0; s->done = 1;
+  } else if (k1 >= s->maxit) {
+    s->status = 1; s->done = 1;
+  } else {
+    select_precisions(s, c.n);  // line 3 of the next iteration
+  }
+  set_loop_cond(c, !s->done);
+}
+
+// NOTE: the loop vectors (r, z, p, q, x) are deliberately NOT __restrict__/read-only qualified:
+// inside the persistent kernel they are written by earlier phases of the same kernel, so they
+// must be read with plain coherent loads (ordered by the grid barrier), never ld.global.nc.
+// Loads are grouped ahead of the stores by hand (kVecUnroll chunks in flight per thread).
+
+// ------------------------------------------------------------------ a2: z and rho ------------
+// RS: precision r is stored in; UR: precision selected for r (RS != UR only at the iteration of
+// the u_r switch, where r <- RN32(r) is fused here, step a6); UZ: precision of z.
+template <int RS, int UR, int UZ>
+__device__ __forceinline__ double phase_z(const Ctx& c, const double omega, int bid, int nb) {
+  const typename Store<RS>::T* rin = rvec<RS>(c);
+  typename Store<UR>::T* rout = rvec<UR>(c);
+  typename Store<UZ>::T* z = zvec<UZ>(c);
+  const int64_t npair = c.npad >> 1;
+  const int64_t stride = (int64_t)nb * kVecThreads;
+  double sum = 0.0;
+  for (int64_t base = (int64_t)bid * kVecThreads + threadIdx.x; base < npair; base += stride * kVecUnroll) {
+    double r0[kVecUnroll], r1[kVecUnroll], d0[kVecUnroll], d1[kVecUnroll];
+#pragma unroll
+    for (int u = 0; u < kVecUnroll; ++u) {
+      const int64_t i = base + u * stride;
+      if (i < npair) {
+        load2(rin, i, r0[u], r1[u]);
+        if (UZ == P64) load2(c.dinv64, i, d0[u], d1[u]);
+        else load2(c.dinv32, i, d0[u], d1[u]);
+      }
+    }
+#pragma unroll
+    for (int u = 0; u < kVecUnroll; ++u) {
+      const int64_t i = base + u * stride;
+      if (i < npair) {
+        double a0 = r0[u], a1 = r1[u];
+        if (RS != UR) {  // r <- RN_{u_r}(r) at the switch iteration
+          a0 = round_to<UR>(a0); a1 = round_to<UR>(a1);
+          store2(rout, i, a0, a1);
+        }
+        const double z0 = round_to<UZ>((a0 * omega) * d0[u]);
+        const double z1 = round_to<UZ>((a1 * omega) * d1[u]);
+        store2(z, i, z0, z1);
+#ifdef AMP_COUNT_FP16
+        if (UZ == P16) {
+          const double t0 = (a0 * omega) * d0[u], t1 = (a1 * omega) * d1[u];
+          count_fp16(c.st, t0, z0); count_fp16(c.st, t1, z1);
+        }
+#endif
+        sum = fma(a0, z0, sum);
+        sum = fma(a1, z1, sum);
+      }
+    }
+  }
+  return sum;
+}
+
+// ------------------------------------------------------------------ a3: p -------------------
+// PS: precision p_{k-1} is stored in; UZ: precision of z_k and p_k (PS != UZ only at a u_z
+// switch, where p_{k-1} <- RN_{u_z}(p_{k-1}) is fused here, reading R9).
+template <int PS, int UZ>
+__device__ __forceinline__ void phase_p(const Ctx& c, const double beta, const bool first, int bid, int nb) {
+  const typename Store<PS>::T* pin = pvec<PS>(c);
+  typename Store<UZ>::T* pout = pvec<UZ>(c);
+  const typename Store<UZ>::T* z = zvec<UZ>(c);
+  const int64_t npair = c.npad >> 1;
+  const int64_t stride = (int64_t)nb * kVecThreads;
+  for (int64_t base = (int64_t)bid * kVecThreads + threadIdx.x; base < npair; base += stride * kVecUnroll) {
+    double p0[kVecUnroll], p1[kVecUnroll], z0[kVecUnroll], z1[kVecUnroll];
+#pragma unroll
+    for (int u = 0; u < kVecUnroll; ++u) {
+      const int64_t i = base + u * stride;
+      if (i < npair) {
+        load2(z, i, z0[u], z1[u]);
+        if (first) { p0[u] = 0.0; p1[u] = 0.0; }
+        else load2(pin, i, p0[u], p1[u]);
+      }
+    }
+#pragma unroll
+    for (int u = 0; u < kVecUnroll; ++u) {
+      const int64_t i = base + u * stride;
+      if (i < npair) {
+        double a0 = p0[u], a1 = p1[u];
+        if (PS != UZ) { a0 = round_to<UZ>(a0); a1 = round_to<UZ>(a1); }
+        const double n0 = fma(beta, a0, z0[u]), n1 = fma(beta, a1, z1[u]);
+        store2(pout, i, n0, n1);
+#ifdef AMP_COUNT_FP16
+        if (UZ == P16) { count_fp16(c.st, n0, round_to<P16>(n0)); count_fp16(c.st, n1, round_to<P16>(n1)); }
+#endif
+      }
+    }
+  }
+}
+
+// ------------------------------------------------------------------ a5: x, r, delta ---------
+template <int UR, int UZ>
+__device__ __forceinline__ double phase_xr(const Ctx& c, const double alpha, double* x, int bid, int nb) {
+  const typename Store<UZ>::T* p = pvec<UZ>(c);
+  const typename Store<UR>::T* q = qvec<UR>(c);
+  typename Store<UR>::T* r = rvec<UR>(c);
+  const int64_t n = c.n;
+  const int64_t npair = c.npad >> 1;
+  const int64_t stride = (int64_t)nb * kVecThreads;
+  double sum = 0.0;
+  for (int64_t base = (int64_t)bid * kVecThreads + threadIdx.x; base < npair; base += stride * kVecUnroll) {
+    double x0[kVecUnroll], x1[kVecUnroll], p0[kVecUnroll], p1[kVecUnroll], q0[kVecUnroll], q1[kVecUnroll],
+        r0[kVecUnroll], r1[kVecUnroll];
+#pragma unroll
+    for (int u = 0; u < kVecUnroll; ++u) {
+      const int64_t i = base + u * stride;
+      if (i < npair) {
+        if (2 * i + 1 < n) load2(x, i, x0[u], x1[u]);
+        else { x0[u] = (2 * i < n) ? x[2 * i] : 0.0; x1[u] = 0.0; }
+        load2(p, i, p0[u], p1[u]);
+        load2(q, i, q0[u], q1[u]);
+        load2(r, i, r0[u], r1[u]);
+      }
+    }
+#pragma unroll
+    for (int u = 0; u < kVecUnroll; ++u) {
+      const int64_t i = base + u * stride;
+      if (i < npair) {
+        const double nx0 = fma(alpha, p0[u], x0[u]), nx1 = fma(alpha, p1[u], x1[u]);  // line 15, FP64
+        if (2 * i + 1 < n) store2(x, i, nx0, nx1);
+        else if (2 * i < n) x[2 * i] = nx0;
+        const double nr0 = round_to<UR>(fma(-alpha, q0[u], r0[u]));  // line 16, one rounding to u_r
+        const double nr1 = round_to<UR>(fma(-alpha, q1[u], r1[u]));
+        store2(r, i, nr0, nr1);
+        sum = fma(nr0, nr0, sum);
+        sum = fma(nr1, nr1, sum);
+      }
+    }
+  }
+  return sum;
+}
+
+// ------------------------------------------------------------------ a4: SpMV ----------------
+// CSR "tile-staged" mat-vec.  Rows are pre-partitioned into tiles of <= kTileRows rows and
+// <= kTileNnz stored entries (a single longer row forms its own tile).  Per tile the block
+//  (1) streams the tile's values and column indices with 128-bit loads (fully coalesced,
+//      independent of row lengths), gathers p_j and writes the products a_ij p_j to shared memory;
+//  (2) reduces each row from shared memory with L lanes per row and writes q_i (coalesced);
+// and accumulates gamma += p_i q_i in FP64 from the stored q_i.
+// UR = P64: FP64 values, products and sums.  UR = P32: FP32 value copy, p_j converted to FP32,
+// FP32 products and sums (q computed and stored in u_r).
+template <int UR> struct SpmvT;
+template <> struct SpmvT<P64> { using A = double; };
+template <> struct SpmvT<P32> { using A = float; };
+
+// COH = true: p is written earlier in the same (persistent) kernel, so it is gathered with
+// plain coherent loads after the grid barrier instead of the read-only (ld.global.nc) path.
+template <int UR, bool COH, class PT>
+__device__ __forceinline__ double phase_spmv(const Ctx& c, const PT* p, typename Store<UR>::T* q, int bid, int nb,
+                                             unsigned char* smem_raw, double* red_sm) {
+  using A = typename SpmvT<UR>::A;
+  A* prod = reinterpret_cast<A*>(smem_raw);
+  int* rp = reinterpret_cast<int*>(smem_raw + sizeof(A) * kTileNnz);
+  const int32_t* __restrict__ rowptr = c.rowptr;
+  const int32_t* __restrict__ colidx = c.colidx;
+  const int L = c.lanes_per_row;
+  const int tid = threadIdx.x;
+  const int64_t nnz = c.nnz;
+  double gsum = 0.0;
+
+  for (int t = bid; t < c.ntiles; t += nb) {
+    const int r0 = c.tile_row[t], r1 = c.tile_row[t + 1];
+    const int nrows = r1 - r0;
+    const int e0 = rowptr[r0], e1 = rowptr[r1];
+
+    if (e1 - e0 > kTileNnz) {  // one long row: block-wide strided accumulation
+      A acc = 0;
+      for (int e = e0 + tid; e < e1; e += kSpmvThreads) {
+        if (UR == P64) acc += (A)(c.vals64[e] * gather64<COH>(p, colidx[e]));
+        else acc += (A)(c.vals32[e] * gather32<COH>(p, colidx[e]));
+      }
+      const double tot = block_sum<kSpmvThreads>((double)acc, red_sm);
+      if (tid == 0) {
+        const A qs = (A)tot;
+        q[r0] = qs;
+        gsum = fma(gather64<COH>(p, r0), (double)qs, gsum);
+      }
+      __syncthreads();
+      continue;
+    }
+
+    for (int i = tid; i <= nrows; i += kSpmvThreads) rp[i] = rowptr[r0 + i] - e0;
+
+    // (1) products.  Vector v covers entries ea+4v .. ea+4v+3, ea = e0 rounded down to 4.
+    const int ea = e0 & ~3;
+    const int nvec = (e1 - ea + 3) >> 2;
+    for (int v = tid; v < nvec; v += kSpmvThreads) {
+      const int e = ea + 4 * v;
+      int cj[4];
+      A aj[4];
+      if ((int64_t)e + 4 <= nnz) {
+        const int4 cc = __ldg(reinterpret_cast<const int4*>(colidx + e));
+        cj[0] = cc.x; cj[1] = cc.y; cj[2] = cc.z; cj[3] = cc.w;
+        if (UR == P64) {
+          const double2 a01 = __ldg(reinterpret_cast<const double2*>(c.vals64 + e));
+          const double2 a23 = __ldg(reinterpret_cast<const double2*>(c.vals64 + e + 2));
+          aj[0] = (A)a01.x; aj[1] = (A)a01.y; aj[2] = (A)a23.x; aj[3] = (A)a23.y;
+        } else {
+          const float4 a = __ldg(reinterpret_cast<const float4*>(c.vals32 + e));
+          aj[0] = (A)a.x; aj[1] = (A)a.y; aj[2] = (A)a.z; aj[3] = (A)a.w;
+        }
+      } else {  // the last, partial vector of the arrays
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+          const bool in = (int64_t)e + j < nnz;
+          cj[j] = in ? colidx[e + j] : 0;
+          if (UR == P64) aj[j] = in ? (A)c.vals64[e + j] : (A)0;
+          else aj[j] = in ? (A)c.vals32[e + j] : (A)0;
+        }
+      }
+#pragma unroll
+      for (int j = 0; j < 4; ++j) {
+        const int idx = e + j - e0;
+        if (idx >= 0 && e + j < e1) {
+          if (UR == P64) prod[idx] = (A)((double)aj[j] * gather64<COH>(p, cj[j]));
+          else prod[idx] = (A)__fmul_rn((float)aj[j], gather32<COH>(p, cj[j]));
+        }
+      }
+    }
+    __syncthreads();
+
+    // (2) row sums: L lanes per row, then a shuffle tree over the L lanes
+    const int rows_per_pass = kSpmvThreads / L;
+    const int sub = tid % L, rl = tid / L;
+    for (int rb = 0; rb < nrows; rb += rows_per_pass) {
+      const int row = rb + rl;
+      A s = 0;
+      if (row < nrows) {
+        const int jb = rp[row], je = rp[row + 1];
+        for (int j = jb + sub; j < je; j += L) s += prod[j];
+      }
+      for (int o = L >> 1; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+      if (row < nrows && sub == 0) {
+        q[r0 + row] = s;
+        gsum = fma(gather64<COH>(p, r0 + row), (double)s, gsum);
+      }
+    }
+    __syncthreads();
+  }
+  return gsum;
+}
+
+}  // namespace amp
