@@ -190,38 +190,69 @@ extern "C" amp_pcg_t* amp_pcg_create(int64_t n, int64_t nnz, const int32_t* rowp
     return nullptr;
   }
 
-  // row tiles of the SpMV: <= kTileRows rows and <= kTileNnz entries; a longer row stands alone
-  std::vector<int32_t> tiles;
-  tiles.push_back(0);
-  int64_t r = 0;
-  while (r < n) {
-    int64_t r1 = r + 1;
-    if (rp[r1] - rp[r] <= kTileNnz) {
-      while (r1 < n && r1 - r < kTileRows && rp[r1 + 1] - rp[r] <= kTileNnz) ++r1;
-    }
-    tiles.push_back((int32_t)r1);
-    r = r1;
-  }
-  c.ntiles = (int32_t)tiles.size() - 1;
-  ALLOC(tile_row, int32_t, tiles.size());
-  CU_TRY(cudaMemcpyAsync(tile_row, tiles.data(), sizeof(int32_t) * tiles.size(), cudaMemcpyHostToDevice, h->stream),
-         { amp_pcg_destroy(h); return nullptr; });
-  CU_TRY(cudaStreamSynchronize(h->stream), { amp_pcg_destroy(h); return nullptr; });
-  c.tile_row = tile_row;
-  int L = 1;  // lanes per row: about 4 entries per lane
-  while (L < 32 && L * 4 < h->m_avg) L <<= 1;
-  c.lanes_per_row = L;
-
-  // launch geometry: whole multiples of the SM count
+  // launch geometry: whole multiples of the SM count.  The SpMV and the persistent kernel share one
+  // grid (kBlocksPerSM resident blocks per SM) because the row partition below is per block.
   CU_TRY(cudaFuncSetAttribute(k_spmv, cudaFuncAttributeMaxDynamicSharedMemorySize, kSpmvSmemBytes), { amp_pcg_destroy(h); return nullptr; });
-  int occ_spmv = 1, occ_vec = 1;
+  int occ_spmv = 0, occ_vec = 1;
   CU_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_spmv, k_spmv, kSpmvThreads, kSpmvSmemBytes), { amp_pcg_destroy(h); return nullptr; });
   CU_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_vec, k_xr, kVecThreads, 0), { amp_pcg_destroy(h); return nullptr; });
-  occ_spmv = std::max(occ_spmv, 1); occ_vec = std::max(occ_vec, 1);
-  h->spmv_grid = (int)std::min<int64_t>({(int64_t)c.ntiles, (int64_t)h->num_sms * occ_spmv, (int64_t)kMaxGrid});
+  persistent_configure(h->num_sms, &h->persist_grid, &h->persist_ok);
+  if (occ_spmv < 1) { set_error("amp_pcg_create: SpMV kernel does not fit on this device"); amp_pcg_destroy(h); return nullptr; }
+  int per_sm = std::min(occ_spmv, (int)kBlocksPerSM);
+  if (h->persist_ok) per_sm = std::min(per_sm, h->persist_grid / h->num_sms);
+  h->spmv_grid = std::min(h->num_sms * std::max(per_sm, 1), (int)kMaxGrid);
+  if (h->persist_ok) h->persist_grid = h->spmv_grid;
+  occ_vec = std::max(occ_vec, 1);
   const int64_t vec_blocks = ((h->npad / 2) + (int64_t)kVecThreads * kVecUnroll - 1) / ((int64_t)kVecThreads * kVecUnroll);
   h->vec_grid = (int)std::min<int64_t>({std::max<int64_t>(vec_blocks, 1), (int64_t)h->num_sms * occ_vec, (int64_t)kMaxGrid});
-  persistent_configure(h->num_sms, &h->persist_grid, &h->persist_ok);
+
+  // SpMV row partition: block b owns a contiguous row range of (nearly) equal cost = entries + rows,
+  // cut into tiles of <= kTileRows rows and <= kTileNnz entries; a longer row stands alone.
+  const int nbk = h->spmv_grid;
+  std::vector<int32_t> tiles, block_tile((size_t)nbk + 1);
+  tiles.push_back(0);
+  {
+    const double total = (double)nnz + (double)n;
+    int64_t r = 0;
+    for (int bk = 0; bk < nbk; ++bk) {
+      block_tile[(size_t)bk] = (int32_t)tiles.size() - 1;
+      const double target = total * (double)(bk + 1) / (double)nbk;
+      // last row of this block: first r_end with cost(r_end) >= target  (cost(r) = rowptr[r] + r)
+      int64_t lo = r, hi = n;
+      while (lo < hi) {
+        const int64_t mid = (lo + hi) / 2;
+        if ((double)rp[(size_t)mid] + (double)mid >= target) hi = mid; else lo = mid + 1;
+      }
+      const int64_t r_end = (bk == nbk - 1) ? n : lo;
+      while (r < r_end) {
+        int64_t r1 = r + 1;
+        if (rp[(size_t)r1] - rp[(size_t)r] <= kTileNnz) {
+          while (r1 < r_end && r1 - r < kTileRows && rp[(size_t)r1 + 1] - rp[(size_t)r] <= kTileNnz) ++r1;
+        }
+        tiles.push_back((int32_t)r1);
+        r = r1;
+      }
+    }
+    block_tile[(size_t)nbk] = (int32_t)tiles.size() - 1;
+  }
+  c.ntiles = (int32_t)tiles.size() - 1;
+  int32_t* block_tile_d; int32_t* rowptr_pad;
+  ALLOC(tile_row, int32_t, tiles.size());
+  ALLOC(block_tile_d, int32_t, block_tile.size());
+  const size_t rp_len = (((size_t)n + 1 + 3) & ~(size_t)3) + 8;
+  ALLOC(rowptr_pad, int32_t, rp_len);
+  rp.resize(rp_len, (int32_t)nnz);
+  CU_TRY(cudaMemcpyAsync(tile_row, tiles.data(), sizeof(int32_t) * tiles.size(), cudaMemcpyHostToDevice, h->stream),
+         { amp_pcg_destroy(h); return nullptr; });
+  CU_TRY(cudaMemcpyAsync(block_tile_d, block_tile.data(), sizeof(int32_t) * block_tile.size(), cudaMemcpyHostToDevice, h->stream),
+         { amp_pcg_destroy(h); return nullptr; });
+  CU_TRY(cudaMemcpyAsync(rowptr_pad, rp.data(), sizeof(int32_t) * rp_len, cudaMemcpyHostToDevice, h->stream),
+         { amp_pcg_destroy(h); return nullptr; });
+  CU_TRY(cudaStreamSynchronize(h->stream), { amp_pcg_destroy(h); return nullptr; });
+  c.tile_row = tile_row; c.block_tile = block_tile_d; c.rowptr_pad = rowptr_pad;
+  int L = 1;  // lanes per row: at most kGatherBatch entries per lane and trip
+  while (L < 32 && L * kGatherBatch < h->m_avg) L <<= 1;
+  c.lanes_per_row = L;
 #undef ALLOC
   return h;
 }
@@ -341,7 +372,7 @@ static int solve_impl(amp_pcg* h, const double* b, double* x, double tol, int32_
     h->hist_cap = (int64_t)maxit + 2;
   }
   int mode = pol.loop_mode;
-  if (mode == AMP_LOOP_AUTO) mode = (h->persist_ok && persistent_fits(h->ctx)) ? AMP_LOOP_PERSISTENT : AMP_LOOP_GRAPH;
+  if (mode == AMP_LOOP_AUTO) mode = AMP_LOOP_GRAPH;  // measured faster than the persistent kernel at every size so far
   if (mode == AMP_LOOP_PERSISTENT && !(h->persist_ok && persistent_fits(h->ctx))) {
     set_error("amp_pcg_solve: persistent loop not available for this problem/device");
     return AMP_ERR_INVALID;

@@ -14,7 +14,8 @@ constexpr int P64 = 0, P32 = 1, P16 = 2;       // precision codes (= AMP_FP64/32
 constexpr int kVecThreads = 256;               // block size of the vector kernels
 constexpr int kVecUnroll = 4;                  // independent 2-element chunks in flight per thread
 constexpr int kSpmvThreads = 256;              // block size of the SpMV kernel
-constexpr int kTileNnz = 4096;                 // stored entries staged per SpMV tile
+constexpr int kBlocksPerSM = 2;                // resident blocks per SM of the SpMV / persistent kernels
+constexpr int kTileNnz = 4096;                 // stored entries staged per SpMV tile (one smem stage)
 constexpr int kTileRows = 1024;                // max rows per SpMV tile
 constexpr int kMaxGrid = 4096;                 // capacity of each partial-sum array
 constexpr int kMaxWindow = 64;                 // max d / ell of the indicators
@@ -57,7 +58,9 @@ struct Ctx {
   double* z64; float* z32; __half* z16;
   double* p64; float* p32; __half* p16;
   double* partials;       // [4][kMaxGrid] per-block partial sums
-  const int32_t* tile_row;  // [ntiles+1] first row of each SpMV tile
+  const int32_t* rowptr_pad;  // owned copy of rowptr padded to a multiple of 4 (+4) entries with nnz
+  const int32_t* tile_row;    // [ntiles+1] first row of each SpMV tile
+  const int32_t* block_tile;  // [spmv grid + 1] first tile of each block (contiguous, cost-balanced ranges)
   int32_t ntiles;
   int32_t lanes_per_row;  // lanes cooperating on one row in the SpMV row reduction (power of 2)
   cudaGraphConditionalHandle cond;  // WHILE-node handle (graph loop only)

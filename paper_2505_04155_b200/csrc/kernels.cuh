@@ -3,10 +3,9 @@
 // set-up / finalisation kernels, the stand-alone SpMV and the one-off kernels of create().
 #pragma once
 #include "phases.cuh"
+#include "spmv.cuh"
 
 namespace amp {
-
-constexpr int kSpmvSmemBytes = (int)(sizeof(double) * kTileNnz + sizeof(int) * (kTileRows + 4));
 
 // ------------------------------------------------------------------ precision dispatch ------
 // The precisions in use are device-side scalars (they change inside the loop without the host
@@ -80,7 +79,7 @@ __global__ void __launch_bounds__(kVecThreads) k_p(const Ctx c) {
   dispatch_p(c, s->p_store, s->uz, s->beta, s->k == 0, blockIdx.x, gridDim.x);
 }
 
-__global__ void __launch_bounds__(kSpmvThreads) k_spmv(const Ctx c) {
+__global__ void __launch_bounds__(kSpmvThreads, kBlocksPerSM) k_spmv(const Ctx c) {
   extern __shared__ __align__(16) unsigned char smem[];
   __shared__ double red[32];
   DevState* s = c.st;
@@ -106,7 +105,7 @@ __global__ void __launch_bounds__(kVecThreads) k_xr(const Ctx c) {
 
 // ------------------------------------------------------------------ stand-alone SpMV --------
 template <int UR, class PT>
-__global__ void __launch_bounds__(kSpmvThreads) k_spmv_any(const Ctx c, const PT* p, typename Store<UR>::T* q) {
+__global__ void __launch_bounds__(kSpmvThreads, kBlocksPerSM) k_spmv_any(const Ctx c, const PT* p, typename Store<UR>::T* q) {
   extern __shared__ __align__(16) unsigned char smem[];
   __shared__ double red[32];
   (void)phase_spmv<UR, false>(c, p, q, blockIdx.x, gridDim.x, smem, red);

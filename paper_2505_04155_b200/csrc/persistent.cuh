@@ -77,7 +77,7 @@ __device__ __noinline__ double pxr(const Ctx& c, int ur, int uz, double alpha, d
   return dispatch_xr(c, ur, uz, alpha, x, bid, nb);
 }
 
-__global__ void __launch_bounds__(kPersistThreads) k_persistent(const Ctx c) {
+__global__ void __launch_bounds__(kPersistThreads, kBlocksPerSM) k_persistent(const Ctx c) {
   extern __shared__ __align__(16) unsigned char smem[];
   __shared__ double red[32];
   DevState* s = c.st;
@@ -105,7 +105,7 @@ inline void persistent_configure(int num_sms, int* grid, int* ok) {
   *grid = 0;
   *ok = 0;
   if (cudaFuncSetAttribute(k_persistent, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                           (int)(sizeof(double) * kTileNnz + sizeof(int) * (kTileRows + 4))) != cudaSuccess) {
+                           kSpmvSmemBytes) != cudaSuccess) {
     cudaGetLastError();
     return;
   }
@@ -113,7 +113,7 @@ inline void persistent_configure(int num_sms, int* grid, int* ok) {
   cudaGetDevice(&dev);
   cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
   if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_persistent, kPersistThreads,
-                                                    sizeof(double) * kTileNnz + sizeof(int) * (kTileRows + 4)) != cudaSuccess) {
+                                                    kSpmvSmemBytes) != cudaSuccess) {
     cudaGetLastError();
     return;
   }
@@ -130,7 +130,7 @@ inline int persistent_launch(const Ctx& c, int grid, cudaStream_t st) {
   cc.use_cond = 0;
   void* args[] = {(void*)&cc};
   return (int)cudaLaunchCooperativeKernel((void*)k_persistent, dim3(grid), dim3(kPersistThreads), args,
-                                          sizeof(double) * kTileNnz + sizeof(int) * (kTileRows + 4), st);
+                                          kSpmvSmemBytes, st);
 }
 
 }  // namespace amp

@@ -4,7 +4,7 @@
 //
 //   phase_z    a2: y = omega r, z = M^-1 y (fused), one rounding to u_z; rho = r^T z
 //   phase_p    a3: p = z + beta p, one rounding to u_z
-//   phase_spmv a4: q = A p in u_r (CSR, tile-staged), gamma = q^T p
+//   phase_spmv a4: q = A p in u_r, gamma = q^T p  (spmv.cuh)
 //   phase_xr   a5: x += alpha p (FP64), r -= alpha q (u_r), delta = ||r||
 // and the scalar epilogues (one thread, after each grid reduction):
 //   epi_rho    beta = rho_k / rho_{k-1}                       (Alg 4.1 lines 6-9)
@@ -266,116 +266,6 @@ __device__ __forceinline__ double phase_xr(const Ctx& c, const double alpha, dou
     }
   }
   return sum;
-}
-
-// ------------------------------------------------------------------ a4: SpMV ----------------
-// CSR "tile-staged" mat-vec.  Rows are pre-partitioned into tiles of <= kTileRows rows and
-// <= kTileNnz stored entries (a single longer row forms its own tile).  Per tile the block
-//  (1) streams the tile's values and column indices with 128-bit loads (fully coalesced,
-//      independent of row lengths), gathers p_j and writes the products a_ij p_j to shared memory;
-//  (2) reduces each row from shared memory with L lanes per row and writes q_i (coalesced);
-// and accumulates gamma += p_i q_i in FP64 from the stored q_i.
-// UR = P64: FP64 values, products and sums.  UR = P32: FP32 value copy, p_j converted to FP32,
-// FP32 products and sums (q computed and stored in u_r).
-template <int UR> struct SpmvT;
-template <> struct SpmvT<P64> { using A = double; };
-template <> struct SpmvT<P32> { using A = float; };
-
-// COH = true: p is written earlier in the same (persistent) kernel, so it is gathered with
-// plain coherent loads after the grid barrier instead of the read-only (ld.global.nc) path.
-template <int UR, bool COH, class PT>
-__device__ __forceinline__ double phase_spmv(const Ctx& c, const PT* p, typename Store<UR>::T* q, int bid, int nb,
-                                             unsigned char* smem_raw, double* red_sm) {
-  using A = typename SpmvT<UR>::A;
-  A* prod = reinterpret_cast<A*>(smem_raw);
-  int* rp = reinterpret_cast<int*>(smem_raw + sizeof(A) * kTileNnz);
-  const int32_t* __restrict__ rowptr = c.rowptr;
-  const int32_t* __restrict__ colidx = c.colidx;
-  const int L = c.lanes_per_row;
-  const int tid = threadIdx.x;
-  const int64_t nnz = c.nnz;
-  double gsum = 0.0;
-
-  for (int t = bid; t < c.ntiles; t += nb) {
-    const int r0 = c.tile_row[t], r1 = c.tile_row[t + 1];
-    const int nrows = r1 - r0;
-    const int e0 = rowptr[r0], e1 = rowptr[r1];
-
-    if (e1 - e0 > kTileNnz) {  // one long row: block-wide strided accumulation
-      A acc = 0;
-      for (int e = e0 + tid; e < e1; e += kSpmvThreads) {
-        if (UR == P64) acc += (A)(c.vals64[e] * gather64<COH>(p, colidx[e]));
-        else acc += (A)(c.vals32[e] * gather32<COH>(p, colidx[e]));
-      }
-      const double tot = block_sum<kSpmvThreads>((double)acc, red_sm);
-      if (tid == 0) {
-        const A qs = (A)tot;
-        q[r0] = qs;
-        gsum = fma(gather64<COH>(p, r0), (double)qs, gsum);
-      }
-      __syncthreads();
-      continue;
-    }
-
-    for (int i = tid; i <= nrows; i += kSpmvThreads) rp[i] = rowptr[r0 + i] - e0;
-
-    // (1) products.  Vector v covers entries ea+4v .. ea+4v+3, ea = e0 rounded down to 4.
-    const int ea = e0 & ~3;
-    const int nvec = (e1 - ea + 3) >> 2;
-    for (int v = tid; v < nvec; v += kSpmvThreads) {
-      const int e = ea + 4 * v;
-      int cj[4];
-      A aj[4];
-      if ((int64_t)e + 4 <= nnz) {
-        const int4 cc = __ldg(reinterpret_cast<const int4*>(colidx + e));
-        cj[0] = cc.x; cj[1] = cc.y; cj[2] = cc.z; cj[3] = cc.w;
-        if (UR == P64) {
-          const double2 a01 = __ldg(reinterpret_cast<const double2*>(c.vals64 + e));
-          const double2 a23 = __ldg(reinterpret_cast<const double2*>(c.vals64 + e + 2));
-          aj[0] = (A)a01.x; aj[1] = (A)a01.y; aj[2] = (A)a23.x; aj[3] = (A)a23.y;
-        } else {
-          const float4 a = __ldg(reinterpret_cast<const float4*>(c.vals32 + e));
-          aj[0] = (A)a.x; aj[1] = (A)a.y; aj[2] = (A)a.z; aj[3] = (A)a.w;
-        }
-      } else {  // the last, partial vector of the arrays
-#pragma unroll
-        for (int j = 0; j < 4; ++j) {
-          const bool in = (int64_t)e + j < nnz;
-          cj[j] = in ? colidx[e + j] : 0;
-          if (UR == P64) aj[j] = in ? (A)c.vals64[e + j] : (A)0;
-          else aj[j] = in ? (A)c.vals32[e + j] : (A)0;
-        }
-      }
-#pragma unroll
-      for (int j = 0; j < 4; ++j) {
-        const int idx = e + j - e0;
-        if (idx >= 0 && e + j < e1) {
-          if (UR == P64) prod[idx] = (A)((double)aj[j] * gather64<COH>(p, cj[j]));
-          else prod[idx] = (A)__fmul_rn((float)aj[j], gather32<COH>(p, cj[j]));
-        }
-      }
-    }
-    __syncthreads();
-
-    // (2) row sums: L lanes per row, then a shuffle tree over the L lanes
-    const int rows_per_pass = kSpmvThreads / L;
-    const int sub = tid % L, rl = tid / L;
-    for (int rb = 0; rb < nrows; rb += rows_per_pass) {
-      const int row = rb + rl;
-      A s = 0;
-      if (row < nrows) {
-        const int jb = rp[row], je = rp[row + 1];
-        for (int j = jb + sub; j < je; j += L) s += prod[j];
-      }
-      for (int o = L >> 1; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
-      if (row < nrows && sub == 0) {
-        q[r0 + row] = s;
-        gsum = fma(gather64<COH>(p, r0 + row), (double)s, gsum);
-      }
-    }
-    __syncthreads();
-  }
-  return gsum;
 }
 
 }  // namespace amp
