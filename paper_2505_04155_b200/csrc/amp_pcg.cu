@@ -46,7 +46,7 @@ struct amp_pcg {
   int* h_flag = nullptr;        // pinned: done flag polled by the stream loop
   double* hist = nullptr;
   int64_t hist_cap = 0;
-  int vec_grid = 1, spmv_grid = 1, persist_grid = 0, persist_ok = 0;
+  int vec_grid = 1, grid_z = 1, grid_p = 1, grid_xr = 1, spmv_grid = 1, persist_grid = 0, persist_ok = 0;
   // graph loop
   cudaGraph_t graph = nullptr;
   cudaGraphExec_t graph_exec = nullptr;
@@ -150,7 +150,7 @@ extern "C" amp_pcg_t* amp_pcg_create(int64_t n, int64_t nnz, const int32_t* rowp
     if (!dst) { amp_pcg_destroy(h); return nullptr; }                   \
   } while (0)
   const size_t np = (size_t)h->npad;
-  double* dinv64; float* dinv32; float* vals32; int* flags; int32_t* tile_row;
+  double* dinv64; float* dinv32; float* vals32; int* flags;
   ALLOC(dinv64, double, np); ALLOC(dinv32, float, np);
   ALLOC(vals32, float, (size_t)nnz + 8);
   ALLOC(c.r64, double, np); ALLOC(c.r32, float, np);
@@ -193,66 +193,80 @@ extern "C" amp_pcg_t* amp_pcg_create(int64_t n, int64_t nnz, const int32_t* rowp
   // launch geometry: whole multiples of the SM count.  The SpMV and the persistent kernel share one
   // grid (kBlocksPerSM resident blocks per SM) because the row partition below is per block.
   CU_TRY(cudaFuncSetAttribute(k_spmv, cudaFuncAttributeMaxDynamicSharedMemorySize, kSpmvSmemBytes), { amp_pcg_destroy(h); return nullptr; });
-  int occ_spmv = 0, occ_vec = 1;
+  int occ_spmv = 0;
   CU_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_spmv, k_spmv, kSpmvThreads, kSpmvSmemBytes), { amp_pcg_destroy(h); return nullptr; });
-  CU_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_vec, k_xr, kVecThreads, 0), { amp_pcg_destroy(h); return nullptr; });
   persistent_configure(h->num_sms, &h->persist_grid, &h->persist_ok);
   if (occ_spmv < 1) { set_error("amp_pcg_create: SpMV kernel does not fit on this device"); amp_pcg_destroy(h); return nullptr; }
   int per_sm = std::min(occ_spmv, (int)kBlocksPerSM);
   if (h->persist_ok) per_sm = std::min(per_sm, h->persist_grid / h->num_sms);
   h->spmv_grid = std::min(h->num_sms * std::max(per_sm, 1), (int)kMaxGrid);
   if (h->persist_ok) h->persist_grid = h->spmv_grid;
-  occ_vec = std::max(occ_vec, 1);
-  const int64_t vec_blocks = ((h->npad / 2) + (int64_t)kVecThreads * kVecUnroll - 1) / ((int64_t)kVecThreads * kVecUnroll);
-  h->vec_grid = (int)std::min<int64_t>({std::max<int64_t>(vec_blocks, 1), (int64_t)h->num_sms * occ_vec, (int64_t)kMaxGrid});
+  // vector kernels: a whole number of equally long grid-stride trips per block, at most one full wave
+  auto vec_grid_for = [&](const void* kern) -> int {
+    int occ = 1;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, kVecThreads, 0) != cudaSuccess) { cudaGetLastError(); occ = 1; }
+    const int64_t per_trip = (int64_t)kVecThreads * kVecUnrollNarrow;  // pairs per block and trip
+    const int64_t max_grid = std::min<int64_t>((int64_t)h->num_sms * std::max(occ, 1), (int64_t)kMaxGrid);
+    const int64_t npair = h->npad / 2;
+    const int64_t trips = std::max<int64_t>(1, (npair + max_grid * per_trip - 1) / (max_grid * per_trip));
+    return (int)std::max<int64_t>(1, (npair + trips * per_trip - 1) / (trips * per_trip));
+  };
+  h->grid_z = vec_grid_for((const void*)k_z);
+  h->grid_p = vec_grid_for((const void*)k_p);
+  h->grid_xr = vec_grid_for((const void*)k_xr);
+  h->vec_grid = vec_grid_for((const void*)k_setup);
 
-  // SpMV row partition: block b owns a contiguous row range of (nearly) equal cost = entries + rows,
-  // cut into tiles of <= kTileRows rows and <= kTileNnz entries; a longer row stands alone.
-  const int nbk = h->spmv_grid;
-  std::vector<int32_t> tiles, block_tile((size_t)nbk + 1);
-  tiles.push_back(0);
+  // SpMV row partition: every warp of the grid owns a contiguous row range of (nearly) equal
+  // cost = entries + rows, cut into tiles of <= kTileRows rows and <= tile_cap entries; a longer
+  // row stands alone.  Small matrices get smaller tiles so that the work spreads over the SMs.
+  // lanes per row (compile-time variants 1, 4, 32)
+  c.lanes_per_row = (h->m_avg <= 12.0) ? 1 : (h->m_avg <= 64.0 ? 4 : 32);
+  const int rpp = 32 / c.lanes_per_row;  // rows per warp pass
+  const int nwarps = h->spmv_grid * kSpmvWarps;
+  int tile_cap = (int)std::min<int64_t>(kTileNnz, std::max<int64_t>(128, ((nnz + nwarps - 1) / nwarps + 31) / 32 * 32));
+  std::vector<int2> tiles;
+  std::vector<int32_t> warp_tile((size_t)nwarps + 1);
   {
     const double total = (double)nnz + (double)n;
     int64_t r = 0;
-    for (int bk = 0; bk < nbk; ++bk) {
-      block_tile[(size_t)bk] = (int32_t)tiles.size() - 1;
-      const double target = total * (double)(bk + 1) / (double)nbk;
-      // last row of this block: first r_end with cost(r_end) >= target  (cost(r) = rowptr[r] + r)
+    for (int w = 0; w < nwarps; ++w) {
+      warp_tile[(size_t)w] = (int32_t)tiles.size();
+      const double target = total * (double)(w + 1) / (double)nwarps;
+      // last row of this warp: first r_end with cost(r_end) >= target  (cost(r) = rowptr[r] + r)
       int64_t lo = r, hi = n;
       while (lo < hi) {
         const int64_t mid = (lo + hi) / 2;
         if ((double)rp[(size_t)mid] + (double)mid >= target) hi = mid; else lo = mid + 1;
       }
-      const int64_t r_end = (bk == nbk - 1) ? n : lo;
+      const int64_t r_end = (w == nwarps - 1) ? n : lo;
       while (r < r_end) {
         int64_t r1 = r + 1;
-        if (rp[(size_t)r1] - rp[(size_t)r] <= kTileNnz) {
-          while (r1 < r_end && r1 - r < kTileRows && rp[(size_t)r1 + 1] - rp[(size_t)r] <= kTileNnz) ++r1;
+        if (rp[(size_t)r1] - rp[(size_t)r] <= tile_cap) {
+          while (r1 < r_end && r1 - r < kTileRows && rp[(size_t)r1 + 1] - rp[(size_t)r] <= tile_cap) ++r1;
+          if (r1 < r_end && r1 - r > rpp) r1 = r + (r1 - r) / rpp * rpp;  // whole warp passes
         }
-        tiles.push_back((int32_t)r1);
+        tiles.push_back(make_int2((int)r, rp[(size_t)r]));
         r = r1;
       }
     }
-    block_tile[(size_t)nbk] = (int32_t)tiles.size() - 1;
+    warp_tile[(size_t)nwarps] = (int32_t)tiles.size();
+    tiles.push_back(make_int2((int)n, (int)nnz));
   }
   c.ntiles = (int32_t)tiles.size() - 1;
-  int32_t* block_tile_d; int32_t* rowptr_pad;
-  ALLOC(tile_row, int32_t, tiles.size());
-  ALLOC(block_tile_d, int32_t, block_tile.size());
+  int2* tile_desc; int32_t* warp_tile_d; int32_t* rowptr_pad;
+  ALLOC(tile_desc, int2, tiles.size());
+  ALLOC(warp_tile_d, int32_t, warp_tile.size());
   const size_t rp_len = (((size_t)n + 1 + 3) & ~(size_t)3) + 8;
   ALLOC(rowptr_pad, int32_t, rp_len);
   rp.resize(rp_len, (int32_t)nnz);
-  CU_TRY(cudaMemcpyAsync(tile_row, tiles.data(), sizeof(int32_t) * tiles.size(), cudaMemcpyHostToDevice, h->stream),
+  CU_TRY(cudaMemcpyAsync(tile_desc, tiles.data(), sizeof(int2) * tiles.size(), cudaMemcpyHostToDevice, h->stream),
          { amp_pcg_destroy(h); return nullptr; });
-  CU_TRY(cudaMemcpyAsync(block_tile_d, block_tile.data(), sizeof(int32_t) * block_tile.size(), cudaMemcpyHostToDevice, h->stream),
+  CU_TRY(cudaMemcpyAsync(warp_tile_d, warp_tile.data(), sizeof(int32_t) * warp_tile.size(), cudaMemcpyHostToDevice, h->stream),
          { amp_pcg_destroy(h); return nullptr; });
   CU_TRY(cudaMemcpyAsync(rowptr_pad, rp.data(), sizeof(int32_t) * rp_len, cudaMemcpyHostToDevice, h->stream),
          { amp_pcg_destroy(h); return nullptr; });
   CU_TRY(cudaStreamSynchronize(h->stream), { amp_pcg_destroy(h); return nullptr; });
-  c.tile_row = tile_row; c.block_tile = block_tile_d; c.rowptr_pad = rowptr_pad;
-  int L = 1;  // lanes per row: at most kGatherBatch entries per lane and trip
-  while (L < 32 && L * kGatherBatch < h->m_avg) L <<= 1;
-  c.lanes_per_row = L;
+  c.tile_desc = tile_desc; c.warp_tile = warp_tile_d; c.rowptr_pad = rowptr_pad;
 #undef ALLOC
   return h;
 }
@@ -308,10 +322,10 @@ extern "C" int amp_spmv(amp_pcg_t* h, int mat_prec, int vec_prec, const void* p,
 
 // ------------------------------------------------------------------ graph loop --------------
 static void launch_iteration(amp_pcg* h, const Ctx& c, cudaStream_t s) {
-  k_z<<<h->vec_grid, kVecThreads, 0, s>>>(c);
-  k_p<<<h->vec_grid, kVecThreads, 0, s>>>(c);
+  k_z<<<h->grid_z, kVecThreads, 0, s>>>(c);
+  k_p<<<h->grid_p, kVecThreads, 0, s>>>(c);
   k_spmv<<<h->spmv_grid, kSpmvThreads, kSpmvSmemBytes, s>>>(c);
-  k_xr<<<h->vec_grid, kVecThreads, 0, s>>>(c);
+  k_xr<<<h->grid_xr, kVecThreads, 0, s>>>(c);
 }
 
 // One graph = one WHILE conditional node whose body is the four loop kernels; the condition is

@@ -12,11 +12,29 @@ namespace amp {
 
 constexpr int P64 = 0, P32 = 1, P16 = 2;       // precision codes (= AMP_FP64/32/16 of the C ABI)
 constexpr int kVecThreads = 256;               // block size of the vector kernels
-constexpr int kVecUnroll = 4;                  // independent 2-element chunks in flight per thread
-constexpr int kSpmvThreads = 256;              // block size of the SpMV kernel
-constexpr int kBlocksPerSM = 2;                // resident blocks per SM of the SpMV / persistent kernels
-constexpr int kTileNnz = 4096;                 // stored entries staged per SpMV tile (one smem stage)
-constexpr int kTileRows = 1024;                // max rows per SpMV tile
+constexpr int kVecUnrollNarrow = 4;            // independent 2-element chunks in flight per thread (some operand < FP64)
+constexpr int kVecUnrollWide = 2;              // ... when every operand is FP64 (same bytes in flight, half the registers)
+#ifndef AMP_SPMV_WARPS
+#define AMP_SPMV_WARPS 32
+#endif
+#ifndef AMP_TILE_NNZ
+#define AMP_TILE_NNZ 256
+#endif
+#ifndef AMP_TILE_ROWS
+#define AMP_TILE_ROWS 64
+#endif
+#ifndef AMP_STAGES
+#define AMP_STAGES 2
+#endif
+#ifndef AMP_BLOCKS_PER_SM
+#define AMP_BLOCKS_PER_SM 1
+#endif
+constexpr int kSpmvWarps = AMP_SPMV_WARPS;     // warps per SpMV block, each with a private stage ring
+constexpr int kSpmvThreads = 32 * kSpmvWarps;  // block size of the SpMV / persistent kernels
+constexpr int kBlocksPerSM = AMP_BLOCKS_PER_SM;  // resident blocks per SM of the SpMV / persistent kernels
+constexpr int kTileNnz = AMP_TILE_NNZ;         // stored entries staged per SpMV tile (one warp stage)
+constexpr int kTileRows = AMP_TILE_ROWS;       // max rows per SpMV tile
+constexpr int kStages = AMP_STAGES;            // stages of each warp's ring
 constexpr int kMaxGrid = 4096;                 // capacity of each partial-sum array
 constexpr int kMaxWindow = 64;                 // max d / ell of the indicators
 
@@ -59,8 +77,8 @@ struct Ctx {
   double* p64; float* p32; __half* p16;
   double* partials;       // [4][kMaxGrid] per-block partial sums
   const int32_t* rowptr_pad;  // owned copy of rowptr padded to a multiple of 4 (+4) entries with nnz
-  const int32_t* tile_row;    // [ntiles+1] first row of each SpMV tile
-  const int32_t* block_tile;  // [spmv grid + 1] first tile of each block (contiguous, cost-balanced ranges)
+  const int2* tile_desc;      // [ntiles+1] (first row, first entry) of each SpMV tile
+  const int32_t* warp_tile;   // [spmv grid * kSpmvWarps + 1] first tile of each warp (contiguous, cost-balanced ranges)
   int32_t ntiles;
   int32_t lanes_per_row;  // lanes cooperating on one row in the SpMV row reduction (power of 2)
   cudaGraphConditionalHandle cond;  // WHILE-node handle (graph loop only)
@@ -94,19 +112,24 @@ template <> __device__ __forceinline__ double round_to<P64>(double v) { return v
 template <> __device__ __forceinline__ double round_to<P32>(double v) { return (double)__double2float_rn(v); }
 template <> __device__ __forceinline__ double round_to<P16>(double v) { return (double)__half2float(__double2half(v)); }
 
-// load / store of 2 consecutive elements (element index 2*pair), values exchanged as FP64.
-// Stored values convert to FP64 exactly; stores round once (RN-even, direct from the double).
-__device__ __forceinline__ void load2(const double* a, int64_t pair, double& v0, double& v1) {
-  const double2 t = reinterpret_cast<const double2*>(a)[pair];
-  v0 = t.x; v1 = t.y;
+// load / store of 2 consecutive elements (element index 2*pair).  Loads return the raw packed
+// pair so that many can be in flight in few registers; unpack() converts to FP64 exactly;
+// stores round once (RN-even, direct from the double).
+template <class T> struct Raw2;
+template <> struct Raw2<double> { using T = double2; };
+template <> struct Raw2<float> { using T = float2; };
+template <> struct Raw2<__half> { using T = __half2; };
+__device__ __forceinline__ double2 load_raw(const double* a, int64_t pair) { return reinterpret_cast<const double2*>(a)[pair]; }
+__device__ __forceinline__ float2 load_raw(const float* a, int64_t pair) { return reinterpret_cast<const float2*>(a)[pair]; }
+__device__ __forceinline__ __half2 load_raw(const __half* a, int64_t pair) { return reinterpret_cast<const __half2*>(a)[pair]; }
+__device__ __forceinline__ void unpack(const double2 t, double& v0, double& v1) { v0 = t.x; v1 = t.y; }
+__device__ __forceinline__ void unpack(const float2 t, double& v0, double& v1) { v0 = (double)t.x; v1 = (double)t.y; }
+__device__ __forceinline__ void unpack(const __half2 t, double& v0, double& v1) {
+  const float2 f = __half22float2(t);
+  v0 = (double)f.x; v1 = (double)f.y;
 }
-__device__ __forceinline__ void load2(const float* a, int64_t pair, double& v0, double& v1) {
-  const float2 t = reinterpret_cast<const float2*>(a)[pair];
-  v0 = (double)t.x; v1 = (double)t.y;
-}
-__device__ __forceinline__ void load2(const __half* a, int64_t pair, double& v0, double& v1) {
-  const float2 t = __half22float2(reinterpret_cast<const __half2*>(a)[pair]);
-  v0 = (double)t.x; v1 = (double)t.y;
+template <class T> __device__ __forceinline__ void load2(const T* a, int64_t pair, double& v0, double& v1) {
+  unpack(load_raw(a, pair), v0, v1);
 }
 __device__ __forceinline__ void store2(double* a, int64_t pair, double v0, double v1) {
   reinterpret_cast<double2*>(a)[pair] = make_double2(v0, v1);

@@ -38,17 +38,23 @@ __device__ __forceinline__ void dispatch_p(const Ctx& c, int ps, int uz, double 
   }
 }
 
-template <bool COH>
-__device__ __forceinline__ double dispatch_spmv(const Ctx& c, int ur, int uz, int bid, int nb, unsigned char* smem,
-                                                double* red) {
+// lanes per row of the SpMV row-sum phase: 1 (short rows), 4 or 32 (Ctx::lanes_per_row, set in create)
+template <bool COH, int L>
+__device__ __forceinline__ double dispatch_spmv_l(const Ctx& c, int ur, int uz, int bid, int nb, unsigned char* smem) {
   if (ur == P64) {
-    if (uz == P64) return phase_spmv<P64, COH>(c, c.p64, c.q64, bid, nb, smem, red);
-    if (uz == P32) return phase_spmv<P64, COH>(c, c.p32, c.q64, bid, nb, smem, red);
-    return phase_spmv<P64, COH>(c, c.p16, c.q64, bid, nb, smem, red);
+    if (uz == P64) return phase_spmv<P64, COH, L>(c, c.p64, c.q64, bid, nb, smem);
+    if (uz == P32) return phase_spmv<P64, COH, L>(c, c.p32, c.q64, bid, nb, smem);
+    return phase_spmv<P64, COH, L>(c, c.p16, c.q64, bid, nb, smem);
   }
-  if (uz == P64) return phase_spmv<P32, COH>(c, c.p64, c.q32, bid, nb, smem, red);
-  if (uz == P32) return phase_spmv<P32, COH>(c, c.p32, c.q32, bid, nb, smem, red);
-  return phase_spmv<P32, COH>(c, c.p16, c.q32, bid, nb, smem, red);
+  if (uz == P64) return phase_spmv<P32, COH, L>(c, c.p64, c.q32, bid, nb, smem);
+  if (uz == P32) return phase_spmv<P32, COH, L>(c, c.p32, c.q32, bid, nb, smem);
+  return phase_spmv<P32, COH, L>(c, c.p16, c.q32, bid, nb, smem);
+}
+template <bool COH>
+__device__ __forceinline__ double dispatch_spmv(const Ctx& c, int ur, int uz, int bid, int nb, unsigned char* smem) {
+  if (c.lanes_per_row == 1) return dispatch_spmv_l<COH, 1>(c, ur, uz, bid, nb, smem);
+  if (c.lanes_per_row == 4) return dispatch_spmv_l<COH, 4>(c, ur, uz, bid, nb, smem);
+  return dispatch_spmv_l<COH, 32>(c, ur, uz, bid, nb, smem);
 }
 
 __device__ __forceinline__ double dispatch_xr(const Ctx& c, int ur, int uz, double alpha, double* x, int bid, int nb) {
@@ -63,17 +69,17 @@ __device__ __forceinline__ double dispatch_xr(const Ctx& c, int ur, int uz, doub
 }
 
 // ------------------------------------------------------------------ loop kernels ------------
-__global__ void __launch_bounds__(kVecThreads) k_z(const Ctx c) {
+__global__ void __launch_bounds__(kVecThreads, 3) k_z(const Ctx c) {
   __shared__ double red[32];
   DevState* s = c.st;
   if (s->done) return;
   const int bid = blockIdx.x, nb = gridDim.x;
   const double v = dispatch_z(c, s->r_store, s->ur, s->uz, s->omega, bid, nb);
   grid_reduce<kVecThreads>(v, c.partials + 0 * kMaxGrid, &s->counter[0], bid, nb, red,
-                           [&](double tot) { epi_rho(c, tot); });
+                           [&](double tot) { epi_rho(epi_ctx(c), tot); });
 }
 
-__global__ void __launch_bounds__(kVecThreads) k_p(const Ctx c) {
+__global__ void __launch_bounds__(kVecThreads, 4) k_p(const Ctx c) {
   const DevState* s = c.st;
   if (s->done) return;
   dispatch_p(c, s->p_store, s->uz, s->beta, s->k == 0, blockIdx.x, gridDim.x);
@@ -85,30 +91,31 @@ __global__ void __launch_bounds__(kSpmvThreads, kBlocksPerSM) k_spmv(const Ctx c
   DevState* s = c.st;
   if (s->done) return;
   const int bid = blockIdx.x, nb = gridDim.x;
-  const double v = dispatch_spmv<false>(c, s->ur, s->uz, bid, nb, smem, red);
+  const double v = dispatch_spmv<false>(c, s->ur, s->uz, bid, nb, smem);
   grid_reduce<kSpmvThreads>(v, c.partials + 1 * kMaxGrid, &s->counter[1], bid, nb, red,
-                            [&](double tot) { epi_gamma(c, tot); });
+                            [&](double tot) { epi_gamma(epi_ctx(c), tot); });
 }
 
-__global__ void __launch_bounds__(kVecThreads) k_xr(const Ctx c) {
+__global__ void __launch_bounds__(kVecThreads, 2) k_xr(const Ctx c) {
   __shared__ double red[32];
   DevState* s = c.st;
   if (s->done) {  // nothing to do (converged at set-up, or breakdown): make sure the WHILE node stops
-    if (blockIdx.x == 0 && threadIdx.x == 0) set_loop_cond(c, 0);
+    if (blockIdx.x == 0 && threadIdx.x == 0) set_loop_cond(epi_ctx(c), 0);
     return;
   }
   const int bid = blockIdx.x, nb = gridDim.x;
   const double v = dispatch_xr(c, s->ur, s->uz, s->alpha, s->x, bid, nb);
   grid_reduce<kVecThreads>(v, c.partials + 2 * kMaxGrid, &s->counter[2], bid, nb, red,
-                           [&](double tot) { epi_delta(c, tot); });
+                           [&](double tot) { epi_delta(epi_ctx(c), tot); });
 }
 
 // ------------------------------------------------------------------ stand-alone SpMV --------
 template <int UR, class PT>
 __global__ void __launch_bounds__(kSpmvThreads, kBlocksPerSM) k_spmv_any(const Ctx c, const PT* p, typename Store<UR>::T* q) {
   extern __shared__ __align__(16) unsigned char smem[];
-  __shared__ double red[32];
-  (void)phase_spmv<UR, false>(c, p, q, blockIdx.x, gridDim.x, smem, red);
+  if (c.lanes_per_row == 1) (void)phase_spmv<UR, false, 1>(c, p, q, blockIdx.x, gridDim.x, smem);
+  else if (c.lanes_per_row == 4) (void)phase_spmv<UR, false, 4>(c, p, q, blockIdx.x, gridDim.x, smem);
+  else (void)phase_spmv<UR, false, 32>(c, p, q, blockIdx.x, gridDim.x, smem);
 }
 
 // ------------------------------------------------------------------ set-up / finalise -------
@@ -152,7 +159,7 @@ __global__ void __launch_bounds__(kVecThreads) k_setup(const Ctx c, int x0_zero)
     const double t2 = block_sum<kVecThreads>(s2, red);
     if (threadIdx.x == 0) {
       s->counter[3] = 0u;
-      epi_setup(c, t1, t2);
+      epi_setup(epi_ctx(c), t1, t2);
     }
   }
 }

@@ -8,8 +8,7 @@
 
 namespace amp {
 
-constexpr int kPersistThreads = 256;
-static_assert(kPersistThreads == kVecThreads && kPersistThreads == kSpmvThreads, "phases assume one block size");
+constexpr int kPersistThreads = kSpmvThreads;  // the vector phases take their block size from blockDim
 
 __device__ __forceinline__ unsigned int ld_acquire_u32(const unsigned int* p) {
   unsigned int v;
@@ -70,8 +69,8 @@ __device__ __noinline__ double pz(const Ctx& c, int rs, int ur, int uz, double o
 __device__ __noinline__ void pp(const Ctx& c, int ps, int uz, double beta, bool first, int bid, int nb) {
   dispatch_p(c, ps, uz, beta, first, bid, nb);
 }
-__device__ __noinline__ double ps_(const Ctx& c, int ur, int uz, int bid, int nb, unsigned char* smem, double* red) {
-  return dispatch_spmv<true>(c, ur, uz, bid, nb, smem, red);
+__device__ __noinline__ double ps_(const Ctx& c, int ur, int uz, int bid, int nb, unsigned char* smem) {
+  return dispatch_spmv<true>(c, ur, uz, bid, nb, smem);
 }
 __device__ __noinline__ double pxr(const Ctx& c, int ur, int uz, double alpha, double* x, int bid, int nb) {
   return dispatch_xr(c, ur, uz, alpha, x, bid, nb);
@@ -90,14 +89,14 @@ __global__ void __launch_bounds__(kPersistThreads, kBlocksPerSM) k_persistent(co
     const double omega = ldv(&s->omega);
     const bool first = (ldv(&s->k) == 0);
     double v = pz(c, rs, ur, uz, omega, bid, nb);                                                   // a2
-    grid_sync_reduce<true>(v, c.partials + 0 * kMaxGrid, s, bid, nb, red, [&](double t) { epi_rho(c, t); });
+    grid_sync_reduce<true>(v, c.partials + 0 * kMaxGrid, s, bid, nb, red, [&](double t) { epi_rho(epi_ctx(c), t); });
     pp(c, ps, uz, ldv(&s->beta), first, bid, nb);                                                   // a3
     grid_sync_reduce<false>(0.0, nullptr, s, bid, nb, red, nop);
-    v = ps_(c, ur, uz, bid, nb, smem, red);                                                         // a4
-    grid_sync_reduce<true>(v, c.partials + 1 * kMaxGrid, s, bid, nb, red, [&](double t) { epi_gamma(c, t); });
+    v = ps_(c, ur, uz, bid, nb, smem);                                                        // a4
+    grid_sync_reduce<true>(v, c.partials + 1 * kMaxGrid, s, bid, nb, red, [&](double t) { epi_gamma(epi_ctx(c), t); });
     if (ldv(&s->done)) break;  // breakdown
     v = pxr(c, ur, uz, ldv(&s->alpha), x, bid, nb);                                                 // a5
-    grid_sync_reduce<true>(v, c.partials + 2 * kMaxGrid, s, bid, nb, red, [&](double t) { epi_delta(c, t); });
+    grid_sync_reduce<true>(v, c.partials + 2 * kMaxGrid, s, bid, nb, red, [&](double t) { epi_delta(epi_ctx(c), t); });
   }
 }
 

@@ -18,7 +18,16 @@
 namespace amp {
 
 // ------------------------------------------------------------------ scalar epilogues --------
-__device__ __forceinline__ void set_loop_cond(const Ctx& c, int keep_going) {
+// what the scalar epilogues need from the kernel context (passed by value: the out-of-line
+// epilogues must not force a stack copy of the whole Ctx)
+struct EpiCtx {
+  DevState* st;
+  int64_t n;
+  cudaGraphConditionalHandle cond;
+  int32_t use_cond;
+};
+__device__ __forceinline__ EpiCtx epi_ctx(const Ctx& c) { return EpiCtx{c.st, c.n, c.cond, c.use_cond}; }
+__device__ __forceinline__ void set_loop_cond(const EpiCtx c, int keep_going) {
   if (c.use_cond) cudaGraphSetConditional(c.cond, keep_going ? 1u : 0u);
 }
 
@@ -72,7 +81,7 @@ __device__ __noinline__ void select_precisions(DevState* s, int64_t n) {
 }
 
 // after the setup reduction: ||b||, delta_0 = ||r_0||, edge cases, selector for k = 0
-__device__ __noinline__ void epi_setup(const Ctx& c, double bb, double rr) {
+__device__ __noinline__ void epi_setup(const EpiCtx c, double bb, double rr) {
   DevState* s = c.st;
   s->bnorm = sqrt(bb);
   s->delta = sqrt(rr);
@@ -95,13 +104,13 @@ __device__ __noinline__ void epi_setup(const Ctx& c, double bb, double rr) {
   }
 }
 
-__device__ __forceinline__ void epi_rho(const Ctx& c, double rho) {
+__device__ __forceinline__ void epi_rho(const EpiCtx c, double rho) {
   DevState* s = c.st;
   s->rho = rho;
   s->beta = (s->k > 0) ? rho / s->rho_prev : 0.0;  // Alg 4.1 lines 7-9
 }
 
-__device__ __forceinline__ void epi_gamma(const Ctx& c, double gamma) {
+__device__ __forceinline__ void epi_gamma(const EpiCtx c, double gamma) {
   DevState* s = c.st;
   s->gamma = gamma;
   const double rho = s->rho;
@@ -114,7 +123,7 @@ __device__ __forceinline__ void epi_gamma(const Ctx& c, double gamma) {
   }
 }
 
-__device__ __noinline__ void epi_delta(const Ctx& c, double rr) {
+__device__ __noinline__ void epi_delta(const EpiCtx c, double rr) {
   DevState* s = c.st;
   const double delta = sqrt(rr);  // line 17
   const int k1 = s->k + 1;
@@ -146,40 +155,41 @@ __device__ __noinline__ void epi_delta(const Ctx& c, double rr) {
 // the u_r switch, where r <- RN32(r) is fused here, step a6); UZ: precision of z.
 template <int RS, int UR, int UZ>
 __device__ __forceinline__ double phase_z(const Ctx& c, const double omega, int bid, int nb) {
-  const typename Store<RS>::T* rin = rvec<RS>(c);
+  using TR = typename Store<RS>::T;
+  using TD = typename Store<(UZ == P64) ? P64 : P32>::T;
+  const TR* rin = rvec<RS>(c);
   typename Store<UR>::T* rout = rvec<UR>(c);
   typename Store<UZ>::T* z = zvec<UZ>(c);
+  const TD* dinv;
+  if constexpr (UZ == P64) dinv = c.dinv64; else dinv = c.dinv32;
   const int64_t npair = c.npad >> 1;
-  const int64_t stride = (int64_t)nb * kVecThreads;
+  const int64_t stride = (int64_t)nb * blockDim.x;
+  constexpr int U = (RS == P64 && UZ == P64) ? kVecUnrollWide : kVecUnrollNarrow;
   double sum = 0.0;
-  for (int64_t base = (int64_t)bid * kVecThreads + threadIdx.x; base < npair; base += stride * kVecUnroll) {
-    double r0[kVecUnroll], r1[kVecUnroll], d0[kVecUnroll], d1[kVecUnroll];
+  for (int64_t base = (int64_t)bid * blockDim.x + threadIdx.x; base < npair; base += stride * U) {
+    typename Raw2<TR>::T rr[U];
+    typename Raw2<TD>::T dd[U];
 #pragma unroll
-    for (int u = 0; u < kVecUnroll; ++u) {
+    for (int u = 0; u < U; ++u) {
       const int64_t i = base + u * stride;
-      if (i < npair) {
-        load2(rin, i, r0[u], r1[u]);
-        if (UZ == P64) load2(c.dinv64, i, d0[u], d1[u]);
-        else load2(c.dinv32, i, d0[u], d1[u]);
-      }
+      if (i < npair) { rr[u] = load_raw(rin, i); dd[u] = load_raw(dinv, i); }
     }
 #pragma unroll
-    for (int u = 0; u < kVecUnroll; ++u) {
+    for (int u = 0; u < U; ++u) {
       const int64_t i = base + u * stride;
       if (i < npair) {
-        double a0 = r0[u], a1 = r1[u];
+        double a0, a1, d0, d1;
+        unpack(rr[u], a0, a1);
+        unpack(dd[u], d0, d1);
         if (RS != UR) {  // r <- RN_{u_r}(r) at the switch iteration
           a0 = round_to<UR>(a0); a1 = round_to<UR>(a1);
           store2(rout, i, a0, a1);
         }
-        const double z0 = round_to<UZ>((a0 * omega) * d0[u]);
-        const double z1 = round_to<UZ>((a1 * omega) * d1[u]);
+        const double z0 = round_to<UZ>((a0 * omega) * d0);
+        const double z1 = round_to<UZ>((a1 * omega) * d1);
         store2(z, i, z0, z1);
 #ifdef AMP_COUNT_FP16
-        if (UZ == P16) {
-          const double t0 = (a0 * omega) * d0[u], t1 = (a1 * omega) * d1[u];
-          count_fp16(c.st, t0, z0); count_fp16(c.st, t1, z1);
-        }
+        if (UZ == P16) { count_fp16(c.st, (a0 * omega) * d0, z0); count_fp16(c.st, (a1 * omega) * d1, z1); }
 #endif
         sum = fma(a0, z0, sum);
         sum = fma(a1, z1, sum);
@@ -194,29 +204,34 @@ __device__ __forceinline__ double phase_z(const Ctx& c, const double omega, int 
 // switch, where p_{k-1} <- RN_{u_z}(p_{k-1}) is fused here, reading R9).
 template <int PS, int UZ>
 __device__ __forceinline__ void phase_p(const Ctx& c, const double beta, const bool first, int bid, int nb) {
-  const typename Store<PS>::T* pin = pvec<PS>(c);
-  typename Store<UZ>::T* pout = pvec<UZ>(c);
-  const typename Store<UZ>::T* z = zvec<UZ>(c);
+  using TP = typename Store<PS>::T;
+  using TZ = typename Store<UZ>::T;
+  const TP* pin = pvec<PS>(c);
+  TZ* pout = pvec<UZ>(c);
+  const TZ* z = zvec<UZ>(c);
   const int64_t npair = c.npad >> 1;
-  const int64_t stride = (int64_t)nb * kVecThreads;
-  for (int64_t base = (int64_t)bid * kVecThreads + threadIdx.x; base < npair; base += stride * kVecUnroll) {
-    double p0[kVecUnroll], p1[kVecUnroll], z0[kVecUnroll], z1[kVecUnroll];
+  const int64_t stride = (int64_t)nb * blockDim.x;
+  constexpr int U = kVecUnrollNarrow;
+  for (int64_t base = (int64_t)bid * blockDim.x + threadIdx.x; base < npair; base += stride * U) {
+    typename Raw2<TP>::T pp[U];
+    typename Raw2<TZ>::T zz[U];
 #pragma unroll
-    for (int u = 0; u < kVecUnroll; ++u) {
+    for (int u = 0; u < U; ++u) {
       const int64_t i = base + u * stride;
       if (i < npair) {
-        load2(z, i, z0[u], z1[u]);
-        if (first) { p0[u] = 0.0; p1[u] = 0.0; }
-        else load2(pin, i, p0[u], p1[u]);
+        zz[u] = load_raw(z, i);
+        if (!first) pp[u] = load_raw(pin, i);
       }
     }
 #pragma unroll
-    for (int u = 0; u < kVecUnroll; ++u) {
+    for (int u = 0; u < U; ++u) {
       const int64_t i = base + u * stride;
       if (i < npair) {
-        double a0 = p0[u], a1 = p1[u];
+        double a0 = 0.0, a1 = 0.0, z0, z1;
+        unpack(zz[u], z0, z1);
+        if (!first) unpack(pp[u], a0, a1);
         if (PS != UZ) { a0 = round_to<UZ>(a0); a1 = round_to<UZ>(a1); }
-        const double n0 = fma(beta, a0, z0[u]), n1 = fma(beta, a1, z1[u]);
+        const double n0 = fma(beta, a0, z0), n1 = fma(beta, a1, z1);
         store2(pout, i, n0, n1);
 #ifdef AMP_COUNT_FP16
         if (UZ == P16) { count_fp16(c.st, n0, round_to<P16>(n0)); count_fp16(c.st, n1, round_to<P16>(n1)); }
@@ -229,36 +244,44 @@ __device__ __forceinline__ void phase_p(const Ctx& c, const double beta, const b
 // ------------------------------------------------------------------ a5: x, r, delta ---------
 template <int UR, int UZ>
 __device__ __forceinline__ double phase_xr(const Ctx& c, const double alpha, double* x, int bid, int nb) {
-  const typename Store<UZ>::T* p = pvec<UZ>(c);
-  const typename Store<UR>::T* q = qvec<UR>(c);
-  typename Store<UR>::T* r = rvec<UR>(c);
+  using TZ = typename Store<UZ>::T;
+  using TR = typename Store<UR>::T;
+  const TZ* p = pvec<UZ>(c);
+  const TR* q = qvec<UR>(c);
+  TR* r = rvec<UR>(c);
   const int64_t n = c.n;
   const int64_t npair = c.npad >> 1;
-  const int64_t stride = (int64_t)nb * kVecThreads;
+  const int64_t stride = (int64_t)nb * blockDim.x;
+  constexpr int U = kVecUnrollNarrow;
   double sum = 0.0;
-  for (int64_t base = (int64_t)bid * kVecThreads + threadIdx.x; base < npair; base += stride * kVecUnroll) {
-    double x0[kVecUnroll], x1[kVecUnroll], p0[kVecUnroll], p1[kVecUnroll], q0[kVecUnroll], q1[kVecUnroll],
-        r0[kVecUnroll], r1[kVecUnroll];
+  for (int64_t base = (int64_t)bid * blockDim.x + threadIdx.x; base < npair; base += stride * U) {
+    double2 xx[U];
+    typename Raw2<TZ>::T pp[U];
+    typename Raw2<TR>::T qq[U], rr[U];
 #pragma unroll
-    for (int u = 0; u < kVecUnroll; ++u) {
+    for (int u = 0; u < U; ++u) {
       const int64_t i = base + u * stride;
       if (i < npair) {
-        if (2 * i + 1 < n) load2(x, i, x0[u], x1[u]);
-        else { x0[u] = (2 * i < n) ? x[2 * i] : 0.0; x1[u] = 0.0; }
-        load2(p, i, p0[u], p1[u]);
-        load2(q, i, q0[u], q1[u]);
-        load2(r, i, r0[u], r1[u]);
+        if (2 * i + 1 < n) xx[u] = load_raw(x, i);
+        else xx[u] = make_double2((2 * i < n) ? x[2 * i] : 0.0, 0.0);  // x is caller-owned: exactly n long
+        pp[u] = load_raw(p, i);
+        qq[u] = load_raw(q, i);
+        rr[u] = load_raw(r, i);
       }
     }
 #pragma unroll
-    for (int u = 0; u < kVecUnroll; ++u) {
+    for (int u = 0; u < U; ++u) {
       const int64_t i = base + u * stride;
       if (i < npair) {
-        const double nx0 = fma(alpha, p0[u], x0[u]), nx1 = fma(alpha, p1[u], x1[u]);  // line 15, FP64
+        double p0, p1, q0, q1, r0, r1;
+        unpack(pp[u], p0, p1);
+        unpack(qq[u], q0, q1);
+        unpack(rr[u], r0, r1);
+        const double nx0 = fma(alpha, p0, xx[u].x), nx1 = fma(alpha, p1, xx[u].y);  // line 15, FP64
         if (2 * i + 1 < n) store2(x, i, nx0, nx1);
         else if (2 * i < n) x[2 * i] = nx0;
-        const double nr0 = round_to<UR>(fma(-alpha, q0[u], r0[u]));  // line 16, one rounding to u_r
-        const double nr1 = round_to<UR>(fma(-alpha, q1[u], r1[u]));
+        const double nr0 = round_to<UR>(fma(-alpha, q0, r0));  // line 16, one rounding to u_r
+        const double nr1 = round_to<UR>(fma(-alpha, q1, r1));
         store2(r, i, nr0, nr1);
         sum = fma(nr0, nr0, sum);
         sum = fma(nr1, nr1, sum);
