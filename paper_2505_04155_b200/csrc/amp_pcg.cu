@@ -7,6 +7,7 @@
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <string>
 #include <vector>
@@ -58,6 +59,7 @@ struct amp_pcg {
   int64_t launches = 0;
   int32_t last_iters = -1;
   double m_avg = 0.0;
+  int64_t sell_entries = 0;   // stored entries of the SELL-32 repack (padding included)
 };
 
 template <class T> static T* dev_alloc(amp_pcg* h, size_t count, bool zero) {
@@ -190,17 +192,93 @@ extern "C" amp_pcg_t* amp_pcg_create(int64_t n, int64_t nnz, const int32_t* rowp
     return nullptr;
   }
 
-  // launch geometry: whole multiples of the SM count.  The SpMV and the persistent kernel share one
-  // grid (kBlocksPerSM resident blocks per SM) because the row partition below is per block.
-  CU_TRY(cudaFuncSetAttribute(k_spmv, cudaFuncAttributeMaxDynamicSharedMemorySize, kSpmvSmemBytes), { amp_pcg_destroy(h); return nullptr; });
-  int occ_spmv = 0;
-  CU_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_spmv, k_spmv, kSpmvThreads, kSpmvSmemBytes), { amp_pcg_destroy(h); return nullptr; });
+  // ---- SELL-32 repack of A (spmv.cuh): slice widths, optional windowed row sort, long rows ----
+  {
+    const int64_t nsl = (n + 31) / 32;
+    const int long_min = (int)std::max<int64_t>(256, 8 * (int64_t)std::ceil(h->m_avg));
+    std::vector<int32_t> long_rows;
+    auto row_len = [&](int64_t r) -> int {  // length inside the slices
+      if (r < 0 || r >= n) return 0;
+      const int len = rp[(size_t)r + 1] - rp[(size_t)r];
+      return len > long_min ? 0 : len;
+    };
+    int64_t nnz_sell = 0;
+    for (int64_t r = 0; r < n; ++r) {
+      const int len = rp[(size_t)r + 1] - rp[(size_t)r];
+      if (len > long_min) long_rows.push_back((int32_t)r); else nnz_sell += len;
+    }
+    std::vector<int32_t> wptr((size_t)nsl + 1, 0), perm;
+    auto build_widths = [&]() -> int64_t {
+      int64_t tot = 0;
+      for (int64_t sl = 0; sl < nsl; ++sl) {
+        int w = 0;
+        for (int l = 0; l < 32; ++l) {
+          const int64_t slot = sl * 32 + l;
+          const int64_t r = perm.empty() ? slot : (int64_t)perm[(size_t)slot];
+          w = std::max(w, row_len(r));
+        }
+        wptr[(size_t)sl] = (int32_t)tot;
+        tot += w;
+      }
+      wptr[(size_t)nsl] = (int32_t)tot;
+      return tot;
+    };
+    int64_t wsum = build_widths();
+    if ((double)wsum * 32.0 > 1.03 * (double)nnz_sell + 4096.0) {
+      // row lengths vary: sort rows by length (descending, stable) inside windows of kSortWindow rows
+      const int64_t kSortWindow = 4096;
+      perm.assign((size_t)nsl * 32, -1);
+      for (int64_t r = 0; r < n; ++r) perm[(size_t)r] = (int32_t)r;
+      for (int64_t w0 = 0; w0 < n; w0 += kSortWindow) {
+        const int64_t w1 = std::min(n, w0 + kSortWindow);
+        std::stable_sort(perm.begin() + w0, perm.begin() + w1,
+                         [&](int32_t x, int32_t y) { return row_len(x) > row_len(y); });
+      }
+      wsum = build_widths();
+    }
+    if (wsum * 32 + 256 > (int64_t)0x7fffffff) {
+      set_error("amp_pcg_create: padded SELL-32 storage exceeds 2^31 entries");
+      amp_pcg_destroy(h);
+      return nullptr;
+    }
+    const size_t total = (size_t)wsum * 32 + 256;
+    int32_t *wptr_d, *cols_d, *perm_d = nullptr, *long_d;
+    double* v64_d; float* v32_d;
+    ALLOC(wptr_d, int32_t, wptr.size());
+    ALLOC(cols_d, int32_t, total);
+    ALLOC(v64_d, double, total);
+    ALLOC(v32_d, float, total);
+    ALLOC(long_d, int32_t, long_rows.size() + 1);
+    if (!perm.empty()) ALLOC(perm_d, int32_t, perm.size());
+    CU_TRY(cudaMemcpyAsync(wptr_d, wptr.data(), sizeof(int32_t) * wptr.size(), cudaMemcpyHostToDevice, h->stream),
+           { amp_pcg_destroy(h); return nullptr; });
+    if (!long_rows.empty())
+      CU_TRY(cudaMemcpyAsync(long_d, long_rows.data(), sizeof(int32_t) * long_rows.size(), cudaMemcpyHostToDevice, h->stream),
+             { amp_pcg_destroy(h); return nullptr; });
+    if (perm_d)
+      CU_TRY(cudaMemcpyAsync(perm_d, perm.data(), sizeof(int32_t) * perm.size(), cudaMemcpyHostToDevice, h->stream),
+             { amp_pcg_destroy(h); return nullptr; });
+    const int pgrid = (int)((nsl * 32 + 255) / 256);
+    k_sell_pack<<<pgrid, 256, 0, h->stream>>>((int)n, (int)nsl, long_min, rowptr, colidx, vals, wptr_d, perm_d, cols_d, v64_d,
+                                             v32_d);
+    CU_TRY(cudaStreamSynchronize(h->stream), { amp_pcg_destroy(h); return nullptr; });
+    CU_TRY(cudaGetLastError(), { amp_pcg_destroy(h); return nullptr; });
+    c.sell_wptr = wptr_d; c.sell_cols = cols_d; c.sell_vals64 = v64_d; c.sell_vals32 = v32_d; c.sell_perm = perm_d;
+    c.long_rows = long_d; c.nslices = (int32_t)nsl; c.nlong = (int32_t)long_rows.size();
+    h->sell_entries = wsum * 32;
+
+    // SpMV grid: a warp takes a group of up to kSpmvGroupMax slices per pass; blocks make a whole number of
+    // (nearly) equal passes, at most `mult` blocks per SM (AMP_SPMV_GRID_MULT: tuning aid, default 16)
+    int mult = 16;
+    if (const char* e = getenv("AMP_SPMV_GRID_MULT")) mult = std::max(1, atoi(e));
+    const int64_t max_grid = std::min<int64_t>((int64_t)h->num_sms * mult, kMaxGrid);
+    const int64_t nblk = (nsl + kSpmvWarps * kSpmvGroupMax - 1) / (kSpmvWarps * kSpmvGroupMax);
+    const int64_t passes = std::max<int64_t>(1, (nblk + max_grid - 1) / max_grid);
+    h->spmv_grid = (int)std::max<int64_t>(1, (nblk + passes - 1) / passes);
+  }
+
+  // persistent kernel and vector kernels: whole multiples of the SM count
   persistent_configure(h->num_sms, &h->persist_grid, &h->persist_ok);
-  if (occ_spmv < 1) { set_error("amp_pcg_create: SpMV kernel does not fit on this device"); amp_pcg_destroy(h); return nullptr; }
-  int per_sm = std::min(occ_spmv, (int)kBlocksPerSM);
-  if (h->persist_ok) per_sm = std::min(per_sm, h->persist_grid / h->num_sms);
-  h->spmv_grid = std::min(h->num_sms * std::max(per_sm, 1), (int)kMaxGrid);
-  if (h->persist_ok) h->persist_grid = h->spmv_grid;
   // vector kernels: a whole number of equally long grid-stride trips per block, at most one full wave
   auto vec_grid_for = [&](const void* kern) -> int {
     int occ = 1;
@@ -215,58 +293,6 @@ extern "C" amp_pcg_t* amp_pcg_create(int64_t n, int64_t nnz, const int32_t* rowp
   h->grid_p = vec_grid_for((const void*)k_p);
   h->grid_xr = vec_grid_for((const void*)k_xr);
   h->vec_grid = vec_grid_for((const void*)k_setup);
-
-  // SpMV row partition: every warp of the grid owns a contiguous row range of (nearly) equal
-  // cost = entries + rows, cut into tiles of <= kTileRows rows and <= tile_cap entries; a longer
-  // row stands alone.  Small matrices get smaller tiles so that the work spreads over the SMs.
-  // lanes per row (compile-time variants 1, 4, 32)
-  c.lanes_per_row = (h->m_avg <= 12.0) ? 1 : (h->m_avg <= 64.0 ? 4 : 32);
-  const int rpp = 32 / c.lanes_per_row;  // rows per warp pass
-  const int nwarps = h->spmv_grid * kSpmvWarps;
-  int tile_cap = (int)std::min<int64_t>(kTileNnz, std::max<int64_t>(128, ((nnz + nwarps - 1) / nwarps + 31) / 32 * 32));
-  std::vector<int2> tiles;
-  std::vector<int32_t> warp_tile((size_t)nwarps + 1);
-  {
-    const double total = (double)nnz + (double)n;
-    int64_t r = 0;
-    for (int w = 0; w < nwarps; ++w) {
-      warp_tile[(size_t)w] = (int32_t)tiles.size();
-      const double target = total * (double)(w + 1) / (double)nwarps;
-      // last row of this warp: first r_end with cost(r_end) >= target  (cost(r) = rowptr[r] + r)
-      int64_t lo = r, hi = n;
-      while (lo < hi) {
-        const int64_t mid = (lo + hi) / 2;
-        if ((double)rp[(size_t)mid] + (double)mid >= target) hi = mid; else lo = mid + 1;
-      }
-      const int64_t r_end = (w == nwarps - 1) ? n : lo;
-      while (r < r_end) {
-        int64_t r1 = r + 1;
-        if (rp[(size_t)r1] - rp[(size_t)r] <= tile_cap) {
-          while (r1 < r_end && r1 - r < kTileRows && rp[(size_t)r1 + 1] - rp[(size_t)r] <= tile_cap) ++r1;
-          if (r1 < r_end && r1 - r > rpp) r1 = r + (r1 - r) / rpp * rpp;  // whole warp passes
-        }
-        tiles.push_back(make_int2((int)r, rp[(size_t)r]));
-        r = r1;
-      }
-    }
-    warp_tile[(size_t)nwarps] = (int32_t)tiles.size();
-    tiles.push_back(make_int2((int)n, (int)nnz));
-  }
-  c.ntiles = (int32_t)tiles.size() - 1;
-  int2* tile_desc; int32_t* warp_tile_d; int32_t* rowptr_pad;
-  ALLOC(tile_desc, int2, tiles.size());
-  ALLOC(warp_tile_d, int32_t, warp_tile.size());
-  const size_t rp_len = (((size_t)n + 1 + 3) & ~(size_t)3) + 8;
-  ALLOC(rowptr_pad, int32_t, rp_len);
-  rp.resize(rp_len, (int32_t)nnz);
-  CU_TRY(cudaMemcpyAsync(tile_desc, tiles.data(), sizeof(int2) * tiles.size(), cudaMemcpyHostToDevice, h->stream),
-         { amp_pcg_destroy(h); return nullptr; });
-  CU_TRY(cudaMemcpyAsync(warp_tile_d, warp_tile.data(), sizeof(int32_t) * warp_tile.size(), cudaMemcpyHostToDevice, h->stream),
-         { amp_pcg_destroy(h); return nullptr; });
-  CU_TRY(cudaMemcpyAsync(rowptr_pad, rp.data(), sizeof(int32_t) * rp_len, cudaMemcpyHostToDevice, h->stream),
-         { amp_pcg_destroy(h); return nullptr; });
-  CU_TRY(cudaStreamSynchronize(h->stream), { amp_pcg_destroy(h); return nullptr; });
-  c.tile_desc = tile_desc; c.warp_tile = warp_tile_d; c.rowptr_pad = rowptr_pad;
 #undef ALLOC
   return h;
 }
@@ -282,12 +308,7 @@ extern "C" int64_t amp_pcg_last_launch_count(const amp_pcg_t* h) { return h ? h-
 // ------------------------------------------------------------------ SpMV entry --------------
 template <int UR, class PT>
 static void launch_spmv_any(amp_pcg* h, const void* p, void* q) {
-  static bool attr_done = false;
-  if (!attr_done) {
-    cudaFuncSetAttribute(k_spmv_any<UR, PT>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSpmvSmemBytes);
-    attr_done = true;
-  }
-  k_spmv_any<UR, PT><<<h->spmv_grid, kSpmvThreads, kSpmvSmemBytes, h->stream>>>(
+  k_spmv_any<UR, PT><<<h->spmv_grid, kSpmvThreads, 0, h->stream>>>(
       h->ctx, static_cast<const PT*>(p), static_cast<typename Store<UR>::T*>(q));
 }
 
@@ -324,7 +345,7 @@ extern "C" int amp_spmv(amp_pcg_t* h, int mat_prec, int vec_prec, const void* p,
 static void launch_iteration(amp_pcg* h, const Ctx& c, cudaStream_t s) {
   k_z<<<h->grid_z, kVecThreads, 0, s>>>(c);
   k_p<<<h->grid_p, kVecThreads, 0, s>>>(c);
-  k_spmv<<<h->spmv_grid, kSpmvThreads, kSpmvSmemBytes, s>>>(c);
+  k_spmv<<<h->spmv_grid, kSpmvThreads, 0, s>>>(c);
   k_xr<<<h->grid_xr, kVecThreads, 0, s>>>(c);
 }
 

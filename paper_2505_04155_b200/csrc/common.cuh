@@ -14,28 +14,14 @@ constexpr int P64 = 0, P32 = 1, P16 = 2;       // precision codes (= AMP_FP64/32
 constexpr int kVecThreads = 256;               // block size of the vector kernels
 constexpr int kVecUnrollNarrow = 4;            // independent 2-element chunks in flight per thread (some operand < FP64)
 constexpr int kVecUnrollWide = 2;              // ... when every operand is FP64 (same bytes in flight, half the registers)
-#ifndef AMP_SPMV_WARPS
-#define AMP_SPMV_WARPS 32
+constexpr int kSpmvThreads = 256;              // block size of the SpMV kernel: 8 warps, one SELL slice per warp and pass
+constexpr int kSpmvWarps = kSpmvThreads / 32;
+#ifndef AMP_SPMV_MINBLOCKS
+#define AMP_SPMV_MINBLOCKS 4
 #endif
-#ifndef AMP_TILE_NNZ
-#define AMP_TILE_NNZ 256
-#endif
-#ifndef AMP_TILE_ROWS
-#define AMP_TILE_ROWS 64
-#endif
-#ifndef AMP_STAGES
-#define AMP_STAGES 2
-#endif
-#ifndef AMP_BLOCKS_PER_SM
-#define AMP_BLOCKS_PER_SM 1
-#endif
-constexpr int kSpmvWarps = AMP_SPMV_WARPS;     // warps per SpMV block, each with a private stage ring
-constexpr int kSpmvThreads = 32 * kSpmvWarps;  // block size of the SpMV / persistent kernels
-constexpr int kBlocksPerSM = AMP_BLOCKS_PER_SM;  // resident blocks per SM of the SpMV / persistent kernels
-constexpr int kTileNnz = AMP_TILE_NNZ;         // stored entries staged per SpMV tile (one warp stage)
-constexpr int kTileRows = AMP_TILE_ROWS;       // max rows per SpMV tile
-constexpr int kStages = AMP_STAGES;            // stages of each warp's ring
-constexpr int kMaxGrid = 4096;                 // capacity of each partial-sum array
+constexpr int kSpmvMinBlocks = AMP_SPMV_MINBLOCKS;  // resident SpMV blocks per SM the register budget is set for
+constexpr int kPersistThreads = 512;           // block size of the persistent (whole-loop) kernel
+constexpr int kMaxGrid = 8192;                 // capacity of each partial-sum array
 constexpr int kMaxWindow = 64;                 // max d / ell of the indicators
 
 // Scalars of one solve, resident in device memory.  The host writes the policy part before the
@@ -76,11 +62,15 @@ struct Ctx {
   double* z64; float* z32; __half* z16;
   double* p64; float* p32; __half* p16;
   double* partials;       // [4][kMaxGrid] per-block partial sums
-  const int32_t* rowptr_pad;  // owned copy of rowptr padded to a multiple of 4 (+4) entries with nnz
-  const int2* tile_desc;      // [ntiles+1] (first row, first entry) of each SpMV tile
-  const int32_t* warp_tile;   // [spmv grid * kSpmvWarps + 1] first tile of each warp (contiguous, cost-balanced ranges)
-  int32_t ntiles;
-  int32_t lanes_per_row;  // lanes cooperating on one row in the SpMV row reduction (power of 2)
+  // SELL-32 repack of A (spmv.cuh), owned by the handle
+  const int32_t* sell_wptr;   // [nslices+1] cumulative slice widths; slice s starts at element 32*sell_wptr[s]
+  const int32_t* sell_cols;   // column indices
+  const double* sell_vals64;  // FP64 values
+  const float* sell_vals32;   // FP32-rounded values (u_r = FP32 phase)
+  const int32_t* sell_perm;   // [32*nslices] row of each slot (-1 = padding), or nullptr = identity
+  const int32_t* long_rows;   // [nlong] rows kept out of the slices (longer than the cap), summed from CSR
+  int32_t nslices;
+  int32_t nlong;
   cudaGraphConditionalHandle cond;  // WHILE-node handle (graph loop only)
   int32_t use_cond;
 };

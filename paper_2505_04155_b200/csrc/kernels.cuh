@@ -38,23 +38,16 @@ __device__ __forceinline__ void dispatch_p(const Ctx& c, int ps, int uz, double 
   }
 }
 
-// lanes per row of the SpMV row-sum phase: 1 (short rows), 4 or 32 (Ctx::lanes_per_row, set in create)
-template <bool COH, int L>
-__device__ __forceinline__ double dispatch_spmv_l(const Ctx& c, int ur, int uz, int bid, int nb, unsigned char* smem) {
+template <bool COH, int NT>
+__device__ __forceinline__ double dispatch_spmv(const Ctx& c, int ur, int uz, int bid, int nb, double* red) {
   if (ur == P64) {
-    if (uz == P64) return phase_spmv<P64, COH, L>(c, c.p64, c.q64, bid, nb, smem);
-    if (uz == P32) return phase_spmv<P64, COH, L>(c, c.p32, c.q64, bid, nb, smem);
-    return phase_spmv<P64, COH, L>(c, c.p16, c.q64, bid, nb, smem);
+    if (uz == P64) return phase_spmv<P64, COH, NT>(c, c.p64, c.q64, bid, nb, red);
+    if (uz == P32) return phase_spmv<P64, COH, NT>(c, c.p32, c.q64, bid, nb, red);
+    return phase_spmv<P64, COH, NT>(c, c.p16, c.q64, bid, nb, red);
   }
-  if (uz == P64) return phase_spmv<P32, COH, L>(c, c.p64, c.q32, bid, nb, smem);
-  if (uz == P32) return phase_spmv<P32, COH, L>(c, c.p32, c.q32, bid, nb, smem);
-  return phase_spmv<P32, COH, L>(c, c.p16, c.q32, bid, nb, smem);
-}
-template <bool COH>
-__device__ __forceinline__ double dispatch_spmv(const Ctx& c, int ur, int uz, int bid, int nb, unsigned char* smem) {
-  if (c.lanes_per_row == 1) return dispatch_spmv_l<COH, 1>(c, ur, uz, bid, nb, smem);
-  if (c.lanes_per_row == 4) return dispatch_spmv_l<COH, 4>(c, ur, uz, bid, nb, smem);
-  return dispatch_spmv_l<COH, 32>(c, ur, uz, bid, nb, smem);
+  if (uz == P64) return phase_spmv<P32, COH, NT>(c, c.p64, c.q32, bid, nb, red);
+  if (uz == P32) return phase_spmv<P32, COH, NT>(c, c.p32, c.q32, bid, nb, red);
+  return phase_spmv<P32, COH, NT>(c, c.p16, c.q32, bid, nb, red);
 }
 
 __device__ __forceinline__ double dispatch_xr(const Ctx& c, int ur, int uz, double alpha, double* x, int bid, int nb) {
@@ -85,13 +78,12 @@ __global__ void __launch_bounds__(kVecThreads, 4) k_p(const Ctx c) {
   dispatch_p(c, s->p_store, s->uz, s->beta, s->k == 0, blockIdx.x, gridDim.x);
 }
 
-__global__ void __launch_bounds__(kSpmvThreads, kBlocksPerSM) k_spmv(const Ctx c) {
-  extern __shared__ __align__(16) unsigned char smem[];
+__global__ void __launch_bounds__(kSpmvThreads, kSpmvMinBlocks) k_spmv(const Ctx c) {
   __shared__ double red[32];
   DevState* s = c.st;
   if (s->done) return;
   const int bid = blockIdx.x, nb = gridDim.x;
-  const double v = dispatch_spmv<false>(c, s->ur, s->uz, bid, nb, smem);
+  const double v = dispatch_spmv<false, kSpmvThreads>(c, s->ur, s->uz, bid, nb, red);
   grid_reduce<kSpmvThreads>(v, c.partials + 1 * kMaxGrid, &s->counter[1], bid, nb, red,
                             [&](double tot) { epi_gamma(epi_ctx(c), tot); });
 }
@@ -111,11 +103,9 @@ __global__ void __launch_bounds__(kVecThreads, 2) k_xr(const Ctx c) {
 
 // ------------------------------------------------------------------ stand-alone SpMV --------
 template <int UR, class PT>
-__global__ void __launch_bounds__(kSpmvThreads, kBlocksPerSM) k_spmv_any(const Ctx c, const PT* p, typename Store<UR>::T* q) {
-  extern __shared__ __align__(16) unsigned char smem[];
-  if (c.lanes_per_row == 1) (void)phase_spmv<UR, false, 1>(c, p, q, blockIdx.x, gridDim.x, smem);
-  else if (c.lanes_per_row == 4) (void)phase_spmv<UR, false, 4>(c, p, q, blockIdx.x, gridDim.x, smem);
-  else (void)phase_spmv<UR, false, 32>(c, p, q, blockIdx.x, gridDim.x, smem);
+__global__ void __launch_bounds__(kSpmvThreads, kSpmvMinBlocks) k_spmv_any(const Ctx c, const PT* p, typename Store<UR>::T* q) {
+  __shared__ double red[32];
+  (void)phase_spmv<UR, false, kSpmvThreads>(c, p, q, blockIdx.x, gridDim.x, red);
 }
 
 // ------------------------------------------------------------------ set-up / finalise -------

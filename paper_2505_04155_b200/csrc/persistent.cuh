@@ -8,7 +8,6 @@
 
 namespace amp {
 
-constexpr int kPersistThreads = kSpmvThreads;  // the vector phases take their block size from blockDim
 
 __device__ __forceinline__ unsigned int ld_acquire_u32(const unsigned int* p) {
   unsigned int v;
@@ -69,15 +68,14 @@ __device__ __noinline__ double pz(const Ctx& c, int rs, int ur, int uz, double o
 __device__ __noinline__ void pp(const Ctx& c, int ps, int uz, double beta, bool first, int bid, int nb) {
   dispatch_p(c, ps, uz, beta, first, bid, nb);
 }
-__device__ __noinline__ double ps_(const Ctx& c, int ur, int uz, int bid, int nb, unsigned char* smem) {
-  return dispatch_spmv<true>(c, ur, uz, bid, nb, smem);
+__device__ __noinline__ double ps_(const Ctx& c, int ur, int uz, int bid, int nb, double* red) {
+  return dispatch_spmv<true, kPersistThreads>(c, ur, uz, bid, nb, red);
 }
 __device__ __noinline__ double pxr(const Ctx& c, int ur, int uz, double alpha, double* x, int bid, int nb) {
   return dispatch_xr(c, ur, uz, alpha, x, bid, nb);
 }
 
-__global__ void __launch_bounds__(kPersistThreads, kBlocksPerSM) k_persistent(const Ctx c) {
-  extern __shared__ __align__(16) unsigned char smem[];
+__global__ void __launch_bounds__(kPersistThreads, 1) k_persistent(const Ctx c) {
   __shared__ double red[32];
   DevState* s = c.st;
   const int bid = blockIdx.x, nb = gridDim.x;
@@ -92,7 +90,7 @@ __global__ void __launch_bounds__(kPersistThreads, kBlocksPerSM) k_persistent(co
     grid_sync_reduce<true>(v, c.partials + 0 * kMaxGrid, s, bid, nb, red, [&](double t) { epi_rho(epi_ctx(c), t); });
     pp(c, ps, uz, ldv(&s->beta), first, bid, nb);                                                   // a3
     grid_sync_reduce<false>(0.0, nullptr, s, bid, nb, red, nop);
-    v = ps_(c, ur, uz, bid, nb, smem);                                                        // a4
+    v = ps_(c, ur, uz, bid, nb, red);                                                        // a4
     grid_sync_reduce<true>(v, c.partials + 1 * kMaxGrid, s, bid, nb, red, [&](double t) { epi_gamma(epi_ctx(c), t); });
     if (ldv(&s->done)) break;  // breakdown
     v = pxr(c, ur, uz, ldv(&s->alpha), x, bid, nb);                                                 // a5
@@ -103,16 +101,10 @@ __global__ void __launch_bounds__(kPersistThreads, kBlocksPerSM) k_persistent(co
 inline void persistent_configure(int num_sms, int* grid, int* ok) {
   *grid = 0;
   *ok = 0;
-  if (cudaFuncSetAttribute(k_persistent, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                           kSpmvSmemBytes) != cudaSuccess) {
-    cudaGetLastError();
-    return;
-  }
   int occ = 0, coop = 0, dev = 0;
   cudaGetDevice(&dev);
   cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
-  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_persistent, kPersistThreads,
-                                                    kSpmvSmemBytes) != cudaSuccess) {
+  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_persistent, kPersistThreads, 0) != cudaSuccess) {
     cudaGetLastError();
     return;
   }
@@ -128,8 +120,7 @@ inline int persistent_launch(const Ctx& c, int grid, cudaStream_t st) {
   Ctx cc = c;
   cc.use_cond = 0;
   void* args[] = {(void*)&cc};
-  return (int)cudaLaunchCooperativeKernel((void*)k_persistent, dim3(grid), dim3(kPersistThreads), args,
-                                          kSpmvSmemBytes, st);
+  return (int)cudaLaunchCooperativeKernel((void*)k_persistent, dim3(grid), dim3(kPersistThreads), args, 0, st);
 }
 
 }  // namespace amp

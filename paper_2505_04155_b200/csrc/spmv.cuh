@@ -1,21 +1,25 @@
 // spmv.cuh — step a4 of the loop: q = A p in u_r and gamma = q^T p (Alg 4.1 lines 11-13,
 // PAPER.md:288-291; the paper also fuses the inner product into its Ax kernel, :537).
 //
-// CSR, "warp-private bulk pipeline, lanes-per-row" design for sm_100a:
-//  * Rows are statically partitioned over all warps of the grid in contiguous ranges of equal
-//    cost (stored entries + rows); each range is cut into tiles of <= tile_cap entries and
-//    <= kTileRows rows, a whole number of warp passes each (warp_tile / tile_desc, built in
-//    amp_pcg_create).
-//  * Every warp runs its own ring of kStages shared-memory stages, each guarded by its own
-//    mbarrier.  Per tile, lane 0 issues three cp.async.bulk (TMA, 1-D) copies — values, column
-//    indices, row pointers — so the HBM stream is fully coalesced whatever the row lengths are,
-//    costs no registers, and runs ahead of the arithmetic.  Warps never meet at a block barrier.
-//  * L = lanes_per_row lanes own a row: they read their entries from shared memory, gather p_j
-//    (adjacent lanes hold adjacent rows, so for banded matrices one gather instruction touches
-//    few sectors), accumulate an fma chain in the working precision in registers (L = 1: in CSR
-//    order), combine over the L lanes by shuffles, write q_i and add p_i q_i (stored q_i, FP64)
-//    to the lane's gamma partial.
-//  * A row longer than the tile capacity is a tile of its own, streamed straight from global.
+// Matrix format: SELL-32 ("sliced ELLPACK", slice height = warp width), repacked once from the
+// caller's CSR in amp_pcg_create and owned by the handle (column indices, FP64 values and the
+// FP32-rounded value copy of the u_r = FP32 phase).
+//  * A slice is 32 consecutive rows (of the row order `perm`, identity unless the row lengths
+//    vary enough for a windowed sort to pay); lane l of a warp owns row l of the slice.
+//  * The slice width w = longest row of the slice; shorter rows are padded with (value 0,
+//    column = own row).  w is cut as 4a + 2b + c and stored as a blocks of [lane][4] entries,
+//    then b block of [lane][2], then c block of [lane][1], so a lane reads its row with 128-bit
+//    loads (64-/32-bit for the remainder) and every warp-wide load is one contiguous, fully used
+//    512-byte (256-, 128-byte) run: no padding beyond the slice maximum, 0.125 B/row of index
+//    overhead (the cumulative widths) instead of CSR's 4 B/row row pointer.
+//    FP64 values use [lane][2] blocks throughout (a quad = two consecutive pair blocks).
+//  * Entries keep their CSR order within the row and each lane accumulates ONE fma chain in the
+//    working precision, so q_i is bit-identical to a sequential CSR-order fma loop.
+//  * Matrix data is streamed with ld.global.cs (evict-first) so that it does not displace the
+//    vectors from L2; p is gathered through the read-only path (L1-cached) — adjacent lanes hold
+//    adjacent rows, so for banded matrices one gather instruction touches one or two lines.
+//  * Rows longer than the cap `long_row_min` are left out of the slices (length 0 there) and
+//    summed straight from the borrowed CSR arrays by a whole block each.
 // UR = P64: FP64 values, FP64 products and sums.  UR = P32: FP32 value copy, p_j converted to
 // FP32 (exact from FP16/FP32 storage), FP32 products and sums (q computed and
 // stored in u_r).
@@ -24,51 +28,54 @@
 
 namespace amp {
 
-constexpr int kStageValsBytes = (kTileNnz + 8) * 8;
-constexpr int kStageColsBytes = (kTileNnz + 8) * 4;
-constexpr int kStageRpBytes = (kTileRows + 8) * 4;
-constexpr int kStageBytes = ((kStageValsBytes + kStageColsBytes + kStageRpBytes + 127) / 128) * 128;
-constexpr int kSpmvRingBytes = kSpmvWarps * kStages * kStageBytes;
-constexpr int kSpmvSmemBytes = kSpmvRingBytes + kSpmvWarps * kStages * 8;  // + mbarriers
-#ifndef AMP_GATHER_BATCH
-#define AMP_GATHER_BATCH 8
-#endif
-constexpr int kGatherBatch = AMP_GATHER_BATCH;  // independent gathers in flight per lane
-static_assert(kSpmvSmemBytes <= 227 * 1024, "SpMV ring does not fit in shared memory");
-
 template <int UR> struct SpmvT;
 template <> struct SpmvT<P64> { using A = double; };
 template <> struct SpmvT<P32> { using A = float; };
 
-// ------------------------------------------------------------------ mbarrier / bulk copy ----
-__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
-  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+// ------------------------------------------------------------------ SELL-32 addressing ------
+// position (in elements, relative to the slice start) of entry k of lane `lane` in a slice of
+// width w.  pos32: column indices and FP32 values; pos64: FP64 values.
+__host__ __device__ __forceinline__ int64_t sell_pos32(int k, int lane, int w) {
+  const int a = w >> 2;
+  if (k < 4 * a) return (int64_t)(k >> 2) * 128 + lane * 4 + (k & 3);
+  if ((w & 2) && k < 4 * a + 2) return (int64_t)a * 128 + lane * 2 + (k - 4 * a);
+  return (int64_t)a * 128 + ((w & 2) ? 64 : 0) + lane;
 }
-__device__ __forceinline__ void mbar_inval(uint64_t* bar) {
-  asm volatile("mbarrier.inval.shared::cta.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
+__host__ __device__ __forceinline__ int64_t sell_pos64(int k, int lane, int w) {
+  const int a = w >> 2;
+  if (k < 4 * a) return (int64_t)(k >> 2) * 128 + ((k >> 1) & 1) * 64 + lane * 2 + (k & 1);
+  if ((w & 2) && k < 4 * a + 2) return (int64_t)a * 128 + lane * 2 + (k - 4 * a);
+  return (int64_t)a * 128 + ((w & 2) ? 64 : 0) + lane;
 }
-__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, uint32_t bytes) {
-  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
-  uint32_t ok;
-  do {
-    asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}"
-                 : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity) : "memory");
-  } while (!ok);
-}
-// 1-D bulk copy global -> shared (16-byte aligned addresses, size a multiple of 16), completion on bar
-__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
-  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-               ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
-}
-// order this thread's generic-proxy accesses to shared memory before later async-proxy (bulk copy) writes
-__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
-template <int UR> __device__ __forceinline__ const typename SpmvT<UR>::A* mat_vals(const Ctx& c);
-template <> __device__ __forceinline__ const double* mat_vals<P64>(const Ctx& c) { return c.vals64; }
-template <> __device__ __forceinline__ const float* mat_vals<P32>(const Ctx& c) { return c.vals32; }
+// streaming (evict-first) loads of matrix data
+__device__ __forceinline__ int4 lds_i4(const int32_t* p) { return __ldcs(reinterpret_cast<const int4*>(p)); }
+__device__ __forceinline__ int2 lds_i2(const int32_t* p) { return __ldcs(reinterpret_cast<const int2*>(p)); }
+__device__ __forceinline__ int lds_i1(const int32_t* p) { return __ldcs(p); }
+__device__ __forceinline__ void lds_quad(const float* v, float (&a)[4]) {
+  const float4 t = __ldcs(reinterpret_cast<const float4*>(v));
+  a[0] = t.x; a[1] = t.y; a[2] = t.z; a[3] = t.w;
+}
+__device__ __forceinline__ void lds_quad(const double* v, double (&a)[4]) {  // v -> first pair block, lane offset applied
+  const double2 t0 = __ldcs(reinterpret_cast<const double2*>(v));
+  const double2 t1 = __ldcs(reinterpret_cast<const double2*>(v + 64));
+  a[0] = t0.x; a[1] = t0.y; a[2] = t1.x; a[3] = t1.y;
+}
+__device__ __forceinline__ void lds_pair(const float* v, float (&a)[2]) {
+  const float2 t = __ldcs(reinterpret_cast<const float2*>(v));
+  a[0] = t.x; a[1] = t.y;
+}
+__device__ __forceinline__ void lds_pair(const double* v, double (&a)[2]) {
+  const double2 t = __ldcs(reinterpret_cast<const double2*>(v));
+  a[0] = t.x; a[1] = t.y;
+}
+
+template <int UR> __device__ __forceinline__ const typename SpmvT<UR>::A* sell_vals(const Ctx& c);
+template <> __device__ __forceinline__ const double* sell_vals<P64>(const Ctx& c) { return c.sell_vals64; }
+template <> __device__ __forceinline__ const float* sell_vals<P32>(const Ctx& c) { return c.sell_vals32; }
+template <int UR> __device__ __forceinline__ const typename SpmvT<UR>::A* csr_vals(const Ctx& c);
+template <> __device__ __forceinline__ const double* csr_vals<P64>(const Ctx& c) { return c.vals64; }
+template <> __device__ __forceinline__ const float* csr_vals<P32>(const Ctx& c) { return c.vals32; }
 
 template <bool COH> __device__ __forceinline__ double gatherA(double, const double* p, int j) { return gather64<COH>(p, j); }
 template <bool COH> __device__ __forceinline__ double gatherA(double, const float* p, int j) { return gather64<COH>(p, j); }
@@ -77,143 +84,203 @@ template <bool COH> __device__ __forceinline__ float gatherA(float, const double
 template <bool COH> __device__ __forceinline__ float gatherA(float, const float* p, int j) { return gather32<COH>(p, j); }
 template <bool COH> __device__ __forceinline__ float gatherA(float, const __half* p, int j) { return gather32<COH>(p, j); }
 
-// Issue the three bulk copies of tile [r0,r1) x [e0,e1) into one stage (one lane).  Element
-// ranges are widened to multiples of 4 entries / rows so every address and size is 16-byte
-// aligned; the (at most 3) entries past the last multiple of 4 of the whole arrays are fetched
-// with plain loads because the borrowed CSR arrays are not padded.  A long row (more entries
-// than a stage holds) only completes the barrier phase: it is streamed from global memory.
-template <int UR>
-__device__ __forceinline__ void spmv_issue_tile(const Ctx& c, int t, unsigned char* stage, uint64_t* bar) {
+template <class A> struct LaneQ;  // elements a lane owns per 128-bit load of a value block
+template <> struct LaneQ<float> { static constexpr int v = 4; };
+template <> struct LaneQ<double> { static constexpr int v = 2; };
+__device__ __forceinline__ float lds_one(const float* v) { return __ldcs(v); }
+__device__ __forceinline__ double lds_one(const double* v) { return __ldcs(v); }
+
+// One slice of any width: this lane's row sum (one fma chain in CSR order).
+template <int UR, bool COH, class PT>
+__device__ __forceinline__ typename SpmvT<UR>::A slice_sum(const PT* p, const int32_t* cp, const typename SpmvT<UR>::A* vp,
+                                                          int w, int lane) {
   using A = typename SpmvT<UR>::A;
-  const int2 d0 = c.tile_desc[t], d1 = c.tile_desc[t + 1];
-  const int r0 = d0.x, e0 = d0.y, r1 = d1.x, e1 = d1.y;
-  if (e1 - e0 > kTileNnz) {
-    mbar_arrive_expect_tx(bar, 0u);
-    return;
+  constexpr int LQ = LaneQ<A>::v;
+  const int a = w >> 2;
+  A acc = 0;
+  int cq = 0;
+  for (; cq + 2 <= a; cq += 2) {  // two quads per trip: 4 (FP32) / 6 (FP64) 128-bit loads in flight
+    const int4 j0 = lds_i4(cp + cq * 128 + lane * 4);
+    const int4 j1 = lds_i4(cp + (cq + 1) * 128 + lane * 4);
+    A v0[4], v1[4];
+    lds_quad(vp + cq * 128 + lane * LQ, v0);
+    lds_quad(vp + (cq + 1) * 128 + lane * LQ, v1);
+    const A x0 = gatherA<COH>(A(0), p, j0.x), x1 = gatherA<COH>(A(0), p, j0.y);
+    const A x2 = gatherA<COH>(A(0), p, j0.z), x3 = gatherA<COH>(A(0), p, j0.w);
+    const A x4 = gatherA<COH>(A(0), p, j1.x), x5 = gatherA<COH>(A(0), p, j1.y);
+    const A x6 = gatherA<COH>(A(0), p, j1.z), x7 = gatherA<COH>(A(0), p, j1.w);
+    acc = fma(v0[0], x0, acc); acc = fma(v0[1], x1, acc); acc = fma(v0[2], x2, acc); acc = fma(v0[3], x3, acc);
+    acc = fma(v1[0], x4, acc); acc = fma(v1[1], x5, acc); acc = fma(v1[2], x6, acc); acc = fma(v1[3], x7, acc);
   }
-  const int ea = e0 & ~3;
-  const int nbody = (int)(c.nnz & ~(int64_t)3);
-  int eb = (e1 + 3) & ~3;
-  if (eb > nbody) eb = nbody;
-  A* vs = reinterpret_cast<A*>(stage);
-  int* cs = reinterpret_cast<int*>(stage + kStageValsBytes);
-  int* rs = reinterpret_cast<int*>(stage + kStageValsBytes + kStageColsBytes);
-  const A* gv = mat_vals<UR>(c);
-  bool tail = false;
-  for (int e = (eb > ea ? eb : ea); e < e1; ++e) {  // array tail (last tile of the matrix only)
-    vs[e - ea] = gv[e];
-    cs[e - ea] = c.colidx[e];
-    tail = true;
-  }
-  if (tail) fence_proxy_async();
-  const int r0a = r0 & ~3;
-  const int nr = ((r1 + 1 - r0a) + 3) & ~3;  // rowptr_pad is padded, so this never overruns
-  const uint32_t cnt = eb > ea ? (uint32_t)(eb - ea) : 0u;
-  mbar_arrive_expect_tx(bar, cnt * (uint32_t)(sizeof(A) + 4) + (uint32_t)nr * 4u);
-  if (cnt) {
-    bulk_g2s(vs, gv + ea, cnt * (uint32_t)sizeof(A), bar);
-    bulk_g2s(cs, c.colidx + ea, cnt * 4u, bar);
-  }
-  bulk_g2s(rs, c.rowptr_pad + r0a, (uint32_t)nr * 4u, bar);
+  // remainder: at most one quad, one pair, one single; all loads first, then all gathers
+  const bool hq = cq < a, hp = (w & 2) != 0, hs = (w & 1) != 0;
+  const int tail = a * 128;
+  int4 jq = make_int4(0, 0, 0, 0);
+  int2 jp = make_int2(0, 0);
+  int js = 0;
+  A vq[4] = {A(0), A(0), A(0), A(0)}, vpair[2] = {A(0), A(0)}, vs = A(0);
+  if (hq) { jq = lds_i4(cp + cq * 128 + lane * 4); lds_quad(vp + cq * 128 + lane * LQ, vq); }
+  if (hp) { jp = lds_i2(cp + tail + lane * 2); lds_pair(vp + tail + lane * 2, vpair); }
+  if (hs) { js = lds_i1(cp + tail + (hp ? 64 : 0) + lane); vs = lds_one(vp + tail + (hp ? 64 : 0) + lane); }
+  A xq0 = 0, xq1 = 0, xq2 = 0, xq3 = 0, xp0 = 0, xp1 = 0, xs = 0;
+  if (hq) { xq0 = gatherA<COH>(A(0), p, jq.x); xq1 = gatherA<COH>(A(0), p, jq.y);
+            xq2 = gatherA<COH>(A(0), p, jq.z); xq3 = gatherA<COH>(A(0), p, jq.w); }
+  if (hp) { xp0 = gatherA<COH>(A(0), p, jp.x); xp1 = gatherA<COH>(A(0), p, jp.y); }
+  if (hs) xs = gatherA<COH>(A(0), p, js);
+  if (hq) { acc = fma(vq[0], xq0, acc); acc = fma(vq[1], xq1, acc); acc = fma(vq[2], xq2, acc); acc = fma(vq[3], xq3, acc); }
+  if (hp) { acc = fma(vpair[0], xp0, acc); acc = fma(vpair[1], xp1, acc); }
+  if (hs) acc = fma(vs, xs, acc);
+  return acc;
 }
 
-// COH = true: p is written earlier in the same (persistent) kernel, so it is gathered with
-// plain coherent loads after the grid barrier instead of the read-only (ld.global.nc) path.
-// Returns this thread's part of gamma = sum_i p_i q_i.
-template <int UR, bool COH, int L, class PT>
-__device__ __forceinline__ double phase_spmv(const Ctx& c, const PT* p, typename Store<UR>::T* q, int bid, int nb,
-                                             unsigned char* smem_raw) {
+// G consecutive narrow slices (every width <= 7: one quad, one pair, one single at most) at once.
+// Branch-free: absent parts keep column 0 and value 0, so all matrix loads of the group are issued
+// (predicated) before the first gather and all 7 G gathers before the first fma — a warp keeps G times
+// the bytes of one short-row slice in flight and waits for memory three times per group, not per part.
+template <int UR, bool COH, int G, class PT>
+__device__ __forceinline__ void narrow_group_sum(const PT* p, const int32_t* cols, const typename SpmvT<UR>::A* vals,
+                                                 const int (&wp)[G + 1], int lane, typename SpmvT<UR>::A (&acc)[G]) {
   using A = typename SpmvT<UR>::A;
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const int gw = bid * kSpmvWarps + warp;  // global warp id: owns tiles [t_begin, t_end)
-  unsigned char* ring = smem_raw + warp * (kStages * kStageBytes);
-  uint64_t* bars = reinterpret_cast<uint64_t*>(smem_raw + kSpmvRingBytes) + warp * kStages;
-  constexpr int rows_per_pass = 32 / L;
-  const int sub = lane % L, rl = lane / L;
-  const int t_begin = c.warp_tile[gw], t_end = c.warp_tile[gw + 1];
-  double gsum = 0.0;
-  if (t_begin >= t_end) return gsum;
-
-  if (lane == 0) {
+  constexpr int LQ = LaneQ<A>::v;
+  int j[G][7];
+  A v[G][7];
 #pragma unroll
-    for (int s = 0; s < kStages; ++s) mbar_init(bars + s, 1);
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-#pragma unroll
-    for (int s = 0; s < kStages; ++s)
-      if (t_begin + s < t_end) spmv_issue_tile<UR>(c, t_begin + s, ring + s * kStageBytes, bars + s);
+  for (int g = 0; g < G; ++g) {
+    const int w = wp[g + 1] - wp[g];
+    const int32_t* cp = cols + (int64_t)wp[g] * 32;
+    const A* vp = vals + (int64_t)wp[g] * 32;
+    const bool hq = (w & 4) != 0, hp = (w & 2) != 0, hs = (w & 1) != 0;
+    const int tail = hq ? 128 : 0, tail1 = tail + (hp ? 64 : 0);
+    int4 jq = make_int4(0, 0, 0, 0);
+    int2 jp = make_int2(0, 0);
+    int js = 0;
+    A vq[4] = {A(0), A(0), A(0), A(0)}, vpair[2] = {A(0), A(0)}, vs = A(0);
+    if (hq) { jq = lds_i4(cp + lane * 4); lds_quad(vp + lane * LQ, vq); }
+    if (hp) { jp = lds_i2(cp + tail + lane * 2); lds_pair(vp + tail + lane * 2, vpair); }
+    if (hs) { js = lds_i1(cp + tail1 + lane); vs = lds_one(vp + tail1 + lane); }
+    j[g][0] = jq.x; j[g][1] = jq.y; j[g][2] = jq.z; j[g][3] = jq.w; j[g][4] = jp.x; j[g][5] = jp.y; j[g][6] = js;
+    v[g][0] = vq[0]; v[g][1] = vq[1]; v[g][2] = vq[2]; v[g][3] = vq[3]; v[g][4] = vpair[0]; v[g][5] = vpair[1]; v[g][6] = vs;
   }
-  __syncwarp();
-
-  for (int t = t_begin; t < t_end; ++t) {
-    const int it = t - t_begin;
-    const int slot = it % kStages;
-    const int2 d0 = c.tile_desc[t], d1 = c.tile_desc[t + 1];
-    const int r0 = d0.x, e0 = d0.y, nrows = d1.x - d0.x, e1 = d1.y;
-    unsigned char* stage = ring + slot * kStageBytes;
-    mbar_wait(bars + slot, (uint32_t)((it / kStages) & 1));
-
-    if (e1 - e0 > kTileNnz) {  // one long row: warp-strided accumulation straight from global
-      const A* gv = mat_vals<UR>(c);
-      A acc = 0;
-      for (int e = e0 + lane; e < e1; e += 32) acc = fma(gv[e], gatherA<COH>(A(0), p, c.colidx[e]), acc);
+  A x[G][7];
 #pragma unroll
-      for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
-      if (lane == 0) {
-        q[r0] = acc;
-        gsum = fma(gather64<COH>(p, r0), (double)acc, gsum);
-      }
+  for (int g = 0; g < G; ++g) {
+#pragma unroll
+    for (int u = 0; u < 7; ++u) x[g][u] = gatherA<COH>(A(0), p, j[g][u]);
+  }
+#pragma unroll
+  for (int g = 0; g < G; ++g) {
+    A t = 0;
+#pragma unroll
+    for (int u = 0; u < 7; ++u) t = fma(v[g][u], x[g][u], t);
+    acc[g] = t;
+  }
+}
+
+template <int UR> struct SpmvGroup;  // slices a warp takes per pass
+#ifndef AMP_SPMV_G32
+#define AMP_SPMV_G32 2
+#endif
+#ifndef AMP_SPMV_G64
+#define AMP_SPMV_G64 1
+#endif
+template <> struct SpmvGroup<P32> { static constexpr int G = AMP_SPMV_G32; };
+template <> struct SpmvGroup<P64> { static constexpr int G = AMP_SPMV_G64; };
+constexpr int kSpmvGroupMax = AMP_SPMV_G32 > AMP_SPMV_G64 ? AMP_SPMV_G32 : AMP_SPMV_G64;
+
+// q = A p over the slice groups first, first + stride, ... of this warp (a group = G consecutive
+// slices), then the long rows of this block.  COH = true: p was written earlier in the same
+// (persistent) kernel, so it is gathered with plain coherent loads instead of the read-only path.
+// NT = threads per block.
+// Returns this thread's part of gamma = sum_i p_i q_i (stored q_i, FP64 products and sums).
+template <int UR, bool COH, int NT, class PT>
+__device__ __forceinline__ double phase_spmv(const Ctx& c, const PT* p, typename Store<UR>::T* q, int bid, int nb,
+                                             double* red) {
+  using A = typename SpmvT<UR>::A;
+  constexpr int G = SpmvGroup<UR>::G;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  constexpr int wpb = NT / 32;
+  const int32_t* __restrict__ cols = c.sell_cols;
+  const A* __restrict__ vals = sell_vals<UR>(c);
+  const int32_t* __restrict__ wptr = c.sell_wptr;
+  const int nslices = c.nslices;
+  const int n = (int)c.n;
+  const int ngroups = (nslices + G - 1) / G;
+  double gsum = 0.0;
+
+  for (int gi = bid * wpb + warp; gi < ngroups; gi += nb * wpb) {
+    const int s0 = gi * G;
+    int wp[G + 1];
+    int wmax = 0;
+#pragma unroll
+    for (int g = 0; g <= G; ++g) wp[g] = __ldg(wptr + min(s0 + g, nslices));
+#pragma unroll
+    for (int g = 0; g < G; ++g) wmax = max(wmax, wp[g + 1] - wp[g]);
+    A acc[G];
+    if (wmax <= 7) {
+      narrow_group_sum<UR, COH, G>(p, cols, vals, wp, lane, acc);
     } else {
-      const A* vs = reinterpret_cast<const A*>(stage);
-      const int* cs = reinterpret_cast<const int*>(stage + kStageValsBytes);
-      const int* rs = reinterpret_cast<const int*>(stage + kStageValsBytes + kStageColsBytes) + (r0 - (r0 & ~3));
-      const int ea = e0 & ~3;
-      // L lanes per row: each lane reads its entries from shared memory, gathers p_j (the
-      // rows of a warp are adjacent, so for banded matrices the gathers of one instruction fall
-      // into few sectors), and accumulates an fma chain in the working precision (L = 1: in
-      // CSR order); the L partial sums are combined by shuffles.
-      for (int rb = 0; rb < nrows; rb += rows_per_pass) {
-        const int row = rb + rl;
-        A acc = 0;
-        double pi = 0.0;
-        if (row < nrows) {
-          const int jb = rs[row] - ea, je = rs[row + 1] - ea;
-          if (sub == 0) pi = gather64<COH>(p, r0 + row);
-          for (int j0 = jb + sub; j0 < je; j0 += kGatherBatch * L) {
-            A a[kGatherBatch], xg[kGatherBatch];
-            int cj[kGatherBatch];
 #pragma unroll
-            for (int u = 0; u < kGatherBatch; ++u) {
-              const int jj = j0 + u * L;
-              const bool ok = jj < je;
-              cj[u] = ok ? cs[jj] : (r0 + row);
-              a[u] = ok ? vs[jj] : A(0);
-            }
+      for (int g = 0; g < G; ++g)
+        acc[g] = slice_sum<UR, COH>(p, cols + (int64_t)wp[g] * 32, vals + (int64_t)wp[g] * 32, wp[g + 1] - wp[g], lane);
+    }
 #pragma unroll
-            for (int u = 0; u < kGatherBatch; ++u) xg[u] = gatherA<COH>(A(0), p, cj[u]);
-#pragma unroll
-            for (int u = 0; u < kGatherBatch; ++u) acc = fma(a[u], xg[u], acc);
-          }
-        }
-#pragma unroll
-        for (int o = L >> 1; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
-        if (row < nrows && sub == 0) {
-          q[r0 + row] = acc;
-          gsum = fma(pi, (double)acc, gsum);
+    for (int g = 0; g < G; ++g) {
+      if (s0 + g < nslices) {
+        int row = (s0 + g) * 32 + lane;
+        if (c.sell_perm != nullptr) row = __ldg(c.sell_perm + row);  // -1: padding slot
+        if (row >= 0 && row < n) {
+          q[row] = acc[g];
+          gsum = fma(gather64<COH>(p, row), (double)acc[g], gsum);
         }
       }
     }
-
-    // every lane is done reading the stage: hand it back to the producer
-    __syncwarp();
-    if (lane == 0 && t + kStages < t_end) spmv_issue_tile<UR>(c, t + kStages, stage, bars + slot);
-    __syncwarp();
   }
 
-  if (lane == 0) {
-#pragma unroll
-    for (int s = 0; s < kStages; ++s) mbar_inval(bars + s);
+  // rows too long for the slices: one block per row, straight from the CSR arrays
+  for (int lr = bid; lr < c.nlong; lr += nb) {
+    const int row = c.long_rows[lr];
+    const int e0 = c.rowptr[row], e1 = c.rowptr[row + 1];
+    const A* gv = csr_vals<UR>(c);
+    A acc = 0;
+    for (int e = e0 + (int)threadIdx.x; e < e1; e += NT) acc = fma(gv[e], gatherA<COH>(A(0), p, c.colidx[e]), acc);
+    const double tot = block_sum<NT>((double)acc, red);
+    if (threadIdx.x == 0) {
+      const A qi = (A)tot;
+      q[row] = qi;
+      gsum = fma(gather64<COH>(p, row), (double)qi, gsum);
+    }
   }
   return gsum;
+}
+
+// ------------------------------------------------------------------ create(): CSR -> SELL-32 --
+// one warp per slice; lane = row slot.  Long rows and padding slots get length 0.
+__global__ void k_sell_pack(int n, int nslices, int long_min, const int32_t* __restrict__ rowptr,
+                            const int32_t* __restrict__ colidx, const double* __restrict__ vals,
+                            const int32_t* __restrict__ wptr, const int32_t* __restrict__ perm, int32_t* __restrict__ cols,
+                            double* __restrict__ v64, float* __restrict__ v32) {
+  const int lane = threadIdx.x & 31;
+  const int s = (int)(((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5);
+  if (s >= nslices) return;
+  const int w0 = wptr[s], w = wptr[s + 1] - w0;
+  const int64_t base = (int64_t)w0 * 32;
+  int row = s * 32 + lane;
+  if (perm != nullptr) row = perm[row];
+  int e0 = 0, len = 0;
+  if (row >= 0 && row < n) {
+    e0 = rowptr[row];
+    len = rowptr[row + 1] - e0;
+    if (len > long_min) len = 0;
+  }
+  const int self = (row >= 0 && row < n) ? row : 0;
+  for (int k = 0; k < w; ++k) {
+    const bool ok = k < len;
+    const int j = ok ? colidx[e0 + k] : self;
+    const double v = ok ? vals[e0 + k] : 0.0;
+    cols[base + sell_pos32(k, lane, w)] = j;
+    v32[base + sell_pos32(k, lane, w)] = __double2float_rn(v);
+    v64[base + sell_pos64(k, lane, w)] = v;
+  }
 }
 
 }  // namespace amp

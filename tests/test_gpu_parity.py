@@ -306,7 +306,16 @@ def test_paper_examples_parity(ex, spec):
             # iteration count is sensitive to every rounding, so reduction order alone moves it; both sides
             # must converge in a comparable number of iterations, and the u_z switch happens in the same phase
             assert abs(st.iters - ref.iters) <= 0.2 * ref.iters, (st.iters, ref.iters)
-            assert switch_close(st.it_uz32, ref.it_uz32, 3)
+            # (4.1) switches u_z at the first k with nu_k < tau_zs; here nu_k oscillates by factors of 2-4 from
+            # one iteration to the next around that crossing (oracle: nu_63..68 = 2.6e-4, 1.4e-4, 1.4e-4, 2.8e-4,
+            # 2.2e-4, 6.8e-5), so the GPU's crossing must fall where the ORACLE's own nu_k is within a factor 3 of
+            # tau_zs: not before the oracle first drops below 3 tau_zs, not after it first drops below tau_zs / 3
+            nu = np.asarray(ref.hist) / ref.bnorm
+            tau_zs = 1e-4
+            lo = int(np.argmax(nu < 3.0 * tau_zs))
+            hi = int(np.argmax(nu < tau_zs / 3.0))
+            assert lo <= ref.it_uz32 <= hi
+            assert lo <= st.it_uz32 <= hi, (st.it_uz32, lo, hi, ref.it_uz32)
         else:
             assert abs(st.iters - ref.iters) <= max(2, math.ceil(0.05 * ref.iters)), (st.iters, ref.iters)
             assert switch_close(st.it_ur32, ref.it_ur32, 3) and switch_close(st.it_uz16, ref.it_uz16, 3)
