@@ -279,15 +279,14 @@ extern "C" amp_pcg_t* amp_pcg_create(int64_t n, int64_t nnz, const int32_t* rowp
 
   // persistent kernel and vector kernels: whole multiples of the SM count
   persistent_configure(h->num_sms, &h->persist_grid, &h->persist_ok);
-  // vector kernels: a whole number of equally long grid-stride trips per block, at most one full wave
+  // vector kernels: one full wave of blocks (grid-stride loops inside); small problems get fewer blocks
+  // (at least 2 chunks of 8 elements per thread)
   auto vec_grid_for = [&](const void* kern) -> int {
     int occ = 1;
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, kVecThreads, 0) != cudaSuccess) { cudaGetLastError(); occ = 1; }
-    const int64_t per_trip = (int64_t)kVecThreads * kVecUnrollNarrow;  // pairs per block and trip
     const int64_t max_grid = std::min<int64_t>((int64_t)h->num_sms * std::max(occ, 1), (int64_t)kMaxGrid);
-    const int64_t npair = h->npad / 2;
-    const int64_t trips = std::max<int64_t>(1, (npair + max_grid * per_trip - 1) / (max_grid * per_trip));
-    return (int)std::max<int64_t>(1, (npair + trips * per_trip - 1) / (trips * per_trip));
+    const int64_t want = (h->npad / 16 + kVecThreads - 1) / kVecThreads;
+    return (int)std::max<int64_t>(1, std::min(max_grid, want));
   };
   h->grid_z = vec_grid_for((const void*)k_z);
   h->grid_p = vec_grid_for((const void*)k_p);

@@ -12,8 +12,6 @@ namespace amp {
 
 constexpr int P64 = 0, P32 = 1, P16 = 2;       // precision codes (= AMP_FP64/32/16 of the C ABI)
 constexpr int kVecThreads = 256;               // block size of the vector kernels
-constexpr int kVecUnrollNarrow = 4;            // independent 2-element chunks in flight per thread (some operand < FP64)
-constexpr int kVecUnrollWide = 2;              // ... when every operand is FP64 (same bytes in flight, half the registers)
 constexpr int kSpmvThreads = 256;              // block size of the SpMV kernel: 8 warps, one SELL slice per warp and pass
 constexpr int kSpmvWarps = kSpmvThreads / 32;
 #ifndef AMP_SPMV_MINBLOCKS
@@ -130,6 +128,80 @@ __device__ __forceinline__ void store2(float* a, int64_t pair, double v0, double
 __device__ __forceinline__ void store2(__half* a, int64_t pair, double v0, double v1) {
   reinterpret_cast<__half2*>(a)[pair] = __halves2half2(__double2half(v0), __double2half(v1));
 }
+
+// ------------------------------------------------------------------ chunked vector access ---
+// The vector kernels give every thread chunks of E consecutive elements; a chunk of an array of
+// type T is E*sizeof(T) contiguous bytes, moved with 128-bit accesses (64-bit for 4 halves).
+// E = min(16 / smallest element, 32 / largest element) over the arrays of a kernel, so the
+// narrowest array moves 16 bytes per access and the widest at most 32 bytes (one sector) per
+// thread.  Raw words are kept packed until they are used (many chunks in flight, few registers).
+template <class T, int E> struct Chunk {
+  static constexpr int W = E * (int)sizeof(T) / 4;  // 32-bit words
+  static_assert(W == 2 || W % 4 == 0, "chunk must be 8 bytes or a multiple of 16");
+  uint32_t w[W];
+};
+template <class T, int E> __device__ __forceinline__ void chunk_load(Chunk<T, E>& k, const T* a, int64_t chunk) {
+  constexpr int W = Chunk<T, E>::W;
+  const char* src = reinterpret_cast<const char*>(a) + chunk * (int64_t)(E * sizeof(T));
+  if constexpr (W == 2) {
+    const uint2 t = *reinterpret_cast<const uint2*>(src);
+    k.w[0] = t.x; k.w[1] = t.y;
+  } else {
+#pragma unroll
+    for (int i = 0; i < W / 4; ++i) {
+      const uint4 t = *reinterpret_cast<const uint4*>(src + 16 * i);
+      k.w[4 * i] = t.x; k.w[4 * i + 1] = t.y; k.w[4 * i + 2] = t.z; k.w[4 * i + 3] = t.w;
+    }
+  }
+}
+template <class T, int E> __device__ __forceinline__ void chunk_store(const Chunk<T, E>& k, T* a, int64_t chunk) {
+  constexpr int W = Chunk<T, E>::W;
+  char* dst = reinterpret_cast<char*>(a) + chunk * (int64_t)(E * sizeof(T));
+  if constexpr (W == 2) {
+    *reinterpret_cast<uint2*>(dst) = make_uint2(k.w[0], k.w[1]);
+  } else {
+#pragma unroll
+    for (int i = 0; i < W / 4; ++i)
+      *reinterpret_cast<uint4*>(dst + 16 * i) = make_uint4(k.w[4 * i], k.w[4 * i + 1], k.w[4 * i + 2], k.w[4 * i + 3]);
+  }
+}
+// exact conversion of the stored values to FP64
+template <int E> __device__ __forceinline__ void chunk_unpack(const Chunk<double, E>& k, double (&v)[E]) {
+#pragma unroll
+  for (int i = 0; i < E; ++i) v[i] = __hiloint2double((int)k.w[2 * i + 1], (int)k.w[2 * i]);
+}
+template <int E> __device__ __forceinline__ void chunk_unpack(const Chunk<float, E>& k, double (&v)[E]) {
+#pragma unroll
+  for (int i = 0; i < E; ++i) v[i] = (double)__uint_as_float(k.w[i]);
+}
+template <int E> __device__ __forceinline__ void chunk_unpack(const Chunk<__half, E>& k, double (&v)[E]) {
+#pragma unroll
+  for (int i = 0; i < E / 2; ++i) {
+    const float2 f = __half22float2(*reinterpret_cast<const __half2*>(&k.w[i]));
+    v[2 * i] = (double)f.x; v[2 * i + 1] = (double)f.y;
+  }
+}
+// one IEEE round-to-nearest-even from FP64 to the storage type (direct, no double rounding)
+template <int E> __device__ __forceinline__ void chunk_pack(Chunk<double, E>& k, const double (&v)[E]) {
+#pragma unroll
+  for (int i = 0; i < E; ++i) { k.w[2 * i] = (uint32_t)__double2loint(v[i]); k.w[2 * i + 1] = (uint32_t)__double2hiint(v[i]); }
+}
+template <int E> __device__ __forceinline__ void chunk_pack(Chunk<float, E>& k, const double (&v)[E]) {
+#pragma unroll
+  for (int i = 0; i < E; ++i) k.w[i] = __float_as_uint(__double2float_rn(v[i]));
+}
+template <int E> __device__ __forceinline__ void chunk_pack(Chunk<__half, E>& k, const double (&v)[E]) {
+#pragma unroll
+  for (int i = 0; i < E / 2; ++i) {
+    const __half2 h = __halves2half2(__double2half(v[2 * i]), __double2half(v[2 * i + 1]));
+    k.w[i] = *reinterpret_cast<const uint32_t*>(&h);
+  }
+}
+__host__ __device__ constexpr int cmin(int a, int b) { return a < b ? a : b; }
+__host__ __device__ constexpr int cmax(int a, int b) { return a > b ? a : b; }
+// elements per chunk for a kernel whose arrays have element sizes in [smin, smax] bytes
+__host__ __device__ constexpr int chunk_elems(int smin, int smax) { return cmin(16 / smin, 32 / smax); }
+constexpr int kVecBytesInFlight = 192;  // target bytes of loads in flight per thread of a vector kernel
 
 // gather of one element of p as the SpMV working type.  COH = false: read-only path (p is not
 // written by the running kernel); COH = true: plain coherent load.

@@ -72,7 +72,7 @@ __global__ void __launch_bounds__(kVecThreads, 3) k_z(const Ctx c) {
                            [&](double tot) { epi_rho(epi_ctx(c), tot); });
 }
 
-__global__ void __launch_bounds__(kVecThreads, 4) k_p(const Ctx c) {
+__global__ void __launch_bounds__(kVecThreads, 3) k_p(const Ctx c) {
   const DevState* s = c.st;
   if (s->done) return;
   dispatch_p(c, s->p_store, s->uz, s->beta, s->k == 0, blockIdx.x, gridDim.x);

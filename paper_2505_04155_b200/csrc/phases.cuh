@@ -145,10 +145,22 @@ __device__ __noinline__ void epi_delta(const EpiCtx c, double rr) {
   set_loop_cond(c, !s->done);
 }
 
+#ifdef AMP_COUNT_FP16
+// counting build: classify every FP16 store of z and p (exact value v, stored value h)
+__device__ __forceinline__ void count_fp16(DevState* s, double v, double h) {
+  if (v == 0.0) return;
+  if (isinf(h) && !isinf(v)) atomicAdd(&s->fp16_inf, 1ull);
+  else if (h == 0.0) atomicAdd(&s->fp16_flushed, 1ull);
+  else if (fabs(h) < 6.103515625e-05) atomicAdd(&s->fp16_subnormal, 1ull);
+}
+#endif
+
 // NOTE: the loop vectors (r, z, p, q, x) are deliberately NOT __restrict__/read-only qualified:
 // inside the persistent kernel they are written by earlier phases of the same kernel, so they
 // must be read with plain coherent loads (ordered by the grid barrier), never ld.global.nc.
-// Loads are grouped ahead of the stores by hand (kVecUnroll chunks in flight per thread).
+// Every thread owns chunks of E consecutive elements (common.cuh: chunk_*), U chunks per trip:
+// all loads of a trip are issued before the first use, so a thread keeps about
+// kVecBytesInFlight bytes in flight whatever the precisions are.
 
 // ------------------------------------------------------------------ a2: z and rho ------------
 // RS: precision r is stored in; UR: precision selected for r (RS != UR only at the iteration of
@@ -156,43 +168,61 @@ __device__ __noinline__ void epi_delta(const EpiCtx c, double rr) {
 template <int RS, int UR, int UZ>
 __device__ __forceinline__ double phase_z(const Ctx& c, const double omega, int bid, int nb) {
   using TR = typename Store<RS>::T;
+  using TO = typename Store<UR>::T;
+  using TZ = typename Store<UZ>::T;
   using TD = typename Store<(UZ == P64) ? P64 : P32>::T;
+  constexpr int smin = cmin(cmin((int)sizeof(TR), (int)sizeof(TO)), cmin((int)sizeof(TD), (int)sizeof(TZ)));
+  constexpr int smax = cmax(cmax((int)sizeof(TR), (int)sizeof(TO)), cmax((int)sizeof(TD), (int)sizeof(TZ)));
+  constexpr int E = chunk_elems(smin, smax);
+  constexpr int U = cmax(1, kVecBytesInFlight / (E * (int)(sizeof(TR) + sizeof(TD))));
   const TR* rin = rvec<RS>(c);
-  typename Store<UR>::T* rout = rvec<UR>(c);
-  typename Store<UZ>::T* z = zvec<UZ>(c);
+  TO* rout = rvec<UR>(c);
+  TZ* z = zvec<UZ>(c);
   const TD* dinv;
   if constexpr (UZ == P64) dinv = c.dinv64; else dinv = c.dinv32;
-  const int64_t npair = c.npad >> 1;
+  const int64_t nchunk = c.npad / E;
   const int64_t stride = (int64_t)nb * blockDim.x;
-  constexpr int U = (RS == P64 && UZ == P64) ? kVecUnrollWide : kVecUnrollNarrow;
   double sum = 0.0;
-  for (int64_t base = (int64_t)bid * blockDim.x + threadIdx.x; base < npair; base += stride * U) {
-    typename Raw2<TR>::T rr[U];
-    typename Raw2<TD>::T dd[U];
+  for (int64_t base = (int64_t)bid * blockDim.x + threadIdx.x; base < nchunk; base += stride * U) {
+    Chunk<TR, E> rr[U];
+    Chunk<TD, E> dd[U];
 #pragma unroll
     for (int u = 0; u < U; ++u) {
       const int64_t i = base + u * stride;
-      if (i < npair) { rr[u] = load_raw(rin, i); dd[u] = load_raw(dinv, i); }
+      if (i < nchunk) { chunk_load(rr[u], rin, i); chunk_load(dd[u], dinv, i); }
     }
 #pragma unroll
     for (int u = 0; u < U; ++u) {
       const int64_t i = base + u * stride;
-      if (i < npair) {
-        double a0, a1, d0, d1;
-        unpack(rr[u], a0, a1);
-        unpack(dd[u], d0, d1);
-        if (RS != UR) {  // r <- RN_{u_r}(r) at the switch iteration
-          a0 = round_to<UR>(a0); a1 = round_to<UR>(a1);
-          store2(rout, i, a0, a1);
+      if (i < nchunk) {
+        double a[E], d[E], zz[E];
+        chunk_unpack(rr[u], a);
+        chunk_unpack(dd[u], d);
+        if constexpr (RS != UR) {  // r <- RN_{u_r}(r) at the switch iteration
+          Chunk<TO, E> ro;
+          chunk_pack(ro, a);
+          chunk_store(ro, rout, i);
+          chunk_unpack(ro, a);
         }
-        const double z0 = round_to<UZ>((a0 * omega) * d0);
-        const double z1 = round_to<UZ>((a1 * omega) * d1);
-        store2(z, i, z0, z1);
+#pragma unroll
+        for (int e = 0; e < E; ++e) zz[e] = (a[e] * omega) * d[e];
+        Chunk<TZ, E> zo;
+        chunk_pack(zo, zz);  // the one rounding to u_z (reading R6)
+        chunk_store(zo, z, i);
 #ifdef AMP_COUNT_FP16
-        if (UZ == P16) { count_fp16(c.st, (a0 * omega) * d0, z0); count_fp16(c.st, (a1 * omega) * d1, z1); }
+        double zx[E];
+#pragma unroll
+        for (int e = 0; e < E; ++e) zx[e] = zz[e];
 #endif
-        sum = fma(a0, z0, sum);
-        sum = fma(a1, z1, sum);
+        chunk_unpack(zo, zz);
+#ifdef AMP_COUNT_FP16
+        if (UZ == P16) {
+#pragma unroll
+          for (int e = 0; e < E; ++e) count_fp16(c.st, zx[e], zz[e]);
+        }
+#endif
+#pragma unroll
+        for (int e = 0; e < E; ++e) sum = fma(a[e], zz[e], sum);  // rho uses the stored z
       }
     }
   }
@@ -206,35 +236,52 @@ template <int PS, int UZ>
 __device__ __forceinline__ void phase_p(const Ctx& c, const double beta, const bool first, int bid, int nb) {
   using TP = typename Store<PS>::T;
   using TZ = typename Store<UZ>::T;
+  constexpr int E = chunk_elems(cmin((int)sizeof(TP), (int)sizeof(TZ)), cmax((int)sizeof(TP), (int)sizeof(TZ)));
+  constexpr int U = cmax(1, kVecBytesInFlight / (E * (int)(sizeof(TP) + sizeof(TZ))));
   const TP* pin = pvec<PS>(c);
   TZ* pout = pvec<UZ>(c);
   const TZ* z = zvec<UZ>(c);
-  const int64_t npair = c.npad >> 1;
+  const int64_t nchunk = c.npad / E;
   const int64_t stride = (int64_t)nb * blockDim.x;
-  constexpr int U = kVecUnrollNarrow;
-  for (int64_t base = (int64_t)bid * blockDim.x + threadIdx.x; base < npair; base += stride * U) {
-    typename Raw2<TP>::T pp[U];
-    typename Raw2<TZ>::T zz[U];
+  for (int64_t base = (int64_t)bid * blockDim.x + threadIdx.x; base < nchunk; base += stride * U) {
+    Chunk<TP, E> pp[U];
+    Chunk<TZ, E> zz[U];
 #pragma unroll
     for (int u = 0; u < U; ++u) {
       const int64_t i = base + u * stride;
-      if (i < npair) {
-        zz[u] = load_raw(z, i);
-        if (!first) pp[u] = load_raw(pin, i);
+      if (i < nchunk) {
+        chunk_load(zz[u], z, i);
+        if (!first) chunk_load(pp[u], pin, i);
       }
     }
 #pragma unroll
     for (int u = 0; u < U; ++u) {
       const int64_t i = base + u * stride;
-      if (i < npair) {
-        double a0 = 0.0, a1 = 0.0, z0, z1;
-        unpack(zz[u], z0, z1);
-        if (!first) unpack(pp[u], a0, a1);
-        if (PS != UZ) { a0 = round_to<UZ>(a0); a1 = round_to<UZ>(a1); }
-        const double n0 = fma(beta, a0, z0), n1 = fma(beta, a1, z1);
-        store2(pout, i, n0, n1);
+      if (i < nchunk) {
+        double a[E], zv[E];
+        chunk_unpack(zz[u], zv);
+        if (!first) {
+          chunk_unpack(pp[u], a);
+          if constexpr (PS != UZ) {
+#pragma unroll
+            for (int e = 0; e < E; ++e) a[e] = round_to<UZ>(a[e]);
+          }
+        } else {
+#pragma unroll
+          for (int e = 0; e < E; ++e) a[e] = 0.0;
+        }
+#pragma unroll
+        for (int e = 0; e < E; ++e) a[e] = fma(beta, a[e], zv[e]);
+        Chunk<TZ, E> po;
+        chunk_pack(po, a);
+        chunk_store(po, pout, i);
 #ifdef AMP_COUNT_FP16
-        if (UZ == P16) { count_fp16(c.st, n0, round_to<P16>(n0)); count_fp16(c.st, n1, round_to<P16>(n1)); }
+        if (UZ == P16) {
+          double h[E];
+          chunk_unpack(po, h);
+#pragma unroll
+          for (int e = 0; e < E; ++e) count_fp16(c.st, a[e], h[e]);
+        }
 #endif
       }
     }
@@ -246,45 +293,64 @@ template <int UR, int UZ>
 __device__ __forceinline__ double phase_xr(const Ctx& c, const double alpha, double* x, int bid, int nb) {
   using TZ = typename Store<UZ>::T;
   using TR = typename Store<UR>::T;
+  constexpr int E = chunk_elems(cmin((int)sizeof(TZ), (int)sizeof(TR)), 8);
+  constexpr int U = cmax(1, kVecBytesInFlight / (E * (int)(8 + sizeof(TZ) + 2 * sizeof(TR))));
   const TZ* p = pvec<UZ>(c);
   const TR* q = qvec<UR>(c);
   TR* r = rvec<UR>(c);
   const int64_t n = c.n;
-  const int64_t npair = c.npad >> 1;
+  const int64_t nchunk = c.npad / E;
   const int64_t stride = (int64_t)nb * blockDim.x;
-  constexpr int U = kVecUnrollNarrow;
   double sum = 0.0;
-  for (int64_t base = (int64_t)bid * blockDim.x + threadIdx.x; base < npair; base += stride * U) {
-    double2 xx[U];
-    typename Raw2<TZ>::T pp[U];
-    typename Raw2<TR>::T qq[U], rr[U];
+  for (int64_t base = (int64_t)bid * blockDim.x + threadIdx.x; base < nchunk; base += stride * U) {
+    Chunk<double, E> xx[U];
+    Chunk<TZ, E> pp[U];
+    Chunk<TR, E> qq[U], rr[U];
 #pragma unroll
     for (int u = 0; u < U; ++u) {
       const int64_t i = base + u * stride;
-      if (i < npair) {
-        if (2 * i + 1 < n) xx[u] = load_raw(x, i);
-        else xx[u] = make_double2((2 * i < n) ? x[2 * i] : 0.0, 0.0);  // x is caller-owned: exactly n long
-        pp[u] = load_raw(p, i);
-        qq[u] = load_raw(q, i);
-        rr[u] = load_raw(r, i);
+      if (i < nchunk) {
+        if ((i + 1) * E <= n) {
+          chunk_load(xx[u], x, i);
+        } else {  // x is caller-owned: exactly n long
+          double t[E];
+#pragma unroll
+          for (int e = 0; e < E; ++e) t[e] = (i * E + e < n) ? x[i * E + e] : 0.0;
+          chunk_pack(xx[u], t);
+        }
+        chunk_load(pp[u], p, i);
+        chunk_load(qq[u], q, i);
+        chunk_load(rr[u], r, i);
       }
     }
 #pragma unroll
     for (int u = 0; u < U; ++u) {
       const int64_t i = base + u * stride;
-      if (i < npair) {
-        double p0, p1, q0, q1, r0, r1;
-        unpack(pp[u], p0, p1);
-        unpack(qq[u], q0, q1);
-        unpack(rr[u], r0, r1);
-        const double nx0 = fma(alpha, p0, xx[u].x), nx1 = fma(alpha, p1, xx[u].y);  // line 15, FP64
-        if (2 * i + 1 < n) store2(x, i, nx0, nx1);
-        else if (2 * i < n) x[2 * i] = nx0;
-        const double nr0 = round_to<UR>(fma(-alpha, q0, r0));  // line 16, one rounding to u_r
-        const double nr1 = round_to<UR>(fma(-alpha, q1, r1));
-        store2(r, i, nr0, nr1);
-        sum = fma(nr0, nr0, sum);
-        sum = fma(nr1, nr1, sum);
+      if (i < nchunk) {
+        double xv[E], pv[E], qv[E], rv[E];
+        chunk_unpack(xx[u], xv);
+        chunk_unpack(pp[u], pv);
+        chunk_unpack(qq[u], qv);
+        chunk_unpack(rr[u], rv);
+#pragma unroll
+        for (int e = 0; e < E; ++e) xv[e] = fma(alpha, pv[e], xv[e]);  // line 15, FP64
+        if ((i + 1) * E <= n) {
+          Chunk<double, E> xo;
+          chunk_pack(xo, xv);
+          chunk_store(xo, x, i);
+        } else {
+#pragma unroll
+          for (int e = 0; e < E; ++e)
+            if (i * E + e < n) x[i * E + e] = xv[e];
+        }
+#pragma unroll
+        for (int e = 0; e < E; ++e) rv[e] = fma(-alpha, qv[e], rv[e]);  // line 16
+        Chunk<TR, E> ro;
+        chunk_pack(ro, rv);  // one rounding to u_r
+        chunk_store(ro, r, i);
+        chunk_unpack(ro, rv);
+#pragma unroll
+        for (int e = 0; e < E; ++e) sum = fma(rv[e], rv[e], sum);
       }
     }
   }
