@@ -59,6 +59,7 @@ struct amp_pcg {
   int64_t launches = 0;
   int32_t last_iters = -1;
   double m_avg = 0.0;
+  double idx_bytes = 4.0;     // column-index bytes per stored entry of the format in use
   int64_t sell_entries = 0;   // stored entries of the SELL-32 repack (padding included)
 };
 
@@ -242,10 +243,15 @@ extern "C" amp_pcg_t* amp_pcg_create(int64_t n, int64_t nnz, const int32_t* rowp
       return nullptr;
     }
     const size_t total = (size_t)wsum * 32 + 256;
-    int32_t *wptr_d, *cols_d, *perm_d = nullptr, *long_d;
+    int32_t *wptr_d, *cols_d, *perm_d = nullptr, *long_d, *base_d;
+    uint16_t* cols16_d;
+    int* flag16_d;
     double* v64_d; float* v32_d;
     ALLOC(wptr_d, int32_t, wptr.size());
     ALLOC(cols_d, int32_t, total);
+    ALLOC(cols16_d, uint16_t, total);
+    ALLOC(base_d, int32_t, (size_t)wsum + 64);
+    ALLOC(flag16_d, int, 1);
     ALLOC(v64_d, double, total);
     ALLOC(v32_d, float, total);
     ALLOC(long_d, int32_t, long_rows.size() + 1);
@@ -259,11 +265,27 @@ extern "C" amp_pcg_t* amp_pcg_create(int64_t n, int64_t nnz, const int32_t* rowp
       CU_TRY(cudaMemcpyAsync(perm_d, perm.data(), sizeof(int32_t) * perm.size(), cudaMemcpyHostToDevice, h->stream),
              { amp_pcg_destroy(h); return nullptr; });
     const int pgrid = (int)((nsl * 32 + 255) / 256);
-    k_sell_pack<<<pgrid, 256, 0, h->stream>>>((int)n, (int)nsl, long_min, rowptr, colidx, vals, wptr_d, perm_d, cols_d, v64_d,
-                                             v32_d);
+    k_sell_pack<<<pgrid, 256, 0, h->stream>>>((int)n, (int)nsl, long_min, rowptr, colidx, vals, wptr_d, perm_d, cols_d,
+                                             cols16_d, base_d, v64_d, v32_d, flag16_d);
+    int wide = 0;
+    CU_TRY(cudaMemcpyAsync(&wide, flag16_d, sizeof(int), cudaMemcpyDeviceToHost, h->stream), { amp_pcg_destroy(h); return nullptr; });
     CU_TRY(cudaStreamSynchronize(h->stream), { amp_pcg_destroy(h); return nullptr; });
     CU_TRY(cudaGetLastError(), { amp_pcg_destroy(h); return nullptr; });
-    c.sell_wptr = wptr_d; c.sell_cols = cols_d; c.sell_vals64 = v64_d; c.sell_vals32 = v32_d; c.sell_perm = perm_d;
+    if (getenv("AMP_SPMV_IDX32")) wide = 1;  // tuning aid: force 32-bit column indices
+    auto release = [&](void* ptr) {
+      cudaFree(ptr);
+      h->owned.erase(std::find(h->owned.begin(), h->owned.end(), ptr));
+    };
+    if (wide) {  // some offset needs more than 16 bits: keep the 32-bit indices
+      release(cols16_d); release(base_d);
+      cols16_d = nullptr; base_d = nullptr;
+    } else {
+      release(cols_d);
+      cols_d = nullptr;
+    }
+    h->idx_bytes = wide ? 4.0 : 2.0 + 4.0 / 32.0;
+    c.sell_wptr = wptr_d; c.sell_cols = cols_d; c.sell_cols16 = cols16_d; c.sell_base = base_d;
+    c.sell_vals64 = v64_d; c.sell_vals32 = v32_d; c.sell_perm = perm_d;
     c.long_rows = long_d; c.nslices = (int32_t)nsl; c.nlong = (int32_t)long_rows.size();
     h->sell_entries = wsum * 32;
 

@@ -62,7 +62,9 @@ struct Ctx {
   double* partials;       // [4][kMaxGrid] per-block partial sums
   // SELL-32 repack of A (spmv.cuh), owned by the handle
   const int32_t* sell_wptr;   // [nslices+1] cumulative slice widths; slice s starts at element 32*sell_wptr[s]
-  const int32_t* sell_cols;   // column indices
+  const int32_t* sell_cols;   // 32-bit column indices (nullptr when the 16-bit format is in use)
+  const uint16_t* sell_cols16;  // 16-bit column offsets from sell_base, or nullptr
+  const int32_t* sell_base;   // [sum of widths] smallest column of entry k of each slice
   const double* sell_vals64;  // FP64 values
   const float* sell_vals32;   // FP32-rounded values (u_r = FP32 phase)
   const int32_t* sell_perm;   // [32*nslices] row of each slot (-1 = padding), or nullptr = identity

@@ -90,82 +90,166 @@ template <> struct LaneQ<double> { static constexpr int v = 2; };
 __device__ __forceinline__ float lds_one(const float* v) { return __ldcs(v); }
 __device__ __forceinline__ double lds_one(const double* v) { return __ldcs(v); }
 
+// ------------------------------------------------------------------ column index sources ----
+// I16 = false: 32-bit column indices.  I16 = true: 16-bit offsets from a per-(slice, entry) base
+// (the smallest column of entry k over the 32 rows of the slice, sell_base[w0 + k]); chosen in
+// create() when every offset fits, which holds for banded / stencil matrices.  The base of entry
+// k is held by lane k % 32 and broadcast by a shuffle, so the index stream is 2 B per entry plus
+// 4 B per 32 entries.
+template <bool I16> struct ColSrc;
+template <> struct ColSrc<false> {
+  using RawQ = int4; using RawP = int2; using RawS = int;
+  const int32_t* cp;
+  __device__ __forceinline__ ColSrc(const Ctx& c, int w0, int, int) : cp(c.sell_cols + (int64_t)w0 * 32) {}
+  __device__ __forceinline__ void refresh(int, int) {}
+  __device__ __forceinline__ RawQ quad(int off, int lane) const { return lds_i4(cp + off + lane * 4); }
+  __device__ __forceinline__ RawP pair(int off, int lane) const { return lds_i2(cp + off + lane * 2); }
+  __device__ __forceinline__ RawS single(int off, int lane) const { return lds_i1(cp + off + lane); }
+  __device__ __forceinline__ void dq(RawQ r, int, int (&j)[4]) const { j[0] = r.x; j[1] = r.y; j[2] = r.z; j[3] = r.w; }
+  __device__ __forceinline__ void dp(RawP r, int, int (&j)[2]) const { j[0] = r.x; j[1] = r.y; }
+  __device__ __forceinline__ int ds(RawS r, int) const { return r; }
+  static __device__ __forceinline__ RawQ zq() { return make_int4(0, 0, 0, 0); }
+  static __device__ __forceinline__ RawP zp() { return make_int2(0, 0); }
+};
+template <> struct ColSrc<true> {
+  using RawQ = uint2; using RawP = uint32_t; using RawS = uint32_t;
+  const uint16_t* cp;
+  const int32_t* bp;  // bases of this slice
+  int w, blk, bl;
+  __device__ __forceinline__ ColSrc(const Ctx& c, int w0, int w_, int lane)
+      : cp(c.sell_cols16 + (int64_t)w0 * 32), bp(c.sell_base + w0), w(w_), blk(0) {
+    bl = (lane < w) ? __ldg(bp + lane) : 0;
+  }
+  // make the bases of entries [32*(k/32), +32) current (slices wider than 32 entries only)
+  __device__ __forceinline__ void refresh(int k, int lane) {
+    if ((k >> 5) != blk) {
+      blk = k >> 5;
+      bl = (blk * 32 + lane < w) ? __ldg(bp + blk * 32 + lane) : 0;
+    }
+  }
+  __device__ __forceinline__ RawQ quad(int off, int lane) const { return __ldcs(reinterpret_cast<const uint2*>(cp + off + lane * 4)); }
+  __device__ __forceinline__ RawP pair(int off, int lane) const { return __ldcs(reinterpret_cast<const uint32_t*>(cp + off + lane * 2)); }
+  __device__ __forceinline__ RawS single(int off, int lane) const { return (uint32_t)__ldcs(cp + off + lane); }
+  __device__ __forceinline__ int base(int k) const { return __shfl_sync(0xffffffffu, bl, k & 31); }
+  __device__ __forceinline__ void dq(RawQ r, int k, int (&j)[4]) const {
+    j[0] = base(k) + (int)(r.x & 0xffffu); j[1] = base(k + 1) + (int)(r.x >> 16);
+    j[2] = base(k + 2) + (int)(r.y & 0xffffu); j[3] = base(k + 3) + (int)(r.y >> 16);
+  }
+  __device__ __forceinline__ void dp(RawP r, int k, int (&j)[2]) const {
+    j[0] = base(k) + (int)(r & 0xffffu); j[1] = base(k + 1) + (int)(r >> 16);
+  }
+  __device__ __forceinline__ int ds(RawS r, int k) const { return base(k) + (int)r; }
+  static __device__ __forceinline__ RawQ zq() { return make_uint2(0u, 0u); }
+  static __device__ __forceinline__ RawP zp() { return 0u; }
+};
+
 // One slice of any width: this lane's row sum (one fma chain in CSR order).
-template <int UR, bool COH, class PT>
-__device__ __forceinline__ typename SpmvT<UR>::A slice_sum(const PT* p, const int32_t* cp, const typename SpmvT<UR>::A* vp,
-                                                          int w, int lane) {
+template <int UR, bool COH, bool I16, class PT>
+__device__ __forceinline__ typename SpmvT<UR>::A slice_sum(const Ctx& c, const PT* p, int w0, int w, int lane) {
   using A = typename SpmvT<UR>::A;
+  using CS = ColSrc<I16>;
   constexpr int LQ = LaneQ<A>::v;
+  CS cs(c, w0, w, lane);
+  const A* vp = sell_vals<UR>(c) + (int64_t)w0 * 32;
   const int a = w >> 2;
   A acc = 0;
   int cq = 0;
-  for (; cq + 2 <= a; cq += 2) {  // two quads per trip: 4 (FP32) / 6 (FP64) 128-bit loads in flight
-    const int4 j0 = lds_i4(cp + cq * 128 + lane * 4);
-    const int4 j1 = lds_i4(cp + (cq + 1) * 128 + lane * 4);
+  for (; cq + 2 <= a; cq += 2) {  // two quads per trip: 4 (FP32) / 6 (FP64) wide loads in flight
+    cs.refresh(4 * cq, lane);
+    const typename CS::RawQ r0 = cs.quad(cq * 128, lane), r1 = cs.quad((cq + 1) * 128, lane);
     A v0[4], v1[4];
     lds_quad(vp + cq * 128 + lane * LQ, v0);
     lds_quad(vp + (cq + 1) * 128 + lane * LQ, v1);
-    const A x0 = gatherA<COH>(A(0), p, j0.x), x1 = gatherA<COH>(A(0), p, j0.y);
-    const A x2 = gatherA<COH>(A(0), p, j0.z), x3 = gatherA<COH>(A(0), p, j0.w);
-    const A x4 = gatherA<COH>(A(0), p, j1.x), x5 = gatherA<COH>(A(0), p, j1.y);
-    const A x6 = gatherA<COH>(A(0), p, j1.z), x7 = gatherA<COH>(A(0), p, j1.w);
+    int j0[4], j1[4];
+    cs.dq(r0, 4 * cq, j0);
+    cs.dq(r1, 4 * cq + 4, j1);
+    const A x0 = gatherA<COH>(A(0), p, j0[0]), x1 = gatherA<COH>(A(0), p, j0[1]);
+    const A x2 = gatherA<COH>(A(0), p, j0[2]), x3 = gatherA<COH>(A(0), p, j0[3]);
+    const A x4 = gatherA<COH>(A(0), p, j1[0]), x5 = gatherA<COH>(A(0), p, j1[1]);
+    const A x6 = gatherA<COH>(A(0), p, j1[2]), x7 = gatherA<COH>(A(0), p, j1[3]);
     acc = fma(v0[0], x0, acc); acc = fma(v0[1], x1, acc); acc = fma(v0[2], x2, acc); acc = fma(v0[3], x3, acc);
     acc = fma(v1[0], x4, acc); acc = fma(v1[1], x5, acc); acc = fma(v1[2], x6, acc); acc = fma(v1[3], x7, acc);
   }
-  // remainder: at most one quad, one pair, one single; all loads first, then all gathers
+  // remainder: at most one quad, one pair, one single
   const bool hq = cq < a, hp = (w & 2) != 0, hs = (w & 1) != 0;
-  const int tail = a * 128;
-  int4 jq = make_int4(0, 0, 0, 0);
-  int2 jp = make_int2(0, 0);
-  int js = 0;
-  A vq[4] = {A(0), A(0), A(0), A(0)}, vpair[2] = {A(0), A(0)}, vs = A(0);
-  if (hq) { jq = lds_i4(cp + cq * 128 + lane * 4); lds_quad(vp + cq * 128 + lane * LQ, vq); }
-  if (hp) { jp = lds_i2(cp + tail + lane * 2); lds_pair(vp + tail + lane * 2, vpair); }
-  if (hs) { js = lds_i1(cp + tail + (hp ? 64 : 0) + lane); vs = lds_one(vp + tail + (hp ? 64 : 0) + lane); }
-  A xq0 = 0, xq1 = 0, xq2 = 0, xq3 = 0, xp0 = 0, xp1 = 0, xs = 0;
-  if (hq) { xq0 = gatherA<COH>(A(0), p, jq.x); xq1 = gatherA<COH>(A(0), p, jq.y);
-            xq2 = gatherA<COH>(A(0), p, jq.z); xq3 = gatherA<COH>(A(0), p, jq.w); }
-  if (hp) { xp0 = gatherA<COH>(A(0), p, jp.x); xp1 = gatherA<COH>(A(0), p, jp.y); }
-  if (hs) xs = gatherA<COH>(A(0), p, js);
-  if (hq) { acc = fma(vq[0], xq0, acc); acc = fma(vq[1], xq1, acc); acc = fma(vq[2], xq2, acc); acc = fma(vq[3], xq3, acc); }
-  if (hp) { acc = fma(vpair[0], xp0, acc); acc = fma(vpair[1], xp1, acc); }
-  if (hs) acc = fma(vs, xs, acc);
+  const int tail = a * 128, tail1 = tail + (hp ? 64 : 0);
+  if (hq) {
+    cs.refresh(4 * cq, lane);
+    const typename CS::RawQ r = cs.quad(cq * 128, lane);
+    A v[4];
+    lds_quad(vp + cq * 128 + lane * LQ, v);
+    int j[4];
+    cs.dq(r, 4 * cq, j);
+    const A x0 = gatherA<COH>(A(0), p, j[0]), x1 = gatherA<COH>(A(0), p, j[1]);
+    const A x2 = gatherA<COH>(A(0), p, j[2]), x3 = gatherA<COH>(A(0), p, j[3]);
+    acc = fma(v[0], x0, acc); acc = fma(v[1], x1, acc); acc = fma(v[2], x2, acc); acc = fma(v[3], x3, acc);
+  }
+  if (hp) {
+    cs.refresh(4 * a, lane);
+    const typename CS::RawP r = cs.pair(tail, lane);
+    A v[2];
+    lds_pair(vp + tail + lane * 2, v);
+    int j[2];
+    cs.dp(r, 4 * a, j);
+    const A x0 = gatherA<COH>(A(0), p, j[0]), x1 = gatherA<COH>(A(0), p, j[1]);
+    acc = fma(v[0], x0, acc); acc = fma(v[1], x1, acc);
+  }
+  if (hs) {
+    cs.refresh(w - 1, lane);
+    const typename CS::RawS r = cs.single(tail1, lane);
+    const A v = lds_one(vp + tail1 + lane);
+    acc = fma(v, gatherA<COH>(A(0), p, cs.ds(r, w - 1)), acc);
+  }
   return acc;
 }
 
 // G consecutive narrow slices (every width <= 7: one quad, one pair, one single at most) at once.
-// Branch-free: absent parts keep column 0 and value 0, so all matrix loads of the group are issued
+// Branch-free: absent parts keep offset 0 and value 0, so all matrix loads of the group are issued
 // (predicated) before the first gather and all 7 G gathers before the first fma — a warp keeps G times
 // the bytes of one short-row slice in flight and waits for memory three times per group, not per part.
-template <int UR, bool COH, int G, class PT>
-__device__ __forceinline__ void narrow_group_sum(const PT* p, const int32_t* cols, const typename SpmvT<UR>::A* vals,
-                                                 const int (&wp)[G + 1], int lane, typename SpmvT<UR>::A (&acc)[G]) {
+template <int UR, bool COH, bool I16, int G, class PT>
+__device__ __forceinline__ void narrow_group_sum(const Ctx& c, const PT* p, const int (&wp)[G + 1], int lane,
+                                                 typename SpmvT<UR>::A (&acc)[G]) {
   using A = typename SpmvT<UR>::A;
+  using CS = ColSrc<I16>;
   constexpr int LQ = LaneQ<A>::v;
-  int j[G][7];
+  const A* vals = sell_vals<UR>(c);
+  typename CS::RawQ rq[G];
+  typename CS::RawP rp[G];
+  typename CS::RawS rs[G];
+  int bl[G];
   A v[G][7];
 #pragma unroll
   for (int g = 0; g < G; ++g) {
     const int w = wp[g + 1] - wp[g];
-    const int32_t* cp = cols + (int64_t)wp[g] * 32;
+    CS cs(c, wp[g], w, lane);
+    if constexpr (I16) bl[g] = cs.bl; else bl[g] = 0;
     const A* vp = vals + (int64_t)wp[g] * 32;
     const bool hq = (w & 4) != 0, hp = (w & 2) != 0, hs = (w & 1) != 0;
     const int tail = hq ? 128 : 0, tail1 = tail + (hp ? 64 : 0);
-    int4 jq = make_int4(0, 0, 0, 0);
-    int2 jp = make_int2(0, 0);
-    int js = 0;
+    rq[g] = CS::zq(); rp[g] = CS::zp(); rs[g] = 0;
     A vq[4] = {A(0), A(0), A(0), A(0)}, vpair[2] = {A(0), A(0)}, vs = A(0);
-    if (hq) { jq = lds_i4(cp + lane * 4); lds_quad(vp + lane * LQ, vq); }
-    if (hp) { jp = lds_i2(cp + tail + lane * 2); lds_pair(vp + tail + lane * 2, vpair); }
-    if (hs) { js = lds_i1(cp + tail1 + lane); vs = lds_one(vp + tail1 + lane); }
-    j[g][0] = jq.x; j[g][1] = jq.y; j[g][2] = jq.z; j[g][3] = jq.w; j[g][4] = jp.x; j[g][5] = jp.y; j[g][6] = js;
+    if (hq) { rq[g] = cs.quad(0, lane); lds_quad(vp + lane * LQ, vq); }
+    if (hp) { rp[g] = cs.pair(tail, lane); lds_pair(vp + tail + lane * 2, vpair); }
+    if (hs) { rs[g] = cs.single(tail1, lane); vs = lds_one(vp + tail1 + lane); }
     v[g][0] = vq[0]; v[g][1] = vq[1]; v[g][2] = vq[2]; v[g][3] = vq[3]; v[g][4] = vpair[0]; v[g][5] = vpair[1]; v[g][6] = vs;
   }
   A x[G][7];
 #pragma unroll
   for (int g = 0; g < G; ++g) {
+    const int w = wp[g + 1] - wp[g];
+    CS cs(c, wp[g], 0, 32);  // addressing only; the bases were loaded above
+    if constexpr (I16) cs.bl = bl[g];
+    const int kp = w & 4, ks = kp + (w & 2);  // entry index of the pair and of the single
+    int jq[4], jp[2];
+    cs.dq(rq[g], 0, jq);
+    cs.dp(rp[g], kp, jp);
+    const int js = cs.ds(rs[g], ks);
 #pragma unroll
-    for (int u = 0; u < 7; ++u) x[g][u] = gatherA<COH>(A(0), p, j[g][u]);
+    for (int u = 0; u < 4; ++u) x[g][u] = gatherA<COH>(A(0), p, jq[u]);
+    x[g][4] = gatherA<COH>(A(0), p, jp[0]);
+    x[g][5] = gatherA<COH>(A(0), p, jp[1]);
+    x[g][6] = gatherA<COH>(A(0), p, js);
   }
 #pragma unroll
   for (int g = 0; g < G; ++g) {
@@ -192,15 +276,13 @@ constexpr int kSpmvGroupMax = AMP_SPMV_G32 > AMP_SPMV_G64 ? AMP_SPMV_G32 : AMP_S
 // (persistent) kernel, so it is gathered with plain coherent loads instead of the read-only path.
 // NT = threads per block.
 // Returns this thread's part of gamma = sum_i p_i q_i (stored q_i, FP64 products and sums).
-template <int UR, bool COH, int NT, class PT>
-__device__ __forceinline__ double phase_spmv(const Ctx& c, const PT* p, typename Store<UR>::T* q, int bid, int nb,
-                                             double* red) {
+template <int UR, bool COH, bool I16, int NT, class PT>
+__device__ __forceinline__ double phase_spmv_fmt(const Ctx& c, const PT* p, typename Store<UR>::T* q, int bid, int nb,
+                                                 double* red) {
   using A = typename SpmvT<UR>::A;
   constexpr int G = SpmvGroup<UR>::G;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   constexpr int wpb = NT / 32;
-  const int32_t* __restrict__ cols = c.sell_cols;
-  const A* __restrict__ vals = sell_vals<UR>(c);
   const int32_t* __restrict__ wptr = c.sell_wptr;
   const int nslices = c.nslices;
   const int n = (int)c.n;
@@ -217,11 +299,11 @@ __device__ __forceinline__ double phase_spmv(const Ctx& c, const PT* p, typename
     for (int g = 0; g < G; ++g) wmax = max(wmax, wp[g + 1] - wp[g]);
     A acc[G];
     if (wmax <= 7) {
-      narrow_group_sum<UR, COH, G>(p, cols, vals, wp, lane, acc);
+      narrow_group_sum<UR, COH, I16, G>(c, p, wp, lane, acc);
     } else {
 #pragma unroll
       for (int g = 0; g < G; ++g)
-        acc[g] = slice_sum<UR, COH>(p, cols + (int64_t)wp[g] * 32, vals + (int64_t)wp[g] * 32, wp[g + 1] - wp[g], lane);
+        acc[g] = slice_sum<UR, COH, I16>(c, p, wp[g], wp[g + 1] - wp[g], lane);
     }
 #pragma unroll
     for (int g = 0; g < G; ++g) {
@@ -253,12 +335,22 @@ __device__ __forceinline__ double phase_spmv(const Ctx& c, const PT* p, typename
   return gsum;
 }
 
+template <int UR, bool COH, int NT, class PT>
+__device__ __forceinline__ double phase_spmv(const Ctx& c, const PT* p, typename Store<UR>::T* q, int bid, int nb,
+                                             double* red) {
+  if (c.sell_cols16 != nullptr) return phase_spmv_fmt<UR, COH, true, NT>(c, p, q, bid, nb, red);
+  return phase_spmv_fmt<UR, COH, false, NT>(c, p, q, bid, nb, red);
+}
+
 // ------------------------------------------------------------------ create(): CSR -> SELL-32 --
-// one warp per slice; lane = row slot.  Long rows and padding slots get length 0.
+// one warp per slice; lane = row slot.  Long rows and padding slots get length 0.  Padding entries
+// take the smallest real column of their entry index k (the base of the 16-bit format) and value 0.
+// flag16 is set when some offset from the base does not fit 16 bits.
 __global__ void k_sell_pack(int n, int nslices, int long_min, const int32_t* __restrict__ rowptr,
                             const int32_t* __restrict__ colidx, const double* __restrict__ vals,
                             const int32_t* __restrict__ wptr, const int32_t* __restrict__ perm, int32_t* __restrict__ cols,
-                            double* __restrict__ v64, float* __restrict__ v32) {
+                            uint16_t* __restrict__ cols16, int32_t* __restrict__ bases, double* __restrict__ v64,
+                            float* __restrict__ v32, int* __restrict__ flag16) {
   const int lane = threadIdx.x & 31;
   const int s = (int)(((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5);
   if (s >= nslices) return;
@@ -272,15 +364,27 @@ __global__ void k_sell_pack(int n, int nslices, int long_min, const int32_t* __r
     len = rowptr[row + 1] - e0;
     if (len > long_min) len = 0;
   }
-  const int self = (row >= 0 && row < n) ? row : 0;
+  bool wide = false;
   for (int k = 0; k < w; ++k) {
     const bool ok = k < len;
-    const int j = ok ? colidx[e0 + k] : self;
+    int j = ok ? colidx[e0 + k] : 0x7fffffff;
+    int mn = j, mx = ok ? j : -1;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      mn = min(mn, __shfl_xor_sync(0xffffffffu, mn, o));
+      mx = max(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+    }
+    if (!ok) j = mn;
+    if (mx - mn > 65535) wide = true;
     const double v = ok ? vals[e0 + k] : 0.0;
-    cols[base + sell_pos32(k, lane, w)] = j;
-    v32[base + sell_pos32(k, lane, w)] = __double2float_rn(v);
+    const int64_t p32 = base + sell_pos32(k, lane, w);
+    cols[p32] = j;
+    cols16[p32] = (uint16_t)min(j - mn, 65535);
+    v32[p32] = __double2float_rn(v);
     v64[base + sell_pos64(k, lane, w)] = v;
+    if (lane == 0) bases[w0 + k] = mn;
   }
+  if (wide && lane == 0) atomicOr(flag16, 1);
 }
 
 }  // namespace amp
