@@ -30,6 +30,11 @@ SMI_QUERY = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.acti
              "clocks_event_reasons.sw_power_cap")
 
 
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the SpMV kernel from the committed ncu --set full
+# captures (profiles/r01c_*.md name the commands); None where no capture exists for that workload
+NCU_TRAFFIC = {}
+
+
 def parse_args():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -260,12 +265,18 @@ def run_ours(args, rank: int, local_rank: int, world: int):
             h.spmv(pvec, matp, out=q)
         e1.record(stream); e1.synchronize()
         dur_ms = e0.elapsed_time(e1) / reps
-        alg_bytes = s.n * (m * (sA + 4) + 4 + sz + sA)  # values+indices, rowptr, p once, q once
+        # bytes this handle's matrix format must move per launch (amp_pcg_spmv_bytes):
+        # stored values + the index data actually read + p once + q once
+        alg_bytes = h.spmv_bytes(matp, A.FP16 if pt == torch.float16 else A.FP64)
+        csr_bytes = s.n * (m * (sA + 4) + 4 + sz + sA)  # the same mat-vec in plain CSR
         roof[tag] = {"bound": "hbm", "achieved": alg_bytes / dur_ms * 1e-6, "peak": peak, "unit": "GB/s",
-                     "frac": alg_bytes / dur_ms * 1e-6 / peak, "traffic": None, "kernel": "k_spmv_any (phase_spmv)",
-                     "us_per_launch": dur_ms * 1e3, "algorithmic_bytes_per_launch": alg_bytes, "peak_source": peak_src}
+                     "frac": alg_bytes / dur_ms * 1e-6 / peak, "traffic": NCU_TRAFFIC.get((s.name.split("@")[0], tag)),
+                     "kernel": "k_spmv_any (phase_spmv)",
+                     "us_per_launch": dur_ms * 1e3, "algorithmic_bytes_per_launch": alg_bytes, "peak_source": peak_src,
+                     "csr_equivalent_bytes_per_launch": csr_bytes, "csr_equivalent_gbs": csr_bytes / dur_ms * 1e-6}
     roofline = dict(roof["fp32mat_fp16vec"])
-    roofline["fp64"] = {k: roof["fp64mat_fp64vec"][k] for k in ("achieved", "frac", "us_per_launch", "algorithmic_bytes_per_launch")}
+    roofline["fp64"] = {k: roof["fp64mat_fp64vec"][k] for k in ("achieved", "frac", "us_per_launch", "algorithmic_bytes_per_launch",
+                                                                "traffic", "csr_equivalent_gbs")}
     loop_gbs = st.algorithmic_bytes / (statistics.median(ms) * 1e-3) * 1e-9
     loop64_gbs = st64.algorithmic_bytes / (statistics.median(ms64) * 1e-3) * 1e-9
     roofline["whole_loop"] = {"amp_gbs": loop_gbs, "amp_frac": loop_gbs / peak, "amp_frac_of_8TBs": loop_gbs / 8000.0,

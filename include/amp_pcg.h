@@ -100,8 +100,8 @@ typedef struct {
   double relres_updated;    /* ||r_m|| / ||b|| of the recursively updated residual */
   double relres_true;       /* ||b - A x_m|| / ||b|| in FP64 if policy.true_residual, else -1 */
   double solve_ms;          /* device time of setup + loop (CUDA events on the solve stream) */
-  double algorithmic_bytes; /* compulsory bytes moved by the loop: sum over iterations of the per-row byte
-                               model of DESIGN.md section 5 for the precisions in use at each iteration */
+  double algorithmic_bytes; /* compulsory bytes moved by the loop: sum over iterations of
+                               amp_pcg_iteration_bytes() for the precisions in use at each iteration */
   uint64_t fp16_subnormal;  /* FP16 stores of z,p that were subnormal / flushed to 0 / overflowed; */
   uint64_t fp16_flushed;    /* filled only when the library is built with -DAMP_COUNT_FP16, else 0 */
   uint64_t fp16_inf;
@@ -118,9 +118,11 @@ void amp_policy_default(amp_policy_t *p);
  *   vals        float64[nnz]
  *   precond     AMP_PRECOND_NONE (M = I) or AMP_PRECOND_JACOBI (M = diag(A); every row needs a
  *               stored, positive diagonal entry)
- * rowptr/colidx/vals are BORROWED: they must stay valid and unchanged until amp_pcg_destroy().
- * The handle owns everything derived (FP32 value copy, 1/diag in FP64 and FP32, row tiles,
- * work vectors in FP64/FP32/FP16, device state, captured graph).  Symmetry is not verified.
+ * rowptr/colidx/vals are BORROWED: they must stay valid and unchanged until amp_pcg_destroy()
+ * (rows longer than max(256, 8 nnz/n) entries are read from them by every mat-vec).
+ * The handle owns everything derived (SELL-32 repack of A: indices, FP64 values and the FP32 value
+ * copy; 1/diag in FP64 and FP32; work vectors in FP64/FP32/FP16; device state; captured graph).
+ * Symmetry is not verified.
  * Returns NULL on failure; amp_pcg_last_error() says why (invalid structure, CUDA, memory). */
 amp_pcg_t *amp_pcg_create(int64_t n, int64_t nnz, const int32_t *rowptr, const int32_t *colidx,
                           const double *vals, int precond);
@@ -165,9 +167,23 @@ void amp_pcg_destroy(amp_pcg_t *h);
 /* Thread-local message of the last failure in this library ("" if none). */
 const char *amp_pcg_last_error(void);
 
-/* Per-row algorithmic bytes of one iteration for m = nnz/n and the given (u_z, u_r): the byte
- * model of DESIGN.md section 5 (4-pass accounting, every vector read/written once per pass). */
+/* Per-row bytes of one iteration for m = nnz/n and the given (u_z, u_r) in the paper-style CSR
+ * reference accounting (Table 2 :524-537 for the vector kernels; CSR values + 4-byte
+ * column index + 4-byte row pointer for the mat-vec; every vector read/written once per pass).
+ * A format-independent yardstick; what THIS library moves is amp_pcg_iteration_bytes(). */
 double amp_pcg_bytes_per_row(double m, int uz, int ur);
+
+/* Compulsory bytes ONE mat-vec q = A p of this handle moves with the matrix format it built
+ * (SELL-32 repack): stored values (zero padding included) in mat_prec, the index
+ * data actually read (slice table, per-entry 32- or 16-bit columns of general slices, 4 bytes per
+ * 32 entries for diagonal-aligned slices, row order if rows were sorted), p read once in vec_prec,
+ * q written once in mat_prec.  The roofline numerator of bench.py for the SpMV kernel. */
+double amp_pcg_spmv_bytes(const amp_pcg_t *h, int mat_prec, int vec_prec);
+
+/* Compulsory bytes of one whole iteration in phase (u_z, u_r): amp_pcg_spmv_bytes(h, u_r, u_z) plus
+ * the three vector kernels (z: r, 1/diag -> z; p: z, p -> p; x/r: x, p, q, r -> x, r).
+ * amp_stats_t.algorithmic_bytes is the sum of this over the iterations of a solve. */
+double amp_pcg_iteration_bytes(const amp_pcg_t *h, int uz, int ur);
 
 #ifdef __cplusplus
 }

@@ -21,7 +21,7 @@ PRECOND_NONE, PRECOND_JACOBI = 0, 1
 EXPORTED_SYMBOLS = (
     "amp_policy_default", "amp_pcg_create", "amp_pcg_solve", "amp_pcg_solve_host", "amp_spmv",
     "amp_pcg_residual_history", "amp_pcg_set_stream", "amp_pcg_last_launch_count", "amp_pcg_destroy",
-    "amp_pcg_last_error", "amp_pcg_bytes_per_row",
+    "amp_pcg_last_error", "amp_pcg_bytes_per_row", "amp_pcg_spmv_bytes", "amp_pcg_iteration_bytes",
 )
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
@@ -108,6 +108,10 @@ def load_library():
     L.amp_pcg_last_error.argtypes = []
     L.amp_pcg_bytes_per_row.restype = dbl
     L.amp_pcg_bytes_per_row.argtypes = [dbl, C.c_int, C.c_int]
+    L.amp_pcg_spmv_bytes.restype = dbl
+    L.amp_pcg_spmv_bytes.argtypes = [vp, C.c_int, C.c_int]
+    L.amp_pcg_iteration_bytes.restype = dbl
+    L.amp_pcg_iteration_bytes.argtypes = [vp, C.c_int, C.c_int]
     _lib = L
     return L
 
@@ -213,6 +217,14 @@ class AmpPcg:
 
     def last_launch_count(self) -> int:
         return int(load_library().amp_pcg_last_launch_count(self._h))
+
+    def spmv_bytes(self, mat_prec: int, vec_prec: int) -> float:
+        """amp_pcg_spmv_bytes: compulsory bytes of one mat-vec with the matrix format this handle built."""
+        return float(load_library().amp_pcg_spmv_bytes(self._h, int(mat_prec), int(vec_prec)))
+
+    def iteration_bytes(self, uz: int, ur: int) -> float:
+        """amp_pcg_iteration_bytes: compulsory bytes of one iteration in phase (u_z, u_r)."""
+        return float(load_library().amp_pcg_iteration_bytes(self._h, int(uz), int(ur)))
 
     def close(self):
         if getattr(self, "_h", None):

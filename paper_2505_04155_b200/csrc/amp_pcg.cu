@@ -59,7 +59,8 @@ struct amp_pcg {
   int64_t launches = 0;
   int32_t last_iters = -1;
   double m_avg = 0.0;
-  double idx_bytes = 4.0;     // column-index bytes per stored entry of the format in use
+  double idx_bytes_total = 0.0;  // bytes of index data one SpMV reads (slice table, bases, per-entry indices, row order)
+  double long_bytes_idx = 0.0, long_entries = 0.0;  // long rows, read from the CSR arrays (4 B index per entry)
   int64_t sell_entries = 0;   // stored entries of the SELL-32 repack (padding included)
 };
 
@@ -96,6 +97,22 @@ extern "C" double amp_pcg_bytes_per_row(double m, int uz, int ur) {
   const double k_p = 3.0 * sz;                             // z, p -> p
   const double k_xr = 16.0 + sz + sr + 2.0 * sr;           // x (r/w FP64), p, q, r (r/w)
   return k_spmv + k_z + k_p + k_xr;
+}
+
+static double vec_size(int prec) { return prec == AMP_FP64 ? 8.0 : (prec == AMP_FP32 ? 4.0 : 2.0); }
+
+extern "C" double amp_pcg_spmv_bytes(const amp_pcg_t* h, int mat_prec, int vec_prec) {
+  if (!h) return 0.0;
+  const double sA = (mat_prec == AMP_FP64) ? 8.0 : 4.0;
+  return (double)h->sell_entries * sA + h->idx_bytes_total + h->long_bytes_idx + h->long_entries * sA +
+         (double)h->n * (vec_size(vec_prec) + sA);  // p read once, q written once
+}
+
+extern "C" double amp_pcg_iteration_bytes(const amp_pcg_t* h, int uz, int ur) {
+  if (!h) return 0.0;
+  const double sr = (ur == AMP_FP64) ? 8.0 : 4.0, sz = vec_size(uz), sd = (uz == AMP_FP64) ? 8.0 : 4.0;
+  const double k_z = sr + sd + sz, k_p = 3.0 * sz, k_xr = 16.0 + sz + 3.0 * sr;
+  return amp_pcg_spmv_bytes(h, ur, uz) + (double)h->n * (k_z + k_p + k_xr);
 }
 
 extern "C" void amp_pcg_destroy(amp_pcg_t* h) {
@@ -227,7 +244,7 @@ extern "C" amp_pcg_t* amp_pcg_create(int64_t n, int64_t nnz, const int32_t* rowp
     int64_t wsum = build_widths();
     if ((double)wsum * 32.0 > 1.03 * (double)nnz_sell + 4096.0) {
       // row lengths vary: sort rows by length (descending, stable) inside windows of kSortWindow rows
-      const int64_t kSortWindow = 4096;
+      const int64_t kSortWindow = 1024;
       perm.assign((size_t)nsl * 32, -1);
       for (int64_t r = 0; r < n; ++r) perm[(size_t)r] = (int32_t)r;
       for (int64_t w0 = 0; w0 < n; w0 += kSortWindow) {
@@ -237,27 +254,12 @@ extern "C" amp_pcg_t* amp_pcg_create(int64_t n, int64_t nnz, const int32_t* rowp
       }
       wsum = build_widths();
     }
-    if (wsum * 32 + 256 > (int64_t)0x7fffffff) {
-      set_error("amp_pcg_create: padded SELL-32 storage exceeds 2^31 entries");
-      amp_pcg_destroy(h);
-      return nullptr;
-    }
-    const size_t total = (size_t)wsum * 32 + 256;
-    int32_t *wptr_d, *cols_d, *perm_d = nullptr, *long_d, *base_d;
-    uint16_t* cols16_d;
-    int* flag16_d;
-    double* v64_d; float* v32_d;
+    // pass 1 on the device: final width of every slice and whether it is stored diagonal-aligned
+    int32_t *wptr_d, *cols_d, *perm_d = nullptr, *long_d, *base_d, *width_d;
     ALLOC(wptr_d, int32_t, wptr.size());
-    ALLOC(cols_d, int32_t, total);
-    ALLOC(cols16_d, uint16_t, total);
-    ALLOC(base_d, int32_t, (size_t)wsum + 64);
-    ALLOC(flag16_d, int, 1);
-    ALLOC(v64_d, double, total);
-    ALLOC(v32_d, float, total);
+    ALLOC(width_d, int32_t, (size_t)nsl + 1);
     ALLOC(long_d, int32_t, long_rows.size() + 1);
     if (!perm.empty()) ALLOC(perm_d, int32_t, perm.size());
-    CU_TRY(cudaMemcpyAsync(wptr_d, wptr.data(), sizeof(int32_t) * wptr.size(), cudaMemcpyHostToDevice, h->stream),
-           { amp_pcg_destroy(h); return nullptr; });
     if (!long_rows.empty())
       CU_TRY(cudaMemcpyAsync(long_d, long_rows.data(), sizeof(int32_t) * long_rows.size(), cudaMemcpyHostToDevice, h->stream),
              { amp_pcg_destroy(h); return nullptr; });
@@ -265,6 +267,41 @@ extern "C" amp_pcg_t* amp_pcg_create(int64_t n, int64_t nnz, const int32_t* rowp
       CU_TRY(cudaMemcpyAsync(perm_d, perm.data(), sizeof(int32_t) * perm.size(), cudaMemcpyHostToDevice, h->stream),
              { amp_pcg_destroy(h); return nullptr; });
     const int pgrid = (int)((nsl * 32 + 255) / 256);
+    const int allow_aligned = getenv("AMP_SPMV_NO_ALIGN") ? 0 : 1;  // tuning aid
+    k_sell_scan<<<pgrid, 256, 0, h->stream>>>((int)n, (int)nsl, long_min, allow_aligned, rowptr, colidx, perm_d, width_d);
+    std::vector<int32_t> width((size_t)nsl);
+    CU_TRY(cudaMemcpyAsync(width.data(), width_d, sizeof(int32_t) * (size_t)nsl, cudaMemcpyDeviceToHost, h->stream),
+           { amp_pcg_destroy(h); return nullptr; });
+    CU_TRY(cudaStreamSynchronize(h->stream), { amp_pcg_destroy(h); return nullptr; });
+    CU_TRY(cudaGetLastError(), { amp_pcg_destroy(h); return nullptr; });
+    wsum = 0;
+    int64_t w_aligned = 0;
+    for (int64_t sl = 0; sl < nsl; ++sl) {
+      const int32_t wv = width[(size_t)sl];
+      const int32_t w = wv & 0x7fffffff;
+      wptr[(size_t)sl] = (int32_t)wsum | (wv & (int32_t)0x80000000u);
+      wsum += w;
+      if (wv < 0) w_aligned += w;
+      if (wsum * 32 + 256 > (int64_t)0x7fffffff) break;
+    }
+    wptr[(size_t)nsl] = (int32_t)wsum;
+    if (wsum * 32 + 256 > (int64_t)0x7fffffff) {
+      set_error("amp_pcg_create: padded SELL-32 storage exceeds 2^31 entries");
+      amp_pcg_destroy(h);
+      return nullptr;
+    }
+    const size_t total = (size_t)wsum * 32 + 256;
+    uint16_t* cols16_d;
+    int* flag16_d;
+    double* v64_d; float* v32_d;
+    ALLOC(cols_d, int32_t, total);
+    ALLOC(cols16_d, uint16_t, total);
+    ALLOC(base_d, int32_t, (size_t)wsum + 64);
+    ALLOC(flag16_d, int, 1);
+    ALLOC(v64_d, double, total);
+    ALLOC(v32_d, float, total);
+    CU_TRY(cudaMemcpyAsync(wptr_d, wptr.data(), sizeof(int32_t) * wptr.size(), cudaMemcpyHostToDevice, h->stream),
+           { amp_pcg_destroy(h); return nullptr; });
     k_sell_pack<<<pgrid, 256, 0, h->stream>>>((int)n, (int)nsl, long_min, rowptr, colidx, vals, wptr_d, perm_d, cols_d,
                                              cols16_d, base_d, v64_d, v32_d, flag16_d);
     int wide = 0;
@@ -276,22 +313,27 @@ extern "C" amp_pcg_t* amp_pcg_create(int64_t n, int64_t nnz, const int32_t* rowp
       cudaFree(ptr);
       h->owned.erase(std::find(h->owned.begin(), h->owned.end(), ptr));
     };
+    release(width_d);
     if (wide) {  // some offset needs more than 16 bits: keep the 32-bit indices
-      release(cols16_d); release(base_d);
-      cols16_d = nullptr; base_d = nullptr;
+      release(cols16_d);
+      cols16_d = nullptr;
     } else {
       release(cols_d);
       cols_d = nullptr;
     }
-    h->idx_bytes = wide ? 4.0 : 2.0 + 4.0 / 32.0;
+    // bytes of index data the SpMV reads: slice table + bases + per-entry indices of the general slices
+    h->idx_bytes_total = 4.0 * (double)(nsl + 1) + 4.0 * (double)wsum + (wide ? 4.0 : 2.0) * 32.0 * (double)(wsum - w_aligned) +
+                         (perm.empty() ? 0.0 : 4.0 * 32.0 * (double)nsl);
     c.sell_wptr = wptr_d; c.sell_cols = cols_d; c.sell_cols16 = cols16_d; c.sell_base = base_d;
     c.sell_vals64 = v64_d; c.sell_vals32 = v32_d; c.sell_perm = perm_d;
     c.long_rows = long_d; c.nslices = (int32_t)nsl; c.nlong = (int32_t)long_rows.size();
+    h->long_entries = (double)(nnz - nnz_sell);
+    h->long_bytes_idx = 4.0 * h->long_entries + 12.0 * (double)long_rows.size();
     h->sell_entries = wsum * 32;
 
     // SpMV grid: a warp takes a group of up to kSpmvGroupMax slices per pass; blocks make a whole number of
-    // (nearly) equal passes, at most `mult` blocks per SM (AMP_SPMV_GRID_MULT: tuning aid, default 16)
-    int mult = 16;
+    // (nearly) equal passes, at most `mult` blocks per SM (AMP_SPMV_GRID_MULT: tuning aid)
+    int mult = perm.empty() ? 8 : 55;  // sorted (irregular) matrices: small blocks even out the slice widths
     if (const char* e = getenv("AMP_SPMV_GRID_MULT")) mult = std::max(1, atoi(e));
     const int64_t max_grid = std::min<int64_t>((int64_t)h->num_sms * mult, kMaxGrid);
     const int64_t nblk = (nsl + kSpmvWarps * kSpmvGroupMax - 1) / (kSpmvWarps * kSpmvGroupMax);
@@ -498,9 +540,9 @@ static int solve_impl(amp_pcg* h, const double* b, double* x, double tol, int32_
       int uz = hs->amp ? hs->u0 : AMP_FP64;
       if (hs->it_uz32 >= 0 && k >= hs->it_uz32) uz = std::max(uz, (int)AMP_FP32);
       if (hs->it_uz16 >= 0 && k >= hs->it_uz16) uz = AMP_FP16;
-      bytes += amp_pcg_bytes_per_row(h->m_avg, uz, ur);
+      bytes += amp_pcg_iteration_bytes(h, uz, ur);
     }
-    stats->algorithmic_bytes = bytes * (double)h->n;
+    stats->algorithmic_bytes = bytes;
     stats->fp16_subnormal = hs->fp16_subnormal; stats->fp16_flushed = hs->fp16_flushed; stats->fp16_inf = hs->fp16_inf;
   }
   return hs->status;

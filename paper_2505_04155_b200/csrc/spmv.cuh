@@ -91,16 +91,22 @@ __device__ __forceinline__ float lds_one(const float* v) { return __ldcs(v); }
 __device__ __forceinline__ double lds_one(const double* v) { return __ldcs(v); }
 
 // ------------------------------------------------------------------ column index sources ----
-// I16 = false: 32-bit column indices.  I16 = true: 16-bit offsets from a per-(slice, entry) base
-// (the smallest column of entry k over the 32 rows of the slice, sell_base[w0 + k]); chosen in
-// create() when every offset fits, which holds for banded / stencil matrices.  The base of entry
-// k is held by lane k % 32 and broadcast by a shuffle, so the index stream is 2 B per entry plus
-// 4 B per 32 entries.
-template <bool I16> struct ColSrc;
-template <> struct ColSrc<false> {
+// CM = 0: 32-bit column indices.
+// CM = 1: 16-bit offsets from a per-(slice, entry) base (the smallest column of entry k over the 32
+//         rows of the slice, sell_base[w0 + k]); chosen for the whole matrix in create() when every
+//         offset fits, which holds for banded matrices: 2 B per entry + 4 B per 32 entries.
+// CM = 2: "aligned" slice (chosen per slice in create()): the entries of the 32 rows were placed so
+//         that entry k of every row lies on the same diagonal, col = row + sell_base[w0 + k]
+//         (rows that lack a diagonal hold an explicit zero there).  No per-entry index is read at
+//         all: 4 B per 32 entries.  Typical for stencil / structured-grid matrices.
+// The base of entry k is held by lane k % 32 and broadcast by a shuffle.
+constexpr int kAlignedFlag = (int)0x80000000u;  // bit 31 of sell_wptr[s]: slice s is aligned
+template <int CM> struct ColSrc;
+template <> struct ColSrc<0> {
   using RawQ = int4; using RawP = int2; using RawS = int;
   const int32_t* cp;
-  __device__ __forceinline__ ColSrc(const Ctx& c, int w0, int, int) : cp(c.sell_cols + (int64_t)w0 * 32) {}
+  __device__ __forceinline__ ColSrc() {}
+  __device__ __forceinline__ ColSrc(const Ctx& c, int w0, int, int, int) : cp(c.sell_cols + (int64_t)w0 * 32) {}
   __device__ __forceinline__ void refresh(int, int) {}
   __device__ __forceinline__ RawQ quad(int off, int lane) const { return lds_i4(cp + off + lane * 4); }
   __device__ __forceinline__ RawP pair(int off, int lane) const { return lds_i2(cp + off + lane * 2); }
@@ -111,13 +117,11 @@ template <> struct ColSrc<false> {
   static __device__ __forceinline__ RawQ zq() { return make_int4(0, 0, 0, 0); }
   static __device__ __forceinline__ RawP zp() { return make_int2(0, 0); }
 };
-template <> struct ColSrc<true> {
-  using RawQ = uint2; using RawP = uint32_t; using RawS = uint32_t;
-  const uint16_t* cp;
-  const int32_t* bp;  // bases of this slice
+struct ColBase {  // bases of the entries of one slice, 32 at a time, one per lane
+  const int32_t* bp;
   int w, blk, bl;
-  __device__ __forceinline__ ColSrc(const Ctx& c, int w0, int w_, int lane)
-      : cp(c.sell_cols16 + (int64_t)w0 * 32), bp(c.sell_base + w0), w(w_), blk(0) {
+  __device__ __forceinline__ void init(const Ctx& c, int w0, int w_, int lane) {
+    bp = c.sell_base + w0; w = w_; blk = 0;
     bl = (lane < w) ? __ldg(bp + lane) : 0;
   }
   // make the bases of entries [32*(k/32), +32) current (slices wider than 32 entries only)
@@ -127,10 +131,18 @@ template <> struct ColSrc<true> {
       bl = (blk * 32 + lane < w) ? __ldg(bp + blk * 32 + lane) : 0;
     }
   }
+  __device__ __forceinline__ int base(int k) const { return __shfl_sync(0xffffffffu, bl, k & 31); }
+};
+template <> struct ColSrc<1> : ColBase {
+  using RawQ = uint2; using RawP = uint32_t; using RawS = uint32_t;
+  const uint16_t* cp;
+  __device__ __forceinline__ ColSrc() {}
+  __device__ __forceinline__ ColSrc(const Ctx& c, int w0, int w_, int lane, int) : cp(c.sell_cols16 + (int64_t)w0 * 32) {
+    init(c, w0, w_, lane);
+  }
   __device__ __forceinline__ RawQ quad(int off, int lane) const { return __ldcs(reinterpret_cast<const uint2*>(cp + off + lane * 4)); }
   __device__ __forceinline__ RawP pair(int off, int lane) const { return __ldcs(reinterpret_cast<const uint32_t*>(cp + off + lane * 2)); }
   __device__ __forceinline__ RawS single(int off, int lane) const { return (uint32_t)__ldcs(cp + off + lane); }
-  __device__ __forceinline__ int base(int k) const { return __shfl_sync(0xffffffffu, bl, k & 31); }
   __device__ __forceinline__ void dq(RawQ r, int k, int (&j)[4]) const {
     j[0] = base(k) + (int)(r.x & 0xffffu); j[1] = base(k + 1) + (int)(r.x >> 16);
     j[2] = base(k + 2) + (int)(r.y & 0xffffu); j[3] = base(k + 3) + (int)(r.y >> 16);
@@ -142,63 +154,110 @@ template <> struct ColSrc<true> {
   static __device__ __forceinline__ RawQ zq() { return make_uint2(0u, 0u); }
   static __device__ __forceinline__ RawP zp() { return 0u; }
 };
+template <> struct ColSrc<2> : ColBase {
+  using RawQ = int; using RawP = int; using RawS = int;  // nothing is loaded per entry
+  int row, nm1;
+  __device__ __forceinline__ ColSrc() {}
+  __device__ __forceinline__ ColSrc(const Ctx& c, int w0, int w_, int lane, int row_) : row(row_ < 0 ? 0 : row_), nm1((int)c.n - 1) {
+    init(c, w0, w_, lane);
+  }
+  __device__ __forceinline__ RawQ quad(int, int) const { return 0; }
+  __device__ __forceinline__ RawP pair(int, int) const { return 0; }
+  __device__ __forceinline__ RawS single(int, int) const { return 0; }
+  // explicit zeros of rows that lack diagonal k may point outside [0, n): clamp (their value is 0)
+  __device__ __forceinline__ int col(int k) const { return min(max(row + base(k), 0), nm1); }
+  __device__ __forceinline__ void dq(RawQ, int k, int (&j)[4]) const { j[0] = col(k); j[1] = col(k + 1); j[2] = col(k + 2); j[3] = col(k + 3); }
+  __device__ __forceinline__ void dp(RawP, int k, int (&j)[2]) const { j[0] = col(k); j[1] = col(k + 1); }
+  __device__ __forceinline__ int ds(RawS, int k) const { return col(k); }
+  static __device__ __forceinline__ RawQ zq() { return 0; }
+  static __device__ __forceinline__ RawP zp() { return 0; }
+};
 
-// One slice of any width: this lane's row sum (one fma chain in CSR order).
-template <int UR, bool COH, bool I16, class PT>
-__device__ __forceinline__ typename SpmvT<UR>::A slice_sum(const Ctx& c, const PT* p, int w0, int w, int lane) {
+// One slice of any width: this lane's row sum (one fma chain in stored order = CSR order).
+// Full trips of QT quads (all wide loads and all 4 QT gathers of a trip issued before its first fma),
+// then ONE tail step for the remaining < QT quads, the pair and the single: branch-free, absent parts
+// keep value 0 and a valid column, so the tail also waits for memory once.
+template <class A> struct SpmvTrip;  // quads per trip
+template <> struct SpmvTrip<float> { static constexpr int QT = 4; };
+template <> struct SpmvTrip<double> { static constexpr int QT = 2; };
+
+template <int UR, bool COH, int CM, class PT>
+__device__ __forceinline__ typename SpmvT<UR>::A slice_sum(const Ctx& c, const PT* p, int w0, int w, int lane, int row) {
   using A = typename SpmvT<UR>::A;
-  using CS = ColSrc<I16>;
+  using CS = ColSrc<CM>;
   constexpr int LQ = LaneQ<A>::v;
-  CS cs(c, w0, w, lane);
+  constexpr int QT = SpmvTrip<A>::QT;
+  CS cs(c, w0, w, lane, row);
   const A* vp = sell_vals<UR>(c) + (int64_t)w0 * 32;
   const int a = w >> 2;
   A acc = 0;
   int cq = 0;
-  for (; cq + 2 <= a; cq += 2) {  // two quads per trip: 4 (FP32) / 6 (FP64) wide loads in flight
+  for (; cq + QT <= a; cq += QT) {
+    cs.refresh(4 * cq, lane);  // QT divides 8: a trip never straddles a block of 32 bases
+    typename CS::RawQ r[QT];
+    A v[QT][4];
+#pragma unroll
+    for (int t = 0; t < QT; ++t) {
+      r[t] = cs.quad((cq + t) * 128, lane);
+      lds_quad(vp + (cq + t) * 128 + lane * LQ, v[t]);
+    }
+    A x[QT][4];
+#pragma unroll
+    for (int t = 0; t < QT; ++t) {
+      int j[4];
+      cs.dq(r[t], 4 * (cq + t), j);
+#pragma unroll
+      for (int u = 0; u < 4; ++u) x[t][u] = gatherA<COH>(A(0), p, j[u]);
+    }
+#pragma unroll
+    for (int t = 0; t < QT; ++t) {
+#pragma unroll
+      for (int u = 0; u < 4; ++u) acc = fma(v[t][u], x[t][u], acc);
+    }
+  }
+  if (cq * 4 == w) return acc;
+  {  // tail: up to QT-1 quads, one pair, one single
     cs.refresh(4 * cq, lane);
-    const typename CS::RawQ r0 = cs.quad(cq * 128, lane), r1 = cs.quad((cq + 1) * 128, lane);
-    A v0[4], v1[4];
-    lds_quad(vp + cq * 128 + lane * LQ, v0);
-    lds_quad(vp + (cq + 1) * 128 + lane * LQ, v1);
-    int j0[4], j1[4];
-    cs.dq(r0, 4 * cq, j0);
-    cs.dq(r1, 4 * cq + 4, j1);
-    const A x0 = gatherA<COH>(A(0), p, j0[0]), x1 = gatherA<COH>(A(0), p, j0[1]);
-    const A x2 = gatherA<COH>(A(0), p, j0[2]), x3 = gatherA<COH>(A(0), p, j0[3]);
-    const A x4 = gatherA<COH>(A(0), p, j1[0]), x5 = gatherA<COH>(A(0), p, j1[1]);
-    const A x6 = gatherA<COH>(A(0), p, j1[2]), x7 = gatherA<COH>(A(0), p, j1[3]);
-    acc = fma(v0[0], x0, acc); acc = fma(v0[1], x1, acc); acc = fma(v0[2], x2, acc); acc = fma(v0[3], x3, acc);
-    acc = fma(v1[0], x4, acc); acc = fma(v1[1], x5, acc); acc = fma(v1[2], x6, acc); acc = fma(v1[3], x7, acc);
-  }
-  // remainder: at most one quad, one pair, one single
-  const bool hq = cq < a, hp = (w & 2) != 0, hs = (w & 1) != 0;
-  const int tail = a * 128, tail1 = tail + (hp ? 64 : 0);
-  if (hq) {
-    cs.refresh(4 * cq, lane);
-    const typename CS::RawQ r = cs.quad(cq * 128, lane);
-    A v[4];
-    lds_quad(vp + cq * 128 + lane * LQ, v);
-    int j[4];
-    cs.dq(r, 4 * cq, j);
-    const A x0 = gatherA<COH>(A(0), p, j[0]), x1 = gatherA<COH>(A(0), p, j[1]);
-    const A x2 = gatherA<COH>(A(0), p, j[2]), x3 = gatherA<COH>(A(0), p, j[3]);
-    acc = fma(v[0], x0, acc); acc = fma(v[1], x1, acc); acc = fma(v[2], x2, acc); acc = fma(v[3], x3, acc);
-  }
-  if (hp) {
-    cs.refresh(4 * a, lane);
-    const typename CS::RawP r = cs.pair(tail, lane);
-    A v[2];
-    lds_pair(vp + tail + lane * 2, v);
-    int j[2];
-    cs.dp(r, 4 * a, j);
-    const A x0 = gatherA<COH>(A(0), p, j[0]), x1 = gatherA<COH>(A(0), p, j[1]);
-    acc = fma(v[0], x0, acc); acc = fma(v[1], x1, acc);
-  }
-  if (hs) {
-    cs.refresh(w - 1, lane);
-    const typename CS::RawS r = cs.single(tail1, lane);
-    const A v = lds_one(vp + tail1 + lane);
-    acc = fma(v, gatherA<COH>(A(0), p, cs.ds(r, w - 1)), acc);
+    const int rem = a - cq;
+    const bool hp = (w & 2) != 0, hs = (w & 1) != 0;
+    const int tail = a * 128, tail1 = tail + (hp ? 64 : 0);
+    typename CS::RawQ rq[QT - 1];
+    typename CS::RawP rp = CS::zp();
+    typename CS::RawS rs = 0;
+    A vq[QT - 1][4], vpair[2] = {A(0), A(0)}, vs = A(0);
+#pragma unroll
+    for (int t = 0; t < QT - 1; ++t) {
+      rq[t] = CS::zq();
+      vq[t][0] = vq[t][1] = vq[t][2] = vq[t][3] = A(0);
+      if (t < rem) { rq[t] = cs.quad((cq + t) * 128, lane); lds_quad(vp + (cq + t) * 128 + lane * LQ, vq[t]); }
+    }
+    if (hp) { rp = cs.pair(tail, lane); lds_pair(vp + tail + lane * 2, vpair); }
+    if (hs) { rs = cs.single(tail1, lane); vs = lds_one(vp + tail1 + lane); }
+    // entries past the real ones decode with k clamped into this block of bases: a valid column
+    const int klast = w - 1;
+    A xq[QT - 1][4], xp[2], xs;
+#pragma unroll
+    for (int t = 0; t < QT - 1; ++t) {
+      int j[4];
+      cs.dq(rq[t], min(4 * (cq + t), klast & ~3), j);
+#pragma unroll
+      for (int u = 0; u < 4; ++u) xq[t][u] = gatherA<COH>(A(0), p, j[u]);
+    }
+    {
+      int j[2];
+      cs.dp(rp, min(4 * a, klast & ~1), j);
+      xp[0] = gatherA<COH>(A(0), p, j[0]);
+      xp[1] = gatherA<COH>(A(0), p, j[1]);
+      xs = gatherA<COH>(A(0), p, cs.ds(rs, klast));
+    }
+#pragma unroll
+    for (int t = 0; t < QT - 1; ++t) {
+#pragma unroll
+      for (int u = 0; u < 4; ++u) acc = fma(vq[t][u], xq[t][u], acc);
+    }
+    acc = fma(vpair[0], xp[0], acc);
+    acc = fma(vpair[1], xp[1], acc);
+    acc = fma(vs, xs, acc);
   }
   return acc;
 }
@@ -207,44 +266,41 @@ __device__ __forceinline__ typename SpmvT<UR>::A slice_sum(const Ctx& c, const P
 // Branch-free: absent parts keep offset 0 and value 0, so all matrix loads of the group are issued
 // (predicated) before the first gather and all 7 G gathers before the first fma — a warp keeps G times
 // the bytes of one short-row slice in flight and waits for memory three times per group, not per part.
-template <int UR, bool COH, bool I16, int G, class PT>
+template <int UR, bool COH, int CM, int G, class PT>
 __device__ __forceinline__ void narrow_group_sum(const Ctx& c, const PT* p, const int (&wp)[G + 1], int lane,
-                                                 typename SpmvT<UR>::A (&acc)[G]) {
+                                                 const int (&rows)[G], typename SpmvT<UR>::A (&acc)[G]) {
   using A = typename SpmvT<UR>::A;
-  using CS = ColSrc<I16>;
+  using CS = ColSrc<CM>;
   constexpr int LQ = LaneQ<A>::v;
   const A* vals = sell_vals<UR>(c);
+  CS cs[G];
   typename CS::RawQ rq[G];
   typename CS::RawP rp[G];
   typename CS::RawS rs[G];
-  int bl[G];
   A v[G][7];
 #pragma unroll
   for (int g = 0; g < G; ++g) {
     const int w = wp[g + 1] - wp[g];
-    CS cs(c, wp[g], w, lane);
-    if constexpr (I16) bl[g] = cs.bl; else bl[g] = 0;
+    cs[g] = CS(c, wp[g], w, lane, rows[g]);
     const A* vp = vals + (int64_t)wp[g] * 32;
     const bool hq = (w & 4) != 0, hp = (w & 2) != 0, hs = (w & 1) != 0;
     const int tail = hq ? 128 : 0, tail1 = tail + (hp ? 64 : 0);
     rq[g] = CS::zq(); rp[g] = CS::zp(); rs[g] = 0;
     A vq[4] = {A(0), A(0), A(0), A(0)}, vpair[2] = {A(0), A(0)}, vs = A(0);
-    if (hq) { rq[g] = cs.quad(0, lane); lds_quad(vp + lane * LQ, vq); }
-    if (hp) { rp[g] = cs.pair(tail, lane); lds_pair(vp + tail + lane * 2, vpair); }
-    if (hs) { rs[g] = cs.single(tail1, lane); vs = lds_one(vp + tail1 + lane); }
+    if (hq) { rq[g] = cs[g].quad(0, lane); lds_quad(vp + lane * LQ, vq); }
+    if (hp) { rp[g] = cs[g].pair(tail, lane); lds_pair(vp + tail + lane * 2, vpair); }
+    if (hs) { rs[g] = cs[g].single(tail1, lane); vs = lds_one(vp + tail1 + lane); }
     v[g][0] = vq[0]; v[g][1] = vq[1]; v[g][2] = vq[2]; v[g][3] = vq[3]; v[g][4] = vpair[0]; v[g][5] = vpair[1]; v[g][6] = vs;
   }
   A x[G][7];
 #pragma unroll
   for (int g = 0; g < G; ++g) {
     const int w = wp[g + 1] - wp[g];
-    CS cs(c, wp[g], 0, 32);  // addressing only; the bases were loaded above
-    if constexpr (I16) cs.bl = bl[g];
     const int kp = w & 4, ks = kp + (w & 2);  // entry index of the pair and of the single
     int jq[4], jp[2];
-    cs.dq(rq[g], 0, jq);
-    cs.dp(rp[g], kp, jp);
-    const int js = cs.ds(rs[g], ks);
+    cs[g].dq(rq[g], 0, jq);
+    cs[g].dp(rp[g], kp, jp);
+    const int js = cs[g].ds(rs[g], ks);
 #pragma unroll
     for (int u = 0; u < 4; ++u) x[g][u] = gatherA<COH>(A(0), p, jq[u]);
     x[g][4] = gatherA<COH>(A(0), p, jp[0]);
@@ -276,7 +332,7 @@ constexpr int kSpmvGroupMax = AMP_SPMV_G32 > AMP_SPMV_G64 ? AMP_SPMV_G32 : AMP_S
 // (persistent) kernel, so it is gathered with plain coherent loads instead of the read-only path.
 // NT = threads per block.
 // Returns this thread's part of gamma = sum_i p_i q_i (stored q_i, FP64 products and sums).
-template <int UR, bool COH, bool I16, int NT, class PT>
+template <int UR, bool COH, int CMG, int NT, class PT>
 __device__ __forceinline__ double phase_spmv_fmt(const Ctx& c, const PT* p, typename Store<UR>::T* q, int bid, int nb,
                                                  double* red) {
   using A = typename SpmvT<UR>::A;
@@ -289,31 +345,72 @@ __device__ __forceinline__ double phase_spmv_fmt(const Ctx& c, const PT* p, type
   const int ngroups = (nslices + G - 1) / G;
   double gsum = 0.0;
 
-  for (int gi = bid * wpb + warp; gi < ngroups; gi += nb * wpb) {
+  int gi = bid * wpb + warp;
+  int wnext[G + 1];
+#pragma unroll
+  for (int g = 0; g <= G; ++g) wnext[g] = (gi < ngroups) ? __ldg(wptr + min(gi * G + g, nslices)) : 0;
+  for (; gi < ngroups; gi += nb * wpb) {
     const int s0 = gi * G;
-    int wp[G + 1];
+    int wp[G + 1], rows[G];
     int wmax = 0;
+    bool all_al = true, any_al = false, al_g[G];
 #pragma unroll
-    for (int g = 0; g <= G; ++g) wp[g] = __ldg(wptr + min(s0 + g, nslices));
+    for (int g = 0; g <= G; ++g) wp[g] = wnext[g];
+    {  // slice table entries of this warp's next group: off the critical path of the next pass
+      const int gn = gi + nb * wpb;
+      if (gn < ngroups) {
 #pragma unroll
-    for (int g = 0; g < G; ++g) wmax = max(wmax, wp[g + 1] - wp[g]);
-    A acc[G];
-    if (wmax <= 7) {
-      narrow_group_sum<UR, COH, I16, G>(c, p, wp, lane, acc);
-    } else {
-#pragma unroll
-      for (int g = 0; g < G; ++g)
-        acc[g] = slice_sum<UR, COH, I16>(c, p, wp[g], wp[g + 1] - wp[g], lane);
+        for (int g = 0; g <= G; ++g) wnext[g] = __ldg(wptr + min(gn * G + g, nslices));
+      }
     }
 #pragma unroll
     for (int g = 0; g < G; ++g) {
-      if (s0 + g < nslices) {
-        int row = (s0 + g) * 32 + lane;
-        if (c.sell_perm != nullptr) row = __ldg(c.sell_perm + row);  // -1: padding slot
-        if (row >= 0 && row < n) {
-          q[row] = acc[g];
-          gsum = fma(gather64<COH>(p, row), (double)acc[g], gsum);
+      al_g[g] = wp[g] < 0;  // kAlignedFlag
+      all_al = all_al && al_g[g];
+      any_al = any_al || al_g[g];
+    }
+#pragma unroll
+    for (int g = 0; g <= G; ++g) wp[g] &= ~kAlignedFlag;
+    double pi[G];
+#pragma unroll
+    for (int g = 0; g < G; ++g) {
+      wmax = max(wmax, wp[g + 1] - wp[g]);
+      int row = (s0 + g) * 32 + lane;
+      if (s0 + g >= nslices) row = -1;
+      else if (c.sell_perm != nullptr) row = __ldg(c.sell_perm + row);  // -1: padding slot
+      if (row >= n) row = -1;
+      rows[g] = row;
+      pi[g] = gather64<COH>(p, row < 0 ? 0 : row);  // p_i for gamma, issued with the other gathers
+    }
+    A acc[G];
+    if (wmax <= 7 && all_al) {
+      narrow_group_sum<UR, COH, 2, G>(c, p, wp, lane, rows, acc);
+    } else if (wmax <= 7 && !any_al) {
+      if constexpr (G <= 2) {
+        narrow_group_sum<UR, COH, CMG, G>(c, p, wp, lane, rows, acc);
+      } else {  // per-entry indices need registers too: two slices at a time
+        static_assert(G % 2 == 0, "group size");
+#pragma unroll
+        for (int h = 0; h < G; h += 2) {
+          const int wp2[3] = {wp[h], wp[h + 1], wp[h + 2]};
+          const int rows2[2] = {rows[h], rows[h + 1]};
+          A acc2[2];
+          narrow_group_sum<UR, COH, CMG, 2>(c, p, wp2, lane, rows2, acc2);
+          acc[h] = acc2[0]; acc[h + 1] = acc2[1];
         }
+      }
+    } else {
+#pragma unroll
+      for (int g = 0; g < G; ++g) {
+        if (al_g[g]) acc[g] = slice_sum<UR, COH, 2>(c, p, wp[g], wp[g + 1] - wp[g], lane, rows[g]);
+        else acc[g] = slice_sum<UR, COH, CMG>(c, p, wp[g], wp[g + 1] - wp[g], lane, rows[g]);
+      }
+    }
+#pragma unroll
+    for (int g = 0; g < G; ++g) {
+      if (rows[g] >= 0) {
+        q[rows[g]] = acc[g];
+        gsum = fma(pi[g], (double)acc[g], gsum);
       }
     }
   }
@@ -338,14 +435,84 @@ __device__ __forceinline__ double phase_spmv_fmt(const Ctx& c, const PT* p, type
 template <int UR, bool COH, int NT, class PT>
 __device__ __forceinline__ double phase_spmv(const Ctx& c, const PT* p, typename Store<UR>::T* q, int bid, int nb,
                                              double* red) {
-  if (c.sell_cols16 != nullptr) return phase_spmv_fmt<UR, COH, true, NT>(c, p, q, bid, nb, red);
-  return phase_spmv_fmt<UR, COH, false, NT>(c, p, q, bid, nb, red);
+  if (c.sell_cols16 != nullptr) return phase_spmv_fmt<UR, COH, 1, NT>(c, p, q, bid, nb, red);
+  return phase_spmv_fmt<UR, COH, 0, NT>(c, p, q, bid, nb, red);
 }
 
 // ------------------------------------------------------------------ create(): CSR -> SELL-32 --
-// one warp per slice; lane = row slot.  Long rows and padding slots get length 0.  Padding entries
-// take the smallest real column of their entry index k (the base of the 16-bit format) and value 0.
-// flag16 is set when some offset from the base does not fit 16 bits.
+__device__ __forceinline__ int warp_min_i(int v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v = min(v, __shfl_xor_sync(0xffffffffu, v, o));
+  return v;
+}
+__device__ __forceinline__ int warp_max_i(int v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v = max(v, __shfl_xor_sync(0xffffffffu, v, o));
+  return v;
+}
+
+// Diagonal alignment of one slice (whole warp): the distinct offsets col - row of its 32 rows are
+// enumerated in increasing order; position k of every row holds its entry on the k-th diagonal or
+// an explicit zero.  place(k, offset, mine, e) is called for every position; returns the number of
+// positions, or -1 if some row is not strictly increasing in column or more than kcap diagonals
+// exist (the slice then keeps the general format).
+template <class F>
+__device__ __forceinline__ int sell_align(int row, int e0, int len, const int32_t* __restrict__ colidx, int kcap, F place) {
+  const int kInf = 0x7fffffff;
+  int ptr = 0, k = 0;
+  bool bad = false;
+  int cur = (ptr < len) ? colidx[e0 + ptr] - row : kInf;
+  while (true) {
+    const int m = warp_min_i(cur);
+    if (m == kInf) break;
+    if (k >= kcap) { bad = true; break; }
+    const bool mine = (cur == m);
+    place(k, m, mine, e0 + ptr);
+    if (mine) {
+      ++ptr;
+      const int nxt = (ptr < len) ? colidx[e0 + ptr] - row : kInf;
+      if (nxt <= m) bad = true;
+      cur = nxt;
+    }
+    ++k;
+  }
+  return __any_sync(0xffffffffu, bad) ? -1 : k;
+}
+
+__device__ __forceinline__ void sell_slot(int n, int s, int lane, int long_min, const int32_t* __restrict__ rowptr,
+                                          const int32_t* __restrict__ perm, int& row, int& e0, int& len) {
+  row = s * 32 + lane;
+  if (perm != nullptr) row = perm[row];
+  e0 = 0; len = 0;
+  if (row >= 0 && row < n) {
+    e0 = rowptr[row];
+    len = rowptr[row + 1] - e0;
+    if (len > long_min) len = 0;
+  } else {
+    row = -1;
+  }
+}
+
+// pass 1: width of every slice; bit 31 set = the slice is stored diagonal-aligned
+__global__ void k_sell_scan(int n, int nslices, int long_min, int allow_aligned, const int32_t* __restrict__ rowptr,
+                            const int32_t* __restrict__ colidx, const int32_t* __restrict__ perm, int32_t* __restrict__ width) {
+  const int lane = threadIdx.x & 31;
+  const int s = (int)(((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5);
+  if (s >= nslices) return;
+  int row, e0, len;
+  sell_slot(n, s, lane, long_min, rowptr, perm, row, e0, len);
+  const int wnat = warp_max_i(len);
+  int w = wnat;
+  if (allow_aligned && wnat > 0) {
+    const int d = sell_align(row < 0 ? 0 : row, e0, len, colidx, wnat + (wnat >> 2), [](int, int, bool, int) {});
+    if (d >= 0) w = d | kAlignedFlag;
+  }
+  if (lane == 0) width[s] = w;
+}
+
+// pass 2: one warp per slice; lane = row slot.  Long rows and padding slots get length 0.
+// General slices: padding entries take the smallest real column of their entry index k (the base of
+// the 16-bit format) and value 0; flag16 is set when some offset from the base does not fit 16 bits.
 __global__ void k_sell_pack(int n, int nslices, int long_min, const int32_t* __restrict__ rowptr,
                             const int32_t* __restrict__ colidx, const double* __restrict__ vals,
                             const int32_t* __restrict__ wptr, const int32_t* __restrict__ perm, int32_t* __restrict__ cols,
@@ -354,26 +521,25 @@ __global__ void k_sell_pack(int n, int nslices, int long_min, const int32_t* __r
   const int lane = threadIdx.x & 31;
   const int s = (int)(((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5);
   if (s >= nslices) return;
-  const int w0 = wptr[s], w = wptr[s + 1] - w0;
+  const bool aligned = wptr[s] < 0;
+  const int w0 = wptr[s] & ~kAlignedFlag, w = (wptr[s + 1] & ~kAlignedFlag) - w0;
   const int64_t base = (int64_t)w0 * 32;
-  int row = s * 32 + lane;
-  if (perm != nullptr) row = perm[row];
-  int e0 = 0, len = 0;
-  if (row >= 0 && row < n) {
-    e0 = rowptr[row];
-    len = rowptr[row + 1] - e0;
-    if (len > long_min) len = 0;
+  int row, e0, len;
+  sell_slot(n, s, lane, long_min, rowptr, perm, row, e0, len);
+  if (aligned) {
+    sell_align(row < 0 ? 0 : row, e0, len, colidx, w, [&](int k, int off, bool mine, int e) {
+      const double v = mine ? vals[e] : 0.0;
+      v32[base + sell_pos32(k, lane, w)] = __double2float_rn(v);
+      v64[base + sell_pos64(k, lane, w)] = v;
+      if (lane == 0) bases[w0 + k] = off;
+    });
+    return;
   }
   bool wide = false;
   for (int k = 0; k < w; ++k) {
     const bool ok = k < len;
     int j = ok ? colidx[e0 + k] : 0x7fffffff;
-    int mn = j, mx = ok ? j : -1;
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
-      mn = min(mn, __shfl_xor_sync(0xffffffffu, mn, o));
-      mx = max(mx, __shfl_xor_sync(0xffffffffu, mx, o));
-    }
+    const int mn = warp_min_i(j), mx = warp_max_i(ok ? j : -1);
     if (!ok) j = mn;
     if (mx - mn > 65535) wide = true;
     const double v = ok ? vals[e0 + k] : 0.0;
