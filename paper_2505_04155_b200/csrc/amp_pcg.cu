@@ -57,6 +57,7 @@ struct amp_pcg {
   double* d_x_stage = nullptr;
   cudaEvent_t ev0 = nullptr, ev1 = nullptr;
   int64_t launches = 0;
+  int pdl = 0;                // graph loop built with programmatic dependent launches
   int32_t last_iters = -1;
   double m_avg = 0.0;
   double idx_bytes_total = 0.0;  // bytes of index data one SpMV reads (slice table, bases, per-entry indices, row order)
@@ -343,6 +344,10 @@ extern "C" amp_pcg_t* amp_pcg_create(int64_t n, int64_t nnz, const int32_t* rowp
 
   // persistent kernel and vector kernels: whole multiples of the SM count
   persistent_configure(h->num_sms, &h->persist_grid, &h->persist_ok);
+  if (h->persist_ok) {  // small problems: no more blocks than there are SpMV groups for their warps (cheaper barriers)
+    const int64_t want = (c.nslices + 2 * (kPersistThreads / 32) - 1) / (2 * (kPersistThreads / 32));
+    h->persist_grid = (int)std::max<int64_t>(1, std::min<int64_t>(h->persist_grid, want));
+  }
   // vector kernels: one full wave of blocks (grid-stride loops inside); small problems get fewer blocks
   // (at least 2 chunks of 8 elements per thread)
   auto vec_grid_for = [&](const void* kern) -> int {
@@ -405,17 +410,33 @@ extern "C" int amp_spmv(amp_pcg_t* h, int mat_prec, int vec_prec, const void* p,
 }
 
 // ------------------------------------------------------------------ graph loop --------------
-static void launch_iteration(amp_pcg* h, const Ctx& c, cudaStream_t s) {
-  k_z<<<h->grid_z, kVecThreads, 0, s>>>(c);
-  k_p<<<h->grid_p, kVecThreads, 0, s>>>(c);
-  k_spmv<<<h->spmv_grid, kSpmvThreads, 0, s>>>(c);
-  k_xr<<<h->grid_xr, kVecThreads, 0, s>>>(c);
+template <class K>
+static cudaError_t launch_loop_kernel(K kern, int grid, int threads, cudaStream_t s, const Ctx& c, bool pdl) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3((unsigned)grid);
+  cfg.blockDim = dim3((unsigned)threads);
+  cfg.dynamicSmemBytes = 0;
+  cfg.stream = s;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = pdl ? 1 : 0;
+  return cudaLaunchKernelEx(&cfg, kern, c);
+}
+
+// the four kernels of one iteration; pdl: the last three are launched as programmatic dependents
+static cudaError_t launch_iteration(amp_pcg* h, const Ctx& c, cudaStream_t s, bool pdl) {
+  cudaError_t e = launch_loop_kernel(k_z, h->grid_z, kVecThreads, s, c, false);
+  if (e == cudaSuccess) e = launch_loop_kernel(k_p, h->grid_p, kVecThreads, s, c, pdl);
+  if (e == cudaSuccess) e = launch_loop_kernel(k_spmv, h->spmv_grid, kSpmvThreads, s, c, pdl);
+  if (e == cudaSuccess) e = launch_loop_kernel(k_xr, h->grid_xr, kVecThreads, s, c, pdl);
+  return e;
 }
 
 // One graph = one WHILE conditional node whose body is the four loop kernels; the condition is
 // written from the device by epi_delta / epi_gamma, so a whole solve is a single launch.
-static int build_graph(amp_pcg* h) {
-  if (h->graph_exec) return AMP_OK;
+static int build_graph_once(amp_pcg* h, bool pdl) {
   CU_TRY(cudaGraphCreate(&h->graph, 0), return AMP_ERR_CUDA);
   CU_TRY(cudaGraphConditionalHandleCreate(&h->cond, h->graph, 1, cudaGraphCondAssignDefault), return AMP_ERR_CUDA);
   cudaGraphNodeParams np = {};
@@ -433,13 +454,27 @@ static int build_graph(amp_pcg* h) {
   c.use_cond = 1;
   cudaError_t e = cudaStreamBeginCaptureToGraph(cap, body, nullptr, nullptr, 0, cudaStreamCaptureModeRelaxed);
   if (e == cudaSuccess) {
-    launch_iteration(h, c, cap);
+    const cudaError_t el = launch_iteration(h, c, cap, pdl);
     e = cudaStreamEndCapture(cap, nullptr);
+    if (e == cudaSuccess) e = el;
   }
   cudaStreamDestroy(cap);
-  if (e != cudaSuccess) { set_error("graph capture failed: %s", cudaGetErrorString(e)); return AMP_ERR_CUDA; }
-  CU_TRY(cudaGraphInstantiate(&h->graph_exec, h->graph, 0), return AMP_ERR_CUDA);
+  if (e != cudaSuccess) { set_error("graph capture failed: %s", cudaGetErrorString(e)); cudaGetLastError(); return AMP_ERR_CUDA; }
+  CU_TRY(cudaGraphInstantiate(&h->graph_exec, h->graph, 0), { cudaGetLastError(); return AMP_ERR_CUDA; });
   return AMP_OK;
+}
+
+static int build_graph(amp_pcg* h) {
+  if (h->graph_exec) return AMP_OK;
+  h->pdl = getenv("AMP_NO_PDL") ? 0 : 1;  // tuning aid
+  int rc = build_graph_once(h, h->pdl != 0);
+  if (rc != AMP_OK && h->pdl) {  // programmatic edges not accepted inside the conditional body: plain edges
+    if (h->graph_exec) { cudaGraphExecDestroy(h->graph_exec); h->graph_exec = nullptr; }
+    if (h->graph) { cudaGraphDestroy(h->graph); h->graph = nullptr; }
+    h->pdl = 0;
+    rc = build_graph_once(h, false);
+  }
+  return rc;
 }
 
 // ------------------------------------------------------------------ solve -------------------
@@ -470,7 +505,9 @@ static int solve_impl(amp_pcg* h, const double* b, double* x, double tol, int32_
     h->hist_cap = (int64_t)maxit + 2;
   }
   int mode = pol.loop_mode;
-  if (mode == AMP_LOOP_AUTO) mode = AMP_LOOP_GRAPH;  // measured faster than the persistent kernel at every size so far
+  // measured on B200: the persistent kernel wins while the iteration is latency-bound (c1, n = 4096: 17 vs 23 us
+  // per iteration), the graph loop wins from c2 (n = 2.1 M) up, where its kernels have their own register budgets
+  if (mode == AMP_LOOP_AUTO) mode = (h->persist_ok && h->n <= kPersistAutoMaxRows) ? AMP_LOOP_PERSISTENT : AMP_LOOP_GRAPH;
   if (mode == AMP_LOOP_PERSISTENT && !(h->persist_ok && persistent_fits(h->ctx))) {
     set_error("amp_pcg_solve: persistent loop not available for this problem/device");
     return AMP_ERR_INVALID;
@@ -505,7 +542,7 @@ static int solve_impl(amp_pcg* h, const double* b, double* x, double tol, int32_
     int done_iters = 0;
     while (done_iters < maxit) {
       const int nb = std::min(batch, maxit - done_iters);
-      for (int i = 0; i < nb; ++i) launch_iteration(h, h->ctx, st);
+      for (int i = 0; i < nb; ++i) launch_iteration(h, h->ctx, st, getenv("AMP_NO_PDL") == nullptr);
       done_iters += nb;
       CU_TRY(cudaMemcpyAsync(h->h_flag, &h->ctx.st->done, sizeof(int), cudaMemcpyDeviceToHost, st), return AMP_ERR_CUDA);
       CU_TRY(cudaStreamSynchronize(st), return AMP_ERR_CUDA);

@@ -10,31 +10,33 @@ namespace amp {
 // ------------------------------------------------------------------ precision dispatch ------
 // The precisions in use are device-side scalars (they change inside the loop without the host
 // knowing), so every loop kernel branches on them once, uniformly, and runs the templated body.
+template <int BIF = kVecBytesInFlight>
 __device__ __forceinline__ double dispatch_z(const Ctx& c, int rs, int ur, int uz, double omega, int bid, int nb) {
   if (rs == P64 && ur == P64) {
-    if (uz == P64) return phase_z<P64, P64, P64>(c, omega, bid, nb);
-    if (uz == P32) return phase_z<P64, P64, P32>(c, omega, bid, nb);
-    return phase_z<P64, P64, P16>(c, omega, bid, nb);
+    if (uz == P64) return phase_z<P64, P64, P64, BIF>(c, omega, bid, nb);
+    if (uz == P32) return phase_z<P64, P64, P32, BIF>(c, omega, bid, nb);
+    return phase_z<P64, P64, P16, BIF>(c, omega, bid, nb);
   }
   if (rs == P64 && ur == P32) {
-    if (uz == P64) return phase_z<P64, P32, P64>(c, omega, bid, nb);
-    if (uz == P32) return phase_z<P64, P32, P32>(c, omega, bid, nb);
-    return phase_z<P64, P32, P16>(c, omega, bid, nb);
+    if (uz == P64) return phase_z<P64, P32, P64, BIF>(c, omega, bid, nb);
+    if (uz == P32) return phase_z<P64, P32, P32, BIF>(c, omega, bid, nb);
+    return phase_z<P64, P32, P16, BIF>(c, omega, bid, nb);
   }
-  if (uz == P64) return phase_z<P32, P32, P64>(c, omega, bid, nb);
-  if (uz == P32) return phase_z<P32, P32, P32>(c, omega, bid, nb);
-  return phase_z<P32, P32, P16>(c, omega, bid, nb);
+  if (uz == P64) return phase_z<P32, P32, P64, BIF>(c, omega, bid, nb);
+  if (uz == P32) return phase_z<P32, P32, P32, BIF>(c, omega, bid, nb);
+  return phase_z<P32, P32, P16, BIF>(c, omega, bid, nb);
 }
 
+template <int BIF = kVecBytesInFlight>
 __device__ __forceinline__ void dispatch_p(const Ctx& c, int ps, int uz, double beta, bool first, int bid, int nb) {
-  if (uz == P64) phase_p<P64, P64>(c, beta, first, bid, nb);
+  if (uz == P64) phase_p<P64, P64, BIF>(c, beta, first, bid, nb);
   else if (uz == P32) {
-    if (ps == P64) phase_p<P64, P32>(c, beta, first, bid, nb);
-    else phase_p<P32, P32>(c, beta, first, bid, nb);
+    if (ps == P64) phase_p<P64, P32, BIF>(c, beta, first, bid, nb);
+    else phase_p<P32, P32, BIF>(c, beta, first, bid, nb);
   } else {
-    if (ps == P64) phase_p<P64, P16>(c, beta, first, bid, nb);
-    else if (ps == P32) phase_p<P32, P16>(c, beta, first, bid, nb);
-    else phase_p<P16, P16>(c, beta, first, bid, nb);
+    if (ps == P64) phase_p<P64, P16, BIF>(c, beta, first, bid, nb);
+    else if (ps == P32) phase_p<P32, P16, BIF>(c, beta, first, bid, nb);
+    else phase_p<P16, P16, BIF>(c, beta, first, bid, nb);
   }
 }
 
@@ -50,21 +52,31 @@ __device__ __forceinline__ double dispatch_spmv(const Ctx& c, int ur, int uz, in
   return phase_spmv<P32, COH, NT>(c, c.p16, c.q32, bid, nb, red);
 }
 
+template <int BIF = kVecBytesInFlight>
 __device__ __forceinline__ double dispatch_xr(const Ctx& c, int ur, int uz, double alpha, double* x, int bid, int nb) {
   if (ur == P64) {
-    if (uz == P64) return phase_xr<P64, P64>(c, alpha, x, bid, nb);
-    if (uz == P32) return phase_xr<P64, P32>(c, alpha, x, bid, nb);
-    return phase_xr<P64, P16>(c, alpha, x, bid, nb);
+    if (uz == P64) return phase_xr<P64, P64, BIF>(c, alpha, x, bid, nb);
+    if (uz == P32) return phase_xr<P64, P32, BIF>(c, alpha, x, bid, nb);
+    return phase_xr<P64, P16, BIF>(c, alpha, x, bid, nb);
   }
-  if (uz == P64) return phase_xr<P32, P64>(c, alpha, x, bid, nb);
-  if (uz == P32) return phase_xr<P32, P32>(c, alpha, x, bid, nb);
-  return phase_xr<P32, P16>(c, alpha, x, bid, nb);
+  if (uz == P64) return phase_xr<P32, P64, BIF>(c, alpha, x, bid, nb);
+  if (uz == P32) return phase_xr<P32, P32, BIF>(c, alpha, x, bid, nb);
+  return phase_xr<P32, P16, BIF>(c, alpha, x, bid, nb);
 }
 
 // ------------------------------------------------------------------ loop kernels ------------
+// Programmatic dependent launch (sm_90+): every loop kernel lets its successor start launching at
+// once and itself waits for its predecessor (completion + visibility of its writes) before the first
+// access to anything the predecessor writes, so the launch latency of kernel N+1 overlaps the
+// reduction tail of kernel N.  Both instructions are no-ops in a launch without the attribute.
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
 __global__ void __launch_bounds__(kVecThreads, 3) k_z(const Ctx c) {
   __shared__ double red[32];
   DevState* s = c.st;
+  pdl_launch_dependents();
+  pdl_wait();
   if (s->done) return;
   const int bid = blockIdx.x, nb = gridDim.x;
   const double v = dispatch_z(c, s->r_store, s->ur, s->uz, s->omega, bid, nb);
@@ -74,6 +86,8 @@ __global__ void __launch_bounds__(kVecThreads, 3) k_z(const Ctx c) {
 
 __global__ void __launch_bounds__(kVecThreads, 3) k_p(const Ctx c) {
   const DevState* s = c.st;
+  pdl_launch_dependents();
+  pdl_wait();
   if (s->done) return;
   dispatch_p(c, s->p_store, s->uz, s->beta, s->k == 0, blockIdx.x, gridDim.x);
 }
@@ -81,6 +95,8 @@ __global__ void __launch_bounds__(kVecThreads, 3) k_p(const Ctx c) {
 __global__ void __launch_bounds__(kSpmvThreads, kSpmvMinBlocks) k_spmv(const Ctx c) {
   __shared__ double red[32];
   DevState* s = c.st;
+  pdl_launch_dependents();
+  pdl_wait();
   if (s->done) return;
   const int bid = blockIdx.x, nb = gridDim.x;
   const double v = dispatch_spmv<false, kSpmvThreads>(c, s->ur, s->uz, bid, nb, red);
@@ -91,6 +107,8 @@ __global__ void __launch_bounds__(kSpmvThreads, kSpmvMinBlocks) k_spmv(const Ctx
 __global__ void __launch_bounds__(kVecThreads, 2) k_xr(const Ctx c) {
   __shared__ double red[32];
   DevState* s = c.st;
+  pdl_launch_dependents();
+  pdl_wait();
   if (s->done) {  // nothing to do (converged at set-up, or breakdown): make sure the WHILE node stops
     if (blockIdx.x == 0 && threadIdx.x == 0) set_loop_cond(epi_ctx(c), 0);
     return;

@@ -1,100 +1,120 @@
 // persistent.cuh — the whole AMP-PCG loop as ONE cooperative kernel (north_star: "a persistent
-// cooperative kernel for small n"): every block stays resident, the three reductions of an
-// iteration (rho, gamma, delta; Alg 4.1 lines 6, 13, 17) double as grid barriers whose last
-// arriver runs the scalar epilogue, and one plain barrier publishes p before the gather.
-// The phases are the same device functions the stand-alone kernels call.
+// cooperative kernel for small n"): every block stays resident and the four synchronisation
+// points of an iteration (rho, p complete, gamma, delta; Alg 4.1 lines 6, 10, 13, 17) are grid
+// barriers instead of kernel boundaries.
+//
+// What makes the barrier cheap: the loop scalars are REPLICATED.  Every block keeps its own copy
+// of the DevState block in shared memory; at a reduction every block publishes its partial sum,
+// arrives (one red.release), waits until all have arrived (one polled ld.acquire), then adds ALL
+// partials itself in index order and runs the scalar epilogue on its own copy.  All blocks add
+// the same numbers in the same order, so they take identical decisions (precision switches, stop,
+// breakdown) without any broadcast: one barrier = arrive + poll + one read of the partials, no
+// "last block computes, then releases the others" round trip.  Block 0 writes the state back for
+// the host when the loop ends.  The phases are the same device functions the stand-alone kernels
+// call; p is gathered with plain (coherent) loads because it is written inside this kernel.
 #pragma once
+#include <cstddef>
+
 #include "kernels.cuh"
 
 namespace amp {
 
+constexpr int kPersistBIF = 96;  // bytes of loads in flight per thread of the vector phases (register budget: 64)
 
 __device__ __forceinline__ unsigned int ld_acquire_u32(const unsigned int* p) {
   unsigned int v;
   asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
   return v;
 }
-__device__ __forceinline__ void st_release_u32(unsigned int* p, unsigned int v) {
-  asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+__device__ __forceinline__ void red_release_add_u32(unsigned int* p, unsigned int v) {
+  asm volatile("red.release.gpu.global.add.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
 }
-template <class T> __device__ __forceinline__ T ldv(const T* p) { return __ldcg(p); }  // L2, never a stale L1 line
 
-// Grid barrier fused with a deterministic reduction: blocks publish partial sums and take a
-// ticket; the last arriver adds the partials in index order, runs epi(total) on one thread,
-// then opens the barrier by bumping the generation.  SUM = false: plain barrier.
-template <bool SUM, class Epi>
-__device__ __forceinline__ void grid_sync_reduce(double v, double* partials, DevState* s, int bid, int nb,
-                                                 double* red, Epi epi) {
-  __shared__ int s_last;
-  __shared__ unsigned int s_gen;
+// Grid barrier fused with a deterministic all-reduce.  `arrivals` counts up over the whole solve
+// (reset by the set-up kernel); `target` is this block's running count of expected arrivals.
+// SUM = false: plain barrier.  Returns the total in warp 0 (SUM = true).
+// `partials` must be a different array at consecutive barriers (a fast block may already publish
+// its next partial while a slow one still reads this one).
+template <bool SUM>
+__device__ __forceinline__ double grid_all_sum(double v, double* partials, unsigned int* arrivals, unsigned int& target,
+                                               int bid, int nb, double* red) {
   double bs = 0.0;
-  if (SUM) bs = block_sum<kPersistThreads>(v, red);
+  if (SUM) bs = block_sum<kPersistThreads>(v, red);  // every thread is past its phase's memory accesses
   else __syncthreads();
+  target += (unsigned int)nb;
   if (threadIdx.x == 0) {
     if (SUM) __stcg(partials + bid, bs);
-    const unsigned int gen = ld_acquire_u32(&s->bar_gen);
-    __threadfence();
-    const unsigned int t = atomicAdd(&s->bar_count, 1u);
-    s_last = (t == (unsigned int)nb - 1u);
-    s_gen = gen;
+    red_release_add_u32(arrivals, 1u);
+    while ((int)(ld_acquire_u32(arrivals) - target) < 0) { }
   }
   __syncthreads();
-  if (s_last) {
-    double tot = 0.0;
-    if (SUM) {
-      __threadfence();
-      double a = 0.0;
-      for (int i = threadIdx.x; i < nb; i += kPersistThreads) a += __ldcg(partials + i);
-      tot = block_sum<kPersistThreads>(a, red);
-    }
-    if (threadIdx.x == 0) {
-      if (SUM) epi(tot);
-      s->bar_count = 0u;
-      __threadfence();
-      st_release_u32(&s->bar_gen, s_gen + 1u);
-    }
-  } else if (threadIdx.x == 0) {
-    while (ld_acquire_u32(&s->bar_gen) == s_gen) { }
-    __threadfence();
+  double tot = 0.0;
+  if (SUM) {
+    double a = 0.0;
+    for (int i = threadIdx.x; i < nb; i += kPersistThreads) a += __ldcg(partials + i);
+    tot = block_sum<kPersistThreads>(a, red);
   }
-  __syncthreads();
+  return tot;
 }
 
 // out-of-line copies of the phase dispatchers: each gets its own register allocation instead of
 // one allocation for the union of all precision variants
 __device__ __noinline__ double pz(const Ctx& c, int rs, int ur, int uz, double omega, int bid, int nb) {
-  return dispatch_z(c, rs, ur, uz, omega, bid, nb);
+  return dispatch_z<kPersistBIF>(c, rs, ur, uz, omega, bid, nb);
 }
 __device__ __noinline__ void pp(const Ctx& c, int ps, int uz, double beta, bool first, int bid, int nb) {
-  dispatch_p(c, ps, uz, beta, first, bid, nb);
+  dispatch_p<kPersistBIF>(c, ps, uz, beta, first, bid, nb);
 }
 __device__ __noinline__ double ps_(const Ctx& c, int ur, int uz, int bid, int nb, double* red) {
   return dispatch_spmv<true, kPersistThreads>(c, ur, uz, bid, nb, red);
 }
 __device__ __noinline__ double pxr(const Ctx& c, int ur, int uz, double alpha, double* x, int bid, int nb) {
-  return dispatch_xr(c, ur, uz, alpha, x, bid, nb);
+  return dispatch_xr<kPersistBIF>(c, ur, uz, alpha, x, bid, nb);
 }
 
-__global__ void __launch_bounds__(kPersistThreads, 1) k_persistent(const Ctx c) {
+__global__ void __launch_bounds__(kPersistThreads, kPersistMinBlocks) k_persistent(const Ctx c) {
   __shared__ double red[32];
-  DevState* s = c.st;
+  __shared__ DevState ls;  // this block's replica of the loop scalars
   const int bid = blockIdx.x, nb = gridDim.x;
-  double* x = s->x;  // host-written before the launch, constant during the solve
-  auto nop = [](double) {};
-  while (true) {
-    if (ldv(&s->done)) break;
-    const int rs = ldv(&s->r_store), ps = ldv(&s->p_store), ur = ldv(&s->ur), uz = ldv(&s->uz);
-    const double omega = ldv(&s->omega);
-    const bool first = (ldv(&s->k) == 0);
-    double v = pz(c, rs, ur, uz, omega, bid, nb);                                                   // a2
-    grid_sync_reduce<true>(v, c.partials + 0 * kMaxGrid, s, bid, nb, red, [&](double t) { epi_rho(epi_ctx(c), t); });
-    pp(c, ps, uz, ldv(&s->beta), first, bid, nb);                                                   // a3
-    grid_sync_reduce<false>(0.0, nullptr, s, bid, nb, red, nop);
-    v = ps_(c, ur, uz, bid, nb, red);                                                        // a4
-    grid_sync_reduce<true>(v, c.partials + 1 * kMaxGrid, s, bid, nb, red, [&](double t) { epi_gamma(epi_ctx(c), t); });
-    if (ldv(&s->done)) break;  // breakdown
-    v = pxr(c, ur, uz, ldv(&s->alpha), x, bid, nb);                                                 // a5
-    grid_sync_reduce<true>(v, c.partials + 2 * kMaxGrid, s, bid, nb, red, [&](double t) { epi_delta(epi_ctx(c), t); });
+  {  // replicate the state block (written by the host and the set-up kernel before this launch)
+    const int* src = reinterpret_cast<const int*>(c.st);
+    int* dst = reinterpret_cast<int*>(&ls);
+    for (int i = threadIdx.x; i < (int)(sizeof(DevState) / sizeof(int)); i += kPersistThreads) dst[i] = __ldcg(src + i);
+  }
+  __syncthreads();
+  DevState* s = &ls;
+  EpiCtx ec = epi_ctx(c);
+  ec.st = s;
+  ec.use_cond = 0;
+  unsigned int* arrivals = &c.st->bar_count;
+  unsigned int target = 0u;
+  double* x = s->x;
+  while (!s->done) {
+    const int rs = s->r_store, ps = s->p_store, ur = s->ur, uz = s->uz;
+    const bool first = (s->k == 0);
+    double v = pz(c, rs, ur, uz, s->omega, bid, nb);                                                 // a2
+    double t = grid_all_sum<true>(v, c.partials + 0 * kMaxGrid, arrivals, target, bid, nb, red);
+    if (threadIdx.x == 0) epi_rho(ec, t);
+    __syncthreads();
+    pp(c, ps, uz, s->beta, first, bid, nb);                                                          // a3
+    grid_all_sum<false>(0.0, nullptr, arrivals, target, bid, nb, red);
+    v = ps_(c, ur, uz, bid, nb, red);                                                                // a4
+    t = grid_all_sum<true>(v, c.partials + 1 * kMaxGrid, arrivals, target, bid, nb, red);
+    if (threadIdx.x == 0) epi_gamma(ec, t);
+    __syncthreads();
+    if (s->done) break;  // breakdown
+    v = pxr(c, ur, uz, s->alpha, x, bid, nb);                                                        // a5
+    t = grid_all_sum<true>(v, c.partials + 2 * kMaxGrid, arrivals, target, bid, nb, red);
+    if (threadIdx.x == 0) epi_delta(ec, t);
+    __syncthreads();
+  }
+  if (bid == 0) {  // publish the result scalars (not the barrier counter: other blocks may still poll it)
+    __syncthreads();
+    int* dst = reinterpret_cast<int*>(c.st);
+    const int* src = reinterpret_cast<const int*>(&ls);
+    const int skip0 = (int)(offsetof(DevState, bar_count) / sizeof(int));
+    for (int i = threadIdx.x; i < (int)(sizeof(DevState) / sizeof(int)); i += kPersistThreads)
+      if (i != skip0 && i != skip0 + 1) dst[i] = src[i];
   }
 }
 

@@ -165,7 +165,7 @@ __device__ __forceinline__ void count_fp16(DevState* s, double v, double h) {
 // ------------------------------------------------------------------ a2: z and rho ------------
 // RS: precision r is stored in; UR: precision selected for r (RS != UR only at the iteration of
 // the u_r switch, where r <- RN32(r) is fused here, step a6); UZ: precision of z.
-template <int RS, int UR, int UZ>
+template <int RS, int UR, int UZ, int BIF = kVecBytesInFlight>
 __device__ __forceinline__ double phase_z(const Ctx& c, const double omega, int bid, int nb) {
   using TR = typename Store<RS>::T;
   using TO = typename Store<UR>::T;
@@ -174,7 +174,7 @@ __device__ __forceinline__ double phase_z(const Ctx& c, const double omega, int 
   constexpr int smin = cmin(cmin((int)sizeof(TR), (int)sizeof(TO)), cmin((int)sizeof(TD), (int)sizeof(TZ)));
   constexpr int smax = cmax(cmax((int)sizeof(TR), (int)sizeof(TO)), cmax((int)sizeof(TD), (int)sizeof(TZ)));
   constexpr int E = chunk_elems(smin, smax);
-  constexpr int U = cmax(1, kVecBytesInFlight / (E * (int)(sizeof(TR) + sizeof(TD))));
+  constexpr int U = cmax(1, BIF / (E * (int)(sizeof(TR) + sizeof(TD))));
   const TR* rin = rvec<RS>(c);
   TO* rout = rvec<UR>(c);
   TZ* z = zvec<UZ>(c);
@@ -232,12 +232,12 @@ __device__ __forceinline__ double phase_z(const Ctx& c, const double omega, int 
 // ------------------------------------------------------------------ a3: p -------------------
 // PS: precision p_{k-1} is stored in; UZ: precision of z_k and p_k (PS != UZ only at a u_z
 // switch, where p_{k-1} <- RN_{u_z}(p_{k-1}) is fused here, reading R9).
-template <int PS, int UZ>
+template <int PS, int UZ, int BIF = kVecBytesInFlight>
 __device__ __forceinline__ void phase_p(const Ctx& c, const double beta, const bool first, int bid, int nb) {
   using TP = typename Store<PS>::T;
   using TZ = typename Store<UZ>::T;
   constexpr int E = chunk_elems(cmin((int)sizeof(TP), (int)sizeof(TZ)), cmax((int)sizeof(TP), (int)sizeof(TZ)));
-  constexpr int U = cmax(1, kVecBytesInFlight / (E * (int)(sizeof(TP) + sizeof(TZ))));
+  constexpr int U = cmax(1, BIF / (E * (int)(sizeof(TP) + sizeof(TZ))));
   const TP* pin = pvec<PS>(c);
   TZ* pout = pvec<UZ>(c);
   const TZ* z = zvec<UZ>(c);
@@ -289,12 +289,12 @@ __device__ __forceinline__ void phase_p(const Ctx& c, const double beta, const b
 }
 
 // ------------------------------------------------------------------ a5: x, r, delta ---------
-template <int UR, int UZ>
+template <int UR, int UZ, int BIF = kVecBytesInFlight>
 __device__ __forceinline__ double phase_xr(const Ctx& c, const double alpha, double* x, int bid, int nb) {
   using TZ = typename Store<UZ>::T;
   using TR = typename Store<UR>::T;
   constexpr int E = chunk_elems(cmin((int)sizeof(TZ), (int)sizeof(TR)), 8);
-  constexpr int U = cmax(1, kVecBytesInFlight / (E * (int)(8 + sizeof(TZ) + 2 * sizeof(TR))));
+  constexpr int U = cmax(1, BIF / (E * (int)(8 + sizeof(TZ) + 2 * sizeof(TR))));
   const TZ* p = pvec<UZ>(c);
   const TR* q = qvec<UR>(c);
   TR* r = rvec<UR>(c);

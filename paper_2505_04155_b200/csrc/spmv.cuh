@@ -49,24 +49,27 @@ __host__ __device__ __forceinline__ int64_t sell_pos64(int k, int lane, int w) {
 }
 
 // streaming (evict-first) loads of matrix data
-__device__ __forceinline__ int4 lds_i4(const int32_t* p) { return __ldcs(reinterpret_cast<const int4*>(p)); }
-__device__ __forceinline__ int2 lds_i2(const int32_t* p) { return __ldcs(reinterpret_cast<const int2*>(p)); }
-__device__ __forceinline__ int lds_i1(const int32_t* p) { return __ldcs(p); }
+#ifndef AMP_SPMV_MATRIX_LOAD
+#define AMP_SPMV_MATRIX_LOAD __ldcs
+#endif
+__device__ __forceinline__ int4 lds_i4(const int32_t* p) { return AMP_SPMV_MATRIX_LOAD(reinterpret_cast<const int4*>(p)); }
+__device__ __forceinline__ int2 lds_i2(const int32_t* p) { return AMP_SPMV_MATRIX_LOAD(reinterpret_cast<const int2*>(p)); }
+__device__ __forceinline__ int lds_i1(const int32_t* p) { return AMP_SPMV_MATRIX_LOAD(p); }
 __device__ __forceinline__ void lds_quad(const float* v, float (&a)[4]) {
-  const float4 t = __ldcs(reinterpret_cast<const float4*>(v));
+  const float4 t = AMP_SPMV_MATRIX_LOAD(reinterpret_cast<const float4*>(v));
   a[0] = t.x; a[1] = t.y; a[2] = t.z; a[3] = t.w;
 }
 __device__ __forceinline__ void lds_quad(const double* v, double (&a)[4]) {  // v -> first pair block, lane offset applied
-  const double2 t0 = __ldcs(reinterpret_cast<const double2*>(v));
-  const double2 t1 = __ldcs(reinterpret_cast<const double2*>(v + 64));
+  const double2 t0 = AMP_SPMV_MATRIX_LOAD(reinterpret_cast<const double2*>(v));
+  const double2 t1 = AMP_SPMV_MATRIX_LOAD(reinterpret_cast<const double2*>(v + 64));
   a[0] = t0.x; a[1] = t0.y; a[2] = t1.x; a[3] = t1.y;
 }
 __device__ __forceinline__ void lds_pair(const float* v, float (&a)[2]) {
-  const float2 t = __ldcs(reinterpret_cast<const float2*>(v));
+  const float2 t = AMP_SPMV_MATRIX_LOAD(reinterpret_cast<const float2*>(v));
   a[0] = t.x; a[1] = t.y;
 }
 __device__ __forceinline__ void lds_pair(const double* v, double (&a)[2]) {
-  const double2 t = __ldcs(reinterpret_cast<const double2*>(v));
+  const double2 t = AMP_SPMV_MATRIX_LOAD(reinterpret_cast<const double2*>(v));
   a[0] = t.x; a[1] = t.y;
 }
 
@@ -87,8 +90,8 @@ template <bool COH> __device__ __forceinline__ float gatherA(float, const __half
 template <class A> struct LaneQ;  // elements a lane owns per 128-bit load of a value block
 template <> struct LaneQ<float> { static constexpr int v = 4; };
 template <> struct LaneQ<double> { static constexpr int v = 2; };
-__device__ __forceinline__ float lds_one(const float* v) { return __ldcs(v); }
-__device__ __forceinline__ double lds_one(const double* v) { return __ldcs(v); }
+__device__ __forceinline__ float lds_one(const float* v) { return AMP_SPMV_MATRIX_LOAD(v); }
+__device__ __forceinline__ double lds_one(const double* v) { return AMP_SPMV_MATRIX_LOAD(v); }
 
 // ------------------------------------------------------------------ column index sources ----
 // CM = 0: 32-bit column indices.
