@@ -334,7 +334,7 @@ extern "C" amp_pcg_t* amp_pcg_create(int64_t n, int64_t nnz, const int32_t* rowp
 
     // SpMV grid: a warp takes a group of up to kSpmvGroupMax slices per pass; blocks make a whole number of
     // (nearly) equal passes, at most `mult` blocks per SM (AMP_SPMV_GRID_MULT: tuning aid)
-    int mult = perm.empty() ? 8 : 55;  // sorted (irregular) matrices: small blocks even out the slice widths
+    int mult = perm.empty() ? 4 : 55;  // sorted (irregular) matrices: small blocks even out the slice widths
     if (const char* e = getenv("AMP_SPMV_GRID_MULT")) mult = std::max(1, atoi(e));
     const int64_t max_grid = std::min<int64_t>((int64_t)h->num_sms * mult, kMaxGrid);
     const int64_t nblk = (nsl + kSpmvWarps * kSpmvGroupMax - 1) / (kSpmvWarps * kSpmvGroupMax);

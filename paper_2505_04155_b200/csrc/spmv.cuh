@@ -103,6 +103,7 @@ __device__ __forceinline__ double lds_one(const double* v) { return AMP_SPMV_MAT
 //         (rows that lack a diagonal hold an explicit zero there).  No per-entry index is read at
 //         all: 4 B per 32 entries.  Typical for stencil / structured-grid matrices.
 // The base of entry k is held by lane k % 32 and broadcast by a shuffle.
+constexpr int kPrefetchMinWidth = 16;  // groups narrower than this many entries per row are not prefetched
 constexpr int kAlignedFlag = (int)0x80000000u;  // bit 31 of sell_wptr[s]: slice s is aligned
 template <int CM> struct ColSrc;
 template <> struct ColSrc<0> {
@@ -366,6 +367,17 @@ __device__ __forceinline__ double phase_spmv_fmt(const Ctx& c, const PT* p, type
         for (int g = 0; g <= G; ++g) wnext[g] = __ldg(wptr + min(gn * G + g, nslices));
       }
     }
+#ifndef AMP_SPMV_NO_PREFETCH
+    // extent of the group two passes ahead: its value stream is prefetched into L2 at the end of this pass
+    int pf0 = 0, pf1 = 0;
+    {
+      const int g2 = gi + 2 * nb * wpb;
+      if (g2 < ngroups) {
+        pf0 = __ldg(wptr + min(g2 * G, nslices)) & ~kAlignedFlag;
+        pf1 = __ldg(wptr + min(g2 * G + G, nslices)) & ~kAlignedFlag;
+      }
+    }
+#endif
 #pragma unroll
     for (int g = 0; g < G; ++g) {
       al_g[g] = wp[g] < 0;  // kAlignedFlag
@@ -416,6 +428,13 @@ __device__ __forceinline__ double phase_spmv_fmt(const Ctx& c, const PT* p, type
         gsum = fma(pi[g], (double)acc[g], gsum);
       }
     }
+#ifndef AMP_SPMV_NO_PREFETCH
+    if (pf1 - pf0 > kPrefetchMinWidth) {  // one 128-byte line per lane and trip
+      const char* src = reinterpret_cast<const char*>(sell_vals<UR>(c) + (int64_t)pf0 * 32);
+      const int nbytes = (pf1 - pf0) * 32 * (int)sizeof(A);
+      for (int off = lane * 128; off < nbytes; off += 32 * 128) asm volatile("prefetch.global.L2 [%0];" ::"l"(src + off));
+    }
+#endif
   }
 
   // rows too long for the slices: one block per row, straight from the CSR arrays
