@@ -32,7 +32,10 @@ SMI_QUERY = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.acti
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the SpMV kernel from the committed ncu --set full
 # captures (profiles/r01c_*.md name the commands); None where no capture exists for that workload
-NCU_TRAFFIC = {}
+NCU_TRAFFIC = {
+    ("c2", "fp32mat_fp16vec"): 64.82e6 + 2.17e6,   # profiles/r01c_c2_ncu_full.csv, k_spmv in phase (FP16, FP32)
+    ("c4", "fp32mat_fp16vec"): 907.34e6 + 28.23e6,  # profiles/r01c_c4_ncu_full.csv
+}
 
 
 def parse_args():
