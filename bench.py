@@ -107,6 +107,20 @@ class ClockSampler:
                            "samples": len(sm)}
 
 
+def reduce_over_ranks(dist, vmax, vsum, device):
+    """Whole-job aggregation of one timed region: element-wise MAX over ranks of `vmax` (device times: the job is as
+    slow as its slowest rank) and SUM over ranks of `vsum` (work done: iterations, launches).  dist = None: one rank."""
+    if dist is None:
+        return [float(v) for v in vmax], [float(v) for v in vsum]
+    import torch
+
+    tm = torch.tensor([float(v) for v in vmax], dtype=torch.float64, device=device)
+    ts = torch.tensor([float(v) for v in vsum], dtype=torch.float64, device=device)
+    dist.all_reduce(tm, op=dist.ReduceOp.MAX)
+    dist.all_reduce(ts, op=dist.ReduceOp.SUM)
+    return tm.tolist(), ts.tolist()
+
+
 def policy_kwargs(name: str):
     return {"amp_fp64_delay": dict(amp=1, u0=0, eta_rule=0), "amp_fp16_linear": dict(amp=1, u0=2, eta_rule=1)}[name]
 
@@ -215,13 +229,8 @@ def run_ours(args, rank: int, local_rank: int, world: int):
         ms, its, launches, st = timed_solves(pol, args.steps)
     barrier()
     total_ms = sum(ms)
-    if dist is not None:
-        t = torch.tensor([total_ms, float(its), float(launches)], dtype=torch.float64, device=dev)
-        tmax = t.clone(); dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-        tsum = t.clone(); dist.all_reduce(tsum, op=dist.ReduceOp.SUM)
-        total_ms_max, its_all, launches_all = float(tmax[0]), float(tsum[1]), int(tsum[2])
-    else:
-        total_ms_max, its_all, launches_all = total_ms, float(its), launches
+    (total_ms_max,), (its_all, launches_all) = reduce_over_ranks(dist, [total_ms], [its, launches], dev)
+    launches_all = int(launches_all)
     value = its_all / (total_ms_max * 1e-3)
 
     # ---- end-to-end through the host-buffer entry point (H2D of b, solve, D2H of x inside) ----
@@ -231,12 +240,7 @@ def run_ours(args, rank: int, local_rank: int, world: int):
     barrier()
     ms_e, its_e, _, _ = timed_solves(pol, args.steps, host=True, bh=bh, xh=xh)
     barrier()
-    tot_e = sum(ms_e)
-    if dist is not None:
-        t = torch.tensor([tot_e, float(its_e)], dtype=torch.float64, device=dev)
-        tm = t.clone(); dist.all_reduce(tm, op=dist.ReduceOp.MAX)
-        ts = t.clone(); dist.all_reduce(ts, op=dist.ReduceOp.SUM)
-        tot_e, its_e = float(tm[0]), float(ts[1])
+    (tot_e,), (its_e,) = reduce_over_ranks(dist, [sum(ms_e)], [its_e], dev)
     e2e_value = its_e / (tot_e * 1e-3)
 
     if rank != 0:

@@ -2,24 +2,31 @@
 // PAPER.md:288-291; the paper also fuses the inner product into its Ax kernel, :537).
 //
 // Matrix format: SELL-32 ("sliced ELLPACK", slice height = warp width), repacked once from the
-// caller's CSR in amp_pcg_create and owned by the handle (column indices, FP64 values and the
-// FP32-rounded value copy of the u_r = FP32 phase).
-//  * A slice is 32 consecutive rows (of the row order `perm`, identity unless the row lengths
-//    vary enough for a windowed sort to pay); lane l of a warp owns row l of the slice.
-//  * The slice width w = longest row of the slice; shorter rows are padded with (value 0,
-//    column = own row).  w is cut as 4a + 2b + c and stored as a blocks of [lane][4] entries,
-//    then b block of [lane][2], then c block of [lane][1], so a lane reads its row with 128-bit
-//    loads (64-/32-bit for the remainder) and every warp-wide load is one contiguous, fully used
-//    512-byte (256-, 128-byte) run: no padding beyond the slice maximum, 0.125 B/row of index
-//    overhead (the cumulative widths) instead of CSR's 4 B/row row pointer.
-//    FP64 values use [lane][2] blocks throughout (a quad = two consecutive pair blocks).
-//  * Entries keep their CSR order within the row and each lane accumulates ONE fma chain in the
-//    working precision, so q_i is bit-identical to a sequential CSR-order fma loop.
+// caller's CSR in amp_pcg_create and owned by the handle (indices, FP64 values and the FP32-rounded
+// value copy of the u_r = FP32 phase).
+//  * A slice is 32 consecutive rows (of the row order `perm`: identity, or rows sorted by length
+//    inside windows of 1024 when the lengths vary enough for padding to cost > 3 %); lane l of a
+//    warp owns row l of the slice.
+//  * The slice width w = longest row of the slice; shorter rows are padded with value 0 and a valid
+//    column.  w is cut as 4a + 2b + c and stored as a blocks of [lane][4] entries, then b block of
+//    [lane][2], then c block of [lane][1], so a lane reads its row with 128-bit loads (64-/32-bit
+//    for the remainder) and every warp-wide load is one contiguous, fully used 512-byte (256-,
+//    128-byte) run: no padding beyond the slice maximum, 4 B per SLICE of table (the cumulative
+//    widths) instead of CSR's 4 B per ROW of row pointer.  FP64 values use [lane][2] blocks
+//    throughout (a quad = two consecutive pair blocks).
+//  * Column indices come in three forms (ColSrc below): diagonal-aligned slices need none at all
+//    (col = row + one offset per entry position), banded matrices get 16-bit offsets, the rest
+//    32-bit indices.
+//  * Entries keep their CSR order within the row (aligned slices interleave explicit zeros, which
+//    leave an fma chain unchanged) and each lane accumulates ONE fma chain in the working
+//    precision, so q_i is bit-identical to a sequential CSR-order fma loop.
 //  * Matrix data is streamed with ld.global.cs (evict-first) so that it does not displace the
-//    vectors from L2; p is gathered through the read-only path (L1-cached) — adjacent lanes hold
-//    adjacent rows, so for banded matrices one gather instruction touches one or two lines.
-//  * Rows longer than the cap `long_row_min` are left out of the slices (length 0 there) and
-//    summed straight from the borrowed CSR arrays by a whole block each.
+//    vectors from L2 (measured: 57 vs 65 us per iteration on c2 against default caching); the value
+//    stream of wide slices is prefetched into L2 two passes ahead; p is gathered through the
+//    read-only path (L1-cached) — adjacent lanes hold adjacent rows, so for banded matrices one
+//    gather instruction touches one or two lines.
+//  * Rows longer than max(256, 8 nnz/n) are left out of the slices (length 0 there) and summed
+//    straight from the borrowed CSR arrays by a whole block each.
 // UR = P64: FP64 values, FP64 products and sums.  UR = P32: FP32 value copy, p_j converted to
 // FP32 (exact from FP16/FP32 storage), FP32 products and sums (q computed and
 // stored in u_r).
