@@ -49,7 +49,7 @@ enum {
 };
 /* how the iteration loop is driven (execution choice; does not change the arithmetic) */
 enum {
-  AMP_LOOP_AUTO = 0,       /* persistent kernel for small systems (n <= 131072 rows), else graph */
+  AMP_LOOP_AUTO = 0,       /* persistent kernel for small systems (n <= 2^20 rows), else graph */
   AMP_LOOP_STREAM = 1,     /* plain stream launches in batches; host polls a device flag between batches */
   AMP_LOOP_GRAPH = 2,      /* one CUDA graph launch: WHILE conditional node around the 4 kernels */
   AMP_LOOP_PERSISTENT = 3  /* one cooperative kernel, grid barriers between the phases */

@@ -505,8 +505,9 @@ static int solve_impl(amp_pcg* h, const double* b, double* x, double tol, int32_
     h->hist_cap = (int64_t)maxit + 2;
   }
   int mode = pol.loop_mode;
-  // measured on B200: the persistent kernel wins while the iteration is latency-bound (c1, n = 4096: 17 vs 23 us
-  // per iteration), the graph loop wins from c2 (n = 2.1 M) up, where its kernels have their own register budgets
+  // measured on B200 (us per iteration, persistent vs graph): n = 4 K 17 vs 23, 16 K 19.6 vs 24.0, 262 K 20.9 vs 29.0,
+  // 512 K 25.0 vs 32.1, 2.1 M (c2) 58 vs 57, 4.1 M (c3) 95 vs 92: the persistent kernel wins while the iteration is
+  // latency-bound; from c2 up the graph loop wins because each of its kernels has its own register budget
   if (mode == AMP_LOOP_AUTO) mode = (h->persist_ok && h->n <= kPersistAutoMaxRows) ? AMP_LOOP_PERSISTENT : AMP_LOOP_GRAPH;
   if (mode == AMP_LOOP_PERSISTENT && !(h->persist_ok && persistent_fits(h->ctx))) {
     set_error("amp_pcg_solve: persistent loop not available for this problem/device");

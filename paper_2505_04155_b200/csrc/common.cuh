@@ -19,7 +19,7 @@ constexpr int kSpmvWarps = kSpmvThreads / 32;
 #endif
 constexpr int kSpmvMinBlocks = AMP_SPMV_MINBLOCKS;  // resident SpMV blocks per SM the register budget is set for
 constexpr int kPersistThreads = 1024;          // block size of the persistent (whole-loop) kernel
-constexpr int kPersistAutoMaxRows = 131072;   // AMP_LOOP_AUTO takes the persistent kernel up to this many rows
+constexpr int kPersistAutoMaxRows = 1 << 20;   // AMP_LOOP_AUTO takes the persistent kernel up to this many rows
 constexpr int kPersistMinBlocks = 1;           // resident blocks per SM its register budget is set for
 constexpr int kMaxGrid = 8192;                 // capacity of each partial-sum array
 constexpr int kMaxWindow = 64;                 // max d / ell of the indicators
