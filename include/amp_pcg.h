@@ -154,6 +154,14 @@ int amp_spmv(amp_pcg_t *h, int mat_prec, int vec_prec, const void *p, void *q);
  * returns the number of values written (<= iters+1), or a negative error code. */
 int32_t amp_pcg_residual_history(amp_pcg_t *h, double *out_host, int32_t count);
 
+/* A-posteriori attainable-accuracy indicator of the last solve, eq. (4.7):
+ *   out[k] = eta_hat_m(k) = sum_{t=0..k} eps64 ((3+C)||r_{t-1}|| + (2+C)||r_t||) + sum_{t=k..m} eps32 ((3+C)||r_{t-1}|| + (2+C)||r_t||)
+ * for k = 0..min(count, m+1)-1, m = iterations of the last solve, ||r_{-1}|| := ||r_0||, eps64 = 2^-53, eps32 = 0 -> 2^-24:
+ * the accuracy the run could have attained had u_r been switched to FP32 at iteration k (the dotted curves of the
+ * paper's Fig. 3 and 8).  Host post-processing of the stored history (HOST out); returns the number of values
+ * written or a negative error code. */
+int32_t amp_pcg_eta_posteriori(amp_pcg_t *h, double C, double eps32, double *out_host, int32_t count);
+
 /* Run all work of this handle on the given cudaStream_t (NULL = legacy default stream). */
 int amp_pcg_set_stream(amp_pcg_t *h, void *cuda_stream);
 

@@ -87,6 +87,8 @@ def lib():
         L.orc_spmv_fp32.argtypes = [C.c_int64] + [C.c_void_p] * 5 + [C.c_int]
         L.orc_eta.restype = C.c_double
         L.orc_eta.argtypes = [C.POINTER(_Policy), C.c_void_p, C.c_int32]
+        L.orc_eta_posteriori.restype = C.c_double
+        L.orc_eta_posteriori.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_double, C.c_double, C.c_double]
         L.orc_select_uz.restype = C.c_int32
         L.orc_select_uz.argtypes = [C.POINTER(_Policy), C.c_double]
         L.orc_amp_pcg.restype = C.c_int32
@@ -157,6 +159,12 @@ def spmv_fp32(rowptr, colidx, vals, p, accumulate64: int = 0) -> np.ndarray:
 def eta(policy: _Policy, hist: np.ndarray, k: int) -> float:
     hist = np.ascontiguousarray(hist, dtype=np.float64)
     return float(lib().orc_eta(C.byref(policy), _ptr(hist), int(k)))
+
+
+def eta_posteriori(hist: np.ndarray, k: int, C_: float = 1.0, eps32: float = 2.0 ** -24, eps64: float = 2.0 ** -53) -> float:
+    """eta_hat_m(k) of (4.7), with m = len(hist) - 1 (the whole history of a finished run)."""
+    hist = np.ascontiguousarray(hist, dtype=np.float64)
+    return float(lib().orc_eta_posteriori(_ptr(hist), len(hist) - 1, int(k), float(C_), float(eps32), float(eps64)))
 
 
 def select_uz(policy: _Policy, nu: float) -> int:

@@ -21,6 +21,7 @@
 //                                     (:245-253) and the indicators (4.9)/(4.10) (:359-366)
 //                                     and (4.11) (:370-375).  x, all inner products, norms
 //                                     and scalars are FP64.
+//   orc_eta_posteriori                the a-posteriori indicator eta_hat_m(k) of (4.7) (:350-354).
 //
 // Low-precision STORAGE is emulated by explicit rounding: every vector is a double array that
 // holds values exactly representable in its storage format.  Readings of the garbled or
@@ -163,6 +164,17 @@ struct orc_stats {
 // scal = {rho, beta, gamma, alpha, delta_k, delta_{k+1}, omega, eta_k, u_r, u_z}
 typedef void (*orc_trace_fn)(int32_t k, const double* x, const double* r, const double* z,
                              const double* p, const double* q, const double* scal, void* user);
+
+// A-posteriori attainable-accuracy indicator eta_hat_m(k), PAPER.md:350-354 (4.7), written out as
+// the two sums of its definition for one k (m = final iteration index, hist[t] = ||r_t||, t = 0..m):
+//   sum_{t=0}^{k} eps64 ((3+C)||r_{t-1}|| + (2+C)||r_t||) + sum_{t=k}^{m} eps32 ((3+C)||r_{t-1}|| + (2+C)||r_t||)
+// Reading R2: ||r_{-1}|| is taken as ||r_0||.  Diagnostic only (needs the whole history).
+double orc_eta_posteriori(const double* hist, int32_t m, int32_t k, double C, double eps32, double eps64) {
+  double s64 = 0.0, s32 = 0.0;
+  for (int32_t t = 0; t <= k; ++t) s64 += eps64 * ((3.0 + C) * hist[t > 0 ? t - 1 : 0] + (2.0 + C) * hist[t]);
+  for (int32_t t = k; t <= m; ++t) s32 += eps32 * ((3.0 + C) * hist[t > 0 ? t - 1 : 0] + (2.0 + C) * hist[t]);
+  return s64 + s32;
+}
 
 // eta_k, PAPER.md:361-362 (4.9) and :372-373 (4.11).  hist[t] = ||r_t||, t = 0..k.
 // Reading R2: for t < 0 the norm is taken as ||r_0||.

@@ -22,6 +22,7 @@ EXPORTED_SYMBOLS = (
     "amp_policy_default", "amp_pcg_create", "amp_pcg_solve", "amp_pcg_solve_host", "amp_spmv",
     "amp_pcg_residual_history", "amp_pcg_set_stream", "amp_pcg_last_launch_count", "amp_pcg_destroy",
     "amp_pcg_last_error", "amp_pcg_bytes_per_row", "amp_pcg_spmv_bytes", "amp_pcg_iteration_bytes",
+    "amp_pcg_eta_posteriori",
 )
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
@@ -108,6 +109,8 @@ def load_library():
     L.amp_pcg_last_error.argtypes = []
     L.amp_pcg_bytes_per_row.restype = dbl
     L.amp_pcg_bytes_per_row.argtypes = [dbl, C.c_int, C.c_int]
+    L.amp_pcg_eta_posteriori.restype = i32
+    L.amp_pcg_eta_posteriori.argtypes = [vp, dbl, dbl, vp, i32]
     L.amp_pcg_spmv_bytes.restype = dbl
     L.amp_pcg_spmv_bytes.argtypes = [vp, C.c_int, C.c_int]
     L.amp_pcg_iteration_bytes.restype = dbl
@@ -217,6 +220,14 @@ class AmpPcg:
 
     def last_launch_count(self) -> int:
         return int(load_library().amp_pcg_last_launch_count(self._h))
+
+    def eta_posteriori(self, C_: float = 1.0, eps32: float = 0.0) -> np.ndarray:
+        """amp_pcg_eta_posteriori: eta_hat_m(k), k = 0..iters, of the last solve (host numpy array)."""
+        buf = np.empty(max(self._last_iters + 1, 1), dtype=np.float64)
+        m = load_library().amp_pcg_eta_posteriori(self._h, float(C_), float(eps32), buf.ctypes.data, buf.size)
+        if m < 0:
+            raise AmpPcgError(_last_error())
+        return buf[:m]
 
     def spmv_bytes(self, mat_prec: int, vec_prec: int) -> float:
         """amp_pcg_spmv_bytes: compulsory bytes of one mat-vec with the matrix format this handle built."""

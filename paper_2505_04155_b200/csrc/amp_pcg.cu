@@ -616,3 +616,28 @@ extern "C" int32_t amp_pcg_residual_history(amp_pcg_t* h, double* out_host, int3
   CU_TRY(cudaStreamSynchronize(h->stream), return AMP_ERR_CUDA);
   return m;
 }
+
+// eta_hat_m(k), k = 0..m, of (4.7) from the residual-norm history of the last solve: with
+// c_t = (3+C)||r_{t-1}|| + (2+C)||r_t|| (||r_{-1}|| := ||r_0||, reading R2), eta_hat_m(k) = eps64 * (c_0 + .. + c_k) +
+// eps32 * (c_k + .. + c_m): one prefix and one suffix sum on the host.  Diagnostic post-processing, not on the hot path.
+extern "C" int32_t amp_pcg_eta_posteriori(amp_pcg_t* h, double C, double eps32, double* out_host, int32_t count) {
+  g_last_error.clear();
+  if (!h || !out_host || count < 0 || !(C >= 0.0) || !(eps32 >= 0.0)) { set_error("amp_pcg_eta_posteriori: invalid argument"); return AMP_ERR_INVALID; }
+  if (h->last_iters < 0 || !h->hist) return 0;
+  if (eps32 == 0.0) eps32 = std::ldexp(1.0, -24);
+  const double eps64 = std::ldexp(1.0, -53);
+  const int32_t m = h->last_iters;
+  std::vector<double> hist((size_t)m + 1), c((size_t)m + 1), suffix((size_t)m + 2, 0.0);
+  CU_TRY(cudaSetDevice(h->device), return AMP_ERR_CUDA);
+  CU_TRY(cudaMemcpyAsync(hist.data(), h->hist, sizeof(double) * hist.size(), cudaMemcpyDeviceToHost, h->stream), return AMP_ERR_CUDA);
+  CU_TRY(cudaStreamSynchronize(h->stream), return AMP_ERR_CUDA);
+  for (int32_t t = 0; t <= m; ++t) c[(size_t)t] = (3.0 + C) * hist[(size_t)(t > 0 ? t - 1 : 0)] + (2.0 + C) * hist[(size_t)t];
+  for (int32_t t = m; t >= 0; --t) suffix[(size_t)t] = suffix[(size_t)t + 1] + c[(size_t)t];
+  const int32_t nout = std::min<int32_t>(count, m + 1);
+  double prefix = 0.0;
+  for (int32_t k = 0; k < nout; ++k) {
+    prefix += c[(size_t)k];
+    out_host[k] = eps64 * prefix + eps32 * suffix[(size_t)k];
+  }
+  return nout;
+}
