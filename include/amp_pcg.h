@@ -45,7 +45,12 @@ enum {
   AMP_SCALE_NORM2 = 0, /* omega = 1/||r_k||                 (Algorithm 4.1 line 4) — default */
   AMP_SCALE_RMS = 1,   /* omega = sqrt(n)/||r_k||            */
   AMP_SCALE_POW2 = 2,  /* omega = 2^round(log2(1/||r_k||))   (exact scaling) */
-  AMP_SCALE_NONE = 3   /* omega = 1                          (diagnostic: naive low precision) */
+  AMP_SCALE_NONE = 3,  /* omega = 1                          (diagnostic: naive low precision) */
+  AMP_SCALE_LAGGED = 4 /* omega_k = 1/||r_{k-1}|| (omega_0 = 1/||r_0||) AND the selector (4.1)/(4.10) of iteration k
+                          evaluated with the norms up to ||r_{k-1}||: every decision of iteration k is known one
+                          iteration early, so z_{k+1} and rho_{k+1} are produced in the pass that updates x and r —
+                          three kernels and reductions per iteration instead of four.  Same iterates in exact
+                          arithmetic (Theorem 3.2); switch iterations move by +1.  Graph and stream loops only. */
 };
 /* how the iteration loop is driven (execution choice; does not change the arithmetic) */
 enum {

@@ -21,7 +21,7 @@ _LIB = os.path.join(_HERE, "liboracle_amp_pcg.so")
 
 FP64, FP32, FP16 = 0, 1, 2
 ETA_DELAY, ETA_LINEAR, ETA_NEVER = 0, 1, 2
-SCALE_NORM2, SCALE_RMS, SCALE_POW2, SCALE_NONE = 0, 1, 2, 3
+SCALE_NORM2, SCALE_RMS, SCALE_POW2, SCALE_NONE, SCALE_LAGGED = 0, 1, 2, 3, 4
 PRECOND_NONE, PRECOND_JACOBI = 0, 1
 
 

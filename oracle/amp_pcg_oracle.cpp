@@ -135,7 +135,7 @@ void orc_spmv_fp32(int64_t n, const int32_t* rowptr, const int32_t* colidx, cons
 // ---------------------------------------------------------------- policy / stats ----------
 enum { ORC_FP64 = 0, ORC_FP32 = 1, ORC_FP16 = 2 };
 enum { ORC_ETA_DELAY = 0, ORC_ETA_LINEAR = 1, ORC_ETA_NEVER = 2 };
-enum { ORC_SCALE_NORM2 = 0, ORC_SCALE_RMS = 1, ORC_SCALE_POW2 = 2, ORC_SCALE_NONE = 3 };
+enum { ORC_SCALE_NORM2 = 0, ORC_SCALE_RMS = 1, ORC_SCALE_POW2 = 2, ORC_SCALE_NONE = 3, ORC_SCALE_LAGGED = 4 };
 
 struct orc_policy {
   int32_t amp;              // 0: Algorithm 3.1 literally; 1: Algorithm 4.1
@@ -210,6 +210,7 @@ int32_t orc_select_uz(const orc_policy* pol, double nu) {
 static double scale_factor(const orc_policy* pol, double delta, int64_t n) {
   switch (pol->scale_mode) {
     case ORC_SCALE_NORM2: return 1.0 / delta;                               // Alg 4.1 line 4
+    case ORC_SCALE_LAGGED: return 1.0 / delta;                              // called with ||r_{k-1}|| (see the loop)
     case ORC_SCALE_RMS:   return std::sqrt((double)n) / delta;
     case ORC_SCALE_POW2:  return std::ldexp(1.0, (int)std::nearbyint(std::log2(1.0 / delta)));
     default:              return 1.0;
@@ -257,6 +258,9 @@ int32_t orc_amp_pcg(int64_t n, const int32_t* rowptr, const int32_t* colidx, con
   hist[0] = delta;
   int32_t ur = ORC_FP64, uz = pol->amp ? pol->u0 : ORC_FP64;
   double rho_prev = 0.0;
+  const bool lag = pol->amp && pol->scale_mode == ORC_SCALE_LAGGED;
+  int32_t ur_n = ur, uz_n = uz;   // lagged variant: decisions for the next iteration
+  double omega_n = 1.0;
   int32_t k = 0, status = 1;
   if (nb == 0.0) {                          // R13: b = 0 -> x = 0
     for (int64_t i = 0; i < n; ++i) x[i] = 0.0;
@@ -267,7 +271,8 @@ int32_t orc_amp_pcg(int64_t n, const int32_t* rowptr, const int32_t* colidx, con
 
   for (k = 0; k < maxit; ++k) {
     double eta = std::numeric_limits<double>::infinity();
-    if (pol->amp) {
+    double omega_lag = 1.0;
+    if (pol->amp && !lag) {
       // O1: eta_k and the precision selector (4.1), Alg 4.1 line 3.
       // Reading R5: both switches are latched (precision never goes back up).
       eta = orc_eta(pol, hist.data(), k);
@@ -283,9 +288,36 @@ int32_t orc_amp_pcg(int64_t n, const int32_t* rowptr, const int32_t* colidx, con
         if (uz == ORC_FP16 && st->it_uz16 < 0) st->it_uz16 = k;
         for (int64_t i = 0; i < n; ++i) p[(size_t)i] = round_store(p[(size_t)i], uz);   // R9
       }
+    } else if (pol->amp) {
+      // Lagged variant (reading R17): lines 3 and 4 of Alg 4.1 for iteration k are evaluated with
+      // ||r_{k-1}|| instead of ||r_k|| ("other scaling factors can be used"; Thm 3.2), i.e. the
+      // decisions D(k) = (u_r, u_z, omega) of iteration k were taken one iteration earlier, from hist[0..k-1]
+      // (k = 0: from hist[0]).  r_k was therefore already stored in u_r,k by line 16 of iteration k-1.
+      auto decide = [&](int32_t t) {  // D(t+1) from hist[0..t]
+        const double e = orc_eta(pol, hist.data(), t);
+        ur_n = (ur == ORC_FP32 || e <= pol->eta_safety * tol * nb) ? ORC_FP32 : ORC_FP64;
+        const int32_t want = orc_select_uz(pol, hist[(size_t)t] / nb);
+        uz_n = want > uz ? want : uz;
+        omega_n = scale_factor(pol, hist[(size_t)t], n);
+        return e;
+      };
+      if (k == 0) decide(0);
+      if (ur_n != ur) {
+        ur = ur_n; st->it_ur32 = k;
+        for (int64_t i = 0; i < n; ++i) r[(size_t)i] = orc_round_fp32(r[(size_t)i]);  // only changes r at k = 0
+        if (vals32.empty()) { vals32.resize((size_t)nnz); for (int64_t e = 0; e < nnz; ++e) vals32[(size_t)e] = (float)vals[e]; }
+      }
+      if (uz_n > uz) {
+        uz = uz_n;
+        if (uz >= ORC_FP32 && st->it_uz32 < 0) st->it_uz32 = k;
+        if (uz == ORC_FP16 && st->it_uz16 < 0) st->it_uz16 = k;
+        for (int64_t i = 0; i < n; ++i) p[(size_t)i] = round_store(p[(size_t)i], uz);   // R9
+      }
+      omega_lag = omega_n;
+      eta = decide(k);  // D(k+1)
     }
     // O2: y = omega r, z = M^-1 y  (Alg 4.1 lines 4-5; Alg 3.2 line 3; fused)
-    const double omega = pol->amp ? scale_factor(pol, delta, n) : 1.0;
+    const double omega = !pol->amp ? 1.0 : (lag ? omega_lag : scale_factor(pol, delta, n));
     const double* dv = (uz == ORC_FP64) ? dinv.data() : dinv32.data();            // R6
     int64_t c_inf = 0, c_flush = 0, c_sub = 0;
 #pragma omp parallel for schedule(static) reduction(+ : c_inf, c_flush, c_sub)
@@ -326,7 +358,7 @@ int32_t orc_amp_pcg(int64_t n, const int32_t* rowptr, const int32_t* colidx, con
 #pragma omp parallel for schedule(static)
     for (int64_t i = 0; i < n; ++i) {
       x[i] = std::fma(alpha, p[(size_t)i], x[i]);
-      r[(size_t)i] = round_store(std::fma(-alpha, q[(size_t)i], r[(size_t)i]), ur);
+      r[(size_t)i] = round_store(std::fma(-alpha, q[(size_t)i], r[(size_t)i]), lag ? ur_n : ur);
     }
     // O11: delta_{k+1} = ||r_{k+1}|| (line 17)
     const double delta_k = delta;

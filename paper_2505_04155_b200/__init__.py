@@ -15,7 +15,7 @@ from .binding import (  # noqa: F401
     library_path,
     FP64, FP32, FP16,
     ETA_DELAY, ETA_LINEAR, ETA_NEVER,
-    SCALE_NORM2, SCALE_RMS, SCALE_POW2, SCALE_NONE,
+    SCALE_NORM2, SCALE_RMS, SCALE_POW2, SCALE_NONE, SCALE_LAGGED,
     LOOP_AUTO, LOOP_STREAM, LOOP_GRAPH, LOOP_PERSISTENT,
     PRECOND_NONE, PRECOND_JACOBI,
     EXPORTED_SYMBOLS,

@@ -14,7 +14,7 @@ import numpy as np
 
 FP64, FP32, FP16 = 0, 1, 2
 ETA_DELAY, ETA_LINEAR, ETA_NEVER = 0, 1, 2
-SCALE_NORM2, SCALE_RMS, SCALE_POW2, SCALE_NONE = 0, 1, 2, 3
+SCALE_NORM2, SCALE_RMS, SCALE_POW2, SCALE_NONE, SCALE_LAGGED = 0, 1, 2, 3, 4
 LOOP_AUTO, LOOP_STREAM, LOOP_GRAPH, LOOP_PERSISTENT = 0, 1, 2, 3
 PRECOND_NONE, PRECOND_JACOBI = 0, 1
 

@@ -52,6 +52,11 @@ struct amp_pcg {
   cudaGraph_t graph = nullptr;
   cudaGraphExec_t graph_exec = nullptr;
   cudaGraphConditionalHandle cond{};
+  // graph loop of the lagged variant (k_p, k_spmv, k_xrz)
+  cudaGraph_t graph_lag = nullptr;
+  cudaGraphExec_t graph_lag_exec = nullptr;
+  cudaGraphConditionalHandle cond_lag{};
+  int grid_xrz = 1;
   // host-buffer staging for amp_pcg_solve_host
   double* d_b_stage = nullptr;
   double* d_x_stage = nullptr;
@@ -122,6 +127,8 @@ extern "C" void amp_pcg_destroy(amp_pcg_t* h) {
   cudaStreamSynchronize(h->stream);
   if (h->graph_exec) cudaGraphExecDestroy(h->graph_exec);
   if (h->graph) cudaGraphDestroy(h->graph);
+  if (h->graph_lag_exec) cudaGraphExecDestroy(h->graph_lag_exec);
+  if (h->graph_lag) cudaGraphDestroy(h->graph_lag);
   for (void* p : h->owned) cudaFree(p);
   if (h->hist) cudaFree(h->hist);
   if (h->h_state) cudaFreeHost(h->h_state);
@@ -360,6 +367,7 @@ extern "C" amp_pcg_t* amp_pcg_create(int64_t n, int64_t nnz, const int32_t* rowp
   h->grid_z = vec_grid_for((const void*)k_z);
   h->grid_p = vec_grid_for((const void*)k_p);
   h->grid_xr = vec_grid_for((const void*)k_xr);
+  h->grid_xrz = vec_grid_for((const void*)k_xrz);
   h->vec_grid = vec_grid_for((const void*)k_setup);
 #undef ALLOC
   return h;
@@ -434,45 +442,58 @@ static cudaError_t launch_iteration(amp_pcg* h, const Ctx& c, cudaStream_t s, bo
   return e;
 }
 
+// lagged variant: three kernels per iteration (z_0 comes from one k_z before the loop)
+static cudaError_t launch_iteration_lagged(amp_pcg* h, const Ctx& c, cudaStream_t s, bool pdl) {
+  cudaError_t e = launch_loop_kernel(k_p, h->grid_p, kVecThreads, s, c, false);
+  if (e == cudaSuccess) e = launch_loop_kernel(k_spmv, h->spmv_grid, kSpmvThreads, s, c, pdl);
+  if (e == cudaSuccess) e = launch_loop_kernel(k_xrz, h->grid_xrz, kVecThreads, s, c, pdl);
+  return e;
+}
+
 // One graph = one WHILE conditional node whose body is the four loop kernels; the condition is
 // written from the device by epi_delta / epi_gamma, so a whole solve is a single launch.
-static int build_graph_once(amp_pcg* h, bool pdl) {
-  CU_TRY(cudaGraphCreate(&h->graph, 0), return AMP_ERR_CUDA);
-  CU_TRY(cudaGraphConditionalHandleCreate(&h->cond, h->graph, 1, cudaGraphCondAssignDefault), return AMP_ERR_CUDA);
+static int build_graph_once(amp_pcg* h, bool pdl, bool lagged) {
+  cudaGraph_t& graph = lagged ? h->graph_lag : h->graph;
+  cudaGraphExec_t& graph_exec = lagged ? h->graph_lag_exec : h->graph_exec;
+  cudaGraphConditionalHandle& cond = lagged ? h->cond_lag : h->cond;
+  CU_TRY(cudaGraphCreate(&graph, 0), return AMP_ERR_CUDA);
+  CU_TRY(cudaGraphConditionalHandleCreate(&cond, graph, 1, cudaGraphCondAssignDefault), return AMP_ERR_CUDA);
   cudaGraphNodeParams np = {};
   np.type = cudaGraphNodeTypeConditional;
-  np.conditional.handle = h->cond;
+  np.conditional.handle = cond;
   np.conditional.type = cudaGraphCondTypeWhile;
   np.conditional.size = 1;
   cudaGraphNode_t node;
-  CU_TRY(cudaGraphAddNode(&node, h->graph, nullptr, 0, &np), return AMP_ERR_CUDA);
+  CU_TRY(cudaGraphAddNode(&node, graph, nullptr, 0, &np), return AMP_ERR_CUDA);
   cudaGraph_t body = np.conditional.phGraph_out[0];
   cudaStream_t cap;
   CU_TRY(cudaStreamCreateWithFlags(&cap, cudaStreamNonBlocking), return AMP_ERR_CUDA);
   Ctx c = h->ctx;
-  c.cond = h->cond;
+  c.cond = cond;
   c.use_cond = 1;
   cudaError_t e = cudaStreamBeginCaptureToGraph(cap, body, nullptr, nullptr, 0, cudaStreamCaptureModeRelaxed);
   if (e == cudaSuccess) {
-    const cudaError_t el = launch_iteration(h, c, cap, pdl);
+    const cudaError_t el = lagged ? launch_iteration_lagged(h, c, cap, pdl) : launch_iteration(h, c, cap, pdl);
     e = cudaStreamEndCapture(cap, nullptr);
     if (e == cudaSuccess) e = el;
   }
   cudaStreamDestroy(cap);
   if (e != cudaSuccess) { set_error("graph capture failed: %s", cudaGetErrorString(e)); cudaGetLastError(); return AMP_ERR_CUDA; }
-  CU_TRY(cudaGraphInstantiate(&h->graph_exec, h->graph, 0), { cudaGetLastError(); return AMP_ERR_CUDA; });
+  CU_TRY(cudaGraphInstantiate(&graph_exec, graph, 0), { cudaGetLastError(); return AMP_ERR_CUDA; });
   return AMP_OK;
 }
 
-static int build_graph(amp_pcg* h) {
-  if (h->graph_exec) return AMP_OK;
+static int build_graph(amp_pcg* h, bool lagged) {
+  cudaGraph_t& graph = lagged ? h->graph_lag : h->graph;
+  cudaGraphExec_t& graph_exec = lagged ? h->graph_lag_exec : h->graph_exec;
+  if (graph_exec) return AMP_OK;
   h->pdl = getenv("AMP_NO_PDL") ? 0 : 1;  // tuning aid
-  int rc = build_graph_once(h, h->pdl != 0);
+  int rc = build_graph_once(h, h->pdl != 0, lagged);
   if (rc != AMP_OK && h->pdl) {  // programmatic edges not accepted inside the conditional body: plain edges
-    if (h->graph_exec) { cudaGraphExecDestroy(h->graph_exec); h->graph_exec = nullptr; }
-    if (h->graph) { cudaGraphDestroy(h->graph); h->graph = nullptr; }
+    if (graph_exec) { cudaGraphExecDestroy(graph_exec); graph_exec = nullptr; }
+    if (graph) { cudaGraphDestroy(graph); graph = nullptr; }
     h->pdl = 0;
-    rc = build_graph_once(h, false);
+    rc = build_graph_once(h, false, lagged);
   }
   return rc;
 }
@@ -489,7 +510,7 @@ static int solve_impl(amp_pcg* h, const double* b, double* x, double tol, int32_
   if (pol.stop_safety == 0.0) pol.stop_safety = 1.0;
   if (pol.C == 0.0 && !policy) pol.C = 1.0;
   if (!(tol > 0.0) || maxit < 1 || maxit > (1 << 24) || !aligned16(b) || !aligned16(x) || pol.u0 < 0 || pol.u0 > 2 ||
-      pol.eta_rule < 0 || pol.eta_rule > 2 || pol.scale_mode < 0 || pol.scale_mode > 3 || pol.d < 1 || pol.d > kMaxWindow ||
+      pol.eta_rule < 0 || pol.eta_rule > 2 || pol.scale_mode < 0 || pol.scale_mode > 4 || pol.d < 1 || pol.d > kMaxWindow ||
       pol.ell < 1 || pol.ell > kMaxWindow || pol.loop_mode < 0 || pol.loop_mode > 3 || !(pol.tau_zs >= 0.0) ||
       !(pol.tau_zh >= 0.0) || !(pol.eps32 > 0.0) || !(pol.eta_safety > 0.0) || !(pol.stop_safety > 0.0)) {
     set_error("amp_pcg_solve: invalid tol/maxit/policy or misaligned b/x");
@@ -508,12 +529,17 @@ static int solve_impl(amp_pcg* h, const double* b, double* x, double tol, int32_
   // measured on B200 (us per iteration, persistent vs graph): n = 4 K 17 vs 23, 16 K 19.6 vs 24.0, 262 K 20.9 vs 29.0,
   // 512 K 25.0 vs 32.1, 2.1 M (c2) 58 vs 57, 4.1 M (c3) 95 vs 92: the persistent kernel wins while the iteration is
   // latency-bound; from c2 up the graph loop wins because each of its kernels has its own register budget
-  if (mode == AMP_LOOP_AUTO) mode = (h->persist_ok && h->n <= kPersistAutoMaxRows) ? AMP_LOOP_PERSISTENT : AMP_LOOP_GRAPH;
+  const bool lagged = pol.amp && pol.scale_mode == AMP_SCALE_LAGGED;
+  if (mode == AMP_LOOP_AUTO) mode = (!lagged && h->persist_ok && h->n <= kPersistAutoMaxRows) ? AMP_LOOP_PERSISTENT : AMP_LOOP_GRAPH;
+  if (lagged && mode == AMP_LOOP_PERSISTENT) {
+    set_error("amp_pcg_solve: AMP_SCALE_LAGGED runs in the graph and stream loops only");
+    return AMP_ERR_INVALID;
+  }
   if (mode == AMP_LOOP_PERSISTENT && !(h->persist_ok && persistent_fits(h->ctx))) {
     set_error("amp_pcg_solve: persistent loop not available for this problem/device");
     return AMP_ERR_INVALID;
   }
-  if (mode == AMP_LOOP_GRAPH) { const int rc = build_graph(h); if (rc != AMP_OK) return rc; }
+  if (mode == AMP_LOOP_GRAPH) { const int rc = build_graph(h, lagged); if (rc != AMP_OK) return rc; }
 
   DevState* hs = h->h_state;
   std::memset(hs, 0, sizeof(DevState));
@@ -533,8 +559,12 @@ static int solve_impl(amp_pcg* h, const double* b, double* x, double tol, int32_
   k_setup<<<h->vec_grid, kVecThreads, 0, st>>>(h->ctx, pol.x0_zero ? 1 : 0);
   h->launches += 1;
 
+  if (lagged) {  // z_0, rho_0 for the first pass of the three-kernel loop
+    k_z<<<h->grid_z, kVecThreads, 0, st>>>(h->ctx);
+    h->launches += 1;
+  }
   if (mode == AMP_LOOP_GRAPH) {
-    CU_TRY(cudaGraphLaunch(h->graph_exec, st), return AMP_ERR_CUDA);
+    CU_TRY(cudaGraphLaunch(lagged ? h->graph_lag_exec : h->graph_exec, st), return AMP_ERR_CUDA);
   } else if (mode == AMP_LOOP_PERSISTENT) {
     const int rc = persistent_launch(h->ctx, h->persist_grid, st);
     if (rc != 0) { set_error("persistent kernel launch failed: %s", cudaGetErrorString((cudaError_t)rc)); return AMP_ERR_CUDA; }
@@ -543,7 +573,10 @@ static int solve_impl(amp_pcg* h, const double* b, double* x, double tol, int32_
     int done_iters = 0;
     while (done_iters < maxit) {
       const int nb = std::min(batch, maxit - done_iters);
-      for (int i = 0; i < nb; ++i) launch_iteration(h, h->ctx, st, getenv("AMP_NO_PDL") == nullptr);
+      for (int i = 0; i < nb; ++i) {
+        if (lagged) launch_iteration_lagged(h, h->ctx, st, getenv("AMP_NO_PDL") == nullptr);
+        else launch_iteration(h, h->ctx, st, getenv("AMP_NO_PDL") == nullptr);
+      }
       done_iters += nb;
       CU_TRY(cudaMemcpyAsync(h->h_flag, &h->ctx.st->done, sizeof(int), cudaMemcpyDeviceToHost, st), return AMP_ERR_CUDA);
       CU_TRY(cudaStreamSynchronize(st), return AMP_ERR_CUDA);
@@ -562,7 +595,7 @@ static int solve_impl(amp_pcg* h, const double* b, double* x, double tol, int32_
 
   const int iters = hs->k;
   h->last_iters = iters;
-  h->launches += (mode == AMP_LOOP_PERSISTENT) ? 1 : (int64_t)4 * iters;
+  h->launches += (mode == AMP_LOOP_PERSISTENT) ? 1 : (int64_t)(lagged ? 3 : 4) * iters;
   if (stats) {
     std::memset(stats, 0, sizeof(*stats));
     stats->status = hs->status; stats->iters = iters;
@@ -579,6 +612,7 @@ static int solve_impl(amp_pcg* h, const double* b, double* x, double tol, int32_
       if (hs->it_uz32 >= 0 && k >= hs->it_uz32) uz = std::max(uz, (int)AMP_FP32);
       if (hs->it_uz16 >= 0 && k >= hs->it_uz16) uz = AMP_FP16;
       bytes += amp_pcg_iteration_bytes(h, uz, ur);
+      if (lagged) bytes -= (double)h->n * ((ur == AMP_FP64) ? 8.0 : 4.0);  // r is not read a second time
     }
     stats->algorithmic_bytes = bytes;
     stats->fp16_subnormal = hs->fp16_subnormal; stats->fp16_flushed = hs->fp16_flushed; stats->fp16_inf = hs->fp16_inf;

@@ -39,6 +39,9 @@ struct DevState {
   int32_t ur, uz;          // precisions selected for iteration k by (4.1)
   int32_t r_store, p_store;  // precisions r and p are currently stored in
   int32_t it_ur32, it_uz32, it_uz16, pad0;
+  // lagged variant (AMP_SCALE_LAGGED): decisions already taken for the NEXT iteration
+  int32_t ur_n, uz_n;
+  double omega_n;
   unsigned int counter[4];  // last-block tickets of the three reductions (+ setup)
   unsigned long long fp16_subnormal, fp16_flushed, fp16_inf;
   // ---- grid barrier of the persistent kernel ----
@@ -258,6 +261,34 @@ __device__ __forceinline__ void grid_reduce(double v, double* partials, unsigned
     if (threadIdx.x == 0) {
       *counter = 0u;
       epi(tot);
+    }
+  }
+}
+
+// the same for two sums at once (partials interleaved: [2*bid], [2*bid+1])
+template <int NT, class Epi>
+__device__ __forceinline__ void grid_reduce2(double v0, double v1, double* partials, unsigned int* counter, int bid, int nb,
+                                             double* sm, Epi epi) {
+  __shared__ int s_last2;
+  const double b0 = block_sum<NT>(v0, sm);
+  const double b1 = block_sum<NT>(v1, sm);
+  if (threadIdx.x == 0) {
+    __stcg(partials + 2 * bid, b0);
+    __stcg(partials + 2 * bid + 1, b1);
+    __threadfence();
+    const unsigned int t = atomicAdd(counter, 1u);
+    s_last2 = (t == (unsigned int)nb - 1u);
+  }
+  __syncthreads();
+  if (s_last2) {
+    __threadfence();
+    double s0 = 0.0, s1 = 0.0;
+    for (int i = threadIdx.x; i < nb; i += NT) { s0 += __ldcg(partials + 2 * i); s1 += __ldcg(partials + 2 * i + 1); }
+    const double t0 = block_sum<NT>(s0, sm);
+    const double t1 = block_sum<NT>(s1, sm);
+    if (threadIdx.x == 0) {
+      *counter = 0u;
+      epi(t0, t1);
     }
   }
 }

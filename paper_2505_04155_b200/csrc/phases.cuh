@@ -80,6 +80,9 @@ __device__ __noinline__ void select_precisions(DevState* s, int64_t n) {
   s->omega = om;
 }
 
+__device__ void decide_next(DevState* s, int t);
+__device__ __forceinline__ void apply_next(DevState* s);
+
 // after the setup reduction: ||b||, delta_0 = ||r_0||, edge cases, selector for k = 0
 __device__ __noinline__ void epi_setup(const EpiCtx c, double bb, double rr) {
   DevState* s = c.st;
@@ -99,6 +102,10 @@ __device__ __noinline__ void epi_setup(const EpiCtx c, double bb, double rr) {
     s->done = 1; s->status = -2;
   } else if (s->delta <= s->stop_safety * s->tol * s->bnorm && !s->no_stop) {
     s->done = 1; s->status = 0;  // x0 already satisfies the stopping test
+  } else if (s->amp && s->scale_mode == 4) {  // lagged: D(0) = D(1) = the decisions from ||r_0||
+    decide_next(s, 0);
+    apply_next(s);
+    s->p_store = s->uz;
   } else {
     select_precisions(s, c.n);
   }
@@ -141,6 +148,80 @@ __device__ __noinline__ void epi_delta(const EpiCtx c, double rr) {
     s->status = 1; s->done = 1;
   } else {
     select_precisions(s, c.n);  // line 3 of the next iteration
+  }
+  set_loop_cond(c, !s->done);
+}
+
+// ------------------------------------------------------------------ lagged variant ----------
+// AMP_SCALE_LAGGED (reading R17): lines 3 and 4 of Alg 4.1 for iteration k are evaluated with
+// ||r_{k-1}|| instead of ||r_k|| (other scaling factors are allowed: Thm 3.2).  The decisions
+// D(k) = (u_r, u_z, omega) of iteration k are then known one iteration early, so z_{k+1} and rho_{k+1} can be
+// produced in the same pass that updates x and r (k_xrz): three kernels and three grid-wide reductions per iteration
+// instead of four, and r is not read again.
+// decide D(t+1) from hist[0..t] into (ur_n, uz_n, omega_n)
+__device__ __noinline__ void decide_next(DevState* s, int t) {
+  const double* hist = s->hist;
+  int ur_n = s->ur;
+  if (ur_n == P64 && s->eta_rule != 2) {
+    double eta = CUDART_INF;
+    const double C = s->C, e32 = s->eps32;
+    if (s->eta_rule == 0) {  // (4.9)
+      eta = 0.0;
+      for (int u = t - s->d; u <= t; ++u) {
+        const double hm1 = hist[(u - 1) > 0 ? (u - 1) : 0], h0 = hist[u > 0 ? u : 0];
+        eta += e32 * ((3.0 + C) * hm1 + (2.0 + C) * h0);
+      }
+    } else {  // (4.11)
+      const int l = s->ell;
+      if (t >= l && hist[t] < hist[t - l]) {
+        const double rate = pow(hist[t] / hist[t - l], 1.0 / (double)l);
+        eta = e32 * (5.0 + 2.0 * C) * hist[t - 1] / (1.0 - rate);
+      }
+    }
+    if (eta <= s->eta_safety * s->tol * s->bnorm) ur_n = P32;  // (4.10)
+  }
+  const double nu = hist[t] / s->bnorm;
+  int want = s->u0;
+  if (nu < s->tau_zs) want = lower_prec(s->u0, nu >= s->tau_zh ? P32 : P16);
+  s->ur_n = ur_n;
+  s->uz_n = want > s->uz ? want : s->uz;
+  s->omega_n = 1.0 / hist[t];
+}
+
+// make D(k) current (k = s->k) and record the switch iterations
+__device__ __forceinline__ void apply_next(DevState* s) {
+  const int k = s->k;
+  if (s->ur_n != s->ur) { s->ur = s->ur_n; s->it_ur32 = k; }
+  if (s->uz_n > s->uz) {
+    s->uz = s->uz_n;
+    if (s->uz >= P32 && s->it_uz32 < 0) s->it_uz32 = k;
+    if (s->uz == P16 && s->it_uz16 < 0) s->it_uz16 = k;
+  }
+  s->omega = s->omega_n;
+}
+
+// after k_xrz of iteration k: rr = ||r_{k+1}||^2, rz = r_{k+1}^T z_{k+1}
+__device__ __noinline__ void epi_delta_lagged(const EpiCtx c, double rr, double rz) {
+  DevState* s = c.st;
+  const double delta = sqrt(rr);
+  const int k1 = s->k + 1;
+  s->delta = delta;
+  s->hist[k1] = delta;
+  s->rho_prev = s->rho;
+  s->rho = rz;
+  s->beta = rz / s->rho_prev;
+  s->k = k1;
+  s->p_store = s->uz;   // p_k is stored in u_z,k
+  apply_next(s);        // D(k+1) becomes current; r_{k+1} and z_{k+1} were stored in it
+  s->r_store = s->ur;
+  if (!(delta == delta) || isinf(delta)) {
+    s->status = -2; s->done = 1;
+  } else if (delta <= s->stop_safety * s->tol * s->bnorm && !s->no_stop) {
+    s->status = 0; s->done = 1;
+  } else if (k1 >= s->maxit) {
+    s->status = 1; s->done = 1;
+  } else {
+    decide_next(s, k1);  // D(k+2)
   }
   set_loop_cond(c, !s->done);
 }
@@ -355,6 +436,96 @@ __device__ __forceinline__ double phase_xr(const Ctx& c, const double alpha, dou
     }
   }
   return sum;
+}
+
+// ------------------------------------------------------------------ lagged: a5 + a2 in one pass
+// x += alpha p (FP64); r <- RN_{URN}(r - alpha q); delta^2 += r^2; z = RN_{UZN}((r omega_n) dinv); rho += r z.
+// UR / UZ: precisions of iteration k (q, r as read, p); URN / UZN: of iteration k+1 (r as written, z).
+template <int UR, int URN, int UZ, int UZN, int BIF = kVecBytesInFlight>
+__device__ __forceinline__ void phase_xrz(const Ctx& c, const double alpha, const double omega_n, double* x, int bid, int nb,
+                                          double& sum_rr, double& sum_rz) {
+  using TP = typename Store<UZ>::T;
+  using TR = typename Store<UR>::T;
+  using TO = typename Store<URN>::T;
+  using TZ = typename Store<UZN>::T;
+  using TD = typename Store<(UZN == P64) ? P64 : P32>::T;
+  constexpr int smin = cmin(cmin((int)sizeof(TP), (int)sizeof(TR)), cmin((int)sizeof(TO), (int)sizeof(TZ)));
+  constexpr int E = chunk_elems(smin, 8);
+  constexpr int U = cmax(1, BIF / (E * (int)(8 + sizeof(TP) + 2 * sizeof(TR) + sizeof(TD))));
+  const TP* p = pvec<UZ>(c);
+  const TR* q = qvec<UR>(c);
+  const TR* rin = rvec<UR>(c);
+  TO* rout = rvec<URN>(c);
+  TZ* z = zvec<UZN>(c);
+  const TD* dinv;
+  if constexpr (UZN == P64) dinv = c.dinv64; else dinv = c.dinv32;
+  const int64_t n = c.n;
+  const int64_t nchunk = c.npad / E;
+  const int64_t stride = (int64_t)nb * blockDim.x;
+  double srr = 0.0, srz = 0.0;
+  for (int64_t base = (int64_t)bid * blockDim.x + threadIdx.x; base < nchunk; base += stride * U) {
+    Chunk<double, E> xx[U];
+    Chunk<TP, E> pp[U];
+    Chunk<TR, E> qq[U], rr[U];
+    Chunk<TD, E> dd[U];
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      const int64_t i = base + u * stride;
+      if (i < nchunk) {
+        if ((i + 1) * E <= n) {
+          chunk_load(xx[u], x, i);
+        } else {  // x is caller-owned: exactly n long
+          double t[E];
+#pragma unroll
+          for (int e = 0; e < E; ++e) t[e] = (i * E + e < n) ? x[i * E + e] : 0.0;
+          chunk_pack(xx[u], t);
+        }
+        chunk_load(pp[u], p, i);
+        chunk_load(qq[u], q, i);
+        chunk_load(rr[u], rin, i);
+        chunk_load(dd[u], dinv, i);
+      }
+    }
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      const int64_t i = base + u * stride;
+      if (i < nchunk) {
+        double xv[E], pv[E], qv[E], rv[E], dv[E], zv[E];
+        chunk_unpack(xx[u], xv);
+        chunk_unpack(pp[u], pv);
+        chunk_unpack(qq[u], qv);
+        chunk_unpack(rr[u], rv);
+        chunk_unpack(dd[u], dv);
+#pragma unroll
+        for (int e = 0; e < E; ++e) xv[e] = fma(alpha, pv[e], xv[e]);  // line 15, FP64
+        if ((i + 1) * E <= n) {
+          Chunk<double, E> xo;
+          chunk_pack(xo, xv);
+          chunk_store(xo, x, i);
+        } else {
+#pragma unroll
+          for (int e = 0; e < E; ++e)
+            if (i * E + e < n) x[i * E + e] = xv[e];
+        }
+#pragma unroll
+        for (int e = 0; e < E; ++e) rv[e] = fma(-alpha, qv[e], rv[e]);  // line 16
+        Chunk<TO, E> ro;
+        chunk_pack(ro, rv);  // one rounding, to the precision of iteration k+1
+        chunk_store(ro, rout, i);
+        chunk_unpack(ro, rv);
+#pragma unroll
+        for (int e = 0; e < E; ++e) zv[e] = (rv[e] * omega_n) * dv[e];  // lines 4-5 of iteration k+1
+        Chunk<TZ, E> zo;
+        chunk_pack(zo, zv);
+        chunk_store(zo, z, i);
+        chunk_unpack(zo, zv);
+#pragma unroll
+        for (int e = 0; e < E; ++e) { srr = fma(rv[e], rv[e], srr); srz = fma(rv[e], zv[e], srz); }
+      }
+    }
+  }
+  sum_rr = srr;
+  sum_rz = srz;
 }
 
 }  // namespace amp

@@ -193,3 +193,44 @@ def test_edge_cases():
     vals[s.colidx == np.repeat(np.arange(s.n), np.diff(s.rowptr))] = 0.5  # diag 0.5 < row sum: indefinite
     res = O.amp_pcg(s.rowptr, s.colidx, vals, s.b, 1e-10, 500, O.make_policy(amp=0))
     assert res.status == -2
+
+
+def test_theorem_3_2_lagged_scaling():
+    """SCALE_LAGGED (reading R17): omega_k = 1/||r_{k-1}|| is one more admissible scaling of Algorithm 3.2
+    (PAPER.md:223 offers ||z_{k-1}||^-1; Theorem 3.2 holds for any non-zero omega_k): with every vector in FP64 the
+    iterates agree with PCG to rounding, omega_k ||r_{k-1}|| = 1 exactly, and ||y_k|| = ||r_k|| / ||r_{k-1}||."""
+    s = make_config("c3", 10)
+    d = np.diag(s.scipy().toarray())
+    r1, ref = _trace_run(s, O.make_policy(amp=0), tol=1e-10)
+    r2, ds = _trace_run(s, _no_switch_policy(O.SCALE_LAGGED), tol=1e-10)
+    assert abs(r1.iters - r2.iters) <= 1
+    hist = np.asarray(r2.hist)
+    for k in range(min(len(ref), len(ds), 60)):
+        a, b = ref[k], ds[k]
+        assert np.linalg.norm(a["x"] - b["x"]) <= 1e-11 * np.linalg.norm(a["x"])
+        prev = hist[max(k - 1, 0)]
+        assert b["omega"] * prev == pytest.approx(1.0, rel=1e-15)
+        assert np.linalg.norm(b["z"] * d) == pytest.approx(hist[k] / prev, rel=1e-12)
+        assert b["rho"] / b["omega"] == pytest.approx(a["rho"], rel=1e-9)
+
+
+@pytest.mark.parametrize("name,size", [("c1", 48), ("c2", 24), ("c3", 20), ("c4", 16)])
+def test_lagged_decisions_take_effect_one_iteration_later(name, size):
+    """In the lagged variant the selector (4.1) and the indicator (4.9)/(4.10) of iteration k see the norms up to
+    ||r_{k-1}||: on these runs (same residual history to rounding) every switch happens exactly one iteration after the
+    paper's, the iteration count is unchanged and the attainable accuracy (<= 2 tol) is kept."""
+    s = make_config(name, size)
+    for kw in (dict(u0=O.FP64, eta_rule=O.ETA_DELAY), dict(u0=O.FP16, eta_rule=O.ETA_LINEAR)):
+        a = O.amp_pcg(s.rowptr, s.colidx, s.vals, s.b, s.tol, s.maxit, O.make_policy(**kw))
+        b = O.amp_pcg(s.rowptr, s.colidx, s.vals, s.b, s.tol, s.maxit, O.make_policy(scale_mode=O.SCALE_LAGGED, **kw))
+        assert a.status == b.status == 0
+        if kw["u0"] == O.FP64:
+            assert abs(a.iters - b.iters) <= 1
+        else:
+            # z, p in FP16 from the start: ||y_k|| = ||r_k|| / ||r_{k-1}|| < 1 uses less of FP16's range than the paper's
+            # ||y_k|| = 1, which can cost a few iterations on fast-converging small systems (c4 at 16^3: 41 vs 37)
+            assert a.iters - 1 <= b.iters <= 1.15 * a.iters + 1
+        for key in ("it_ur32", "it_uz32", "it_uz16"):
+            va, vb = getattr(a, key), getattr(b, key)
+            assert (va < 0 and vb < 0) or vb == va + 1, (key, va, vb)
+        assert b.relres_true <= 2 * s.tol
