@@ -253,6 +253,16 @@ def run_ours(args, rank: int, local_rank: int, world: int):
     ms64, its64, _, st64 = timed_solves(pol_fp64, max(2, min(args.steps, 3)))
     t_amp = statistics.median(ms) * 1e-3
     t_fp64 = statistics.median(ms64) * 1e-3
+    # ---- the lagged variant (AMP_SCALE_LAGGED, reading R17): same policy, three kernels per iteration ----
+    lagged = None
+    if loop != A.LOOP_PERSISTENT:
+        pol_lag = A.Policy.default(x0_zero=1, loop_mode=loop, scale_mode=A.SCALE_LAGGED, **kw)
+        timed_solves(pol_lag, 1)
+        ms_l, _, _, st_l = timed_solves(pol_lag, max(2, min(args.steps, 3)))
+        t_lag = statistics.median(ms_l) * 1e-3
+        lagged = {"time_to_tol_s": t_lag, "iters": st_l.iters, "iterations_per_s": st_l.iters / t_lag,
+                  "switch_iters": {"ur32": st_l.it_ur32, "uz32": st_l.it_uz32, "uz16": st_l.it_uz16},
+                  "relres_updated": st_l.relres_updated, "speedup_vs_own_fp64": t_fp64 / t_lag}
 
     # ---- roofline of the dominant kernel (SpMV) timed alone with CUDA events ----
     peak, peak_src = peaks()
@@ -313,6 +323,7 @@ def run_ours(args, rank: int, local_rank: int, world: int):
         "relres_updated": st.relres_updated,
         "fp64_pcg": {"time_to_tol_s": t_fp64, "iters": st64.iters, "iterations_per_s": st64.iters / t_fp64},
         "amp_speedup_vs_own_fp64": t_fp64 / t_amp,
+        "lagged_scale_variant": lagged,
         "paper_speedup_context": "1.63x on A100 SXM 40GB, matrix-free FEM (PAPER.md:506) - other hardware and operator",
         "create_s": create_s,
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 8 * s.n, "d2h_bytes_per_step": 8 * s.n,
