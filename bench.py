@@ -52,7 +52,7 @@ def parse_args():
     ap.add_argument("--profile-iters", type=int, default=0,
                     help="profiling aid for ncu: run ONE solve of this many iterations with plain stream launches "
                          "(u_r forced to FP32 from k=ell so the low-precision kernels appear) and exit; prints no bench line")
-    ap.add_argument("--profile-policy", default="amp_fp16_linear", choices=["pcg_fp64", "amp_fp16_linear", "amp_fp64_delay"])
+    ap.add_argument("--profile-policy", default="amp_fp16_linear", choices=["pcg_fp64", "amp_fp16_linear", "amp_fp64_delay", "amp_fp16_linear_lagged"])
     ap.add_argument("--ref-iters", type=int, default=100, help="--impl reference: iterations per step (bounded sample)")
     return ap.parse_args()
 
@@ -186,6 +186,7 @@ def run_ours(args, rank: int, local_rank: int, world: int):
     create_s = time.perf_counter() - t0
     if args.profile_iters > 0:
         kwp = {"pcg_fp64": dict(amp=0), "amp_fp16_linear": dict(u0=A.FP16, eta_rule=A.ETA_LINEAR, eps32=1e-30),
+               "amp_fp16_linear_lagged": dict(u0=A.FP16, eta_rule=A.ETA_LINEAR, eps32=1e-30, scale_mode=A.SCALE_LAGGED),
                "amp_fp64_delay": dict()}[args.profile_policy]
         lp = A.LOOP_STREAM if args.loop == "auto" else {"stream": A.LOOP_STREAM, "graph": A.LOOP_GRAPH, "persistent": A.LOOP_PERSISTENT}[args.loop]
         xp = torch.zeros(s.n, dtype=torch.float64, device=dev)
