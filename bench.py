@@ -256,7 +256,7 @@ def run_ours(args, rank: int, local_rank: int, world: int):
     t_fp64 = statistics.median(ms64) * 1e-3
     # ---- the lagged variant (AMP_SCALE_LAGGED, reading R17): same policy, three kernels per iteration ----
     lagged = None
-    if loop != A.LOOP_PERSISTENT:
+    if True:
         pol_lag = A.Policy.default(x0_zero=1, loop_mode=loop, scale_mode=A.SCALE_LAGGED, **kw)
         timed_solves(pol_lag, 1)
         ms_l, _, _, st_l = timed_solves(pol_lag, max(2, min(args.steps, 3)))

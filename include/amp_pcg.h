@@ -50,7 +50,7 @@ enum {
                           evaluated with the norms up to ||r_{k-1}||: every decision of iteration k is known one
                           iteration early, so z_{k+1} and rho_{k+1} are produced in the pass that updates x and r —
                           three kernels and reductions per iteration instead of four.  Same iterates in exact
-                          arithmetic (Theorem 3.2); switch iterations move by +1.  Graph and stream loops only. */
+                          arithmetic (Theorem 3.2); switch iterations move by +1. */
 };
 /* how the iteration loop is driven (execution choice; does not change the arithmetic) */
 enum {

@@ -530,11 +530,7 @@ static int solve_impl(amp_pcg* h, const double* b, double* x, double tol, int32_
   // 512 K 25.0 vs 32.1, 2.1 M (c2) 58 vs 57, 4.1 M (c3) 95 vs 92: the persistent kernel wins while the iteration is
   // latency-bound; from c2 up the graph loop wins because each of its kernels has its own register budget
   const bool lagged = pol.amp && pol.scale_mode == AMP_SCALE_LAGGED;
-  if (mode == AMP_LOOP_AUTO) mode = (!lagged && h->persist_ok && h->n <= kPersistAutoMaxRows) ? AMP_LOOP_PERSISTENT : AMP_LOOP_GRAPH;
-  if (lagged && mode == AMP_LOOP_PERSISTENT) {
-    set_error("amp_pcg_solve: AMP_SCALE_LAGGED runs in the graph and stream loops only");
-    return AMP_ERR_INVALID;
-  }
+  if (mode == AMP_LOOP_AUTO) mode = (h->persist_ok && h->n <= kPersistAutoMaxRows) ? AMP_LOOP_PERSISTENT : AMP_LOOP_GRAPH;
   if (mode == AMP_LOOP_PERSISTENT && !(h->persist_ok && persistent_fits(h->ctx))) {
     set_error("amp_pcg_solve: persistent loop not available for this problem/device");
     return AMP_ERR_INVALID;
@@ -559,7 +555,7 @@ static int solve_impl(amp_pcg* h, const double* b, double* x, double tol, int32_
   k_setup<<<h->vec_grid, kVecThreads, 0, st>>>(h->ctx, pol.x0_zero ? 1 : 0);
   h->launches += 1;
 
-  if (lagged) {  // z_0, rho_0 for the first pass of the three-kernel loop
+  if (lagged && mode != AMP_LOOP_PERSISTENT) {  // z_0, rho_0 for the first pass of the three-kernel loop
     k_z<<<h->grid_z, kVecThreads, 0, st>>>(h->ctx);
     h->launches += 1;
   }

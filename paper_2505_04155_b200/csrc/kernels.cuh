@@ -120,19 +120,26 @@ __global__ void __launch_bounds__(kVecThreads, 2) k_xr(const Ctx c) {
 }
 
 // ------------------------------------------------------------------ lagged variant: k_xrz ----
-template <int UR, int URN>
+template <int UR, int URN, int BIF>
 __device__ __forceinline__ void dispatch_xrz_z(const Ctx& c, int uz, int uzn, double alpha, double omega_n, double* x, int bid,
                                                int nb, double& rr, double& rz) {
   if (uz == P64) {
-    if (uzn == P64) phase_xrz<UR, URN, P64, P64>(c, alpha, omega_n, x, bid, nb, rr, rz);
-    else if (uzn == P32) phase_xrz<UR, URN, P64, P32>(c, alpha, omega_n, x, bid, nb, rr, rz);
-    else phase_xrz<UR, URN, P64, P16>(c, alpha, omega_n, x, bid, nb, rr, rz);
+    if (uzn == P64) phase_xrz<UR, URN, P64, P64, BIF>(c, alpha, omega_n, x, bid, nb, rr, rz);
+    else if (uzn == P32) phase_xrz<UR, URN, P64, P32, BIF>(c, alpha, omega_n, x, bid, nb, rr, rz);
+    else phase_xrz<UR, URN, P64, P16, BIF>(c, alpha, omega_n, x, bid, nb, rr, rz);
   } else if (uz == P32) {
-    if (uzn == P32) phase_xrz<UR, URN, P32, P32>(c, alpha, omega_n, x, bid, nb, rr, rz);
-    else phase_xrz<UR, URN, P32, P16>(c, alpha, omega_n, x, bid, nb, rr, rz);
+    if (uzn == P32) phase_xrz<UR, URN, P32, P32, BIF>(c, alpha, omega_n, x, bid, nb, rr, rz);
+    else phase_xrz<UR, URN, P32, P16, BIF>(c, alpha, omega_n, x, bid, nb, rr, rz);
   } else {
-    phase_xrz<UR, URN, P16, P16>(c, alpha, omega_n, x, bid, nb, rr, rz);
+    phase_xrz<UR, URN, P16, P16, BIF>(c, alpha, omega_n, x, bid, nb, rr, rz);
   }
+}
+template <int BIF = kVecBytesInFlight>
+__device__ __forceinline__ void dispatch_xrz(const Ctx& c, int ur, int urn, int uz, int uzn, double alpha, double omega_n,
+                                             double* x, int bid, int nb, double& rr, double& rz) {
+  if (ur == P64 && urn == P64) dispatch_xrz_z<P64, P64, BIF>(c, uz, uzn, alpha, omega_n, x, bid, nb, rr, rz);
+  else if (ur == P64) dispatch_xrz_z<P64, P32, BIF>(c, uz, uzn, alpha, omega_n, x, bid, nb, rr, rz);
+  else dispatch_xrz_z<P32, P32, BIF>(c, uz, uzn, alpha, omega_n, x, bid, nb, rr, rz);
 }
 
 // a5 of iteration k fused with a2 of iteration k+1 (AMP_SCALE_LAGGED): x, r, delta, z, rho in one pass
@@ -146,12 +153,8 @@ __global__ void __launch_bounds__(kVecThreads, 2) k_xrz(const Ctx c) {
     return;
   }
   const int bid = blockIdx.x, nb = gridDim.x;
-  const int ur = s->ur, urn = s->ur_n, uz = s->uz, uzn = s->uz_n;
-  const double alpha = s->alpha, omega_n = s->omega_n;
   double rr = 0.0, rz = 0.0;
-  if (ur == P64 && urn == P64) dispatch_xrz_z<P64, P64>(c, uz, uzn, alpha, omega_n, s->x, bid, nb, rr, rz);
-  else if (ur == P64) dispatch_xrz_z<P64, P32>(c, uz, uzn, alpha, omega_n, s->x, bid, nb, rr, rz);
-  else dispatch_xrz_z<P32, P32>(c, uz, uzn, alpha, omega_n, s->x, bid, nb, rr, rz);
+  dispatch_xrz(c, s->ur, s->ur_n, s->uz, s->uz_n, s->alpha, s->omega_n, s->x, bid, nb, rr, rz);
   grid_reduce2<kVecThreads>(rr, rz, c.partials + 2 * kMaxGrid, &s->counter[2], bid, nb, red,
                             [&](double t0, double t1) { epi_delta_lagged(epi_ctx(c), t0, t1); });
 }

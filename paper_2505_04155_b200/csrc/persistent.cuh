@@ -57,6 +57,25 @@ __device__ __forceinline__ double grid_all_sum(double v, double* partials, unsig
   return tot;
 }
 
+// the same for two sums (lagged variant: delta^2 and rho), partials interleaved; totals valid in warp 0
+__device__ __forceinline__ void grid_all_sum2(double v0, double v1, double* partials, unsigned int* arrivals, unsigned int& target,
+                                              int bid, int nb, double* red, double& t0, double& t1) {
+  const double b0 = block_sum<kPersistThreads>(v0, red);
+  const double b1 = block_sum<kPersistThreads>(v1, red);
+  target += (unsigned int)nb;
+  if (threadIdx.x == 0) {
+    __stcg(partials + 2 * bid, b0);
+    __stcg(partials + 2 * bid + 1, b1);
+    red_release_add_u32(arrivals, 1u);
+    while ((int)(ld_acquire_u32(arrivals) - target) < 0) { }
+  }
+  __syncthreads();
+  double a0 = 0.0, a1 = 0.0;
+  for (int i = threadIdx.x; i < nb; i += kPersistThreads) { a0 += __ldcg(partials + 2 * i); a1 += __ldcg(partials + 2 * i + 1); }
+  t0 = block_sum<kPersistThreads>(a0, red);
+  t1 = block_sum<kPersistThreads>(a1, red);
+}
+
 // out-of-line copies of the phase dispatchers: each gets its own register allocation instead of
 // one allocation for the union of all precision variants
 __device__ __noinline__ double pz(const Ctx& c, int rs, int ur, int uz, double omega, int bid, int nb) {
@@ -70,6 +89,11 @@ __device__ __noinline__ double ps_(const Ctx& c, int ur, int uz, int bid, int nb
 }
 __device__ __noinline__ double pxr(const Ctx& c, int ur, int uz, double alpha, double* x, int bid, int nb) {
   return dispatch_xr<kPersistBIF>(c, ur, uz, alpha, x, bid, nb);
+}
+
+__device__ __noinline__ void pxrz(const Ctx& c, int ur, int urn, int uz, int uzn, double alpha, double omega_n, double* x,
+                                  int bid, int nb, double& rr, double& rz) {
+  dispatch_xrz<kPersistBIF>(c, ur, urn, uz, uzn, alpha, omega_n, x, bid, nb, rr, rz);
 }
 
 __global__ void __launch_bounds__(kPersistThreads, kPersistMinBlocks) k_persistent(const Ctx c) {
@@ -89,6 +113,29 @@ __global__ void __launch_bounds__(kPersistThreads, kPersistMinBlocks) k_persiste
   unsigned int* arrivals = &c.st->bar_count;
   unsigned int target = 0u;
   double* x = s->x;
+  if (s->amp && s->scale_mode == 4) {
+    // lagged variant (reading R17): z_0, rho_0 once, then three phases and three barriers per iteration
+    if (!s->done) {
+      const double v = pz(c, s->r_store, s->ur, s->uz, s->omega, bid, nb);
+      const double t = grid_all_sum<true>(v, c.partials + 0 * kMaxGrid, arrivals, target, bid, nb, red);
+      if (threadIdx.x == 0) epi_rho(ec, t);
+      __syncthreads();
+    }
+    while (!s->done) {
+      pp(c, s->p_store, s->uz, s->beta, s->k == 0, bid, nb);                                         // a3
+      grid_all_sum<false>(0.0, nullptr, arrivals, target, bid, nb, red);
+      const double v = ps_(c, s->ur, s->uz, bid, nb, red);                                           // a4
+      const double t = grid_all_sum<true>(v, c.partials + 1 * kMaxGrid, arrivals, target, bid, nb, red);
+      if (threadIdx.x == 0) epi_gamma(ec, t);
+      __syncthreads();
+      if (s->done) break;  // breakdown
+      double rr = 0.0, rz = 0.0, t0, t1;
+      pxrz(c, s->ur, s->ur_n, s->uz, s->uz_n, s->alpha, s->omega_n, x, bid, nb, rr, rz);              // a5 + a2
+      grid_all_sum2(rr, rz, c.partials + 2 * kMaxGrid, arrivals, target, bid, nb, red, t0, t1);
+      if (threadIdx.x == 0) epi_delta_lagged(ec, t0, t1);
+      __syncthreads();
+    }
+  }
   while (!s->done) {
     const int rs = s->r_store, ps = s->p_store, ur = s->ur, uz = s->uz;
     const bool first = (s->k == 0);
