@@ -27,6 +27,7 @@ POLICIES = {
     "amp_fp64_delay": dict(amp=1, u0=O.FP64, eta_rule=O.ETA_DELAY),
     "amp_fp16_linear": dict(amp=1, u0=O.FP16, eta_rule=O.ETA_LINEAR),
     "amp_fp64_delay_strict": dict(amp=1, u0=O.FP64, eta_rule=O.ETA_DELAY, eta_safety=0.1, stop_safety=0.9),
+    "amp_fp64_delay_lagged": dict(amp=1, u0=O.FP64, eta_rule=O.ETA_DELAY, scale_mode=O.SCALE_LAGGED),
 }
 
 

@@ -15,6 +15,7 @@ POLICY_SPECS = {
     "amp_fp32_never": dict(amp=1, u0=1, eta_rule=2),
     "amp_fp64_rms": dict(amp=1, u0=0, eta_rule=0, scale_mode=1),
     "amp_fp64_pow2": dict(amp=1, u0=0, eta_rule=0, scale_mode=2),
+    "amp_fp64_delay_lagged": dict(amp=1, u0=0, eta_rule=0, scale_mode=4),
 }
 
 
