@@ -44,8 +44,9 @@ struct DevState {
   double omega_n;
   unsigned int counter[4];  // last-block tickets of the three reductions (+ setup)
   unsigned long long fp16_subnormal, fp16_flushed, fp16_inf;
-  // ---- grid barrier of the persistent kernel ----
-  unsigned int bar_count, bar_gen;
+  // ---- grid barrier of the persistent kernel: arrivals since the start of the solve (host-zeroed); never
+  //      written back from a block's replica ----
+  unsigned int bar_count, bar_pad;
 };
 
 // Handle-lifetime constants, passed to every kernel by value.
