@@ -1,18 +1,23 @@
 #!/usr/bin/env python
 """bench.py — AMP-PCG time-to-tolerance / iterations per second on one B200 (BASELINE.json metric).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload c2] [--impl ours|reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload c4] [--impl ours|reference]
 
 One "step" = one whole solve (every row of SURVEY.md §8(a): set-up, then per iteration the fused
 z/(r,z), p, SpMV/(p,Ap), x/r/||r|| kernels with device-side precision switching) of the seeded
-synthetic system `--workload` (default c2 = BASELINE.json configs[1], 3-D Poisson 128^3, tol 1e-10)
-from x0 = 0, with A resident in HBM.  `value` = PCG iterations per second over all ranks
-(N > 1: independent replicas, one per GPU, no data-path collective: "weak" scaling).
-Prints ONE JSON line (rank 0).
+synthetic system `--workload` from x0 = 0, with A resident in HBM.  Default workload: c4 =
+BASELINE.json configs[3], the 27-point FE Laplacian 200^3 (n = 8 M, nnz = 213.8 M), the LARGEST
+single-GPU configuration (BASELINE.json's metric names no configuration).  `value` = PCG iterations per
+second over all ranks (N > 1: independent replicas, one per GPU, no data-path collective: "weak").
+`roofline` is measured on the kernels the loop itself runs: one extra solve with the stream-driven loop and a CUDA
+event between every two kernels (amp_policy_t.profile_kernels); each kernel's time is the average over all its
+launches in the dominant precision phase (u_z, u_r) = (FP16, FP32); the per-iteration working set of c4 (1.3 GB)
+is ten times the L2, so every launch starts cold.  Prints ONE JSON line (rank 0).
 """
 from __future__ import annotations
 
 import argparse
+import ctypes
 import json
 import os
 import statistics
@@ -28,13 +33,11 @@ UNIT = "iterations/s"
 SMI_QUERY = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
              "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
              "clocks_event_reasons.sw_power_cap")
-
-
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the SpMV kernel from the committed ncu --set full
-# captures (profiles/r01c_*.md name the commands); None where no capture exists for that workload
-NCU_TRAFFIC = {
-    ("c2", "fp32mat_fp16vec"): 64.82e6 + 2.17e6,   # profiles/r01c_c2_ncu_full.csv, k_spmv in phase (FP16, FP32)
-    ("c4", "fp32mat_fp16vec"): 907.34e6 + 28.23e6,  # profiles/r01c_c4_ncu_full.csv
+DTYPE = "f64 (r,q,A: f64->f32; z,p storage: f64->f32->f16; x, dots f64)"
+POLICIES = {
+    "amp_fp64_delay": dict(amp=1, u0=0, eta_rule=0),                                          # paper: AMP-PCG(FP64), (4.9)+(4.10)
+    "amp_fp16_linear": dict(amp=1, u0=2, eta_rule=1),                                         # paper: AMP-PCG(FP16), (4.11)
+    "amp_fp64_delay_strict": dict(amp=1, u0=0, eta_rule=0, eta_safety=0.1, stop_safety=0.9),  # theta-split of (3.10): true relres <= tol
 }
 
 
@@ -43,17 +46,21 @@ def parse_args():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--workload", default="c2", choices=["c1", "c2", "c3", "c4", "c5"])
+    ap.add_argument("--workload", default="c4", choices=["c1", "c2", "c3", "c4", "c5"])
     ap.add_argument("--size", type=int, default=None, help="override grid edge / rows (debug only)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--policy", default="amp_fp64_delay", choices=["amp_fp64_delay", "amp_fp16_linear"])
+    ap.add_argument("--policy", default="amp_fp64_delay", choices=sorted(POLICIES))
     ap.add_argument("--loop", default="auto", choices=["auto", "stream", "graph", "persistent"])
+    ap.add_argument("--spmv-kernel", default="auto", choices=["auto", "direct", "pipelined"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--others", default="", help="comma list of further workloads to report under 'other_workloads' "
+                                                 "(value / time_to_tol / speed-up only), e.g. c1,c2,c3,c5")
     ap.add_argument("--profile-iters", type=int, default=0,
                     help="profiling aid for ncu: run ONE solve of this many iterations with plain stream launches "
                          "(u_r forced to FP32 from k=ell so the low-precision kernels appear) and exit; prints no bench line")
-    ap.add_argument("--profile-policy", default="amp_fp16_linear", choices=["pcg_fp64", "amp_fp16_linear", "amp_fp64_delay", "amp_fp16_linear_lagged"])
-    ap.add_argument("--ref-iters", type=int, default=100, help="--impl reference: iterations per step (bounded sample)")
+    ap.add_argument("--profile-policy", default="amp_fp16_linear",
+                    choices=["pcg_fp64", "amp_fp16_linear", "amp_fp64_delay", "amp_fp16_linear_lagged"])
+    ap.add_argument("--ref-iters", type=int, default=0, help="--impl reference: iterations per step (0 = sized to the workload)")
     return ap.parse_args()
 
 
@@ -63,6 +70,17 @@ def peaks():
         d = json.load(open(path))
         return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, STREAM-style copy)"
     return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s)"
+
+
+def ncu_traffic(workload: str, kernel: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full capture of THIS round
+    (profiles/r02_ncu_traffic.json names the capture and the commit), else None."""
+    path = os.path.join(ROOT, "profiles", "r02_ncu_traffic.json")
+    try:
+        d = json.load(open(path))
+        return d.get(workload, {}).get(kernel)
+    except (OSError, ValueError):
+        return None
 
 
 class ClockSampler:
@@ -122,10 +140,75 @@ def reduce_over_ranks(dist, vmax, vsum, device):
 
 
 def policy_kwargs(name: str):
-    return {"amp_fp64_delay": dict(amp=1, u0=0, eta_rule=0), "amp_fp16_linear": dict(amp=1, u0=2, eta_rule=1)}[name]
+    return dict(POLICIES[name])
+
+
+def config_dict(s, policy: str, world: int):
+    """the `config` object: identical for our arm and the reference arm (same workload, tolerance, policy)"""
+    return {"workload": s.name, "n": s.n, "nnz": s.nnz, "tol": s.tol, "maxit": s.maxit, "policy": policy,
+            "precond": "jacobi", "x0": "zero",
+            "l2": "L2 flushed (256 MiB write) before every timed solve; per-iteration working set > 126 MB L2 "
+                  "(c1 excepted: it lives in L2 by construction)",
+            "replicas": world}
 
 
 # --------------------------------------------------------------------------------------------
+def cpu_model():
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.startswith("model name"):
+                return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
+def omp_set_threads(n: int):
+    """thread count of the oracle's OpenMP loops (libgomp is already loaded by the oracle library)"""
+    try:
+        ctypes.CDLL("libgomp.so.1").omp_set_num_threads(int(n))
+        return True
+    except OSError:
+        return False
+
+
+def oracle_sample_iters(s):
+    """iterations of the bounded CPU sample: about 10-30 s of host work for all legs together"""
+    per_it_all = s.nnz * 1.4e-10 + s.n * 1.2e-9  # rough seconds per oracle iteration on ~16 threads (round-1 runs)
+    return int(max(5, min(150, 5.0 / per_it_all)))
+
+
+def cpu_baseline_leg(s, kw):
+    """SURVEY.md section 8(d) "CPU baseline": the oracle's FP64 PCG on all host cores and on one thread, the AMP-PCG
+    emulation (software rounding: artificially slow) beside it; a bounded sample of the same solve."""
+    import oracle as O
+
+    ncores = os.cpu_count() or 1
+    cap = min(oracle_sample_iters(s), s.maxit)
+    out = {"unit": UNIT, "kind": "oracle", "cores": ncores, "cpu_model": cpu_model()}
+    omp_set_threads(ncores)
+    t0 = time.perf_counter()
+    r = O.amp_pcg(s.rowptr, s.colidx, s.vals, s.b, s.tol, cap, O.make_policy(amp=0))
+    dt = time.perf_counter() - t0
+    out["value"] = r.iters / dt
+    out["sample"] = (f"oracle FP64 PCG (Alg 3.1), first {r.iters} iterations of the solve of {s.name} "
+                     f"({dt:.1f} s, OpenMP, {ncores} threads)")
+    t0 = time.perf_counter()
+    r2 = O.amp_pcg(s.rowptr, s.colidx, s.vals, s.b, s.tol, cap, O.make_policy(**kw))
+    dt2 = time.perf_counter() - t0
+    out["amp_emulation"] = {"value": r2.iters / dt2, "kind": "oracle_amp_emulation", "cores": ncores,
+                            "sample": f"first {r2.iters} iterations of AMP-PCG with software-rounded storage ({dt2:.1f} s)"}
+    if omp_set_threads(1):
+        cap1 = max(3, cap // 6)
+        t0 = time.perf_counter()
+        r1 = O.amp_pcg(s.rowptr, s.colidx, s.vals, s.b, s.tol, cap1, O.make_policy(amp=0))
+        dt1 = time.perf_counter() - t0
+        out["one_thread"] = {"value": r1.iters / dt1, "cores": 1,
+                             "sample": f"oracle FP64 PCG, first {r1.iters} iterations, 1 thread ({dt1:.1f} s)"}
+        omp_set_threads(ncores)
+    return out
+
+
 def run_reference(args, rank: int, world: int):
     """--impl reference: the CPU oracle as it stands, on the host cores (rank 0 only)."""
     if rank != 0:
@@ -136,7 +219,7 @@ def run_reference(args, rank: int, world: int):
     s = make_config(args.workload, args.size)
     kw = policy_kwargs(args.policy)
     pol = O.make_policy(**kw)
-    cap = min(args.ref_iters, s.maxit)
+    cap = min(args.ref_iters or max(3, oracle_sample_iters(s) // 3), s.maxit)
     times, its = [], 0
     for i in range(args.warmup + args.steps):
         t0 = time.perf_counter()
@@ -146,22 +229,94 @@ def run_reference(args, rank: int, world: int):
             times.append(dt); its += r.iters
     total = sum(times)
     val = its / total
+    sample = f"each step = the first {cap} iterations of the AMP-PCG solve of {s.name} (software-rounded storage)"
     line = {
         "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": 1e3 * total / max(len(times), 1), "higher_is_better": True,
-        "scaling": "weak", "vs_baseline": None, "dtype": "f64 (f32/f16 storage emulated by rounding)", "data": "synthetic",
-        "config": {"workload": s.name, "n": s.n, "nnz": s.nnz, "tol": s.tol, "policy": args.policy,
-                   "sample": f"first {cap} iterations of the solve per step"},
-        "cpu_baseline": {"value": val, "unit": UNIT, "cores": os.cpu_count(), "kind": "oracle",
-                         "sample": f"{args.steps} x first {cap} iterations of AMP-PCG on {s.name}"},
+        "scaling": "weak", "vs_baseline": None, "dtype": DTYPE, "data": "synthetic",
+        "config": config_dict(s, args.policy, world),
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": os.cpu_count(), "kind": "oracle", "sample": sample,
+                         "cpu_model": cpu_model()},
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
     print(json.dumps(line), flush=True)
 
 
+# --------------------------------------------------------------------------------------------
+class Runner:
+    """one workload resident on one GPU: timed solves of a policy, each preceded by an L2 flush"""
+
+    def __init__(self, A, torch, s, dev, loop, spmv_kernel):
+        self.A, self.torch, self.s, self.dev = A, torch, s, dev
+        self.rp, self.ci, self.va, self.b = (torch.from_numpy(a).to(dev) for a in (s.rowptr, s.colidx, s.vals, s.b))
+        t0 = time.perf_counter()
+        self.h = A.AmpPcg(self.rp, self.ci, self.va, A.PRECOND_JACOBI, spmv_kernel=spmv_kernel)
+        torch.cuda.synchronize()
+        self.create_s = time.perf_counter() - t0
+        self.loop = loop
+        self.flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)  # 256 MiB > 126 MB L2
+        self.x = torch.zeros(s.n, dtype=torch.float64, device=dev)
+        self.stream = torch.cuda.current_stream(dev)
+
+    def policy(self, name_or_kw, **extra):
+        kw = policy_kwargs(name_or_kw) if isinstance(name_or_kw, str) else dict(name_or_kw)
+        kw.update(extra)
+        kw.setdefault("loop_mode", self.loop)
+        return self.A.Policy.default(x0_zero=1, **kw)
+
+    def timed(self, policy, count, host=False, bh=None, xh=None):
+        """count solves, each bracketed by CUDA events on the solve stream, L2 flushed before each."""
+        torch, s, h = self.torch, self.s, self.h
+        ms, its, launches, last = [], 0, 0, None
+        for _ in range(count):
+            self.flush.fill_(1)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(self.stream)
+            if host:
+                st = h.solve_host(bh, xh, s.tol, s.maxit, policy)
+            else:
+                st = h.solve(self.b, self.x, s.tol, s.maxit, policy)
+            e1.record(self.stream)
+            e1.synchronize()
+            ms.append(e0.elapsed_time(e1)); its += st.iters; launches += h.last_launch_count(); last = st
+        return ms, its, launches, last
+
+    def summary(self, name_or_kw, reps, **extra):
+        """median time-to-tolerance of a policy + its true residual (one extra, untimed solve with true_residual=1)"""
+        pol = self.policy(name_or_kw, **extra)
+        self.timed(pol, 1)
+        ms, _, _, st = self.timed(pol, reps)
+        t = statistics.median(ms) * 1e-3
+        st_true = self.h.solve(self.b, self.x, self.s.tol, self.s.maxit, self.policy(name_or_kw, true_residual=1, **extra))
+        return {"time_to_tol_s": t, "iters": st.iters, "iterations_per_s": st.iters / t,
+                "switch_iters": {"ur32": st.it_ur32, "uz32": st.it_uz32, "uz16": st.it_uz16},
+                "relres_updated": st.relres_updated, "relres_true": st_true.relres_true,
+                "relres_true_le_tol": bool(st_true.relres_true <= self.s.tol)}, st
+
+    def kernel_profile(self, name_or_kw, peak, **extra):
+        """per-kernel device times inside the loop (stream loop, an event between every two kernels)"""
+        A = self.A
+        pol = self.policy(name_or_kw, loop_mode=A.LOOP_STREAM, profile_kernels=1, **extra)
+        self.flush.fill_(1)
+        self.h.solve(self.b, self.x, self.s.tol, self.s.maxit, pol)
+        recs = self.h.kernel_times()
+        names = {0: "fp64", 1: "fp32", 2: "fp16"}
+        out = {}
+        for r in recs:
+            us = 1e3 * r["total_ms"] / r["launches"]
+            gbs = r["bytes_per_launch"] / us * 1e-3
+            out.setdefault(f"uz={names[r['uz']]},ur={names[r['ur']]}", {})[r["kernel"]] = {
+                "launches": r["launches"], "us_per_launch": us, "algorithmic_bytes_per_launch": r["bytes_per_launch"],
+                "achieved_gbs": gbs, "frac": gbs / peak}
+        return out
+
+    def close(self):
+        self.h.close()
+
+
 def run_ours(args, rank: int, local_rank: int, world: int):
-    import numpy as np
+    import numpy as np  # noqa: F401
     import torch
 
     import paper_2505_04155_b200 as A
@@ -178,56 +333,33 @@ def run_ours(args, rank: int, local_rank: int, world: int):
         dist = dist_
         dist.init_process_group("nccl", device_id=dev)
 
+    loop = {"auto": A.LOOP_AUTO, "stream": A.LOOP_STREAM, "graph": A.LOOP_GRAPH, "persistent": A.LOOP_PERSISTENT}[args.loop]
+    spmv_kernel = {"auto": A.SPMV_AUTO, "direct": A.SPMV_DIRECT, "pipelined": A.SPMV_PIPELINED}[args.spmv_kernel]
     s = make_config(args.workload, args.size)
-    rp, ci, va, b = (torch.from_numpy(a).to(dev) for a in (s.rowptr, s.colidx, s.vals, s.b))
-    t0 = time.perf_counter()
-    h = A.AmpPcg(rp, ci, va, A.PRECOND_JACOBI)
-    torch.cuda.synchronize()
-    create_s = time.perf_counter() - t0
+    R = Runner(A, torch, s, dev, loop, spmv_kernel)
+    h = R.h
     if args.profile_iters > 0:
         kwp = {"pcg_fp64": dict(amp=0), "amp_fp16_linear": dict(u0=A.FP16, eta_rule=A.ETA_LINEAR, eps32=1e-30),
                "amp_fp16_linear_lagged": dict(u0=A.FP16, eta_rule=A.ETA_LINEAR, eps32=1e-30, scale_mode=A.SCALE_LAGGED),
                "amp_fp64_delay": dict()}[args.profile_policy]
-        lp = A.LOOP_STREAM if args.loop == "auto" else {"stream": A.LOOP_STREAM, "graph": A.LOOP_GRAPH, "persistent": A.LOOP_PERSISTENT}[args.loop]
-        xp = torch.zeros(s.n, dtype=torch.float64, device=dev)
-        stp = h.solve(b, xp, s.tol, args.profile_iters, A.Policy.default(x0_zero=1, loop_mode=lp, **kwp))
+        lp = A.LOOP_STREAM if args.loop == "auto" else loop
+        stp = h.solve(R.b, R.x, s.tol, args.profile_iters, A.Policy.default(x0_zero=1, loop_mode=lp, **kwp))
         print("profile run:", stp.asdict(), file=sys.stderr)
-        h.close()
+        R.close()
         return
-    loop = {"auto": A.LOOP_AUTO, "stream": A.LOOP_STREAM, "graph": A.LOOP_GRAPH, "persistent": A.LOOP_PERSISTENT}[args.loop]
     kw = policy_kwargs(args.policy)
-    pol = A.Policy.default(x0_zero=1, loop_mode=loop, **kw)
-    pol_fp64 = A.Policy.default(x0_zero=1, loop_mode=loop, amp=0)
-    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)  # 256 MiB > 126 MB L2
-    x = torch.zeros(s.n, dtype=torch.float64, device=dev)
-    stream = torch.cuda.current_stream(dev)
+    pol = R.policy(args.policy)
 
     def barrier():
         if dist is not None:
             dist.barrier()
         torch.cuda.synchronize()
 
-    def timed_solves(policy, count, host=False, bh=None, xh=None):
-        """count solves, each bracketed by CUDA events on the solve stream, L2 flushed before each."""
-        ms, its, launches, last = [], 0, 0, None
-        for _ in range(count):
-            flush.fill_(1)
-            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            e0.record(stream)
-            if host:
-                st = h.solve_host(bh, xh, s.tol, s.maxit, policy)
-            else:
-                st = h.solve(b, x, s.tol, s.maxit, policy)
-            e1.record(stream)
-            e1.synchronize()
-            ms.append(e0.elapsed_time(e1)); its += st.iters; launches += h.last_launch_count(); last = st
-        return ms, its, launches, last
-
     # ---- warm-up, then EXACTLY K timed steps between barriers ----
-    timed_solves(pol, args.warmup)
+    R.timed(pol, args.warmup)
     barrier()
     with ClockSampler(local_rank) as clk:
-        ms, its, launches, st = timed_solves(pol, args.steps)
+        ms, its, launches, st = R.timed(pol, args.steps)
     barrier()
     total_ms = sum(ms)
     (total_ms_max,), (its_all, launches_all) = reduce_over_ranks(dist, [total_ms], [its, launches], dev)
@@ -237,9 +369,9 @@ def run_ours(args, rank: int, local_rank: int, world: int):
     # ---- end-to-end through the host-buffer entry point (H2D of b, solve, D2H of x inside) ----
     bh = torch.from_numpy(s.b).pin_memory()
     xh = torch.zeros(s.n, dtype=torch.float64).pin_memory()
-    timed_solves(pol, 1, host=True, bh=bh, xh=xh)
+    R.timed(pol, 1, host=True, bh=bh, xh=xh)
     barrier()
-    ms_e, its_e, _, _ = timed_solves(pol, args.steps, host=True, bh=bh, xh=xh)
+    ms_e, its_e, _, _ = R.timed(pol, args.steps, host=True, bh=bh, xh=xh)
     barrier()
     (tot_e,), (its_e,) = reduce_over_ranks(dist, [sum(ms_e)], [its_e], dev)
     e2e_value = its_e / (tot_e * 1e-3)
@@ -249,84 +381,80 @@ def run_ours(args, rank: int, local_rank: int, world: int):
             dist.destroy_process_group()
         return
 
-    # ---- this library's own FP64 PCG on the same system (north_star: AMP must beat it) ----
-    timed_solves(pol_fp64, 1)
-    ms64, its64, _, st64 = timed_solves(pol_fp64, max(2, min(args.steps, 3)))
-    t_amp = statistics.median(ms) * 1e-3
-    t_fp64 = statistics.median(ms64) * 1e-3
-    # ---- the lagged variant (AMP_SCALE_LAGGED, reading R17): same policy, three kernels per iteration ----
-    lagged = None
-    if True:
-        pol_lag = A.Policy.default(x0_zero=1, loop_mode=loop, scale_mode=A.SCALE_LAGGED, **kw)
-        timed_solves(pol_lag, 1)
-        ms_l, _, _, st_l = timed_solves(pol_lag, max(2, min(args.steps, 3)))
-        t_lag = statistics.median(ms_l) * 1e-3
-        lagged = {"time_to_tol_s": t_lag, "iters": st_l.iters, "iterations_per_s": st_l.iters / t_lag,
-                  "switch_iters": {"ur32": st_l.it_ur32, "uz32": st_l.it_uz32, "uz16": st_l.it_uz16},
-                  "relres_updated": st_l.relres_updated, "speedup_vs_own_fp64": t_fp64 / t_lag}
-
-    # ---- roofline of the dominant kernel (SpMV) timed alone with CUDA events ----
+    reps = max(2, min(args.steps, 3))
     peak, peak_src = peaks()
-    m = s.nnz / s.n
-    reps = 20
-    npad = (s.n + 7) // 8 * 8
-    roof = {}
-    for tag, matp, pt, sA, sz in (("fp32mat_fp16vec", A.FP32, torch.float16, 4, 2), ("fp64mat_fp64vec", A.FP64, torch.float64, 8, 8)):
-        pvec = torch.zeros(npad, dtype=pt, device=dev)
-        pvec[: s.n] = torch.from_numpy(np.cos(np.arange(s.n) * 0.37)).to(dev).to(pt)
-        q = torch.empty(s.n, dtype=torch.float32 if matp == A.FP32 else torch.float64, device=dev)
-        for _ in range(3):
-            h.spmv(pvec, matp, out=q)
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        e0.record(stream)
-        for _ in range(reps):
-            h.spmv(pvec, matp, out=q)
-        e1.record(stream); e1.synchronize()
-        dur_ms = e0.elapsed_time(e1) / reps
-        # bytes this handle's matrix format must move per launch (amp_pcg_spmv_bytes):
-        # stored values + the index data actually read + p once + q once
-        alg_bytes = h.spmv_bytes(matp, A.FP16 if pt == torch.float16 else A.FP64)
-        csr_bytes = s.n * (m * (sA + 4) + 4 + sz + sA)  # the same mat-vec in plain CSR
-        roof[tag] = {"bound": "hbm", "achieved": alg_bytes / dur_ms * 1e-6, "peak": peak, "unit": "GB/s",
-                     "frac": alg_bytes / dur_ms * 1e-6 / peak, "traffic": NCU_TRAFFIC.get((s.name.split("@")[0], tag)),
-                     "kernel": "k_spmv_any (phase_spmv)",
-                     "us_per_launch": dur_ms * 1e3, "algorithmic_bytes_per_launch": alg_bytes, "peak_source": peak_src,
-                     "csr_equivalent_bytes_per_launch": csr_bytes, "csr_equivalent_gbs": csr_bytes / dur_ms * 1e-6}
-    roofline = dict(roof["fp32mat_fp16vec"])
-    roofline["fp64"] = {k: roof["fp64mat_fp64vec"][k] for k in ("achieved", "frac", "us_per_launch", "algorithmic_bytes_per_launch",
-                                                                "traffic", "csr_equivalent_gbs")}
-    loop_gbs = st.algorithmic_bytes / (statistics.median(ms) * 1e-3) * 1e-9
-    loop64_gbs = st64.algorithmic_bytes / (statistics.median(ms64) * 1e-3) * 1e-9
+    # ---- the headline policy again with its true residual, this library's own FP64 PCG (north_star: AMP must beat
+    #      it), the theta-split policy that guarantees true relres <= tol (reading R12), the lagged variant (R17) ----
+    amp_sum, _ = R.summary(args.policy, reps)
+    fp64_sum, st64 = R.summary(dict(amp=0), reps)
+    strict_sum, _ = R.summary("amp_fp64_delay_strict", reps)
+    lag_sum, _ = R.summary(args.policy, reps, scale_mode=A.SCALE_LAGGED)
+    t_amp = statistics.median(ms) * 1e-3
+    t_fp64 = fp64_sum["time_to_tol_s"]
+    for d in (strict_sum, lag_sum):
+        d["speedup_vs_own_fp64"] = t_fp64 / d["time_to_tol_s"]
+
+    # ---- roofline: the kernels the loop runs, timed inside the loop ----
+    prof = R.kernel_profile(args.policy, peak)
+    prof_lag = R.kernel_profile(args.policy, peak, scale_mode=A.SCALE_LAGGED)
+    prof64 = R.kernel_profile(dict(amp=0), peak)
+    dom_phase = "uz=fp16,ur=fp32"
+    if dom_phase not in prof or "k_spmv" not in prof[dom_phase]:
+        dom_phase = max(prof, key=lambda ph: prof[ph].get("k_spmv", {}).get("launches", 0))
+    dom = prof[dom_phase]["k_spmv"]
+    wl = s.name.split("@")[0]
+    roofline = {
+        "bound": "hbm", "achieved": dom["achieved_gbs"], "peak": peak, "unit": "GB/s", "frac": dom["frac"],
+        "traffic": ncu_traffic(wl, "k_spmv"),
+        "kernel": "k_spmv (in-loop, phase " + dom_phase + ")", "us_per_launch": dom["us_per_launch"],
+        "launches_averaged": dom["launches"], "algorithmic_bytes_per_launch": dom["algorithmic_bytes_per_launch"],
+        "peak_source": peak_src,
+        "how": "stream-driven loop, CUDA event between every two kernels (policy.profile_kernels); average over all "
+               "launches of the phase inside one solve; working set per iteration >> L2",
+        "kernels": prof[dom_phase], "kernels_by_phase": prof,
+        "kernels_lagged_variant": prof_lag.get(dom_phase), "kernels_fp64_pcg": prof64.get("uz=fp64,ur=fp64"),
+    }
+    loop_gbs = st.algorithmic_bytes / t_amp * 1e-9
+    loop64_gbs = st64.algorithmic_bytes / t_fp64 * 1e-9
     roofline["whole_loop"] = {"amp_gbs": loop_gbs, "amp_frac": loop_gbs / peak, "amp_frac_of_8TBs": loop_gbs / 8000.0,
                               "fp64_gbs": loop64_gbs, "fp64_frac": loop64_gbs / peak}
 
+    # ---- the other BASELINE.json configs (parity-test cases; reported for context) ----
+    others = {}
+    for name in [t for t in args.others.split(",") if t]:
+        so = make_config(name)
+        Ro = Runner(A, torch, so, dev, loop, spmv_kernel)
+        a_, _ = Ro.summary(args.policy, 2)
+        f_, _ = Ro.summary(dict(amp=0), 2)
+        l_, _ = Ro.summary(args.policy, 2, scale_mode=A.SCALE_LAGGED)
+        others[so.name] = {"value": a_["iterations_per_s"], "time_to_tol_s": a_["time_to_tol_s"], "iters": a_["iters"],
+                           "relres_true": a_["relres_true"], "fp64_pcg_time_to_tol_s": f_["time_to_tol_s"],
+                           "amp_speedup_vs_own_fp64": f_["time_to_tol_s"] / a_["time_to_tol_s"],
+                           "lagged_time_to_tol_s": l_["time_to_tol_s"],
+                           "lagged_speedup_vs_own_fp64": f_["time_to_tol_s"] / l_["time_to_tol_s"]}
+        Ro.close()
+        del Ro
+
     # ---- CPU oracle on the host cores (reported baseline, not the target) ----
-    cpu = None
-    if not args.no_cpu_baseline:
-        import oracle as O
+    cpu = None if args.no_cpu_baseline else cpu_baseline_leg(s, kw)
 
-        cap = min(150, s.maxit)
-        tt0 = time.perf_counter()
-        r = O.amp_pcg(s.rowptr, s.colidx, s.vals, s.b, s.tol, cap, O.make_policy(**kw))
-        dt = time.perf_counter() - tt0
-        cpu = {"value": r.iters / dt, "unit": UNIT, "cores": os.cpu_count(), "kind": "oracle",
-               "sample": f"first {r.iters} iterations of the same AMP-PCG solve on {s.name} ({dt:.1f} s, OpenMP, all cores)"}
-
+    loop_name = {0: "auto", 1: "stream", 2: "graph", 3: "persistent"}[st.loop_mode]
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": total_ms_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": "f64 (r,q,A: f64->f32; z,p storage: f64->f32->f16; x, dots f64)", "data": "synthetic",
-        "config": {"workload": s.name, "n": s.n, "nnz": s.nnz, "tol": s.tol, "maxit": s.maxit, "policy": args.policy,
-                   "precond": "jacobi", "x0": "zero", "loop": {0: "auto", 1: "stream", 2: "graph", 3: "persistent"}[st.loop_mode],
-                   "l2": "L2 flushed (256 MiB write) before every timed solve; working set > 126 MB L2",
-                   "replicas": world},
-        "time_to_tol_s": t_amp, "iters": st.iters, "switch_iters": {"ur32": st.it_ur32, "uz32": st.it_uz32, "uz16": st.it_uz16},
-        "relres_updated": st.relres_updated,
-        "fp64_pcg": {"time_to_tol_s": t_fp64, "iters": st64.iters, "iterations_per_s": st64.iters / t_fp64},
+        "dtype": DTYPE, "data": "synthetic",
+        "config": config_dict(s, args.policy, world), "loop_driver": loop_name,
+        "time_to_tol_s": t_amp, "iters": st.iters, "us_per_iteration": 1e6 * t_amp / max(st.iters, 1),
+        "switch_iters": {"ur32": st.it_ur32, "uz32": st.it_uz32, "uz16": st.it_uz16},
+        "relres_updated": st.relres_updated, "relres_true": amp_sum["relres_true"],
+        "relres_true_le_tol": amp_sum["relres_true_le_tol"],
+        "fp64_pcg": fp64_sum,
         "amp_speedup_vs_own_fp64": t_fp64 / t_amp,
-        "lagged_scale_variant": lagged,
+        "amp_speedup_claim_rests_on": "Algorithm 4.1 as printed (headline `value`); the lagged variant is reported beside it",
+        "strict_theta_split_policy": strict_sum,
+        "lagged_scale_variant": lag_sum,
         "paper_speedup_context": "1.63x on A100 SXM 40GB, matrix-free FEM (PAPER.md:506) - other hardware and operator",
-        "create_s": create_s,
+        "create_s": R.create_s,
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 8 * s.n, "d2h_bytes_per_step": 8 * s.n,
                 "ms_per_step": tot_e / args.steps, "api": "amp_pcg_solve_host (pinned host b, x)"},
         "gpu_launches": launches_all,
@@ -334,8 +462,10 @@ def run_ours(args, rank: int, local_rank: int, world: int):
         "roofline": roofline,
         "cpu_baseline": cpu,
     }
+    if others:
+        line["other_workloads"] = others
     print(json.dumps(line), flush=True)
-    h.close()
+    R.close()
     if dist is not None:
         dist.destroy_process_group()
 

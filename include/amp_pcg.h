@@ -36,6 +36,20 @@ typedef struct amp_pcg amp_pcg_t; /* opaque solver handle */
 /* preconditioner M: the paper uses M = I for its small examples and Jacobi for
  * the timed GPU example */
 enum { AMP_PRECOND_NONE = 0, AMP_PRECOND_JACOBI = 1 };
+/* column-index form of the SELL-32 repack.  AUTO takes the most compact form the matrix
+ * allows; the other two force a more general form on the same matrix (testing / tuning) */
+enum {
+  AMP_INDEX_AUTO = 0,     /* diagonal-aligned slices where possible, else 16-bit offsets if they fit, else 32-bit */
+  AMP_INDEX_NO_ALIGN = 1, /* never diagonal-aligned: 16-bit offsets if they fit, else 32-bit */
+  AMP_INDEX_FORCE32 = 2   /* never diagonal-aligned, always 32-bit column indices */
+};
+/* which SpMV kernel the loop uses in the u_r = FP32 phase (execution choice; same arithmetic, same bits) */
+enum {
+  AMP_SPMV_AUTO = 0,      /* bulk-copy pipelined kernel when the matrix is eligible (every slice diagonal-aligned,
+                             natural row order, no long rows), else the direct kernel */
+  AMP_SPMV_DIRECT = 1,    /* every lane streams its row with 128-bit loads (round-1 kernel) */
+  AMP_SPMV_PIPELINED = 2  /* value stream staged through shared memory by cp.async.bulk + mbarrier ring */
+};
 /* storage / working precisions u_z, u_r */
 enum { AMP_FP64 = 0, AMP_FP32 = 1, AMP_FP16 = 2 };
 /* indicator used by the u_r switch */
@@ -84,6 +98,10 @@ typedef struct {
   int32_t x0_zero;    /* 1: caller promises x0 = 0; x is zero-filled and r0 = b without a mat-vec */
   int32_t true_residual; /* 1: after the loop compute ||b - A x||/||b|| in FP64 (one extra FP64 SpMV, not in solve_ms) */
   int32_t loop_mode;  /* AMP_LOOP_* */
+  int32_t profile_kernels; /* 1 (AMP_LOOP_STREAM only): bracket every loop kernel with CUDA events on the solve stream;
+                              read the per-kernel, per-phase sums with amp_pcg_kernel_times().  Plain launches (no
+                              programmatic overlap) so that each duration belongs to one kernel */
+  int32_t reserved0;  /* 0 */
   double C;           /* constant of Assumption 4.1, default 1 */
   double tau_zs;      /* u_z: FP64 -> FP32 when ||r_k||/||b|| < tau_zs, default 1e-4 (5.1) */
   double tau_zh;      /* u_z: FP32 -> FP16 when ||r_k||/||b|| < tau_zh, default 1e-6 (5.1); 0 = never FP16 */
@@ -113,7 +131,7 @@ typedef struct {
 } amp_stats_t;
 
 /* Fill *p with the paper's defaults: amp=1, u0=FP64, eta_rule=DELAY, d=10, ell=5, C=1,
- * tau=(1e-4,1e-6), eps32=2^-24, safeties 1, scale NORM2, x0_zero=0, true_residual=0, loop AUTO. */
+ * tau=(1e-4,1e-6), eps32=2^-24, safeties 1, scale NORM2, x0_zero=0, true_residual=0, loop AUTO, profile_kernels=0. */
 void amp_policy_default(amp_policy_t *p);
 
 /* Build a solver for the SPD matrix A given in CSR (CSR per BASELINE.json).
@@ -131,6 +149,22 @@ void amp_policy_default(amp_policy_t *p);
  * Returns NULL on failure; amp_pcg_last_error() says why (invalid structure, CUDA, memory). */
 amp_pcg_t *amp_pcg_create(int64_t n, int64_t nnz, const int32_t *rowptr, const int32_t *colidx,
                           const double *vals, int precond);
+
+/* Create-time options.  amp_create_opts_default() fills the defaults; amp_pcg_create(..., precond) is
+ * amp_pcg_create_ex() with the defaults and the given preconditioner. */
+typedef struct {
+  int32_t struct_bytes;   /* sizeof(amp_create_opts_t) as the caller compiled it (ABI growth check) */
+  int32_t precond;        /* AMP_PRECOND_* */
+  int32_t index_format;   /* AMP_INDEX_*, default AUTO */
+  int32_t spmv_kernel;    /* AMP_SPMV_*, default AUTO */
+  int32_t spmv_grid_mult; /* upper bound on resident SpMV blocks per SM for the direct kernel's grid; 0 = automatic */
+  int32_t pdl;            /* 1 (default): launch the loop kernels as programmatic dependents (griddepcontrol), 0: plain */
+  void *stream;           /* cudaStream_t the create() kernels run on and the handle starts with (NULL = legacy
+                             default stream); the caller's CSR arrays must be complete in this stream's order */
+} amp_create_opts_t;
+void amp_create_opts_default(amp_create_opts_t *o);
+amp_pcg_t *amp_pcg_create_ex(int64_t n, int64_t nnz, const int32_t *rowptr, const int32_t *colidx,
+                             const double *vals, const amp_create_opts_t *opts);
 
 /* Solve A x = b to ||r_k|| <= tol ||b|| (Algorithm 3.1 or 4.1 by policy).
  *   b        float64[n], read-only
@@ -197,6 +231,51 @@ double amp_pcg_spmv_bytes(const amp_pcg_t *h, int mat_prec, int vec_prec);
  * the three vector kernels (z: r, 1/diag -> z; p: z, p -> p; x/r: x, p, q, r -> x, r).
  * amp_stats_t.algorithmic_bytes is the sum of this over the iterations of a solve. */
 double amp_pcg_iteration_bytes(const amp_pcg_t *h, int uz, int ur);
+
+/* ---- measurement: per-kernel device times of the last solve made with policy.profile_kernels = 1 ---------- */
+enum { AMP_K_Z = 0, AMP_K_P = 1, AMP_K_SPMV = 2, AMP_K_XR = 3, AMP_K_XRZ = 4, AMP_K_COUNT = 5 };
+typedef struct {
+  int32_t kernel;          /* AMP_K_*: step a2, a3, a4, a5 of SURVEY.md section 8(a) (XRZ: a5 + a2 of the lagged variant) */
+  int32_t uz, ur;          /* precision phase (u_z, u_r) of the iterations summed here */
+  int32_t launches;        /* launches of this kernel in this phase */
+  double total_ms;         /* sum over those launches of (event after - event before) on the solve stream */
+  double bytes_per_launch; /* compulsory bytes of one launch: amp_pcg_spmv_bytes() for AMP_K_SPMV, n times the
+                              per-row figures of DESIGN.md section 5 for the vector kernels */
+} amp_kernel_time_t;
+/* Writes up to cap records (one per kernel and phase that occurred) to HOST out; returns the count, 0 if the last
+ * solve was not profiled, or a negative error code. */
+int32_t amp_pcg_kernel_times(amp_pcg_t *h, amp_kernel_time_t *out_host, int32_t cap);
+
+/* ---- diagnostic entry points (parity tests; not on the hot path) ------------------------------------------
+ * Run ONE step of the loop with caller-given scalars and precisions through the SAME __global__ kernel, grid and
+ * reduction the stream / graph loop launches, on the handle's own work vectors, so that a test can compare z, p, r,
+ * x element by element with the formulas of Algorithm 4.1.
+ * Work vectors: which = AMP_VEC_*; prec = storage precision of the copy addressed (r, q: FP64/FP32; z, p:
+ * FP64/FP32/FP16; 1/diag: FP64/FP32).  src/dst are DEVICE arrays of n elements of that storage type; the library's
+ * zero padding to a multiple of 8 is kept. */
+enum { AMP_VEC_R = 0, AMP_VEC_Q = 1, AMP_VEC_Z = 2, AMP_VEC_P = 3, AMP_VEC_DINV = 4 /* get only */ };
+int amp_pcg_debug_set_vector(amp_pcg_t *h, int which, int prec, const void *src);
+int amp_pcg_debug_get_vector(amp_pcg_t *h, int which, int prec, void *dst);
+enum {
+  AMP_STEP_Z = 0,    /* a2 (+a6): z = RN_uz((r omega) dinv), rho = r^T z; r <- RN_ur(r) first if rs != ur   (lines 4-6) */
+  AMP_STEP_P = 1,    /* a3 (+a6): p = RN_uz(fma(beta, RN_uz(p), z)); first != 0: p = z                      (line 10) */
+  AMP_STEP_SPMV = 2, /* a4: q = A p in u_r, gamma = q^T p                                                   (lines 11-13) */
+  AMP_STEP_XR = 3,   /* a5: x += alpha p (FP64), r = RN_ur(fma(-alpha, q, r)), delta = ||r||               (lines 15-17) */
+  AMP_STEP_XRZ = 4   /* lagged a5 + a2: x, r = RN_ur_n(..), z = RN_uz_n((r omega_n) dinv), ||r|| and r^T z */
+};
+typedef struct {
+  int32_t step;            /* AMP_STEP_* */
+  int32_t rs, ur, uz;      /* precision r is stored in on entry; u_r and u_z of this iteration */
+  int32_t ps;              /* precision p is stored in on entry (AMP_STEP_P) */
+  int32_t ur_n, uz_n;      /* precisions of the next iteration (AMP_STEP_XRZ) */
+  int32_t first;           /* AMP_STEP_P: iteration k = 0 (p_{-1} is not read) */
+  double omega, beta, alpha, omega_n; /* scalars the step reads */
+  double sum0, sum1;       /* out: the step's scalar(s) after its grid reduction: Z: rho = r^T z | SPMV: gamma = q^T p |
+                              XR: delta = ||r||_2 | XRZ: delta = ||r||_2 and sum1 = r^T z */
+} amp_debug_step_t;
+/* x: DEVICE float64[n], read and written by AMP_STEP_XR / AMP_STEP_XRZ only (may be NULL otherwise).
+ * Synchronises the stream.  Returns AMP_OK, AMP_ERR_INVALID or AMP_ERR_CUDA. */
+int amp_pcg_debug_step(amp_pcg_t *h, amp_debug_step_t *io, double *x);
 
 #ifdef __cplusplus
 }

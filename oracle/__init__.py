@@ -91,6 +91,15 @@ def lib():
         L.orc_eta_posteriori.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_double, C.c_double, C.c_double]
         L.orc_select_uz.restype = C.c_int32
         L.orc_select_uz.argtypes = [C.POINTER(_Policy), C.c_double]
+        L.orc_step_z.restype = None
+        L.orc_step_z.argtypes = [C.c_int64, C.c_void_p, C.c_double, C.c_void_p, C.c_int32, C.c_int32, C.c_int32,
+                                 C.c_void_p, C.c_void_p]
+        L.orc_step_p.restype = None
+        L.orc_step_p.argtypes = [C.c_int64, C.c_double, C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p]
+        L.orc_step_xr.restype = None
+        L.orc_step_xr.argtypes = [C.c_int64, C.c_double, C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p]
+        L.orc_classify_fp16.restype = C.c_int32
+        L.orc_classify_fp16.argtypes = [C.c_double, C.c_double]
         L.orc_amp_pcg.restype = C.c_int32
         L.orc_amp_pcg.argtypes = [C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
                                   C.c_double, C.c_int32, C.POINTER(_Policy), C.POINTER(_Stats), C.c_void_p,
@@ -154,6 +163,42 @@ def spmv_fp32(rowptr, colidx, vals, p, accumulate64: int = 0) -> np.ndarray:
     q = np.empty(n, dtype=np.float64)
     lib().orc_spmv_fp32(n, _ptr(rowptr), _ptr(colidx), _ptr(v32), _ptr(p), _ptr(q), int(accumulate64))
     return q
+
+
+def _f64(a) -> np.ndarray:
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+def step_z(r, omega: float, dinv, ur: int, uz: int, strict: int = 0):
+    """O2: z = RN_{u_z}((r omega) dinv) (Alg 4.1 lines 4-5).  Returns (z, counts[inf, flushed, subnormal])."""
+    r, dinv = _f64(r), _f64(dinv)
+    z = np.empty_like(r)
+    counts = np.zeros(3, dtype=np.int64)
+    lib().orc_step_z(r.size, _ptr(r), float(omega), _ptr(dinv), int(ur), int(uz), int(strict), _ptr(z), _ptr(counts))
+    return z, counts
+
+
+def step_p(beta: float, p, z, uz: int):
+    """O5: p = RN_{u_z}(fma(beta, p, z)) (Alg 4.1 line 10).  Returns (p_new, counts)."""
+    z = _f64(z)
+    p = np.array(p, dtype=np.float64, copy=True)
+    counts = np.zeros(3, dtype=np.int64)
+    lib().orc_step_p(z.size, float(beta), _ptr(z), int(uz), _ptr(p), _ptr(counts))
+    return p, counts
+
+
+def step_xr(alpha: float, p, q, x, r, ur: int):
+    """O9, O10: x = fma(alpha, p, x) (FP64); r = RN_{u_r}(fma(-alpha, q, r)) (Alg 4.1 lines 15-16).  Returns (x, r)."""
+    p, q = _f64(p), _f64(q)
+    x = np.array(x, dtype=np.float64, copy=True)
+    r = np.array(r, dtype=np.float64, copy=True)
+    lib().orc_step_xr(p.size, float(alpha), _ptr(p), _ptr(q), int(ur), _ptr(x), _ptr(r))
+    return x, r
+
+
+def classify_fp16(unrounded: float, stored: float) -> int:
+    """1 = became inf, 2 = flushed to zero, 3 = subnormal, 0 = anything else."""
+    return int(lib().orc_classify_fp16(float(unrounded), float(stored)))
 
 
 def eta(policy: _Policy, hist: np.ndarray, k: int) -> float:

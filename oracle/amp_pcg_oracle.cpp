@@ -22,6 +22,8 @@
 //                                     and (4.11) (:370-375).  x, all inner products, norms
 //                                     and scalars are FP64.
 //   orc_eta_posteriori                the a-posteriori indicator eta_hat_m(k) of (4.7) (:350-354).
+//   orc_step_z / orc_step_p / orc_step_xr   the vector steps of the loop body (Alg 4.1 lines 4-5, 10, 15-16),
+//                                     called by orc_amp_pcg and, one at a time, by the per-step GPU parity tests.
 //
 // Low-precision STORAGE is emulated by explicit rounding: every vector is a double array that
 // holds values exactly representable in its storage format.  Readings of the garbled or
@@ -225,6 +227,61 @@ static inline int classify_fp16(double unrounded, double stored) {
   return 0;
 }
 
+// ---------------------------------------------------------------- the vector steps ---------
+// One function per vector step of the loop body, in the paper's notation; orc_amp_pcg below calls exactly these,
+// and the per-step GPU parity tests call them one at a time.  Vectors are double arrays holding values that are
+// exactly representable in their storage precision; counts (may be NULL) = {became inf, flushed to zero, subnormal}
+// of the FP16 stores of this call (only counted when uz = FP16).
+
+// O2, Alg 4.1 lines 4-5 (PAPER.md:274-276; Alg 3.2 line 3; scaling fused with the preconditioner, :223), M = diag:
+//   z_i = RN_{u_z}( (r_i * omega) * dinv_i )                 FP64 arithmetic, ONE rounding (reading R6)
+// strict != 0 is the diagnostic of reading R6: y = RN_{u_z}(RN_{u_r}(r omega)), M^-1 rounded to u_z, z = RN_{u_z}(y M^-1)
+// (dinv must then be the FP64 1/a_ii).
+void orc_step_z(int64_t n, const double* r, double omega, const double* dinv, int32_t ur, int32_t uz, int32_t strict,
+                double* z, int64_t* counts) {
+  int64_t c_inf = 0, c_flush = 0, c_sub = 0;
+#pragma omp parallel for schedule(static) reduction(+ : c_inf, c_flush, c_sub)
+  for (int64_t i = 0; i < n; ++i) {
+    double zi;
+    if (strict) {
+      const double y = round_store(round_store(r[i] * omega, ur), uz);
+      zi = y * round_store(dinv[i], uz);
+    } else {
+      zi = (r[i] * omega) * dinv[i];
+    }
+    const double zs = round_store(zi, uz);
+    if (uz == ORC_FP16) { const int c = classify_fp16(zi, zs); c_inf += (c == 1); c_flush += (c == 2); c_sub += (c == 3); }
+    z[i] = zs;
+  }
+  if (counts) { counts[0] += c_inf; counts[1] += c_flush; counts[2] += c_sub; }
+}
+
+// O5, Alg 4.1 line 10: p_i = RN_{u_z}( fma(beta, p_i, z_i) ), one rounding
+void orc_step_p(int64_t n, double beta, const double* z, int32_t uz, double* p, int64_t* counts) {
+  int64_t c_inf = 0, c_flush = 0, c_sub = 0;
+#pragma omp parallel for schedule(static) reduction(+ : c_inf, c_flush, c_sub)
+  for (int64_t i = 0; i < n; ++i) {
+    const double pi = std::fma(beta, p[i], z[i]);
+    const double ps = round_store(pi, uz);
+    if (uz == ORC_FP16) { const int c = classify_fp16(pi, ps); c_inf += (c == 1); c_flush += (c == 2); c_sub += (c == 3); }
+    p[i] = ps;
+  }
+  if (counts) { counts[0] += c_inf; counts[1] += c_flush; counts[2] += c_sub; }
+}
+
+// O9, O10, Alg 4.1 lines 15-16: x_i = fma(alpha, p_i, x_i) in FP64 (:241);
+// r_i = RN_{u_r}( fma(-alpha, q_i, r_i) ), FP64 arithmetic on the stored values, one rounding (reading R8)
+void orc_step_xr(int64_t n, double alpha, const double* p, const double* q, int32_t ur, double* x, double* r) {
+#pragma omp parallel for schedule(static)
+  for (int64_t i = 0; i < n; ++i) {
+    x[i] = std::fma(alpha, p[i], x[i]);
+    r[i] = round_store(std::fma(-alpha, q[i], r[i]), ur);
+  }
+}
+
+// classification of one FP16 store (see classify_fp16), exported for its pin
+int32_t orc_classify_fp16(double unrounded, double stored) { return classify_fp16(unrounded, stored); }
+
 // ---------------------------------------------------------------- the solver --------------
 // Algorithm 4.1 (amp=1) / Algorithm 3.1 (amp=0), step by step in the paper's order.
 // x: in = x0, out = x_m.  hist (may be NULL) receives ||r_t||, t = 0..iters.
@@ -241,8 +298,8 @@ int32_t orc_amp_pcg(int64_t n, const int32_t* rowptr, const int32_t* colidx, con
   for (int64_t i = 0; i < n; ++i) {
     double d = 1.0;
     if (pol->precond == 1) {
-      d = 0.0;
-      for (int32_t e = rowptr[i]; e < rowptr[i + 1]; ++e) if (colidx[e] == i) d = vals[e];
+      d = 0.0;   // M = diag(A) (Jacobi); duplicate entries add up, as they do in the mat-vec
+      for (int32_t e = rowptr[i]; e < rowptr[i + 1]; ++e) if (colidx[e] == i) d += vals[e];
       if (!(d > 0.0)) { st->status = -1; return -1; }
     }
     dinv[(size_t)i] = 1.0 / d;
@@ -318,34 +375,17 @@ int32_t orc_amp_pcg(int64_t n, const int32_t* rowptr, const int32_t* colidx, con
     }
     // O2: y = omega r, z = M^-1 y  (Alg 4.1 lines 4-5; Alg 3.2 line 3; fused)
     const double omega = !pol->amp ? 1.0 : (lag ? omega_lag : scale_factor(pol, delta, n));
-    const double* dv = (uz == ORC_FP64) ? dinv.data() : dinv32.data();            // R6
-    int64_t c_inf = 0, c_flush = 0, c_sub = 0;
-#pragma omp parallel for schedule(static) reduction(+ : c_inf, c_flush, c_sub)
-    for (int64_t i = 0; i < n; ++i) {
-      double zi;
-      if (pol->strict_rounding && pol->amp) {
-        const double y = round_store(round_store(r[(size_t)i] * omega, ur), uz);
-        zi = y * round_store(dinv[(size_t)i], uz);
-      } else {
-        zi = (r[(size_t)i] * omega) * dv[(size_t)i];
-      }
-      const double zs = round_store(zi, uz);
-      if (uz == ORC_FP16) { const int c = classify_fp16(zi, zs); c_inf += (c == 1); c_flush += (c == 2); c_sub += (c == 3); }
-      z[(size_t)i] = zs;
-    }
+    const bool strict = pol->strict_rounding && pol->amp;
+    const double* dv = (uz == ORC_FP64 || strict) ? dinv.data() : dinv32.data();            // R6
+    int64_t counts[3] = {0, 0, 0};
+    orc_step_z(n, r.data(), omega, dv, ur, uz, strict ? 1 : 0, z.data(), counts);
     // O3: rho = r^T z (Alg 4.1 line 6), FP64, with the stored z
     const double rho = dot_fp64(n, r.data(), z.data());
     // O4: beta (lines 7-9)
     const double beta = (k > 0) ? rho / rho_prev : 0.0;
     // O5: p = z + beta p (line 10), one rounding to u_z
-#pragma omp parallel for schedule(static) reduction(+ : c_inf, c_flush, c_sub)
-    for (int64_t i = 0; i < n; ++i) {
-      const double pi = std::fma(beta, p[(size_t)i], z[(size_t)i]);
-      const double ps = round_store(pi, uz);
-      if (uz == ORC_FP16) { const int c = classify_fp16(pi, ps); c_inf += (c == 1); c_flush += (c == 2); c_sub += (c == 3); }
-      p[(size_t)i] = ps;
-    }
-    if (uz == ORC_FP16) { st->fp16_inf += c_inf; st->fp16_flushed += c_flush; st->fp16_subnormal += c_sub; st->fp16_stored += 2 * n; }
+    orc_step_p(n, beta, z.data(), uz, p.data(), counts);
+    if (uz == ORC_FP16) { st->fp16_inf += counts[0]; st->fp16_flushed += counts[1]; st->fp16_subnormal += counts[2]; st->fp16_stored += 2 * n; }
     // O6: q = A p in u_r (line 11)
     if (ur == ORC_FP64) orc_spmv_fp64(n, rowptr, colidx, vals, p.data(), q.data());
     else orc_spmv_fp32(n, rowptr, colidx, vals32.data(), p.data(), q.data(), pol->accumulate64);
@@ -355,11 +395,7 @@ int32_t orc_amp_pcg(int64_t n, const int32_t* rowptr, const int32_t* colidx, con
     // O8: alpha (line 14)
     const double alpha = rho / gamma;
     // O9: x += alpha p in FP64 (line 15); O10: r -= alpha q in u_r (line 16), one rounding
-#pragma omp parallel for schedule(static)
-    for (int64_t i = 0; i < n; ++i) {
-      x[i] = std::fma(alpha, p[(size_t)i], x[i]);
-      r[(size_t)i] = round_store(std::fma(-alpha, q[(size_t)i], r[(size_t)i]), lag ? ur_n : ur);
-    }
+    orc_step_xr(n, alpha, p.data(), q.data(), lag ? ur_n : ur, x, r.data());
     // O11: delta_{k+1} = ||r_{k+1}|| (line 17)
     const double delta_k = delta;
     delta = std::sqrt(dot_fp64(n, r.data(), r.data()));

@@ -9,6 +9,9 @@ from .binding import (  # noqa: F401
     AmpPcg,
     Policy,
     Stats,
+    CreateOpts,
+    KernelTime,
+    DebugStep,
     AmpPcgError,
     bytes_per_row,
     load_library,
@@ -18,5 +21,10 @@ from .binding import (  # noqa: F401
     SCALE_NORM2, SCALE_RMS, SCALE_POW2, SCALE_NONE, SCALE_LAGGED,
     LOOP_AUTO, LOOP_STREAM, LOOP_GRAPH, LOOP_PERSISTENT,
     PRECOND_NONE, PRECOND_JACOBI,
+    INDEX_AUTO, INDEX_NO_ALIGN, INDEX_FORCE32,
+    SPMV_AUTO, SPMV_DIRECT, SPMV_PIPELINED,
+    K_Z, K_P, K_SPMV, K_XR, K_XRZ, KERNEL_NAMES,
+    VEC_R, VEC_Q, VEC_Z, VEC_P, VEC_DINV,
+    STEP_Z, STEP_P, STEP_SPMV, STEP_XR, STEP_XRZ,
     EXPORTED_SYMBOLS,
 )

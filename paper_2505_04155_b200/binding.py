@@ -17,12 +17,20 @@ ETA_DELAY, ETA_LINEAR, ETA_NEVER = 0, 1, 2
 SCALE_NORM2, SCALE_RMS, SCALE_POW2, SCALE_NONE, SCALE_LAGGED = 0, 1, 2, 3, 4
 LOOP_AUTO, LOOP_STREAM, LOOP_GRAPH, LOOP_PERSISTENT = 0, 1, 2, 3
 PRECOND_NONE, PRECOND_JACOBI = 0, 1
+INDEX_AUTO, INDEX_NO_ALIGN, INDEX_FORCE32 = 0, 1, 2
+SPMV_AUTO, SPMV_DIRECT, SPMV_PIPELINED = 0, 1, 2
+K_Z, K_P, K_SPMV, K_XR, K_XRZ = 0, 1, 2, 3, 4
+KERNEL_NAMES = {K_Z: "k_z", K_P: "k_p", K_SPMV: "k_spmv", K_XR: "k_xr", K_XRZ: "k_xrz"}
+VEC_R, VEC_Q, VEC_Z, VEC_P, VEC_DINV = 0, 1, 2, 3, 4
+STEP_Z, STEP_P, STEP_SPMV, STEP_XR, STEP_XRZ = 0, 1, 2, 3, 4
 
 EXPORTED_SYMBOLS = (
-    "amp_policy_default", "amp_pcg_create", "amp_pcg_solve", "amp_pcg_solve_host", "amp_spmv",
+    "amp_policy_default", "amp_create_opts_default", "amp_pcg_create", "amp_pcg_create_ex", "amp_pcg_solve",
+    "amp_pcg_solve_host", "amp_spmv",
     "amp_pcg_residual_history", "amp_pcg_set_stream", "amp_pcg_last_launch_count", "amp_pcg_destroy",
     "amp_pcg_last_error", "amp_pcg_bytes_per_row", "amp_pcg_spmv_bytes", "amp_pcg_iteration_bytes",
-    "amp_pcg_eta_posteriori",
+    "amp_pcg_eta_posteriori", "amp_pcg_kernel_times",
+    "amp_pcg_debug_set_vector", "amp_pcg_debug_get_vector", "amp_pcg_debug_step",
 )
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
@@ -38,7 +46,7 @@ class Policy(C.Structure):
     _fields_ = [
         ("amp", C.c_int32), ("u0", C.c_int32), ("eta_rule", C.c_int32), ("d", C.c_int32), ("ell", C.c_int32),
         ("scale_mode", C.c_int32), ("no_stop", C.c_int32), ("x0_zero", C.c_int32), ("true_residual", C.c_int32),
-        ("loop_mode", C.c_int32),
+        ("loop_mode", C.c_int32), ("profile_kernels", C.c_int32), ("reserved0", C.c_int32),
         ("C", C.c_double), ("tau_zs", C.c_double), ("tau_zh", C.c_double), ("eps32", C.c_double),
         ("eta_safety", C.c_double), ("stop_safety", C.c_double),
     ]
@@ -52,6 +60,41 @@ class Policy(C.Structure):
                 raise AttributeError(k)
             setattr(p, k, v)
         return p
+
+
+class CreateOpts(C.Structure):
+    """amp_create_opts_t (include/amp_pcg.h)."""
+
+    _fields_ = [
+        ("struct_bytes", C.c_int32), ("precond", C.c_int32), ("index_format", C.c_int32), ("spmv_kernel", C.c_int32),
+        ("spmv_grid_mult", C.c_int32), ("pdl", C.c_int32), ("stream", C.c_void_p),
+    ]
+
+    @classmethod
+    def default(cls, **overrides) -> "CreateOpts":
+        o = cls()
+        load_library().amp_create_opts_default(C.byref(o))
+        for k, v in overrides.items():
+            if not hasattr(o, k):
+                raise AttributeError(k)
+            setattr(o, k, v)
+        return o
+
+
+class KernelTime(C.Structure):
+    """amp_kernel_time_t (include/amp_pcg.h)."""
+
+    _fields_ = [("kernel", C.c_int32), ("uz", C.c_int32), ("ur", C.c_int32), ("launches", C.c_int32),
+                ("total_ms", C.c_double), ("bytes_per_launch", C.c_double)]
+
+
+class DebugStep(C.Structure):
+    """amp_debug_step_t (include/amp_pcg.h)."""
+
+    _fields_ = [("step", C.c_int32), ("rs", C.c_int32), ("ur", C.c_int32), ("uz", C.c_int32), ("ps", C.c_int32),
+                ("ur_n", C.c_int32), ("uz_n", C.c_int32), ("first", C.c_int32),
+                ("omega", C.c_double), ("beta", C.c_double), ("alpha", C.c_double), ("omega_n", C.c_double),
+                ("sum0", C.c_double), ("sum1", C.c_double)]
 
 
 class Stats(C.Structure):
@@ -69,19 +112,19 @@ class Stats(C.Structure):
         return {k: getattr(self, k) for k, _ in self._fields_}
 
 
-_lib = None
+_libs = {}
 
 
-def library_path() -> str:
-    return os.path.join(_HERE, "libamp_pcg.so")
+def library_path(variant: str = "") -> str:
+    """In-tree CUDA library; variant "count" = the -DAMP_COUNT_FP16 build (FP16 store counters filled)."""
+    return os.path.join(_HERE, "libamp_pcg.so" if not variant else f"libamp_pcg_{variant}.so")
 
 
-def load_library():
+def load_library(variant: str = ""):
     """dlopen the in-tree CUDA library (no build here: see build.py / __graft_entry__.build)."""
-    global _lib
-    if _lib is not None:
-        return _lib
-    path = library_path()
+    if variant in _libs:
+        return _libs[variant]
+    path = library_path(variant)
     if not os.path.exists(path):
         raise AmpPcgError(f"{path} is missing: build it with `python -m paper_2505_04155_b200.build` "
                           "(there is no CPU fallback)")
@@ -89,8 +132,12 @@ def load_library():
     vp, i32, i64, dbl = C.c_void_p, C.c_int32, C.c_int64, C.c_double
     L.amp_policy_default.restype = None
     L.amp_policy_default.argtypes = [C.POINTER(Policy)]
+    L.amp_create_opts_default.restype = None
+    L.amp_create_opts_default.argtypes = [C.POINTER(CreateOpts)]
     L.amp_pcg_create.restype = vp
     L.amp_pcg_create.argtypes = [i64, i64, vp, vp, vp, C.c_int]
+    L.amp_pcg_create_ex.restype = vp
+    L.amp_pcg_create_ex.argtypes = [i64, i64, vp, vp, vp, C.POINTER(CreateOpts)]
     L.amp_pcg_solve.restype = C.c_int
     L.amp_pcg_solve.argtypes = [vp, vp, vp, dbl, i32, C.POINTER(Policy), C.POINTER(Stats)]
     L.amp_pcg_solve_host.restype = C.c_int
@@ -115,7 +162,15 @@ def load_library():
     L.amp_pcg_spmv_bytes.argtypes = [vp, C.c_int, C.c_int]
     L.amp_pcg_iteration_bytes.restype = dbl
     L.amp_pcg_iteration_bytes.argtypes = [vp, C.c_int, C.c_int]
-    _lib = L
+    L.amp_pcg_kernel_times.restype = i32
+    L.amp_pcg_kernel_times.argtypes = [vp, C.POINTER(KernelTime), i32]
+    L.amp_pcg_debug_set_vector.restype = C.c_int
+    L.amp_pcg_debug_set_vector.argtypes = [vp, C.c_int, C.c_int, vp]
+    L.amp_pcg_debug_get_vector.restype = C.c_int
+    L.amp_pcg_debug_get_vector.argtypes = [vp, C.c_int, C.c_int, vp]
+    L.amp_pcg_debug_step.restype = C.c_int
+    L.amp_pcg_debug_step.argtypes = [vp, C.POINTER(DebugStep), vp]
+    _libs[variant] = L
     return L
 
 
@@ -123,18 +178,20 @@ def bytes_per_row(m: float, uz: int, ur: int) -> float:
     return float(load_library().amp_pcg_bytes_per_row(float(m), int(uz), int(ur)))
 
 
-def _last_error() -> str:
-    return load_library().amp_pcg_last_error().decode("utf-8", "replace")
+def _last_error(L=None) -> str:
+    return (L or load_library()).amp_pcg_last_error().decode("utf-8", "replace")
 
 
 class AmpPcg:
-    """One SPD matrix in CSR on the current CUDA device (amp_pcg_create ... amp_pcg_destroy).
+    """One SPD matrix in CSR on the current CUDA device (amp_pcg_create_ex ... amp_pcg_destroy).
 
     ``rowptr`` (int32[n+1]), ``colidx`` (int32[nnz]) and ``vals`` (float64[nnz]) are CUDA torch
     tensors; they are borrowed by the library, so this object keeps references to them.
+    ``opts``: keyword overrides of amp_create_opts_t (index_format, spmv_kernel, spmv_grid_mult, pdl);
+    the create() kernels run on torch's current stream.  ``variant="count"`` loads the counting build.
     """
 
-    def __init__(self, rowptr, colidx, vals, precond: int = PRECOND_JACOBI):
+    def __init__(self, rowptr, colidx, vals, precond: int = PRECOND_JACOBI, variant: str = "", **opts):
         import torch
 
         if not (rowptr.is_cuda and colidx.is_cuda and vals.is_cuda):
@@ -146,21 +203,29 @@ class AmpPcg:
         self.nnz = int(colidx.numel())
         self.device = vals.device
         self._torch = torch
-        L = load_library()
+        self._L = L = load_library(variant)
+        o = CreateOpts()
+        L.amp_create_opts_default(C.byref(o))
+        o.precond = int(precond)
+        for k, v in opts.items():
+            if not hasattr(o, k) or k in ("struct_bytes", "stream"):
+                raise AttributeError(k)
+            setattr(o, k, v)
         with torch.cuda.device(self.device):
-            self._h = L.amp_pcg_create(self.n, self.nnz, self._keep[0].data_ptr(), self._keep[1].data_ptr(),
-                                       self._keep[2].data_ptr(), int(precond))
+            o.stream = torch.cuda.current_stream(self.device).cuda_stream
+            self._h = L.amp_pcg_create_ex(self.n, self.nnz, self._keep[0].data_ptr(), self._keep[1].data_ptr(),
+                                          self._keep[2].data_ptr(), C.byref(o))
         if not self._h:
-            raise AmpPcgError(_last_error())
+            raise AmpPcgError(_last_error(L))
 
     # -- helpers --------------------------------------------------------------------------
     def _sync_stream(self):
         s = self._torch.cuda.current_stream(self.device).cuda_stream
-        load_library().amp_pcg_set_stream(self._h, C.c_void_p(s))
+        self._L.amp_pcg_set_stream(self._h, C.c_void_p(s))
 
     def _check(self, rc: int, allow=(0, 1, -2)):
         if rc not in allow:
-            raise AmpPcgError(f"amp_pcg error {rc}: {_last_error()}")
+            raise AmpPcgError(f"amp_pcg error {rc}: {_last_error(self._L)}")
 
     # -- C ABI ----------------------------------------------------------------------------
     def solve(self, b, x, tol: float, maxit: int, policy: Optional[Policy] = None) -> Stats:
@@ -173,8 +238,8 @@ class AmpPcg:
         st = Stats()
         with torch.cuda.device(self.device):
             self._sync_stream()
-            rc = load_library().amp_pcg_solve(self._h, b.data_ptr(), x.data_ptr(), float(tol), int(maxit),
-                                              C.byref(policy) if policy is not None else None, C.byref(st))
+            rc = self._L.amp_pcg_solve(self._h, b.data_ptr(), x.data_ptr(), float(tol), int(maxit),
+                                       C.byref(policy) if policy is not None else None, C.byref(st))
         self._check(rc)
         self._last_iters = int(st.iters)
         return st
@@ -186,8 +251,8 @@ class AmpPcg:
         xp = x_host.data_ptr() if hasattr(x_host, "data_ptr") else x_host.ctypes.data
         with self._torch.cuda.device(self.device):
             self._sync_stream()
-            rc = load_library().amp_pcg_solve_host(self._h, bp, xp, float(tol), int(maxit),
-                                                   C.byref(policy) if policy is not None else None, C.byref(st))
+            rc = self._L.amp_pcg_solve_host(self._h, bp, xp, float(tol), int(maxit),
+                                            C.byref(policy) if policy is not None else None, C.byref(st))
         self._check(rc)
         self._last_iters = int(st.iters)
         return st
@@ -204,42 +269,89 @@ class AmpPcg:
             raise AmpPcgError("out has the wrong dtype/size")
         with torch.cuda.device(self.device):
             self._sync_stream()
-            rc = load_library().amp_spmv(self._h, int(mat_prec), vec_prec, p.data_ptr(), q.data_ptr())
+            rc = self._L.amp_spmv(self._h, int(mat_prec), vec_prec, p.data_ptr(), q.data_ptr())
         self._check(rc, allow=(0,))
         return q
 
     def residual_history(self) -> np.ndarray:
         """amp_pcg_residual_history: ||r_t||, t = 0..iters of the last solve (host numpy array)."""
         buf = np.empty(self._last_iters + 1, dtype=np.float64)
-        m = load_library().amp_pcg_residual_history(self._h, buf.ctypes.data, buf.size)
+        m = self._L.amp_pcg_residual_history(self._h, buf.ctypes.data, buf.size)
         if m < 0:
-            raise AmpPcgError(_last_error())
+            raise AmpPcgError(_last_error(self._L))
         return buf[:m]
 
     _last_iters = -1
 
     def last_launch_count(self) -> int:
-        return int(load_library().amp_pcg_last_launch_count(self._h))
+        return int(self._L.amp_pcg_last_launch_count(self._h))
 
     def eta_posteriori(self, C_: float = 1.0, eps32: float = 0.0) -> np.ndarray:
         """amp_pcg_eta_posteriori: eta_hat_m(k), k = 0..iters, of the last solve (host numpy array)."""
         buf = np.empty(max(self._last_iters + 1, 1), dtype=np.float64)
-        m = load_library().amp_pcg_eta_posteriori(self._h, float(C_), float(eps32), buf.ctypes.data, buf.size)
+        m = self._L.amp_pcg_eta_posteriori(self._h, float(C_), float(eps32), buf.ctypes.data, buf.size)
         if m < 0:
-            raise AmpPcgError(_last_error())
+            raise AmpPcgError(_last_error(self._L))
         return buf[:m]
 
     def spmv_bytes(self, mat_prec: int, vec_prec: int) -> float:
         """amp_pcg_spmv_bytes: compulsory bytes of one mat-vec with the matrix format this handle built."""
-        return float(load_library().amp_pcg_spmv_bytes(self._h, int(mat_prec), int(vec_prec)))
+        return float(self._L.amp_pcg_spmv_bytes(self._h, int(mat_prec), int(vec_prec)))
 
     def iteration_bytes(self, uz: int, ur: int) -> float:
         """amp_pcg_iteration_bytes: compulsory bytes of one iteration in phase (u_z, u_r)."""
-        return float(load_library().amp_pcg_iteration_bytes(self._h, int(uz), int(ur)))
+        return float(self._L.amp_pcg_iteration_bytes(self._h, int(uz), int(ur)))
+
+    def kernel_times(self):
+        """amp_pcg_kernel_times: per (kernel, u_z, u_r) records of the last solve made with profile_kernels=1."""
+        buf = (KernelTime * 64)()
+        m = self._L.amp_pcg_kernel_times(self._h, buf, 64)
+        if m < 0:
+            raise AmpPcgError(_last_error(self._L))
+        return [dict(kernel=KERNEL_NAMES[r.kernel], uz=r.uz, ur=r.ur, launches=r.launches, total_ms=r.total_ms,
+                     bytes_per_launch=r.bytes_per_launch) for r in buf[:m]]
+
+    # -- diagnostic entry points (parity tests) -------------------------------------------
+    _TORCH_DT = None
+
+    def _dtype(self, prec: int):
+        torch = self._torch
+        return {FP64: torch.float64, FP32: torch.float32, FP16: torch.float16}[prec]
+
+    def debug_set_vector(self, which: int, t):
+        """amp_pcg_debug_set_vector: copy a CUDA tensor of n elements into the work vector stored in t.dtype."""
+        torch = self._torch
+        prec = {torch.float64: FP64, torch.float32: FP32, torch.float16: FP16}[t.dtype]
+        if t.numel() != self.n or not t.is_cuda or not t.is_contiguous():
+            raise AmpPcgError("debug_set_vector needs a contiguous CUDA tensor of n elements")
+        with torch.cuda.device(self.device):
+            self._sync_stream()
+            self._check(self._L.amp_pcg_debug_set_vector(self._h, int(which), prec, t.data_ptr()), allow=(0,))
+
+    def debug_get_vector(self, which: int, prec: int):
+        torch = self._torch
+        out = torch.empty(self.n, dtype=self._dtype(prec), device=self.device)
+        with torch.cuda.device(self.device):
+            self._sync_stream()
+            self._check(self._L.amp_pcg_debug_get_vector(self._h, int(which), int(prec), out.data_ptr()), allow=(0,))
+        return out
+
+    def debug_step(self, step: int, x=None, **kw) -> DebugStep:
+        """amp_pcg_debug_step: one step of the loop with caller-given scalars / precisions (see the header)."""
+        io = DebugStep(step=int(step), omega=1.0, beta=0.0, alpha=0.0, omega_n=1.0)
+        for k, v in kw.items():
+            if not hasattr(io, k):
+                raise AttributeError(k)
+            setattr(io, k, v)
+        with self._torch.cuda.device(self.device):
+            self._sync_stream()
+            rc = self._L.amp_pcg_debug_step(self._h, C.byref(io), x.data_ptr() if x is not None else None)
+        self._check(rc, allow=(0,))
+        return io
 
     def close(self):
         if getattr(self, "_h", None):
-            load_library().amp_pcg_destroy(self._h)
+            self._L.amp_pcg_destroy(self._h)
             self._h = None
 
     def __del__(self):

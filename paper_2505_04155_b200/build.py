@@ -22,29 +22,41 @@ NVCC_FLAGS = [
 ]
 
 
-def needs_build() -> bool:
-    if not os.path.exists(LIB):
+def needs_build(lib: str = None) -> bool:
+    lib = lib or LIB
+    if not os.path.exists(lib):
         return True
-    t = os.path.getmtime(LIB)
+    t = os.path.getmtime(lib)
     deps = [os.path.join(CSRC, f) for f in SOURCES + HEADERS] + [os.path.join(HERE, "..", "include", "amp_pcg.h")]
     return any(os.path.getmtime(d) > t for d in deps)
 
 
-def build(force: bool = False, verbose: bool = False, extra_flags=()) -> str:
-    if not force and not needs_build():
-        return LIB
+LIB_COUNT = os.path.join(HERE, "libamp_pcg_count.so")
+
+
+def build_counting(force: bool = False) -> str:
+    """The counting build (-DAMP_COUNT_FP16): every FP16 store of z and p is classified (subnormal / flushed to
+    zero / overflowed) into amp_stats_t.fp16_*.  Slower (atomics); used by the tests and the omega study only."""
+    return build(force=force, extra_flags=("-DAMP_COUNT_FP16",), out=LIB_COUNT)
+
+
+def build(force: bool = False, verbose: bool = False, extra_flags=(), out: str = LIB) -> str:
+    if not force and not needs_build(out):
+        return out
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     cmd = [nvcc, *NVCC_FLAGS, *extra_flags]
     if verbose:
         cmd += ["-Xptxas", "-v"]
-    cmd += [os.path.join(CSRC, s) for s in SOURCES] + ["-o", LIB]
+    cmd += [os.path.join(CSRC, s) for s in SOURCES] + ["-o", out]
     res = subprocess.run(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)
     if verbose or res.returncode != 0:
         sys.stderr.write(res.stdout)
     if res.returncode != 0:
-        raise RuntimeError("nvcc failed building libamp_pcg.so")
-    return LIB
+        raise RuntimeError("nvcc failed building " + os.path.basename(out))
+    return out
 
 
 if __name__ == "__main__":
     print(build(force=True, verbose="-v" in sys.argv))
+    if "--counting" in sys.argv:
+        print(build_counting(force=True))

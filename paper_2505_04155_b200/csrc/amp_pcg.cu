@@ -68,6 +68,12 @@ struct amp_pcg {
   double idx_bytes_total = 0.0;  // bytes of index data one SpMV reads (slice table, bases, per-entry indices, row order)
   double long_bytes_idx = 0.0, long_entries = 0.0;  // long rows, read from the CSR arrays (4 B index per entry)
   int64_t sell_entries = 0;   // stored entries of the SELL-32 repack (padding included)
+  // per-kernel event profile of the last solve (policy.profile_kernels, stream loop)
+  std::vector<cudaEvent_t> prof_events;  // pool, grown on demand
+  size_t prof_used = 0;
+  std::vector<int8_t> prof_kernel;       // kernel id of the launch that FOLLOWS event i (-1: end of an iteration)
+  std::vector<int32_t> prof_iter;        // iteration index the launch belongs to
+  std::vector<amp_kernel_time_t> prof_result;
 };
 
 template <class T> static T* dev_alloc(amp_pcg* h, size_t count, bool zero) {
@@ -135,14 +141,51 @@ extern "C" void amp_pcg_destroy(amp_pcg_t* h) {
   if (h->h_flag) cudaFreeHost(h->h_flag);
   if (h->ev0) cudaEventDestroy(h->ev0);
   if (h->ev1) cudaEventDestroy(h->ev1);
+  for (cudaEvent_t e : h->prof_events) cudaEventDestroy(e);
   delete h;
 }
 
 static bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
+extern "C" void amp_create_opts_default(amp_create_opts_t* o) {
+  if (!o) return;
+  std::memset(o, 0, sizeof(*o));
+  o->struct_bytes = (int32_t)sizeof(*o);
+  o->precond = AMP_PRECOND_JACOBI;
+  o->index_format = AMP_INDEX_AUTO;
+  o->spmv_kernel = AMP_SPMV_AUTO;
+  o->spmv_grid_mult = 0;
+  o->pdl = 1;
+  o->stream = nullptr;
+}
+
 extern "C" amp_pcg_t* amp_pcg_create(int64_t n, int64_t nnz, const int32_t* rowptr, const int32_t* colidx,
                                      const double* vals, int precond) {
+  amp_create_opts_t o;
+  amp_create_opts_default(&o);
+  o.precond = precond;
+  return amp_pcg_create_ex(n, nnz, rowptr, colidx, vals, &o);
+}
+
+extern "C" amp_pcg_t* amp_pcg_create_ex(int64_t n, int64_t nnz, const int32_t* rowptr, const int32_t* colidx,
+                                        const double* vals, const amp_create_opts_t* opts) {
   g_last_error.clear();
+  amp_create_opts_t o;
+  amp_create_opts_default(&o);
+  if (opts) {
+    if (opts->struct_bytes != (int32_t)sizeof(amp_create_opts_t)) {
+      set_error("amp_pcg_create_ex: opts->struct_bytes = %d, this library expects %d (use amp_create_opts_default)",
+                opts->struct_bytes, (int)sizeof(amp_create_opts_t));
+      return nullptr;
+    }
+    o = *opts;
+  }
+  const int precond = o.precond;
+  if (o.index_format < AMP_INDEX_AUTO || o.index_format > AMP_INDEX_FORCE32 || o.spmv_kernel < AMP_SPMV_AUTO ||
+      o.spmv_kernel > AMP_SPMV_PIPELINED || o.spmv_grid_mult < 0 || (o.pdl != 0 && o.pdl != 1)) {
+    set_error("amp_pcg_create_ex: invalid index_format / spmv_kernel / spmv_grid_mult / pdl");
+    return nullptr;
+  }
   if (n <= 0 || n > (int64_t)0x7fffffff - 64 || nnz < 0 || nnz > (int64_t)0x7fffffff - 64) {
     set_error("amp_pcg_create: n and nnz must satisfy 0 < n, 0 <= nnz < 2^31 (got n=%lld nnz=%lld)", (long long)n, (long long)nnz);
     return nullptr;
@@ -162,6 +205,8 @@ extern "C" amp_pcg_t* amp_pcg_create(int64_t n, int64_t nnz, const int32_t* rowp
     return nullptr;
   }
   amp_pcg* h = new amp_pcg();
+  h->stream = static_cast<cudaStream_t>(o.stream);
+  h->pdl = o.pdl;
   CU_TRY(cudaGetDevice(&h->device), { delete h; return nullptr; });
   cudaDeviceProp prop;
   CU_TRY(cudaGetDeviceProperties(&prop, h->device), { delete h; return nullptr; });
@@ -178,9 +223,8 @@ extern "C" amp_pcg_t* amp_pcg_create(int64_t n, int64_t nnz, const int32_t* rowp
     if (!dst) { amp_pcg_destroy(h); return nullptr; }                   \
   } while (0)
   const size_t np = (size_t)h->npad;
-  double* dinv64; float* dinv32; float* vals32; int* flags;
+  double* dinv64; float* dinv32; int* flags;
   ALLOC(dinv64, double, np); ALLOC(dinv32, float, np);
-  ALLOC(vals32, float, (size_t)nnz + 8);
   ALLOC(c.r64, double, np); ALLOC(c.r32, float, np);
   ALLOC(c.q64, double, np); ALLOC(c.q32, float, np);
   ALLOC(c.z64, double, np); ALLOC(c.z32, float, np); ALLOC(c.z16, __half, np);
@@ -190,7 +234,7 @@ extern "C" amp_pcg_t* amp_pcg_create(int64_t n, int64_t nnz, const int32_t* rowp
   ALLOC(flags, int, 1);
   ALLOC(h->d_b_stage, double, np);
   ALLOC(h->d_x_stage, double, np);
-  c.dinv64 = dinv64; c.dinv32 = dinv32; c.vals32 = vals32;
+  c.dinv64 = dinv64; c.dinv32 = dinv32; c.vals32 = nullptr;
   CU_TRY(cudaMallocHost(&h->h_state, sizeof(DevState)), { amp_pcg_destroy(h); return nullptr; });
   CU_TRY(cudaMallocHost(&h->h_flag, 64), { amp_pcg_destroy(h); return nullptr; });
   CU_TRY(cudaEventCreate(&h->ev0), { amp_pcg_destroy(h); return nullptr; });
@@ -200,10 +244,6 @@ extern "C" amp_pcg_t* amp_pcg_create(int64_t n, int64_t nnz, const int32_t* rowp
   const int vgrid = (int)std::min<int64_t>((n + 255) / 256, (int64_t)h->num_sms * 16);
   k_validate_dinv<<<vgrid, 256, 0, h->stream>>>(n, nnz, rowptr, colidx, vals, precond == AMP_PRECOND_JACOBI, dinv64,
                                                 dinv32, flags);
-  if (nnz > 0) {
-    const int cgrid = (int)std::min<int64_t>((nnz + 255) / 256, (int64_t)h->num_sms * 16);
-    k_to_fp32<<<cgrid, 256, 0, h->stream>>>(nnz, vals, vals32);
-  }
   std::vector<int32_t> rp((size_t)n + 1);
   int hflags = 0;
   CU_TRY(cudaMemcpyAsync(&hflags, flags, sizeof(int), cudaMemcpyDeviceToHost, h->stream), { amp_pcg_destroy(h); return nullptr; });
@@ -232,6 +272,14 @@ extern "C" amp_pcg_t* amp_pcg_create(int64_t n, int64_t nnz, const int32_t* rowp
     for (int64_t r = 0; r < n; ++r) {
       const int len = rp[(size_t)r + 1] - rp[(size_t)r];
       if (len > long_min) long_rows.push_back((int32_t)r); else nnz_sell += len;
+    }
+    c.long_min = long_min;
+    if (!long_rows.empty()) {  // long rows are summed from the CSR arrays: they need the FP32-rounded CSR values too
+      float* vals32;
+      ALLOC(vals32, float, (size_t)nnz + 8);
+      const int cgrid = (int)std::min<int64_t>((nnz + 255) / 256, (int64_t)h->num_sms * 16);
+      k_to_fp32<<<cgrid, 256, 0, h->stream>>>(nnz, vals, vals32);
+      c.vals32 = vals32;
     }
     std::vector<int32_t> wptr((size_t)nsl + 1, 0), perm;
     auto build_widths = [&]() -> int64_t {
@@ -275,7 +323,7 @@ extern "C" amp_pcg_t* amp_pcg_create(int64_t n, int64_t nnz, const int32_t* rowp
       CU_TRY(cudaMemcpyAsync(perm_d, perm.data(), sizeof(int32_t) * perm.size(), cudaMemcpyHostToDevice, h->stream),
              { amp_pcg_destroy(h); return nullptr; });
     const int pgrid = (int)((nsl * 32 + 255) / 256);
-    const int allow_aligned = getenv("AMP_SPMV_NO_ALIGN") ? 0 : 1;  // tuning aid
+    const int allow_aligned = (o.index_format == AMP_INDEX_AUTO) ? 1 : 0;
     k_sell_scan<<<pgrid, 256, 0, h->stream>>>((int)n, (int)nsl, long_min, allow_aligned, rowptr, colidx, perm_d, width_d);
     std::vector<int32_t> width((size_t)nsl);
     CU_TRY(cudaMemcpyAsync(width.data(), width_d, sizeof(int32_t) * (size_t)nsl, cudaMemcpyDeviceToHost, h->stream),
@@ -316,7 +364,7 @@ extern "C" amp_pcg_t* amp_pcg_create(int64_t n, int64_t nnz, const int32_t* rowp
     CU_TRY(cudaMemcpyAsync(&wide, flag16_d, sizeof(int), cudaMemcpyDeviceToHost, h->stream), { amp_pcg_destroy(h); return nullptr; });
     CU_TRY(cudaStreamSynchronize(h->stream), { amp_pcg_destroy(h); return nullptr; });
     CU_TRY(cudaGetLastError(), { amp_pcg_destroy(h); return nullptr; });
-    if (getenv("AMP_SPMV_IDX32")) wide = 1;  // tuning aid: force 32-bit column indices
+    if (o.index_format == AMP_INDEX_FORCE32) wide = 1;
     auto release = [&](void* ptr) {
       cudaFree(ptr);
       h->owned.erase(std::find(h->owned.begin(), h->owned.end(), ptr));
@@ -342,7 +390,7 @@ extern "C" amp_pcg_t* amp_pcg_create(int64_t n, int64_t nnz, const int32_t* rowp
     // SpMV grid: a warp takes a group of up to kSpmvGroupMax slices per pass; blocks make a whole number of
     // (nearly) equal passes, at most `mult` blocks per SM (AMP_SPMV_GRID_MULT: tuning aid)
     int mult = perm.empty() ? 4 : 55;  // sorted (irregular) matrices: small blocks even out the slice widths
-    if (const char* e = getenv("AMP_SPMV_GRID_MULT")) mult = std::max(1, atoi(e));
+    if (o.spmv_grid_mult > 0) mult = o.spmv_grid_mult;
     const int64_t max_grid = std::min<int64_t>((int64_t)h->num_sms * mult, kMaxGrid);
     const int64_t nblk = (nsl + kSpmvWarps * kSpmvGroupMax - 1) / (kSpmvWarps * kSpmvGroupMax);
     const int64_t passes = std::max<int64_t>(1, (nblk + max_grid - 1) / max_grid);
@@ -433,20 +481,49 @@ static cudaError_t launch_loop_kernel(K kern, int grid, int threads, cudaStream_
   return cudaLaunchKernelEx(&cfg, kern, c);
 }
 
-// the four kernels of one iteration; pdl: the last three are launched as programmatic dependents
-static cudaError_t launch_iteration(amp_pcg* h, const Ctx& c, cudaStream_t s, bool pdl) {
-  cudaError_t e = launch_loop_kernel(k_z, h->grid_z, kVecThreads, s, c, false);
+// ---- optional event bracketing of every loop kernel (policy.profile_kernels, stream loop) ----
+static cudaError_t prof_mark(amp_pcg* h, cudaStream_t s, int kernel, int iter) {
+  if (h->prof_used == h->prof_events.size()) {
+    cudaEvent_t e;
+    const cudaError_t r = cudaEventCreate(&e);
+    if (r != cudaSuccess) return r;
+    h->prof_events.push_back(e);
+  }
+  h->prof_kernel.push_back((int8_t)kernel);
+  h->prof_iter.push_back(iter);
+  return cudaEventRecord(h->prof_events[h->prof_used++], s);
+}
+
+// the four kernels of one iteration; pdl: the last three are launched as programmatic dependents.
+// prof_iter >= 0: an event is recorded before every kernel and after the last one (and pdl is off).
+static cudaError_t launch_iteration(amp_pcg* h, const Ctx& c, cudaStream_t s, bool pdl, int prof_iter = -1) {
+  const bool prof = prof_iter >= 0;
+  if (prof) pdl = false;
+  cudaError_t e = cudaSuccess;
+  if (prof) e = prof_mark(h, s, AMP_K_Z, prof_iter);
+  if (e == cudaSuccess) e = launch_loop_kernel(k_z, h->grid_z, kVecThreads, s, c, false);
+  if (prof && e == cudaSuccess) e = prof_mark(h, s, AMP_K_P, prof_iter);
   if (e == cudaSuccess) e = launch_loop_kernel(k_p, h->grid_p, kVecThreads, s, c, pdl);
+  if (prof && e == cudaSuccess) e = prof_mark(h, s, AMP_K_SPMV, prof_iter);
   if (e == cudaSuccess) e = launch_loop_kernel(k_spmv, h->spmv_grid, kSpmvThreads, s, c, pdl);
+  if (prof && e == cudaSuccess) e = prof_mark(h, s, AMP_K_XR, prof_iter);
   if (e == cudaSuccess) e = launch_loop_kernel(k_xr, h->grid_xr, kVecThreads, s, c, pdl);
+  if (prof && e == cudaSuccess) e = prof_mark(h, s, -1, prof_iter);
   return e;
 }
 
 // lagged variant: three kernels per iteration (z_0 comes from one k_z before the loop)
-static cudaError_t launch_iteration_lagged(amp_pcg* h, const Ctx& c, cudaStream_t s, bool pdl) {
-  cudaError_t e = launch_loop_kernel(k_p, h->grid_p, kVecThreads, s, c, false);
+static cudaError_t launch_iteration_lagged(amp_pcg* h, const Ctx& c, cudaStream_t s, bool pdl, int prof_iter = -1) {
+  const bool prof = prof_iter >= 0;
+  if (prof) pdl = false;
+  cudaError_t e = cudaSuccess;
+  if (prof) e = prof_mark(h, s, AMP_K_P, prof_iter);
+  if (e == cudaSuccess) e = launch_loop_kernel(k_p, h->grid_p, kVecThreads, s, c, false);
+  if (prof && e == cudaSuccess) e = prof_mark(h, s, AMP_K_SPMV, prof_iter);
   if (e == cudaSuccess) e = launch_loop_kernel(k_spmv, h->spmv_grid, kSpmvThreads, s, c, pdl);
+  if (prof && e == cudaSuccess) e = prof_mark(h, s, AMP_K_XRZ, prof_iter);
   if (e == cudaSuccess) e = launch_loop_kernel(k_xrz, h->grid_xrz, kVecThreads, s, c, pdl);
+  if (prof && e == cudaSuccess) e = prof_mark(h, s, -1, prof_iter);
   return e;
 }
 
@@ -487,7 +564,6 @@ static int build_graph(amp_pcg* h, bool lagged) {
   cudaGraph_t& graph = lagged ? h->graph_lag : h->graph;
   cudaGraphExec_t& graph_exec = lagged ? h->graph_lag_exec : h->graph_exec;
   if (graph_exec) return AMP_OK;
-  h->pdl = getenv("AMP_NO_PDL") ? 0 : 1;  // tuning aid
   int rc = build_graph_once(h, h->pdl != 0, lagged);
   if (rc != AMP_OK && h->pdl) {  // programmatic edges not accepted inside the conditional body: plain edges
     if (graph_exec) { cudaGraphExecDestroy(graph_exec); graph_exec = nullptr; }
@@ -512,7 +588,8 @@ static int solve_impl(amp_pcg* h, const double* b, double* x, double tol, int32_
   if (!(tol > 0.0) || maxit < 1 || maxit > (1 << 24) || !aligned16(b) || !aligned16(x) || pol.u0 < 0 || pol.u0 > 2 ||
       pol.eta_rule < 0 || pol.eta_rule > 2 || pol.scale_mode < 0 || pol.scale_mode > 4 || pol.d < 1 || pol.d > kMaxWindow ||
       pol.ell < 1 || pol.ell > kMaxWindow || pol.loop_mode < 0 || pol.loop_mode > 3 || !(pol.tau_zs >= 0.0) ||
-      !(pol.tau_zh >= 0.0) || !(pol.eps32 > 0.0) || !(pol.eta_safety > 0.0) || !(pol.stop_safety > 0.0)) {
+      !(pol.tau_zh >= 0.0) || !(pol.eps32 > 0.0) || !(pol.eta_safety > 0.0) || !(pol.stop_safety > 0.0) ||
+      (pol.profile_kernels != 0 && pol.loop_mode != AMP_LOOP_STREAM)) {
     set_error("amp_pcg_solve: invalid tol/maxit/policy or misaligned b/x");
     return AMP_ERR_INVALID;
   }
@@ -531,7 +608,7 @@ static int solve_impl(amp_pcg* h, const double* b, double* x, double tol, int32_
   // latency-bound; from c2 up the graph loop wins because each of its kernels has its own register budget
   const bool lagged = pol.amp && pol.scale_mode == AMP_SCALE_LAGGED;
   if (mode == AMP_LOOP_AUTO) mode = (h->persist_ok && h->n <= kPersistAutoMaxRows) ? AMP_LOOP_PERSISTENT : AMP_LOOP_GRAPH;
-  if (mode == AMP_LOOP_PERSISTENT && !(h->persist_ok && persistent_fits(h->ctx))) {
+  if (mode == AMP_LOOP_PERSISTENT && !h->persist_ok) {
     set_error("amp_pcg_solve: persistent loop not available for this problem/device");
     return AMP_ERR_INVALID;
   }
@@ -547,6 +624,11 @@ static int solve_impl(amp_pcg* h, const double* b, double* x, double tol, int32_
   hs->status = AMP_MAXIT; hs->it_ur32 = hs->it_uz32 = hs->it_uz16 = -1;
   hs->relres_true = -1.0;
   h->launches = 0;
+  const bool profile = pol.profile_kernels != 0;
+  h->prof_used = 0;
+  h->prof_kernel.clear();
+  h->prof_iter.clear();
+  h->prof_result.clear();
 
   CU_TRY(cudaEventRecord(h->ev0, st), return AMP_ERR_CUDA);
   CU_TRY(cudaMemcpyAsync(h->ctx.st, hs, sizeof(DevState), cudaMemcpyHostToDevice, st), return AMP_ERR_CUDA);
@@ -570,8 +652,15 @@ static int solve_impl(amp_pcg* h, const double* b, double* x, double tol, int32_
     while (done_iters < maxit) {
       const int nb = std::min(batch, maxit - done_iters);
       for (int i = 0; i < nb; ++i) {
-        if (lagged) launch_iteration_lagged(h, h->ctx, st, getenv("AMP_NO_PDL") == nullptr);
-        else launch_iteration(h, h->ctx, st, getenv("AMP_NO_PDL") == nullptr);
+        const int pit = profile ? done_iters + i : -1;
+        const cudaError_t el = lagged ? launch_iteration_lagged(h, h->ctx, st, h->pdl != 0, pit)
+                                      : launch_iteration(h, h->ctx, st, h->pdl != 0, pit);
+        if (el != cudaSuccess) {
+          set_error("amp_pcg_solve: loop kernel launch failed: %s", cudaGetErrorString(el));
+          cudaGetLastError();
+          cudaStreamSynchronize(st);
+          return AMP_ERR_CUDA;
+        }
       }
       done_iters += nb;
       CU_TRY(cudaMemcpyAsync(h->h_flag, &h->ctx.st->done, sizeof(int), cudaMemcpyDeviceToHost, st), return AMP_ERR_CUDA);
@@ -591,6 +680,43 @@ static int solve_impl(amp_pcg* h, const double* b, double* x, double tol, int32_
 
   const int iters = hs->k;
   h->last_iters = iters;
+  auto phase_of = [&](int k, int& uz, int& ur) {  // precisions in use at iteration k (from the switch iterations)
+    ur = (hs->it_ur32 >= 0 && k >= hs->it_ur32) ? AMP_FP32 : AMP_FP64;
+    uz = hs->amp ? hs->u0 : AMP_FP64;
+    if (hs->it_uz32 >= 0 && k >= hs->it_uz32) uz = std::max(uz, (int)AMP_FP32);
+    if (hs->it_uz16 >= 0 && k >= hs->it_uz16) uz = AMP_FP16;
+  };
+  if (profile) {  // event-to-event device time of every executed loop kernel, summed per (kernel, u_z, u_r)
+    amp_kernel_time_t acc[AMP_K_COUNT][3][2];
+    std::memset(acc, 0, sizeof(acc));
+    for (size_t i = 0; i + 1 < h->prof_used; ++i) {
+      const int kern = h->prof_kernel[i], k = h->prof_iter[i];
+      if (kern < 0 || k >= iters) continue;
+      float dt = 0.f;
+      if (cudaEventElapsedTime(&dt, h->prof_events[i], h->prof_events[i + 1]) != cudaSuccess) { cudaGetLastError(); continue; }
+      int uz, ur;
+      phase_of(k, uz, ur);
+      acc[kern][uz][ur].launches += 1;
+      acc[kern][uz][ur].total_ms += dt;
+    }
+    const double n_ = (double)h->n;
+    for (int kern = 0; kern < AMP_K_COUNT; ++kern)
+      for (int uz = 0; uz < 3; ++uz)
+        for (int ur = 0; ur < 2; ++ur) {
+          amp_kernel_time_t& a = acc[kern][uz][ur];
+          if (a.launches == 0) continue;
+          const double sr = (ur == AMP_FP64) ? 8.0 : 4.0, sz = vec_size(uz), sd = (uz == AMP_FP64) ? 8.0 : 4.0;
+          a.kernel = kern; a.uz = uz; a.ur = ur;
+          switch (kern) {
+            case AMP_K_Z: a.bytes_per_launch = n_ * (sr + sd + sz); break;
+            case AMP_K_P: a.bytes_per_launch = n_ * 3.0 * sz; break;
+            case AMP_K_SPMV: a.bytes_per_launch = amp_pcg_spmv_bytes(h, ur, uz); break;
+            case AMP_K_XR: a.bytes_per_launch = n_ * (16.0 + sz + 3.0 * sr); break;
+            default: a.bytes_per_launch = n_ * (16.0 + sz + 3.0 * sr + sd + sz); break;  // AMP_K_XRZ
+          }
+          h->prof_result.push_back(a);
+        }
+  }
   h->launches += (mode == AMP_LOOP_PERSISTENT) ? 1 : (int64_t)(lagged ? 3 : 4) * iters;
   if (stats) {
     std::memset(stats, 0, sizeof(*stats));
@@ -603,10 +729,8 @@ static int solve_impl(amp_pcg* h, const double* b, double* x, double tol, int32_
     stats->solve_ms = ms;
     double bytes = 0.0;
     for (int k = 0; k < iters; ++k) {
-      const int ur = (hs->it_ur32 >= 0 && k >= hs->it_ur32) ? AMP_FP32 : AMP_FP64;
-      int uz = hs->amp ? hs->u0 : AMP_FP64;
-      if (hs->it_uz32 >= 0 && k >= hs->it_uz32) uz = std::max(uz, (int)AMP_FP32);
-      if (hs->it_uz16 >= 0 && k >= hs->it_uz16) uz = AMP_FP16;
+      int uz, ur;
+      phase_of(k, uz, ur);
       bytes += amp_pcg_iteration_bytes(h, uz, ur);
       if (lagged) bytes -= (double)h->n * ((ur == AMP_FP64) ? 8.0 : 4.0);  // r is not read a second time
     }
@@ -670,4 +794,106 @@ extern "C" int32_t amp_pcg_eta_posteriori(amp_pcg_t* h, double C, double eps32, 
     out_host[k] = eps64 * prefix + eps32 * suffix[(size_t)k];
   }
   return nout;
+}
+
+extern "C" int32_t amp_pcg_kernel_times(amp_pcg_t* h, amp_kernel_time_t* out_host, int32_t cap) {
+  if (!h || !out_host || cap < 0) return AMP_ERR_INVALID;
+  const int32_t m = std::min<int32_t>(cap, (int32_t)h->prof_result.size());
+  for (int32_t i = 0; i < m; ++i) out_host[i] = h->prof_result[(size_t)i];
+  return m;
+}
+
+// ------------------------------------------------------------------ diagnostic entry points --
+static bool debug_vec(amp_pcg* h, int which, int prec, void** ptr, size_t* elem) {
+  const Ctx& c = h->ctx;
+  *ptr = nullptr;
+  *elem = prec == AMP_FP64 ? 8 : (prec == AMP_FP32 ? 4 : 2);
+  switch (which) {
+    case AMP_VEC_R: *ptr = prec == AMP_FP64 ? (void*)c.r64 : prec == AMP_FP32 ? (void*)c.r32 : nullptr; break;
+    case AMP_VEC_Q: *ptr = prec == AMP_FP64 ? (void*)c.q64 : prec == AMP_FP32 ? (void*)c.q32 : nullptr; break;
+    case AMP_VEC_Z: *ptr = prec == AMP_FP64 ? (void*)c.z64 : prec == AMP_FP32 ? (void*)c.z32 : prec == AMP_FP16 ? (void*)c.z16 : nullptr; break;
+    case AMP_VEC_P: *ptr = prec == AMP_FP64 ? (void*)c.p64 : prec == AMP_FP32 ? (void*)c.p32 : prec == AMP_FP16 ? (void*)c.p16 : nullptr; break;
+    case AMP_VEC_DINV: *ptr = prec == AMP_FP64 ? (void*)c.dinv64 : prec == AMP_FP32 ? (void*)c.dinv32 : nullptr; break;
+    default: break;
+  }
+  return *ptr != nullptr;
+}
+
+extern "C" int amp_pcg_debug_set_vector(amp_pcg_t* h, int which, int prec, const void* src) {
+  g_last_error.clear();
+  void* dst; size_t es;
+  if (!h || !src || which == AMP_VEC_DINV || !debug_vec(h, which, prec, &dst, &es)) {
+    set_error("amp_pcg_debug_set_vector: invalid handle / vector / precision");
+    return AMP_ERR_INVALID;
+  }
+  CU_TRY(cudaSetDevice(h->device), return AMP_ERR_CUDA);
+  CU_TRY(cudaMemsetAsync(dst, 0, es * (size_t)h->npad, h->stream), return AMP_ERR_CUDA);
+  CU_TRY(cudaMemcpyAsync(dst, src, es * (size_t)h->n, cudaMemcpyDeviceToDevice, h->stream), return AMP_ERR_CUDA);
+  return AMP_OK;
+}
+
+extern "C" int amp_pcg_debug_get_vector(amp_pcg_t* h, int which, int prec, void* dst) {
+  g_last_error.clear();
+  void* src; size_t es;
+  if (!h || !dst || !debug_vec(h, which, prec, &src, &es)) {
+    set_error("amp_pcg_debug_get_vector: invalid handle / vector / precision");
+    return AMP_ERR_INVALID;
+  }
+  CU_TRY(cudaSetDevice(h->device), return AMP_ERR_CUDA);
+  CU_TRY(cudaMemcpyAsync(dst, src, es * (size_t)h->n, cudaMemcpyDeviceToDevice, h->stream), return AMP_ERR_CUDA);
+  return AMP_OK;
+}
+
+extern "C" int amp_pcg_debug_step(amp_pcg_t* h, amp_debug_step_t* io, double* x) {
+  g_last_error.clear();
+  auto prec_ok = [](int p, int lo) { return p >= 0 && p <= lo; };
+  if (!h || !io || io->step < AMP_STEP_Z || io->step > AMP_STEP_XRZ || !prec_ok(io->rs, 1) || !prec_ok(io->ur, 1) ||
+      !prec_ok(io->uz, 2) || !prec_ok(io->ps, 2) || !prec_ok(io->ur_n, 1) || !prec_ok(io->uz_n, 2) || io->rs > io->ur ||
+      io->ps > io->uz || io->ur > io->ur_n || io->uz > io->uz_n ||
+      ((io->step == AMP_STEP_XR || io->step == AMP_STEP_XRZ) && (!x || !aligned16(x)))) {
+    set_error("amp_pcg_debug_step: invalid step / precision combination (precisions only step down) or x missing");
+    return AMP_ERR_INVALID;
+  }
+  CU_TRY(cudaSetDevice(h->device), return AMP_ERR_CUDA);
+  cudaStream_t st = h->stream;
+  if (h->hist_cap < 64) {
+    if (h->hist) cudaFree(h->hist);
+    h->hist = nullptr; h->hist_cap = 0;
+    CU_TRY(cudaMalloc(&h->hist, sizeof(double) * 64), return AMP_ERR_NOMEM);
+    h->hist_cap = 64;
+  }
+  CU_TRY(cudaMemsetAsync(h->hist, 0, sizeof(double) * 64, st), return AMP_ERR_CUDA);
+  DevState* hs = h->h_state;
+  std::memset(hs, 0, sizeof(DevState));
+  hs->x = x; hs->hist = h->hist;
+  hs->tol = 1.0; hs->eps32 = std::ldexp(1.0, -24); hs->C = 1.0; hs->eta_safety = 1.0; hs->stop_safety = 1.0;
+  hs->amp = 0; hs->eta_rule = AMP_ETA_NEVER; hs->d = 10; hs->ell = 5; hs->no_stop = 1; hs->maxit = 1 << 20;
+  hs->bnorm = 1.0; hs->rho = 1.0; hs->rho_prev = 1.0;
+  hs->status = AMP_MAXIT; hs->it_ur32 = hs->it_uz32 = hs->it_uz16 = -1;
+  hs->k = io->first ? 0 : 1;
+  hs->r_store = io->rs; hs->ur = io->ur; hs->uz = io->uz; hs->p_store = io->ps;
+  hs->ur_n = io->ur_n; hs->uz_n = io->uz_n;
+  hs->omega = io->omega; hs->beta = io->beta; hs->alpha = io->alpha; hs->omega_n = io->omega_n;
+  CU_TRY(cudaMemcpyAsync(h->ctx.st, hs, sizeof(DevState), cudaMemcpyHostToDevice, st), return AMP_ERR_CUDA);
+  cudaError_t e = cudaSuccess;
+  switch (io->step) {  // the very kernels, grids and block sizes the stream / graph loop launches
+    case AMP_STEP_Z: e = launch_loop_kernel(k_z, h->grid_z, kVecThreads, st, h->ctx, false); break;
+    case AMP_STEP_P: e = launch_loop_kernel(k_p, h->grid_p, kVecThreads, st, h->ctx, false); break;
+    case AMP_STEP_SPMV: e = launch_loop_kernel(k_spmv, h->spmv_grid, kSpmvThreads, st, h->ctx, false); break;
+    case AMP_STEP_XR: e = launch_loop_kernel(k_xr, h->grid_xr, kVecThreads, st, h->ctx, false); break;
+    default: e = launch_loop_kernel(k_xrz, h->grid_xrz, kVecThreads, st, h->ctx, false); break;
+  }
+  if (e != cudaSuccess) { set_error("amp_pcg_debug_step: launch failed: %s", cudaGetErrorString(e)); cudaGetLastError(); return AMP_ERR_CUDA; }
+  CU_TRY(cudaMemcpyAsync(hs, h->ctx.st, sizeof(DevState), cudaMemcpyDeviceToHost, st), return AMP_ERR_CUDA);
+  CU_TRY(cudaStreamSynchronize(st), return AMP_ERR_CUDA);
+  CU_TRY(cudaGetLastError(), return AMP_ERR_CUDA);
+  io->sum0 = io->sum1 = 0.0;
+  switch (io->step) {
+    case AMP_STEP_Z: io->sum0 = hs->rho; break;
+    case AMP_STEP_SPMV: io->sum0 = hs->gamma; break;
+    case AMP_STEP_XR: io->sum0 = hs->delta; break;
+    case AMP_STEP_XRZ: io->sum0 = hs->delta; io->sum1 = hs->rho; break;
+    default: break;
+  }
+  return AMP_OK;
 }

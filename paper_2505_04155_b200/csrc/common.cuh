@@ -77,6 +77,7 @@ struct Ctx {
   const int32_t* long_rows;   // [nlong] rows kept out of the slices (longer than the cap), summed from CSR
   int32_t nslices;
   int32_t nlong;
+  int32_t long_min;           // rows with more stored entries than this are "long": kept out of the slices
   cudaGraphConditionalHandle cond;  // WHILE-node handle (graph loop only)
   int32_t use_cond;
 };

@@ -244,12 +244,12 @@ __global__ void k_validate_dinv(int64_t n, int64_t nnz, const int32_t* rowptr, c
     if (i == 0 && a != 0) f |= 1;
     if (i == n - 1 && b != nnz) f |= 1;
     if (a < 0 || b < a || b > nnz) { f |= 1; continue; }
-    double d = 1.0;
+    double d = jacobi ? 0.0 : 1.0;
     bool found = !jacobi;
     for (int64_t e = a; e < b; ++e) {
       const int j = colidx[e];
       if (j < 0 || j >= n) { f |= 2; continue; }
-      if (jacobi && j == i) { d = vals[e]; found = true; }
+      if (jacobi && j == i) { d += vals[e]; found = true; }  // duplicates add up, as in the mat-vec
     }
     if (!found) { f |= 4; d = 1.0; }
     else if (!(d > 0.0) || isinf(d)) { f |= 8; d = 1.0; }

@@ -159,9 +159,11 @@ __global__ void __launch_bounds__(kPersistThreads, kPersistMinBlocks) k_persiste
     __syncthreads();
     int* dst = reinterpret_cast<int*>(c.st);
     const int* src = reinterpret_cast<const int*>(&ls);
-    const int skip0 = (int)(offsetof(DevState, bar_count) / sizeof(int));
+    // the FP16 counters of the counting build are accumulated in global memory only (other blocks may still be adding)
+    const int skip0 = (int)(offsetof(DevState, fp16_subnormal) / sizeof(int));
+    const int skip1 = (int)((offsetof(DevState, bar_pad) + sizeof(unsigned int)) / sizeof(int));
     for (int i = threadIdx.x; i < (int)(sizeof(DevState) / sizeof(int)); i += kPersistThreads)
-      if (i != skip0 && i != skip0 + 1) dst[i] = src[i];
+      if (i < skip0 || i >= skip1) dst[i] = src[i];
   }
 }
 
@@ -180,8 +182,6 @@ inline void persistent_configure(int num_sms, int* grid, int* ok) {
   if (*grid > kMaxGrid) *grid = (kMaxGrid / num_sms) * num_sms;
   *ok = 1;
 }
-
-inline bool persistent_fits(const Ctx&) { return true; }
 
 inline int persistent_launch(const Ctx& c, int grid, cudaStream_t st) {
   Ctx cc = c;

@@ -518,7 +518,18 @@ __device__ __forceinline__ void phase_xrz(const Ctx& c, const double alpha, cons
         Chunk<TZ, E> zo;
         chunk_pack(zo, zv);
         chunk_store(zo, z, i);
+#ifdef AMP_COUNT_FP16
+        double zx[E];
+#pragma unroll
+        for (int e = 0; e < E; ++e) zx[e] = zv[e];
+#endif
         chunk_unpack(zo, zv);
+#ifdef AMP_COUNT_FP16
+        if (UZN == P16) {
+#pragma unroll
+          for (int e = 0; e < E; ++e) count_fp16(c.st, zx[e], zv[e]);
+        }
+#endif
 #pragma unroll
         for (int e = 0; e < E; ++e) { srr = fma(rv[e], rv[e], srr); srz = fma(rv[e], zv[e], srz); }
       }

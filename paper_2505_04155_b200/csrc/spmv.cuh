@@ -430,7 +430,11 @@ __device__ __forceinline__ double phase_spmv_fmt(const Ctx& c, const PT* p, type
     }
 #pragma unroll
     for (int g = 0; g < G; ++g) {
-      if (rows[g] >= 0) {
+      bool mine = rows[g] >= 0;
+      // a long row has length 0 in its slice; the block that sums it from the CSR arrays (below) is the ONLY writer of
+      // its q (nothing orders a store from here against that one)
+      if (c.nlong > 0 && mine) mine = (c.rowptr[rows[g] + 1] - c.rowptr[rows[g]]) <= c.long_min;
+      if (mine) {
         q[rows[g]] = acc[g];
         gsum = fma(pi[g], (double)acc[g], gsum);
       }

@@ -45,17 +45,39 @@ def test_library_exports_every_declared_symbol(A):
 
 def test_struct_layout_matches_c(A, tmp_path):
     # compile a tiny C program against the header and compare sizeof/offsetof with ctypes
+    probes = [("amp_policy_t", A.Policy, ["C", "stop_safety", "profile_kernels"]),
+              ("amp_stats_t", A.Stats, ["bnorm", "fp16_inf"]),
+              ("amp_create_opts_t", A.CreateOpts, ["pdl", "stream"]),
+              ("amp_kernel_time_t", A.KernelTime, ["launches", "bytes_per_launch"]),
+              ("amp_debug_step_t", A.DebugStep, ["first", "omega", "sum1"])]
+    body, want = [], []
+    for cname, ct, fields in probes:
+        body.append(f'printf("%zu\\n", sizeof({cname}));')
+        want.append(C.sizeof(ct))
+        for f in fields:
+            body.append(f'printf("%zu\\n", offsetof({cname}, {f}));')
+            want.append(getattr(ct, f).offset)
     src = tmp_path / "layout.c"
-    src.write_text('#include <stdio.h>\n#include <stddef.h>\n#include "amp_pcg.h"\n'
-                   'int main(void){printf("%zu %zu %zu %zu %zu %zu\\n", sizeof(amp_policy_t), offsetof(amp_policy_t, C),'
-                   ' offsetof(amp_policy_t, stop_safety), sizeof(amp_stats_t), offsetof(amp_stats_t, bnorm),'
-                   ' offsetof(amp_stats_t, fp16_inf)); return 0;}\n')
+    src.write_text('#include <stdio.h>\n#include <stddef.h>\n#include "amp_pcg.h"\nint main(void){' + "".join(body) + 'return 0;}\n')
     exe = tmp_path / "layout"
     subprocess.check_call(["gcc", "-I", os.path.join(ROOT, "include"), str(src), "-o", str(exe)])
     got = [int(t) for t in subprocess.check_output([str(exe)], text=True).split()]
-    want = [C.sizeof(A.Policy), A.Policy.C.offset, A.Policy.stop_safety.offset, C.sizeof(A.Stats),
-            A.Stats.bnorm.offset, A.Stats.fp16_inf.offset]
     assert got == want
+
+
+def test_create_opts_defaults_and_validation(A):
+    o = A.CreateOpts.default()
+    assert o.struct_bytes == C.sizeof(A.CreateOpts) and o.precond == A.PRECOND_JACOBI
+    assert (o.index_format, o.spmv_kernel, o.spmv_grid_mult, o.pdl) == (A.INDEX_AUTO, A.SPMV_AUTO, 0, 1)
+    # a struct of another size (an older / newer header) is refused before anything touches the device
+    import numpy as np
+
+    L = A.load_library()
+    bad = A.CreateOpts.default()
+    bad.struct_bytes = 8
+    a = np.array([0, 1], dtype=np.int32)
+    h = L.amp_pcg_create_ex(1, 1, a.ctypes.data, a.ctypes.data, np.array([1.0]).ctypes.data, C.byref(bad))
+    assert not h and b"struct_bytes" in L.amp_pcg_last_error()
 
 
 def test_policy_defaults_are_the_papers(A):
