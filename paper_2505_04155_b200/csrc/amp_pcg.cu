@@ -14,6 +14,7 @@
 
 #include "kernels.cuh"
 #include "persistent.cuh"
+#include "spmv_pipe.cuh"
 
 using namespace amp;
 
@@ -68,6 +69,10 @@ struct amp_pcg {
   double idx_bytes_total = 0.0;  // bytes of index data one SpMV reads (slice table, bases, per-entry indices, row order)
   double long_bytes_idx = 0.0, long_entries = 0.0;  // long rows, read from the CSR arrays (4 B index per entry)
   int64_t sell_entries = 0;   // stored entries of the SELL-32 repack (padding included)
+  int use_pipe = 0;           // the loop's SpMV is the bulk-copy pipelined kernel (spmv_pipe.cuh)
+  int pipe_grid = 0;
+  int64_t pipe_chunks = 0;
+  int64_t guard = 0;          // zero guard band (elements) on both sides of the p vectors
   // per-kernel event profile of the last solve (policy.profile_kernels, stream loop)
   std::vector<cudaEvent_t> prof_events;  // pool, grown on demand
   size_t prof_used = 0;
@@ -228,7 +233,6 @@ extern "C" amp_pcg_t* amp_pcg_create_ex(int64_t n, int64_t nnz, const int32_t* r
   ALLOC(c.r64, double, np); ALLOC(c.r32, float, np);
   ALLOC(c.q64, double, np); ALLOC(c.q32, float, np);
   ALLOC(c.z64, double, np); ALLOC(c.z32, float, np); ALLOC(c.z16, __half, np);
-  ALLOC(c.p64, double, np); ALLOC(c.p32, float, np); ALLOC(c.p16, __half, np);
   ALLOC(c.partials, double, (size_t)4 * kMaxGrid);
   ALLOC(c.st, DevState, 1);
   ALLOC(flags, int, 1);
@@ -312,7 +316,7 @@ extern "C" amp_pcg_t* amp_pcg_create_ex(int64_t n, int64_t nnz, const int32_t* r
     }
     // pass 1 on the device: final width of every slice and whether it is stored diagonal-aligned
     int32_t *wptr_d, *cols_d, *perm_d = nullptr, *long_d, *base_d, *width_d;
-    ALLOC(wptr_d, int32_t, wptr.size());
+    ALLOC(wptr_d, int32_t, wptr.size() + 8);
     ALLOC(width_d, int32_t, (size_t)nsl + 1);
     ALLOC(long_d, int32_t, long_rows.size() + 1);
     if (!perm.empty()) ALLOC(perm_d, int32_t, perm.size());
@@ -360,8 +364,12 @@ extern "C" amp_pcg_t* amp_pcg_create_ex(int64_t n, int64_t nnz, const int32_t* r
            { amp_pcg_destroy(h); return nullptr; });
     k_sell_pack<<<pgrid, 256, 0, h->stream>>>((int)n, (int)nsl, long_min, rowptr, colidx, vals, wptr_d, perm_d, cols_d,
                                              cols16_d, base_d, v64_d, v32_d, flag16_d);
-    int wide = 0;
+    int wide = 0, maxbase = 0;
+    int* maxbase_d;
+    ALLOC(maxbase_d, int, 1);
+    if (wsum > 0) k_absmax_i32<<<(int)std::min<int64_t>((wsum + 255) / 256, 4096), 256, 0, h->stream>>>(wsum, base_d, maxbase_d);
     CU_TRY(cudaMemcpyAsync(&wide, flag16_d, sizeof(int), cudaMemcpyDeviceToHost, h->stream), { amp_pcg_destroy(h); return nullptr; });
+    CU_TRY(cudaMemcpyAsync(&maxbase, maxbase_d, sizeof(int), cudaMemcpyDeviceToHost, h->stream), { amp_pcg_destroy(h); return nullptr; });
     CU_TRY(cudaStreamSynchronize(h->stream), { amp_pcg_destroy(h); return nullptr; });
     CU_TRY(cudaGetLastError(), { amp_pcg_destroy(h); return nullptr; });
     if (o.index_format == AMP_INDEX_FORCE32) wide = 1;
@@ -386,6 +394,75 @@ extern "C" amp_pcg_t* amp_pcg_create_ex(int64_t n, int64_t nnz, const int32_t* r
     h->long_entries = (double)(nnz - nnz_sell);
     h->long_bytes_idx = 4.0 * h->long_entries + 12.0 * (double)long_rows.size();
     h->sell_entries = wsum * 32;
+
+    // ---- bulk-copy pipelined SpMV (spmv_pipe.cuh): eligibility, zero guard band of p, stage plan ----
+    {
+      bool eligible = o.spmv_kernel != AMP_SPMV_DIRECT && perm.empty() && long_rows.empty() && w_aligned == wsum;
+      int wmax = 0;
+      for (int64_t sl = 0; sl < nsl; ++sl) wmax = std::max(wmax, (int)(width[(size_t)sl] & 0x7fffffff));
+      const int64_t guard = (((int64_t)maxbase + 64 + 127) / 128) * 128;
+      if (wmax > kPipeChunkW || guard > kPipeMaxGuard) eligible = false;
+      // measured (B200, profiles/r02.md): the pipelined kernel wins for wide slices (c4, 27 entries per row: 181 vs 210 us
+      // in the FP32 phase) and loses for narrow ones (c2/c3, 7 per row: 43 vs 29 us), where the per-slice bookkeeping of
+      // a consumer warp outweighs its 7 entries; AUTO therefore takes it from an average slice width of 12
+      if (o.spmv_kernel == AMP_SPMV_AUTO && (double)wsum < 12.0 * (double)nsl) eligible = false;
+      if (eligible) {
+        cudaError_t ea = cudaFuncSetAttribute((const void*)k_spmv_pipe, cudaFuncAttributeMaxDynamicSharedMemorySize, kPipeSmemBytes);
+        if (ea != cudaSuccess) { cudaGetLastError(); eligible = false; }
+      }
+      if (!eligible && o.spmv_kernel == AMP_SPMV_PIPELINED) {
+        set_error("amp_pcg_create_ex: AMP_SPMV_PIPELINED needs a matrix whose SELL-32 slices are all diagonal-aligned "
+                  "(natural row order, no long rows, slice width <= %d)", kPipeChunkW);
+        amp_pcg_destroy(h);
+        return nullptr;
+      }
+      if (eligible) {
+        auto wof = [&](int64_t sl) { return (int)(width[(size_t)sl] & 0x7fffffff); };
+        const int cap = (int)std::min<int64_t>(kPipeChunkW, std::max<int64_t>(std::max(wmax, 1), wsum / ((int64_t)h->num_sms * 6)));
+        std::vector<int32_t> chunks;       // {first slice, first entry column} per stage
+        std::vector<int64_t> cost;         // per stage
+        for (int64_t sl = 0; sl < nsl;) {
+          chunks.push_back((int32_t)sl);
+          chunks.push_back(wptr[(size_t)sl] & 0x7fffffff);
+          int acc = 0, cnt = 0;
+          while (sl < nsl && cnt < kPipeChunkSlices && acc + wof(sl) <= cap) { acc += wof(sl); ++cnt; ++sl; }
+          cost.push_back((int64_t)acc + 2 * cnt);
+        }
+        const int64_t nch = (int64_t)cost.size();
+        chunks.push_back((int32_t)nsl);
+        chunks.push_back((int32_t)wsum);
+        const int nb = (int)std::max<int64_t>(1, std::min<int64_t>(h->num_sms, nch));
+        int64_t total = 0;
+        for (int64_t v : cost) total += v;
+        std::vector<int32_t> blk((size_t)nb + 1, 0);
+        {  // contiguous stage ranges of (nearly) equal cost
+          int64_t run = 0;
+          int b = 1;
+          for (int64_t ch = 0; ch < nch && b < nb; ++ch) {
+            run += cost[(size_t)ch];
+            while (b < nb && run * nb >= total * b) blk[(size_t)b++] = (int32_t)(ch + 1);
+          }
+          for (; b <= nb; ++b) blk[(size_t)b] = (int32_t)nch;
+        }
+        int32_t *chunks_d, *blk_d;
+        ALLOC(chunks_d, int32_t, chunks.size());
+        ALLOC(blk_d, int32_t, blk.size());
+        CU_TRY(cudaMemcpyAsync(chunks_d, chunks.data(), sizeof(int32_t) * chunks.size(), cudaMemcpyHostToDevice, h->stream),
+               { amp_pcg_destroy(h); return nullptr; });
+        CU_TRY(cudaMemcpyAsync(blk_d, blk.data(), sizeof(int32_t) * blk.size(), cudaMemcpyHostToDevice, h->stream),
+               { amp_pcg_destroy(h); return nullptr; });
+        CU_TRY(cudaStreamSynchronize(h->stream), { amp_pcg_destroy(h); return nullptr; });
+        c.pipe_chunks = chunks_d; c.pipe_blk_chunk = blk_d; c.use_pipe = 1;
+        h->use_pipe = 1; h->pipe_grid = nb; h->pipe_chunks = nch; h->guard = guard;
+        h->idx_bytes_total += 8.0 * (double)(nch + 1) + 4.0 * (double)(nb + 1);  // stage descriptors
+      }
+    }
+    {  // p in its three storage precisions, with the zero guard band on both sides (0 elements unless pipelined)
+      const size_t g = (size_t)h->guard;
+      double* b64; float* b32; __half* b16;
+      ALLOC(b64, double, np + 2 * g); ALLOC(b32, float, np + 2 * g); ALLOC(b16, __half, np + 2 * g);
+      c.p64 = b64 + g; c.p32 = b32 + g; c.p16 = b16 + g;
+    }
 
     // SpMV grid: a warp takes a group of up to kSpmvGroupMax slices per pass; blocks make a whole number of
     // (nearly) equal passes, at most `mult` blocks per SM (AMP_SPMV_GRID_MULT: tuning aid)
@@ -467,11 +544,11 @@ extern "C" int amp_spmv(amp_pcg_t* h, int mat_prec, int vec_prec, const void* p,
 
 // ------------------------------------------------------------------ graph loop --------------
 template <class K>
-static cudaError_t launch_loop_kernel(K kern, int grid, int threads, cudaStream_t s, const Ctx& c, bool pdl) {
+static cudaError_t launch_loop_kernel(K kern, int grid, int threads, cudaStream_t s, const Ctx& c, bool pdl, size_t smem = 0) {
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = dim3((unsigned)grid);
   cfg.blockDim = dim3((unsigned)threads);
-  cfg.dynamicSmemBytes = 0;
+  cfg.dynamicSmemBytes = smem;
   cfg.stream = s;
   cudaLaunchAttribute attr[1];
   attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
@@ -479,6 +556,13 @@ static cudaError_t launch_loop_kernel(K kern, int grid, int threads, cudaStream_
   cfg.attrs = attr;
   cfg.numAttrs = pdl ? 1 : 0;
   return cudaLaunchKernelEx(&cfg, kern, c);
+}
+
+// step a4 inside the loop: the bulk-copy pipelined kernel when the matrix is eligible, else the direct kernel
+static cudaError_t launch_spmv_loop(amp_pcg* h, cudaStream_t s, const Ctx& c, bool pdl) {
+  cudaError_t e = launch_loop_kernel(k_spmv, h->spmv_grid, kSpmvThreads, s, c, pdl);
+  if (e == cudaSuccess && h->use_pipe) e = launch_loop_kernel(k_spmv_pipe, h->pipe_grid, kPipeThreads, s, c, pdl, (size_t)kPipeSmemBytes);
+  return e;
 }
 
 // ---- optional event bracketing of every loop kernel (policy.profile_kernels, stream loop) ----
@@ -505,7 +589,7 @@ static cudaError_t launch_iteration(amp_pcg* h, const Ctx& c, cudaStream_t s, bo
   if (prof && e == cudaSuccess) e = prof_mark(h, s, AMP_K_P, prof_iter);
   if (e == cudaSuccess) e = launch_loop_kernel(k_p, h->grid_p, kVecThreads, s, c, pdl);
   if (prof && e == cudaSuccess) e = prof_mark(h, s, AMP_K_SPMV, prof_iter);
-  if (e == cudaSuccess) e = launch_loop_kernel(k_spmv, h->spmv_grid, kSpmvThreads, s, c, pdl);
+  if (e == cudaSuccess) e = launch_spmv_loop(h, s, c, pdl);
   if (prof && e == cudaSuccess) e = prof_mark(h, s, AMP_K_XR, prof_iter);
   if (e == cudaSuccess) e = launch_loop_kernel(k_xr, h->grid_xr, kVecThreads, s, c, pdl);
   if (prof && e == cudaSuccess) e = prof_mark(h, s, -1, prof_iter);
@@ -520,7 +604,7 @@ static cudaError_t launch_iteration_lagged(amp_pcg* h, const Ctx& c, cudaStream_
   if (prof) e = prof_mark(h, s, AMP_K_P, prof_iter);
   if (e == cudaSuccess) e = launch_loop_kernel(k_p, h->grid_p, kVecThreads, s, c, false);
   if (prof && e == cudaSuccess) e = prof_mark(h, s, AMP_K_SPMV, prof_iter);
-  if (e == cudaSuccess) e = launch_loop_kernel(k_spmv, h->spmv_grid, kSpmvThreads, s, c, pdl);
+  if (e == cudaSuccess) e = launch_spmv_loop(h, s, c, pdl);
   if (prof && e == cudaSuccess) e = prof_mark(h, s, AMP_K_XRZ, prof_iter);
   if (e == cudaSuccess) e = launch_loop_kernel(k_xrz, h->grid_xrz, kVecThreads, s, c, pdl);
   if (prof && e == cudaSuccess) e = prof_mark(h, s, -1, prof_iter);
@@ -717,7 +801,7 @@ static int solve_impl(amp_pcg* h, const double* b, double* x, double tol, int32_
           h->prof_result.push_back(a);
         }
   }
-  h->launches += (mode == AMP_LOOP_PERSISTENT) ? 1 : (int64_t)(lagged ? 3 : 4) * iters;
+  h->launches += (mode == AMP_LOOP_PERSISTENT) ? 1 : (int64_t)((lagged ? 3 : 4) + (h->use_pipe ? 1 : 0)) * iters;
   if (stats) {
     std::memset(stats, 0, sizeof(*stats));
     stats->status = hs->status; stats->iters = iters;
@@ -879,7 +963,7 @@ extern "C" int amp_pcg_debug_step(amp_pcg_t* h, amp_debug_step_t* io, double* x)
   switch (io->step) {  // the very kernels, grids and block sizes the stream / graph loop launches
     case AMP_STEP_Z: e = launch_loop_kernel(k_z, h->grid_z, kVecThreads, st, h->ctx, false); break;
     case AMP_STEP_P: e = launch_loop_kernel(k_p, h->grid_p, kVecThreads, st, h->ctx, false); break;
-    case AMP_STEP_SPMV: e = launch_loop_kernel(k_spmv, h->spmv_grid, kSpmvThreads, st, h->ctx, false); break;
+    case AMP_STEP_SPMV: e = launch_spmv_loop(h, st, h->ctx, false); break;
     case AMP_STEP_XR: e = launch_loop_kernel(k_xr, h->grid_xr, kVecThreads, st, h->ctx, false); break;
     default: e = launch_loop_kernel(k_xrz, h->grid_xrz, kVecThreads, st, h->ctx, false); break;
   }

@@ -78,9 +78,20 @@ struct Ctx {
   int32_t nslices;
   int32_t nlong;
   int32_t long_min;           // rows with more stored entries than this are "long": kept out of the slices
+  // bulk-copy pipelined SpMV (spmv_pipe.cuh), only when the matrix is eligible (use_pipe)
+  const int32_t* pipe_chunks;     // [nchunks+1] x {first slice, first entry column} of every stage
+  const int32_t* pipe_blk_chunk;  // [pipe_grid+1] stage range of every block
+  int32_t use_pipe;               // 1: iterations with u_r = FP32 run k_spmv_pipe, those with u_r = FP64 the direct k_spmv
   cudaGraphConditionalHandle cond;  // WHILE-node handle (graph loop only)
   int32_t use_cond;
 };
+
+// Programmatic dependent launch (sm_90+): every loop kernel lets its successor start launching at
+// once and itself waits for its predecessor (completion + visibility of its writes) before the first
+// access to anything the predecessor writes, so the launch latency of kernel N+1 overlaps the
+// reduction tail of kernel N.  Both instructions are no-ops in a launch without the attribute.
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 
 // ------------------------------------------------------------------ typed storage access ----
 template <int P> struct Store;

@@ -65,13 +65,6 @@ __device__ __forceinline__ double dispatch_xr(const Ctx& c, int ur, int uz, doub
 }
 
 // ------------------------------------------------------------------ loop kernels ------------
-// Programmatic dependent launch (sm_90+): every loop kernel lets its successor start launching at
-// once and itself waits for its predecessor (completion + visibility of its writes) before the first
-// access to anything the predecessor writes, so the launch latency of kernel N+1 overlaps the
-// reduction tail of kernel N.  Both instructions are no-ops in a launch without the attribute.
-__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
-__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
-
 __global__ void __launch_bounds__(kVecThreads, 3) k_z(const Ctx c) {
   __shared__ double red[32];
   DevState* s = c.st;
@@ -98,6 +91,7 @@ __global__ void __launch_bounds__(kSpmvThreads, kSpmvMinBlocks) k_spmv(const Ctx
   pdl_launch_dependents();
   pdl_wait();
   if (s->done) return;
+  if (c.use_pipe && s->ur == P32) return;  // this iteration's mat-vec is k_spmv_pipe's (next in the chain)
   const int bid = blockIdx.x, nb = gridDim.x;
   const double v = dispatch_spmv<false, kSpmvThreads>(c, s->ur, s->uz, bid, nb, red);
   grid_reduce<kSpmvThreads>(v, c.partials + 1 * kMaxGrid, &s->counter[1], bid, nb, red,
@@ -257,6 +251,17 @@ __global__ void k_validate_dinv(int64_t n, int64_t nnz, const int32_t* rowptr, c
     dinv32[i] = __double2float_rn(1.0 / d);
   }
   if (f) atomicOr(flags, f);
+}
+
+// max |a_i| of an int32 array (the largest diagonal offset of the aligned slices: size of p's guard band)
+__global__ void k_absmax_i32(int64_t n, const int32_t* __restrict__ a, int* __restrict__ out) {
+  const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+  int m = 0;
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) m = max(m, abs(a[i]));
+  m = max(m, __shfl_xor_sync(0xffffffffu, m, 16)); m = max(m, __shfl_xor_sync(0xffffffffu, m, 8));
+  m = max(m, __shfl_xor_sync(0xffffffffu, m, 4)); m = max(m, __shfl_xor_sync(0xffffffffu, m, 2));
+  m = max(m, __shfl_xor_sync(0xffffffffu, m, 1));
+  if ((threadIdx.x & 31) == 0 && m > 0) atomicMax(out, m);
 }
 
 __global__ void k_to_fp32(int64_t n, const double* __restrict__ a, float* __restrict__ o) {

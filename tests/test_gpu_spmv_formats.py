@@ -77,9 +77,18 @@ def _check_bitwise(rowptr, colidx, vals, n, expect_bytes_per_entry=None, **opts)
 
 @pytest.mark.parametrize("name,size", [("c1", 37), ("c2", 19), ("c3", 21), ("c4", 17)])
 @pytest.mark.parametrize("fmt", [A.INDEX_AUTO, A.INDEX_NO_ALIGN, A.INDEX_FORCE32])
-@pytest.mark.parametrize("kernel", [A.SPMV_DIRECT, A.SPMV_AUTO])
+@pytest.mark.parametrize("kernel", [A.SPMV_DIRECT, A.SPMV_PIPELINED])
 def test_stencils_in_every_format(name, size, fmt, kernel):
     s = make_config(name, size)
+    if kernel == A.SPMV_PIPELINED and fmt != A.INDEX_AUTO:
+        # the bulk-copy pipelined kernel exists for diagonal-aligned slices only: asking for it on another format is an error
+        with pytest.raises(A.AmpPcgError):
+            A.AmpPcg(*[torch.from_numpy(a).cuda() for a in (s.rowptr, s.colidx, s.vals)], A.PRECOND_NONE, index_format=fmt,
+                     spmv_kernel=kernel)
+        return
+    if kernel == A.SPMV_PIPELINED:
+        # every slice must be diagonal-aligned: take grid edges that are multiples of the slice height
+        s = make_config(name, {"c1": 96, "c2": 32, "c3": 32, "c4": 32}[name])
     # FP32 phase: 4 B value + index bytes per stored entry (padding included, so a little above the nominal)
     expect = {A.INDEX_AUTO: (4.0, 4.9), A.INDEX_NO_ALIGN: (6.0, 7.2), A.INDEX_FORCE32: (8.0, 9.3)}[fmt]
     _check_bitwise(s.rowptr, s.colidx, s.vals, s.n, expect, index_format=fmt, spmv_kernel=kernel)

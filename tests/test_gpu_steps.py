@@ -172,17 +172,31 @@ def test_step_xrz_bitwise(handle, ur, urn, uz, uzn):
             assert sum_close(io.sum1, r_ref, z_ref)
 
 
+@pytest.fixture(scope="module", params=[("c3", 32), ("c4", 32), ("c2", 64), ("c1", 320)], ids=lambda p: f"{p[0]}@{p[1]}")
+def spmv_handles(request):
+    """the same matrix behind both in-loop SpMV kernels: the direct one and the bulk-copy pipelined one"""
+    name, size = request.param
+    s = make_config(name, size)
+    devm = [torch.from_numpy(a).cuda() for a in (s.rowptr, s.colidx, s.vals)]
+    hs = [A.AmpPcg(*devm, A.PRECOND_JACOBI, spmv_kernel=k) for k in (A.SPMV_DIRECT, A.SPMV_PIPELINED)]
+    yield s, hs
+    for h in hs:
+        h.close()
+
+
 @pytest.mark.parametrize("ur,uz", XR_INST)
-def test_step_spmv_in_loop_kernel_bitwise(handle, ur, uz):
-    # the in-loop k_spmv (not the stand-alone amp_spmv kernel): q bit-identical, gamma to reduction accuracy
-    s, h, _ = handle
+def test_step_spmv_in_loop_kernel_bitwise(spmv_handles, ur, uz):
+    # the in-loop SpMV kernels (not the stand-alone amp_spmv kernel): q bit-identical, gamma to reduction accuracy
+    s, hs = spmv_handles
     rng = np.random.default_rng(500 + 3 * ur + uz)
     p = RND[uz](rng.standard_normal(s.n))
-    h.debug_set_vector(A.VEC_P, dev(p, uz))
-    io = h.debug_step(A.STEP_SPMV, rs=ur, ur=ur, uz=uz, ps=uz, ur_n=ur, uz_n=uz)
     q_ref = O.spmv_fp64(s.rowptr, s.colidx, s.vals, p) if ur == 0 else O.spmv_fp32(s.rowptr, s.colidx, s.vals, p)
-    assert_bits(host(h.debug_get_vector(A.VEC_Q, ur)), q_ref, "q")
-    assert sum_close(io.sum0, q_ref, p)
+    for h in hs:
+        h.debug_set_vector(A.VEC_P, dev(p, uz))
+        h.debug_set_vector(A.VEC_Q, dev(np.full(s.n, 7.0), ur))
+        io = h.debug_step(A.STEP_SPMV, rs=ur, ur=ur, uz=uz, ps=uz, ur_n=ur, uz_n=uz)
+        assert_bits(host(h.debug_get_vector(A.VEC_Q, ur)), q_ref, "q")
+        assert sum_close(io.sum0, q_ref, p)
 
 
 def test_debug_step_rejects_impossible_combinations(handle):
