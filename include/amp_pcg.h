@@ -228,7 +228,8 @@ double amp_pcg_bytes_per_row(double m, int uz, int ur);
 double amp_pcg_spmv_bytes(const amp_pcg_t *h, int mat_prec, int vec_prec);
 
 /* Compulsory bytes of one whole iteration in phase (u_z, u_r): amp_pcg_spmv_bytes(h, u_r, u_z) plus
- * the three vector kernels (z: r, 1/diag -> z; p: z, p -> p; x/r: x, p, q, r -> x, r).
+ * the three vector kernels (z: r, 1/diag -> z; p: z, p -> p; x/r: x, p, q, r -> x, r).  In phase (FP64, FP32) the p
+ * update also writes RN32(p) (4 B per row) and the mat-vec gathers that copy instead of converting every gathered entry.
  * amp_stats_t.algorithmic_bytes is the sum of this over the iterations of a solve. */
 double amp_pcg_iteration_bytes(const amp_pcg_t *h, int uz, int ur);
 

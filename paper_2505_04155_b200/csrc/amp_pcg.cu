@@ -125,11 +125,17 @@ extern "C" double amp_pcg_spmv_bytes(const amp_pcg_t* h, int mat_prec, int vec_p
          (double)h->n * (vec_size(vec_prec) + sA);  // p read once, q written once
 }
 
+// phase (u_z = FP64, u_r = FP32): the p update also writes RN32(p) (4 B per row) and the mat-vec gathers that copy
+static bool shadow_phase(int uz, int ur) { return uz == AMP_FP64 && ur == AMP_FP32; }
+static double loop_spmv_bytes(const amp_pcg_t* h, int uz, int ur) {
+  return amp_pcg_spmv_bytes(h, ur, shadow_phase(uz, ur) ? AMP_FP32 : uz);
+}
+
 extern "C" double amp_pcg_iteration_bytes(const amp_pcg_t* h, int uz, int ur) {
   if (!h) return 0.0;
   const double sr = (ur == AMP_FP64) ? 8.0 : 4.0, sz = vec_size(uz), sd = (uz == AMP_FP64) ? 8.0 : 4.0;
-  const double k_z = sr + sd + sz, k_p = 3.0 * sz, k_xr = 16.0 + sz + 3.0 * sr;
-  return amp_pcg_spmv_bytes(h, ur, uz) + (double)h->n * (k_z + k_p + k_xr);
+  const double k_z = sr + sd + sz, k_p = 3.0 * sz + (shadow_phase(uz, ur) ? 4.0 : 0.0), k_xr = 16.0 + sz + 3.0 * sr;
+  return loop_spmv_bytes(h, uz, ur) + (double)h->n * (k_z + k_p + k_xr);
 }
 
 extern "C" void amp_pcg_destroy(amp_pcg_t* h) {
@@ -793,8 +799,8 @@ static int solve_impl(amp_pcg* h, const double* b, double* x, double tol, int32_
           a.kernel = kern; a.uz = uz; a.ur = ur;
           switch (kern) {
             case AMP_K_Z: a.bytes_per_launch = n_ * (sr + sd + sz); break;
-            case AMP_K_P: a.bytes_per_launch = n_ * 3.0 * sz; break;
-            case AMP_K_SPMV: a.bytes_per_launch = amp_pcg_spmv_bytes(h, ur, uz); break;
+            case AMP_K_P: a.bytes_per_launch = n_ * (3.0 * sz + (shadow_phase(uz, ur) ? 4.0 : 0.0)); break;
+            case AMP_K_SPMV: a.bytes_per_launch = loop_spmv_bytes(h, uz, ur); break;
             case AMP_K_XR: a.bytes_per_launch = n_ * (16.0 + sz + 3.0 * sr); break;
             default: a.bytes_per_launch = n_ * (16.0 + sz + 3.0 * sr + sd + sz); break;  // AMP_K_XRZ
           }
@@ -913,6 +919,10 @@ extern "C" int amp_pcg_debug_set_vector(amp_pcg_t* h, int which, int prec, const
   CU_TRY(cudaSetDevice(h->device), return AMP_ERR_CUDA);
   CU_TRY(cudaMemsetAsync(dst, 0, es * (size_t)h->npad, h->stream), return AMP_ERR_CUDA);
   CU_TRY(cudaMemcpyAsync(dst, src, es * (size_t)h->n, cudaMemcpyDeviceToDevice, h->stream), return AMP_ERR_CUDA);
+  if (which == AMP_VEC_P && prec == AMP_FP64) {  // keep the FP32 copy RN32(p) the (FP64, FP32) phase gathers in step
+    const int cgrid = (int)std::min<int64_t>((h->n + 255) / 256, (int64_t)h->num_sms * 16);
+    k_to_fp32<<<cgrid, 256, 0, h->stream>>>(h->n, h->ctx.p64, h->ctx.p32);
+  }
   return AMP_OK;
 }
 

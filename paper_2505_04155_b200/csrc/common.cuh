@@ -221,7 +221,10 @@ __host__ __device__ constexpr int cmin(int a, int b) { return a < b ? a : b; }
 __host__ __device__ constexpr int cmax(int a, int b) { return a > b ? a : b; }
 // elements per chunk for a kernel whose arrays have element sizes in [smin, smax] bytes
 __host__ __device__ constexpr int chunk_elems(int smin, int smax) { return cmin(16 / smin, 32 / smax); }
-constexpr int kVecBytesInFlight = 192;  // target bytes of loads in flight per thread of a vector kernel
+#ifndef AMP_VEC_BIF
+#define AMP_VEC_BIF 192
+#endif
+constexpr int kVecBytesInFlight = AMP_VEC_BIF;  // target bytes of loads in flight per thread of a vector kernel
 
 // gather of one element of p as the SpMV working type.  COH = false: read-only path (p is not
 // written by the running kernel); COH = true: plain coherent load.

@@ -5,6 +5,19 @@
 #include "phases.cuh"
 #include "spmv.cuh"
 
+#ifndef AMP_KZ_BLOCKS
+#define AMP_KZ_BLOCKS 3
+#endif
+#ifndef AMP_KP_BLOCKS
+#define AMP_KP_BLOCKS 3
+#endif
+#ifndef AMP_KXR_BLOCKS
+#define AMP_KXR_BLOCKS 2
+#endif
+#ifndef AMP_VEC_BIF
+#define AMP_VEC_BIF 192
+#endif
+
 namespace amp {
 
 // ------------------------------------------------------------------ precision dispatch ------
@@ -28,28 +41,29 @@ __device__ __forceinline__ double dispatch_z(const Ctx& c, int rs, int ur, int u
 }
 
 template <int BIF = kVecBytesInFlight>
-__device__ __forceinline__ void dispatch_p(const Ctx& c, int ps, int uz, double beta, bool first, int bid, int nb) {
-  if (uz == P64) phase_p<P64, P64, BIF>(c, beta, first, bid, nb);
+__device__ __forceinline__ void dispatch_p(const Ctx& c, int ps, int uz, int ur, double beta, bool first, int bid, int nb) {
+  if (uz == P64) phase_p<P64, P64, BIF>(c, beta, first, ur == P32, bid, nb);
   else if (uz == P32) {
-    if (ps == P64) phase_p<P64, P32, BIF>(c, beta, first, bid, nb);
-    else phase_p<P32, P32, BIF>(c, beta, first, bid, nb);
+    if (ps == P64) phase_p<P64, P32, BIF>(c, beta, first, false, bid, nb);
+    else phase_p<P32, P32, BIF>(c, beta, first, false, bid, nb);
   } else {
-    if (ps == P64) phase_p<P64, P16, BIF>(c, beta, first, bid, nb);
-    else if (ps == P32) phase_p<P32, P16, BIF>(c, beta, first, bid, nb);
-    else phase_p<P16, P16, BIF>(c, beta, first, bid, nb);
+    if (ps == P64) phase_p<P64, P16, BIF>(c, beta, first, false, bid, nb);
+    else if (ps == P32) phase_p<P32, P16, BIF>(c, beta, first, false, bid, nb);
+    else phase_p<P16, P16, BIF>(c, beta, first, false, bid, nb);
   }
 }
 
 template <bool COH, int NT>
 __device__ __forceinline__ double dispatch_spmv(const Ctx& c, int ur, int uz, int bid, int nb, double* red) {
   if (ur == P64) {
-    if (uz == P64) return phase_spmv<P64, COH, NT>(c, c.p64, c.q64, bid, nb, red);
-    if (uz == P32) return phase_spmv<P64, COH, NT>(c, c.p32, c.q64, bid, nb, red);
-    return phase_spmv<P64, COH, NT>(c, c.p16, c.q64, bid, nb, red);
+    if (uz == P64) return phase_spmv<P64, COH, NT>(c, c.p64, c.p64, c.q64, bid, nb, red);
+    if (uz == P32) return phase_spmv<P64, COH, NT>(c, c.p32, c.p32, c.q64, bid, nb, red);
+    return phase_spmv<P64, COH, NT>(c, c.p16, c.p16, c.q64, bid, nb, red);
   }
-  if (uz == P64) return phase_spmv<P32, COH, NT>(c, c.p64, c.q32, bid, nb, red);
-  if (uz == P32) return phase_spmv<P32, COH, NT>(c, c.p32, c.q32, bid, nb, red);
-  return phase_spmv<P32, COH, NT>(c, c.p16, c.q32, bid, nb, red);
+  // u_z = FP64 with u_r = FP32: the p update left RN32(p) in the FP32 copy (phase_p, shadow32): gather that
+  if (uz == P64) return phase_spmv<P32, COH, NT>(c, c.p32, c.p64, c.q32, bid, nb, red);
+  if (uz == P32) return phase_spmv<P32, COH, NT>(c, c.p32, c.p32, c.q32, bid, nb, red);
+  return phase_spmv<P32, COH, NT>(c, c.p16, c.p16, c.q32, bid, nb, red);
 }
 
 template <int BIF = kVecBytesInFlight>
@@ -65,7 +79,7 @@ __device__ __forceinline__ double dispatch_xr(const Ctx& c, int ur, int uz, doub
 }
 
 // ------------------------------------------------------------------ loop kernels ------------
-__global__ void __launch_bounds__(kVecThreads, 3) k_z(const Ctx c) {
+__global__ void __launch_bounds__(kVecThreads, AMP_KZ_BLOCKS) k_z(const Ctx c) {
   __shared__ double red[32];
   DevState* s = c.st;
   pdl_launch_dependents();
@@ -77,12 +91,12 @@ __global__ void __launch_bounds__(kVecThreads, 3) k_z(const Ctx c) {
                            [&](double tot) { epi_rho(epi_ctx(c), tot); });
 }
 
-__global__ void __launch_bounds__(kVecThreads, 3) k_p(const Ctx c) {
+__global__ void __launch_bounds__(kVecThreads, AMP_KP_BLOCKS) k_p(const Ctx c) {
   const DevState* s = c.st;
   pdl_launch_dependents();
   pdl_wait();
   if (s->done) return;
-  dispatch_p(c, s->p_store, s->uz, s->beta, s->k == 0, blockIdx.x, gridDim.x);
+  dispatch_p(c, s->p_store, s->uz, s->ur, s->beta, s->k == 0, blockIdx.x, gridDim.x);
 }
 
 __global__ void __launch_bounds__(kSpmvThreads, kSpmvMinBlocks) k_spmv(const Ctx c) {
@@ -98,7 +112,7 @@ __global__ void __launch_bounds__(kSpmvThreads, kSpmvMinBlocks) k_spmv(const Ctx
                             [&](double tot) { epi_gamma(epi_ctx(c), tot); });
 }
 
-__global__ void __launch_bounds__(kVecThreads, 2) k_xr(const Ctx c) {
+__global__ void __launch_bounds__(kVecThreads, AMP_KXR_BLOCKS) k_xr(const Ctx c) {
   __shared__ double red[32];
   DevState* s = c.st;
   pdl_launch_dependents();
@@ -157,7 +171,7 @@ __global__ void __launch_bounds__(kVecThreads, 2) k_xrz(const Ctx c) {
 template <int UR, class PT>
 __global__ void __launch_bounds__(kSpmvThreads, kSpmvMinBlocks) k_spmv_any(const Ctx c, const PT* p, typename Store<UR>::T* q) {
   __shared__ double red[32];
-  (void)phase_spmv<UR, false, kSpmvThreads>(c, p, q, blockIdx.x, gridDim.x, red);
+  (void)phase_spmv<UR, false, kSpmvThreads>(c, p, p, q, blockIdx.x, gridDim.x, red);
 }
 
 // ------------------------------------------------------------------ set-up / finalise -------

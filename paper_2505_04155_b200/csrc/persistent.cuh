@@ -81,8 +81,8 @@ __device__ __forceinline__ void grid_all_sum2(double v0, double v1, double* part
 __device__ __noinline__ double pz(const Ctx& c, int rs, int ur, int uz, double omega, int bid, int nb) {
   return dispatch_z<kPersistBIF>(c, rs, ur, uz, omega, bid, nb);
 }
-__device__ __noinline__ void pp(const Ctx& c, int ps, int uz, double beta, bool first, int bid, int nb) {
-  dispatch_p<kPersistBIF>(c, ps, uz, beta, first, bid, nb);
+__device__ __noinline__ void pp(const Ctx& c, int ps, int uz, int ur, double beta, bool first, int bid, int nb) {
+  dispatch_p<kPersistBIF>(c, ps, uz, ur, beta, first, bid, nb);
 }
 __device__ __noinline__ double ps_(const Ctx& c, int ur, int uz, int bid, int nb, double* red) {
   return dispatch_spmv<true, kPersistThreads>(c, ur, uz, bid, nb, red);
@@ -122,7 +122,7 @@ __global__ void __launch_bounds__(kPersistThreads, kPersistMinBlocks) k_persiste
       __syncthreads();
     }
     while (!s->done) {
-      pp(c, s->p_store, s->uz, s->beta, s->k == 0, bid, nb);                                         // a3
+      pp(c, s->p_store, s->uz, s->ur, s->beta, s->k == 0, bid, nb);                                  // a3
       grid_all_sum<false>(0.0, nullptr, arrivals, target, bid, nb, red);
       const double v = ps_(c, s->ur, s->uz, bid, nb, red);                                           // a4
       const double t = grid_all_sum<true>(v, c.partials + 1 * kMaxGrid, arrivals, target, bid, nb, red);
@@ -143,7 +143,7 @@ __global__ void __launch_bounds__(kPersistThreads, kPersistMinBlocks) k_persiste
     double t = grid_all_sum<true>(v, c.partials + 0 * kMaxGrid, arrivals, target, bid, nb, red);
     if (threadIdx.x == 0) epi_rho(ec, t);
     __syncthreads();
-    pp(c, ps, uz, s->beta, first, bid, nb);                                                          // a3
+    pp(c, ps, uz, ur, s->beta, first, bid, nb);                                                      // a3
     grid_all_sum<false>(0.0, nullptr, arrivals, target, bid, nb, red);
     v = ps_(c, ur, uz, bid, nb, red);                                                                // a4
     t = grid_all_sum<true>(v, c.partials + 1 * kMaxGrid, arrivals, target, bid, nb, red);

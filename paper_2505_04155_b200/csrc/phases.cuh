@@ -313,8 +313,11 @@ __device__ __forceinline__ double phase_z(const Ctx& c, const double omega, int 
 // ------------------------------------------------------------------ a3: p -------------------
 // PS: precision p_{k-1} is stored in; UZ: precision of z_k and p_k (PS != UZ only at a u_z
 // switch, where p_{k-1} <- RN_{u_z}(p_{k-1}) is fused here, reading R9).
+// shadow32 (only with UZ = P64): also store RN32(p) into the FP32 copy of p.  While u_z = FP64 and u_r = FP32 the
+// mat-vec needs RN32(p_j) for every gathered entry (reading R7); rounding each row once here instead of once per
+// gather there takes an FP64->FP32 conversion per ENTRY out of the SpMV (c4: 27 per row) for 4 B per row more here.
 template <int PS, int UZ, int BIF = kVecBytesInFlight>
-__device__ __forceinline__ void phase_p(const Ctx& c, const double beta, const bool first, int bid, int nb) {
+__device__ __forceinline__ void phase_p(const Ctx& c, const double beta, const bool first, const bool shadow32, int bid, int nb) {
   using TP = typename Store<PS>::T;
   using TZ = typename Store<UZ>::T;
   constexpr int E = chunk_elems(cmin((int)sizeof(TP), (int)sizeof(TZ)), cmax((int)sizeof(TP), (int)sizeof(TZ)));
@@ -356,6 +359,13 @@ __device__ __forceinline__ void phase_p(const Ctx& c, const double beta, const b
         Chunk<TZ, E> po;
         chunk_pack(po, a);
         chunk_store(po, pout, i);
+        if constexpr (UZ == P64) {
+          if (shadow32) {
+            Chunk<float, E> p32;
+            chunk_pack(p32, a);
+            chunk_store(p32, c.p32, i);
+          }
+        }
 #ifdef AMP_COUNT_FP16
         if (UZ == P16) {
           double h[E];

@@ -343,8 +343,10 @@ constexpr int kSpmvGroupMax = AMP_SPMV_G32 > AMP_SPMV_G64 ? AMP_SPMV_G32 : AMP_S
 // (persistent) kernel, so it is gathered with plain coherent loads instead of the read-only path.
 // NT = threads per block.
 // Returns this thread's part of gamma = sum_i p_i q_i (stored q_i, FP64 products and sums).
-template <int UR, bool COH, int CMG, int NT, class PT>
-__device__ __forceinline__ double phase_spmv_fmt(const Ctx& c, const PT* p, typename Store<UR>::T* q, int bid, int nb,
+// pg: the STORED p (u_z precision) for gamma = q^T p; it differs from the gathered operand p only in phase
+// (u_z = FP64, u_r = FP32), where p is the FP32 copy RN32(p) written by the p update.
+template <int UR, bool COH, int CMG, int NT, class PT, class PG>
+__device__ __forceinline__ double phase_spmv_fmt(const Ctx& c, const PT* p, const PG* pg, typename Store<UR>::T* q, int bid, int nb,
                                                  double* red) {
   using A = typename SpmvT<UR>::A;
   constexpr int G = SpmvGroup<UR>::G;
@@ -402,7 +404,7 @@ __device__ __forceinline__ double phase_spmv_fmt(const Ctx& c, const PT* p, type
       else if (c.sell_perm != nullptr) row = __ldg(c.sell_perm + row);  // -1: padding slot
       if (row >= n) row = -1;
       rows[g] = row;
-      pi[g] = gather64<COH>(p, row < 0 ? 0 : row);  // p_i for gamma, issued with the other gathers
+      pi[g] = gather64<COH>(pg, row < 0 ? 0 : row);  // p_i for gamma, issued with the other gathers
     }
     A acc[G];
     if (wmax <= 7 && all_al) {
@@ -459,17 +461,17 @@ __device__ __forceinline__ double phase_spmv_fmt(const Ctx& c, const PT* p, type
     if (threadIdx.x == 0) {
       const A qi = (A)tot;
       q[row] = qi;
-      gsum = fma(gather64<COH>(p, row), (double)qi, gsum);
+      gsum = fma(gather64<COH>(pg, row), (double)qi, gsum);
     }
   }
   return gsum;
 }
 
-template <int UR, bool COH, int NT, class PT>
-__device__ __forceinline__ double phase_spmv(const Ctx& c, const PT* p, typename Store<UR>::T* q, int bid, int nb,
+template <int UR, bool COH, int NT, class PT, class PG>
+__device__ __forceinline__ double phase_spmv(const Ctx& c, const PT* p, const PG* pg, typename Store<UR>::T* q, int bid, int nb,
                                              double* red) {
-  if (c.sell_cols16 != nullptr) return phase_spmv_fmt<UR, COH, 1, NT>(c, p, q, bid, nb, red);
-  return phase_spmv_fmt<UR, COH, 0, NT>(c, p, q, bid, nb, red);
+  if (c.sell_cols16 != nullptr) return phase_spmv_fmt<UR, COH, 1, NT>(c, p, pg, q, bid, nb, red);
+  return phase_spmv_fmt<UR, COH, 0, NT>(c, p, pg, q, bid, nb, red);
 }
 
 // ------------------------------------------------------------------ create(): CSR -> SELL-32 --

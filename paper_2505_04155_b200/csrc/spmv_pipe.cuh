@@ -150,8 +150,8 @@ __device__ __forceinline__ A pipe_slice_sum(const A* sv, const int* sb, int w, i
 // entry nchunks closes the list
 struct PipeChunk { int32_t s0, w0; };
 
-template <int UR, class PT>
-__device__ __forceinline__ double pipe_body(const Ctx& c, const PT* p, typename Store<UR>::T* q, unsigned char* smem) {
+template <int UR, class PT, class PG>
+__device__ __forceinline__ double pipe_body(const Ctx& c, const PT* p, const PG* pg, typename Store<UR>::T* q, unsigned char* smem) {
   using A = typename SpmvT<UR>::A;
   constexpr int STAGE = 32 * kPipeChunkW * (int)sizeof(A);
   constexpr int NST = kPipeValueBytes / STAGE;
@@ -210,7 +210,7 @@ __device__ __forceinline__ double pipe_body(const Ctx& c, const PT* p, typename 
         const int w0 = sw0[sl] & ~kAlignedFlag, w = (sw0[sl + 1] & ~kAlignedFlag) - w0;
         const int row = sl * 32 + lane;
         const PT* pl = p + row;
-        const double pi = gather64<false>(pl, 0);
+        const double pi = gather64<false>(pg, row);  // the stored p_i (u_z precision) for gamma
         A acc = 0;
         if (w > 0) acc = pipe_slice_sum<A, PT>(sv0 + (size_t)(w0 - hd.z) * 32, sb0 + w0, w, lane, pl);
         if (row < n) {
@@ -239,9 +239,9 @@ __global__ void __launch_bounds__(kPipeThreads, 1) k_spmv_pipe(const Ctx c) {
   const int ur = s->ur, uz = s->uz;
   if (s->done || ur != P32) { pdl_wait(); return; }
   double v;
-  if (uz == P64) v = pipe_body<P32>(c, c.p64, c.q32, pipe_smem);
-  else if (uz == P32) v = pipe_body<P32>(c, c.p32, c.q32, pipe_smem);
-  else v = pipe_body<P32>(c, c.p16, c.q32, pipe_smem);
+  if (uz == P16) v = pipe_body<P32>(c, c.p16, c.p16, c.q32, pipe_smem);
+  else if (uz == P32) v = pipe_body<P32>(c, c.p32, c.p32, c.q32, pipe_smem);
+  else v = pipe_body<P32>(c, c.p32, c.p64, c.q32, pipe_smem);  // gathers the FP32 copy RN32(p) written by the p update
   pdl_wait();  // (the producer warp has not waited yet) before touching the reduction scratch shared with other kernels
   grid_reduce<kPipeThreads>(v, c.partials + 1 * kMaxGrid, &s->counter[1], blockIdx.x, gridDim.x, red,
                             [&](double tot) { epi_gamma(epi_ctx(c), tot); });

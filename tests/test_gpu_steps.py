@@ -121,6 +121,20 @@ def test_step_p_bitwise(handle, ps, uz, first):
         assert_bits(host(h.debug_get_vector(A.VEC_P, uz)), p_ref, "p")
 
 
+def test_step_p_writes_the_fp32_copy_in_phase_fp64_fp32(handle):
+    # while u_z = FP64 and u_r = FP32 the mat-vec gathers RN32(p_j) (reading R7): the p update stores that copy
+    s, h, _ = handle
+    rng = np.random.default_rng(77)
+    z = special(rng, s.n); z[~np.isfinite(z)] = 0.0
+    p = rng.standard_normal(s.n)
+    h.debug_set_vector(A.VEC_Z, dev(z, 0))
+    h.debug_set_vector(A.VEC_P, dev(p, 0))
+    h.debug_step(A.STEP_P, rs=1, ur=1, uz=0, ps=0, ur_n=1, uz_n=0, beta=0.61)
+    p_ref, _ = O.step_p(0.61, p, z, 0)
+    assert_bits(host(h.debug_get_vector(A.VEC_P, 0)), p_ref, "p")
+    assert_bits(host(h.debug_get_vector(A.VEC_P, 1)), O.round_fp32(p_ref), "RN32(p)")
+
+
 XR_INST = [(ur, uz) for ur in (0, 1) for uz in (0, 1, 2)]
 
 
