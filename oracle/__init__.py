@@ -22,7 +22,7 @@ _LIB = os.path.join(_HERE, "liboracle_amp_pcg.so")
 FP64, FP32, FP16 = 0, 1, 2
 ETA_DELAY, ETA_LINEAR, ETA_NEVER = 0, 1, 2
 SCALE_NORM2, SCALE_RMS, SCALE_POW2, SCALE_NONE, SCALE_LAGGED = 0, 1, 2, 3, 4
-PRECOND_NONE, PRECOND_JACOBI = 0, 1
+PRECOND_NONE, PRECOND_JACOBI, PRECOND_CHEBJACOBI = 0, 1, 2
 
 
 def build(force: bool = False) -> str:
@@ -46,7 +46,8 @@ class _Policy(C.Structure):
     _fields_ = [
         ("amp", C.c_int32), ("u0", C.c_int32), ("eta_rule", C.c_int32), ("d", C.c_int32), ("ell", C.c_int32),
         ("scale_mode", C.c_int32), ("no_stop", C.c_int32), ("strict_rounding", C.c_int32),
-        ("accumulate64", C.c_int32), ("precond", C.c_int32),
+        ("accumulate64", C.c_int32), ("precond", C.c_int32), ("cheb_degree", C.c_int32), ("pad0", C.c_int32),
+        ("cheb_lmin", C.c_double), ("cheb_lmax", C.c_double),
         ("C", C.c_double), ("tau_zs", C.c_double), ("tau_zh", C.c_double), ("eps32", C.c_double),
         ("eta_safety", C.c_double), ("stop_safety", C.c_double),
     ]
@@ -100,6 +101,19 @@ def lib():
         L.orc_step_xr.argtypes = [C.c_int64, C.c_double, C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p]
         L.orc_classify_fp16.restype = C.c_int32
         L.orc_classify_fp16.argtypes = [C.c_double, C.c_double]
+        L.orc_cheb_default_bounds.restype = None
+        L.orc_cheb_default_bounds.argtypes = [C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_double, C.c_void_p, C.c_void_p]
+        L.orc_cheb_coeffs.restype = None
+        L.orc_cheb_coeffs.argtypes = [C.c_int32, C.c_double, C.c_double, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.orc_cheb_first.restype = None
+        L.orc_cheb_first.argtypes = [C.c_int64, C.c_void_p, C.c_double, C.c_void_p, C.c_double, C.c_int32, C.c_void_p, C.c_void_p]
+        L.orc_cheb_step.restype = None
+        L.orc_cheb_step.argtypes = [C.c_int64, C.c_void_p, C.c_double, C.c_void_p, C.c_void_p, C.c_double, C.c_double,
+                                    C.c_int32, C.c_void_p, C.c_void_p]
+        L.orc_cheb_apply.restype = None
+        L.orc_cheb_apply.argtypes = [C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_double,
+                                     C.c_void_p, C.c_int32, C.c_double, C.c_double, C.c_int32, C.c_int32, C.c_void_p,
+                                     C.c_void_p, C.c_void_p]
         L.orc_amp_pcg.restype = C.c_int32
         L.orc_amp_pcg.argtypes = [C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
                                   C.c_double, C.c_int32, C.POINTER(_Policy), C.POINTER(_Stats), C.c_void_p,
@@ -113,10 +127,12 @@ def lib():
 def make_policy(amp: int = 1, u0: int = FP64, eta_rule: int = ETA_DELAY, d: int = 10, ell: int = 5, C_: float = 1.0,
                 tau_zs: float = 1e-4, tau_zh: float = 1e-6, eps32: float = 2.0 ** -24, eta_safety: float = 1.0,
                 stop_safety: float = 1.0, scale_mode: int = SCALE_NORM2, no_stop: int = 0,
-                strict_rounding: int = 0, accumulate64: int = 0, precond: int = PRECOND_JACOBI) -> _Policy:
+                strict_rounding: int = 0, accumulate64: int = 0, precond: int = PRECOND_JACOBI, cheb_degree: int = 2,
+                cheb_lmin: float = 0.0, cheb_lmax: float = 0.0) -> _Policy:
     """Paper defaults: d=10, C=1, ell=5 (:400), tau (5.1) (:404-405), eps32 = 2^-24 (:354)."""
     return _Policy(amp=amp, u0=u0, eta_rule=eta_rule, d=d, ell=ell, scale_mode=scale_mode, no_stop=no_stop,
-                   strict_rounding=strict_rounding, accumulate64=accumulate64, precond=precond, C=C_,
+                   strict_rounding=strict_rounding, accumulate64=accumulate64, precond=precond, cheb_degree=cheb_degree,
+                   cheb_lmin=cheb_lmin, cheb_lmax=cheb_lmax, C=C_,
                    tau_zs=tau_zs, tau_zh=tau_zh, eps32=eps32, eta_safety=eta_safety, stop_safety=stop_safety)
 
 
@@ -199,6 +215,47 @@ def step_xr(alpha: float, p, q, x, r, ur: int):
 def classify_fp16(unrounded: float, stored: float) -> int:
     """1 = became inf, 2 = flushed to zero, 3 = subnormal, 0 = anything else."""
     return int(lib().orc_classify_fp16(float(unrounded), float(stored)))
+
+
+def cheb_default_bounds(rowptr, colidx, vals, ratio: float = 30.0):
+    """(lmin, lmax): Gershgorin bound of D^-1 A and lmax / ratio (the defaults of the Chebyshev-Jacobi preconditioner)."""
+    lo, hi = C.c_double(), C.c_double()
+    lib().orc_cheb_default_bounds(len(rowptr) - 1, _ptr(rowptr), _ptr(colidx), _ptr(vals), float(ratio), C.byref(lo), C.byref(hi))
+    return lo.value, hi.value
+
+
+def cheb_coeffs(s: int, lmin: float, lmax: float):
+    """(1/theta, c1[0..s-1], c2[0..s-1]) of the Chebyshev recurrence (index 0 unused)."""
+    it = C.c_double()
+    c1 = np.zeros(s + 1); c2 = np.zeros(s + 1)
+    lib().orc_cheb_coeffs(int(s), float(lmin), float(lmax), C.byref(it), _ptr(c1), _ptr(c2))
+    return it.value, c1[:s], c2[:s]
+
+
+def cheb_first(r, omega: float, dinv, inv_theta: float, uz: int):
+    r, dinv = _f64(r), _f64(dinv)
+    d = np.empty_like(r); z = np.empty_like(r)
+    lib().orc_cheb_first(r.size, _ptr(r), float(omega), _ptr(dinv), float(inv_theta), int(uz), _ptr(d), _ptr(z))
+    return d, z
+
+
+def cheb_step(r, omega: float, w, dinv, c1: float, c2: float, uz: int, d, z):
+    r, w, dinv = _f64(r), _f64(w), _f64(dinv)
+    d = np.array(d, dtype=np.float64, copy=True); z = np.array(z, dtype=np.float64, copy=True)
+    lib().orc_cheb_step(r.size, _ptr(r), float(omega), _ptr(w), _ptr(dinv), float(c1), float(c2), int(uz), _ptr(d), _ptr(z))
+    return d, z
+
+
+def cheb_apply(rowptr, colidx, vals, r, omega: float, dinv, s: int, lmin: float, lmax: float, uz: int = FP64, ur: int = FP64):
+    """z = M^-1 (omega r): s sweeps of Chebyshev-accelerated Jacobi in precisions (u_z, u_r)."""
+    rowptr = np.ascontiguousarray(rowptr, dtype=np.int32); colidx = np.ascontiguousarray(colidx, dtype=np.int32)
+    vals = _f64(vals); r = _f64(r); dinv = _f64(dinv)
+    v32 = vals.astype(np.float32)
+    n = r.size
+    z = np.empty(n); d = np.empty(n); w = np.empty(n)
+    lib().orc_cheb_apply(n, _ptr(rowptr), _ptr(colidx), _ptr(vals), _ptr(v32), _ptr(r), float(omega), _ptr(dinv), int(s),
+                         float(lmin), float(lmax), int(uz), int(ur), _ptr(z), _ptr(d), _ptr(w))
+    return z
 
 
 def eta(policy: _Policy, hist: np.ndarray, k: int) -> float:

@@ -22,6 +22,7 @@
 //                                     and (4.11) (:370-375).  x, all inner products, norms
 //                                     and scalars are FP64.
 //   orc_eta_posteriori                the a-posteriori indicator eta_hat_m(k) of (4.7) (:350-354).
+//   orc_cheb_*                        Chebyshev-accelerated Jacobi preconditioner (the paper's smoother, :461; reading R18).
 //   orc_step_z / orc_step_p / orc_step_xr   the vector steps of the loop body (Alg 4.1 lines 4-5, 10, 15-16),
 //                                     called by orc_amp_pcg and, one at a time, by the per-step GPU parity tests.
 //
@@ -148,7 +149,10 @@ struct orc_policy {
   int32_t no_stop;          // 1: ignore the stopping test, run maxit iterations
   int32_t strict_rounding;  // diagnostic R6: y and M^-1 stored in u_z, two roundings
   int32_t accumulate64;     // diagnostic R7: FP32-phase SpMV accumulated in FP64
-  int32_t precond;          // 0: M = I ; 1: Jacobi, M = diag(A)
+  int32_t precond;          // 0: M = I ; 1: Jacobi, M = diag(A) ; 2: Chebyshev-accelerated Jacobi (reading R18)
+  int32_t cheb_degree;      // number of Jacobi sweeps s >= 1 of one application (s - 1 mat-vecs); "second-order": 2
+  int32_t pad0;
+  double cheb_lmin, cheb_lmax;  // bounds of the spectrum of D^-1 A the polynomial is built for; 0, 0: orc_cheb_default_bounds
   double C;                 // constant of Assumption 4.1, default 1
   double tau_zs, tau_zh;    // thresholds (5.1)
   double eps32;             // unit roundoff of FP32, 2^-24
@@ -282,6 +286,90 @@ void orc_step_xr(int64_t n, double alpha, const double* p, const double* q, int3
 // classification of one FP16 store (see classify_fp16), exported for its pin
 int32_t orc_classify_fp16(double unrounded, double stored) { return classify_fp16(unrounded, stored); }
 
+// ---------------------------------------------------------------- Chebyshev-accelerated Jacobi ----
+// The paper's smoother ("second-order Chebyshev-accelerated Jacobi smoother [35]"; stronger
+// preconditioners are its stated remedy for hard spectra, :584) used as the preconditioner M^-1 of the loop.  The paper
+// gives no formulas; this is the textbook Chebyshev iteration for A z = y with the Jacobi splitting, started from
+// z = 0 and stopped after s sweeps (reading R18 of DESIGN.md), D = diag(A), [lmin, lmax] bounds of the spectrum of
+// D^-1 A:   theta = (lmax+lmin)/2, dc = (lmax-lmin)/2, sigma = theta/dc, rho_0 = 1/sigma,
+//   d_0 = D^-1 y / theta,                     z_1 = d_0
+//   for i = 1 .. s-1:  rho_i = 1/(2 sigma - rho_{i-1}),  t = y - A z_i,
+//                      d_i = rho_i rho_{i-1} d_{i-1} + (2 rho_i / dc) D^-1 t,   z_{i+1} = z_i + d_i
+// i.e. z_s = (I - q_s(D^-1 A)) A^-1 y with q_s(l) = T_s((theta - l)/dc) / T_s(sigma) (T_s: Chebyshev polynomial).
+// In the mixed-precision loop y = omega r is never stored (recomputed from the stored r in FP64), d and z are stored in
+// u_z with ONE rounding per update, w = A z is computed and stored in u_r like q, all scalars FP64.
+
+// lmax = max_i (sum_j |a_ij|) / a_ii  (Gershgorin bound of D^-1 A, sums in CSR order), lmin = lmax / ratio
+void orc_cheb_default_bounds(int64_t n, const int32_t* rowptr, const int32_t* colidx, const double* vals, double ratio,
+                             double* lmin, double* lmax) {
+  double m = 0.0;
+  for (int64_t i = 0; i < n; ++i) {
+    double d = 0.0, srow = 0.0;
+    for (int32_t e = rowptr[i]; e < rowptr[i + 1]; ++e) {
+      srow += std::fabs(vals[e]);
+      if (colidx[e] == i) d += vals[e];
+    }
+    const double g = srow / d;
+    if (g > m) m = g;
+  }
+  *lmax = m;
+  *lmin = m / ratio;
+}
+
+// inv_theta = 1/theta; c1[i] = rho_i rho_{i-1}, c2[i] = 2 rho_i / dc for i = 1 .. s-1 (index 0 unused)
+void orc_cheb_coeffs(int32_t s, double lmin, double lmax, double* inv_theta, double* c1, double* c2) {
+  const double theta = (lmax + lmin) / 2.0, dc = (lmax - lmin) / 2.0, sigma = theta / dc;
+  *inv_theta = 1.0 / theta;
+  double rho_prev = 1.0 / sigma;
+  c1[0] = c2[0] = 0.0;
+  for (int32_t i = 1; i < s; ++i) {
+    const double rho = 1.0 / (2.0 * sigma - rho_prev);
+    c1[i] = rho * rho_prev;
+    c2[i] = 2.0 * rho / dc;
+    rho_prev = rho;
+  }
+}
+
+// first sweep: d_i = RN_{u_z}( ((r_i omega) dinv_i) inv_theta ), z = d
+void orc_cheb_first(int64_t n, const double* r, double omega, const double* dinv, double inv_theta, int32_t uz,
+                    double* d, double* z) {
+#pragma omp parallel for schedule(static)
+  for (int64_t i = 0; i < n; ++i) {
+    const double v = round_store(((r[i] * omega) * dinv[i]) * inv_theta, uz);
+    d[i] = v;
+    z[i] = v;
+  }
+}
+
+// sweep i >= 1, given w = A z: t = r omega - w; u = t dinv; d = RN_{u_z}(fma(c1, d, c2 u)); z = RN_{u_z}(z + d)
+void orc_cheb_step(int64_t n, const double* r, double omega, const double* w, const double* dinv, double c1, double c2,
+                   int32_t uz, double* d, double* z) {
+#pragma omp parallel for schedule(static)
+  for (int64_t i = 0; i < n; ++i) {
+    const double t = r[i] * omega - w[i];
+    const double u = t * dinv[i];
+    const double dn = round_store(std::fma(c1, d[i], c2 * u), uz);
+    d[i] = dn;
+    z[i] = round_store(z[i] + dn, uz);
+  }
+}
+
+// one whole application z = M^-1 (omega r) in precisions (u_z, u_r); vals32 (FP32-rounded values) is read when ur = FP32;
+// dinv = 1/a_ii in FP64 when uz = FP64, else its FP32-rounded copy (reading R6); work: d, w of length n
+void orc_cheb_apply(int64_t n, const int32_t* rowptr, const int32_t* colidx, const double* vals, const float* vals32,
+                    const double* r, double omega, const double* dinv, int32_t s, double lmin, double lmax, int32_t uz,
+                    int32_t ur, double* z, double* d, double* w) {
+  std::vector<double> c1((size_t)s + 1), c2((size_t)s + 1);
+  double inv_theta;
+  orc_cheb_coeffs(s, lmin, lmax, &inv_theta, c1.data(), c2.data());
+  orc_cheb_first(n, r, omega, dinv, inv_theta, uz, d, z);
+  for (int32_t i = 1; i < s; ++i) {
+    if (ur == ORC_FP64) orc_spmv_fp64(n, rowptr, colidx, vals, z, w);
+    else orc_spmv_fp32(n, rowptr, colidx, vals32, z, w, 0);
+    orc_cheb_step(n, r, omega, w, dinv, c1[(size_t)i], c2[(size_t)i], uz, d, z);
+  }
+}
+
 // ---------------------------------------------------------------- the solver --------------
 // Algorithm 4.1 (amp=1) / Algorithm 3.1 (amp=0), step by step in the paper's order.
 // x: in = x0, out = x_m.  hist (may be NULL) receives ||r_t||, t = 0..iters.
@@ -297,13 +385,26 @@ int32_t orc_amp_pcg(int64_t n, const int32_t* rowptr, const int32_t* colidx, con
 
   for (int64_t i = 0; i < n; ++i) {
     double d = 1.0;
-    if (pol->precond == 1) {
+    if (pol->precond >= 1) {
       d = 0.0;   // M = diag(A) (Jacobi); duplicate entries add up, as they do in the mat-vec
       for (int32_t e = rowptr[i]; e < rowptr[i + 1]; ++e) if (colidx[e] == i) d += vals[e];
       if (!(d > 0.0)) { st->status = -1; return -1; }
     }
     dinv[(size_t)i] = 1.0 / d;
     dinv32[(size_t)i] = orc_round_fp32(1.0 / d);
+  }
+
+  const bool cheb = pol->precond == 2;
+  double cheb_lmin = pol->cheb_lmin, cheb_lmax = pol->cheb_lmax;
+  std::vector<double> cheb_d, cheb_w;
+  if (cheb) {
+    if (pol->cheb_degree < 1 || pol->cheb_degree > 16 || (pol->amp && pol->scale_mode == ORC_SCALE_LAGGED) || pol->strict_rounding) {
+      st->status = -1; return -1;
+    }
+    if (!(cheb_lmax > 0.0)) orc_cheb_default_bounds(n, rowptr, colidx, vals, 30.0, &cheb_lmin, &cheb_lmax);
+    if (!(cheb_lmin > 0.0) || !(cheb_lmax > cheb_lmin)) { st->status = -1; return -1; }
+    cheb_d.resize((size_t)n); cheb_w.resize((size_t)n);
+    if (vals32.empty()) { vals32.resize((size_t)nnz); for (int64_t e = 0; e < nnz; ++e) vals32[(size_t)e] = (float)vals[e]; }
   }
 
   // O0: r0 = b - A x0 in FP64, delta0 = ||r0||   (Alg 4.1 line 1)
@@ -378,7 +479,11 @@ int32_t orc_amp_pcg(int64_t n, const int32_t* rowptr, const int32_t* colidx, con
     const bool strict = pol->strict_rounding && pol->amp;
     const double* dv = (uz == ORC_FP64 || strict) ? dinv.data() : dinv32.data();            // R6
     int64_t counts[3] = {0, 0, 0};
-    orc_step_z(n, r.data(), omega, dv, ur, uz, strict ? 1 : 0, z.data(), counts);
+    if (cheb)   // M^-1 = s sweeps of Chebyshev-accelerated Jacobi (reading R18); needs s - 1 mat-vecs in u_r
+      orc_cheb_apply(n, rowptr, colidx, vals, vals32.data(), r.data(), omega, dv, pol->cheb_degree, cheb_lmin, cheb_lmax, uz, ur,
+                     z.data(), cheb_d.data(), cheb_w.data());
+    else
+      orc_step_z(n, r.data(), omega, dv, ur, uz, strict ? 1 : 0, z.data(), counts);
     // O3: rho = r^T z (Alg 4.1 line 6), FP64, with the stored z
     const double rho = dot_fp64(n, r.data(), z.data());
     // O4: beta (lines 7-9)
