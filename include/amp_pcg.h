@@ -35,7 +35,20 @@ typedef struct amp_pcg amp_pcg_t; /* opaque solver handle */
 
 /* preconditioner M: the paper uses M = I for its small examples and Jacobi for
  * the timed GPU example */
-enum { AMP_PRECOND_NONE = 0, AMP_PRECOND_JACOBI = 1 };
+enum {
+  AMP_PRECOND_NONE = 0,
+  AMP_PRECOND_JACOBI = 1,
+  /* s sweeps of Chebyshev-accelerated Jacobi, the paper's smoother ("second-order Chebyshev-accelerated
+   * Jacobi smoother [35]"; stronger preconditioning is what the paper asks for when the spectrum is hard, :584), used as
+   * M^-1 of the loop (reading R18): with D = diag(A), [lmin, lmax] bounds of the spectrum of D^-1 A,
+   * theta = (lmax+lmin)/2, dc = (lmax-lmin)/2, sigma = theta/dc, rho_0 = 1/sigma and y = omega r (Alg 4.1 line 4):
+   *   d = D^-1 y / theta, z = d;   then for i = 1..s-1:  rho_i = 1/(2 sigma - rho_{i-1}),
+   *   d = rho_i rho_{i-1} d + (2 rho_i/dc) D^-1 (y - A z),  z = z + d.
+   * d, z are stored in u_z (one rounding per update), A z is computed and stored in u_r (like q), scalars FP64.
+   * Costs s - 1 extra mat-vecs per iteration and divides the iteration count by about s.  Needs amp_pcg_create_ex
+   * (cheb_degree, bounds); not available with AMP_SCALE_LAGGED or AMP_LOOP_PERSISTENT. */
+  AMP_PRECOND_CHEBJACOBI = 2
+};
 /* column-index form of the SELL-32 repack.  AUTO takes the most compact form the matrix
  * allows; the other two force a more general form on the same matrix (testing / tuning) */
 enum {
@@ -159,6 +172,10 @@ typedef struct {
   int32_t spmv_kernel;    /* AMP_SPMV_*, default AUTO */
   int32_t spmv_grid_mult; /* upper bound on resident SpMV blocks per SM for the direct kernel's grid; 0 = automatic */
   int32_t pdl;            /* 1 (default): launch the loop kernels as programmatic dependents (griddepcontrol), 0: plain */
+  int32_t cheb_degree;    /* AMP_PRECOND_CHEBJACOBI: sweeps s, 1 <= s <= 16; default 2 (the paper's "second-order") */
+  int32_t reserved0;      /* 0 */
+  double cheb_lmin;       /* bounds of the spectrum of D^-1 A the polynomial is built for; cheb_lmax = 0 (default): */
+  double cheb_lmax;       /*   lmax = max_i sum_j |a_ij| / a_ii (Gershgorin), lmin = lmax / 30, computed in create() */
   void *stream;           /* cudaStream_t the create() kernels run on and the handle starts with (NULL = legacy
                              default stream); the caller's CSR arrays must be complete in this stream's order */
 } amp_create_opts_t;
@@ -234,9 +251,11 @@ double amp_pcg_spmv_bytes(const amp_pcg_t *h, int mat_prec, int vec_prec);
 double amp_pcg_iteration_bytes(const amp_pcg_t *h, int uz, int ur);
 
 /* ---- measurement: per-kernel device times of the last solve made with policy.profile_kernels = 1 ---------- */
-enum { AMP_K_Z = 0, AMP_K_P = 1, AMP_K_SPMV = 2, AMP_K_XR = 3, AMP_K_XRZ = 4, AMP_K_COUNT = 5 };
+enum { AMP_K_Z = 0, AMP_K_P = 1, AMP_K_SPMV = 2, AMP_K_XR = 3, AMP_K_XRZ = 4,
+       AMP_K_CHEB0 = 5 /* first Chebyshev sweep */, AMP_K_CHEBSTEP = 6 /* further sweeps */, AMP_K_COUNT = 7 };
 typedef struct {
-  int32_t kernel;          /* AMP_K_*: step a2, a3, a4, a5 of SURVEY.md section 8(a) (XRZ: a5 + a2 of the lagged variant) */
+  int32_t kernel;          /* AMP_K_*: step a2, a3, a4, a5 of SURVEY.md section 8(a) (XRZ: a5 + a2 of the lagged variant;
+                              with AMP_PRECOND_CHEBJACOBI step a2 is CHEB0 + (s-1) x (SPMV + CHEBSTEP), all mat-vecs under SPMV) */
   int32_t uz, ur;          /* precision phase (u_z, u_r) of the iterations summed here */
   int32_t launches;        /* launches of this kernel in this phase */
   double total_ms;         /* sum over those launches of (event after - event before) on the solve stream */
@@ -254,7 +273,8 @@ int32_t amp_pcg_kernel_times(amp_pcg_t *h, amp_kernel_time_t *out_host, int32_t 
  * Work vectors: which = AMP_VEC_*; prec = storage precision of the copy addressed (r, q: FP64/FP32; z, p:
  * FP64/FP32/FP16; 1/diag: FP64/FP32).  src/dst are DEVICE arrays of n elements of that storage type; the library's
  * zero padding to a multiple of 8 is kept. */
-enum { AMP_VEC_R = 0, AMP_VEC_Q = 1, AMP_VEC_Z = 2, AMP_VEC_P = 3, AMP_VEC_DINV = 4 /* get only */ };
+enum { AMP_VEC_R = 0, AMP_VEC_Q = 1, AMP_VEC_Z = 2, AMP_VEC_P = 3, AMP_VEC_DINV = 4 /* get only */,
+       AMP_VEC_D = 5 /* Chebyshev direction d (AMP_PRECOND_CHEBJACOBI handles only), stored like z */ };
 int amp_pcg_debug_set_vector(amp_pcg_t *h, int which, int prec, const void *src);
 int amp_pcg_debug_get_vector(amp_pcg_t *h, int which, int prec, void *dst);
 enum {
@@ -262,14 +282,19 @@ enum {
   AMP_STEP_P = 1,    /* a3 (+a6): p = RN_uz(fma(beta, RN_uz(p), z)); first != 0: p = z                      (line 10) */
   AMP_STEP_SPMV = 2, /* a4: q = A p in u_r, gamma = q^T p                                                   (lines 11-13) */
   AMP_STEP_XR = 3,   /* a5: x += alpha p (FP64), r = RN_ur(fma(-alpha, q, r)), delta = ||r||               (lines 15-17) */
-  AMP_STEP_XRZ = 4   /* lagged a5 + a2: x, r = RN_ur_n(..), z = RN_uz_n((r omega_n) dinv), ||r|| and r^T z */
+  AMP_STEP_XRZ = 4,  /* lagged a5 + a2: x, r = RN_ur_n(..), z = RN_uz_n((r omega_n) dinv), ||r|| and r^T z */
+  /* AMP_PRECOND_CHEBJACOBI handles only: */
+  AMP_STEP_CHEB0 = 5,    /* d = z = RN_uz(((r omega) dinv) / theta) (+a6 as AMP_STEP_Z); rho = r^T z if s = 1 */
+  AMP_STEP_SPMV_Z = 6,   /* q = A z in u_r (the mat-vec inside M^-1; no reduction) */
+  AMP_STEP_CHEBSTEP = 7  /* sweep i = `first` (1 <= i < s): d = RN_uz(fma(c1_i, d, c2_i ((r omega - q) dinv))), z = RN_uz(z + d);
+                            rho = r^T z if i = s - 1 */
 };
 typedef struct {
   int32_t step;            /* AMP_STEP_* */
   int32_t rs, ur, uz;      /* precision r is stored in on entry; u_r and u_z of this iteration */
   int32_t ps;              /* precision p is stored in on entry (AMP_STEP_P) */
   int32_t ur_n, uz_n;      /* precisions of the next iteration (AMP_STEP_XRZ) */
-  int32_t first;           /* AMP_STEP_P: iteration k = 0 (p_{-1} is not read) */
+  int32_t first;           /* AMP_STEP_P: iteration k = 0 (p_{-1} is not read); AMP_STEP_CHEBSTEP: sweep index i */
   double omega, beta, alpha, omega_n; /* scalars the step reads */
   double sum0, sum1;       /* out: the step's scalar(s) after its grid reduction: Z: rho = r^T z | SPMV: gamma = q^T p |
                               XR: delta = ||r||_2 | XRZ: delta = ||r||_2 and sum1 = r^T z */

@@ -20,11 +20,11 @@ from .binding import (  # noqa: F401
     ETA_DELAY, ETA_LINEAR, ETA_NEVER,
     SCALE_NORM2, SCALE_RMS, SCALE_POW2, SCALE_NONE, SCALE_LAGGED,
     LOOP_AUTO, LOOP_STREAM, LOOP_GRAPH, LOOP_PERSISTENT,
-    PRECOND_NONE, PRECOND_JACOBI,
+    PRECOND_NONE, PRECOND_JACOBI, PRECOND_CHEBJACOBI,
     INDEX_AUTO, INDEX_NO_ALIGN, INDEX_FORCE32,
     SPMV_AUTO, SPMV_DIRECT, SPMV_PIPELINED,
-    K_Z, K_P, K_SPMV, K_XR, K_XRZ, KERNEL_NAMES,
-    VEC_R, VEC_Q, VEC_Z, VEC_P, VEC_DINV,
-    STEP_Z, STEP_P, STEP_SPMV, STEP_XR, STEP_XRZ,
+    K_Z, K_P, K_SPMV, K_XR, K_XRZ, K_CHEB0, K_CHEBSTEP, KERNEL_NAMES,
+    VEC_R, VEC_Q, VEC_Z, VEC_P, VEC_DINV, VEC_D,
+    STEP_Z, STEP_P, STEP_SPMV, STEP_XR, STEP_XRZ, STEP_CHEB0, STEP_SPMV_Z, STEP_CHEBSTEP,
     EXPORTED_SYMBOLS,
 )

@@ -16,13 +16,14 @@ FP64, FP32, FP16 = 0, 1, 2
 ETA_DELAY, ETA_LINEAR, ETA_NEVER = 0, 1, 2
 SCALE_NORM2, SCALE_RMS, SCALE_POW2, SCALE_NONE, SCALE_LAGGED = 0, 1, 2, 3, 4
 LOOP_AUTO, LOOP_STREAM, LOOP_GRAPH, LOOP_PERSISTENT = 0, 1, 2, 3
-PRECOND_NONE, PRECOND_JACOBI = 0, 1
+PRECOND_NONE, PRECOND_JACOBI, PRECOND_CHEBJACOBI = 0, 1, 2
 INDEX_AUTO, INDEX_NO_ALIGN, INDEX_FORCE32 = 0, 1, 2
 SPMV_AUTO, SPMV_DIRECT, SPMV_PIPELINED = 0, 1, 2
-K_Z, K_P, K_SPMV, K_XR, K_XRZ = 0, 1, 2, 3, 4
-KERNEL_NAMES = {K_Z: "k_z", K_P: "k_p", K_SPMV: "k_spmv", K_XR: "k_xr", K_XRZ: "k_xrz"}
-VEC_R, VEC_Q, VEC_Z, VEC_P, VEC_DINV = 0, 1, 2, 3, 4
-STEP_Z, STEP_P, STEP_SPMV, STEP_XR, STEP_XRZ = 0, 1, 2, 3, 4
+K_Z, K_P, K_SPMV, K_XR, K_XRZ, K_CHEB0, K_CHEBSTEP = 0, 1, 2, 3, 4, 5, 6
+KERNEL_NAMES = {K_Z: "k_z", K_P: "k_p", K_SPMV: "k_spmv", K_XR: "k_xr", K_XRZ: "k_xrz", K_CHEB0: "k_cheb0",
+                K_CHEBSTEP: "k_cheb_step"}
+VEC_R, VEC_Q, VEC_Z, VEC_P, VEC_DINV, VEC_D = 0, 1, 2, 3, 4, 5
+STEP_Z, STEP_P, STEP_SPMV, STEP_XR, STEP_XRZ, STEP_CHEB0, STEP_SPMV_Z, STEP_CHEBSTEP = 0, 1, 2, 3, 4, 5, 6, 7
 
 EXPORTED_SYMBOLS = (
     "amp_policy_default", "amp_create_opts_default", "amp_pcg_create", "amp_pcg_create_ex", "amp_pcg_solve",
@@ -67,7 +68,8 @@ class CreateOpts(C.Structure):
 
     _fields_ = [
         ("struct_bytes", C.c_int32), ("precond", C.c_int32), ("index_format", C.c_int32), ("spmv_kernel", C.c_int32),
-        ("spmv_grid_mult", C.c_int32), ("pdl", C.c_int32), ("stream", C.c_void_p),
+        ("spmv_grid_mult", C.c_int32), ("pdl", C.c_int32), ("cheb_degree", C.c_int32), ("reserved0", C.c_int32),
+        ("cheb_lmin", C.c_double), ("cheb_lmax", C.c_double), ("stream", C.c_void_p),
     ]
 
     @classmethod

@@ -72,7 +72,10 @@ struct amp_pcg {
   int use_pipe = 0;           // the loop's SpMV is the bulk-copy pipelined kernel (spmv_pipe.cuh)
   int pipe_grid = 0;
   int64_t pipe_chunks = 0;
-  int64_t guard = 0;          // zero guard band (elements) on both sides of the p vectors
+  int64_t guard = 0;          // zero guard band (elements) on both sides of the p (and z) vectors
+  int cheb_s = 0;             // sweeps of the Chebyshev-Jacobi preconditioner (0: not in use)
+  double cheb_lmin = 0.0, cheb_lmax = 0.0;
+  int grid_cheb0 = 1, grid_cheb_step = 1;
   // per-kernel event profile of the last solve (policy.profile_kernels, stream loop)
   std::vector<cudaEvent_t> prof_events;  // pool, grown on demand
   size_t prof_used = 0;
@@ -134,8 +137,14 @@ static double loop_spmv_bytes(const amp_pcg_t* h, int uz, int ur) {
 extern "C" double amp_pcg_iteration_bytes(const amp_pcg_t* h, int uz, int ur) {
   if (!h) return 0.0;
   const double sr = (ur == AMP_FP64) ? 8.0 : 4.0, sz = vec_size(uz), sd = (uz == AMP_FP64) ? 8.0 : 4.0;
-  const double k_z = sr + sd + sz, k_p = 3.0 * sz + (shadow_phase(uz, ur) ? 4.0 : 0.0), k_xr = 16.0 + sz + 3.0 * sr;
-  return loop_spmv_bytes(h, uz, ur) + (double)h->n * (k_z + k_p + k_xr);
+  double k_z = sr + sd + sz;
+  const double k_p = 3.0 * sz + (shadow_phase(uz, ur) ? 4.0 : 0.0), k_xr = 16.0 + sz + 3.0 * sr;
+  double spmv = loop_spmv_bytes(h, uz, ur);
+  if (h->cheb_s > 0) {  // first sweep: r, 1/diag -> d, z; each further sweep: a mat-vec (z -> w) and r, w, 1/diag, d, z -> d, z
+    k_z = (sr + sd + 2.0 * sz) + (double)(h->cheb_s - 1) * (2.0 * sr + sd + 4.0 * sz);
+    spmv += (double)(h->cheb_s - 1) * amp_pcg_spmv_bytes(h, ur, uz);
+  }
+  return spmv + (double)h->n * (k_z + k_p + k_xr);
 }
 
 extern "C" void amp_pcg_destroy(amp_pcg_t* h) {
@@ -167,6 +176,9 @@ extern "C" void amp_create_opts_default(amp_create_opts_t* o) {
   o->spmv_kernel = AMP_SPMV_AUTO;
   o->spmv_grid_mult = 0;
   o->pdl = 1;
+  o->cheb_degree = 2;
+  o->cheb_lmin = 0.0;
+  o->cheb_lmax = 0.0;
   o->stream = nullptr;
 }
 
@@ -201,8 +213,14 @@ extern "C" amp_pcg_t* amp_pcg_create_ex(int64_t n, int64_t nnz, const int32_t* r
     set_error("amp_pcg_create: n and nnz must satisfy 0 < n, 0 <= nnz < 2^31 (got n=%lld nnz=%lld)", (long long)n, (long long)nnz);
     return nullptr;
   }
-  if (!rowptr || (nnz > 0 && (!colidx || !vals)) || (precond != AMP_PRECOND_NONE && precond != AMP_PRECOND_JACOBI)) {
+  if (!rowptr || (nnz > 0 && (!colidx || !vals)) || precond < AMP_PRECOND_NONE || precond > AMP_PRECOND_CHEBJACOBI) {
     set_error("amp_pcg_create: null pointer or unknown preconditioner %d", precond);
+    return nullptr;
+  }
+  if (precond == AMP_PRECOND_CHEBJACOBI &&
+      (o.cheb_degree < 1 || o.cheb_degree > kMaxChebDegree || !(o.cheb_lmax >= 0.0) || !(o.cheb_lmin >= 0.0) ||
+       (o.cheb_lmax > 0.0 && !(o.cheb_lmin > 0.0 && o.cheb_lmin < o.cheb_lmax)))) {
+    set_error("amp_pcg_create_ex: Chebyshev-Jacobi needs 1 <= cheb_degree <= %d and 0 < cheb_lmin < cheb_lmax (or both 0)", kMaxChebDegree);
     return nullptr;
   }
   if (!aligned16(rowptr) || !aligned16(colidx) || !aligned16(vals)) {
@@ -238,7 +256,6 @@ extern "C" amp_pcg_t* amp_pcg_create_ex(int64_t n, int64_t nnz, const int32_t* r
   ALLOC(dinv64, double, np); ALLOC(dinv32, float, np);
   ALLOC(c.r64, double, np); ALLOC(c.r32, float, np);
   ALLOC(c.q64, double, np); ALLOC(c.q32, float, np);
-  ALLOC(c.z64, double, np); ALLOC(c.z32, float, np); ALLOC(c.z16, __half, np);
   ALLOC(c.partials, double, (size_t)4 * kMaxGrid);
   ALLOC(c.st, DevState, 1);
   ALLOC(flags, int, 1);
@@ -252,7 +269,7 @@ extern "C" amp_pcg_t* amp_pcg_create_ex(int64_t n, int64_t nnz, const int32_t* r
 
   // structure check + 1/diag, FP32 value copy
   const int vgrid = (int)std::min<int64_t>((n + 255) / 256, (int64_t)h->num_sms * 16);
-  k_validate_dinv<<<vgrid, 256, 0, h->stream>>>(n, nnz, rowptr, colidx, vals, precond == AMP_PRECOND_JACOBI, dinv64,
+  k_validate_dinv<<<vgrid, 256, 0, h->stream>>>(n, nnz, rowptr, colidx, vals, precond != AMP_PRECOND_NONE, dinv64,
                                                 dinv32, flags);
   std::vector<int32_t> rp((size_t)n + 1);
   int hflags = 0;
@@ -463,11 +480,44 @@ extern "C" amp_pcg_t* amp_pcg_create_ex(int64_t n, int64_t nnz, const int32_t* r
         h->idx_bytes_total += 8.0 * (double)(nch + 1) + 4.0 * (double)(nb + 1);  // stage descriptors
       }
     }
-    {  // p in its three storage precisions, with the zero guard band on both sides (0 elements unless pipelined)
+    {  // p and z (both are gathered by a mat-vec: z inside the Chebyshev-Jacobi preconditioner) in their three storage
+       // precisions, with the zero guard band on both sides (0 elements unless pipelined)
       const size_t g = (size_t)h->guard;
       double* b64; float* b32; __half* b16;
       ALLOC(b64, double, np + 2 * g); ALLOC(b32, float, np + 2 * g); ALLOC(b16, __half, np + 2 * g);
       c.p64 = b64 + g; c.p32 = b32 + g; c.p16 = b16 + g;
+      ALLOC(b64, double, np + 2 * g); ALLOC(b32, float, np + 2 * g); ALLOC(b16, __half, np + 2 * g);
+      c.z64 = b64 + g; c.z32 = b32 + g; c.z16 = b16 + g;
+    }
+    if (precond == AMP_PRECOND_CHEBJACOBI) {  // direction vector d, spectrum bounds, recurrence coefficients
+      ALLOC(c.d64, double, np); ALLOC(c.d32, float, np); ALLOC(c.d16, __half, np);
+      double lmin = o.cheb_lmin, lmax = o.cheb_lmax;
+      if (!(lmax > 0.0)) {  // Gershgorin bound of D^-1 A (row sums in CSR order: the same number the oracle computes)
+        unsigned long long* gmax_d;
+        ALLOC(gmax_d, unsigned long long, 1);
+        k_gershgorin<<<vgrid, 256, 0, h->stream>>>(n, rowptr, colidx, vals, gmax_d);
+        unsigned long long bits = 0;
+        CU_TRY(cudaMemcpyAsync(&bits, gmax_d, sizeof(bits), cudaMemcpyDeviceToHost, h->stream), { amp_pcg_destroy(h); return nullptr; });
+        CU_TRY(cudaStreamSynchronize(h->stream), { amp_pcg_destroy(h); return nullptr; });
+        std::memcpy(&lmax, &bits, sizeof(double));
+        lmin = lmax / 30.0;
+      }
+      if (!(lmin > 0.0) || !(lmax > lmin) || std::isinf(lmax)) {
+        set_error("amp_pcg_create_ex: Chebyshev-Jacobi spectrum bounds are not usable (lmin %g, lmax %g)", lmin, lmax);
+        amp_pcg_destroy(h);
+        return nullptr;
+      }
+      h->cheb_s = o.cheb_degree; h->cheb_lmin = lmin; h->cheb_lmax = lmax;
+      const double theta = (lmax + lmin) / 2.0, dc = (lmax - lmin) / 2.0, sigma = theta / dc;
+      c.cheb_s = o.cheb_degree;
+      c.cheb_inv_theta = 1.0 / theta;
+      double rho_prev = 1.0 / sigma;
+      for (int i = 1; i < o.cheb_degree; ++i) {
+        const double rho = 1.0 / (2.0 * sigma - rho_prev);
+        c.cheb_c1[i] = rho * rho_prev;
+        c.cheb_c2[i] = 2.0 * rho / dc;
+        rho_prev = rho;
+      }
     }
 
     // SpMV grid: a warp takes a group of up to kSpmvGroupMax slices per pass; blocks make a whole number of
@@ -499,6 +549,8 @@ extern "C" amp_pcg_t* amp_pcg_create_ex(int64_t n, int64_t nnz, const int32_t* r
   h->grid_p = vec_grid_for((const void*)k_p);
   h->grid_xr = vec_grid_for((const void*)k_xr);
   h->grid_xrz = vec_grid_for((const void*)k_xrz);
+  h->grid_cheb0 = vec_grid_for((const void*)k_cheb0);
+  h->grid_cheb_step = vec_grid_for((const void*)k_cheb_step);
   h->vec_grid = vec_grid_for((const void*)k_setup);
 #undef ALLOC
   return h;
@@ -549,8 +601,8 @@ extern "C" int amp_spmv(amp_pcg_t* h, int mat_prec, int vec_prec, const void* p,
 }
 
 // ------------------------------------------------------------------ graph loop --------------
-template <class K>
-static cudaError_t launch_loop_kernel(K kern, int grid, int threads, cudaStream_t s, const Ctx& c, bool pdl, size_t smem = 0) {
+template <class K, class... Args>
+static cudaError_t launch_loop_kernel_ex(K kern, int grid, int threads, cudaStream_t s, bool pdl, size_t smem, Args... args) {
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = dim3((unsigned)grid);
   cfg.blockDim = dim3((unsigned)threads);
@@ -561,13 +613,20 @@ static cudaError_t launch_loop_kernel(K kern, int grid, int threads, cudaStream_
   attr[0].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = attr;
   cfg.numAttrs = pdl ? 1 : 0;
-  return cudaLaunchKernelEx(&cfg, kern, c);
+  return cudaLaunchKernelEx(&cfg, kern, args...);
+}
+template <class K>
+static cudaError_t launch_loop_kernel(K kern, int grid, int threads, cudaStream_t s, const Ctx& c, bool pdl) {
+  return launch_loop_kernel_ex(kern, grid, threads, s, pdl, 0, c);
 }
 
-// step a4 inside the loop: the bulk-copy pipelined kernel when the matrix is eligible, else the direct kernel
-static cudaError_t launch_spmv_loop(amp_pcg* h, cudaStream_t s, const Ctx& c, bool pdl) {
-  cudaError_t e = launch_loop_kernel(k_spmv, h->spmv_grid, kSpmvThreads, s, c, pdl);
-  if (e == cudaSuccess && h->use_pipe) e = launch_loop_kernel(k_spmv_pipe, h->pipe_grid, kPipeThreads, s, c, pdl, (size_t)kPipeSmemBytes);
+// step a4 inside the loop (zmode = 0), or the mat-vec q = A z inside the Chebyshev-Jacobi preconditioner (zmode = 1):
+// the direct kernel, followed by the bulk-copy pipelined kernel when the matrix is eligible (it takes the u_r = FP32
+// phases; whichever kernel's phase it is not returns at once)
+static cudaError_t launch_spmv_loop(amp_pcg* h, cudaStream_t s, const Ctx& c, bool pdl, int zmode = 0) {
+  cudaError_t e = launch_loop_kernel_ex(k_spmv, h->spmv_grid, kSpmvThreads, s, pdl, 0, c, zmode);
+  if (e == cudaSuccess && h->use_pipe)
+    e = launch_loop_kernel_ex(k_spmv_pipe, h->pipe_grid, kPipeThreads, s, pdl, (size_t)kPipeSmemBytes, c, zmode);
   return e;
 }
 
@@ -590,8 +649,19 @@ static cudaError_t launch_iteration(amp_pcg* h, const Ctx& c, cudaStream_t s, bo
   const bool prof = prof_iter >= 0;
   if (prof) pdl = false;
   cudaError_t e = cudaSuccess;
-  if (prof) e = prof_mark(h, s, AMP_K_Z, prof_iter);
-  if (e == cudaSuccess) e = launch_loop_kernel(k_z, h->grid_z, kVecThreads, s, c, false);
+  if (h->cheb_s > 0) {  // step a2 with M^-1 = Chebyshev-accelerated Jacobi: first sweep, then (mat-vec, sweep) s - 1 times
+    if (prof) e = prof_mark(h, s, AMP_K_CHEB0, prof_iter);
+    if (e == cudaSuccess) e = launch_loop_kernel(k_cheb0, h->grid_cheb0, kVecThreads, s, c, false);
+    for (int i = 1; i < h->cheb_s && e == cudaSuccess; ++i) {
+      if (prof) e = prof_mark(h, s, AMP_K_SPMV, prof_iter);
+      if (e == cudaSuccess) e = launch_spmv_loop(h, s, c, pdl, 1);
+      if (prof && e == cudaSuccess) e = prof_mark(h, s, AMP_K_CHEBSTEP, prof_iter);
+      if (e == cudaSuccess) e = launch_loop_kernel_ex(k_cheb_step, h->grid_cheb_step, kVecThreads, s, pdl, 0, c, i);
+    }
+  } else {
+    if (prof) e = prof_mark(h, s, AMP_K_Z, prof_iter);
+    if (e == cudaSuccess) e = launch_loop_kernel(k_z, h->grid_z, kVecThreads, s, c, false);
+  }
   if (prof && e == cudaSuccess) e = prof_mark(h, s, AMP_K_P, prof_iter);
   if (e == cudaSuccess) e = launch_loop_kernel(k_p, h->grid_p, kVecThreads, s, c, pdl);
   if (prof && e == cudaSuccess) e = prof_mark(h, s, AMP_K_SPMV, prof_iter);
@@ -697,7 +767,12 @@ static int solve_impl(amp_pcg* h, const double* b, double* x, double tol, int32_
   // 512 K 25.0 vs 32.1, 2.1 M (c2) 58 vs 57, 4.1 M (c3) 95 vs 92: the persistent kernel wins while the iteration is
   // latency-bound; from c2 up the graph loop wins because each of its kernels has its own register budget
   const bool lagged = pol.amp && pol.scale_mode == AMP_SCALE_LAGGED;
-  if (mode == AMP_LOOP_AUTO) mode = (h->persist_ok && h->n <= kPersistAutoMaxRows) ? AMP_LOOP_PERSISTENT : AMP_LOOP_GRAPH;
+  if (h->cheb_s > 0 && (lagged || mode == AMP_LOOP_PERSISTENT)) {
+    set_error("amp_pcg_solve: the Chebyshev-Jacobi preconditioner is not available with AMP_SCALE_LAGGED or AMP_LOOP_PERSISTENT");
+    return AMP_ERR_INVALID;
+  }
+  if (mode == AMP_LOOP_AUTO)
+    mode = (h->persist_ok && h->n <= kPersistAutoMaxRows && h->cheb_s == 0) ? AMP_LOOP_PERSISTENT : AMP_LOOP_GRAPH;
   if (mode == AMP_LOOP_PERSISTENT && !h->persist_ok) {
     set_error("amp_pcg_solve: persistent loop not available for this problem/device");
     return AMP_ERR_INVALID;
@@ -800,14 +875,20 @@ static int solve_impl(amp_pcg* h, const double* b, double* x, double tol, int32_
           switch (kern) {
             case AMP_K_Z: a.bytes_per_launch = n_ * (sr + sd + sz); break;
             case AMP_K_P: a.bytes_per_launch = n_ * (3.0 * sz + (shadow_phase(uz, ur) ? 4.0 : 0.0)); break;
-            case AMP_K_SPMV: a.bytes_per_launch = loop_spmv_bytes(h, uz, ur); break;
+            case AMP_K_SPMV: a.bytes_per_launch = loop_spmv_bytes(h, uz, ur); break;  // (z-mode launches: within 4 B per row of it)
+            case AMP_K_CHEB0: a.bytes_per_launch = n_ * (sr + sd + 2.0 * sz); break;
+            case AMP_K_CHEBSTEP: a.bytes_per_launch = n_ * (2.0 * sr + sd + 4.0 * sz); break;
             case AMP_K_XR: a.bytes_per_launch = n_ * (16.0 + sz + 3.0 * sr); break;
             default: a.bytes_per_launch = n_ * (16.0 + sz + 3.0 * sr + sd + sz); break;  // AMP_K_XRZ
           }
           h->prof_result.push_back(a);
         }
   }
-  h->launches += (mode == AMP_LOOP_PERSISTENT) ? 1 : (int64_t)((lagged ? 3 : 4) + (h->use_pipe ? 1 : 0)) * iters;
+  {
+    const int spmv_k = h->use_pipe ? 2 : 1, sweeps = std::max(h->cheb_s, 1);
+    const int per_it = (lagged ? 2 : 3) + spmv_k + (sweeps - 1) * (spmv_k + 1);  // vector kernels + a4 + extra sweeps
+    h->launches += (mode == AMP_LOOP_PERSISTENT) ? 1 : (int64_t)per_it * iters;
+  }
   if (stats) {
     std::memset(stats, 0, sizeof(*stats));
     stats->status = hs->status; stats->iters = iters;
@@ -904,6 +985,7 @@ static bool debug_vec(amp_pcg* h, int which, int prec, void** ptr, size_t* elem)
     case AMP_VEC_Z: *ptr = prec == AMP_FP64 ? (void*)c.z64 : prec == AMP_FP32 ? (void*)c.z32 : prec == AMP_FP16 ? (void*)c.z16 : nullptr; break;
     case AMP_VEC_P: *ptr = prec == AMP_FP64 ? (void*)c.p64 : prec == AMP_FP32 ? (void*)c.p32 : prec == AMP_FP16 ? (void*)c.p16 : nullptr; break;
     case AMP_VEC_DINV: *ptr = prec == AMP_FP64 ? (void*)c.dinv64 : prec == AMP_FP32 ? (void*)c.dinv32 : nullptr; break;
+    case AMP_VEC_D: *ptr = prec == AMP_FP64 ? (void*)c.d64 : prec == AMP_FP32 ? (void*)c.d32 : prec == AMP_FP16 ? (void*)c.d16 : nullptr; break;
     default: break;
   }
   return *ptr != nullptr;
@@ -941,10 +1023,12 @@ extern "C" int amp_pcg_debug_get_vector(amp_pcg_t* h, int which, int prec, void*
 extern "C" int amp_pcg_debug_step(amp_pcg_t* h, amp_debug_step_t* io, double* x) {
   g_last_error.clear();
   auto prec_ok = [](int p, int lo) { return p >= 0 && p <= lo; };
-  if (!h || !io || io->step < AMP_STEP_Z || io->step > AMP_STEP_XRZ || !prec_ok(io->rs, 1) || !prec_ok(io->ur, 1) ||
+  if (!h || !io || io->step < AMP_STEP_Z || io->step > AMP_STEP_CHEBSTEP || !prec_ok(io->rs, 1) || !prec_ok(io->ur, 1) ||
       !prec_ok(io->uz, 2) || !prec_ok(io->ps, 2) || !prec_ok(io->ur_n, 1) || !prec_ok(io->uz_n, 2) || io->rs > io->ur ||
       io->ps > io->uz || io->ur > io->ur_n || io->uz > io->uz_n ||
-      ((io->step == AMP_STEP_XR || io->step == AMP_STEP_XRZ) && (!x || !aligned16(x)))) {
+      ((io->step == AMP_STEP_XR || io->step == AMP_STEP_XRZ) && (!x || !aligned16(x))) ||
+      (io->step >= AMP_STEP_CHEB0 && h->cheb_s == 0) ||
+      (io->step == AMP_STEP_CHEBSTEP && (io->first < 1 || io->first >= h->cheb_s))) {
     set_error("amp_pcg_debug_step: invalid step / precision combination (precisions only step down) or x missing");
     return AMP_ERR_INVALID;
   }
@@ -964,7 +1048,7 @@ extern "C" int amp_pcg_debug_step(amp_pcg_t* h, amp_debug_step_t* io, double* x)
   hs->amp = 0; hs->eta_rule = AMP_ETA_NEVER; hs->d = 10; hs->ell = 5; hs->no_stop = 1; hs->maxit = 1 << 20;
   hs->bnorm = 1.0; hs->rho = 1.0; hs->rho_prev = 1.0;
   hs->status = AMP_MAXIT; hs->it_ur32 = hs->it_uz32 = hs->it_uz16 = -1;
-  hs->k = io->first ? 0 : 1;
+  hs->k = (io->first && io->step == AMP_STEP_P) ? 0 : 1;
   hs->r_store = io->rs; hs->ur = io->ur; hs->uz = io->uz; hs->p_store = io->ps;
   hs->ur_n = io->ur_n; hs->uz_n = io->uz_n;
   hs->omega = io->omega; hs->beta = io->beta; hs->alpha = io->alpha; hs->omega_n = io->omega_n;
@@ -975,7 +1059,10 @@ extern "C" int amp_pcg_debug_step(amp_pcg_t* h, amp_debug_step_t* io, double* x)
     case AMP_STEP_P: e = launch_loop_kernel(k_p, h->grid_p, kVecThreads, st, h->ctx, false); break;
     case AMP_STEP_SPMV: e = launch_spmv_loop(h, st, h->ctx, false); break;
     case AMP_STEP_XR: e = launch_loop_kernel(k_xr, h->grid_xr, kVecThreads, st, h->ctx, false); break;
-    default: e = launch_loop_kernel(k_xrz, h->grid_xrz, kVecThreads, st, h->ctx, false); break;
+    case AMP_STEP_XRZ: e = launch_loop_kernel(k_xrz, h->grid_xrz, kVecThreads, st, h->ctx, false); break;
+    case AMP_STEP_CHEB0: e = launch_loop_kernel(k_cheb0, h->grid_cheb0, kVecThreads, st, h->ctx, false); break;
+    case AMP_STEP_SPMV_Z: e = launch_spmv_loop(h, st, h->ctx, false, 1); break;
+    default: e = launch_loop_kernel_ex(k_cheb_step, h->grid_cheb_step, kVecThreads, st, false, 0, h->ctx, (int)io->first); break;
   }
   if (e != cudaSuccess) { set_error("amp_pcg_debug_step: launch failed: %s", cudaGetErrorString(e)); cudaGetLastError(); return AMP_ERR_CUDA; }
   CU_TRY(cudaMemcpyAsync(hs, h->ctx.st, sizeof(DevState), cudaMemcpyDeviceToHost, st), return AMP_ERR_CUDA);
@@ -983,7 +1070,7 @@ extern "C" int amp_pcg_debug_step(amp_pcg_t* h, amp_debug_step_t* io, double* x)
   CU_TRY(cudaGetLastError(), return AMP_ERR_CUDA);
   io->sum0 = io->sum1 = 0.0;
   switch (io->step) {
-    case AMP_STEP_Z: io->sum0 = hs->rho; break;
+    case AMP_STEP_Z: case AMP_STEP_CHEB0: case AMP_STEP_CHEBSTEP: io->sum0 = hs->rho; break;
     case AMP_STEP_SPMV: io->sum0 = hs->gamma; break;
     case AMP_STEP_XR: io->sum0 = hs->delta; break;
     case AMP_STEP_XRZ: io->sum0 = hs->delta; io->sum1 = hs->rho; break;

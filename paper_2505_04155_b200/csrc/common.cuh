@@ -23,6 +23,7 @@ constexpr int kPersistAutoMaxRows = 1 << 20;   // AMP_LOOP_AUTO takes the persis
 constexpr int kPersistMinBlocks = 1;           // resident blocks per SM its register budget is set for
 constexpr int kMaxGrid = 8192;                 // capacity of each partial-sum array
 constexpr int kMaxWindow = 64;                 // max d / ell of the indicators
+constexpr int kMaxChebDegree = 16;             // max sweeps of the Chebyshev-Jacobi preconditioner
 
 // Scalars of one solve, resident in device memory.  The host writes the policy part before the
 // loop and reads the whole block once after it; inside the loop only kernels touch it.
@@ -65,6 +66,7 @@ struct Ctx {
   double* q64; float* q32;
   double* z64; float* z32; __half* z16;
   double* p64; float* p32; __half* p16;
+  double* d64; float* d32; __half* d16;   // Chebyshev direction d (AMP_PRECOND_CHEBJACOBI only), stored like z
   double* partials;       // [4][kMaxGrid] per-block partial sums
   // SELL-32 repack of A (spmv.cuh), owned by the handle
   const int32_t* sell_wptr;   // [nslices+1] cumulative slice widths; slice s starts at element 32*sell_wptr[s]
@@ -82,6 +84,10 @@ struct Ctx {
   const int32_t* pipe_chunks;     // [nchunks+1] x {first slice, first entry column} of every stage
   const int32_t* pipe_blk_chunk;  // [pipe_grid+1] stage range of every block
   int32_t use_pipe;               // 1: iterations with u_r = FP32 run k_spmv_pipe, those with u_r = FP64 the direct k_spmv
+  // Chebyshev-accelerated Jacobi (cheb_s = 0: not in use): sweeps, 1/theta, c1_i = rho_i rho_{i-1}, c2_i = 2 rho_i / dc
+  int32_t cheb_s;
+  double cheb_inv_theta;
+  double cheb_c1[kMaxChebDegree], cheb_c2[kMaxChebDegree];
   cudaGraphConditionalHandle cond;  // WHILE-node handle (graph loop only)
   int32_t use_cond;
 };
@@ -109,6 +115,10 @@ template <int P> __device__ __forceinline__ typename Store<P>::T* zvec(const Ctx
 template <> __device__ __forceinline__ double* zvec<P64>(const Ctx& c) { return c.z64; }
 template <> __device__ __forceinline__ float* zvec<P32>(const Ctx& c) { return c.z32; }
 template <> __device__ __forceinline__ __half* zvec<P16>(const Ctx& c) { return c.z16; }
+template <int P> __device__ __forceinline__ typename Store<P>::T* dvec(const Ctx& c);
+template <> __device__ __forceinline__ double* dvec<P64>(const Ctx& c) { return c.d64; }
+template <> __device__ __forceinline__ float* dvec<P32>(const Ctx& c) { return c.d32; }
+template <> __device__ __forceinline__ __half* dvec<P16>(const Ctx& c) { return c.d16; }
 template <int P> __device__ __forceinline__ typename Store<P>::T* pvec(const Ctx& c);
 template <> __device__ __forceinline__ double* pvec<P64>(const Ctx& c) { return c.p64; }
 template <> __device__ __forceinline__ float* pvec<P32>(const Ctx& c) { return c.p32; }

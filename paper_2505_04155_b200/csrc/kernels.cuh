@@ -53,8 +53,20 @@ __device__ __forceinline__ void dispatch_p(const Ctx& c, int ps, int uz, int ur,
   }
 }
 
+// zmode = 0: q = A p (step a4).  zmode = 1: q = A z, the mat-vec inside the Chebyshev-Jacobi preconditioner (the q
+// buffers are free between two a4 steps); the returned sum is then not used.
 template <bool COH, int NT>
-__device__ __forceinline__ double dispatch_spmv(const Ctx& c, int ur, int uz, int bid, int nb, double* red) {
+__device__ __forceinline__ double dispatch_spmv(const Ctx& c, int ur, int uz, int zmode, int bid, int nb, double* red) {
+  if (zmode) {
+    if (ur == P64) {
+      if (uz == P64) return phase_spmv<P64, COH, NT>(c, c.z64, c.z64, c.q64, bid, nb, red);
+      if (uz == P32) return phase_spmv<P64, COH, NT>(c, c.z32, c.z32, c.q64, bid, nb, red);
+      return phase_spmv<P64, COH, NT>(c, c.z16, c.z16, c.q64, bid, nb, red);
+    }
+    if (uz == P64) return phase_spmv<P32, COH, NT>(c, c.z64, c.z64, c.q32, bid, nb, red);  // RN32(z_j) per gathered entry
+    if (uz == P32) return phase_spmv<P32, COH, NT>(c, c.z32, c.z32, c.q32, bid, nb, red);
+    return phase_spmv<P32, COH, NT>(c, c.z16, c.z16, c.q32, bid, nb, red);
+  }
   if (ur == P64) {
     if (uz == P64) return phase_spmv<P64, COH, NT>(c, c.p64, c.p64, c.q64, bid, nb, red);
     if (uz == P32) return phase_spmv<P64, COH, NT>(c, c.p32, c.p32, c.q64, bid, nb, red);
@@ -99,7 +111,7 @@ __global__ void __launch_bounds__(kVecThreads, AMP_KP_BLOCKS) k_p(const Ctx c) {
   dispatch_p(c, s->p_store, s->uz, s->ur, s->beta, s->k == 0, blockIdx.x, gridDim.x);
 }
 
-__global__ void __launch_bounds__(kSpmvThreads, kSpmvMinBlocks) k_spmv(const Ctx c) {
+__global__ void __launch_bounds__(kSpmvThreads, kSpmvMinBlocks) k_spmv(const Ctx c, int zmode) {
   __shared__ double red[32];
   DevState* s = c.st;
   pdl_launch_dependents();
@@ -107,7 +119,8 @@ __global__ void __launch_bounds__(kSpmvThreads, kSpmvMinBlocks) k_spmv(const Ctx
   if (s->done) return;
   if (c.use_pipe && s->ur == P32) return;  // this iteration's mat-vec is k_spmv_pipe's (next in the chain)
   const int bid = blockIdx.x, nb = gridDim.x;
-  const double v = dispatch_spmv<false, kSpmvThreads>(c, s->ur, s->uz, bid, nb, red);
+  const double v = dispatch_spmv<false, kSpmvThreads>(c, s->ur, s->uz, zmode, bid, nb, red);
+  if (zmode) return;  // q = A z inside M^-1: no inner product
   grid_reduce<kSpmvThreads>(v, c.partials + 1 * kMaxGrid, &s->counter[1], bid, nb, red,
                             [&](double tot) { epi_gamma(epi_ctx(c), tot); });
 }
@@ -125,6 +138,67 @@ __global__ void __launch_bounds__(kVecThreads, AMP_KXR_BLOCKS) k_xr(const Ctx c)
   const double v = dispatch_xr(c, s->ur, s->uz, s->alpha, s->x, bid, nb);
   grid_reduce<kVecThreads>(v, c.partials + 2 * kMaxGrid, &s->counter[2], bid, nb, red,
                            [&](double tot) { epi_delta(epi_ctx(c), tot); });
+}
+
+// ------------------------------------------------------------------ Chebyshev-Jacobi kernels --
+template <int BIF = kVecBytesInFlight>
+__device__ __forceinline__ double dispatch_cheb0(const Ctx& c, int rs, int ur, int uz, double omega, bool with_rho, int bid, int nb) {
+  if (rs == P64 && ur == P64) {
+    if (uz == P64) return phase_cheb0<P64, P64, P64, BIF>(c, omega, with_rho, bid, nb);
+    if (uz == P32) return phase_cheb0<P64, P64, P32, BIF>(c, omega, with_rho, bid, nb);
+    return phase_cheb0<P64, P64, P16, BIF>(c, omega, with_rho, bid, nb);
+  }
+  if (rs == P64 && ur == P32) {
+    if (uz == P64) return phase_cheb0<P64, P32, P64, BIF>(c, omega, with_rho, bid, nb);
+    if (uz == P32) return phase_cheb0<P64, P32, P32, BIF>(c, omega, with_rho, bid, nb);
+    return phase_cheb0<P64, P32, P16, BIF>(c, omega, with_rho, bid, nb);
+  }
+  if (uz == P64) return phase_cheb0<P32, P32, P64, BIF>(c, omega, with_rho, bid, nb);
+  if (uz == P32) return phase_cheb0<P32, P32, P32, BIF>(c, omega, with_rho, bid, nb);
+  return phase_cheb0<P32, P32, P16, BIF>(c, omega, with_rho, bid, nb);
+}
+
+template <int BIF = kVecBytesInFlight>
+__device__ __forceinline__ double dispatch_cheb_step(const Ctx& c, int ur, int uz, double omega, double c1, double c2, bool with_rho,
+                                                     int bid, int nb) {
+  if (ur == P64) {
+    if (uz == P64) return phase_cheb_step<P64, P64, BIF>(c, omega, c1, c2, with_rho, bid, nb);
+    if (uz == P32) return phase_cheb_step<P64, P32, BIF>(c, omega, c1, c2, with_rho, bid, nb);
+    return phase_cheb_step<P64, P16, BIF>(c, omega, c1, c2, with_rho, bid, nb);
+  }
+  if (uz == P64) return phase_cheb_step<P32, P64, BIF>(c, omega, c1, c2, with_rho, bid, nb);
+  if (uz == P32) return phase_cheb_step<P32, P32, BIF>(c, omega, c1, c2, with_rho, bid, nb);
+  return phase_cheb_step<P32, P16, BIF>(c, omega, c1, c2, with_rho, bid, nb);
+}
+
+// first sweep of M^-1 (takes k_z's place in the loop); the reduction and epi_rho only when it is also the last sweep
+__global__ void __launch_bounds__(kVecThreads, 2) k_cheb0(const Ctx c) {
+  __shared__ double red[32];
+  DevState* s = c.st;
+  pdl_launch_dependents();
+  pdl_wait();
+  if (s->done) return;
+  const int bid = blockIdx.x, nb = gridDim.x;
+  const bool last = c.cheb_s == 1;
+  const double v = dispatch_cheb0(c, s->r_store, s->ur, s->uz, s->omega, last, bid, nb);
+  if (last)
+    grid_reduce<kVecThreads>(v, c.partials + 0 * kMaxGrid, &s->counter[0], bid, nb, red,
+                             [&](double tot) { epi_rho(epi_ctx(c), tot); });
+}
+
+// sweep i (1 <= i < s) of M^-1, after the mat-vec w = A z (k_spmv in mode 1)
+__global__ void __launch_bounds__(kVecThreads, 2) k_cheb_step(const Ctx c, int i) {
+  __shared__ double red[32];
+  DevState* s = c.st;
+  pdl_launch_dependents();
+  pdl_wait();
+  if (s->done) return;
+  const int bid = blockIdx.x, nb = gridDim.x;
+  const bool last = i == c.cheb_s - 1;
+  const double v = dispatch_cheb_step(c, s->ur, s->uz, s->omega, c.cheb_c1[i], c.cheb_c2[i], last, bid, nb);
+  if (last)
+    grid_reduce<kVecThreads>(v, c.partials + 0 * kMaxGrid, &s->counter[0], bid, nb, red,
+                             [&](double tot) { epi_rho(epi_ctx(c), tot); });
 }
 
 // ------------------------------------------------------------------ lagged variant: k_xrz ----
@@ -276,6 +350,24 @@ __global__ void k_absmax_i32(int64_t n, const int32_t* __restrict__ a, int* __re
   m = max(m, __shfl_xor_sync(0xffffffffu, m, 4)); m = max(m, __shfl_xor_sync(0xffffffffu, m, 2));
   m = max(m, __shfl_xor_sync(0xffffffffu, m, 1));
   if ((threadIdx.x & 31) == 0 && m > 0) atomicMax(out, m);
+}
+
+// max_i (sum_j |a_ij|) / a_ii: Gershgorin bound of the spectrum of D^-1 A (row sums in CSR order, duplicates of the
+// diagonal add up); the maximum of positive doubles is the maximum of their bit patterns
+__global__ void k_gershgorin(int64_t n, const int32_t* __restrict__ rowptr, const int32_t* __restrict__ colidx,
+                             const double* __restrict__ vals, unsigned long long* __restrict__ out) {
+  const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+  double m = 0.0;
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
+    double d = 0.0, srow = 0.0;
+    for (int32_t e = rowptr[i]; e < rowptr[i + 1]; ++e) {
+      srow = __dadd_rn(srow, fabs(vals[e]));
+      if (colidx[e] == i) d = __dadd_rn(d, vals[e]);
+    }
+    const double g = __ddiv_rn(srow, d);
+    if (g > m) m = g;
+  }
+  if (m > 0.0) atomicMax(out, (unsigned long long)__double_as_longlong(m));
 }
 
 __global__ void k_to_fp32(int64_t n, const double* __restrict__ a, float* __restrict__ o) {

@@ -85,7 +85,7 @@ __device__ __noinline__ void pp(const Ctx& c, int ps, int uz, int ur, double bet
   dispatch_p<kPersistBIF>(c, ps, uz, ur, beta, first, bid, nb);
 }
 __device__ __noinline__ double ps_(const Ctx& c, int ur, int uz, int bid, int nb, double* red) {
-  return dispatch_spmv<true, kPersistThreads>(c, ur, uz, bid, nb, red);
+  return dispatch_spmv<true, kPersistThreads>(c, ur, uz, 0, bid, nb, red);
 }
 __device__ __noinline__ double pxr(const Ctx& c, int ur, int uz, double alpha, double* x, int bid, int nb) {
   return dispatch_xr<kPersistBIF>(c, ur, uz, alpha, x, bid, nb);

@@ -310,6 +310,135 @@ __device__ __forceinline__ double phase_z(const Ctx& c, const double omega, int 
   return sum;
 }
 
+// ------------------------------------------------------------------ a2 with Chebyshev-Jacobi --
+// M^-1 = s sweeps of Chebyshev-accelerated Jacobi (the paper's smoother; reading R18).
+// Explicit __dmul_rn / __dsub_rn / __dadd_rn / __fma_rn: the operation order IS the definition (the oracle's
+// orc_cheb_first / orc_cheb_step do the same operations), so nothing may be contracted into an fma.
+// first sweep: d = z = RN_{u_z}( ((r omega) dinv) / theta ); WITH_RHO (s = 1): rho = r^T z.  RS/UR/UZ as in phase_z.
+template <int RS, int UR, int UZ, int BIF = kVecBytesInFlight>
+__device__ __forceinline__ double phase_cheb0(const Ctx& c, const double omega, const bool with_rho, int bid, int nb) {
+  using TR = typename Store<RS>::T;
+  using TO = typename Store<UR>::T;
+  using TZ = typename Store<UZ>::T;
+  using TD = typename Store<(UZ == P64) ? P64 : P32>::T;
+  constexpr int smin = cmin(cmin((int)sizeof(TR), (int)sizeof(TO)), cmin((int)sizeof(TD), (int)sizeof(TZ)));
+  constexpr int smax = cmax(cmax((int)sizeof(TR), (int)sizeof(TO)), cmax((int)sizeof(TD), (int)sizeof(TZ)));
+  constexpr int E = chunk_elems(smin, smax);
+  constexpr int U = cmax(1, BIF / (E * (int)(sizeof(TR) + sizeof(TD))));
+  const TR* rin = rvec<RS>(c);
+  TO* rout = rvec<UR>(c);
+  TZ* z = zvec<UZ>(c);
+  TZ* dd_out = dvec<UZ>(c);
+  const TD* dinv;
+  if constexpr (UZ == P64) dinv = c.dinv64; else dinv = c.dinv32;
+  const double inv_theta = c.cheb_inv_theta;
+  const int64_t nchunk = c.npad / E;
+  const int64_t stride = (int64_t)nb * blockDim.x;
+  double sum = 0.0;
+  for (int64_t base = (int64_t)bid * blockDim.x + threadIdx.x; base < nchunk; base += stride * U) {
+    Chunk<TR, E> rr[U];
+    Chunk<TD, E> dd[U];
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      const int64_t i = base + u * stride;
+      if (i < nchunk) { chunk_load(rr[u], rin, i); chunk_load(dd[u], dinv, i); }
+    }
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      const int64_t i = base + u * stride;
+      if (i < nchunk) {
+        double a[E], d[E], zz[E];
+        chunk_unpack(rr[u], a);
+        chunk_unpack(dd[u], d);
+        if constexpr (RS != UR) {  // r <- RN_{u_r}(r) at the switch iteration (step a6)
+          Chunk<TO, E> ro;
+          chunk_pack(ro, a);
+          chunk_store(ro, rout, i);
+          chunk_unpack(ro, a);
+        }
+#pragma unroll
+        for (int e = 0; e < E; ++e) zz[e] = __dmul_rn(__dmul_rn(__dmul_rn(a[e], omega), d[e]), inv_theta);
+        Chunk<TZ, E> zo;
+        chunk_pack(zo, zz);  // one rounding to u_z
+        chunk_store(zo, z, i);
+        chunk_store(zo, dd_out, i);
+        if (with_rho) {
+          chunk_unpack(zo, zz);
+#pragma unroll
+          for (int e = 0; e < E; ++e) sum = fma(a[e], zz[e], sum);
+        }
+      }
+    }
+  }
+  return sum;
+}
+
+// sweep i >= 1, w = A z in u_r (the q buffers): t = r omega - w; u = t dinv; d = RN_{u_z}(fma(c1, d, c2 u));
+// z = RN_{u_z}(z + d); with_rho (last sweep): rho = r^T z with the stored z
+template <int UR, int UZ, int BIF = kVecBytesInFlight>
+__device__ __forceinline__ double phase_cheb_step(const Ctx& c, const double omega, const double c1, const double c2,
+                                                  const bool with_rho, int bid, int nb) {
+  using TR = typename Store<UR>::T;
+  using TZ = typename Store<UZ>::T;
+  using TD = typename Store<(UZ == P64) ? P64 : P32>::T;
+  constexpr int smin = cmin(cmin((int)sizeof(TR), (int)sizeof(TD)), (int)sizeof(TZ));
+  constexpr int smax = cmax(cmax((int)sizeof(TR), (int)sizeof(TD)), (int)sizeof(TZ));
+  constexpr int E = chunk_elems(smin, smax);
+  constexpr int U = cmax(1, BIF / (E * (int)(2 * sizeof(TR) + sizeof(TD) + 2 * sizeof(TZ))));
+  const TR* r = rvec<UR>(c);
+  const TR* w = qvec<UR>(c);
+  TZ* z = zvec<UZ>(c);
+  TZ* dv = dvec<UZ>(c);
+  const TD* dinv;
+  if constexpr (UZ == P64) dinv = c.dinv64; else dinv = c.dinv32;
+  const int64_t nchunk = c.npad / E;
+  const int64_t stride = (int64_t)nb * blockDim.x;
+  double sum = 0.0;
+  for (int64_t base = (int64_t)bid * blockDim.x + threadIdx.x; base < nchunk; base += stride * U) {
+    Chunk<TR, E> rr[U], ww[U];
+    Chunk<TD, E> ii[U];
+    Chunk<TZ, E> dd[U], zz[U];
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      const int64_t i = base + u * stride;
+      if (i < nchunk) {
+        chunk_load(rr[u], r, i); chunk_load(ww[u], w, i); chunk_load(ii[u], dinv, i);
+        chunk_load(dd[u], dv, i); chunk_load(zz[u], z, i);
+      }
+    }
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      const int64_t i = base + u * stride;
+      if (i < nchunk) {
+        double rv[E], wv[E], iv[E], dvv[E], zv[E];
+        chunk_unpack(rr[u], rv); chunk_unpack(ww[u], wv); chunk_unpack(ii[u], iv);
+        chunk_unpack(dd[u], dvv); chunk_unpack(zz[u], zv);
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+          const double t = __dsub_rn(__dmul_rn(rv[e], omega), wv[e]);
+          const double uu = __dmul_rn(t, iv[e]);
+          dvv[e] = __fma_rn(c1, dvv[e], __dmul_rn(c2, uu));
+        }
+        Chunk<TZ, E> dout;
+        chunk_pack(dout, dvv);   // one rounding to u_z
+        chunk_store(dout, dv, i);
+        chunk_unpack(dout, dvv);
+#pragma unroll
+        for (int e = 0; e < E; ++e) zv[e] = __dadd_rn(zv[e], dvv[e]);
+        Chunk<TZ, E> zout;
+        chunk_pack(zout, zv);    // one rounding to u_z
+        chunk_store(zout, z, i);
+        if (with_rho) {
+          chunk_unpack(zout, zv);
+#pragma unroll
+          for (int e = 0; e < E; ++e) sum = fma(rv[e], zv[e], sum);
+        }
+      }
+    }
+  }
+  return sum;
+}
+
 // ------------------------------------------------------------------ a3: p -------------------
 // PS: precision p_{k-1} is stored in; UZ: precision of z_k and p_k (PS != UZ only at a u_z
 // switch, where p_{k-1} <- RN_{u_z}(p_{k-1}) is fused here, reading R9).

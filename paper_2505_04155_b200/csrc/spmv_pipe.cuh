@@ -229,7 +229,7 @@ __device__ __forceinline__ double pipe_body(const Ctx& c, const PT* p, const PG*
 // (The u_r = FP64 phases stay with the direct kernel, which already streams at the copy rate there: measured on c4,
 // 303 us direct against 327-349 us pipelined, profiles/r02.md.  Both kernels sit in the loop; the one whose phase it
 // is not returns at once.)
-__global__ void __launch_bounds__(kPipeThreads, 1) k_spmv_pipe(const Ctx c) {
+__global__ void __launch_bounds__(kPipeThreads, 1) k_spmv_pipe(const Ctx c, int zmode) {
   extern __shared__ __align__(128) unsigned char pipe_smem[];
   __shared__ double red[32];
   DevState* s = c.st;
@@ -239,6 +239,13 @@ __global__ void __launch_bounds__(kPipeThreads, 1) k_spmv_pipe(const Ctx c) {
   const int ur = s->ur, uz = s->uz;
   if (s->done || ur != P32) { pdl_wait(); return; }
   double v;
+  if (zmode) {  // q = A z inside the Chebyshev-Jacobi preconditioner
+    if (uz == P16) v = pipe_body<P32>(c, c.z16, c.z16, c.q32, pipe_smem);
+    else if (uz == P32) v = pipe_body<P32>(c, c.z32, c.z32, c.q32, pipe_smem);
+    else v = pipe_body<P32>(c, c.z64, c.z64, c.q32, pipe_smem);  // RN32(z_j) per gathered entry
+    pdl_wait();
+    return;
+  }
   if (uz == P16) v = pipe_body<P32>(c, c.p16, c.p16, c.q32, pipe_smem);
   else if (uz == P32) v = pipe_body<P32>(c, c.p32, c.p32, c.q32, pipe_smem);
   else v = pipe_body<P32>(c, c.p32, c.p64, c.q32, pipe_smem);  // gathers the FP32 copy RN32(p) written by the p update

@@ -47,7 +47,7 @@ def test_struct_layout_matches_c(A, tmp_path):
     # compile a tiny C program against the header and compare sizeof/offsetof with ctypes
     probes = [("amp_policy_t", A.Policy, ["C", "stop_safety", "profile_kernels"]),
               ("amp_stats_t", A.Stats, ["bnorm", "fp16_inf"]),
-              ("amp_create_opts_t", A.CreateOpts, ["pdl", "stream"]),
+              ("amp_create_opts_t", A.CreateOpts, ["pdl", "cheb_degree", "cheb_lmax", "stream"]),
               ("amp_kernel_time_t", A.KernelTime, ["launches", "bytes_per_launch"]),
               ("amp_debug_step_t", A.DebugStep, ["first", "omega", "sum1"])]
     body, want = [], []
@@ -69,6 +69,7 @@ def test_create_opts_defaults_and_validation(A):
     o = A.CreateOpts.default()
     assert o.struct_bytes == C.sizeof(A.CreateOpts) and o.precond == A.PRECOND_JACOBI
     assert (o.index_format, o.spmv_kernel, o.spmv_grid_mult, o.pdl) == (A.INDEX_AUTO, A.SPMV_AUTO, 0, 1)
+    assert (o.cheb_degree, o.cheb_lmin, o.cheb_lmax) == (2, 0.0, 0.0)  # PAPER.md:461 "second-order"; bounds computed in create()
     # a struct of another size (an older / newer header) is refused before anything touches the device
     import numpy as np
 
