@@ -55,6 +55,8 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--others", default="", help="comma list of further workloads to report under 'other_workloads' "
                                                  "(value / time_to_tol / speed-up only), e.g. c1,c2,c3,c5")
+    ap.add_argument("--cheb-degrees", default="2,3", help="degrees of the Chebyshev-Jacobi preconditioner to time beside "
+                                                           "the Jacobi headline ('' = none)")
     ap.add_argument("--profile-iters", type=int, default=0,
                     help="profiling aid for ncu: run ONE solve of this many iterations with plain stream launches "
                          "(u_r forced to FP32 from k=ell so the low-precision kernels appear) and exit; prints no bench line")
@@ -247,11 +249,15 @@ def run_reference(args, rank: int, world: int):
 class Runner:
     """one workload resident on one GPU: timed solves of a policy, each preceded by an L2 flush"""
 
-    def __init__(self, A, torch, s, dev, loop, spmv_kernel):
+    def __init__(self, A, torch, s, dev, loop, spmv_kernel, share=None, precond=None, **opts):
         self.A, self.torch, self.s, self.dev = A, torch, s, dev
-        self.rp, self.ci, self.va, self.b = (torch.from_numpy(a).to(dev) for a in (s.rowptr, s.colidx, s.vals, s.b))
+        if share is not None:  # same matrix already on the device
+            self.rp, self.ci, self.va, self.b = share.rp, share.ci, share.va, share.b
+        else:
+            self.rp, self.ci, self.va, self.b = (torch.from_numpy(a).to(dev) for a in (s.rowptr, s.colidx, s.vals, s.b))
         t0 = time.perf_counter()
-        self.h = A.AmpPcg(self.rp, self.ci, self.va, A.PRECOND_JACOBI, spmv_kernel=spmv_kernel)
+        self.h = A.AmpPcg(self.rp, self.ci, self.va, A.PRECOND_JACOBI if precond is None else precond,
+                          spmv_kernel=spmv_kernel, **opts)
         torch.cuda.synchronize()
         self.create_s = time.perf_counter() - t0
         self.loop = loop
@@ -419,6 +425,18 @@ def run_ours(args, rank: int, local_rank: int, world: int):
     roofline["whole_loop"] = {"amp_gbs": loop_gbs, "amp_frac": loop_gbs / peak, "amp_frac_of_8TBs": loop_gbs / 8000.0,
                               "fp64_gbs": loop64_gbs, "fp64_frac": loop64_gbs / peak}
 
+    # ---- NEXT-4: the same solve with the Chebyshev-accelerated Jacobi preconditioner (the paper's smoother) ----
+    cheb = {}
+    for deg in [int(t) for t in args.cheb_degrees.split(",") if t]:
+        Rc = Runner(A, torch, s, dev, loop, spmv_kernel, share=R, precond=A.PRECOND_CHEBJACOBI, cheb_degree=deg)
+        a_, _ = Rc.summary(args.policy, 2)
+        f_, _ = Rc.summary(dict(amp=0), 2)
+        cheb[f"degree_{deg}"] = {"amp": a_, "fp64_pcg": f_, "amp_speedup_vs_fp64_same_precond": f_["time_to_tol_s"] / a_["time_to_tol_s"],
+                                 "speedup_vs_jacobi_amp": t_amp / a_["time_to_tol_s"],
+                                 "matvecs_per_solve": deg * a_["iters"]}
+        Rc.close()
+        del Rc
+
     # ---- the other BASELINE.json configs (parity-test cases; reported for context) ----
     others = {}
     for name in [t for t in args.others.split(",") if t]:
@@ -462,6 +480,8 @@ def run_ours(args, rank: int, local_rank: int, world: int):
         "roofline": roofline,
         "cpu_baseline": cpu,
     }
+    if cheb:
+        line["chebyshev_jacobi_preconditioner"] = cheb
     if others:
         line["other_workloads"] = others
     print(json.dumps(line), flush=True)
