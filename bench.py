@@ -76,13 +76,16 @@ def peaks():
 
 def ncu_traffic(workload: str, kernel: str):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full capture of THIS round
-    (profiles/r02_ncu_traffic.json names the capture and the commit), else None."""
-    path = os.path.join(ROOT, "profiles", "r02_ncu_traffic.json")
+    (profiles/r02_ncu_traffic.csv names the capture each value comes from), else None."""
+    path = os.path.join(ROOT, "profiles", "r02_ncu_traffic.csv")
     try:
-        d = json.load(open(path))
-        return d.get(workload, {}).get(kernel)
+        for line in open(path).read().splitlines()[1:]:
+            f = line.split(",")
+            if len(f) >= 3 and f[0] == workload and f[1] == kernel:
+                return float(f[2])
     except (OSError, ValueError):
-        return None
+        pass
+    return None
 
 
 class ClockSampler:

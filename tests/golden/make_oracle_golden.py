@@ -5,7 +5,10 @@ This script calls only ``oracle/`` and ``workloads/`` (never the CUDA path).  Th
 no iteration counts for these synthetic systems, so these values are "parity unpinned" by the
 paper: they pin GPU <-> oracle agreement only ("Oracle pins").
 
-    python tests/golden/make_oracle_golden.py [c1 c2 ...]      # minutes of CPU time
+    python tests/golden/make_oracle_golden.py [--force] [c1 c2 ...]      # minutes of CPU time
+
+Policies already present in the file for a config are kept (their inputs are seeded and the oracle is
+deterministic); --force recomputes them.
 """
 import json
 import os
@@ -28,6 +31,10 @@ POLICIES = {
     "amp_fp16_linear": dict(amp=1, u0=O.FP16, eta_rule=O.ETA_LINEAR),
     "amp_fp64_delay_strict": dict(amp=1, u0=O.FP64, eta_rule=O.ETA_DELAY, eta_safety=0.1, stop_safety=0.9),
     "amp_fp64_delay_lagged": dict(amp=1, u0=O.FP64, eta_rule=O.ETA_DELAY, scale_mode=O.SCALE_LAGGED),
+    # omega = sqrt(n)/||r_k|| ("other scaling factors can be used"): the evidence for the scaling
+    # decision of DESIGN.md section 2 (reading R10) — FP16 subnormal exposure and iteration counts at full size
+    "amp_fp64_delay_rms": dict(amp=1, u0=O.FP64, eta_rule=O.ETA_DELAY, scale_mode=O.SCALE_RMS),
+    "amp_fp16_linear_rms": dict(amp=1, u0=O.FP16, eta_rule=O.ETA_LINEAR, scale_mode=O.SCALE_RMS),
 }
 
 
@@ -41,11 +48,15 @@ def main(names):
         rng_p = 2.0 * np.modf(np.arange(s.n) * 0.6180339887498949)[0] - 1.0  # deterministic probe vector
         q = O.spmv_fp64(s.rowptr, s.colidx, s.vals, rng_p)
         sample = np.linspace(0, s.n - 1, 64).astype(np.int64)
+        old = data.get(name, {}).get("policies", {}) if not FORCE else {}
         entry = {"n": s.n, "nnz": s.nnz, "tol": s.tol, "maxit": s.maxit, "gen_s": round(time.time() - t0, 1),
                  "spmv_probe": {"rows": sample.tolist(), "q": [float(v) for v in q[sample]],
                                 "q_norm2": float(np.sqrt(O.dot(q, q)))},
                  "policies": {}}
         for pname, kw in POLICIES.items():
+            if pname in old:
+                entry["policies"][pname] = old[pname]
+                continue
             t1 = time.time()
             r = O.amp_pcg(s.rowptr, s.colidx, s.vals, s.b, s.tol, s.maxit, O.make_policy(**kw))
             entry["policies"][pname] = {
@@ -60,5 +71,7 @@ def main(names):
         json.dump(data, open(OUT, "w"), indent=1)
 
 
+FORCE = "--force" in sys.argv
+
 if __name__ == "__main__":
-    main(sys.argv[1:] or list(CONFIGS))
+    main([a for a in sys.argv[1:] if not a.startswith("--")] or list(CONFIGS))
