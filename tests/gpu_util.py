@@ -16,6 +16,8 @@ POLICY_SPECS = {
     "amp_fp64_rms": dict(amp=1, u0=0, eta_rule=0, scale_mode=1),
     "amp_fp64_pow2": dict(amp=1, u0=0, eta_rule=0, scale_mode=2),
     "amp_fp64_delay_lagged": dict(amp=1, u0=0, eta_rule=0, scale_mode=4),
+    "amp_fp64_delay_rms": dict(amp=1, u0=0, eta_rule=0, scale_mode=1),
+    "amp_fp16_linear_rms": dict(amp=1, u0=2, eta_rule=1, scale_mode=1),
 }
 
 

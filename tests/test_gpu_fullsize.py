@@ -2,7 +2,9 @@
 (loop_mode AUTO, x0 = 0), against values the CPU oracle wrote to
 tests/golden/oracle_full_size.json (tests/golden/make_oracle_golden.py, oracle-only script):
 
-* SpMV: 64 sampled rows of q = A p for a fixed probe vector, <= 1e-13 relative, plus ||q||_2;
+* SpMV: 64 sampled rows of q = A p for a fixed probe vector, <= 1e-13 relative, plus ||q||_2 (stored values), and the
+  WHOLE vector bit for bit against the oracle's mat-vec called here, in FP64 and in the u_r = FP32 phase with FP16 p
+  (both sides: one fma chain per row in CSR order);
 * solves: iteration count within 5 % (+-1 for FP64 PCG), switch iterations +-2, status,
   true residual <= 2 tol (paper policy) / <= tol (strict policy) recomputed here in FP64 by torch
   (an independent sparse mat-vec, not the library's).
@@ -42,6 +44,16 @@ def test_full_size_against_oracle_golden(name):
         qref = np.array(g["spmv_probe"]["q"])
         assert np.max(np.abs(qs - qref)) <= 1e-13 * max(np.max(np.abs(qref)), float(q.abs().max()))
         assert float(torch.linalg.norm(q)) == pytest.approx(g["spmv_probe"]["q_norm2"], rel=1e-12)
+        # the whole vector, bit for bit (FP64; FP32 matrix copy with FP16-stored p), against the oracle called here
+        import oracle as O
+
+        assert np.array_equal(q.cpu().numpy(), O.spmv_fp64(s.rowptr, s.colidx, s.vals, p))
+        npad = (s.n + 7) // 8 * 8
+        p16 = torch.zeros(npad, dtype=torch.float16, device="cuda")
+        p16[:s.n] = torch.from_numpy(p).cuda().to(torch.float16)
+        q32 = h.spmv(p16, A.FP32).cpu().numpy()
+        q32_ref = O.spmv_fp32(s.rowptr, s.colidx, s.vals, p16[:s.n].cpu().numpy().astype(np.float64))
+        assert np.array_equal(q32.astype(np.float64), q32_ref)
         # independent FP64 mat-vec for the true residual
         crow = rp.to(torch.int64)
         At = torch.sparse_csr_tensor(crow, ci.to(torch.int64), va, size=(s.n, s.n))
