@@ -66,6 +66,12 @@ def parse_args():
     ap.add_argument("--profile-policy", default="amp_fp16_linear",
                     choices=["pcg_fp64", "amp_fp16_linear", "amp_fp64_delay", "amp_fp16_linear_lagged"])
     ap.add_argument("--ref-iters", type=int, default=0, help="--impl reference: iterations per step (0 = sized to the workload)")
+    ap.add_argument("--shard", action="store_true",
+                    help="N > 1: ONE system row-sharded over the N ranks (amp_pcg_solve_sharded: halo of p and the three inner "
+                         "products exchanged by the loop kernels over peer memory; strong scaling) instead of N replicas")
+    ap.add_argument("--shard-local", type=int, default=0,
+                    help="one GPU: emulate this many ranks of the row-sharded solve in one process (lock-step launches on one "
+                         "stream; functional check and overhead of the sharded kernels, not a scaling number)")
     return ap.parse_args()
 
 
@@ -502,6 +508,93 @@ def run_ours(args, rank: int, local_rank: int, world: int):
         dist.destroy_process_group()
 
 
+def run_sharded(args, rank: int, local_rank: int, world: int):
+    """One system row-sharded over the ranks: --shard under torchrun (one process per
+    GPU, peers wired through CUDA IPC) or --shard-local W (W ranks emulated on one GPU by one process)."""
+    import torch
+
+    import paper_2505_04155_b200 as A
+    from workloads import make_config
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the library has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    s = make_config(args.workload, args.size)
+    local = args.shard_local > 0
+    nranks = args.shard_local if local else world
+    dist = None
+    if not local:
+        import torch.distributed as dist_
+
+        dist = dist_
+        dist.init_process_group("nccl", device_id=dev)
+    plan = A.shard_plan(s.rowptr, s.colidx, nranks)
+    mine = list(range(nranks)) if local else [rank]
+    handles, bs, xs = [], [], []
+    for r in mine:
+        sh = plan[r]
+        rp, ci, va = A.shard_extract(s.rowptr, s.colidx, s.vals, sh)
+        handles.append(A.AmpPcg(torch.from_numpy(rp).to(dev), torch.from_numpy(ci).to(dev), torch.from_numpy(va).to(dev),
+                                A.PRECOND_JACOBI, halo_lo=sh.halo_lo, halo_hi=sh.halo_hi))
+        bs.append(torch.from_numpy(s.b[sh.row0:sh.row1].copy()).to(dev))
+        xs.append(torch.zeros(sh.row1 - sh.row0, dtype=torch.float64, device=dev))
+    if local:
+        g = A.ShardGroup.attach_local(handles)
+    else:
+        blobs = [None] * world
+        dist.all_gather_object(blobs, A.ShardGroup.export(handles[0]))   # plumbing: the IPC handles of every rank
+        g = A.ShardGroup.attach_ipc(handles[0], rank, blobs)
+    pol = A.Policy.default(x0_zero=1, **policy_kwargs(args.policy))
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    stream = torch.cuda.current_stream(dev)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()      # also required by the library: no rank starts a solve before all have finished the last
+        torch.cuda.synchronize()
+
+    def timed(count):
+        ms, st = [], None
+        for _ in range(count):
+            flush.fill_(1)
+            barrier()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            st = g.solve(bs, xs, s.tol, s.maxit, pol)[0]
+            e1.record(stream)
+            e1.synchronize()
+            ms.append(e0.elapsed_time(e1))
+        return ms, st
+
+    timed(args.warmup)
+    barrier()
+    with ClockSampler(local_rank) as clk:
+        ms, st = timed(args.steps)
+    barrier()
+    (tot,), _ = reduce_over_ranks(dist, [sum(ms)], [0], dev)
+    st_true = g.solve(bs, xs, s.tol, s.maxit, A.Policy.default(x0_zero=1, true_residual=1, **policy_kwargs(args.policy)))[0]
+    launches = sum(h.last_launch_count() for h in handles)
+    if rank == 0:
+        halo = [int(p_.halo_lo + p_.halo_hi) for p_ in plan]
+        line = {
+            "metric": METRIC, "value": args.steps * st.iters / (tot * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": tot / args.steps, "higher_is_better": True,
+            "scaling": "strong", "vs_baseline": None, "dtype": DTYPE, "data": "synthetic",
+            "config": dict(config_dict(s, args.policy, 1), sharded_ranks=nranks,
+                           mode="emulated on one GPU (lock-step launches)" if local else "one process per GPU, CUDA IPC peers"),
+            "iters": st.iters, "switch_iters": {"ur32": st.it_ur32, "uz32": st.it_uz32, "uz16": st.it_uz16},
+            "relres_updated": st.relres_updated, "relres_true": st_true.relres_true, "time_to_tol_s": statistics.median(ms) * 1e-3,
+            "rows_per_rank": [int(p_.row1 - p_.row0) for p_ in plan], "halo_entries_per_rank": halo,
+            "halo_bytes_per_iteration_fp16": 2 * sum(halo), "halo_bytes_per_iteration_fp64": 8 * sum(halo),
+            "gpu_launches": launches, "clocks": clk.result,
+        }
+        print(json.dumps(line), flush=True)
+    g.close()
+    if dist is not None:
+        dist.destroy_process_group()
+
+
 def main():
     args = parse_args()
     rank = int(os.environ.get("RANK", "0"))
@@ -509,6 +602,8 @@ def main():
     world = int(os.environ.get("WORLD_SIZE", "1"))
     if args.impl == "reference":
         run_reference(args, rank, world)
+    elif args.shard_local > 0 or (args.shard and world > 1):
+        run_sharded(args, rank, local_rank, world)
     else:
         run_ours(args, rank, local_rank, world)
 

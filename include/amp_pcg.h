@@ -178,6 +178,10 @@ typedef struct {
   double cheb_lmax;       /*   lmax = max_i sum_j |a_ij| / a_ii (Gershgorin), lmin = lmax / 30, computed in create() */
   void *stream;           /* cudaStream_t the create() kernels run on and the handle starts with (NULL = legacy
                              default stream); the caller's CSR arrays must be complete in this stream's order */
+  int64_t halo_lo;        /* row-sharded solve (see "row-sharded solve" below): the matrix is one block row of a larger */
+  int64_t halo_hi;        /*   system, n rows by halo_lo + n + halo_hi columns; column index halo_lo + i is the diagonal of
+                               row i, columns below halo_lo / from halo_lo + n on are the neighbour ranks' entries of p
+                               (filled by the halo exchange).  Both 0 (default): an ordinary square matrix */
 } amp_create_opts_t;
 void amp_create_opts_default(amp_create_opts_t *o);
 amp_pcg_t *amp_pcg_create_ex(int64_t n, int64_t nnz, const int32_t *rowptr, const int32_t *colidx,
@@ -265,6 +269,67 @@ typedef struct {
 /* Writes up to cap records (one per kernel and phase that occurred) to HOST out; returns the count, 0 if the last
  * solve was not profiled, or a negative error code. */
 int32_t amp_pcg_kernel_times(amp_pcg_t *h, amp_kernel_time_t *out_host, int32_t cap);
+
+/* ---- row-sharded solve over several GPUs ------------------------------------
+ * The paper runs on one GPU; how Algorithm 4.1 shards follows from its data flow: the rows of A, and
+ * with them r, z, p, q, x, are split into contiguous blocks, one per rank.  Per iteration the only data that crosses ranks
+ * are  (1) the entries of p the local block row touches outside its own rows (the halo), needed by q = A p (line 11) —
+ * exchanged in the precision the mat-vec gathers (u_z; RN32(p) while u_z = FP64 and u_r = FP32), so AMP shrinks it up
+ * to 4x;  (2) the three inner products rho = r^T z, gamma = q^T p, ||r||^2 (lines 6, 13, 17): every rank publishes its
+ * partial sum to every rank and each adds all partials in rank order, so all ranks hold bit-identical scalars and take
+ * the same decisions (stop, switches, breakdown) without any broadcast.
+ * Both exchanges are done by the loop kernels themselves over peer-mapped device memory (NVLink / NVSwitch stores, or
+ * plain stores when the ranks share a device): the p update writes the boundary entries straight into the neighbours'
+ * halo bands and then raises their flags, the mat-vec waits for its two flags, the reducing kernels post their partial
+ * sums into every rank's mailbox and a one-warp kernel per reduction point adds them and runs the scalar step.  No NCCL
+ * call, no host on the data path; the host launches the same graph / stream loop as in the single-GPU solve.
+ *
+ * Partition: contiguous row blocks whose boundaries are multiples of 32 rows (whole SELL-32 slices), balanced by stored
+ * entries.  A rank's halo must lie inside its two neighbour ranks (banded coupling: stencils, c5's 50 000-row band).
+ * All pointers of amp_shard_plan / amp_shard_extract are HOST pointers; they do not touch the device. */
+typedef struct {
+  int64_t row0, row1;       /* this rank owns the global rows [row0, row1) */
+  int64_t halo_lo, halo_hi; /* entries of p needed below row0 / from row1 on (rounded up to multiples of 8) */
+  int64_t nnz;              /* stored entries of the block row */
+} amp_shard_t;
+/* Plan the block-row partition of an n x n CSR pattern over `world` ranks (1 <= world <= 16) into out[world].
+ * Returns AMP_OK, or AMP_ERR_INVALID (bad arguments; fewer than 32 rows per rank; a halo reaching past the neighbour). */
+int amp_shard_plan(int64_t n, const int32_t *rowptr, const int32_t *colidx, int32_t world, amp_shard_t *out);
+/* Extract the block row `s` as a CSR of s->row1 - s->row0 rows whose column indices are shifted to the extended vector
+ * [halo_lo | owned | halo_hi] (global column j becomes j - row0 + halo_lo) — the arrays amp_pcg_create_ex takes together
+ * with opts.halo_lo / halo_hi.  rowptr_out: int32[rows + 1]; colidx_out / vals_out: s->nnz entries, CSR order kept. */
+int amp_shard_extract(int64_t n, const int32_t *rowptr, const int32_t *colidx, const double *vals, const amp_shard_t *s,
+                      int32_t *rowptr_out, int32_t *colidx_out, double *vals_out);
+
+/* Wiring.  Every rank creates its handle with amp_pcg_create_ex (opts.halo_lo / halo_hi from the plan), then either
+ *  (a) one process drives all ranks (handles on one device — the testable emulation — or on peer-accessible devices):
+ *      amp_pcg_shard_attach_local(handles, world), handles[r] = rank r; or
+ *  (b) one process per GPU: every rank fills an amp_shard_export_t (amp_pcg_shard_export), the blobs are all-gathered by
+ *      the caller (torch.distributed: plumbing), and every rank calls amp_pcg_shard_attach(h, rank, world, blobs), which
+ *      opens its neighbours' buffers with CUDA IPC.
+ * Handles of one group must agree in preconditioner (NONE / JACOBI) and be created from one amp_shard_plan. */
+#define AMP_SHARD_MAX_WORLD 16
+typedef struct {
+  int64_t n, halo_lo, halo_hi, guard; /* geometry of this rank's extended p vectors */
+  unsigned char mem[4][64];           /* cudaIpcMemHandle_t of: the exchange block (mailboxes + flags), p64, p32, p16 */
+  int64_t off[4];                     /* byte offset of each object inside its allocation */
+} amp_shard_export_t;
+int amp_pcg_shard_export(amp_pcg_t *h, amp_shard_export_t *out_host);
+int amp_pcg_shard_attach(amp_pcg_t *h, int32_t rank, int32_t world, const amp_shard_export_t *all_host);
+int amp_pcg_shard_attach_local(amp_pcg_t *const *handles, int32_t world);
+
+/* Solve the sharded system: handles[0..nlocal) are the ranks this process drives (nlocal = world after
+ * amp_pcg_shard_attach_local, 1 after amp_pcg_shard_attach), b[i] / x[i] their DEVICE block rows of b and x (x: x0 in,
+ * x_m out), stats[i] HOST (may be NULL).  Same policy semantics as amp_pcg_solve; every rank must pass the same tol,
+ * maxit and policy.  Not available with AMP_PRECOND_CHEBJACOBI and AMP_LOOP_PERSISTENT; AMP_LOOP_AUTO = graph when
+ * nlocal = 1, else stream (the ranks of one process are launched in lock step).  In mode (b) no rank may start a
+ * solve before every rank has returned from the previous one (a host barrier between solves).
+ * A rank that waits longer than ~10 s for a peer gives up with AMP_ERR_CUDA.  Returns the common status. */
+int amp_pcg_solve_sharded(amp_pcg_t *const *handles, int32_t nlocal, const double *const *b, double *const *x, double tol,
+                          int32_t maxit, const amp_policy_t *policy, amp_stats_t *stats);
+/* q = A p on the sharded system (mat_prec / vec_prec as amp_spmv; p[i]: this rank's n entries, q[i]: its rows): halo
+ * exchange of p, then the loop's mat-vec.  For tests and for callers that need the operator alone. */
+int amp_spmv_sharded(amp_pcg_t *const *handles, int32_t nlocal, int mat_prec, int vec_prec, const void *const *p, void *const *q);
 
 /* ---- diagnostic entry points (parity tests; not on the hot path) ------------------------------------------
  * Run ONE step of the loop with caller-given scalars and precisions through the SAME __global__ kernel, grid and

@@ -27,4 +27,5 @@ from .binding import (  # noqa: F401
     VEC_R, VEC_Q, VEC_Z, VEC_P, VEC_DINV, VEC_D,
     STEP_Z, STEP_P, STEP_SPMV, STEP_XR, STEP_XRZ, STEP_CHEB0, STEP_SPMV_Z, STEP_CHEBSTEP,
     EXPORTED_SYMBOLS,
+    Shard, ShardExport, ShardGroup, shard_plan, shard_extract, SHARD_MAX_WORLD,
 )

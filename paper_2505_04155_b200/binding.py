@@ -32,7 +32,10 @@ EXPORTED_SYMBOLS = (
     "amp_pcg_last_error", "amp_pcg_bytes_per_row", "amp_pcg_spmv_bytes", "amp_pcg_iteration_bytes",
     "amp_pcg_eta_posteriori", "amp_pcg_kernel_times",
     "amp_pcg_debug_set_vector", "amp_pcg_debug_get_vector", "amp_pcg_debug_step",
+    "amp_shard_plan", "amp_shard_extract", "amp_pcg_shard_export", "amp_pcg_shard_attach", "amp_pcg_shard_attach_local",
+    "amp_pcg_solve_sharded", "amp_spmv_sharded",
 )
+SHARD_MAX_WORLD = 16
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 
@@ -70,6 +73,7 @@ class CreateOpts(C.Structure):
         ("struct_bytes", C.c_int32), ("precond", C.c_int32), ("index_format", C.c_int32), ("spmv_kernel", C.c_int32),
         ("spmv_grid_mult", C.c_int32), ("pdl", C.c_int32), ("cheb_degree", C.c_int32), ("reserved0", C.c_int32),
         ("cheb_lmin", C.c_double), ("cheb_lmax", C.c_double), ("stream", C.c_void_p),
+        ("halo_lo", C.c_int64), ("halo_hi", C.c_int64),
     ]
 
     @classmethod
@@ -81,6 +85,19 @@ class CreateOpts(C.Structure):
                 raise AttributeError(k)
             setattr(o, k, v)
         return o
+
+
+class Shard(C.Structure):
+    """amp_shard_t (include/amp_pcg.h): one rank's block row of the partition."""
+
+    _fields_ = [("row0", C.c_int64), ("row1", C.c_int64), ("halo_lo", C.c_int64), ("halo_hi", C.c_int64), ("nnz", C.c_int64)]
+
+
+class ShardExport(C.Structure):
+    """amp_shard_export_t (include/amp_pcg.h): what a rank publishes to its peers (CUDA IPC handles + geometry)."""
+
+    _fields_ = [("n", C.c_int64), ("halo_lo", C.c_int64), ("halo_hi", C.c_int64), ("guard", C.c_int64),
+                ("mem", (C.c_ubyte * 64) * 4), ("off", C.c_int64 * 4)]
 
 
 class KernelTime(C.Structure):
@@ -172,6 +189,21 @@ def load_library(variant: str = ""):
     L.amp_pcg_debug_get_vector.argtypes = [vp, C.c_int, C.c_int, vp]
     L.amp_pcg_debug_step.restype = C.c_int
     L.amp_pcg_debug_step.argtypes = [vp, C.POINTER(DebugStep), vp]
+    L.amp_shard_plan.restype = C.c_int
+    L.amp_shard_plan.argtypes = [i64, vp, vp, i32, C.POINTER(Shard)]
+    L.amp_shard_extract.restype = C.c_int
+    L.amp_shard_extract.argtypes = [i64, vp, vp, vp, C.POINTER(Shard), vp, vp, vp]
+    L.amp_pcg_shard_export.restype = C.c_int
+    L.amp_pcg_shard_export.argtypes = [vp, C.POINTER(ShardExport)]
+    L.amp_pcg_shard_attach.restype = C.c_int
+    L.amp_pcg_shard_attach.argtypes = [vp, i32, i32, C.POINTER(ShardExport)]
+    L.amp_pcg_shard_attach_local.restype = C.c_int
+    L.amp_pcg_shard_attach_local.argtypes = [C.POINTER(vp), i32]
+    L.amp_pcg_solve_sharded.restype = C.c_int
+    L.amp_pcg_solve_sharded.argtypes = [C.POINTER(vp), i32, C.POINTER(vp), C.POINTER(vp), dbl, i32, C.POINTER(Policy),
+                                        C.POINTER(Stats)]
+    L.amp_spmv_sharded.restype = C.c_int
+    L.amp_spmv_sharded.argtypes = [C.POINTER(vp), i32, C.c_int, C.c_int, C.POINTER(vp), C.POINTER(vp)]
     _libs[variant] = L
     return L
 
@@ -367,3 +399,119 @@ class AmpPcg:
 
     def __exit__(self, *exc):
         self.close()
+
+
+# ---- row-sharded solve (include/amp_pcg.h "row-sharded solve") ------------------------------------------------------
+def shard_plan(rowptr: np.ndarray, colidx: np.ndarray, world: int):
+    """amp_shard_plan: block-row partition of a HOST CSR pattern over `world` ranks; returns a list of Shard."""
+    L = load_library()
+    rowptr = np.ascontiguousarray(rowptr, dtype=np.int32)
+    colidx = np.ascontiguousarray(colidx, dtype=np.int32)
+    out = (Shard * int(world))()
+    rc = L.amp_shard_plan(len(rowptr) - 1, rowptr.ctypes.data, colidx.ctypes.data, int(world), out)
+    if rc != 0:
+        raise AmpPcgError(f"amp_shard_plan error {rc}: {_last_error(L)}")
+    return list(out)
+
+
+def shard_extract(rowptr: np.ndarray, colidx: np.ndarray, vals: np.ndarray, shard: Shard):
+    """amp_shard_extract: the block row of `shard` as HOST CSR arrays with columns shifted to [halo_lo | owned | halo_hi]."""
+    L = load_library()
+    rowptr = np.ascontiguousarray(rowptr, dtype=np.int32)
+    colidx = np.ascontiguousarray(colidx, dtype=np.int32)
+    vals = np.ascontiguousarray(vals, dtype=np.float64)
+    rows = int(shard.row1 - shard.row0)
+    rp = np.empty(rows + 1, dtype=np.int32)
+    ci = np.empty(max(int(shard.nnz), 1), dtype=np.int32)
+    va = np.empty(max(int(shard.nnz), 1), dtype=np.float64)
+    rc = L.amp_shard_extract(len(rowptr) - 1, rowptr.ctypes.data, colidx.ctypes.data, vals.ctypes.data, C.byref(shard),
+                             rp.ctypes.data, ci.ctypes.data, va.ctypes.data)
+    if rc != 0:
+        raise AmpPcgError(f"amp_shard_extract error {rc}: {_last_error(L)}")
+    return rp, ci[:int(shard.nnz)], va[:int(shard.nnz)]
+
+
+def _vp_array(ptrs):
+    return (C.c_void_p * len(ptrs))(*[C.c_void_p(int(p)) for p in ptrs])
+
+
+class ShardGroup:
+    """The ranks of a sharded system that THIS process drives: all of them (``attach_local``: handles on one device or
+    on peer-accessible devices) or one (``attach_ipc``: one process per GPU; the export blobs are all-gathered by the
+    caller, e.g. with torch.distributed).  Argument marshalling only."""
+
+    def __init__(self, handles):
+        self.handles = list(handles)
+        self._L = self.handles[0]._L
+        self._torch = self.handles[0]._torch
+
+    @classmethod
+    def attach_local(cls, handles) -> "ShardGroup":
+        g = cls(handles)
+        arr = _vp_array([h._h for h in g.handles])
+        rc = g._L.amp_pcg_shard_attach_local(arr, len(g.handles))
+        if rc != 0:
+            raise AmpPcgError(f"amp_pcg_shard_attach_local error {rc}: {_last_error(g._L)}")
+        return g
+
+    @staticmethod
+    def export(handle) -> bytes:
+        """amp_pcg_shard_export: this rank's blob (bytes) for the all-gather."""
+        e = ShardExport()
+        rc = handle._L.amp_pcg_shard_export(handle._h, C.byref(e))
+        if rc != 0:
+            raise AmpPcgError(f"amp_pcg_shard_export error {rc}: {_last_error(handle._L)}")
+        return bytes(e)
+
+    @classmethod
+    def attach_ipc(cls, handle, rank: int, blobs) -> "ShardGroup":
+        """amp_pcg_shard_attach: blobs[r] = export() of rank r, for every rank of the group."""
+        g = cls([handle])
+        arr = (ShardExport * len(blobs))(*[ShardExport.from_buffer_copy(b) for b in blobs])
+        rc = g._L.amp_pcg_shard_attach(handle._h, int(rank), len(blobs), arr)
+        if rc != 0:
+            raise AmpPcgError(f"amp_pcg_shard_attach error {rc}: {_last_error(g._L)}")
+        return g
+
+    def _streams(self):
+        for h in self.handles:
+            with self._torch.cuda.device(h.device):
+                h._sync_stream()
+
+    def solve(self, b, x, tol: float, maxit: int, policy: Optional[Policy] = None):
+        """amp_pcg_solve_sharded: b[i], x[i] = float64 CUDA block rows of the local ranks; returns a list of Stats."""
+        torch = self._torch
+        for h, bi, xi in zip(self.handles, b, x):
+            if bi.dtype != torch.float64 or xi.dtype != torch.float64 or bi.numel() != h.n or xi.numel() != h.n or \
+                    not (bi.is_cuda and xi.is_cuda and bi.is_contiguous() and xi.is_contiguous()):
+                raise AmpPcgError("b[i] and x[i] must be contiguous float64 CUDA tensors with the rank's n entries")
+        st = (Stats * len(self.handles))()
+        self._streams()
+        rc = self._L.amp_pcg_solve_sharded(_vp_array([h._h for h in self.handles]), len(self.handles),
+                                           _vp_array([t.data_ptr() for t in b]), _vp_array([t.data_ptr() for t in x]),
+                                           float(tol), int(maxit), C.byref(policy) if policy is not None else None, st)
+        if rc not in (0, 1, -2):
+            raise AmpPcgError(f"amp_pcg_solve_sharded error {rc}: {_last_error(self._L)}")
+        for h, s in zip(self.handles, st):
+            h._last_iters = int(s.iters)
+        return list(st)
+
+    def spmv(self, p, mat_prec: int = FP64):
+        """amp_spmv_sharded: q = A p; p[i] = the local ranks' blocks (float64 / float32 / float16 CUDA tensors)."""
+        torch = self._torch
+        vec_prec = {torch.float64: FP64, torch.float32: FP32, torch.float16: FP16}[p[0].dtype]
+        qdt = torch.float64 if mat_prec == FP64 else torch.float32
+        q = [torch.empty(h.n, dtype=qdt, device=h.device) for h in self.handles]
+        for h, pi in zip(self.handles, p):
+            if pi.numel() != h.n or not pi.is_cuda or not pi.is_contiguous() or pi.dtype != p[0].dtype:
+                raise AmpPcgError("p[i] must be a contiguous CUDA tensor with the rank's n entries")
+        self._streams()
+        rc = self._L.amp_spmv_sharded(_vp_array([h._h for h in self.handles]), len(self.handles), int(mat_prec), vec_prec,
+                                      _vp_array([t.data_ptr() for t in p]), _vp_array([t.data_ptr() for t in q]))
+        if rc != 0:
+            raise AmpPcgError(f"amp_spmv_sharded error {rc}: {_last_error(self._L)}")
+        return q
+
+    def close(self):
+        for h in self.handles:
+            h.close()

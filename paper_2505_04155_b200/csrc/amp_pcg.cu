@@ -48,7 +48,7 @@ struct amp_pcg {
   int* h_flag = nullptr;        // pinned: done flag polled by the stream loop
   double* hist = nullptr;
   int64_t hist_cap = 0;
-  int vec_grid = 1, grid_z = 1, grid_p = 1, grid_xr = 1, spmv_grid = 1, persist_grid = 0, persist_ok = 0;
+  int vec_grid = 1, grid_z = 1, grid_p = 1, grid_p_sh = 1, grid_xr = 1, spmv_grid = 1, persist_grid = 0, persist_ok = 0;
   // graph loop
   cudaGraph_t graph = nullptr;
   cudaGraphExec_t graph_exec = nullptr;
@@ -82,7 +82,19 @@ struct amp_pcg {
   std::vector<int8_t> prof_kernel;       // kernel id of the launch that FOLLOWS event i (-1: end of an iteration)
   std::vector<int32_t> prof_iter;        // iteration index the launch belongs to
   std::vector<amp_kernel_time_t> prof_result;
+  // row-sharded solve (block row of a larger system; include/amp_pcg.h "row-sharded solve")
+  int64_t halo_lo = 0, halo_hi = 0;
+  void* p_base[3] = {nullptr, nullptr, nullptr};  // allocations behind ctx.p64 / p32 / p16 (guard band included)
+  char* xchg = nullptr;                  // exchange block: mailbox [kMailEntries] then 2 halo flags (owned, zeroed once)
+  ShardCtx* d_shard = nullptr;           // device copy of the peer table (owned)
+  int shard_rank = -1, shard_world = 0;  // set by amp_pcg_shard_attach*
+  unsigned int shard_epoch = 0;          // sharded solves / mat-vecs made so far (identical on all ranks of the group)
+  std::vector<void*> ipc_opened;         // peer allocations opened with cudaIpcOpenMemHandle
+  cudaGraph_t graph_sh[2] = {nullptr, nullptr};          // [lagged] graph loops of the sharded solve
+  cudaGraphExec_t graph_sh_exec[2] = {nullptr, nullptr};
+  cudaGraphConditionalHandle cond_sh[2] = {};
 };
+constexpr size_t kXchgBytes = sizeof(Mail) * kMailEntries + 64;
 
 template <class T> static T* dev_alloc(amp_pcg* h, size_t count, bool zero) {
   void* p = nullptr;
@@ -155,6 +167,11 @@ extern "C" void amp_pcg_destroy(amp_pcg_t* h) {
   if (h->graph) cudaGraphDestroy(h->graph);
   if (h->graph_lag_exec) cudaGraphExecDestroy(h->graph_lag_exec);
   if (h->graph_lag) cudaGraphDestroy(h->graph_lag);
+  for (int i = 0; i < 2; ++i) {
+    if (h->graph_sh_exec[i]) cudaGraphExecDestroy(h->graph_sh_exec[i]);
+    if (h->graph_sh[i]) cudaGraphDestroy(h->graph_sh[i]);
+  }
+  for (void* p : h->ipc_opened) cudaIpcCloseMemHandle(p);
   for (void* p : h->owned) cudaFree(p);
   if (h->hist) cudaFree(h->hist);
   if (h->h_state) cudaFreeHost(h->h_state);
@@ -180,6 +197,8 @@ extern "C" void amp_create_opts_default(amp_create_opts_t* o) {
   o->cheb_lmin = 0.0;
   o->cheb_lmax = 0.0;
   o->stream = nullptr;
+  o->halo_lo = 0;
+  o->halo_hi = 0;
 }
 
 extern "C" amp_pcg_t* amp_pcg_create(int64_t n, int64_t nnz, const int32_t* rowptr, const int32_t* colidx,
@@ -207,6 +226,11 @@ extern "C" amp_pcg_t* amp_pcg_create_ex(int64_t n, int64_t nnz, const int32_t* r
   if (o.index_format < AMP_INDEX_AUTO || o.index_format > AMP_INDEX_FORCE32 || o.spmv_kernel < AMP_SPMV_AUTO ||
       o.spmv_kernel > AMP_SPMV_PIPELINED || o.spmv_grid_mult < 0 || (o.pdl != 0 && o.pdl != 1)) {
     set_error("amp_pcg_create_ex: invalid index_format / spmv_kernel / spmv_grid_mult / pdl");
+    return nullptr;
+  }
+  if (o.halo_lo < 0 || o.halo_hi < 0 || (o.halo_lo & 7) || (o.halo_hi & 7) || o.halo_lo > (1 << 26) || o.halo_hi > (1 << 26) ||
+      ((o.halo_lo > 0 || o.halo_hi > 0) && precond == AMP_PRECOND_CHEBJACOBI)) {
+    set_error("amp_pcg_create_ex: halo_lo / halo_hi must be multiples of 8 in [0, 2^26] (not available with AMP_PRECOND_CHEBJACOBI)");
     return nullptr;
   }
   if (n <= 0 || n > (int64_t)0x7fffffff - 64 || nnz < 0 || nnz > (int64_t)0x7fffffff - 64) {
@@ -242,8 +266,11 @@ extern "C" amp_pcg_t* amp_pcg_create_ex(int64_t n, int64_t nnz, const int32_t* r
   h->num_sms = prop.multiProcessorCount;
   h->n = n; h->nnz = nnz; h->npad = (n + 7) & ~(int64_t)7; h->precond = precond;
   h->m_avg = (double)nnz / (double)n;
+  h->halo_lo = o.halo_lo; h->halo_hi = o.halo_hi;
   Ctx& c = h->ctx;
   c.n = n; c.npad = h->npad; c.nnz = nnz;
+  c.col_shift = (int32_t)o.halo_lo;
+  c.n_scale = n;
   c.rowptr = rowptr; c.colidx = colidx; c.vals64 = vals;
 
 #define ALLOC(dst, T, count)                                            \
@@ -269,8 +296,8 @@ extern "C" amp_pcg_t* amp_pcg_create_ex(int64_t n, int64_t nnz, const int32_t* r
 
   // structure check + 1/diag, FP32 value copy
   const int vgrid = (int)std::min<int64_t>((n + 255) / 256, (int64_t)h->num_sms * 16);
-  k_validate_dinv<<<vgrid, 256, 0, h->stream>>>(n, nnz, rowptr, colidx, vals, precond != AMP_PRECOND_NONE, dinv64,
-                                                dinv32, flags);
+  k_validate_dinv<<<vgrid, 256, 0, h->stream>>>(n, nnz, n + o.halo_lo + o.halo_hi, o.halo_lo, rowptr, colidx, vals,
+                                                precond != AMP_PRECOND_NONE, dinv64, dinv32, flags);
   std::vector<int32_t> rp((size_t)n + 1);
   int hflags = 0;
   CU_TRY(cudaMemcpyAsync(&hflags, flags, sizeof(int), cudaMemcpyDeviceToHost, h->stream), { amp_pcg_destroy(h); return nullptr; });
@@ -351,7 +378,8 @@ extern "C" amp_pcg_t* amp_pcg_create_ex(int64_t n, int64_t nnz, const int32_t* r
              { amp_pcg_destroy(h); return nullptr; });
     const int pgrid = (int)((nsl * 32 + 255) / 256);
     const int allow_aligned = (o.index_format == AMP_INDEX_AUTO) ? 1 : 0;
-    k_sell_scan<<<pgrid, 256, 0, h->stream>>>((int)n, (int)nsl, long_min, allow_aligned, rowptr, colidx, perm_d, width_d);
+    k_sell_scan<<<pgrid, 256, 0, h->stream>>>((int)n, (int)nsl, long_min, allow_aligned, (int)o.halo_lo, rowptr, colidx, perm_d,
+                                             width_d);
     std::vector<int32_t> width((size_t)nsl);
     CU_TRY(cudaMemcpyAsync(width.data(), width_d, sizeof(int32_t) * (size_t)nsl, cudaMemcpyDeviceToHost, h->stream),
            { amp_pcg_destroy(h); return nullptr; });
@@ -385,8 +413,8 @@ extern "C" amp_pcg_t* amp_pcg_create_ex(int64_t n, int64_t nnz, const int32_t* r
     ALLOC(v32_d, float, total);
     CU_TRY(cudaMemcpyAsync(wptr_d, wptr.data(), sizeof(int32_t) * wptr.size(), cudaMemcpyHostToDevice, h->stream),
            { amp_pcg_destroy(h); return nullptr; });
-    k_sell_pack<<<pgrid, 256, 0, h->stream>>>((int)n, (int)nsl, long_min, rowptr, colidx, vals, wptr_d, perm_d, cols_d,
-                                             cols16_d, base_d, v64_d, v32_d, flag16_d);
+    k_sell_pack<<<pgrid, 256, 0, h->stream>>>((int)n, (int)nsl, long_min, (int)o.halo_lo, rowptr, colidx, vals, wptr_d, perm_d,
+                                             cols_d, cols16_d, base_d, v64_d, v32_d, flag16_d);
     int wide = 0, maxbase = 0;
     int* maxbase_d;
     ALLOC(maxbase_d, int, 1);
@@ -481,10 +509,16 @@ extern "C" amp_pcg_t* amp_pcg_create_ex(int64_t n, int64_t nnz, const int32_t* r
       }
     }
     {  // p and z (both are gathered by a mat-vec: z inside the Chebyshev-Jacobi preconditioner) in their three storage
-       // precisions, with the zero guard band on both sides (0 elements unless pipelined)
+       // precisions, with the zero guard band on both sides (0 elements unless pipelined); a block row of a sharded
+       // system keeps its halo bands there (the guard covers them)
+      const int64_t halo = ((std::max(o.halo_lo, o.halo_hi) + 127) / 128) * 128;
+      h->guard = std::max(h->guard, halo);
       const size_t g = (size_t)h->guard;
+      c.col_min = -(int32_t)h->guard;
+      c.col_max = (int32_t)(n - 1 + h->guard);
       double* b64; float* b32; __half* b16;
       ALLOC(b64, double, np + 2 * g); ALLOC(b32, float, np + 2 * g); ALLOC(b16, __half, np + 2 * g);
+      h->p_base[0] = b64; h->p_base[1] = b32; h->p_base[2] = b16;
       c.p64 = b64 + g; c.p32 = b32 + g; c.p16 = b16 + g;
       ALLOC(b64, double, np + 2 * g); ALLOC(b32, float, np + 2 * g); ALLOC(b16, __half, np + 2 * g);
       c.z64 = b64 + g; c.z32 = b32 + g; c.z16 = b16 + g;
@@ -547,6 +581,7 @@ extern "C" amp_pcg_t* amp_pcg_create_ex(int64_t n, int64_t nnz, const int32_t* r
   };
   h->grid_z = vec_grid_for((const void*)k_z);
   h->grid_p = vec_grid_for((const void*)k_p);
+  h->grid_p_sh = vec_grid_for((const void*)k_p_sh);
   h->grid_xr = vec_grid_for((const void*)k_xr);
   h->grid_xrz = vec_grid_for((const void*)k_xrz);
   h->grid_cheb0 = vec_grid_for((const void*)k_cheb0);
@@ -566,21 +601,27 @@ extern "C" int64_t amp_pcg_last_launch_count(const amp_pcg_t* h) { return h ? h-
 
 // ------------------------------------------------------------------ SpMV entry --------------
 template <int UR, class PT>
-static void launch_spmv_any(amp_pcg* h, const void* p, void* q) {
+static void launch_spmv_any(amp_pcg* h, const void* p, void* q, unsigned int halo_seq) {
+  Ctx c = h->ctx;
+  if (halo_seq == 0u) {  // p is a caller's vector of exactly n entries: no halo bands, no guard band around it
+    c.col_min = 0;
+    c.col_max = (int32_t)(h->n - 1);
+  }
   k_spmv_any<UR, PT><<<h->spmv_grid, kSpmvThreads, 0, h->stream>>>(
-      h->ctx, static_cast<const PT*>(p), static_cast<typename Store<UR>::T*>(q));
+      c, static_cast<const PT*>(p), static_cast<typename Store<UR>::T*>(q), halo_seq);
 }
 
-static int spmv_dispatch(amp_pcg* h, int mat_prec, int vec_prec, const void* p, void* q) {
+// halo_seq != 0 (row-sharded solve): p is the handle's own extended p vector; wait for the neighbours' push first
+static int spmv_dispatch(amp_pcg* h, int mat_prec, int vec_prec, const void* p, void* q, unsigned int halo_seq = 0u) {
   if (mat_prec == AMP_FP64) {
-    if (vec_prec == AMP_FP64) launch_spmv_any<P64, double>(h, p, q);
-    else if (vec_prec == AMP_FP32) launch_spmv_any<P64, float>(h, p, q);
-    else if (vec_prec == AMP_FP16) launch_spmv_any<P64, __half>(h, p, q);
+    if (vec_prec == AMP_FP64) launch_spmv_any<P64, double>(h, p, q, halo_seq);
+    else if (vec_prec == AMP_FP32) launch_spmv_any<P64, float>(h, p, q, halo_seq);
+    else if (vec_prec == AMP_FP16) launch_spmv_any<P64, __half>(h, p, q, halo_seq);
     else return AMP_ERR_INVALID;
   } else if (mat_prec == AMP_FP32) {
-    if (vec_prec == AMP_FP64) launch_spmv_any<P32, double>(h, p, q);
-    else if (vec_prec == AMP_FP32) launch_spmv_any<P32, float>(h, p, q);
-    else if (vec_prec == AMP_FP16) launch_spmv_any<P32, __half>(h, p, q);
+    if (vec_prec == AMP_FP64) launch_spmv_any<P32, double>(h, p, q, halo_seq);
+    else if (vec_prec == AMP_FP32) launch_spmv_any<P32, float>(h, p, q, halo_seq);
+    else if (vec_prec == AMP_FP16) launch_spmv_any<P32, __half>(h, p, q, halo_seq);
     else return AMP_ERR_INVALID;
   } else {
     return AMP_ERR_INVALID;
@@ -592,6 +633,10 @@ static int spmv_dispatch(amp_pcg* h, int mat_prec, int vec_prec, const void* p, 
 extern "C" int amp_spmv(amp_pcg_t* h, int mat_prec, int vec_prec, const void* p, void* q) {
   g_last_error.clear();
   if (!h || !p || !q) { set_error("amp_spmv: null argument"); return AMP_ERR_INVALID; }
+  if (h->halo_lo > 0 || h->halo_hi > 0 || h->shard_world > 0) {
+    set_error("amp_spmv: this handle is a block row of a sharded system; use amp_spmv_sharded");
+    return AMP_ERR_INVALID;
+  }
   CU_TRY(cudaSetDevice(h->device), return AMP_ERR_CUDA);
   h->launches = 0;
   const int rc = spmv_dispatch(h, mat_prec, vec_prec, p, q);
@@ -689,10 +734,12 @@ static cudaError_t launch_iteration_lagged(amp_pcg* h, const Ctx& c, cudaStream_
 
 // One graph = one WHILE conditional node whose body is the four loop kernels; the condition is
 // written from the device by epi_delta / epi_gamma, so a whole solve is a single launch.
-static int build_graph_once(amp_pcg* h, bool pdl, bool lagged) {
-  cudaGraph_t& graph = lagged ? h->graph_lag : h->graph;
-  cudaGraphExec_t& graph_exec = lagged ? h->graph_lag_exec : h->graph_exec;
-  cudaGraphConditionalHandle& cond = lagged ? h->cond_lag : h->cond;
+static cudaError_t launch_iteration_sharded(amp_pcg* h, const Ctx& c, cudaStream_t s, bool pdl, bool lagged);
+
+static int build_graph_once(amp_pcg* h, bool pdl, bool lagged, bool sharded) {
+  cudaGraph_t& graph = sharded ? h->graph_sh[lagged] : (lagged ? h->graph_lag : h->graph);
+  cudaGraphExec_t& graph_exec = sharded ? h->graph_sh_exec[lagged] : (lagged ? h->graph_lag_exec : h->graph_exec);
+  cudaGraphConditionalHandle& cond = sharded ? h->cond_sh[lagged] : (lagged ? h->cond_lag : h->cond);
   CU_TRY(cudaGraphCreate(&graph, 0), return AMP_ERR_CUDA);
   CU_TRY(cudaGraphConditionalHandleCreate(&cond, graph, 1, cudaGraphCondAssignDefault), return AMP_ERR_CUDA);
   cudaGraphNodeParams np = {};
@@ -710,7 +757,8 @@ static int build_graph_once(amp_pcg* h, bool pdl, bool lagged) {
   c.use_cond = 1;
   cudaError_t e = cudaStreamBeginCaptureToGraph(cap, body, nullptr, nullptr, 0, cudaStreamCaptureModeRelaxed);
   if (e == cudaSuccess) {
-    const cudaError_t el = lagged ? launch_iteration_lagged(h, c, cap, pdl) : launch_iteration(h, c, cap, pdl);
+    const cudaError_t el = sharded ? launch_iteration_sharded(h, c, cap, pdl, lagged)
+                                   : (lagged ? launch_iteration_lagged(h, c, cap, pdl) : launch_iteration(h, c, cap, pdl));
     e = cudaStreamEndCapture(cap, nullptr);
     if (e == cudaSuccess) e = el;
   }
@@ -720,41 +768,50 @@ static int build_graph_once(amp_pcg* h, bool pdl, bool lagged) {
   return AMP_OK;
 }
 
-static int build_graph(amp_pcg* h, bool lagged) {
-  cudaGraph_t& graph = lagged ? h->graph_lag : h->graph;
-  cudaGraphExec_t& graph_exec = lagged ? h->graph_lag_exec : h->graph_exec;
+static int build_graph(amp_pcg* h, bool lagged, bool sharded = false) {
+  cudaGraph_t& graph = sharded ? h->graph_sh[lagged] : (lagged ? h->graph_lag : h->graph);
+  cudaGraphExec_t& graph_exec = sharded ? h->graph_sh_exec[lagged] : (lagged ? h->graph_lag_exec : h->graph_exec);
   if (graph_exec) return AMP_OK;
-  int rc = build_graph_once(h, h->pdl != 0, lagged);
+  int rc = build_graph_once(h, h->pdl != 0, lagged, sharded);
   if (rc != AMP_OK && h->pdl) {  // programmatic edges not accepted inside the conditional body: plain edges
     if (graph_exec) { cudaGraphExecDestroy(graph_exec); graph_exec = nullptr; }
     if (graph) { cudaGraphDestroy(graph); graph = nullptr; }
     h->pdl = 0;
-    rc = build_graph_once(h, false, lagged);
+    rc = build_graph_once(h, false, lagged, sharded);
   }
   return rc;
 }
 
 // ------------------------------------------------------------------ solve -------------------
-static int solve_impl(amp_pcg* h, const double* b, double* x, double tol, int32_t maxit, const amp_policy_t* policy,
-                      amp_stats_t* stats) {
-  g_last_error.clear();
-  if (!h || !b || !x) { set_error("amp_pcg_solve: null argument"); return AMP_ERR_INVALID; }
+// policy with its "0 means default" fields resolved; false = invalid tol / maxit / policy
+static bool resolve_policy(const amp_policy_t* policy, double tol, int32_t maxit, amp_policy_t* out) {
   amp_policy_t pol;
   if (policy) pol = *policy; else amp_policy_default(&pol);
   if (pol.eps32 == 0.0) pol.eps32 = std::ldexp(1.0, -24);
   if (pol.eta_safety == 0.0) pol.eta_safety = 1.0;
   if (pol.stop_safety == 0.0) pol.stop_safety = 1.0;
   if (pol.C == 0.0 && !policy) pol.C = 1.0;
-  if (!(tol > 0.0) || maxit < 1 || maxit > (1 << 24) || !aligned16(b) || !aligned16(x) || pol.u0 < 0 || pol.u0 > 2 ||
-      pol.eta_rule < 0 || pol.eta_rule > 2 || pol.scale_mode < 0 || pol.scale_mode > 4 || pol.d < 1 || pol.d > kMaxWindow ||
-      pol.ell < 1 || pol.ell > kMaxWindow || pol.loop_mode < 0 || pol.loop_mode > 3 || !(pol.tau_zs >= 0.0) ||
-      !(pol.tau_zh >= 0.0) || !(pol.eps32 > 0.0) || !(pol.eta_safety > 0.0) || !(pol.stop_safety > 0.0) ||
-      (pol.profile_kernels != 0 && pol.loop_mode != AMP_LOOP_STREAM)) {
-    set_error("amp_pcg_solve: invalid tol/maxit/policy or misaligned b/x");
-    return AMP_ERR_INVALID;
-  }
-  CU_TRY(cudaSetDevice(h->device), return AMP_ERR_CUDA);
-  cudaStream_t st = h->stream;
+  *out = pol;
+  return !(!(tol > 0.0) || maxit < 1 || maxit > (1 << 24) || pol.u0 < 0 || pol.u0 > 2 ||
+           pol.eta_rule < 0 || pol.eta_rule > 2 || pol.scale_mode < 0 || pol.scale_mode > 4 || pol.d < 1 || pol.d > kMaxWindow ||
+           pol.ell < 1 || pol.ell > kMaxWindow || pol.loop_mode < 0 || pol.loop_mode > 3 || !(pol.tau_zs >= 0.0) ||
+           !(pol.tau_zh >= 0.0) || !(pol.eps32 > 0.0) || !(pol.eta_safety > 0.0) || !(pol.stop_safety > 0.0) ||
+           (pol.profile_kernels != 0 && pol.loop_mode != AMP_LOOP_STREAM));
+}
+
+// the host-written part of the device state of one solve
+static void fill_state(DevState* hs, const amp_pcg* h, const double* b, double* x, double tol, int32_t maxit, const amp_policy_t& pol) {
+  std::memset(hs, 0, sizeof(DevState));
+  hs->b = b; hs->x = x; hs->hist = h->hist;
+  hs->tol = tol; hs->tau_zs = pol.tau_zs; hs->tau_zh = pol.tau_zh; hs->eps32 = pol.eps32; hs->C = pol.C;
+  hs->eta_safety = pol.eta_safety; hs->stop_safety = pol.stop_safety;
+  hs->amp = pol.amp ? 1 : 0; hs->u0 = pol.u0; hs->eta_rule = pol.eta_rule; hs->d = pol.d; hs->ell = pol.ell;
+  hs->scale_mode = pol.scale_mode; hs->no_stop = pol.no_stop ? 1 : 0; hs->maxit = maxit;
+  hs->status = AMP_MAXIT; hs->it_ur32 = hs->it_uz32 = hs->it_uz16 = -1;
+  hs->relres_true = -1.0;
+}
+
+static int ensure_hist(amp_pcg* h, int32_t maxit) {
   if ((int64_t)maxit + 2 > h->hist_cap) {
     if (h->hist) cudaFree(h->hist);
     h->hist = nullptr;
@@ -762,6 +819,54 @@ static int solve_impl(amp_pcg* h, const double* b, double* x, double tol, int32_
     CU_TRY(cudaMalloc(&h->hist, sizeof(double) * ((size_t)maxit + 2)), return AMP_ERR_NOMEM);
     h->hist_cap = (int64_t)maxit + 2;
   }
+  return AMP_OK;
+}
+
+// precisions in use at iteration k (from the switch iterations)
+static void phase_of(const DevState* hs, int k, int& uz, int& ur) {
+  ur = (hs->it_ur32 >= 0 && k >= hs->it_ur32) ? AMP_FP32 : AMP_FP64;
+  uz = hs->amp ? hs->u0 : AMP_FP64;
+  if (hs->it_uz32 >= 0 && k >= hs->it_uz32) uz = std::max(uz, (int)AMP_FP32);
+  if (hs->it_uz16 >= 0 && k >= hs->it_uz16) uz = AMP_FP16;
+}
+
+static void fill_stats(const amp_pcg* h, const DevState* hs, int mode, bool lagged, float ms, amp_stats_t* stats) {
+  const int iters = hs->k;
+  std::memset(stats, 0, sizeof(*stats));
+  stats->status = hs->status; stats->iters = iters;
+  stats->it_ur32 = hs->it_ur32; stats->it_uz32 = hs->it_uz32; stats->it_uz16 = hs->it_uz16;
+  stats->loop_mode = mode;
+  stats->bnorm = hs->bnorm;
+  stats->relres_updated = (hs->bnorm > 0.0) ? hs->delta / hs->bnorm : 0.0;
+  stats->relres_true = hs->relres_true;
+  stats->solve_ms = ms;
+  double bytes = 0.0;
+  for (int k = 0; k < iters; ++k) {
+    int uz, ur;
+    phase_of(hs, k, uz, ur);
+    bytes += amp_pcg_iteration_bytes(h, uz, ur);
+    if (lagged) bytes -= (double)h->n * ((ur == AMP_FP64) ? 8.0 : 4.0);  // r is not read a second time
+  }
+  stats->algorithmic_bytes = bytes;
+  stats->fp16_subnormal = hs->fp16_subnormal; stats->fp16_flushed = hs->fp16_flushed; stats->fp16_inf = hs->fp16_inf;
+}
+
+static int solve_impl(amp_pcg* h, const double* b, double* x, double tol, int32_t maxit, const amp_policy_t* policy,
+                      amp_stats_t* stats) {
+  g_last_error.clear();
+  if (!h || !b || !x) { set_error("amp_pcg_solve: null argument"); return AMP_ERR_INVALID; }
+  if (h->halo_lo > 0 || h->halo_hi > 0 || h->shard_world > 0) {
+    set_error("amp_pcg_solve: this handle is a block row of a sharded system; use amp_pcg_solve_sharded");
+    return AMP_ERR_INVALID;
+  }
+  amp_policy_t pol;
+  if (!resolve_policy(policy, tol, maxit, &pol) || !aligned16(b) || !aligned16(x)) {
+    set_error("amp_pcg_solve: invalid tol/maxit/policy or misaligned b/x");
+    return AMP_ERR_INVALID;
+  }
+  CU_TRY(cudaSetDevice(h->device), return AMP_ERR_CUDA);
+  cudaStream_t st = h->stream;
+  { const int rc = ensure_hist(h, maxit); if (rc != AMP_OK) return rc; }
   int mode = pol.loop_mode;
   // measured on B200 (us per iteration, persistent vs graph): n = 4 K 17 vs 23, 16 K 19.6 vs 24.0, 262 K 20.9 vs 29.0,
   // 512 K 25.0 vs 32.1, 2.1 M (c2) 58 vs 57, 4.1 M (c3) 95 vs 92: the persistent kernel wins while the iteration is
@@ -780,14 +885,7 @@ static int solve_impl(amp_pcg* h, const double* b, double* x, double tol, int32_
   if (mode == AMP_LOOP_GRAPH) { const int rc = build_graph(h, lagged); if (rc != AMP_OK) return rc; }
 
   DevState* hs = h->h_state;
-  std::memset(hs, 0, sizeof(DevState));
-  hs->b = b; hs->x = x; hs->hist = h->hist;
-  hs->tol = tol; hs->tau_zs = pol.tau_zs; hs->tau_zh = pol.tau_zh; hs->eps32 = pol.eps32; hs->C = pol.C;
-  hs->eta_safety = pol.eta_safety; hs->stop_safety = pol.stop_safety;
-  hs->amp = pol.amp ? 1 : 0; hs->u0 = pol.u0; hs->eta_rule = pol.eta_rule; hs->d = pol.d; hs->ell = pol.ell;
-  hs->scale_mode = pol.scale_mode; hs->no_stop = pol.no_stop ? 1 : 0; hs->maxit = maxit;
-  hs->status = AMP_MAXIT; hs->it_ur32 = hs->it_uz32 = hs->it_uz16 = -1;
-  hs->relres_true = -1.0;
+  fill_state(hs, h, b, x, tol, maxit, pol);
   h->launches = 0;
   const bool profile = pol.profile_kernels != 0;
   h->prof_used = 0;
@@ -845,12 +943,6 @@ static int solve_impl(amp_pcg* h, const double* b, double* x, double tol, int32_
 
   const int iters = hs->k;
   h->last_iters = iters;
-  auto phase_of = [&](int k, int& uz, int& ur) {  // precisions in use at iteration k (from the switch iterations)
-    ur = (hs->it_ur32 >= 0 && k >= hs->it_ur32) ? AMP_FP32 : AMP_FP64;
-    uz = hs->amp ? hs->u0 : AMP_FP64;
-    if (hs->it_uz32 >= 0 && k >= hs->it_uz32) uz = std::max(uz, (int)AMP_FP32);
-    if (hs->it_uz16 >= 0 && k >= hs->it_uz16) uz = AMP_FP16;
-  };
   if (profile) {  // event-to-event device time of every executed loop kernel, summed per (kernel, u_z, u_r)
     amp_kernel_time_t acc[AMP_K_COUNT][3][2];
     std::memset(acc, 0, sizeof(acc));
@@ -860,7 +952,7 @@ static int solve_impl(amp_pcg* h, const double* b, double* x, double tol, int32_
       float dt = 0.f;
       if (cudaEventElapsedTime(&dt, h->prof_events[i], h->prof_events[i + 1]) != cudaSuccess) { cudaGetLastError(); continue; }
       int uz, ur;
-      phase_of(k, uz, ur);
+      phase_of(hs, k, uz, ur);
       acc[kern][uz][ur].launches += 1;
       acc[kern][uz][ur].total_ms += dt;
     }
@@ -889,27 +981,11 @@ static int solve_impl(amp_pcg* h, const double* b, double* x, double tol, int32_
     const int per_it = (lagged ? 2 : 3) + spmv_k + (sweeps - 1) * (spmv_k + 1);  // vector kernels + a4 + extra sweeps
     h->launches += (mode == AMP_LOOP_PERSISTENT) ? 1 : (int64_t)per_it * iters;
   }
-  if (stats) {
-    std::memset(stats, 0, sizeof(*stats));
-    stats->status = hs->status; stats->iters = iters;
-    stats->it_ur32 = hs->it_ur32; stats->it_uz32 = hs->it_uz32; stats->it_uz16 = hs->it_uz16;
-    stats->loop_mode = mode;
-    stats->bnorm = hs->bnorm;
-    stats->relres_updated = (hs->bnorm > 0.0) ? hs->delta / hs->bnorm : 0.0;
-    stats->relres_true = hs->relres_true;
-    stats->solve_ms = ms;
-    double bytes = 0.0;
-    for (int k = 0; k < iters; ++k) {
-      int uz, ur;
-      phase_of(k, uz, ur);
-      bytes += amp_pcg_iteration_bytes(h, uz, ur);
-      if (lagged) bytes -= (double)h->n * ((ur == AMP_FP64) ? 8.0 : 4.0);  // r is not read a second time
-    }
-    stats->algorithmic_bytes = bytes;
-    stats->fp16_subnormal = hs->fp16_subnormal; stats->fp16_flushed = hs->fp16_flushed; stats->fp16_inf = hs->fp16_inf;
-  }
+  if (stats) fill_stats(h, hs, mode, lagged, ms, stats);
   return hs->status;
 }
+
+#include "shard_host.cuh"
 
 extern "C" int amp_pcg_solve(amp_pcg_t* h, const double* b, double* x, double tol, int32_t maxit,
                              const amp_policy_t* policy, amp_stats_t* stats) {

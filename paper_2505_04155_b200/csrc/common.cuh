@@ -24,6 +24,7 @@ constexpr int kPersistMinBlocks = 1;           // resident blocks per SM its reg
 constexpr int kMaxGrid = 8192;                 // capacity of each partial-sum array
 constexpr int kMaxWindow = 64;                 // max d / ell of the indicators
 constexpr int kMaxChebDegree = 16;             // max sweeps of the Chebyshev-Jacobi preconditioner
+constexpr int kMaxWorld = 16;                  // max ranks of a row-sharded solve (= AMP_SHARD_MAX_WORLD)
 
 // Scalars of one solve, resident in device memory.  The host writes the policy part before the
 // loop and reads the whole block once after it; inside the loop only kernels touch it.
@@ -43,11 +44,31 @@ struct DevState {
   // lagged variant (AMP_SCALE_LAGGED): decisions already taken for the NEXT iteration
   int32_t ur_n, uz_n;
   double omega_n;
-  unsigned int counter[4];  // last-block tickets of the three reductions (+ setup)
+  // row-sharded solve: number of cross-rank reductions completed in this solve (written by k_epi only) and the solve
+  // counter of the group (host-written); together they tag every mailbox entry and halo flag
+  unsigned int xseq, epoch;
+  unsigned int counter[4];  // last-block tickets of the three reductions (+ setup; + the halo push of the p update)
   unsigned long long fp16_subnormal, fp16_flushed, fp16_inf;
   // ---- grid barrier of the persistent kernel: arrivals since the start of the solve (host-zeroed); never
   //      written back from a block's replica ----
   unsigned int bar_count, bar_pad;
+};
+
+// Row-sharded solve (shard.cuh): what a rank needs to reach its peers.  One entry of a mailbox = one rank's partial sums
+// of one reduction point; 2 halves (solve parity) x 4 slots (reduction sequence number mod 4) x kMaxWorld senders.
+struct Mail { double v0, v1; unsigned long long tag, pad; };
+constexpr int kMailSlots = 4;
+constexpr int kMailEntries = 2 * kMailSlots * kMaxWorld;
+struct ShardCtx {
+  int32_t rank, world;
+  int32_t send_lo, send_hi;            // entries of p pushed to rank-1 (its upper halo) / rank+1 (its lower halo); multiples of 8
+  Mail* mbox;                          // this rank's mailbox [kMailEntries]
+  Mail* peer_mbox[kMaxWorld];          // every rank's mailbox (own included), peer-mapped
+  unsigned long long* flags;           // this rank's halo flags: [0] set by rank-1 (lower band complete), [1] by rank+1
+  unsigned long long* peer_flag_lo;    // flags[1] of rank-1, or nullptr
+  unsigned long long* peer_flag_hi;    // flags[0] of rank+1, or nullptr
+  char* peer_lo_band[3];               // [precision] where this rank's entry 0 goes in rank-1's p vector (its p + its n)
+  char* peer_hi_band[3];               // [precision] where this rank's entry n - send_hi goes in rank+1's p vector (its p - send_hi)
 };
 
 // Handle-lifetime constants, passed to every kernel by value.
@@ -90,6 +111,12 @@ struct Ctx {
   double cheb_c1[kMaxChebDegree], cheb_c2[kMaxChebDegree];
   cudaGraphConditionalHandle cond;  // WHILE-node handle (graph loop only)
   int32_t use_cond;
+  // block row of a sharded system (create opts halo_lo / halo_hi): stored column indices are relative to the first owned
+  // entry of p, gathers may reach col_min .. col_max (halo bands, then zero guard); col_shift = halo_lo is subtracted from
+  // the borrowed CSR column indices (long rows)
+  int32_t col_shift, col_min, col_max;
+  int64_t n_scale;                  // rows of the WHOLE system (= n unless sharded): the n of the RMS scale sqrt(n)/||r||
+  const ShardCtx* sh;               // device pointer, nullptr unless attached to a group (amp_pcg_shard_attach*)
 };
 
 // Programmatic dependent launch (sm_90+): every loop kernel lets its successor start launching at
@@ -235,6 +262,32 @@ __host__ __device__ constexpr int chunk_elems(int smin, int smax) { return cmin(
 #define AMP_VEC_BIF 192
 #endif
 constexpr int kVecBytesInFlight = AMP_VEC_BIF;  // target bytes of loads in flight per thread of a vector kernel
+
+// Row-sharded solve: where the chunks of p that a neighbour needs go: element index e of this rank's p lands at lo[e] (e < send_lo) and at
+// hi[e - hi0] (e >= hi0 = n - send_hi)
+template <class T> struct HaloPush {
+  T* lo;
+  T* hi;
+  int64_t send_lo, hi0, n;
+};
+template <int P> __device__ __forceinline__ HaloPush<typename Store<P>::T> halo_push_of(const Ctx& c) {
+  using T = typename Store<P>::T;
+  HaloPush<T> h{nullptr, nullptr, 0, 0, 0};
+  const ShardCtx* sh = c.sh;
+  if (sh != nullptr) {
+    h.lo = reinterpret_cast<T*>(sh->peer_lo_band[P]);
+    h.hi = reinterpret_cast<T*>(sh->peer_hi_band[P]);
+    h.send_lo = h.lo ? sh->send_lo : 0;
+    h.n = c.n;
+    h.hi0 = h.hi ? c.n - sh->send_hi : c.npad;
+  }
+  return h;
+}
+template <class T, int E> __device__ __forceinline__ void halo_push_chunk(const HaloPush<T>& h, const Chunk<T, E>& k, int64_t chunk) {
+  const int64_t e = chunk * E;  // E divides 8 and the send ranges are multiples of 8: a chunk is inside a range or outside
+  if (e < h.send_lo) chunk_store(k, h.lo, chunk);
+  if (e >= h.hi0 && e < h.n) chunk_store(k, h.hi, chunk - h.hi0 / E);
+}
 
 // gather of one element of p as the SpMV working type.  COH = false: read-only path (p is not
 // written by the running kernel); COH = true: plain coherent load.

@@ -3,6 +3,7 @@
 // set-up / finalisation kernels, the stand-alone SpMV and the one-off kernels of create().
 #pragma once
 #include "phases.cuh"
+#include "shard.cuh"
 #include "spmv.cuh"
 
 #ifndef AMP_KZ_BLOCKS
@@ -40,16 +41,16 @@ __device__ __forceinline__ double dispatch_z(const Ctx& c, int rs, int ur, int u
   return phase_z<P32, P32, P16, BIF>(c, omega, bid, nb);
 }
 
-template <int BIF = kVecBytesInFlight>
+template <int BIF = kVecBytesInFlight, bool PUSH = false>
 __device__ __forceinline__ void dispatch_p(const Ctx& c, int ps, int uz, int ur, double beta, bool first, int bid, int nb) {
-  if (uz == P64) phase_p<P64, P64, BIF>(c, beta, first, ur == P32, bid, nb);
+  if (uz == P64) phase_p<P64, P64, BIF, PUSH>(c, beta, first, ur == P32, bid, nb);
   else if (uz == P32) {
-    if (ps == P64) phase_p<P64, P32, BIF>(c, beta, first, false, bid, nb);
-    else phase_p<P32, P32, BIF>(c, beta, first, false, bid, nb);
+    if (ps == P64) phase_p<P64, P32, BIF, PUSH>(c, beta, first, false, bid, nb);
+    else phase_p<P32, P32, BIF, PUSH>(c, beta, first, false, bid, nb);
   } else {
-    if (ps == P64) phase_p<P64, P16, BIF>(c, beta, first, false, bid, nb);
-    else if (ps == P32) phase_p<P32, P16, BIF>(c, beta, first, false, bid, nb);
-    else phase_p<P16, P16, BIF>(c, beta, first, false, bid, nb);
+    if (ps == P64) phase_p<P64, P16, BIF, PUSH>(c, beta, first, false, bid, nb);
+    else if (ps == P32) phase_p<P32, P16, BIF, PUSH>(c, beta, first, false, bid, nb);
+    else phase_p<P16, P16, BIF, PUSH>(c, beta, first, false, bid, nb);
   }
 }
 
@@ -99,8 +100,9 @@ __global__ void __launch_bounds__(kVecThreads, AMP_KZ_BLOCKS) k_z(const Ctx c) {
   if (s->done) return;
   const int bid = blockIdx.x, nb = gridDim.x;
   const double v = dispatch_z(c, s->r_store, s->ur, s->uz, s->omega, bid, nb);
+  // row-sharded solve (c.sh != nullptr): the partial sum goes to every rank's mailbox, k_epi runs the scalar step
   grid_reduce<kVecThreads>(v, c.partials + 0 * kMaxGrid, &s->counter[0], bid, nb, red,
-                           [&](double tot) { epi_rho(epi_ctx(c), tot); });
+                           [&](double tot) { if (c.sh != nullptr) shard_post(c, tot, 0.0); else epi_rho(epi_ctx(c), tot); });
 }
 
 __global__ void __launch_bounds__(kVecThreads, AMP_KP_BLOCKS) k_p(const Ctx c) {
@@ -111,6 +113,18 @@ __global__ void __launch_bounds__(kVecThreads, AMP_KP_BLOCKS) k_p(const Ctx c) {
   dispatch_p(c, s->p_store, s->uz, s->ur, s->beta, s->k == 0, blockIdx.x, gridDim.x);
 }
 
+// the p update of the row-sharded solve: the chunks of the send ranges also go straight into the neighbours' halo bands
+// (peer stores), then the block that finishes last raises the neighbours' flags
+__global__ void __launch_bounds__(kVecThreads, 2) k_p_sh(const Ctx c) {
+  DevState* s = c.st;
+  pdl_launch_dependents();
+  pdl_wait();
+  if (s->done) return;
+  const int k = s->k;
+  dispatch_p<kVecBytesInFlight, true>(c, s->p_store, s->uz, s->ur, s->beta, k == 0, blockIdx.x, gridDim.x);
+  shard_signal_halo(c, (unsigned int)k + 1u, &s->counter[3], (int)gridDim.x);
+}
+
 __global__ void __launch_bounds__(kSpmvThreads, kSpmvMinBlocks) k_spmv(const Ctx c, int zmode) {
   __shared__ double red[32];
   DevState* s = c.st;
@@ -119,10 +133,11 @@ __global__ void __launch_bounds__(kSpmvThreads, kSpmvMinBlocks) k_spmv(const Ctx
   if (s->done) return;
   if (c.use_pipe && s->ur == P32) return;  // this iteration's mat-vec is k_spmv_pipe's (next in the chain)
   const int bid = blockIdx.x, nb = gridDim.x;
+  if (c.sh != nullptr) shard_wait_halo(c, (unsigned int)s->k + 1u);  // the neighbours' entries of p are in the halo bands
   const double v = dispatch_spmv<false, kSpmvThreads>(c, s->ur, s->uz, zmode, bid, nb, red);
   if (zmode) return;  // q = A z inside M^-1: no inner product
   grid_reduce<kSpmvThreads>(v, c.partials + 1 * kMaxGrid, &s->counter[1], bid, nb, red,
-                            [&](double tot) { epi_gamma(epi_ctx(c), tot); });
+                            [&](double tot) { if (c.sh != nullptr) shard_post(c, tot, 0.0); else epi_gamma(epi_ctx(c), tot); });
 }
 
 __global__ void __launch_bounds__(kVecThreads, AMP_KXR_BLOCKS) k_xr(const Ctx c) {
@@ -137,7 +152,7 @@ __global__ void __launch_bounds__(kVecThreads, AMP_KXR_BLOCKS) k_xr(const Ctx c)
   const int bid = blockIdx.x, nb = gridDim.x;
   const double v = dispatch_xr(c, s->ur, s->uz, s->alpha, s->x, bid, nb);
   grid_reduce<kVecThreads>(v, c.partials + 2 * kMaxGrid, &s->counter[2], bid, nb, red,
-                           [&](double tot) { epi_delta(epi_ctx(c), tot); });
+                           [&](double tot) { if (c.sh != nullptr) shard_post(c, tot, 0.0); else epi_delta(epi_ctx(c), tot); });
 }
 
 // ------------------------------------------------------------------ Chebyshev-Jacobi kernels --
@@ -237,14 +252,18 @@ __global__ void __launch_bounds__(kVecThreads, 2) k_xrz(const Ctx c) {
   const int bid = blockIdx.x, nb = gridDim.x;
   double rr = 0.0, rz = 0.0;
   dispatch_xrz(c, s->ur, s->ur_n, s->uz, s->uz_n, s->alpha, s->omega_n, s->x, bid, nb, rr, rz);
-  grid_reduce2<kVecThreads>(rr, rz, c.partials + 2 * kMaxGrid, &s->counter[2], bid, nb, red,
-                            [&](double t0, double t1) { epi_delta_lagged(epi_ctx(c), t0, t1); });
+  grid_reduce2<kVecThreads>(rr, rz, c.partials + 2 * kMaxGrid, &s->counter[2], bid, nb, red, [&](double t0, double t1) {
+    if (c.sh != nullptr) shard_post(c, t0, t1); else epi_delta_lagged(epi_ctx(c), t0, t1);
+  });
 }
 
 // ------------------------------------------------------------------ stand-alone SpMV --------
+// halo_seq != 0 (row-sharded solve): wait for the neighbours' halo push with that sequence number first
 template <int UR, class PT>
-__global__ void __launch_bounds__(kSpmvThreads, kSpmvMinBlocks) k_spmv_any(const Ctx c, const PT* p, typename Store<UR>::T* q) {
+__global__ void __launch_bounds__(kSpmvThreads, kSpmvMinBlocks) k_spmv_any(const Ctx c, const PT* p, typename Store<UR>::T* q,
+                                                                           unsigned int halo_seq) {
   __shared__ double red[32];
+  if (halo_seq != 0u && c.sh != nullptr) shard_wait_halo(c, halo_seq);
   (void)phase_spmv<UR, false, kSpmvThreads>(c, p, p, q, blockIdx.x, gridDim.x, red);
 }
 
@@ -289,7 +308,7 @@ __global__ void __launch_bounds__(kVecThreads) k_setup(const Ctx c, int x0_zero)
     const double t2 = block_sum<kVecThreads>(s2, red);
     if (threadIdx.x == 0) {
       s->counter[3] = 0u;
-      epi_setup(epi_ctx(c), t1, t2);
+      if (c.sh != nullptr) shard_post(c, t1, t2); else epi_setup(epi_ctx(c), t1, t2);
     }
   }
 }
@@ -310,14 +329,18 @@ __global__ void __launch_bounds__(kVecThreads) k_finalize(const Ctx c, int true_
       rr = fma(t, t, rr);
     }
   }
-  grid_reduce<kVecThreads>(rr, c.partials + 3 * kMaxGrid, &s->counter[3], blockIdx.x, gridDim.x, red,
-                           [&](double tot) { s->relres_true = (s->bnorm > 0.0) ? sqrt(tot) / s->bnorm : 0.0; });
+  if (c.sh != nullptr && s->zero_x) return;  // b = 0 on every rank: k_epi sets relres_true = 0 without a reduction
+  grid_reduce<kVecThreads>(rr, c.partials + 3 * kMaxGrid, &s->counter[3], blockIdx.x, gridDim.x, red, [&](double tot) {
+    if (c.sh != nullptr) shard_post(c, tot, 0.0);
+    else s->relres_true = (s->bnorm > 0.0) ? sqrt(tot) / s->bnorm : 0.0;
+  });
 }
 
 // ------------------------------------------------------------------ create() kernels --------
 // flags: bit0 rowptr not monotone / out of range, bit1 column out of range,
 //        bit2 missing diagonal, bit3 non-positive or non-finite diagonal
-__global__ void k_validate_dinv(int64_t n, int64_t nnz, const int32_t* rowptr, const int32_t* colidx,
+// ncols / shift: a block row of a sharded system has n + halo_lo + halo_hi columns and its diagonal at column i + halo_lo
+__global__ void k_validate_dinv(int64_t n, int64_t nnz, int64_t ncols, int64_t shift, const int32_t* rowptr, const int32_t* colidx,
                                 const double* vals, int jacobi, double* dinv64, float* dinv32, int* flags) {
   const int64_t stride = (int64_t)gridDim.x * blockDim.x;
   int f = 0;
@@ -330,8 +353,8 @@ __global__ void k_validate_dinv(int64_t n, int64_t nnz, const int32_t* rowptr, c
     bool found = !jacobi;
     for (int64_t e = a; e < b; ++e) {
       const int j = colidx[e];
-      if (j < 0 || j >= n) { f |= 2; continue; }
-      if (jacobi && j == i) { d += vals[e]; found = true; }  // duplicates add up, as in the mat-vec
+      if (j < 0 || j >= ncols) { f |= 2; continue; }
+      if (jacobi && j == i + shift) { d += vals[e]; found = true; }  // duplicates add up, as in the mat-vec
     }
     if (!found) { f |= 4; d = 1.0; }
     else if (!(d > 0.0) || isinf(d)) { f |= 8; d = 1.0; }

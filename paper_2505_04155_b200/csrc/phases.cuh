@@ -22,11 +22,11 @@ namespace amp {
 // epilogues must not force a stack copy of the whole Ctx)
 struct EpiCtx {
   DevState* st;
-  int64_t n;
+  int64_t n;   // rows of the whole system (RMS scale)
   cudaGraphConditionalHandle cond;
   int32_t use_cond;
 };
-__device__ __forceinline__ EpiCtx epi_ctx(const Ctx& c) { return EpiCtx{c.st, c.n, c.cond, c.use_cond}; }
+__device__ __forceinline__ EpiCtx epi_ctx(const Ctx& c) { return EpiCtx{c.st, c.n_scale, c.cond, c.use_cond}; }
 __device__ __forceinline__ void set_loop_cond(const EpiCtx c, int keep_going) {
   if (c.use_cond) cudaGraphSetConditional(c.cond, keep_going ? 1u : 0u);
 }
@@ -445,7 +445,8 @@ __device__ __forceinline__ double phase_cheb_step(const Ctx& c, const double ome
 // shadow32 (only with UZ = P64): also store RN32(p) into the FP32 copy of p.  While u_z = FP64 and u_r = FP32 the
 // mat-vec needs RN32(p_j) for every gathered entry (reading R7); rounding each row once here instead of once per
 // gather there takes an FP64->FP32 conversion per ENTRY out of the SpMV (c4: 27 per row) for 4 B per row more here.
-template <int PS, int UZ, int BIF = kVecBytesInFlight>
+// PUSH (row-sharded solve, k_p_sh): chunks inside a send range are also stored into the neighbour's halo band.
+template <int PS, int UZ, int BIF = kVecBytesInFlight, bool PUSH = false>
 __device__ __forceinline__ void phase_p(const Ctx& c, const double beta, const bool first, const bool shadow32, int bid, int nb) {
   using TP = typename Store<PS>::T;
   using TZ = typename Store<UZ>::T;
@@ -456,6 +457,12 @@ __device__ __forceinline__ void phase_p(const Ctx& c, const double beta, const b
   const TZ* z = zvec<UZ>(c);
   const int64_t nchunk = c.npad / E;
   const int64_t stride = (int64_t)nb * blockDim.x;
+  // row-sharded solve: chunks inside a send range are also stored into the neighbour's halo band, in the precision the
+  // mat-vec gathers (the FP32 copy in the shadow32 phase)
+  constexpr bool push = PUSH;
+  HaloPush<TZ> hp{nullptr, nullptr, 0, 0, 0};
+  HaloPush<float> hp32{nullptr, nullptr, 0, 0, 0};
+  if constexpr (PUSH) { hp = halo_push_of<UZ>(c); hp32 = halo_push_of<P32>(c); }
   for (int64_t base = (int64_t)bid * blockDim.x + threadIdx.x; base < nchunk; base += stride * U) {
     Chunk<TP, E> pp[U];
     Chunk<TZ, E> zz[U];
@@ -488,13 +495,17 @@ __device__ __forceinline__ void phase_p(const Ctx& c, const double beta, const b
         Chunk<TZ, E> po;
         chunk_pack(po, a);
         chunk_store(po, pout, i);
+        bool pushed = false;
         if constexpr (UZ == P64) {
           if (shadow32) {
             Chunk<float, E> p32;
             chunk_pack(p32, a);
             chunk_store(p32, c.p32, i);
+            if (push) halo_push_chunk(hp32, p32, i);
+            pushed = true;
           }
         }
+        if (push && !pushed) halo_push_chunk(hp, po, i);
 #ifdef AMP_COUNT_FP16
         if (UZ == P16) {
           double h[E];

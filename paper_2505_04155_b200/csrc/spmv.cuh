@@ -167,16 +167,18 @@ template <> struct ColSrc<1> : ColBase {
 };
 template <> struct ColSrc<2> : ColBase {
   using RawQ = int; using RawP = int; using RawS = int;  // nothing is loaded per entry
-  int row, nm1;
+  int row, cmin_, cmax_;
   __device__ __forceinline__ ColSrc() {}
-  __device__ __forceinline__ ColSrc(const Ctx& c, int w0, int w_, int lane, int row_) : row(row_ < 0 ? 0 : row_), nm1((int)c.n - 1) {
+  __device__ __forceinline__ ColSrc(const Ctx& c, int w0, int w_, int lane, int row_)
+      : row(row_ < 0 ? 0 : row_), cmin_(c.col_min), cmax_(c.col_max) {
     init(c, w0, w_, lane);
   }
   __device__ __forceinline__ RawQ quad(int, int) const { return 0; }
   __device__ __forceinline__ RawP pair(int, int) const { return 0; }
   __device__ __forceinline__ RawS single(int, int) const { return 0; }
-  // explicit zeros of rows that lack diagonal k may point outside [0, n): clamp (their value is 0)
-  __device__ __forceinline__ int col(int k) const { return min(max(row + base(k), 0), nm1); }
+  // explicit zeros of rows that lack diagonal k may point outside the vector (owned entries, halo bands, zero guard):
+  // clamp (their value is 0)
+  __device__ __forceinline__ int col(int k) const { return min(max(row + base(k), cmin_), cmax_); }
   __device__ __forceinline__ void dq(RawQ, int k, int (&j)[4]) const { j[0] = col(k); j[1] = col(k + 1); j[2] = col(k + 2); j[3] = col(k + 3); }
   __device__ __forceinline__ void dp(RawP, int k, int (&j)[2]) const { j[0] = col(k); j[1] = col(k + 1); }
   __device__ __forceinline__ int ds(RawS, int k) const { return col(k); }
@@ -456,7 +458,7 @@ __device__ __forceinline__ double phase_spmv_fmt(const Ctx& c, const PT* p, cons
     const int e0 = c.rowptr[row], e1 = c.rowptr[row + 1];
     const A* gv = csr_vals<UR>(c);
     A acc = 0;
-    for (int e = e0 + (int)threadIdx.x; e < e1; e += NT) acc = fma(gv[e], gatherA<COH>(A(0), p, c.colidx[e]), acc);
+    for (int e = e0 + (int)threadIdx.x; e < e1; e += NT) acc = fma(gv[e], gatherA<COH>(A(0), p, c.colidx[e] - c.col_shift), acc);
     const double tot = block_sum<NT>((double)acc, red);
     if (threadIdx.x == 0) {
       const A qi = (A)tot;
@@ -529,7 +531,9 @@ __device__ __forceinline__ void sell_slot(int n, int s, int lane, int long_min, 
 }
 
 // pass 1: width of every slice; bit 31 set = the slice is stored diagonal-aligned
-__global__ void k_sell_scan(int n, int nslices, int long_min, int allow_aligned, const int32_t* __restrict__ rowptr,
+// shift (= halo_lo of a block row of a sharded system, else 0) is subtracted from every column index: stored columns are
+// relative to the first OWNED entry of p
+__global__ void k_sell_scan(int n, int nslices, int long_min, int allow_aligned, int shift, const int32_t* __restrict__ rowptr,
                             const int32_t* __restrict__ colidx, const int32_t* __restrict__ perm, int32_t* __restrict__ width) {
   const int lane = threadIdx.x & 31;
   const int s = (int)(((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5);
@@ -539,7 +543,7 @@ __global__ void k_sell_scan(int n, int nslices, int long_min, int allow_aligned,
   const int wnat = warp_max_i(len);
   int w = wnat;
   if (allow_aligned && wnat > 0) {
-    const int d = sell_align(row < 0 ? 0 : row, e0, len, colidx, wnat + (wnat >> 2), [](int, int, bool, int) {});
+    const int d = sell_align((row < 0 ? 0 : row) + shift, e0, len, colidx, wnat + (wnat >> 2), [](int, int, bool, int) {});
     if (d >= 0) w = d | kAlignedFlag;
   }
   if (lane == 0) width[s] = w;
@@ -548,7 +552,7 @@ __global__ void k_sell_scan(int n, int nslices, int long_min, int allow_aligned,
 // pass 2: one warp per slice; lane = row slot.  Long rows and padding slots get length 0.
 // General slices: padding entries take the smallest real column of their entry index k (the base of
 // the 16-bit format) and value 0; flag16 is set when some offset from the base does not fit 16 bits.
-__global__ void k_sell_pack(int n, int nslices, int long_min, const int32_t* __restrict__ rowptr,
+__global__ void k_sell_pack(int n, int nslices, int long_min, int shift, const int32_t* __restrict__ rowptr,
                             const int32_t* __restrict__ colidx, const double* __restrict__ vals,
                             const int32_t* __restrict__ wptr, const int32_t* __restrict__ perm, int32_t* __restrict__ cols,
                             uint16_t* __restrict__ cols16, int32_t* __restrict__ bases, double* __restrict__ v64,
@@ -562,7 +566,7 @@ __global__ void k_sell_pack(int n, int nslices, int long_min, const int32_t* __r
   int row, e0, len;
   sell_slot(n, s, lane, long_min, rowptr, perm, row, e0, len);
   if (aligned) {
-    sell_align(row < 0 ? 0 : row, e0, len, colidx, w, [&](int k, int off, bool mine, int e) {
+    sell_align((row < 0 ? 0 : row) + shift, e0, len, colidx, w, [&](int k, int off, bool mine, int e) {
       const double v = mine ? vals[e] : 0.0;
       v32[base + sell_pos32(k, lane, w)] = __double2float_rn(v);
       v64[base + sell_pos64(k, lane, w)] = v;
@@ -573,10 +577,10 @@ __global__ void k_sell_pack(int n, int nslices, int long_min, const int32_t* __r
   bool wide = false;
   for (int k = 0; k < w; ++k) {
     const bool ok = k < len;
-    int j = ok ? colidx[e0 + k] : 0x7fffffff;
-    const int mn = warp_min_i(j), mx = warp_max_i(ok ? j : -1);
+    int j = ok ? colidx[e0 + k] - shift : 0x7fffffff;
+    const int mn = warp_min_i(j), mx = warp_max_i(ok ? j : (int)0x80000000);
     if (!ok) j = mn;
-    if (mx - mn > 65535) wide = true;
+    if (mx >= mn && mx - mn > 65535) wide = true;
     const double v = ok ? vals[e0 + k] : 0.0;
     const int64_t p32 = base + sell_pos32(k, lane, w);
     cols[p32] = j;

@@ -21,6 +21,7 @@
 // Under programmatic dependent launch the producer starts streaming the (constant) matrix BEFORE griddepcontrol.wait,
 // i.e. while the p update of the same iteration is still finishing.
 #pragma once
+#include "shard.cuh"
 #include "spmv.cuh"
 
 namespace amp {
@@ -151,7 +152,8 @@ __device__ __forceinline__ A pipe_slice_sum(const A* sv, const int* sb, int w, i
 struct PipeChunk { int32_t s0, w0; };
 
 template <int UR, class PT, class PG>
-__device__ __forceinline__ double pipe_body(const Ctx& c, const PT* p, const PG* pg, typename Store<UR>::T* q, unsigned char* smem) {
+__device__ __forceinline__ double pipe_body(const Ctx& c, const PT* p, const PG* pg, typename Store<UR>::T* q, unsigned char* smem,
+                                            unsigned int halo_seq) {
   using A = typename SpmvT<UR>::A;
   constexpr int STAGE = 32 * kPipeChunkW * (int)sizeof(A);
   constexpr int NST = kPipeValueBytes / STAGE;
@@ -197,6 +199,7 @@ __device__ __forceinline__ double pipe_body(const Ctx& c, const PT* p, const PG*
     }
   } else {
     pdl_wait();  // p (and q's previous readers) belong to the predecessor kernels
+    if (c.sh != nullptr) shard_wait_halo_warp(c, halo_seq);  // row-sharded solve: the neighbours' entries of p have arrived
     static_assert(NST % kPipeGroups == 0, "a stage slot must always serve the same group");
     const int grp = warp % kPipeGroups, wg = warp / kPipeGroups;  // this warp's group and its rank inside it
     for (int ch = c0 + grp; ch < c1; ch += kPipeGroups) {
@@ -238,20 +241,21 @@ __global__ void __launch_bounds__(kPipeThreads, 1) k_spmv_pipe(const Ctx c, int 
   // before the first kernel of this iteration started (plain dependency): safe to read before the wait
   const int ur = s->ur, uz = s->uz;
   if (s->done || ur != P32) { pdl_wait(); return; }
+  const unsigned int hseq = (unsigned int)s->k + 1u;
   double v;
   if (zmode) {  // q = A z inside the Chebyshev-Jacobi preconditioner
-    if (uz == P16) v = pipe_body<P32>(c, c.z16, c.z16, c.q32, pipe_smem);
-    else if (uz == P32) v = pipe_body<P32>(c, c.z32, c.z32, c.q32, pipe_smem);
-    else v = pipe_body<P32>(c, c.z64, c.z64, c.q32, pipe_smem);  // RN32(z_j) per gathered entry
+    if (uz == P16) v = pipe_body<P32>(c, c.z16, c.z16, c.q32, pipe_smem, hseq);
+    else if (uz == P32) v = pipe_body<P32>(c, c.z32, c.z32, c.q32, pipe_smem, hseq);
+    else v = pipe_body<P32>(c, c.z64, c.z64, c.q32, pipe_smem, hseq);  // RN32(z_j) per gathered entry
     pdl_wait();
     return;
   }
-  if (uz == P16) v = pipe_body<P32>(c, c.p16, c.p16, c.q32, pipe_smem);
-  else if (uz == P32) v = pipe_body<P32>(c, c.p32, c.p32, c.q32, pipe_smem);
-  else v = pipe_body<P32>(c, c.p32, c.p64, c.q32, pipe_smem);  // gathers the FP32 copy RN32(p) written by the p update
+  if (uz == P16) v = pipe_body<P32>(c, c.p16, c.p16, c.q32, pipe_smem, hseq);
+  else if (uz == P32) v = pipe_body<P32>(c, c.p32, c.p32, c.q32, pipe_smem, hseq);
+  else v = pipe_body<P32>(c, c.p32, c.p64, c.q32, pipe_smem, hseq);  // gathers the FP32 copy RN32(p) written by the p update
   pdl_wait();  // (the producer warp has not waited yet) before touching the reduction scratch shared with other kernels
   grid_reduce<kPipeThreads>(v, c.partials + 1 * kMaxGrid, &s->counter[1], blockIdx.x, gridDim.x, red,
-                            [&](double tot) { epi_gamma(epi_ctx(c), tot); });
+                            [&](double tot) { if (c.sh != nullptr) shard_post(c, tot, 0.0); else epi_gamma(epi_ctx(c), tot); });
 }
 
 }  // namespace amp
