@@ -55,6 +55,7 @@ def parse_args():
     ap.add_argument("--policy", default="amp_fp64_delay", choices=sorted(POLICIES))
     ap.add_argument("--loop", default="auto", choices=["auto", "stream", "graph", "persistent"])
     ap.add_argument("--spmv-kernel", default="auto", choices=["auto", "direct", "pipelined"])
+    ap.add_argument("--vec-kernel", default="auto", choices=["auto", "direct", "staged"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--others", default="", help="comma list of further workloads to report under 'other_workloads' "
                                                  "(value / time_to_tol / speed-up only), e.g. c1,c2,c3,c5")
@@ -64,7 +65,8 @@ def parse_args():
                     help="profiling aid for ncu: run ONE solve of this many iterations with plain stream launches "
                          "(u_r forced to FP32 from k=ell so the low-precision kernels appear) and exit; prints no bench line")
     ap.add_argument("--profile-policy", default="amp_fp16_linear",
-                    choices=["pcg_fp64", "amp_fp16_linear", "amp_fp64_delay", "amp_fp16_linear_lagged"])
+                    choices=["pcg_fp64", "amp_fp16_linear", "amp_fp64_delay", "amp_fp16_linear_lagged", "amp_fp64_ur32",
+                             "amp_fp32_ur32"])
     ap.add_argument("--ref-iters", type=int, default=0, help="--impl reference: iterations per step (0 = sized to the workload)")
     ap.add_argument("--shard", action="store_true",
                     help="N > 1: ONE system row-sharded over the N ranks (amp_pcg_solve_sharded: halo of p and the three inner "
@@ -354,11 +356,15 @@ def run_ours(args, rank: int, local_rank: int, world: int):
     loop = {"auto": A.LOOP_AUTO, "stream": A.LOOP_STREAM, "graph": A.LOOP_GRAPH, "persistent": A.LOOP_PERSISTENT}[args.loop]
     spmv_kernel = {"auto": A.SPMV_AUTO, "direct": A.SPMV_DIRECT, "pipelined": A.SPMV_PIPELINED}[args.spmv_kernel]
     s = make_config(args.workload, args.size)
-    R = Runner(A, torch, s, dev, loop, spmv_kernel)
+    vec_kernel = {"auto": A.VEC_AUTO, "direct": A.VEC_DIRECT, "staged": A.VEC_STAGED}[args.vec_kernel]
+    R = Runner(A, torch, s, dev, loop, spmv_kernel, vec_kernel=vec_kernel)
     h = R.h
     if args.profile_iters > 0:
         kwp = {"pcg_fp64": dict(amp=0), "amp_fp16_linear": dict(u0=A.FP16, eta_rule=A.ETA_LINEAR, eps32=1e-30),
                "amp_fp16_linear_lagged": dict(u0=A.FP16, eta_rule=A.ETA_LINEAR, eps32=1e-30, scale_mode=A.SCALE_LAGGED),
+               # phases (FP64, FP32) and (FP32, FP32) from k = 5 on: u_z held by the thresholds, u_r forced down
+               "amp_fp64_ur32": dict(u0=A.FP64, eta_rule=A.ETA_LINEAR, eps32=1e-30, tau_zs=0.0, tau_zh=0.0),
+               "amp_fp32_ur32": dict(u0=A.FP32, eta_rule=A.ETA_LINEAR, eps32=1e-30, tau_zs=0.0, tau_zh=0.0),
                "amp_fp64_delay": dict()}[args.profile_policy]
         lp = A.LOOP_STREAM if args.loop == "auto" else loop
         stp = h.solve(R.b, R.x, s.tol, args.profile_iters, A.Policy.default(x0_zero=1, loop_mode=lp, **kwp))
@@ -441,7 +447,7 @@ def run_ours(args, rank: int, local_rank: int, world: int):
     # ---- NEXT-4: the same solve with the Chebyshev-accelerated Jacobi preconditioner (the paper's smoother) ----
     cheb = {}
     for deg in [int(t) for t in args.cheb_degrees.split(",") if t]:
-        Rc = Runner(A, torch, s, dev, loop, spmv_kernel, share=R, precond=A.PRECOND_CHEBJACOBI, cheb_degree=deg)
+        Rc = Runner(A, torch, s, dev, loop, spmv_kernel, share=R, precond=A.PRECOND_CHEBJACOBI, cheb_degree=deg, vec_kernel=vec_kernel)
         a_, _ = Rc.summary(args.policy, 2)
         f_, _ = Rc.summary(dict(amp=0), 2)
         cheb[f"degree_{deg}"] = {"amp": a_, "fp64_pcg": f_, "amp_speedup_vs_fp64_same_precond": f_["time_to_tol_s"] / a_["time_to_tol_s"],
@@ -454,7 +460,7 @@ def run_ours(args, rank: int, local_rank: int, world: int):
     others = {}
     for name in [t for t in args.others.split(",") if t]:
         so = make_config(name)
-        Ro = Runner(A, torch, so, dev, loop, spmv_kernel)
+        Ro = Runner(A, torch, so, dev, loop, spmv_kernel, vec_kernel=vec_kernel)
         a_, _ = Ro.summary(args.policy, 2)
         f_, _ = Ro.summary(dict(amp=0), 2)
         l_, _ = Ro.summary(args.policy, 2, scale_mode=A.SCALE_LAGGED)

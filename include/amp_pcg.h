@@ -63,6 +63,12 @@ enum {
   AMP_SPMV_DIRECT = 1,    /* every lane streams its row with 128-bit loads (round-1 kernel) */
   AMP_SPMV_PIPELINED = 2  /* value stream staged through shared memory by cp.async.bulk + mbarrier ring */
 };
+/* which vector kernels (steps a2, a3, a5) the loop uses (execution choice; same arithmetic, same bits) */
+enum {
+  AMP_VEC_AUTO = 0,       /* from 4 M rows on the z and p updates are staged, the x/r update stays direct; below: all direct */
+  AMP_VEC_DIRECT = 1,     /* every thread loads its chunks of the vectors from global memory */
+  AMP_VEC_STAGED = 2      /* persistent blocks; the input vectors are streamed into a shared-memory ring by cp.async.bulk */
+};
 /* storage / working precisions u_z, u_r */
 enum { AMP_FP64 = 0, AMP_FP32 = 1, AMP_FP16 = 2 };
 /* indicator used by the u_r switch */
@@ -182,6 +188,8 @@ typedef struct {
   int64_t halo_hi;        /*   system, n rows by halo_lo + n + halo_hi columns; column index halo_lo + i is the diagonal of
                                row i, columns below halo_lo / from halo_lo + n on are the neighbour ranks' entries of p
                                (filled by the halo exchange).  Both 0 (default): an ordinary square matrix */
+  int32_t vec_kernel;     /* AMP_VEC_*, default AUTO */
+  int32_t reserved1;      /* 0 */
 } amp_create_opts_t;
 void amp_create_opts_default(amp_create_opts_t *o);
 amp_pcg_t *amp_pcg_create_ex(int64_t n, int64_t nnz, const int32_t *rowptr, const int32_t *colidx,

@@ -19,6 +19,7 @@ LOOP_AUTO, LOOP_STREAM, LOOP_GRAPH, LOOP_PERSISTENT = 0, 1, 2, 3
 PRECOND_NONE, PRECOND_JACOBI, PRECOND_CHEBJACOBI = 0, 1, 2
 INDEX_AUTO, INDEX_NO_ALIGN, INDEX_FORCE32 = 0, 1, 2
 SPMV_AUTO, SPMV_DIRECT, SPMV_PIPELINED = 0, 1, 2
+VEC_AUTO, VEC_DIRECT, VEC_STAGED = 0, 1, 2
 K_Z, K_P, K_SPMV, K_XR, K_XRZ, K_CHEB0, K_CHEBSTEP = 0, 1, 2, 3, 4, 5, 6
 KERNEL_NAMES = {K_Z: "k_z", K_P: "k_p", K_SPMV: "k_spmv", K_XR: "k_xr", K_XRZ: "k_xrz", K_CHEB0: "k_cheb0",
                 K_CHEBSTEP: "k_cheb_step"}
@@ -73,7 +74,7 @@ class CreateOpts(C.Structure):
         ("struct_bytes", C.c_int32), ("precond", C.c_int32), ("index_format", C.c_int32), ("spmv_kernel", C.c_int32),
         ("spmv_grid_mult", C.c_int32), ("pdl", C.c_int32), ("cheb_degree", C.c_int32), ("reserved0", C.c_int32),
         ("cheb_lmin", C.c_double), ("cheb_lmax", C.c_double), ("stream", C.c_void_p),
-        ("halo_lo", C.c_int64), ("halo_hi", C.c_int64),
+        ("halo_lo", C.c_int64), ("halo_hi", C.c_int64), ("vec_kernel", C.c_int32), ("reserved1", C.c_int32),
     ]
 
     @classmethod

@@ -15,6 +15,7 @@
 #include "kernels.cuh"
 #include "persistent.cuh"
 #include "spmv_pipe.cuh"
+#include "vec_pipe.cuh"
 
 using namespace amp;
 
@@ -88,12 +89,15 @@ struct amp_pcg {
   char* xchg = nullptr;                  // exchange block: mailbox [kMailEntries] then 2 halo flags (owned, zeroed once)
   ShardCtx* d_shard = nullptr;           // device copy of the peer table (owned)
   int shard_rank = -1, shard_world = 0;  // set by amp_pcg_shard_attach*
+  int use_vstage = 0;                    // bit 0: k_z and k_p, bit 1: k_xr and k_xrz are the bulk-copy staged kernels (vec_pipe.cuh)
+  int shard_inline = 0;                  // the reducing kernels also collect and step (ranks run concurrently): no k_epi launches
   unsigned int shard_epoch = 0;          // sharded solves / mat-vecs made so far (identical on all ranks of the group)
   std::vector<void*> ipc_opened;         // peer allocations opened with cudaIpcOpenMemHandle
   cudaGraph_t graph_sh[2] = {nullptr, nullptr};          // [lagged] graph loops of the sharded solve
   cudaGraphExec_t graph_sh_exec[2] = {nullptr, nullptr};
   cudaGraphConditionalHandle cond_sh[2] = {};
 };
+constexpr int64_t kVecStagedAutoMinRows = 4000000;  // AMP_VEC_AUTO stages the z and p updates from here on
 constexpr size_t kXchgBytes = sizeof(Mail) * kMailEntries + 64;
 
 template <class T> static T* dev_alloc(amp_pcg* h, size_t count, bool zero) {
@@ -199,6 +203,8 @@ extern "C" void amp_create_opts_default(amp_create_opts_t* o) {
   o->stream = nullptr;
   o->halo_lo = 0;
   o->halo_hi = 0;
+  o->vec_kernel = AMP_VEC_AUTO;
+  o->reserved1 = 0;
 }
 
 extern "C" amp_pcg_t* amp_pcg_create(int64_t n, int64_t nnz, const int32_t* rowptr, const int32_t* colidx,
@@ -224,8 +230,9 @@ extern "C" amp_pcg_t* amp_pcg_create_ex(int64_t n, int64_t nnz, const int32_t* r
   }
   const int precond = o.precond;
   if (o.index_format < AMP_INDEX_AUTO || o.index_format > AMP_INDEX_FORCE32 || o.spmv_kernel < AMP_SPMV_AUTO ||
-      o.spmv_kernel > AMP_SPMV_PIPELINED || o.spmv_grid_mult < 0 || (o.pdl != 0 && o.pdl != 1)) {
-    set_error("amp_pcg_create_ex: invalid index_format / spmv_kernel / spmv_grid_mult / pdl");
+      o.spmv_kernel > AMP_SPMV_PIPELINED || o.spmv_grid_mult < 0 || (o.pdl != 0 && o.pdl != 1) || o.vec_kernel < AMP_VEC_AUTO ||
+      o.vec_kernel > AMP_VEC_STAGED) {
+    set_error("amp_pcg_create_ex: invalid index_format / spmv_kernel / vec_kernel / spmv_grid_mult / pdl");
     return nullptr;
   }
   if (o.halo_lo < 0 || o.halo_hi < 0 || (o.halo_lo & 7) || (o.halo_hi & 7) || o.halo_lo > (1 << 26) || o.halo_hi > (1 << 26) ||
@@ -587,6 +594,25 @@ extern "C" amp_pcg_t* amp_pcg_create_ex(int64_t n, int64_t nnz, const int32_t* r
   h->grid_cheb0 = vec_grid_for((const void*)k_cheb0);
   h->grid_cheb_step = vec_grid_for((const void*)k_cheb_step);
   h->vec_grid = vec_grid_for((const void*)k_setup);
+  // bulk-copy staged vector kernels (vec_pipe.cuh).  Measured on B200 (profiles/r02.md, us per launch, staged vs direct):
+  // c4 (8 M rows) k_z 23.1 vs 27.4 (FP16 phase), 25.1 vs 31.8 (FP32 phase), k_p 18.5 vs 20.5, but k_xr 47.8 vs 44.6; c3
+  // (4.1 M) k_z 16.9 vs 21.0, k_p 12.5 vs 14.5, k_xr 29.1 vs 28.4; c2 (2.1 M) a tie.  AUTO therefore stages the z and p
+  // updates from 4 M rows on and keeps the direct x/r update; STAGED stages all four (tests, tuning).
+  h->use_vstage = o.vec_kernel == AMP_VEC_STAGED ? 3 : ((o.vec_kernel == AMP_VEC_AUTO && n >= kVecStagedAutoMinRows) ? 1 : 0);
+  if (h->use_vstage) {
+    const void* ks[4] = {(const void*)k_z_st, (const void*)k_p_st, (const void*)k_xr_st, (const void*)k_xrz_st};
+    for (const void* k : ks) {
+      if (cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, kVpSmemBytes) != cudaSuccess) {
+        cudaGetLastError();
+        if (o.vec_kernel == AMP_VEC_STAGED) {
+          set_error("amp_pcg_create_ex: AMP_VEC_STAGED needs %d bytes of shared memory per block", kVpSmemBytes);
+          amp_pcg_destroy(h);
+          return nullptr;
+        }
+        h->use_vstage = 0;
+      }
+    }
+  }
 #undef ALLOC
   return h;
 }
@@ -665,6 +691,21 @@ static cudaError_t launch_loop_kernel(K kern, int grid, int threads, cudaStream_
   return launch_loop_kernel_ex(kern, grid, threads, s, pdl, 0, c);
 }
 
+// the vector kernels of the loop: direct (kernels.cuh) or bulk-copy staged (vec_pipe.cuh), by the handle's vec_kernel
+enum { VK_Z = 0, VK_P = 1, VK_XR = 2, VK_XRZ = 3 };
+static cudaError_t launch_vec(amp_pcg* h, int which, cudaStream_t s, const Ctx& c, bool pdl) {
+  if (h->use_vstage & ((which == VK_Z || which == VK_P) ? 1 : 2)) {
+    void (*kern)(const Ctx) = which == VK_Z ? k_z_st : which == VK_P ? k_p_st : which == VK_XR ? k_xr_st : k_xrz_st;
+    return launch_loop_kernel_ex(kern, h->num_sms, kVpThreads, s, pdl, (size_t)kVpSmemBytes, c);
+  }
+  switch (which) {
+    case VK_Z: return launch_loop_kernel(k_z, h->grid_z, kVecThreads, s, c, pdl);
+    case VK_P: return launch_loop_kernel(k_p, h->grid_p, kVecThreads, s, c, pdl);
+    case VK_XR: return launch_loop_kernel(k_xr, h->grid_xr, kVecThreads, s, c, pdl);
+    default: return launch_loop_kernel(k_xrz, h->grid_xrz, kVecThreads, s, c, pdl);
+  }
+}
+
 // step a4 inside the loop (zmode = 0), or the mat-vec q = A z inside the Chebyshev-Jacobi preconditioner (zmode = 1):
 // the direct kernel, followed by the bulk-copy pipelined kernel when the matrix is eligible (it takes the u_r = FP32
 // phases; whichever kernel's phase it is not returns at once)
@@ -705,14 +746,14 @@ static cudaError_t launch_iteration(amp_pcg* h, const Ctx& c, cudaStream_t s, bo
     }
   } else {
     if (prof) e = prof_mark(h, s, AMP_K_Z, prof_iter);
-    if (e == cudaSuccess) e = launch_loop_kernel(k_z, h->grid_z, kVecThreads, s, c, false);
+    if (e == cudaSuccess) e = launch_vec(h, VK_Z, s, c, false);
   }
   if (prof && e == cudaSuccess) e = prof_mark(h, s, AMP_K_P, prof_iter);
-  if (e == cudaSuccess) e = launch_loop_kernel(k_p, h->grid_p, kVecThreads, s, c, pdl);
+  if (e == cudaSuccess) e = launch_vec(h, VK_P, s, c, pdl);
   if (prof && e == cudaSuccess) e = prof_mark(h, s, AMP_K_SPMV, prof_iter);
   if (e == cudaSuccess) e = launch_spmv_loop(h, s, c, pdl);
   if (prof && e == cudaSuccess) e = prof_mark(h, s, AMP_K_XR, prof_iter);
-  if (e == cudaSuccess) e = launch_loop_kernel(k_xr, h->grid_xr, kVecThreads, s, c, pdl);
+  if (e == cudaSuccess) e = launch_vec(h, VK_XR, s, c, pdl);
   if (prof && e == cudaSuccess) e = prof_mark(h, s, -1, prof_iter);
   return e;
 }
@@ -723,11 +764,11 @@ static cudaError_t launch_iteration_lagged(amp_pcg* h, const Ctx& c, cudaStream_
   if (prof) pdl = false;
   cudaError_t e = cudaSuccess;
   if (prof) e = prof_mark(h, s, AMP_K_P, prof_iter);
-  if (e == cudaSuccess) e = launch_loop_kernel(k_p, h->grid_p, kVecThreads, s, c, false);
+  if (e == cudaSuccess) e = launch_vec(h, VK_P, s, c, false);
   if (prof && e == cudaSuccess) e = prof_mark(h, s, AMP_K_SPMV, prof_iter);
   if (e == cudaSuccess) e = launch_spmv_loop(h, s, c, pdl);
   if (prof && e == cudaSuccess) e = prof_mark(h, s, AMP_K_XRZ, prof_iter);
-  if (e == cudaSuccess) e = launch_loop_kernel(k_xrz, h->grid_xrz, kVecThreads, s, c, pdl);
+  if (e == cudaSuccess) e = launch_vec(h, VK_XRZ, s, c, pdl);
   if (prof && e == cudaSuccess) e = prof_mark(h, s, -1, prof_iter);
   return e;
 }
@@ -901,7 +942,7 @@ static int solve_impl(amp_pcg* h, const double* b, double* x, double tol, int32_
   h->launches += 1;
 
   if (lagged && mode != AMP_LOOP_PERSISTENT) {  // z_0, rho_0 for the first pass of the three-kernel loop
-    k_z<<<h->grid_z, kVecThreads, 0, st>>>(h->ctx);
+    CU_TRY(launch_vec(h, VK_Z, st, h->ctx, false), return AMP_ERR_CUDA);
     h->launches += 1;
   }
   if (mode == AMP_LOOP_GRAPH) {
@@ -1131,11 +1172,11 @@ extern "C" int amp_pcg_debug_step(amp_pcg_t* h, amp_debug_step_t* io, double* x)
   CU_TRY(cudaMemcpyAsync(h->ctx.st, hs, sizeof(DevState), cudaMemcpyHostToDevice, st), return AMP_ERR_CUDA);
   cudaError_t e = cudaSuccess;
   switch (io->step) {  // the very kernels, grids and block sizes the stream / graph loop launches
-    case AMP_STEP_Z: e = launch_loop_kernel(k_z, h->grid_z, kVecThreads, st, h->ctx, false); break;
-    case AMP_STEP_P: e = launch_loop_kernel(k_p, h->grid_p, kVecThreads, st, h->ctx, false); break;
+    case AMP_STEP_Z: e = launch_vec(h, VK_Z, st, h->ctx, false); break;
+    case AMP_STEP_P: e = launch_vec(h, VK_P, st, h->ctx, false); break;
     case AMP_STEP_SPMV: e = launch_spmv_loop(h, st, h->ctx, false); break;
-    case AMP_STEP_XR: e = launch_loop_kernel(k_xr, h->grid_xr, kVecThreads, st, h->ctx, false); break;
-    case AMP_STEP_XRZ: e = launch_loop_kernel(k_xrz, h->grid_xrz, kVecThreads, st, h->ctx, false); break;
+    case AMP_STEP_XR: e = launch_vec(h, VK_XR, st, h->ctx, false); break;
+    case AMP_STEP_XRZ: e = launch_vec(h, VK_XRZ, st, h->ctx, false); break;
     case AMP_STEP_CHEB0: e = launch_loop_kernel(k_cheb0, h->grid_cheb0, kVecThreads, st, h->ctx, false); break;
     case AMP_STEP_SPMV_Z: e = launch_spmv_loop(h, st, h->ctx, false, 1); break;
     default: e = launch_loop_kernel_ex(k_cheb_step, h->grid_cheb_step, kVecThreads, st, false, 0, h->ctx, (int)io->first); break;

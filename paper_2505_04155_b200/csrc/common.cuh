@@ -18,7 +18,10 @@ constexpr int kSpmvWarps = kSpmvThreads / 32;
 #define AMP_SPMV_MINBLOCKS 4
 #endif
 constexpr int kSpmvMinBlocks = AMP_SPMV_MINBLOCKS;  // resident SpMV blocks per SM the register budget is set for
-constexpr int kPersistThreads = 1024;          // block size of the persistent (whole-loop) kernel
+#ifndef AMP_PERSIST_THREADS
+#define AMP_PERSIST_THREADS 1024
+#endif
+constexpr int kPersistThreads = AMP_PERSIST_THREADS;  // block size of the persistent (whole-loop) kernel
 constexpr int kPersistAutoMaxRows = 1 << 20;   // AMP_LOOP_AUTO takes the persistent kernel up to this many rows
 constexpr int kPersistMinBlocks = 1;           // resident blocks per SM its register budget is set for
 constexpr int kMaxGrid = 8192;                 // capacity of each partial-sum array
@@ -61,6 +64,9 @@ constexpr int kMailSlots = 4;
 constexpr int kMailEntries = 2 * kMailSlots * kMaxWorld;
 struct ShardCtx {
   int32_t rank, world;
+  int32_t inline_epi, pad0;            // 1: the block that completes a reduction also collects the other ranks' partial sums
+                                       //    and runs the scalar step (ranks run concurrently: one per GPU); 0: k_epi does
+                                       //    (ranks share a device and run one after the other)
   int32_t send_lo, send_hi;            // entries of p pushed to rank-1 (its upper halo) / rank+1 (its lower halo); multiples of 8
   Mail* mbox;                          // this rank's mailbox [kMailEntries]
   Mail* peer_mbox[kMaxWorld];          // every rank's mailbox (own included), peer-mapped

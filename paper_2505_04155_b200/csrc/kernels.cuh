@@ -102,7 +102,7 @@ __global__ void __launch_bounds__(kVecThreads, AMP_KZ_BLOCKS) k_z(const Ctx c) {
   const double v = dispatch_z(c, s->r_store, s->ur, s->uz, s->omega, bid, nb);
   // row-sharded solve (c.sh != nullptr): the partial sum goes to every rank's mailbox, k_epi runs the scalar step
   grid_reduce<kVecThreads>(v, c.partials + 0 * kMaxGrid, &s->counter[0], bid, nb, red,
-                           [&](double tot) { if (c.sh != nullptr) shard_post(c, tot, 0.0); else epi_rho(epi_ctx(c), tot); });
+                           [&](double tot) { if (c.sh != nullptr) shard_reduce_point(c, kEpiRho, tot, 0.0); else epi_rho(epi_ctx(c), tot); });
 }
 
 __global__ void __launch_bounds__(kVecThreads, AMP_KP_BLOCKS) k_p(const Ctx c) {
@@ -137,7 +137,7 @@ __global__ void __launch_bounds__(kSpmvThreads, kSpmvMinBlocks) k_spmv(const Ctx
   const double v = dispatch_spmv<false, kSpmvThreads>(c, s->ur, s->uz, zmode, bid, nb, red);
   if (zmode) return;  // q = A z inside M^-1: no inner product
   grid_reduce<kSpmvThreads>(v, c.partials + 1 * kMaxGrid, &s->counter[1], bid, nb, red,
-                            [&](double tot) { if (c.sh != nullptr) shard_post(c, tot, 0.0); else epi_gamma(epi_ctx(c), tot); });
+                            [&](double tot) { if (c.sh != nullptr) shard_reduce_point(c, kEpiGamma, tot, 0.0); else epi_gamma(epi_ctx(c), tot); });
 }
 
 __global__ void __launch_bounds__(kVecThreads, AMP_KXR_BLOCKS) k_xr(const Ctx c) {
@@ -152,7 +152,7 @@ __global__ void __launch_bounds__(kVecThreads, AMP_KXR_BLOCKS) k_xr(const Ctx c)
   const int bid = blockIdx.x, nb = gridDim.x;
   const double v = dispatch_xr(c, s->ur, s->uz, s->alpha, s->x, bid, nb);
   grid_reduce<kVecThreads>(v, c.partials + 2 * kMaxGrid, &s->counter[2], bid, nb, red,
-                           [&](double tot) { if (c.sh != nullptr) shard_post(c, tot, 0.0); else epi_delta(epi_ctx(c), tot); });
+                           [&](double tot) { if (c.sh != nullptr) shard_reduce_point(c, kEpiDelta, tot, 0.0); else epi_delta(epi_ctx(c), tot); });
 }
 
 // ------------------------------------------------------------------ Chebyshev-Jacobi kernels --
@@ -253,7 +253,7 @@ __global__ void __launch_bounds__(kVecThreads, 2) k_xrz(const Ctx c) {
   double rr = 0.0, rz = 0.0;
   dispatch_xrz(c, s->ur, s->ur_n, s->uz, s->uz_n, s->alpha, s->omega_n, s->x, bid, nb, rr, rz);
   grid_reduce2<kVecThreads>(rr, rz, c.partials + 2 * kMaxGrid, &s->counter[2], bid, nb, red, [&](double t0, double t1) {
-    if (c.sh != nullptr) shard_post(c, t0, t1); else epi_delta_lagged(epi_ctx(c), t0, t1);
+    if (c.sh != nullptr) shard_reduce_point(c, kEpiDeltaLagged, t0, t1); else epi_delta_lagged(epi_ctx(c), t0, t1);
   });
 }
 
@@ -308,7 +308,7 @@ __global__ void __launch_bounds__(kVecThreads) k_setup(const Ctx c, int x0_zero)
     const double t2 = block_sum<kVecThreads>(s2, red);
     if (threadIdx.x == 0) {
       s->counter[3] = 0u;
-      if (c.sh != nullptr) shard_post(c, t1, t2); else epi_setup(epi_ctx(c), t1, t2);
+      if (c.sh != nullptr) shard_reduce_point(c, kEpiSetup, t1, t2); else epi_setup(epi_ctx(c), t1, t2);
     }
   }
 }
@@ -329,9 +329,12 @@ __global__ void __launch_bounds__(kVecThreads) k_finalize(const Ctx c, int true_
       rr = fma(t, t, rr);
     }
   }
-  if (c.sh != nullptr && s->zero_x) return;  // b = 0 on every rank: k_epi sets relres_true = 0 without a reduction
+  if (c.sh != nullptr && s->zero_x) {  // b = 0 on every rank: no reduction
+    if (blockIdx.x == 0 && threadIdx.x == 0) s->relres_true = 0.0;
+    return;
+  }
   grid_reduce<kVecThreads>(rr, c.partials + 3 * kMaxGrid, &s->counter[3], blockIdx.x, gridDim.x, red, [&](double tot) {
-    if (c.sh != nullptr) shard_post(c, tot, 0.0);
+    if (c.sh != nullptr) shard_reduce_point(c, kEpiFinal, tot, 0.0);
     else s->relres_true = (s->bnorm > 0.0) ? sqrt(tot) / s->bnorm : 0.0;
   });
 }

@@ -96,12 +96,18 @@ __device__ __noinline__ void pxrz(const Ctx& c, int ur, int urn, int uz, int uzn
   dispatch_xrz<kPersistBIF>(c, ur, urn, uz, uzn, alpha, omega_n, x, bid, nb, rr, rz);
 }
 
-__global__ void __launch_bounds__(kPersistThreads, kPersistMinBlocks) k_persistent(const Ctx c) {
+__global__ void __launch_bounds__(kPersistThreads, kPersistMinBlocks) k_persistent(const Ctx cparam) {
   __shared__ double red[32];
   __shared__ DevState ls;  // this block's replica of the loop scalars
+  // The out-of-line phase dispatchers take the context by reference.  A reference to the kernel parameter would make
+  // every thread keep a 600-byte copy of it on its stack and read every pointer from local memory (round 1: 1.7 KB of
+  // stack, 1800 local loads and stores); one copy per block in shared memory is read with plain LDS instead.
+  __shared__ Ctx cshared;
   const int bid = blockIdx.x, nb = gridDim.x;
+  if (threadIdx.x == 0) cshared = cparam;  // (a plain assignment: taking the parameter's address would spill it again)
+  const Ctx& c = cshared;
   {  // replicate the state block (written by the host and the set-up kernel before this launch)
-    const int* src = reinterpret_cast<const int*>(c.st);
+    const int* src = reinterpret_cast<const int*>(cparam.st);
     int* dst = reinterpret_cast<int*>(&ls);
     for (int i = threadIdx.x; i < (int)(sizeof(DevState) / sizeof(int)); i += kPersistThreads) dst[i] = __ldcg(src + i);
   }

@@ -246,21 +246,67 @@ __device__ __forceinline__ void count_fp16(DevState* s, double v, double h) {
 // ------------------------------------------------------------------ a2: z and rho ------------
 // RS: precision r is stored in; UR: precision selected for r (RS != UR only at the iteration of
 // the u_r switch, where r <- RN32(r) is fused here, step a6); UZ: precision of z.
-template <int RS, int UR, int UZ, int BIF = kVecBytesInFlight>
-__device__ __forceinline__ double phase_z(const Ctx& c, const double omega, int bid, int nb) {
+// Every vector step below comes as (1) a traits struct with its storage types and chunk size E, (2) a chunk body: the
+// arithmetic of ONE chunk of E consecutive elements from raw loaded chunks, shared by (3) the direct driver (every
+// thread loads its chunks from global memory, U chunks in flight) and the staged drivers of vec_pipe.cuh (the input
+// streams arrive in shared memory through bulk copies).
+template <int RS, int UR, int UZ> struct ZT {
   using TR = typename Store<RS>::T;
   using TO = typename Store<UR>::T;
   using TZ = typename Store<UZ>::T;
   using TD = typename Store<(UZ == P64) ? P64 : P32>::T;
-  constexpr int smin = cmin(cmin((int)sizeof(TR), (int)sizeof(TO)), cmin((int)sizeof(TD), (int)sizeof(TZ)));
-  constexpr int smax = cmax(cmax((int)sizeof(TR), (int)sizeof(TO)), cmax((int)sizeof(TD), (int)sizeof(TZ)));
-  constexpr int E = chunk_elems(smin, smax);
+  static constexpr int smin = cmin(cmin((int)sizeof(TR), (int)sizeof(TO)), cmin((int)sizeof(TD), (int)sizeof(TZ)));
+  static constexpr int smax = cmax(cmax((int)sizeof(TR), (int)sizeof(TO)), cmax((int)sizeof(TD), (int)sizeof(TZ)));
+  static constexpr int E = chunk_elems(smin, smax);
+  static __device__ __forceinline__ const TD* dinv(const Ctx& c) {
+    if constexpr (UZ == P64) return c.dinv64; else return c.dinv32;
+  }
+};
+// z = RN_{u_z}((r omega) dinv) for chunk i; sum += r^T z with the STORED z (Alg 4.1 lines 4-6)
+template <int RS, int UR, int UZ>
+__device__ __forceinline__ void z_chunk(const Ctx& c, const double omega, const Chunk<typename ZT<RS, UR, UZ>::TR, ZT<RS, UR, UZ>::E>& rr,
+                                        const Chunk<typename ZT<RS, UR, UZ>::TD, ZT<RS, UR, UZ>::E>& dd, const int64_t i, double& sum) {
+  using T = ZT<RS, UR, UZ>;
+  constexpr int E = T::E;
+  double a[E], d[E], zz[E];
+  chunk_unpack(rr, a);
+  chunk_unpack(dd, d);
+  if constexpr (RS != UR) {  // r <- RN_{u_r}(r) at the switch iteration
+    Chunk<typename T::TO, E> ro;
+    chunk_pack(ro, a);
+    chunk_store(ro, rvec<UR>(c), i);
+    chunk_unpack(ro, a);
+  }
+#pragma unroll
+  for (int e = 0; e < E; ++e) zz[e] = (a[e] * omega) * d[e];
+  Chunk<typename T::TZ, E> zo;
+  chunk_pack(zo, zz);  // the one rounding to u_z (reading R6)
+  chunk_store(zo, zvec<UZ>(c), i);
+#ifdef AMP_COUNT_FP16
+  double zx[E];
+#pragma unroll
+  for (int e = 0; e < E; ++e) zx[e] = zz[e];
+#endif
+  chunk_unpack(zo, zz);
+#ifdef AMP_COUNT_FP16
+  if (UZ == P16) {
+#pragma unroll
+    for (int e = 0; e < E; ++e) count_fp16(c.st, zx[e], zz[e]);
+  }
+#endif
+#pragma unroll
+  for (int e = 0; e < E; ++e) sum = fma(a[e], zz[e], sum);  // rho uses the stored z
+}
+
+template <int RS, int UR, int UZ, int BIF = kVecBytesInFlight>
+__device__ __forceinline__ double phase_z(const Ctx& c, const double omega, int bid, int nb) {
+  using T = ZT<RS, UR, UZ>;
+  using TR = typename T::TR;
+  using TD = typename T::TD;
+  constexpr int E = T::E;
   constexpr int U = cmax(1, BIF / (E * (int)(sizeof(TR) + sizeof(TD))));
   const TR* rin = rvec<RS>(c);
-  TO* rout = rvec<UR>(c);
-  TZ* z = zvec<UZ>(c);
-  const TD* dinv;
-  if constexpr (UZ == P64) dinv = c.dinv64; else dinv = c.dinv32;
+  const TD* dinv = T::dinv(c);
   const int64_t nchunk = c.npad / E;
   const int64_t stride = (int64_t)nb * blockDim.x;
   double sum = 0.0;
@@ -275,36 +321,7 @@ __device__ __forceinline__ double phase_z(const Ctx& c, const double omega, int 
 #pragma unroll
     for (int u = 0; u < U; ++u) {
       const int64_t i = base + u * stride;
-      if (i < nchunk) {
-        double a[E], d[E], zz[E];
-        chunk_unpack(rr[u], a);
-        chunk_unpack(dd[u], d);
-        if constexpr (RS != UR) {  // r <- RN_{u_r}(r) at the switch iteration
-          Chunk<TO, E> ro;
-          chunk_pack(ro, a);
-          chunk_store(ro, rout, i);
-          chunk_unpack(ro, a);
-        }
-#pragma unroll
-        for (int e = 0; e < E; ++e) zz[e] = (a[e] * omega) * d[e];
-        Chunk<TZ, E> zo;
-        chunk_pack(zo, zz);  // the one rounding to u_z (reading R6)
-        chunk_store(zo, z, i);
-#ifdef AMP_COUNT_FP16
-        double zx[E];
-#pragma unroll
-        for (int e = 0; e < E; ++e) zx[e] = zz[e];
-#endif
-        chunk_unpack(zo, zz);
-#ifdef AMP_COUNT_FP16
-        if (UZ == P16) {
-#pragma unroll
-          for (int e = 0; e < E; ++e) count_fp16(c.st, zx[e], zz[e]);
-        }
-#endif
-#pragma unroll
-        for (int e = 0; e < E; ++e) sum = fma(a[e], zz[e], sum);  // rho uses the stored z
-      }
+      if (i < nchunk) z_chunk<RS, UR, UZ>(c, omega, rr[u], dd[u], i, sum);
     }
   }
   return sum;
@@ -445,24 +462,77 @@ __device__ __forceinline__ double phase_cheb_step(const Ctx& c, const double ome
 // shadow32 (only with UZ = P64): also store RN32(p) into the FP32 copy of p.  While u_z = FP64 and u_r = FP32 the
 // mat-vec needs RN32(p_j) for every gathered entry (reading R7); rounding each row once here instead of once per
 // gather there takes an FP64->FP32 conversion per ENTRY out of the SpMV (c4: 27 per row) for 4 B per row more here.
-// PUSH (row-sharded solve, k_p_sh): chunks inside a send range are also stored into the neighbour's halo band.
-template <int PS, int UZ, int BIF = kVecBytesInFlight, bool PUSH = false>
-__device__ __forceinline__ void phase_p(const Ctx& c, const double beta, const bool first, const bool shadow32, int bid, int nb) {
+// PUSH (row-sharded solve, k_p_sh): chunks inside a send range are also stored into the neighbour's halo band, in the
+// precision the mat-vec gathers (the FP32 copy in the shadow32 phase).
+template <int PS, int UZ> struct PT_ {
   using TP = typename Store<PS>::T;
   using TZ = typename Store<UZ>::T;
-  constexpr int E = chunk_elems(cmin((int)sizeof(TP), (int)sizeof(TZ)), cmax((int)sizeof(TP), (int)sizeof(TZ)));
+  static constexpr int E = chunk_elems(cmin((int)sizeof(TP), (int)sizeof(TZ)), cmax((int)sizeof(TP), (int)sizeof(TZ)));
+};
+template <int UZ> struct PPush {  // where the chunks of the send ranges go (all null unless PUSH)
+  HaloPush<typename Store<UZ>::T> hp{nullptr, nullptr, 0, 0, 0};
+  HaloPush<float> hp32{nullptr, nullptr, 0, 0, 0};
+};
+// p = RN_{u_z}(fma(beta, RN_{u_z}(p), z)) for chunk i (Alg 4.1 line 10); first: p = z
+template <int PS, int UZ, bool PUSH>
+__device__ __forceinline__ void p_chunk(const Ctx& c, const double beta, const bool first, const bool shadow32, const PPush<UZ>& ph,
+                                        const Chunk<typename PT_<PS, UZ>::TZ, PT_<PS, UZ>::E>& zz,
+                                        const Chunk<typename PT_<PS, UZ>::TP, PT_<PS, UZ>::E>& pp, const int64_t i) {
+  using T = PT_<PS, UZ>;
+  constexpr int E = T::E;
+  double a[E], zv[E];
+  chunk_unpack(zz, zv);
+  if (!first) {
+    chunk_unpack(pp, a);
+    if constexpr (PS != UZ) {
+#pragma unroll
+      for (int e = 0; e < E; ++e) a[e] = round_to<UZ>(a[e]);
+    }
+  } else {
+#pragma unroll
+    for (int e = 0; e < E; ++e) a[e] = 0.0;
+  }
+#pragma unroll
+  for (int e = 0; e < E; ++e) a[e] = fma(beta, a[e], zv[e]);
+  Chunk<typename T::TZ, E> po;
+  chunk_pack(po, a);
+  chunk_store(po, pvec<UZ>(c), i);
+  bool pushed = false;
+  if constexpr (UZ == P64) {
+    if (shadow32) {
+      Chunk<float, E> p32;
+      chunk_pack(p32, a);
+      chunk_store(p32, c.p32, i);
+      if constexpr (PUSH) halo_push_chunk(ph.hp32, p32, i);
+      pushed = true;
+    }
+  }
+  if constexpr (PUSH) {
+    if (!pushed) halo_push_chunk(ph.hp, po, i);
+  }
+#ifdef AMP_COUNT_FP16
+  if (UZ == P16) {
+    double h[E];
+    chunk_unpack(po, h);
+#pragma unroll
+    for (int e = 0; e < E; ++e) count_fp16(c.st, a[e], h[e]);
+  }
+#endif
+}
+
+template <int PS, int UZ, int BIF = kVecBytesInFlight, bool PUSH = false>
+__device__ __forceinline__ void phase_p(const Ctx& c, const double beta, const bool first, const bool shadow32, int bid, int nb) {
+  using T = PT_<PS, UZ>;
+  using TP = typename T::TP;
+  using TZ = typename T::TZ;
+  constexpr int E = T::E;
   constexpr int U = cmax(1, BIF / (E * (int)(sizeof(TP) + sizeof(TZ))));
   const TP* pin = pvec<PS>(c);
-  TZ* pout = pvec<UZ>(c);
   const TZ* z = zvec<UZ>(c);
   const int64_t nchunk = c.npad / E;
   const int64_t stride = (int64_t)nb * blockDim.x;
-  // row-sharded solve: chunks inside a send range are also stored into the neighbour's halo band, in the precision the
-  // mat-vec gathers (the FP32 copy in the shadow32 phase)
-  constexpr bool push = PUSH;
-  HaloPush<TZ> hp{nullptr, nullptr, 0, 0, 0};
-  HaloPush<float> hp32{nullptr, nullptr, 0, 0, 0};
-  if constexpr (PUSH) { hp = halo_push_of<UZ>(c); hp32 = halo_push_of<P32>(c); }
+  PPush<UZ> ph;
+  if constexpr (PUSH) { ph.hp = halo_push_of<UZ>(c); ph.hp32 = halo_push_of<P32>(c); }
   for (int64_t base = (int64_t)bid * blockDim.x + threadIdx.x; base < nchunk; base += stride * U) {
     Chunk<TP, E> pp[U];
     Chunk<TZ, E> zz[U];
@@ -477,58 +547,75 @@ __device__ __forceinline__ void phase_p(const Ctx& c, const double beta, const b
 #pragma unroll
     for (int u = 0; u < U; ++u) {
       const int64_t i = base + u * stride;
-      if (i < nchunk) {
-        double a[E], zv[E];
-        chunk_unpack(zz[u], zv);
-        if (!first) {
-          chunk_unpack(pp[u], a);
-          if constexpr (PS != UZ) {
-#pragma unroll
-            for (int e = 0; e < E; ++e) a[e] = round_to<UZ>(a[e]);
-          }
-        } else {
-#pragma unroll
-          for (int e = 0; e < E; ++e) a[e] = 0.0;
-        }
-#pragma unroll
-        for (int e = 0; e < E; ++e) a[e] = fma(beta, a[e], zv[e]);
-        Chunk<TZ, E> po;
-        chunk_pack(po, a);
-        chunk_store(po, pout, i);
-        bool pushed = false;
-        if constexpr (UZ == P64) {
-          if (shadow32) {
-            Chunk<float, E> p32;
-            chunk_pack(p32, a);
-            chunk_store(p32, c.p32, i);
-            if (push) halo_push_chunk(hp32, p32, i);
-            pushed = true;
-          }
-        }
-        if (push && !pushed) halo_push_chunk(hp, po, i);
-#ifdef AMP_COUNT_FP16
-        if (UZ == P16) {
-          double h[E];
-          chunk_unpack(po, h);
-#pragma unroll
-          for (int e = 0; e < E; ++e) count_fp16(c.st, a[e], h[e]);
-        }
-#endif
-      }
+      if (i < nchunk) p_chunk<PS, UZ, PUSH>(c, beta, first, shadow32, ph, zz[u], pp[u], i);
     }
   }
 }
 
 // ------------------------------------------------------------------ a5: x, r, delta ---------
-template <int UR, int UZ, int BIF = kVecBytesInFlight>
-__device__ __forceinline__ double phase_xr(const Ctx& c, const double alpha, double* x, int bid, int nb) {
+template <int UR, int UZ> struct XRT {
   using TZ = typename Store<UZ>::T;
   using TR = typename Store<UR>::T;
-  constexpr int E = chunk_elems(cmin((int)sizeof(TZ), (int)sizeof(TR)), 8);
+  static constexpr int E = chunk_elems(cmin((int)sizeof(TZ), (int)sizeof(TR)), 8);
+};
+// chunk i of x, which is caller-owned and exactly n long: the last chunk may be partial
+template <int E> __device__ __forceinline__ void x_chunk_load(Chunk<double, E>& k, const double* x, const int64_t i, const int64_t n) {
+  if ((i + 1) * E <= n) {
+    chunk_load(k, x, i);
+  } else {
+    double t[E];
+#pragma unroll
+    for (int e = 0; e < E; ++e) t[e] = (i * E + e < n) ? x[i * E + e] : 0.0;
+    chunk_pack(k, t);
+  }
+}
+template <int E> __device__ __forceinline__ void x_chunk_store(const double (&xv)[E], double* x, const int64_t i, const int64_t n) {
+  if ((i + 1) * E <= n) {
+    Chunk<double, E> xo;
+    chunk_pack(xo, xv);
+    chunk_store(xo, x, i);
+  } else {
+#pragma unroll
+    for (int e = 0; e < E; ++e)
+      if (i * E + e < n) x[i * E + e] = xv[e];
+  }
+}
+// x += alpha p (FP64); r = RN_{u_r}(fma(-alpha, q, r)); sum += r^2 with the stored r (Alg 4.1 lines 15-17)
+template <int UR, int UZ>
+__device__ __forceinline__ void xr_chunk(const Ctx& c, const double alpha, double* x, const Chunk<double, XRT<UR, UZ>::E>& xx,
+                                         const Chunk<typename XRT<UR, UZ>::TZ, XRT<UR, UZ>::E>& pp,
+                                         const Chunk<typename XRT<UR, UZ>::TR, XRT<UR, UZ>::E>& qq,
+                                         const Chunk<typename XRT<UR, UZ>::TR, XRT<UR, UZ>::E>& rr, const int64_t i, double& sum) {
+  using T = XRT<UR, UZ>;
+  constexpr int E = T::E;
+  double xv[E], pv[E], qv[E], rv[E];
+  chunk_unpack(xx, xv);
+  chunk_unpack(pp, pv);
+  chunk_unpack(qq, qv);
+  chunk_unpack(rr, rv);
+#pragma unroll
+  for (int e = 0; e < E; ++e) xv[e] = fma(alpha, pv[e], xv[e]);  // line 15, FP64
+  x_chunk_store<E>(xv, x, i, c.n);
+#pragma unroll
+  for (int e = 0; e < E; ++e) rv[e] = fma(-alpha, qv[e], rv[e]);  // line 16
+  Chunk<typename T::TR, E> ro;
+  chunk_pack(ro, rv);  // one rounding to u_r
+  chunk_store(ro, rvec<UR>(c), i);
+  chunk_unpack(ro, rv);
+#pragma unroll
+  for (int e = 0; e < E; ++e) sum = fma(rv[e], rv[e], sum);
+}
+
+template <int UR, int UZ, int BIF = kVecBytesInFlight>
+__device__ __forceinline__ double phase_xr(const Ctx& c, const double alpha, double* x, int bid, int nb) {
+  using T = XRT<UR, UZ>;
+  using TZ = typename T::TZ;
+  using TR = typename T::TR;
+  constexpr int E = T::E;
   constexpr int U = cmax(1, BIF / (E * (int)(8 + sizeof(TZ) + 2 * sizeof(TR))));
   const TZ* p = pvec<UZ>(c);
   const TR* q = qvec<UR>(c);
-  TR* r = rvec<UR>(c);
+  const TR* r = rvec<UR>(c);
   const int64_t n = c.n;
   const int64_t nchunk = c.npad / E;
   const int64_t stride = (int64_t)nb * blockDim.x;
@@ -541,14 +628,7 @@ __device__ __forceinline__ double phase_xr(const Ctx& c, const double alpha, dou
     for (int u = 0; u < U; ++u) {
       const int64_t i = base + u * stride;
       if (i < nchunk) {
-        if ((i + 1) * E <= n) {
-          chunk_load(xx[u], x, i);
-        } else {  // x is caller-owned: exactly n long
-          double t[E];
-#pragma unroll
-          for (int e = 0; e < E; ++e) t[e] = (i * E + e < n) ? x[i * E + e] : 0.0;
-          chunk_pack(xx[u], t);
-        }
+        x_chunk_load<E>(xx[u], x, i, n);
         chunk_load(pp[u], p, i);
         chunk_load(qq[u], q, i);
         chunk_load(rr[u], r, i);
@@ -557,32 +637,7 @@ __device__ __forceinline__ double phase_xr(const Ctx& c, const double alpha, dou
 #pragma unroll
     for (int u = 0; u < U; ++u) {
       const int64_t i = base + u * stride;
-      if (i < nchunk) {
-        double xv[E], pv[E], qv[E], rv[E];
-        chunk_unpack(xx[u], xv);
-        chunk_unpack(pp[u], pv);
-        chunk_unpack(qq[u], qv);
-        chunk_unpack(rr[u], rv);
-#pragma unroll
-        for (int e = 0; e < E; ++e) xv[e] = fma(alpha, pv[e], xv[e]);  // line 15, FP64
-        if ((i + 1) * E <= n) {
-          Chunk<double, E> xo;
-          chunk_pack(xo, xv);
-          chunk_store(xo, x, i);
-        } else {
-#pragma unroll
-          for (int e = 0; e < E; ++e)
-            if (i * E + e < n) x[i * E + e] = xv[e];
-        }
-#pragma unroll
-        for (int e = 0; e < E; ++e) rv[e] = fma(-alpha, qv[e], rv[e]);  // line 16
-        Chunk<TR, E> ro;
-        chunk_pack(ro, rv);  // one rounding to u_r
-        chunk_store(ro, r, i);
-        chunk_unpack(ro, rv);
-#pragma unroll
-        for (int e = 0; e < E; ++e) sum = fma(rv[e], rv[e], sum);
-      }
+      if (i < nchunk) xr_chunk<UR, UZ>(c, alpha, x, xx[u], pp[u], qq[u], rr[u], i, sum);
     }
   }
   return sum;
@@ -591,24 +646,77 @@ __device__ __forceinline__ double phase_xr(const Ctx& c, const double alpha, dou
 // ------------------------------------------------------------------ lagged: a5 + a2 in one pass
 // x += alpha p (FP64); r <- RN_{URN}(r - alpha q); delta^2 += r^2; z = RN_{UZN}((r omega_n) dinv); rho += r z.
 // UR / UZ: precisions of iteration k (q, r as read, p); URN / UZN: of iteration k+1 (r as written, z).
-template <int UR, int URN, int UZ, int UZN, int BIF = kVecBytesInFlight>
-__device__ __forceinline__ void phase_xrz(const Ctx& c, const double alpha, const double omega_n, double* x, int bid, int nb,
-                                          double& sum_rr, double& sum_rz) {
+template <int UR, int URN, int UZ, int UZN> struct XRZT {
   using TP = typename Store<UZ>::T;
   using TR = typename Store<UR>::T;
   using TO = typename Store<URN>::T;
   using TZ = typename Store<UZN>::T;
   using TD = typename Store<(UZN == P64) ? P64 : P32>::T;
-  constexpr int smin = cmin(cmin((int)sizeof(TP), (int)sizeof(TR)), cmin((int)sizeof(TO), (int)sizeof(TZ)));
-  constexpr int E = chunk_elems(smin, 8);
+  static constexpr int smin = cmin(cmin((int)sizeof(TP), (int)sizeof(TR)), cmin((int)sizeof(TO), (int)sizeof(TZ)));
+  static constexpr int E = chunk_elems(smin, 8);
+  static __device__ __forceinline__ const TD* dinv(const Ctx& c) {
+    if constexpr (UZN == P64) return c.dinv64; else return c.dinv32;
+  }
+};
+template <int UR, int URN, int UZ, int UZN>
+__device__ __forceinline__ void xrz_chunk(const Ctx& c, const double alpha, const double omega_n, double* x,
+                                          const Chunk<double, XRZT<UR, URN, UZ, UZN>::E>& xx,
+                                          const Chunk<typename XRZT<UR, URN, UZ, UZN>::TP, XRZT<UR, URN, UZ, UZN>::E>& pp,
+                                          const Chunk<typename XRZT<UR, URN, UZ, UZN>::TR, XRZT<UR, URN, UZ, UZN>::E>& qq,
+                                          const Chunk<typename XRZT<UR, URN, UZ, UZN>::TR, XRZT<UR, URN, UZ, UZN>::E>& rr,
+                                          const Chunk<typename XRZT<UR, URN, UZ, UZN>::TD, XRZT<UR, URN, UZ, UZN>::E>& dd, const int64_t i,
+                                          double& srr, double& srz) {
+  using T = XRZT<UR, URN, UZ, UZN>;
+  constexpr int E = T::E;
+  double xv[E], pv[E], qv[E], rv[E], dv[E], zv[E];
+  chunk_unpack(xx, xv);
+  chunk_unpack(pp, pv);
+  chunk_unpack(qq, qv);
+  chunk_unpack(rr, rv);
+  chunk_unpack(dd, dv);
+#pragma unroll
+  for (int e = 0; e < E; ++e) xv[e] = fma(alpha, pv[e], xv[e]);  // line 15, FP64
+  x_chunk_store<E>(xv, x, i, c.n);
+#pragma unroll
+  for (int e = 0; e < E; ++e) rv[e] = fma(-alpha, qv[e], rv[e]);  // line 16
+  Chunk<typename T::TO, E> ro;
+  chunk_pack(ro, rv);  // one rounding, to the precision of iteration k+1
+  chunk_store(ro, rvec<URN>(c), i);
+  chunk_unpack(ro, rv);
+#pragma unroll
+  for (int e = 0; e < E; ++e) zv[e] = (rv[e] * omega_n) * dv[e];  // lines 4-5 of iteration k+1
+  Chunk<typename T::TZ, E> zo;
+  chunk_pack(zo, zv);
+  chunk_store(zo, zvec<UZN>(c), i);
+#ifdef AMP_COUNT_FP16
+  double zx[E];
+#pragma unroll
+  for (int e = 0; e < E; ++e) zx[e] = zv[e];
+#endif
+  chunk_unpack(zo, zv);
+#ifdef AMP_COUNT_FP16
+  if (UZN == P16) {
+#pragma unroll
+    for (int e = 0; e < E; ++e) count_fp16(c.st, zx[e], zv[e]);
+  }
+#endif
+#pragma unroll
+  for (int e = 0; e < E; ++e) { srr = fma(rv[e], rv[e], srr); srz = fma(rv[e], zv[e], srz); }
+}
+
+template <int UR, int URN, int UZ, int UZN, int BIF = kVecBytesInFlight>
+__device__ __forceinline__ void phase_xrz(const Ctx& c, const double alpha, const double omega_n, double* x, int bid, int nb,
+                                          double& sum_rr, double& sum_rz) {
+  using T = XRZT<UR, URN, UZ, UZN>;
+  using TP = typename T::TP;
+  using TR = typename T::TR;
+  using TD = typename T::TD;
+  constexpr int E = T::E;
   constexpr int U = cmax(1, BIF / (E * (int)(8 + sizeof(TP) + 2 * sizeof(TR) + sizeof(TD))));
   const TP* p = pvec<UZ>(c);
   const TR* q = qvec<UR>(c);
   const TR* rin = rvec<UR>(c);
-  TO* rout = rvec<URN>(c);
-  TZ* z = zvec<UZN>(c);
-  const TD* dinv;
-  if constexpr (UZN == P64) dinv = c.dinv64; else dinv = c.dinv32;
+  const TD* dinv = T::dinv(c);
   const int64_t n = c.n;
   const int64_t nchunk = c.npad / E;
   const int64_t stride = (int64_t)nb * blockDim.x;
@@ -622,14 +730,7 @@ __device__ __forceinline__ void phase_xrz(const Ctx& c, const double alpha, cons
     for (int u = 0; u < U; ++u) {
       const int64_t i = base + u * stride;
       if (i < nchunk) {
-        if ((i + 1) * E <= n) {
-          chunk_load(xx[u], x, i);
-        } else {  // x is caller-owned: exactly n long
-          double t[E];
-#pragma unroll
-          for (int e = 0; e < E; ++e) t[e] = (i * E + e < n) ? x[i * E + e] : 0.0;
-          chunk_pack(xx[u], t);
-        }
+        x_chunk_load<E>(xx[u], x, i, n);
         chunk_load(pp[u], p, i);
         chunk_load(qq[u], q, i);
         chunk_load(rr[u], rin, i);
@@ -639,50 +740,7 @@ __device__ __forceinline__ void phase_xrz(const Ctx& c, const double alpha, cons
 #pragma unroll
     for (int u = 0; u < U; ++u) {
       const int64_t i = base + u * stride;
-      if (i < nchunk) {
-        double xv[E], pv[E], qv[E], rv[E], dv[E], zv[E];
-        chunk_unpack(xx[u], xv);
-        chunk_unpack(pp[u], pv);
-        chunk_unpack(qq[u], qv);
-        chunk_unpack(rr[u], rv);
-        chunk_unpack(dd[u], dv);
-#pragma unroll
-        for (int e = 0; e < E; ++e) xv[e] = fma(alpha, pv[e], xv[e]);  // line 15, FP64
-        if ((i + 1) * E <= n) {
-          Chunk<double, E> xo;
-          chunk_pack(xo, xv);
-          chunk_store(xo, x, i);
-        } else {
-#pragma unroll
-          for (int e = 0; e < E; ++e)
-            if (i * E + e < n) x[i * E + e] = xv[e];
-        }
-#pragma unroll
-        for (int e = 0; e < E; ++e) rv[e] = fma(-alpha, qv[e], rv[e]);  // line 16
-        Chunk<TO, E> ro;
-        chunk_pack(ro, rv);  // one rounding, to the precision of iteration k+1
-        chunk_store(ro, rout, i);
-        chunk_unpack(ro, rv);
-#pragma unroll
-        for (int e = 0; e < E; ++e) zv[e] = (rv[e] * omega_n) * dv[e];  // lines 4-5 of iteration k+1
-        Chunk<TZ, E> zo;
-        chunk_pack(zo, zv);
-        chunk_store(zo, z, i);
-#ifdef AMP_COUNT_FP16
-        double zx[E];
-#pragma unroll
-        for (int e = 0; e < E; ++e) zx[e] = zv[e];
-#endif
-        chunk_unpack(zo, zv);
-#ifdef AMP_COUNT_FP16
-        if (UZN == P16) {
-#pragma unroll
-          for (int e = 0; e < E; ++e) count_fp16(c.st, zx[e], zv[e]);
-        }
-#endif
-#pragma unroll
-        for (int e = 0; e < E; ++e) { srr = fma(rv[e], rv[e], srr); srz = fma(rv[e], zv[e], srz); }
-      }
+      if (i < nchunk) xrz_chunk<UR, URN, UZ, UZN>(c, alpha, omega_n, x, xx[u], pp[u], qq[u], rr[u], dd[u], i, srr, srz);
     }
   }
   sum_rr = srr;

@@ -34,6 +34,17 @@ __device__ __forceinline__ unsigned long long global_timer_ns() {
   asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
   return t;
 }
+// wait until *p == want with relaxed loads (the caller fences once after all its waits); false on timeout
+__device__ __forceinline__ bool shard_spin_relaxed(const unsigned long long* p, unsigned long long want) {
+  const volatile unsigned long long* vp = p;
+  if (*vp == want) return true;
+  const unsigned long long t0 = global_timer_ns();
+  while (*vp != want) {
+    if (global_timer_ns() - t0 > kShardTimeoutNs) return false;
+    __nanosleep(50);
+  }
+  return true;
+}
 // wait until *p == want; false on timeout
 __device__ __forceinline__ bool shard_spin(const unsigned long long* p, unsigned long long want) {
   if (ld_acquire_sys_u64(p) == want) return true;
@@ -52,9 +63,10 @@ __device__ __forceinline__ int shard_slot(const DevState* s, unsigned int xseq) 
 }
 
 // ---- sums: post this rank's partial sums of the reduction point that follows s->xseq completed ones (one thread) ----
-__device__ __noinline__ void shard_post(const Ctx& c, double v0, double v1) {
-  const ShardCtx* sh = c.sh;
-  const DevState* s = c.st;
+// Values to every rank first, ONE system-scope fence, then the tags (fence + relaxed store = release): the cost of a
+// reduction point does not grow with a fence per peer.
+// (small arguments by value: a reference to the kernel's Ctx would force a stack copy of the whole parameter block)
+__device__ __noinline__ void shard_post(const DevState* s, const ShardCtx* sh, double v0, double v1) {
   const unsigned int xseq = s->xseq;
   const unsigned long long tag = shard_tag(s, xseq + 1u);
   const int slot = shard_slot(s, xseq) + sh->rank;
@@ -62,8 +74,9 @@ __device__ __noinline__ void shard_post(const Ctx& c, double v0, double v1) {
     Mail* m = sh->peer_mbox[r] + slot;
     *reinterpret_cast<volatile double*>(&m->v0) = v0;
     *reinterpret_cast<volatile double*>(&m->v1) = v1;
-    st_release_sys_u64(&m->tag, tag);  // orders the two value stores before the tag, system scope
   }
+  __threadfence_system();
+  for (int r = 0; r < sh->world; ++r) *reinterpret_cast<volatile unsigned long long*>(&(sh->peer_mbox[r] + slot)->tag) = tag;
 }
 
 // ---- halo: wait until both neighbours have completed their push with sequence number seq (whole block) ----
@@ -133,39 +146,21 @@ __global__ void __launch_bounds__(kVecThreads) k_shard_load_p(const Ctx c, const
 // ---- the scalar step of a reduction point, from the partial sums of all ranks ----
 enum { kEpiSetup = 0, kEpiRho = 1, kEpiGamma = 2, kEpiDelta = 3, kEpiDeltaLagged = 4, kEpiFinal = 5 };
 
-__global__ void __launch_bounds__(32) k_epi(const Ctx c, int which) {
-  pdl_launch_dependents();
-  pdl_wait();
-  DevState* s = c.st;
-  const ShardCtx* sh = c.sh;
-  const int lane = threadIdx.x;
-  const EpiCtx ec = epi_ctx(c);
-  const bool in_loop = which >= kEpiRho && which <= kEpiDeltaLagged;
-  if (in_loop && s->done) {  // the reducing kernel returned without posting (converged, breakdown, time-out)
-    if (lane == 0 && (which == kEpiDelta || which == kEpiDeltaLagged)) set_loop_cond(ec, 0);
-    return;
-  }
-  if (which == kEpiFinal && s->zero_x) {  // b = 0 (identical on all ranks): nothing was posted
-    if (lane == 0) s->relres_true = 0.0;
-    return;
-  }
+// one thread: wait until the entries of all ranks carry the tag of the reduction point that follows s->xseq completed
+// ones, add them in rank order (the same sum on every rank), count the point, run the scalar step
+__device__ __noinline__ void shard_collect_and_step(const EpiCtx ec, const ShardCtx* sh, int which) {
+  DevState* s = ec.st;
   const unsigned int xseq = s->xseq;
   const unsigned long long tag = shard_tag(s, xseq + 1u);
-  const Mail* m = sh->mbox + shard_slot(s, xseq) + lane;
-  double v0 = 0.0, v1 = 0.0;
-  bool ok = true;
-  if (lane < sh->world) {
-    ok = shard_spin(&m->tag, tag);
-    v0 = *reinterpret_cast<const volatile double*>(&m->v0);
-    v1 = *reinterpret_cast<const volatile double*>(&m->v1);
-  }
-  ok = __all_sync(0xffffffffu, ok);
+  const Mail* m = sh->mbox + shard_slot(s, xseq);
   double t0 = 0.0, t1 = 0.0;
+  bool ok = true;
+  for (int r = 0; r < sh->world && ok; ++r) ok = shard_spin_relaxed(&m[r].tag, tag);
+  __threadfence_system();  // relaxed loads + fence = acquire: the values below are the ones posted before the tags
   for (int r = 0; r < sh->world; ++r) {  // rank order: the same sum on every rank
-    t0 += __shfl_sync(0xffffffffu, v0, r);
-    t1 += __shfl_sync(0xffffffffu, v1, r);
+    t0 += *reinterpret_cast<const volatile double*>(&m[r].v0);
+    t1 += *reinterpret_cast<const volatile double*>(&m[r].v1);
   }
-  if (lane != 0) return;
   s->xseq = xseq + 1u;
   if (!ok) {
     s->status = -3; s->done = 1;
@@ -180,6 +175,29 @@ __global__ void __launch_bounds__(32) k_epi(const Ctx c, int which) {
     case kEpiDeltaLagged: epi_delta_lagged(ec, t0, t1); break;
     default: s->relres_true = (s->bnorm > 0.0) ? sqrt(t0) / s->bnorm : 0.0; break;
   }
+}
+
+// what the thread that completes a grid reduction does in a sharded solve: publish, and — when the ranks run
+// concurrently — collect and step at once (no extra kernel on the critical path)
+__device__ __forceinline__ void shard_reduce_point(const Ctx& c, int which, double v0, double v1) {
+  shard_post(c.st, c.sh, v0, v1);
+  if (c.sh->inline_epi) shard_collect_and_step(epi_ctx(c), c.sh, which);
+}
+
+// the same step as a kernel of its own (one thread), for ranks that share a device: launched for every rank AFTER the
+// reducing kernels of all ranks, so that the wait finds every entry in place
+__global__ void __launch_bounds__(32) k_epi(const Ctx c, int which) {
+  pdl_launch_dependents();
+  pdl_wait();
+  if (threadIdx.x != 0) return;
+  DevState* s = c.st;
+  const bool in_loop = which >= kEpiRho && which <= kEpiDeltaLagged;
+  if (in_loop && s->done) {  // the reducing kernel returned without posting (converged, breakdown, time-out)
+    if (which == kEpiDelta || which == kEpiDeltaLagged) set_loop_cond(epi_ctx(c), 0);
+    return;
+  }
+  if (which == kEpiFinal && s->zero_x) return;  // b = 0 (identical on all ranks): nothing was posted
+  shard_collect_and_step(epi_ctx(c), c.sh, which);
 }
 
 }  // namespace amp

@@ -99,12 +99,13 @@ struct ShardPeer {  // what a rank needs to know about another rank
 };
 
 // build and upload this rank's peer table
-static int shard_wire(amp_pcg* h, int rank, int world, const ShardPeer* peers) {
+static int shard_wire(amp_pcg* h, int rank, int world, const ShardPeer* peers, bool concurrent) {
   const ShardPeer& me = peers[rank];
   if (me.n != h->n || me.halo_lo != h->halo_lo || me.halo_hi != h->halo_hi) { set_error("shard attach: inconsistent geometry of rank %d", rank); return AMP_ERR_INVALID; }
   ShardCtx sc;
   std::memset(&sc, 0, sizeof(sc));
   sc.rank = rank; sc.world = world;
+  sc.inline_epi = concurrent ? 1 : 0;
   sc.mbox = xchg_mbox(h->xchg);
   sc.flags = xchg_flags(h->xchg);
   for (int r = 0; r < world; ++r) sc.peer_mbox[r] = xchg_mbox(peers[r].xchg);
@@ -145,6 +146,7 @@ static int shard_wire(amp_pcg* h, int rank, int world, const ShardPeer* peers) {
   h->ctx.n_scale = 0;
   for (int r = 0; r < world; ++r) h->ctx.n_scale += peers[r].n;  // the n of omega = sqrt(n)/||r|| is the whole system's
   h->shard_rank = rank; h->shard_world = world; h->shard_epoch = 0;
+  h->shard_inline = concurrent ? 1 : 0;
   for (int i = 0; i < 2; ++i) {  // graphs captured with another wiring are stale
     if (h->graph_sh_exec[i]) { cudaGraphExecDestroy(h->graph_sh_exec[i]); h->graph_sh_exec[i] = nullptr; }
     if (h->graph_sh[i]) { cudaGraphDestroy(h->graph_sh[i]); h->graph_sh[i] = nullptr; }
@@ -177,8 +179,13 @@ extern "C" int amp_pcg_shard_attach_local(amp_pcg_t* const* handles, int32_t wor
         if (e != cudaSuccess && e != cudaErrorPeerAccessAlreadyEnabled) { set_error("cudaDeviceEnablePeerAccess failed: %s", cudaGetErrorString(e)); return AMP_ERR_CUDA; }
         cudaGetLastError();
       }
+  // ranks that share a device run one after the other: the scalar steps then need kernels of their own (k_epi), launched
+  // after the reducing kernels of ALL ranks; ranks on distinct devices (and a single rank) run concurrently
+  bool concurrent = true;
+  for (int r = 0; r < world; ++r)
+    for (int q = 0; q < r; ++q) concurrent = concurrent && handles[r]->device != handles[q]->device;
   for (int r = 0; r < world; ++r) {
-    const int rc = shard_wire(handles[r], r, world, peers);
+    const int rc = shard_wire(handles[r], r, world, peers, concurrent);
     if (rc != AMP_OK) return rc;
   }
   return AMP_OK;
@@ -245,7 +252,7 @@ extern "C" int amp_pcg_shard_attach(amp_pcg_t* h, int32_t rank, int32_t world, c
       }
     }
   }
-  return shard_wire(h, rank, world, peers);
+  return shard_wire(h, rank, world, peers, true);  // one process per GPU: all ranks run concurrently
 }
 
 // ------------------------------------------------------------------ driver ------------------------
@@ -253,16 +260,21 @@ enum ShardStep { SS_Z, SS_EPI_RHO, SS_P, SS_SPMV, SS_EPI_GAMMA, SS_XR, SS_EPI_DE
 static const int kShardStepsPlain[] = {SS_Z, SS_EPI_RHO, SS_P, SS_SPMV, SS_EPI_GAMMA, SS_XR, SS_EPI_DELTA};
 static const int kShardStepsLagged[] = {SS_P, SS_SPMV, SS_EPI_GAMMA, SS_XRZ, SS_EPI_DELTA_LAGGED};
 
+static bool shard_step_is_epi(int step) {
+  return step == SS_EPI_RHO || step == SS_EPI_GAMMA || step == SS_EPI_DELTA || step == SS_EPI_DELTA_LAGGED;
+}
+
 static cudaError_t launch_shard_step(amp_pcg* h, const Ctx& c, cudaStream_t s, bool pdl, int step) {
+  if (h->shard_inline && shard_step_is_epi(step)) return cudaSuccess;  // done by the reducing kernel itself
   switch (step) {
-    case SS_Z: return launch_loop_kernel(k_z, h->grid_z, kVecThreads, s, c, pdl);
+    case SS_Z: return launch_vec(h, VK_Z, s, c, pdl);
     case SS_EPI_RHO: return launch_loop_kernel_ex(k_epi, 1, 32, s, pdl, 0, c, (int)kEpiRho);
     case SS_P: return launch_loop_kernel(k_p_sh, h->grid_p_sh, kVecThreads, s, c, pdl);
     case SS_SPMV: return launch_spmv_loop(h, s, c, pdl);
     case SS_EPI_GAMMA: return launch_loop_kernel_ex(k_epi, 1, 32, s, pdl, 0, c, (int)kEpiGamma);
-    case SS_XR: return launch_loop_kernel(k_xr, h->grid_xr, kVecThreads, s, c, pdl);
+    case SS_XR: return launch_vec(h, VK_XR, s, c, pdl);
     case SS_EPI_DELTA: return launch_loop_kernel_ex(k_epi, 1, 32, s, pdl, 0, c, (int)kEpiDelta);
-    case SS_XRZ: return launch_loop_kernel(k_xrz, h->grid_xrz, kVecThreads, s, c, pdl);
+    case SS_XRZ: return launch_vec(h, VK_XRZ, s, c, pdl);
     default: return launch_loop_kernel_ex(k_epi, 1, 32, s, pdl, 0, c, (int)kEpiDeltaLagged);
   }
 }
@@ -285,7 +297,8 @@ static int shard_group_check(amp_pcg_t* const* handles, int32_t nlocal, const ch
   }
   for (int i = 0; i < nlocal; ++i) {
     const amp_pcg* h = handles[i];
-    if (!h || h->shard_world != world || (nlocal > 1 && h->shard_rank != i) || h->shard_epoch != handles[0]->shard_epoch) {
+    if (!h || h->shard_world != world || (nlocal > 1 && h->shard_rank != i) || h->shard_epoch != handles[0]->shard_epoch ||
+        h->shard_inline != handles[0]->shard_inline) {
       set_error("%s: handle %d does not belong to the group (rank order, group size or solve count differ)", who, i);
       return AMP_ERR_INVALID;
     }
@@ -339,10 +352,11 @@ extern "C" int amp_pcg_solve_sharded(amp_pcg_t* const* handles, int32_t nlocal, 
     FOR_RANKS(spmv_dispatch(h, AMP_FP64, AMP_FP64, h->ctx.p64, h->ctx.q64, kHaloTagSetup));
   }
   FOR_RANKS(k_setup<<<h->vec_grid, kVecThreads, 0, h->stream>>>(h->ctx, pol.x0_zero ? 1 : 0));
-  FOR_RANKS(k_epi<<<1, 32, 0, h->stream>>>(h->ctx, (int)kEpiSetup));
+  const bool split_epi = handles[0]->shard_inline == 0;
+  if (split_epi) { FOR_RANKS(k_epi<<<1, 32, 0, h->stream>>>(h->ctx, (int)kEpiSetup)); }
   if (lagged) {
-    FOR_RANKS(k_z<<<h->grid_z, kVecThreads, 0, h->stream>>>(h->ctx));
-    FOR_RANKS(k_epi<<<1, 32, 0, h->stream>>>(h->ctx, (int)kEpiRho));
+    FOR_RANKS(CU_TRY(launch_vec(h, VK_Z, h->stream, h->ctx, false), return AMP_ERR_CUDA));
+    if (split_epi) { FOR_RANKS(k_epi<<<1, 32, 0, h->stream>>>(h->ctx, (int)kEpiRho)); }
   }
   if (mode == AMP_LOOP_GRAPH) {
     FOR_RANKS(CU_TRY(cudaGraphLaunch(h->graph_sh_exec[lagged], h->stream), return AMP_ERR_CUDA));
@@ -379,7 +393,7 @@ extern "C" int amp_pcg_solve_sharded(amp_pcg_t* const* handles, int32_t nlocal, 
     FOR_RANKS(spmv_dispatch(h, AMP_FP64, AMP_FP64, h->ctx.p64, h->ctx.q64, kHaloTagFinal));
   }
   FOR_RANKS(k_finalize<<<h->vec_grid, kVecThreads, 0, h->stream>>>(h->ctx, pol.true_residual ? 1 : 0));
-  if (pol.true_residual) { FOR_RANKS(k_epi<<<1, 32, 0, h->stream>>>(h->ctx, (int)kEpiFinal)); }
+  if (pol.true_residual && split_epi) { FOR_RANKS(k_epi<<<1, 32, 0, h->stream>>>(h->ctx, (int)kEpiFinal)); }
   FOR_RANKS(CU_TRY(cudaMemcpyAsync(h->h_state, h->ctx.st, sizeof(DevState), cudaMemcpyDeviceToHost, h->stream), return AMP_ERR_CUDA));
   int status = AMP_OK;
   for (int i = 0; i < nlocal; ++i) {
@@ -392,8 +406,9 @@ extern "C" int amp_pcg_solve_sharded(amp_pcg_t* const* handles, int32_t nlocal, 
     const DevState* hs = h->h_state;
     h->last_iters = hs->k;
     const int spmv_k = h->use_pipe ? 2 : 1;
-    h->launches = 2 + (pol.x0_zero ? 0 : 2) + (lagged ? 2 : 0) + (pol.true_residual ? 4 : 1) +
-                  (int64_t)hs->k * ((lagged ? 4 : 6) + spmv_k);
+    const int epi = split_epi ? 1 : 0;  // k_epi launches per reduction point
+    h->launches = 1 + epi + (pol.x0_zero ? 0 : 2) + (lagged ? 1 + epi : 0) + (pol.true_residual ? 3 + epi : 1) +
+                  (int64_t)hs->k * ((lagged ? 2 : 3) + spmv_k + (lagged ? 2 : 3) * epi);
     if (stats) fill_stats(h, hs, mode, lagged, ms, stats + i);
     if (i == 0) status = hs->status;
     else if (hs->status != status || hs->k != handles[0]->h_state->k) {

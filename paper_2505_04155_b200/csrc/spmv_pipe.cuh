@@ -21,6 +21,7 @@
 // Under programmatic dependent launch the producer starts streaming the (constant) matrix BEFORE griddepcontrol.wait,
 // i.e. while the p update of the same iteration is still finishing.
 #pragma once
+#include "async_copy.cuh"
 #include "shard.cuh"
 #include "spmv.cuh"
 
@@ -39,35 +40,6 @@ constexpr int kPipeWptrInts = kPipeChunkSlices + 8;          // staged slice tab
 constexpr int kPipeSmemBytes = kPipeValueBytes + kPipeMaxStages * 4 * (kPipeBaseInts + kPipeWptrInts) +
                                kPipeMaxStages * 16 /* headers */ + 2 * kPipeMaxStages * 8 /* mbarriers */;
 constexpr int kPipeMaxGuard = 1 << 22;                       // elements of zero guard band per side we are willing to pay
-
-__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
-  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, uint32_t bytes) {
-  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
-  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
-  uint32_t ok;
-  do {
-    asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}"
-                 : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity) : "memory");
-  } while (!ok);
-}
-// 1-D bulk copy global -> shared (16-byte aligned addresses, size a multiple of 16), completion counted on bar;
-// L2 evict-first (the matrix is streamed once per mat-vec)
-__device__ __forceinline__ void bulk_g2s_stream(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
-  const uint64_t evict_first = 0x12F0000000000000ull;
-  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;"
-               ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)), "l"(evict_first) : "memory");
-}
-__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
-  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-               ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
-}
 
 // gather of p[j] converted to the working type; j may be negative or >= n (guard band)
 template <class A, class PT> __device__ __forceinline__ A pipe_gather(const PT* pl, int off) { return gatherA<false>(A(0), pl, off); }
@@ -255,7 +227,7 @@ __global__ void __launch_bounds__(kPipeThreads, 1) k_spmv_pipe(const Ctx c, int 
   else v = pipe_body<P32>(c, c.p32, c.p64, c.q32, pipe_smem, hseq);  // gathers the FP32 copy RN32(p) written by the p update
   pdl_wait();  // (the producer warp has not waited yet) before touching the reduction scratch shared with other kernels
   grid_reduce<kPipeThreads>(v, c.partials + 1 * kMaxGrid, &s->counter[1], blockIdx.x, gridDim.x, red,
-                            [&](double tot) { if (c.sh != nullptr) shard_post(c, tot, 0.0); else epi_gamma(epi_ctx(c), tot); });
+                            [&](double tot) { if (c.sh != nullptr) shard_reduce_point(c, kEpiGamma, tot, 0.0); else epi_gamma(epi_ctx(c), tot); });
 }
 
 }  // namespace amp

@@ -43,12 +43,16 @@ def special(rng, n, scale=1.0):
     return v
 
 
-@pytest.fixture(scope="module", params=[("c3", 11), ("c2", 47), ("c3", 107)], ids=lambda p: f"{p[0]}@{p[1]}")
+# every case with the direct vector kernels and with the bulk-copy staged ones (vec_pipe.cuh): same chunk bodies, same bits
+@pytest.fixture(scope="module", params=[("c3", 11, "direct"), ("c2", 47, "direct"), ("c3", 107, "direct"),
+                                        ("c3", 11, "staged"), ("c2", 47, "staged"), ("c3", 107, "staged")],
+                ids=lambda p: f"{p[0]}@{p[1]}-{p[2]}")
 def handle(request):
-    name, size = request.param
+    name, size, vec = request.param
     s = make_config(name, size)
     assert s.n % 2 == 1 and s.n % 8 != 0
-    h = A.AmpPcg(*(torch.from_numpy(a).cuda() for a in (s.rowptr, s.colidx, s.vals)), A.PRECOND_JACOBI)
+    h = A.AmpPcg(*(torch.from_numpy(a).cuda() for a in (s.rowptr, s.colidx, s.vals)), A.PRECOND_JACOBI,
+                 vec_kernel={"direct": A.VEC_DIRECT, "staged": A.VEC_STAGED}[vec])
     rows = np.repeat(np.arange(s.n), np.diff(s.rowptr))
     diag = s.vals[s.colidx == rows]
     assert len(diag) == s.n
