@@ -56,6 +56,7 @@ def parse_args():
     ap.add_argument("--loop", default="auto", choices=["auto", "stream", "graph", "persistent"])
     ap.add_argument("--spmv-kernel", default="auto", choices=["auto", "direct", "pipelined"])
     ap.add_argument("--vec-kernel", default="auto", choices=["auto", "direct", "staged"])
+    ap.add_argument("--fuse", default="auto", choices=["auto", "off", "on"], help="fused vector kernel (create option fuse_vec)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--others", default="", help="comma list of further workloads to report under 'other_workloads' "
                                                  "(value / time_to_tol / speed-up only), e.g. c1,c2,c3,c5")
@@ -357,7 +358,8 @@ def run_ours(args, rank: int, local_rank: int, world: int):
     spmv_kernel = {"auto": A.SPMV_AUTO, "direct": A.SPMV_DIRECT, "pipelined": A.SPMV_PIPELINED}[args.spmv_kernel]
     s = make_config(args.workload, args.size)
     vec_kernel = {"auto": A.VEC_AUTO, "direct": A.VEC_DIRECT, "staged": A.VEC_STAGED}[args.vec_kernel]
-    R = Runner(A, torch, s, dev, loop, spmv_kernel, vec_kernel=vec_kernel)
+    fuse = {"auto": A.FUSE_AUTO, "off": A.FUSE_OFF, "on": A.FUSE_ON}[args.fuse]
+    R = Runner(A, torch, s, dev, loop, spmv_kernel, vec_kernel=vec_kernel, fuse_vec=fuse)
     h = R.h
     if args.profile_iters > 0:
         kwp = {"pcg_fp64": dict(amp=0), "amp_fp16_linear": dict(u0=A.FP16, eta_rule=A.ETA_LINEAR, eps32=1e-30),
@@ -460,7 +462,7 @@ def run_ours(args, rank: int, local_rank: int, world: int):
     others = {}
     for name in [t for t in args.others.split(",") if t]:
         so = make_config(name)
-        Ro = Runner(A, torch, so, dev, loop, spmv_kernel, vec_kernel=vec_kernel)
+        Ro = Runner(A, torch, so, dev, loop, spmv_kernel, vec_kernel=vec_kernel, fuse_vec=fuse)
         a_, _ = Ro.summary(args.policy, 2)
         f_, _ = Ro.summary(dict(amp=0), 2)
         l_, _ = Ro.summary(args.policy, 2, scale_mode=A.SCALE_LAGGED)

@@ -69,6 +69,10 @@ enum {
   AMP_VEC_DIRECT = 1,     /* every thread loads its chunks of the vectors from global memory */
   AMP_VEC_STAGED = 2      /* persistent blocks; the input vectors are streamed into a shared-memory ring by cp.async.bulk */
 };
+/* whether the three vector steps between two mat-vecs run as ONE cooperative kernel with two grid barriers
+ * (execution choice; the vectors are bit-identical, the inner products are added in another fixed order) */
+enum { AMP_FUSE_AUTO = 0 /* on wherever it can run: Jacobi / no preconditioner, not a block row of a sharded system */,
+       AMP_FUSE_OFF = 1, AMP_FUSE_ON = 2 };
 /* storage / working precisions u_z, u_r */
 enum { AMP_FP64 = 0, AMP_FP32 = 1, AMP_FP16 = 2 };
 /* indicator used by the u_r switch */
@@ -189,7 +193,7 @@ typedef struct {
                                row i, columns below halo_lo / from halo_lo + n on are the neighbour ranks' entries of p
                                (filled by the halo exchange).  Both 0 (default): an ordinary square matrix */
   int32_t vec_kernel;     /* AMP_VEC_*, default AUTO */
-  int32_t reserved1;      /* 0 */
+  int32_t fuse_vec;       /* AMP_FUSE_*, default AUTO */
 } amp_create_opts_t;
 void amp_create_opts_default(amp_create_opts_t *o);
 amp_pcg_t *amp_pcg_create_ex(int64_t n, int64_t nnz, const int32_t *rowptr, const int32_t *colidx,
@@ -262,9 +266,27 @@ double amp_pcg_spmv_bytes(const amp_pcg_t *h, int mat_prec, int vec_prec);
  * amp_stats_t.algorithmic_bytes is the sum of this over the iterations of a solve. */
 double amp_pcg_iteration_bytes(const amp_pcg_t *h, int uz, int ur);
 
+/* What create() built for this matrix: for tests, tuning and reports. */
+typedef struct {
+  int64_t slices;          /* SELL-32 slices */
+  int64_t aligned_slices;  /* diagonal-aligned slices (no per-entry column index) */
+  int64_t uniform_slices;  /* of those: slices of the uniform stencil (columns = row + a constant of the handle) */
+  int64_t stored_entries;  /* entries of the repack, zero padding included */
+  int64_t long_rows;       /* rows kept out of the slices (summed from the CSR arrays) */
+  int64_t guard;           /* zero guard band (entries) on each side of p and z */
+  int32_t index_bits;      /* 0: every slice aligned; 16 / 32: width of the per-entry column data of the general slices */
+  int32_t rows_sorted;     /* 1: rows sorted by length inside windows of 1024 */
+  int32_t spmv_pipelined;  /* 1: the u_r = FP32 phases run the bulk-copy pipelined mat-vec */
+  int32_t vec_staged;      /* bit 0: z and p updates, bit 1: x/r update run the bulk-copy staged kernels */
+  int32_t uniform_width;   /* entries per row of the uniform stencil, 0 if none */
+  int32_t reserved0;
+} amp_format_info_t;
+int amp_pcg_format_info(const amp_pcg_t *h, amp_format_info_t *out_host);
+
 /* ---- measurement: per-kernel device times of the last solve made with policy.profile_kernels = 1 ---------- */
 enum { AMP_K_Z = 0, AMP_K_P = 1, AMP_K_SPMV = 2, AMP_K_XR = 3, AMP_K_XRZ = 4,
-       AMP_K_CHEB0 = 5 /* first Chebyshev sweep */, AMP_K_CHEBSTEP = 6 /* further sweeps */, AMP_K_COUNT = 7 };
+       AMP_K_CHEB0 = 5 /* first Chebyshev sweep */, AMP_K_CHEBSTEP = 6 /* further sweeps */,
+       AMP_K_VEC_FUSED = 7 /* a5 of iteration k + a2, a3 of iteration k + 1 in one kernel (AMP_FUSE_ON) */, AMP_K_COUNT = 8 };
 typedef struct {
   int32_t kernel;          /* AMP_K_*: step a2, a3, a4, a5 of SURVEY.md section 8(a) (XRZ: a5 + a2 of the lagged variant;
                               with AMP_PRECOND_CHEBJACOBI step a2 is CHEB0 + (s-1) x (SPMV + CHEBSTEP), all mat-vecs under SPMV) */

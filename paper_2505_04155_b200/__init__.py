@@ -11,6 +11,7 @@ from .binding import (  # noqa: F401
     Stats,
     CreateOpts,
     KernelTime,
+    FormatInfo,
     DebugStep,
     AmpPcgError,
     bytes_per_row,
@@ -24,7 +25,8 @@ from .binding import (  # noqa: F401
     INDEX_AUTO, INDEX_NO_ALIGN, INDEX_FORCE32,
     SPMV_AUTO, SPMV_DIRECT, SPMV_PIPELINED,
     VEC_AUTO, VEC_DIRECT, VEC_STAGED,
-    K_Z, K_P, K_SPMV, K_XR, K_XRZ, K_CHEB0, K_CHEBSTEP, KERNEL_NAMES,
+    FUSE_AUTO, FUSE_OFF, FUSE_ON,
+    K_Z, K_P, K_SPMV, K_XR, K_XRZ, K_CHEB0, K_CHEBSTEP, K_VEC_FUSED, KERNEL_NAMES,
     VEC_R, VEC_Q, VEC_Z, VEC_P, VEC_DINV, VEC_D,
     STEP_Z, STEP_P, STEP_SPMV, STEP_XR, STEP_XRZ, STEP_CHEB0, STEP_SPMV_Z, STEP_CHEBSTEP,
     EXPORTED_SYMBOLS,

@@ -20,9 +20,10 @@ PRECOND_NONE, PRECOND_JACOBI, PRECOND_CHEBJACOBI = 0, 1, 2
 INDEX_AUTO, INDEX_NO_ALIGN, INDEX_FORCE32 = 0, 1, 2
 SPMV_AUTO, SPMV_DIRECT, SPMV_PIPELINED = 0, 1, 2
 VEC_AUTO, VEC_DIRECT, VEC_STAGED = 0, 1, 2
-K_Z, K_P, K_SPMV, K_XR, K_XRZ, K_CHEB0, K_CHEBSTEP = 0, 1, 2, 3, 4, 5, 6
+FUSE_AUTO, FUSE_OFF, FUSE_ON = 0, 1, 2
+K_Z, K_P, K_SPMV, K_XR, K_XRZ, K_CHEB0, K_CHEBSTEP, K_VEC_FUSED = 0, 1, 2, 3, 4, 5, 6, 7
 KERNEL_NAMES = {K_Z: "k_z", K_P: "k_p", K_SPMV: "k_spmv", K_XR: "k_xr", K_XRZ: "k_xrz", K_CHEB0: "k_cheb0",
-                K_CHEBSTEP: "k_cheb_step"}
+                K_CHEBSTEP: "k_cheb_step", K_VEC_FUSED: "k_vec_fused"}
 VEC_R, VEC_Q, VEC_Z, VEC_P, VEC_DINV, VEC_D = 0, 1, 2, 3, 4, 5
 STEP_Z, STEP_P, STEP_SPMV, STEP_XR, STEP_XRZ, STEP_CHEB0, STEP_SPMV_Z, STEP_CHEBSTEP = 0, 1, 2, 3, 4, 5, 6, 7
 
@@ -33,7 +34,7 @@ EXPORTED_SYMBOLS = (
     "amp_pcg_last_error", "amp_pcg_bytes_per_row", "amp_pcg_spmv_bytes", "amp_pcg_iteration_bytes",
     "amp_pcg_eta_posteriori", "amp_pcg_kernel_times",
     "amp_pcg_debug_set_vector", "amp_pcg_debug_get_vector", "amp_pcg_debug_step",
-    "amp_shard_plan", "amp_shard_extract", "amp_pcg_shard_export", "amp_pcg_shard_attach", "amp_pcg_shard_attach_local",
+    "amp_pcg_format_info", "amp_shard_plan", "amp_shard_extract", "amp_pcg_shard_export", "amp_pcg_shard_attach", "amp_pcg_shard_attach_local",
     "amp_pcg_solve_sharded", "amp_spmv_sharded",
 )
 SHARD_MAX_WORLD = 16
@@ -74,7 +75,7 @@ class CreateOpts(C.Structure):
         ("struct_bytes", C.c_int32), ("precond", C.c_int32), ("index_format", C.c_int32), ("spmv_kernel", C.c_int32),
         ("spmv_grid_mult", C.c_int32), ("pdl", C.c_int32), ("cheb_degree", C.c_int32), ("reserved0", C.c_int32),
         ("cheb_lmin", C.c_double), ("cheb_lmax", C.c_double), ("stream", C.c_void_p),
-        ("halo_lo", C.c_int64), ("halo_hi", C.c_int64), ("vec_kernel", C.c_int32), ("reserved1", C.c_int32),
+        ("halo_lo", C.c_int64), ("halo_hi", C.c_int64), ("vec_kernel", C.c_int32), ("fuse_vec", C.c_int32),
     ]
 
     @classmethod
@@ -99,6 +100,18 @@ class ShardExport(C.Structure):
 
     _fields_ = [("n", C.c_int64), ("halo_lo", C.c_int64), ("halo_hi", C.c_int64), ("guard", C.c_int64),
                 ("mem", (C.c_ubyte * 64) * 4), ("off", C.c_int64 * 4)]
+
+
+class FormatInfo(C.Structure):
+    """amp_format_info_t (include/amp_pcg.h)."""
+
+    _fields_ = [("slices", C.c_int64), ("aligned_slices", C.c_int64), ("uniform_slices", C.c_int64),
+                ("stored_entries", C.c_int64), ("long_rows", C.c_int64), ("guard", C.c_int64),
+                ("index_bits", C.c_int32), ("rows_sorted", C.c_int32), ("spmv_pipelined", C.c_int32),
+                ("vec_staged", C.c_int32), ("uniform_width", C.c_int32), ("reserved0", C.c_int32)]
+
+    def asdict(self):
+        return {k: getattr(self, k) for k, _ in self._fields_ if k != "reserved0"}
 
 
 class KernelTime(C.Structure):
@@ -190,6 +203,8 @@ def load_library(variant: str = ""):
     L.amp_pcg_debug_get_vector.argtypes = [vp, C.c_int, C.c_int, vp]
     L.amp_pcg_debug_step.restype = C.c_int
     L.amp_pcg_debug_step.argtypes = [vp, C.POINTER(DebugStep), vp]
+    L.amp_pcg_format_info.restype = C.c_int
+    L.amp_pcg_format_info.argtypes = [vp, C.POINTER(FormatInfo)]
     L.amp_shard_plan.restype = C.c_int
     L.amp_shard_plan.argtypes = [i64, vp, vp, i32, C.POINTER(Shard)]
     L.amp_shard_extract.restype = C.c_int
@@ -336,6 +351,12 @@ class AmpPcg:
     def iteration_bytes(self, uz: int, ur: int) -> float:
         """amp_pcg_iteration_bytes: compulsory bytes of one iteration in phase (u_z, u_r)."""
         return float(self._L.amp_pcg_iteration_bytes(self._h, int(uz), int(ur)))
+
+    def format_info(self) -> FormatInfo:
+        """amp_pcg_format_info: what create() built for this matrix."""
+        fi = FormatInfo()
+        self._check(self._L.amp_pcg_format_info(self._h, C.byref(fi)), allow=(0,))
+        return fi
 
     def kernel_times(self):
         """amp_pcg_kernel_times: per (kernel, u_z, u_r) records of the last solve made with profile_kernels=1."""

@@ -15,6 +15,7 @@
 #include "kernels.cuh"
 #include "persistent.cuh"
 #include "spmv_pipe.cuh"
+#include "vec_fused.cuh"
 #include "vec_pipe.cuh"
 
 using namespace amp;
@@ -89,6 +90,12 @@ struct amp_pcg {
   char* xchg = nullptr;                  // exchange block: mailbox [kMailEntries] then 2 halo flags (owned, zeroed once)
   ShardCtx* d_shard = nullptr;           // device copy of the peer table (owned)
   int shard_rank = -1, shard_world = 0;  // set by amp_pcg_shard_attach*
+  int64_t nslices_aligned = 0, nslices_uniform = 0;
+  int index_bits = 0, rows_sorted = 0;
+  int use_fused = 0, grid_fused = 1;     // the loop runs k_vec_fused (vec_fused.cuh) instead of k_xr, k_z, k_p
+  cudaGraph_t graph_fu[2] = {nullptr, nullptr};          // [lagged] graph loops with the fused vector kernel
+  cudaGraphExec_t graph_fu_exec[2] = {nullptr, nullptr};
+  cudaGraphConditionalHandle cond_fu[2] = {};
   int use_vstage = 0;                    // bit 0: k_z and k_p, bit 1: k_xr and k_xrz are the bulk-copy staged kernels (vec_pipe.cuh)
   int shard_inline = 0;                  // the reducing kernels also collect and step (ranks run concurrently): no k_epi launches
   unsigned int shard_epoch = 0;          // sharded solves / mat-vecs made so far (identical on all ranks of the group)
@@ -174,6 +181,8 @@ extern "C" void amp_pcg_destroy(amp_pcg_t* h) {
   for (int i = 0; i < 2; ++i) {
     if (h->graph_sh_exec[i]) cudaGraphExecDestroy(h->graph_sh_exec[i]);
     if (h->graph_sh[i]) cudaGraphDestroy(h->graph_sh[i]);
+    if (h->graph_fu_exec[i]) cudaGraphExecDestroy(h->graph_fu_exec[i]);
+    if (h->graph_fu[i]) cudaGraphDestroy(h->graph_fu[i]);
   }
   for (void* p : h->ipc_opened) cudaIpcCloseMemHandle(p);
   for (void* p : h->owned) cudaFree(p);
@@ -204,7 +213,7 @@ extern "C" void amp_create_opts_default(amp_create_opts_t* o) {
   o->halo_lo = 0;
   o->halo_hi = 0;
   o->vec_kernel = AMP_VEC_AUTO;
-  o->reserved1 = 0;
+  o->fuse_vec = AMP_FUSE_AUTO;
 }
 
 extern "C" amp_pcg_t* amp_pcg_create(int64_t n, int64_t nnz, const int32_t* rowptr, const int32_t* colidx,
@@ -231,7 +240,7 @@ extern "C" amp_pcg_t* amp_pcg_create_ex(int64_t n, int64_t nnz, const int32_t* r
   const int precond = o.precond;
   if (o.index_format < AMP_INDEX_AUTO || o.index_format > AMP_INDEX_FORCE32 || o.spmv_kernel < AMP_SPMV_AUTO ||
       o.spmv_kernel > AMP_SPMV_PIPELINED || o.spmv_grid_mult < 0 || (o.pdl != 0 && o.pdl != 1) || o.vec_kernel < AMP_VEC_AUTO ||
-      o.vec_kernel > AMP_VEC_STAGED) {
+      o.vec_kernel > AMP_VEC_STAGED || o.fuse_vec < AMP_FUSE_AUTO || o.fuse_vec > AMP_FUSE_ON) {
     set_error("amp_pcg_create_ex: invalid index_format / spmv_kernel / vec_kernel / spmv_grid_mult / pdl");
     return nullptr;
   }
@@ -452,6 +461,9 @@ extern "C" amp_pcg_t* amp_pcg_create_ex(int64_t n, int64_t nnz, const int32_t* r
     h->long_entries = (double)(nnz - nnz_sell);
     h->long_bytes_idx = 4.0 * h->long_entries + 12.0 * (double)long_rows.size();
     h->sell_entries = wsum * 32;
+    for (int64_t sl = 0; sl < nsl; ++sl) h->nslices_aligned += width[(size_t)sl] < 0 ? 1 : 0;
+    h->index_bits = (w_aligned == wsum) ? 0 : (wide ? 32 : 16);
+    h->rows_sorted = perm.empty() ? 0 : 1;
 
     // ---- bulk-copy pipelined SpMV (spmv_pipe.cuh): eligibility, zero guard band of p, stage plan ----
     {
@@ -513,6 +525,38 @@ extern "C" amp_pcg_t* amp_pcg_create_ex(int64_t n, int64_t nnz, const int32_t* r
         c.pipe_chunks = chunks_d; c.pipe_blk_chunk = blk_d; c.use_pipe = 1;
         h->use_pipe = 1; h->pipe_grid = nb; h->pipe_chunks = nch; h->guard = guard;
         h->idx_bytes_total += 8.0 * (double)(nch + 1) + 4.0 * (double)(nb + 1);  // stage descriptors
+      }
+    }
+    // ---- uniform stencil (spmv.cuh, narrow_uniform_sum): narrow diagonal-aligned slices that share one set of offsets ----
+    {
+      int wmax_all = 0;
+      for (int64_t sl = 0; sl < nsl; ++sl) wmax_all = std::max(wmax_all, (int)(width[(size_t)sl] & 0x7fffffff));
+      // reference slice: the first diagonal-aligned slice of full width from the middle of the matrix on (boundary slices
+      // of a grid lack some diagonals)
+      int64_t ref = -1;
+      for (int64_t sl = nsl / 2; sl < nsl && ref < 0; ++sl)
+        if (width[(size_t)sl] < 0 && (int)(width[(size_t)sl] & 0x7fffffff) == wmax_all) ref = sl;
+      const int ref_w = wmax_all;
+      if (o.index_format == AMP_INDEX_AUTO && wmax_all >= 1 && wmax_all <= 7 && ref >= 0) {
+        const int ref_w0 = wptr[(size_t)ref] & 0x7fffffff;
+        int* cnt_d;
+        ALLOC(cnt_d, int, 1);
+        k_mark_uniform<<<(int)((nsl + 255) / 256), 256, 0, h->stream>>>((int)nsl, wptr_d, base_d, ref_w0, ref_w, cnt_d);
+        int cnt = 0;
+        int32_t ub[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+        CU_TRY(cudaMemcpyAsync(&cnt, cnt_d, sizeof(int), cudaMemcpyDeviceToHost, h->stream), { amp_pcg_destroy(h); return nullptr; });
+        CU_TRY(cudaMemcpyAsync(ub, base_d + ref_w0, sizeof(int32_t) * (size_t)ref_w, cudaMemcpyDeviceToHost, h->stream),
+               { amp_pcg_destroy(h); return nullptr; });
+        CU_TRY(cudaStreamSynchronize(h->stream), { amp_pcg_destroy(h); return nullptr; });
+        CU_TRY(cudaGetLastError(), { amp_pcg_destroy(h); return nullptr; });
+        h->nslices_uniform = cnt;
+        if (cnt > 0) {  // (slices that do not match keep the general aligned path: the flag is per slice)
+          int maxoff = 0;
+          for (int k = 0; k < ref_w; ++k) { c.uni_base[k] = ub[k]; maxoff = std::max(maxoff, std::abs(ub[k])); }
+          c.uni_w = ref_w;
+          const int64_t uguard = (((int64_t)maxoff + 64 + 127) / 128) * 128;
+          if (uguard <= kPipeMaxGuard) { h->guard = std::max(h->guard, uguard); c.uni_noclamp = 1; }
+        }
       }
     }
     {  // p and z (both are gathered by a mat-vec: z inside the Chebyshev-Jacobi preconditioner) in their three storage
@@ -594,6 +638,28 @@ extern "C" amp_pcg_t* amp_pcg_create_ex(int64_t n, int64_t nnz, const int32_t* r
   h->grid_cheb0 = vec_grid_for((const void*)k_cheb0);
   h->grid_cheb_step = vec_grid_for((const void*)k_cheb_step);
   h->vec_grid = vec_grid_for((const void*)k_setup);
+  // fused vector kernel (vec_fused.cuh): one cooperative kernel per iteration instead of k_xr, k_z, k_p
+  {
+    int occ = 0, coop = 0;
+    cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, h->device);
+    const bool ok = coop && cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_vec_fused<false>, kFusedThreads, 0) == cudaSuccess &&
+                    occ >= 1;
+    int occ2 = occ;
+    if (ok && cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ2, k_vec_fused<true>, kFusedThreads, 0) != cudaSuccess) occ2 = 0;
+    cudaGetLastError();
+    const int64_t cap = (int64_t)h->num_sms * std::min(occ, occ2);
+    const int64_t want = (h->npad / 16 + kFusedThreads - 1) / kFusedThreads;
+    h->grid_fused = (int)std::max<int64_t>(1, std::min<int64_t>(std::min<int64_t>(cap, kMaxGrid), want));
+    const bool can = ok && occ2 >= 1 && h->cheb_s == 0 && h->halo_lo == 0 && h->halo_hi == 0;
+    if (o.fuse_vec == AMP_FUSE_ON && !can) {
+      set_error("amp_pcg_create_ex: AMP_FUSE_ON needs cooperative launch and is not available with Chebyshev-Jacobi or block rows");
+      amp_pcg_destroy(h);
+      return nullptr;
+    }
+    // measured (B200, profiles/r02.md, ms per solve fused vs unfused): c2 20.98 vs 23.92, c3 78.6 vs 82.6, c4 113.6 vs 119.4;
+    // the fused kernel reaches 0.75-0.97 of the copy rate on c4 where k_z / k_p alone sat at 0.45: AUTO = on wherever it can run
+    h->use_fused = can && o.fuse_vec != AMP_FUSE_OFF;
+  }
   // bulk-copy staged vector kernels (vec_pipe.cuh).  Measured on B200 (profiles/r02.md, us per launch, staged vs direct):
   // c4 (8 M rows) k_z 23.1 vs 27.4 (FP16 phase), 25.1 vs 31.8 (FP32 phase), k_p 18.5 vs 20.5, but k_xr 47.8 vs 44.6; c3
   // (4.1 M) k_z 16.9 vs 21.0, k_p 12.5 vs 14.5, k_xr 29.1 vs 28.4; c2 (2.1 M) a tie.  AUTO therefore stages the z and p
@@ -625,6 +691,16 @@ extern "C" int amp_pcg_set_stream(amp_pcg_t* h, void* cuda_stream) {
 
 extern "C" int64_t amp_pcg_last_launch_count(const amp_pcg_t* h) { return h ? h->launches : 0; }
 
+extern "C" int amp_pcg_format_info(const amp_pcg_t* h, amp_format_info_t* out) {
+  if (!h || !out) return AMP_ERR_INVALID;
+  std::memset(out, 0, sizeof(*out));
+  out->slices = h->ctx.nslices; out->aligned_slices = h->nslices_aligned; out->uniform_slices = h->nslices_uniform;
+  out->stored_entries = h->sell_entries; out->long_rows = h->ctx.nlong; out->guard = h->guard;
+  out->index_bits = h->index_bits; out->rows_sorted = h->rows_sorted; out->spmv_pipelined = h->use_pipe;
+  out->vec_staged = h->use_vstage; out->uniform_width = h->ctx.uni_w;
+  return AMP_OK;
+}
+
 // ------------------------------------------------------------------ SpMV entry --------------
 template <int UR, class PT>
 static void launch_spmv_any(amp_pcg* h, const void* p, void* q, unsigned int halo_seq) {
@@ -632,6 +708,7 @@ static void launch_spmv_any(amp_pcg* h, const void* p, void* q, unsigned int hal
   if (halo_seq == 0u) {  // p is a caller's vector of exactly n entries: no halo bands, no guard band around it
     c.col_min = 0;
     c.col_max = (int32_t)(h->n - 1);
+    c.uni_noclamp = 0;
   }
   k_spmv_any<UR, PT><<<h->spmv_grid, kSpmvThreads, 0, h->stream>>>(
       c, static_cast<const PT*>(p), static_cast<typename Store<UR>::T*>(q), halo_seq);
@@ -686,6 +763,20 @@ static cudaError_t launch_loop_kernel_ex(K kern, int grid, int threads, cudaStre
   cfg.numAttrs = pdl ? 1 : 0;
   return cudaLaunchKernelEx(&cfg, kern, args...);
 }
+// a kernel whose blocks wait for one another at a grid barrier: cooperative launch (all blocks resident or the launch fails)
+template <class K, class... Args>
+static cudaError_t launch_coop_kernel(K kern, int grid, int threads, cudaStream_t s, Args... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3((unsigned)grid);
+  cfg.blockDim = dim3((unsigned)threads);
+  cfg.stream = s;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeCooperative;
+  attr[0].val.cooperative = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, kern, args...);
+}
 template <class K>
 static cudaError_t launch_loop_kernel(K kern, int grid, int threads, cudaStream_t s, const Ctx& c, bool pdl) {
   return launch_loop_kernel_ex(kern, grid, threads, s, pdl, 0, c);
@@ -709,8 +800,9 @@ static cudaError_t launch_vec(amp_pcg* h, int which, cudaStream_t s, const Ctx& 
 // step a4 inside the loop (zmode = 0), or the mat-vec q = A z inside the Chebyshev-Jacobi preconditioner (zmode = 1):
 // the direct kernel, followed by the bulk-copy pipelined kernel when the matrix is eligible (it takes the u_r = FP32
 // phases; whichever kernel's phase it is not returns at once)
-static cudaError_t launch_spmv_loop(amp_pcg* h, cudaStream_t s, const Ctx& c, bool pdl, int zmode = 0) {
-  cudaError_t e = launch_loop_kernel_ex(k_spmv, h->spmv_grid, kSpmvThreads, s, pdl, 0, c, zmode);
+// pdl_first: whether the first of the (up to) two kernels may start early (false when the mat-vec opens an iteration)
+static cudaError_t launch_spmv_loop(amp_pcg* h, cudaStream_t s, const Ctx& c, bool pdl, int zmode = 0, int pdl_first = -1) {
+  cudaError_t e = launch_loop_kernel_ex(k_spmv, h->spmv_grid, kSpmvThreads, s, pdl_first < 0 ? pdl : pdl_first != 0, 0, c, zmode);
   if (e == cudaSuccess && h->use_pipe)
     e = launch_loop_kernel_ex(k_spmv_pipe, h->pipe_grid, kPipeThreads, s, pdl, (size_t)kPipeSmemBytes, c, zmode);
   return e;
@@ -773,14 +865,33 @@ static cudaError_t launch_iteration_lagged(amp_pcg* h, const Ctx& c, cudaStream_
   return e;
 }
 
+// loop body with the fused vector kernel (vec_fused.cuh): the mat-vec of iteration k, then x/r of k and z, p of k + 1 in
+// one cooperative kernel (z_0, p_0 come from k_z, k_p before the loop)
+static cudaError_t launch_iteration_fused(amp_pcg* h, const Ctx& c, cudaStream_t s, bool pdl, bool lagged, int prof_iter = -1) {
+  const bool prof = prof_iter >= 0;
+  if (prof) pdl = false;
+  cudaError_t e = cudaSuccess;
+  if (prof) e = prof_mark(h, s, AMP_K_SPMV, prof_iter);
+  if (e == cudaSuccess) e = launch_spmv_loop(h, s, c, pdl, 0, 0);
+  if (prof && e == cudaSuccess) e = prof_mark(h, s, AMP_K_VEC_FUSED, prof_iter);
+  if (e == cudaSuccess)
+    e = lagged ? launch_coop_kernel(k_vec_fused<true>, h->grid_fused, kFusedThreads, s, c)
+               : launch_coop_kernel(k_vec_fused<false>, h->grid_fused, kFusedThreads, s, c);
+  if (prof && e == cudaSuccess) e = prof_mark(h, s, -1, prof_iter);
+  return e;
+}
+
 // One graph = one WHILE conditional node whose body is the four loop kernels; the condition is
 // written from the device by epi_delta / epi_gamma, so a whole solve is a single launch.
 static cudaError_t launch_iteration_sharded(amp_pcg* h, const Ctx& c, cudaStream_t s, bool pdl, bool lagged);
 
-static int build_graph_once(amp_pcg* h, bool pdl, bool lagged, bool sharded) {
-  cudaGraph_t& graph = sharded ? h->graph_sh[lagged] : (lagged ? h->graph_lag : h->graph);
-  cudaGraphExec_t& graph_exec = sharded ? h->graph_sh_exec[lagged] : (lagged ? h->graph_lag_exec : h->graph_exec);
-  cudaGraphConditionalHandle& cond = sharded ? h->cond_sh[lagged] : (lagged ? h->cond_lag : h->cond);
+enum { GK_PLAIN = 0, GK_SHARDED = 1, GK_FUSED = 2 };
+static int build_graph_once(amp_pcg* h, bool pdl, bool lagged, int kind) {
+  const bool sharded = kind == GK_SHARDED, fused = kind == GK_FUSED;
+  cudaGraph_t& graph = fused ? h->graph_fu[lagged] : sharded ? h->graph_sh[lagged] : (lagged ? h->graph_lag : h->graph);
+  cudaGraphExec_t& graph_exec =
+      fused ? h->graph_fu_exec[lagged] : sharded ? h->graph_sh_exec[lagged] : (lagged ? h->graph_lag_exec : h->graph_exec);
+  cudaGraphConditionalHandle& cond = fused ? h->cond_fu[lagged] : sharded ? h->cond_sh[lagged] : (lagged ? h->cond_lag : h->cond);
   CU_TRY(cudaGraphCreate(&graph, 0), return AMP_ERR_CUDA);
   CU_TRY(cudaGraphConditionalHandleCreate(&cond, graph, 1, cudaGraphCondAssignDefault), return AMP_ERR_CUDA);
   cudaGraphNodeParams np = {};
@@ -798,8 +909,9 @@ static int build_graph_once(amp_pcg* h, bool pdl, bool lagged, bool sharded) {
   c.use_cond = 1;
   cudaError_t e = cudaStreamBeginCaptureToGraph(cap, body, nullptr, nullptr, 0, cudaStreamCaptureModeRelaxed);
   if (e == cudaSuccess) {
-    const cudaError_t el = sharded ? launch_iteration_sharded(h, c, cap, pdl, lagged)
-                                   : (lagged ? launch_iteration_lagged(h, c, cap, pdl) : launch_iteration(h, c, cap, pdl));
+    const cudaError_t el = fused     ? launch_iteration_fused(h, c, cap, pdl, lagged)
+                           : sharded ? launch_iteration_sharded(h, c, cap, pdl, lagged)
+                                     : (lagged ? launch_iteration_lagged(h, c, cap, pdl) : launch_iteration(h, c, cap, pdl));
     e = cudaStreamEndCapture(cap, nullptr);
     if (e == cudaSuccess) e = el;
   }
@@ -809,16 +921,18 @@ static int build_graph_once(amp_pcg* h, bool pdl, bool lagged, bool sharded) {
   return AMP_OK;
 }
 
-static int build_graph(amp_pcg* h, bool lagged, bool sharded = false) {
-  cudaGraph_t& graph = sharded ? h->graph_sh[lagged] : (lagged ? h->graph_lag : h->graph);
-  cudaGraphExec_t& graph_exec = sharded ? h->graph_sh_exec[lagged] : (lagged ? h->graph_lag_exec : h->graph_exec);
+static int build_graph(amp_pcg* h, bool lagged, int kind = GK_PLAIN) {
+  const bool sharded = kind == GK_SHARDED, fused = kind == GK_FUSED;
+  cudaGraph_t& graph = fused ? h->graph_fu[lagged] : sharded ? h->graph_sh[lagged] : (lagged ? h->graph_lag : h->graph);
+  cudaGraphExec_t& graph_exec =
+      fused ? h->graph_fu_exec[lagged] : sharded ? h->graph_sh_exec[lagged] : (lagged ? h->graph_lag_exec : h->graph_exec);
   if (graph_exec) return AMP_OK;
-  int rc = build_graph_once(h, h->pdl != 0, lagged, sharded);
+  int rc = build_graph_once(h, h->pdl != 0, lagged, kind);
   if (rc != AMP_OK && h->pdl) {  // programmatic edges not accepted inside the conditional body: plain edges
     if (graph_exec) { cudaGraphExecDestroy(graph_exec); graph_exec = nullptr; }
     if (graph) { cudaGraphDestroy(graph); graph = nullptr; }
     h->pdl = 0;
-    rc = build_graph_once(h, false, lagged, sharded);
+    rc = build_graph_once(h, false, lagged, kind);
   }
   return rc;
 }
@@ -923,7 +1037,8 @@ static int solve_impl(amp_pcg* h, const double* b, double* x, double tol, int32_
     set_error("amp_pcg_solve: persistent loop not available for this problem/device");
     return AMP_ERR_INVALID;
   }
-  if (mode == AMP_LOOP_GRAPH) { const int rc = build_graph(h, lagged); if (rc != AMP_OK) return rc; }
+  const bool fused = h->use_fused && mode != AMP_LOOP_PERSISTENT;
+  if (mode == AMP_LOOP_GRAPH) { const int rc = build_graph(h, lagged, fused ? GK_FUSED : GK_PLAIN); if (rc != AMP_OK) return rc; }
 
   DevState* hs = h->h_state;
   fill_state(hs, h, b, x, tol, maxit, pol);
@@ -941,12 +1056,16 @@ static int solve_impl(amp_pcg* h, const double* b, double* x, double tol, int32_
   k_setup<<<h->vec_grid, kVecThreads, 0, st>>>(h->ctx, pol.x0_zero ? 1 : 0);
   h->launches += 1;
 
-  if (lagged && mode != AMP_LOOP_PERSISTENT) {  // z_0, rho_0 for the first pass of the three-kernel loop
+  if ((lagged || fused) && mode != AMP_LOOP_PERSISTENT) {  // z_0, rho_0 for the first pass of a loop that opens with p or A p
     CU_TRY(launch_vec(h, VK_Z, st, h->ctx, false), return AMP_ERR_CUDA);
     h->launches += 1;
   }
+  if (fused) {  // p_0 too: the fused loop opens with the mat-vec
+    CU_TRY(launch_vec(h, VK_P, st, h->ctx, false), return AMP_ERR_CUDA);
+    h->launches += 1;
+  }
   if (mode == AMP_LOOP_GRAPH) {
-    CU_TRY(cudaGraphLaunch(lagged ? h->graph_lag_exec : h->graph_exec, st), return AMP_ERR_CUDA);
+    CU_TRY(cudaGraphLaunch(fused ? h->graph_fu_exec[lagged] : (lagged ? h->graph_lag_exec : h->graph_exec), st), return AMP_ERR_CUDA);
   } else if (mode == AMP_LOOP_PERSISTENT) {
     const int rc = persistent_launch(h->ctx, h->persist_grid, st);
     if (rc != 0) { set_error("persistent kernel launch failed: %s", cudaGetErrorString((cudaError_t)rc)); return AMP_ERR_CUDA; }
@@ -957,8 +1076,9 @@ static int solve_impl(amp_pcg* h, const double* b, double* x, double tol, int32_
       const int nb = std::min(batch, maxit - done_iters);
       for (int i = 0; i < nb; ++i) {
         const int pit = profile ? done_iters + i : -1;
-        const cudaError_t el = lagged ? launch_iteration_lagged(h, h->ctx, st, h->pdl != 0, pit)
-                                      : launch_iteration(h, h->ctx, st, h->pdl != 0, pit);
+        const cudaError_t el = fused    ? launch_iteration_fused(h, h->ctx, st, h->pdl != 0, lagged, pit)
+                               : lagged ? launch_iteration_lagged(h, h->ctx, st, h->pdl != 0, pit)
+                                        : launch_iteration(h, h->ctx, st, h->pdl != 0, pit);
         if (el != cudaSuccess) {
           set_error("amp_pcg_solve: loop kernel launch failed: %s", cudaGetErrorString(el));
           cudaGetLastError();
@@ -1012,6 +1132,10 @@ static int solve_impl(amp_pcg* h, const double* b, double* x, double tol, int32_
             case AMP_K_CHEB0: a.bytes_per_launch = n_ * (sr + sd + 2.0 * sz); break;
             case AMP_K_CHEBSTEP: a.bytes_per_launch = n_ * (2.0 * sr + sd + 4.0 * sz); break;
             case AMP_K_XR: a.bytes_per_launch = n_ * (16.0 + sz + 3.0 * sr); break;
+            case AMP_K_VEC_FUSED:  // x/r of this iteration, then z and p (of the next one: its phase, but for 1-3 launches, is this one's)
+              a.bytes_per_launch = n_ * ((16.0 + sz + 3.0 * sr) + (lagged ? sd + sz : sr + sd + sz) + 3.0 * sz +
+                                         (shadow_phase(uz, ur) ? 4.0 : 0.0));
+              break;
             default: a.bytes_per_launch = n_ * (16.0 + sz + 3.0 * sr + sd + sz); break;  // AMP_K_XRZ
           }
           h->prof_result.push_back(a);
@@ -1019,7 +1143,7 @@ static int solve_impl(amp_pcg* h, const double* b, double* x, double tol, int32_
   }
   {
     const int spmv_k = h->use_pipe ? 2 : 1, sweeps = std::max(h->cheb_s, 1);
-    const int per_it = (lagged ? 2 : 3) + spmv_k + (sweeps - 1) * (spmv_k + 1);  // vector kernels + a4 + extra sweeps
+    const int per_it = fused ? 1 + spmv_k : (lagged ? 2 : 3) + spmv_k + (sweeps - 1) * (spmv_k + 1);  // vector kernels + a4 + extra sweeps
     h->launches += (mode == AMP_LOOP_PERSISTENT) ? 1 : (int64_t)per_it * iters;
   }
   if (stats) fill_stats(h, hs, mode, lagged, ms, stats);

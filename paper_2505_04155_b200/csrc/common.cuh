@@ -19,9 +19,11 @@ constexpr int kSpmvWarps = kSpmvThreads / 32;
 #endif
 constexpr int kSpmvMinBlocks = AMP_SPMV_MINBLOCKS;  // resident SpMV blocks per SM the register budget is set for
 #ifndef AMP_PERSIST_THREADS
-#define AMP_PERSIST_THREADS 1024
+#define AMP_PERSIST_THREADS 512
 #endif
-constexpr int kPersistThreads = AMP_PERSIST_THREADS;  // block size of the persistent (whole-loop) kernel
+constexpr int kPersistThreads = AMP_PERSIST_THREADS;  // block size of the persistent (whole-loop) kernel: one block per SM; 512 threads
+                                                      // = 128 registers each (measured, us per iteration, 512 vs 1024 threads: c1 13.9 vs 18.8,
+                                                      // 262 K rows 17.6 vs 20.6, 1 M rows 34.7 vs 35.8; profiles/r02.md)
 constexpr int kPersistAutoMaxRows = 1 << 20;   // AMP_LOOP_AUTO takes the persistent kernel up to this many rows
 constexpr int kPersistMinBlocks = 1;           // resident blocks per SM its register budget is set for
 constexpr int kMaxGrid = 8192;                 // capacity of each partial-sum array
@@ -121,6 +123,11 @@ struct Ctx {
   // entry of p, gathers may reach col_min .. col_max (halo bands, then zero guard); col_shift = halo_lo is subtracted from
   // the borrowed CSR column indices (long rows)
   int32_t col_shift, col_min, col_max;
+  // uniform stencil (spmv.cuh): slices flagged kUniformFlag in sell_wptr are diagonal-aligned, uni_w wide and share these
+  // diagonal offsets, so their columns are row + a constant; uni_noclamp: the operand vector has a guard band that covers
+  // every row + offset (the handle's own p / z), so no clamp is needed either
+  int32_t uni_w, uni_noclamp;
+  int32_t uni_base[8];
   int64_t n_scale;                  // rows of the WHOLE system (= n unless sharded): the n of the RMS scale sqrt(n)/||r||
   const ShardCtx* sh;               // device pointer, nullptr unless attached to a group (amp_pcg_shard_attach*)
 };

@@ -35,11 +35,11 @@ __device__ __forceinline__ void red_release_add_u32(unsigned int* p, unsigned in
 // SUM = false: plain barrier.  Returns the total in warp 0 (SUM = true).
 // `partials` must be a different array at consecutive barriers (a fast block may already publish
 // its next partial while a slow one still reads this one).
-template <bool SUM>
+template <bool SUM, int NT = kPersistThreads>
 __device__ __forceinline__ double grid_all_sum(double v, double* partials, unsigned int* arrivals, unsigned int& target,
                                                int bid, int nb, double* red) {
   double bs = 0.0;
-  if (SUM) bs = block_sum<kPersistThreads>(v, red);  // every thread is past its phase's memory accesses
+  if (SUM) bs = block_sum<NT>(v, red);  // every thread is past its phase's memory accesses
   else __syncthreads();
   target += (unsigned int)nb;
   if (threadIdx.x == 0) {
@@ -51,17 +51,18 @@ __device__ __forceinline__ double grid_all_sum(double v, double* partials, unsig
   double tot = 0.0;
   if (SUM) {
     double a = 0.0;
-    for (int i = threadIdx.x; i < nb; i += kPersistThreads) a += __ldcg(partials + i);
-    tot = block_sum<kPersistThreads>(a, red);
+    for (int i = threadIdx.x; i < nb; i += NT) a += __ldcg(partials + i);
+    tot = block_sum<NT>(a, red);
   }
   return tot;
 }
 
 // the same for two sums (lagged variant: delta^2 and rho), partials interleaved; totals valid in warp 0
+template <int NT = kPersistThreads>
 __device__ __forceinline__ void grid_all_sum2(double v0, double v1, double* partials, unsigned int* arrivals, unsigned int& target,
                                               int bid, int nb, double* red, double& t0, double& t1) {
-  const double b0 = block_sum<kPersistThreads>(v0, red);
-  const double b1 = block_sum<kPersistThreads>(v1, red);
+  const double b0 = block_sum<NT>(v0, red);
+  const double b1 = block_sum<NT>(v1, red);
   target += (unsigned int)nb;
   if (threadIdx.x == 0) {
     __stcg(partials + 2 * bid, b0);
@@ -71,9 +72,9 @@ __device__ __forceinline__ void grid_all_sum2(double v0, double v1, double* part
   }
   __syncthreads();
   double a0 = 0.0, a1 = 0.0;
-  for (int i = threadIdx.x; i < nb; i += kPersistThreads) { a0 += __ldcg(partials + 2 * i); a1 += __ldcg(partials + 2 * i + 1); }
-  t0 = block_sum<kPersistThreads>(a0, red);
-  t1 = block_sum<kPersistThreads>(a1, red);
+  for (int i = threadIdx.x; i < nb; i += NT) { a0 += __ldcg(partials + 2 * i); a1 += __ldcg(partials + 2 * i + 1); }
+  t0 = block_sum<NT>(a0, red);
+  t1 = block_sum<NT>(a1, red);
 }
 
 // out-of-line copies of the phase dispatchers: each gets its own register allocation instead of

@@ -112,6 +112,8 @@ __device__ __forceinline__ double lds_one(const double* v) { return AMP_SPMV_MAT
 // The base of entry k is held by lane k % 32 and broadcast by a shuffle.
 constexpr int kPrefetchMinWidth = 16;  // groups narrower than this many entries per row are not prefetched
 constexpr int kAlignedFlag = (int)0x80000000u;  // bit 31 of sell_wptr[s]: slice s is aligned
+constexpr int kUniformFlag = 0x40000000;        // bit 30: slice s is aligned, Ctx::uni_w wide, with the diagonal offsets Ctx::uni_base
+constexpr int kWptrFlags = kAlignedFlag | kUniformFlag;
 template <int CM> struct ColSrc;
 template <> struct ColSrc<0> {
   using RawQ = int4; using RawP = int2; using RawS = int;
@@ -329,6 +331,58 @@ __device__ __forceinline__ void narrow_group_sum(const Ctx& c, const PT* p, cons
   }
 }
 
+// G consecutive slices of the handle's UNIFORM STENCIL (structured-grid matrices: every such slice is diagonal-aligned,
+// Ctx::uni_w <= 7 wide and has the diagonal offsets Ctx::uni_base, flagged in create()).  The columns are row + a
+// constant held in the kernel's parameter block: no base load, no shuffle, and — CLAMP = false: the operand has a guard
+// band — no clamp per entry.  The narrow slices were instruction-bound, not memory-bound (c2, FP32 phase: 130
+// instructions per slice); this path issues about half of them.  Same entries in the same order: same bits.
+template <int UR, bool COH, int G, bool CLAMP, class PT>
+__device__ __forceinline__ void narrow_uniform_sum(const Ctx& c, const PT* p, const int (&wp)[G + 1], int lane, const int (&rows)[G],
+                                                   typename SpmvT<UR>::A (&acc)[G]) {
+  using A = typename SpmvT<UR>::A;
+  constexpr int LQ = LaneQ<A>::v;
+  const A* vals = sell_vals<UR>(c);
+  const int w = c.uni_w;
+  const bool hq = (w & 4) != 0, hp = (w & 2) != 0, hs = (w & 1) != 0;
+  const int tail = hq ? 128 : 0, tail1 = tail + (hp ? 64 : 0);
+  const int kp = w & 4, ks = kp + (w & 2);  // entry index of the pair and of the single
+  // offsets of the 7 value slots (quad 0-3, pair 4-5, single 6); absent parts keep value 0 and take offset 0 of entry 0
+  int off[7];
+#pragma unroll
+  for (int u = 0; u < 4; ++u) off[u] = hq ? c.uni_base[u] : c.uni_base[0];
+  off[4] = hp ? c.uni_base[kp] : c.uni_base[0];
+  off[5] = hp ? c.uni_base[kp + 1] : c.uni_base[0];
+  off[6] = hs ? c.uni_base[ks] : c.uni_base[0];
+  A v[G][7];
+#pragma unroll
+  for (int g = 0; g < G; ++g) {
+    const A* vp = vals + (int64_t)wp[g] * 32;
+    A vq[4] = {A(0), A(0), A(0), A(0)}, vpair[2] = {A(0), A(0)}, vs = A(0);
+    if (hq) lds_quad(vp + lane * LQ, vq);
+    if (hp) lds_pair(vp + tail + lane * 2, vpair);
+    if (hs) vs = lds_one(vp + tail1 + lane);
+    v[g][0] = vq[0]; v[g][1] = vq[1]; v[g][2] = vq[2]; v[g][3] = vq[3]; v[g][4] = vpair[0]; v[g][5] = vpair[1]; v[g][6] = vs;
+  }
+  A x[G][7];
+#pragma unroll
+  for (int g = 0; g < G; ++g) {
+    const int r = rows[g] < 0 ? 0 : rows[g];
+#pragma unroll
+    for (int u = 0; u < 7; ++u) {
+      int j = r + off[u];
+      if (CLAMP) j = min(max(j, c.col_min), c.col_max);
+      x[g][u] = gatherA<COH>(A(0), p, j);
+    }
+  }
+#pragma unroll
+  for (int g = 0; g < G; ++g) {
+    A t = 0;
+#pragma unroll
+    for (int u = 0; u < 7; ++u) t = fma(v[g][u], x[g][u], t);
+    acc[g] = t;
+  }
+}
+
 template <int UR> struct SpmvGroup;  // slices a warp takes per pass
 #ifndef AMP_SPMV_G32
 #define AMP_SPMV_G32 2
@@ -347,11 +401,11 @@ constexpr int kSpmvGroupMax = AMP_SPMV_G32 > AMP_SPMV_G64 ? AMP_SPMV_G32 : AMP_S
 // Returns this thread's part of gamma = sum_i p_i q_i (stored q_i, FP64 products and sums).
 // pg: the STORED p (u_z precision) for gamma = q^T p; it differs from the gathered operand p only in phase
 // (u_z = FP64, u_r = FP32), where p is the FP32 copy RN32(p) written by the p update.
-template <int UR, bool COH, int CMG, int NT, class PT, class PG>
+// G: slices a warp takes per pass (SpmvGroup<UR>::G)
+template <int UR, bool COH, int CMG, int NT, int G, class PT, class PG>
 __device__ __forceinline__ double phase_spmv_fmt(const Ctx& c, const PT* p, const PG* pg, typename Store<UR>::T* q, int bid, int nb,
                                                  double* red) {
   using A = typename SpmvT<UR>::A;
-  constexpr int G = SpmvGroup<UR>::G;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   constexpr int wpb = NT / 32;
   const int32_t* __restrict__ wptr = c.sell_wptr;
@@ -368,7 +422,7 @@ __device__ __forceinline__ double phase_spmv_fmt(const Ctx& c, const PT* p, cons
     const int s0 = gi * G;
     int wp[G + 1], rows[G];
     int wmax = 0;
-    bool all_al = true, any_al = false, al_g[G];
+    bool all_al = true, any_al = false, all_uni = true, al_g[G];
 #pragma unroll
     for (int g = 0; g <= G; ++g) wp[g] = wnext[g];
     {  // slice table entries of this warp's next group: off the critical path of the next pass
@@ -384,19 +438,20 @@ __device__ __forceinline__ double phase_spmv_fmt(const Ctx& c, const PT* p, cons
     {
       const int g2 = gi + 2 * nb * wpb;
       if (g2 < ngroups) {
-        pf0 = __ldg(wptr + min(g2 * G, nslices)) & ~kAlignedFlag;
-        pf1 = __ldg(wptr + min(g2 * G + G, nslices)) & ~kAlignedFlag;
+        pf0 = __ldg(wptr + min(g2 * G, nslices)) & ~kWptrFlags;
+        pf1 = __ldg(wptr + min(g2 * G + G, nslices)) & ~kWptrFlags;
       }
     }
 #endif
 #pragma unroll
     for (int g = 0; g < G; ++g) {
       al_g[g] = wp[g] < 0;  // kAlignedFlag
+      all_uni = all_uni && (wp[g] & kUniformFlag) != 0;
       all_al = all_al && al_g[g];
       any_al = any_al || al_g[g];
     }
 #pragma unroll
-    for (int g = 0; g <= G; ++g) wp[g] &= ~kAlignedFlag;
+    for (int g = 0; g <= G; ++g) wp[g] &= ~kWptrFlags;
     double pi[G];
 #pragma unroll
     for (int g = 0; g < G; ++g) {
@@ -409,19 +464,22 @@ __device__ __forceinline__ double phase_spmv_fmt(const Ctx& c, const PT* p, cons
       pi[g] = gather64<COH>(pg, row < 0 ? 0 : row);  // p_i for gamma, issued with the other gathers
     }
     A acc[G];
-    if (wmax <= 7 && all_al) {
-      narrow_group_sum<UR, COH, 2, G>(c, p, wp, lane, rows, acc);
-    } else if (wmax <= 7 && !any_al) {
+    if (all_uni) {  // uniform stencil: columns are row + a constant of the handle
+      if (c.uni_noclamp) narrow_uniform_sum<UR, COH, G, false>(c, p, wp, lane, rows, acc);
+      else narrow_uniform_sum<UR, COH, G, true>(c, p, wp, lane, rows, acc);
+    } else if (wmax <= 7 && (all_al || !any_al)) {
       if constexpr (G <= 2) {
-        narrow_group_sum<UR, COH, CMG, G>(c, p, wp, lane, rows, acc);
-      } else {  // per-entry indices need registers too: two slices at a time
+        if (all_al) narrow_group_sum<UR, COH, 2, G>(c, p, wp, lane, rows, acc);
+        else narrow_group_sum<UR, COH, CMG, G>(c, p, wp, lane, rows, acc);
+      } else {  // bases / per-entry indices need registers too: two slices at a time
         static_assert(G % 2 == 0, "group size");
 #pragma unroll
         for (int h = 0; h < G; h += 2) {
           const int wp2[3] = {wp[h], wp[h + 1], wp[h + 2]};
           const int rows2[2] = {rows[h], rows[h + 1]};
           A acc2[2];
-          narrow_group_sum<UR, COH, CMG, 2>(c, p, wp2, lane, rows2, acc2);
+          if (all_al) narrow_group_sum<UR, COH, 2, 2>(c, p, wp2, lane, rows2, acc2);
+          else narrow_group_sum<UR, COH, CMG, 2>(c, p, wp2, lane, rows2, acc2);
           acc[h] = acc2[0]; acc[h + 1] = acc2[1];
         }
       }
@@ -472,8 +530,11 @@ __device__ __forceinline__ double phase_spmv_fmt(const Ctx& c, const PT* p, cons
 template <int UR, bool COH, int NT, class PT, class PG>
 __device__ __forceinline__ double phase_spmv(const Ctx& c, const PT* p, const PG* pg, typename Store<UR>::T* q, int bid, int nb,
                                              double* red) {
-  if (c.sell_cols16 != nullptr) return phase_spmv_fmt<UR, COH, 1, NT>(c, p, pg, q, bid, nb, red);
-  return phase_spmv_fmt<UR, COH, 0, NT>(c, p, pg, q, bid, nb, red);
+  // (measured, profiles/r02.md: groups of 4 slices in the FP32 phase of uniform-stencil matrices spill at the 64-register
+  // budget and are slower: c2 32.1 vs 25.0 us, c3 52.4 vs 40.7 us)
+  constexpr int G = SpmvGroup<UR>::G;
+  if (c.sell_cols16 != nullptr) return phase_spmv_fmt<UR, COH, 1, NT, G>(c, p, pg, q, bid, nb, red);
+  return phase_spmv_fmt<UR, COH, 0, NT, G>(c, p, pg, q, bid, nb, red);
 }
 
 // ------------------------------------------------------------------ create(): CSR -> SELL-32 --
@@ -549,6 +610,22 @@ __global__ void k_sell_scan(int n, int nslices, int long_min, int allow_aligned,
   if (lane == 0) width[s] = w;
 }
 
+// after pass 2: flag (bit 30 of wptr) every diagonal-aligned slice that is ref_w wide and has the diagonal offsets of the
+// reference slice (bases[ref_w0 .. ref_w0 + ref_w)); counts the flagged slices
+__global__ void k_mark_uniform(int nslices, int32_t* __restrict__ wptr, const int32_t* __restrict__ bases, int ref_w0, int ref_w,
+                               int* __restrict__ count) {
+  const int s = blockIdx.x * blockDim.x + threadIdx.x;
+  if (s >= nslices) return;
+  const int a = wptr[s], b = wptr[s + 1];
+  if (a >= 0) return;  // not aligned
+  const int w0 = a & ~kWptrFlags, w = (b & ~kWptrFlags) - w0;
+  if (w != ref_w) return;
+  for (int k = 0; k < w; ++k)
+    if (bases[w0 + k] != bases[ref_w0 + k]) return;
+  atomicOr(wptr + s, kUniformFlag);
+  atomicAdd(count, 1);
+}
+
 // pass 2: one warp per slice; lane = row slot.  Long rows and padding slots get length 0.
 // General slices: padding entries take the smallest real column of their entry index k (the base of
 // the 16-bit format) and value 0; flag16 is set when some offset from the base does not fit 16 bits.
@@ -561,7 +638,7 @@ __global__ void k_sell_pack(int n, int nslices, int long_min, int shift, const i
   const int s = (int)(((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5);
   if (s >= nslices) return;
   const bool aligned = wptr[s] < 0;
-  const int w0 = wptr[s] & ~kAlignedFlag, w = (wptr[s + 1] & ~kAlignedFlag) - w0;
+  const int w0 = wptr[s] & ~kWptrFlags, w = (wptr[s + 1] & ~kWptrFlags) - w0;
   const int64_t base = (int64_t)w0 * 32;
   int row, e0, len;
   sell_slot(n, s, lane, long_min, rowptr, perm, row, e0, len);

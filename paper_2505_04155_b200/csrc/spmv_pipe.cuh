@@ -182,7 +182,7 @@ __device__ __forceinline__ double pipe_body(const Ctx& c, const PT* p, const PG*
       const int* sb0 = sbase + st * kPipeBaseInts - (hd.z & ~3);
       const int* sw0 = swptr + st * kPipeWptrInts - (hd.x & ~3);
       for (int sl = hd.x + wg; sl < hd.y; sl += kPipeGroupWarps) {
-        const int w0 = sw0[sl] & ~kAlignedFlag, w = (sw0[sl + 1] & ~kAlignedFlag) - w0;
+        const int w0 = sw0[sl] & ~kWptrFlags, w = (sw0[sl + 1] & ~kWptrFlags) - w0;
         const int row = sl * 32 + lane;
         const PT* pl = p + row;
         const double pi = gather64<false>(pg, row);  // the stored p_i (u_z precision) for gamma

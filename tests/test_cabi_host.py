@@ -47,8 +47,9 @@ def test_struct_layout_matches_c(A, tmp_path):
     # compile a tiny C program against the header and compare sizeof/offsetof with ctypes
     probes = [("amp_policy_t", A.Policy, ["C", "stop_safety", "profile_kernels"]),
               ("amp_stats_t", A.Stats, ["bnorm", "fp16_inf"]),
-              ("amp_create_opts_t", A.CreateOpts, ["pdl", "cheb_degree", "cheb_lmax", "stream", "halo_lo", "halo_hi"]),
+              ("amp_create_opts_t", A.CreateOpts, ["pdl", "cheb_degree", "cheb_lmax", "stream", "halo_lo", "halo_hi", "vec_kernel"]),
               ("amp_shard_t", A.Shard, ["row1", "halo_hi", "nnz"]),
+              ("amp_format_info_t", A.FormatInfo, ["uniform_slices", "guard", "index_bits", "uniform_width"]),
               ("amp_shard_export_t", A.ShardExport, ["guard", "mem", "off"]),
               ("amp_kernel_time_t", A.KernelTime, ["launches", "bytes_per_launch"]),
               ("amp_debug_step_t", A.DebugStep, ["first", "omega", "sum1"])]

@@ -25,20 +25,23 @@ def test_lagged_parity(name, size, pname):
     kw = POLICIES[pname]
     ref = O.amp_pcg(s.rowptr, s.colidx, s.vals, s.b, s.tol, s.maxit, O.make_policy(scale_mode=O.SCALE_LAGGED, **kw))
     rp, ci, va, b = to_device(s)
-    with A.AmpPcg(rp, ci, va) as h:
-        for loop in (A.LOOP_GRAPH, A.LOOP_STREAM, A.LOOP_PERSISTENT, A.LOOP_AUTO):
-            x = torch.zeros(s.n, dtype=torch.float64, device="cuda")
-            st = h.solve(b, x, s.tol, s.maxit,
-                         A.Policy.default(scale_mode=A.SCALE_LAGGED, loop_mode=loop, true_residual=1, x0_zero=1, **kw))
-            assert st.status == ref.status == 0
-            assert iters_close(st.iters, ref.iters), (st.iters, ref.iters)
-            for key in ("it_ur32", "it_uz32", "it_uz16"):
-                assert switch_close(getattr(st, key), getattr(ref, key)), (key, getattr(st, key), getattr(ref, key))
-            true = np.linalg.norm(s.b - O.spmv_fp64(s.rowptr, s.colidx, s.vals, x.cpu().numpy())) / np.linalg.norm(s.b)
-            assert st.relres_true == pytest.approx(true, rel=1e-6) and true <= 2 * s.tol
-            assert st.relres_updated <= s.tol
-            if st.loop_mode != A.LOOP_PERSISTENT:  # 3 kernels per iteration + setup, first k_z, residual SpMV, finalize
-                assert h.last_launch_count() == 3 * st.iters + 4
+    for fuse in (A.FUSE_OFF, A.FUSE_ON):
+        with A.AmpPcg(rp, ci, va, fuse_vec=fuse) as h:
+            for loop in (A.LOOP_GRAPH, A.LOOP_STREAM, A.LOOP_PERSISTENT, A.LOOP_AUTO):
+                x = torch.zeros(s.n, dtype=torch.float64, device="cuda")
+                st = h.solve(b, x, s.tol, s.maxit,
+                             A.Policy.default(scale_mode=A.SCALE_LAGGED, loop_mode=loop, true_residual=1, x0_zero=1, **kw))
+                assert st.status == ref.status == 0
+                assert iters_close(st.iters, ref.iters), (st.iters, ref.iters)
+                for key in ("it_ur32", "it_uz32", "it_uz16"):
+                    assert switch_close(getattr(st, key), getattr(ref, key)), (key, getattr(st, key), getattr(ref, key))
+                true = np.linalg.norm(s.b - O.spmv_fp64(s.rowptr, s.colidx, s.vals, x.cpu().numpy())) / np.linalg.norm(s.b)
+                assert st.relres_true == pytest.approx(true, rel=1e-6) and true <= 2 * s.tol
+                assert st.relres_updated <= s.tol
+                if st.loop_mode != A.LOOP_PERSISTENT:
+                    # unfused: 3 kernels per iteration + setup, first k_z, residual SpMV, finalize;
+                    # fused: mat-vec + k_vec_fused per iteration + setup, first k_z and k_p, residual SpMV, finalize
+                    assert h.last_launch_count() == (3 * st.iters + 4 if fuse == A.FUSE_OFF else 2 * st.iters + 5)
 
 
 def test_lagged_edge_cases():

@@ -272,7 +272,7 @@ def test_solve_host_matches_device(systems):
         xh = torch.zeros(s.n, dtype=torch.float64).pin_memory()
         st_h = h.solve_host(bh, xh, s.tol, s.maxit, cuda_policy(spec, loop_mode=A.LOOP_GRAPH, x0_zero=1))
         assert st_h.iters == st_d.iters and np.array_equal(xh.numpy(), x_d)
-        assert h.last_launch_count() >= 4 * st_h.iters
+        assert h.last_launch_count() >= 2 * st_h.iters   # mat-vec + fused vector kernel per iteration (4 kernels unfused)
 
 
 # ------------------------------------------------------------------ the paper's examples ------

@@ -193,3 +193,28 @@ def test_long_rows_at_high_indices_of_a_large_irregular_matrix():
                 st = h.solve(torch.from_numpy(b).cuda(), x, 1e-30, 8, A.Policy.default(x0_zero=1, loop_mode=loop, **spec))
                 assert st.iters == 8
                 assert np.allclose(h.residual_history(), ref.hist, rtol=1e-6), (spec, loop)
+
+
+def test_format_info_reports_what_create_built():
+    """amp_pcg_format_info: structured-grid matrices are diagonal-aligned throughout; narrow stencils (c1-c3) mark nearly
+    all slices as the uniform stencil (columns = row + a constant; boundary slices of the grid lack diagonals and keep the
+    general aligned path); c4 runs the pipelined mat-vec; c5 has sorted rows and 16-bit offsets."""
+    def info(name, size, **opts):
+        s = make_config(name, size)
+        with A.AmpPcg(*[torch.from_numpy(a).cuda() for a in (s.rowptr, s.colidx, s.vals)], **opts) as h:
+            return s, h.format_info()
+
+    for name, size, w, maxoff in (("c1", 64, 5, 64), ("c2", 64, 7, 64 * 64), ("c3", 64, 7, 64 * 64)):
+        s, fi = info(name, size)
+        assert fi.slices == (s.n + 31) // 32 and fi.aligned_slices == fi.slices and fi.index_bits == 0, fi.asdict()
+        assert fi.uniform_width == w and fi.uniform_slices >= 0.9 * fi.slices, fi.asdict()
+        assert fi.guard >= maxoff and fi.long_rows == 0 and fi.rows_sorted == 0, fi.asdict()
+        assert fi.stored_entries >= s.nnz
+        _, fi2 = info(name, size, index_format=A.INDEX_NO_ALIGN)
+        assert fi2.aligned_slices == 0 and fi2.uniform_slices == 0 and fi2.index_bits == 16
+    s, fi = info("c4", 32)
+    assert fi.aligned_slices == fi.slices and fi.spmv_pipelined == 1 and fi.uniform_slices == 0   # 27 entries per row: not narrow
+    s, fi = info("c5", 30000)
+    assert fi.aligned_slices == 0 and fi.rows_sorted == 1 and fi.index_bits == 16
+    s, fi = info("c2", 24, vec_kernel=A.VEC_STAGED)
+    assert fi.vec_staged == 3
