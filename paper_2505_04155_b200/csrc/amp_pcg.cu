@@ -92,6 +92,7 @@ struct amp_pcg {
   int shard_rank = -1, shard_world = 0;  // set by amp_pcg_shard_attach*
   int64_t nslices_aligned = 0, nslices_uniform = 0;
   int index_bits = 0, rows_sorted = 0;
+  int use_uni_kernel = 0;                // the loop's direct mat-vec is k_spmv_uni (every slice aligned, natural order, no long rows)
   int use_fused = 0, grid_fused = 1;     // the loop runs k_vec_fused (vec_fused.cuh) instead of k_xr, k_z, k_p
   cudaGraph_t graph_fu[2] = {nullptr, nullptr};          // [lagged] graph loops with the fused vector kernel
   cudaGraphExec_t graph_fu_exec[2] = {nullptr, nullptr};
@@ -556,6 +557,7 @@ extern "C" amp_pcg_t* amp_pcg_create_ex(int64_t n, int64_t nnz, const int32_t* r
           c.uni_w = ref_w;
           const int64_t uguard = (((int64_t)maxoff + 64 + 127) / 128) * 128;
           if (uguard <= kPipeMaxGuard) { h->guard = std::max(h->guard, uguard); c.uni_noclamp = 1; }
+          h->use_uni_kernel = perm.empty() && long_rows.empty() && w_aligned == wsum && !h->use_pipe;
         }
       }
     }
@@ -802,7 +804,9 @@ static cudaError_t launch_vec(amp_pcg* h, int which, cudaStream_t s, const Ctx& 
 // phases; whichever kernel's phase it is not returns at once)
 // pdl_first: whether the first of the (up to) two kernels may start early (false when the mat-vec opens an iteration)
 static cudaError_t launch_spmv_loop(amp_pcg* h, cudaStream_t s, const Ctx& c, bool pdl, int zmode = 0, int pdl_first = -1) {
-  cudaError_t e = launch_loop_kernel_ex(k_spmv, h->spmv_grid, kSpmvThreads, s, pdl_first < 0 ? pdl : pdl_first != 0, 0, c, zmode);
+  const bool p1 = pdl_first < 0 ? pdl : pdl_first != 0;
+  cudaError_t e = (h->use_uni_kernel && zmode == 0) ? launch_loop_kernel_ex(k_spmv_uni, h->spmv_grid, kSpmvThreads, s, p1, 0, c)
+                                                    : launch_loop_kernel_ex(k_spmv, h->spmv_grid, kSpmvThreads, s, p1, 0, c, zmode);
   if (e == cudaSuccess && h->use_pipe)
     e = launch_loop_kernel_ex(k_spmv_pipe, h->pipe_grid, kPipeThreads, s, pdl, (size_t)kPipeSmemBytes, c, zmode);
   return e;

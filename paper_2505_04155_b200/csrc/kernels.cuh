@@ -140,6 +140,32 @@ __global__ void __launch_bounds__(kSpmvThreads, kSpmvMinBlocks) k_spmv(const Ctx
                             [&](double tot) { if (c.sh != nullptr) shard_reduce_point(c, kEpiGamma, tot, 0.0); else epi_gamma(epi_ctx(c), tot); });
 }
 
+// step a4 for uniform-stencil matrices (phase_spmv_uni); takes k_spmv's place in the loop when the handle qualifies
+template <int NT>
+__device__ __forceinline__ double dispatch_spmv_uni(const Ctx& c, int ur, int uz, int bid, int nb) {
+  if (ur == P64) {
+    if (uz == P64) return phase_spmv_uni<P64, NT>(c, c.p64, c.p64, c.q64, bid, nb);
+    if (uz == P32) return phase_spmv_uni<P64, NT>(c, c.p32, c.p32, c.q64, bid, nb);
+    return phase_spmv_uni<P64, NT>(c, c.p16, c.p16, c.q64, bid, nb);
+  }
+  if (uz == P64) return phase_spmv_uni<P32, NT>(c, c.p32, c.p64, c.q32, bid, nb);  // gathers RN32(p) (phase_p, shadow32)
+  if (uz == P32) return phase_spmv_uni<P32, NT>(c, c.p32, c.p32, c.q32, bid, nb);
+  return phase_spmv_uni<P32, NT>(c, c.p16, c.p16, c.q32, bid, nb);
+}
+
+__global__ void __launch_bounds__(kSpmvThreads, kSpmvMinBlocks) k_spmv_uni(const Ctx c) {
+  __shared__ double red[32];
+  DevState* s = c.st;
+  pdl_launch_dependents();
+  pdl_wait();
+  if (s->done) return;
+  const int bid = blockIdx.x, nb = gridDim.x;
+  if (c.sh != nullptr) shard_wait_halo(c, (unsigned int)s->k + 1u);
+  const double v = dispatch_spmv_uni<kSpmvThreads>(c, s->ur, s->uz, bid, nb);
+  grid_reduce<kSpmvThreads>(v, c.partials + 1 * kMaxGrid, &s->counter[1], bid, nb, red,
+                            [&](double tot) { if (c.sh != nullptr) shard_reduce_point(c, kEpiGamma, tot, 0.0); else epi_gamma(epi_ctx(c), tot); });
+}
+
 __global__ void __launch_bounds__(kVecThreads, AMP_KXR_BLOCKS) k_xr(const Ctx c) {
   __shared__ double red[32];
   DevState* s = c.st;

@@ -527,6 +527,67 @@ __device__ __forceinline__ double phase_spmv_fmt(const Ctx& c, const PT* p, cons
   return gsum;
 }
 
+// The mat-vec of a UNIFORM-STENCIL matrix as a lean loop of its own (k_spmv_uni): every slice diagonal-aligned, natural
+// row order, no long rows (create() checks).  The general loop above carries the row order, the long-row test, the L2
+// prefetch and three index formats through every pass: at 7 entries per row that bookkeeping was more than half of the
+// 267 instructions of a pass and spilled loop-carried values at the 64-register budget (ncu source page, c2).
+// Slices that are not flagged uniform (grid boundaries) take the aligned slice_sum.  Same fma chains: same bits.
+template <int UR, int NT, class PT, class PG>
+__device__ __forceinline__ double phase_spmv_uni(const Ctx& c, const PT* p, const PG* pg, typename Store<UR>::T* q, int bid, int nb) {
+  using A = typename SpmvT<UR>::A;
+  constexpr int G = SpmvGroup<UR>::G;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  constexpr int wpb = NT / 32;
+  const int32_t* __restrict__ wptr = c.sell_wptr;
+  const int nslices = c.nslices;
+  const int n = (int)c.n;
+  const int ngroups = (nslices + G - 1) / G;
+  const int stride = nb * wpb;
+  double gsum = 0.0;
+  int gi = bid * wpb + warp;
+  int wnext[G + 1];
+#pragma unroll
+  for (int g = 0; g <= G; ++g) wnext[g] = (gi < ngroups) ? __ldg(wptr + min(gi * G + g, nslices)) : 0;
+  for (; gi < ngroups; gi += stride) {
+    int wp[G + 1];
+#pragma unroll
+    for (int g = 0; g <= G; ++g) wp[g] = wnext[g];
+    if (gi + stride < ngroups) {  // slice table of the next pass: off the critical path
+#pragma unroll
+      for (int g = 0; g <= G; ++g) wnext[g] = __ldg(wptr + min((gi + stride) * G + g, nslices));
+    }
+    bool all_uni = true;
+#pragma unroll
+    for (int g = 0; g < G; ++g) all_uni = all_uni && (wp[g] & kUniformFlag) != 0;
+#pragma unroll
+    for (int g = 0; g <= G; ++g) wp[g] &= ~kWptrFlags;
+    int rows[G];
+    double pi[G];
+#pragma unroll
+    for (int g = 0; g < G; ++g) {
+      const int row = (gi * G + g) * 32 + lane;
+      rows[g] = (gi * G + g < nslices && row < n) ? row : -1;
+      pi[g] = gather64<false>(pg, rows[g] < 0 ? 0 : rows[g]);  // the stored p_i for gamma
+    }
+    A acc[G];
+    if (all_uni) {
+      if (c.uni_noclamp) narrow_uniform_sum<UR, false, G, false>(c, p, wp, lane, rows, acc);
+      else narrow_uniform_sum<UR, false, G, true>(c, p, wp, lane, rows, acc);
+    } else {
+#pragma unroll
+      for (int g = 0; g < G; ++g) acc[g] = slice_sum<UR, false, 2>(c, p, wp[g], wp[g + 1] - wp[g], lane, rows[g]);
+    }
+#pragma unroll
+    for (int g = 0; g < G; ++g) {
+      if (rows[g] >= 0) {
+        q[rows[g]] = acc[g];
+        gsum = fma(pi[g], (double)acc[g], gsum);
+      }
+    }
+  }
+  return gsum;
+}
+
 template <int UR, bool COH, int NT, class PT, class PG>
 __device__ __forceinline__ double phase_spmv(const Ctx& c, const PT* p, const PG* pg, typename Store<UR>::T* q, int bid, int nb,
                                              double* red) {
