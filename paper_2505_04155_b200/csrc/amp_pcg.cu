@@ -472,6 +472,39 @@ extern "C" amp_pcg_t* amp_pcg_create_ex(int64_t n, int64_t nnz, const int32_t* r
     h->index_bits = (w_aligned == wsum) ? 0 : (wide ? 32 : 16);
     h->rows_sorted = perm.empty() ? 0 : 1;
 
+    // ---- uniform stencil (spmv.cuh, narrow_uniform_sum): narrow diagonal-aligned slices that share one set of offsets ----
+    {
+      int wmax_all = 0;
+      for (int64_t sl = 0; sl < nsl; ++sl) wmax_all = std::max(wmax_all, (int)(width[(size_t)sl] & 0x7fffffff));
+      // reference slice: the first diagonal-aligned slice of full width from the middle of the matrix on (boundary slices
+      // of a grid lack some diagonals)
+      int64_t ref = -1;
+      for (int64_t sl = nsl / 2; sl < nsl && ref < 0; ++sl)
+        if (width[(size_t)sl] < 0 && (int)(width[(size_t)sl] & 0x7fffffff) == wmax_all) ref = sl;
+      const int ref_w = wmax_all;
+      if (o.index_format == AMP_INDEX_AUTO && wmax_all >= 1 && wmax_all <= 7 && ref >= 0) {
+        const int ref_w0 = wptr[(size_t)ref] & 0x7fffffff;
+        int* cnt_d;
+        ALLOC(cnt_d, int, 1);
+        k_mark_uniform<<<(int)((nsl + 255) / 256), 256, 0, h->stream>>>((int)nsl, wptr_d, base_d, ref_w0, ref_w, cnt_d);
+        int cnt = 0;
+        int32_t ub[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+        CU_TRY(cudaMemcpyAsync(&cnt, cnt_d, sizeof(int), cudaMemcpyDeviceToHost, h->stream), { amp_pcg_destroy(h); return nullptr; });
+        CU_TRY(cudaMemcpyAsync(ub, base_d + ref_w0, sizeof(int32_t) * (size_t)ref_w, cudaMemcpyDeviceToHost, h->stream),
+               { amp_pcg_destroy(h); return nullptr; });
+        CU_TRY(cudaStreamSynchronize(h->stream), { amp_pcg_destroy(h); return nullptr; });
+        CU_TRY(cudaGetLastError(), { amp_pcg_destroy(h); return nullptr; });
+        h->nslices_uniform = cnt;
+        if (cnt > 0) {  // (slices that do not match keep the general aligned path: the flag is per slice)
+          int maxoff = 0;
+          for (int k = 0; k < ref_w; ++k) { c.uni_base[k] = ub[k]; maxoff = std::max(maxoff, std::abs(ub[k])); }
+          c.uni_w = ref_w;
+          const int64_t uguard = (((int64_t)maxoff + 64 + 127) / 128) * 128;
+          if (uguard <= kPipeMaxGuard) { h->guard = std::max(h->guard, uguard); c.uni_noclamp = 1; }
+          h->use_uni_kernel = perm.empty() && long_rows.empty() && w_aligned == wsum;
+        }
+      }
+    }
     // ---- bulk-copy pipelined SpMV (spmv_pipe.cuh): eligibility, zero guard band of p, stage plan ----
     {
       bool eligible = o.spmv_kernel != AMP_SPMV_DIRECT && perm.empty() && long_rows.empty() && w_aligned == wsum;
@@ -482,6 +515,9 @@ extern "C" amp_pcg_t* amp_pcg_create_ex(int64_t n, int64_t nnz, const int32_t* r
       // measured (B200, profiles/r02.md): the pipelined kernel wins for wide slices (c4, 27 entries per row: 181 vs 210 us
       // in the FP32 phase) and loses for narrow ones (c2/c3, 7 per row: 43 vs 29 us), where the per-slice bookkeeping of
       // a consumer warp outweighs its 7 entries; AUTO therefore takes it from an average slice width of 12
+      // (also tried for narrow uniform stencils with a consumer path that takes four slices at once with constant
+      // offsets: c2 41.5 vs 25.0 us, c3 66.0 vs 39.3 us against the direct k_spmv_uni — 15 consumer warps per SM cannot keep
+      // enough gathers of p in flight; dropped)
       if (o.spmv_kernel == AMP_SPMV_AUTO && (double)wsum < 12.0 * (double)nsl) eligible = false;
       if (eligible) {
         cudaError_t ea = cudaFuncSetAttribute((const void*)k_spmv_pipe, cudaFuncAttributeMaxDynamicSharedMemorySize, kPipeSmemBytes);
@@ -530,41 +566,8 @@ extern "C" amp_pcg_t* amp_pcg_create_ex(int64_t n, int64_t nnz, const int32_t* r
                { amp_pcg_destroy(h); return nullptr; });
         CU_TRY(cudaStreamSynchronize(h->stream), { amp_pcg_destroy(h); return nullptr; });
         c.pipe_chunks = chunks_d; c.pipe_blk_chunk = blk_d; c.use_pipe = 1;
-        h->use_pipe = 1; h->pipe_grid = nb; h->pipe_chunks = nch; h->guard = guard;
+        h->use_pipe = 1; h->pipe_grid = nb; h->pipe_chunks = nch; h->guard = std::max(h->guard, guard);
         h->idx_bytes_total += 8.0 * (double)(nch + 1) + 4.0 * (double)(nb + 1);  // stage descriptors
-      }
-    }
-    // ---- uniform stencil (spmv.cuh, narrow_uniform_sum): narrow diagonal-aligned slices that share one set of offsets ----
-    {
-      int wmax_all = 0;
-      for (int64_t sl = 0; sl < nsl; ++sl) wmax_all = std::max(wmax_all, (int)(width[(size_t)sl] & 0x7fffffff));
-      // reference slice: the first diagonal-aligned slice of full width from the middle of the matrix on (boundary slices
-      // of a grid lack some diagonals)
-      int64_t ref = -1;
-      for (int64_t sl = nsl / 2; sl < nsl && ref < 0; ++sl)
-        if (width[(size_t)sl] < 0 && (int)(width[(size_t)sl] & 0x7fffffff) == wmax_all) ref = sl;
-      const int ref_w = wmax_all;
-      if (o.index_format == AMP_INDEX_AUTO && wmax_all >= 1 && wmax_all <= 7 && ref >= 0) {
-        const int ref_w0 = wptr[(size_t)ref] & 0x7fffffff;
-        int* cnt_d;
-        ALLOC(cnt_d, int, 1);
-        k_mark_uniform<<<(int)((nsl + 255) / 256), 256, 0, h->stream>>>((int)nsl, wptr_d, base_d, ref_w0, ref_w, cnt_d);
-        int cnt = 0;
-        int32_t ub[8] = {0, 0, 0, 0, 0, 0, 0, 0};
-        CU_TRY(cudaMemcpyAsync(&cnt, cnt_d, sizeof(int), cudaMemcpyDeviceToHost, h->stream), { amp_pcg_destroy(h); return nullptr; });
-        CU_TRY(cudaMemcpyAsync(ub, base_d + ref_w0, sizeof(int32_t) * (size_t)ref_w, cudaMemcpyDeviceToHost, h->stream),
-               { amp_pcg_destroy(h); return nullptr; });
-        CU_TRY(cudaStreamSynchronize(h->stream), { amp_pcg_destroy(h); return nullptr; });
-        CU_TRY(cudaGetLastError(), { amp_pcg_destroy(h); return nullptr; });
-        h->nslices_uniform = cnt;
-        if (cnt > 0) {  // (slices that do not match keep the general aligned path: the flag is per slice)
-          int maxoff = 0;
-          for (int k = 0; k < ref_w; ++k) { c.uni_base[k] = ub[k]; maxoff = std::max(maxoff, std::abs(ub[k])); }
-          c.uni_w = ref_w;
-          const int64_t uguard = (((int64_t)maxoff + 64 + 127) / 128) * 128;
-          if (uguard <= kPipeMaxGuard) { h->guard = std::max(h->guard, uguard); c.uni_noclamp = 1; }
-          h->use_uni_kernel = perm.empty() && long_rows.empty() && w_aligned == wsum && !h->use_pipe;
-        }
       }
     }
     {  // p and z (both are gathered by a mat-vec: z inside the Chebyshev-Jacobi preconditioner) in their three storage

@@ -159,6 +159,7 @@ __global__ void __launch_bounds__(kSpmvThreads, kSpmvMinBlocks) k_spmv_uni(const
   pdl_launch_dependents();
   pdl_wait();
   if (s->done) return;
+  if (c.use_pipe && s->ur == P32) return;  // this iteration's mat-vec is k_spmv_pipe's (next in the chain)
   const int bid = blockIdx.x, nb = gridDim.x;
   if (c.sh != nullptr) shard_wait_halo(c, (unsigned int)s->k + 1u);
   const double v = dispatch_spmv_uni<kSpmvThreads>(c, s->ur, s->uz, bid, nb);

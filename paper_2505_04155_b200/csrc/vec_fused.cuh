@@ -16,8 +16,14 @@
 
 namespace amp {
 
-constexpr int kFusedThreads = 256;
-constexpr int kFusedMinBlocks = 2;  // the x/r update needs 128 registers
+#ifndef AMP_FUSED_THREADS
+#define AMP_FUSED_THREADS 256
+#endif
+#ifndef AMP_FUSED_BLOCKS
+#define AMP_FUSED_BLOCKS 2
+#endif
+constexpr int kFusedThreads = AMP_FUSED_THREADS;
+constexpr int kFusedMinBlocks = AMP_FUSED_BLOCKS;  // 256 x 2: the x/r update needs 128 registers
 
 // LAGGED = false: [xr | sum | z | sum | p];  LAGGED = true (AMP_SCALE_LAGGED): [xrz | sum2 | p]
 template <bool LAGGED>
