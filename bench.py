@@ -58,8 +58,12 @@ def parse_args():
     ap.add_argument("--vec-kernel", default="auto", choices=["auto", "direct", "staged"])
     ap.add_argument("--fuse", default="auto", choices=["auto", "off", "on"], help="fused vector kernel (create option fuse_vec)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--others", default="", help="comma list of further workloads to report under 'other_workloads' "
-                                                 "(value / time_to_tol / speed-up only), e.g. c1,c2,c3,c5")
+    ap.add_argument("--others", default="c2,c3,c1,c5",
+                    help="comma list of further workloads to report under 'other_workloads' (value / time_to_tol / speed-up "
+                         "only; '' = none); a workload is skipped once --time-budget seconds have passed")
+    ap.add_argument("--time-budget", type=float, default=150.0,
+                    help="seconds after which the optional legs (other workloads) are skipped, so that the default run ends "
+                         "within a few minutes")
     ap.add_argument("--cheb-degrees", default="2,3", help="degrees of the Chebyshev-Jacobi preconditioner to time beside "
                                                            "the Jacobi headline ('' = none)")
     ap.add_argument("--profile-iters", type=int, default=0,
@@ -340,6 +344,8 @@ def run_ours(args, rank: int, local_rank: int, world: int):
     import numpy as np  # noqa: F401
     import torch
 
+    t_start = time.perf_counter()
+
     import paper_2505_04155_b200 as A
     from workloads import make_config
 
@@ -460,7 +466,10 @@ def run_ours(args, rank: int, local_rank: int, world: int):
 
     # ---- the other BASELINE.json configs (parity-test cases; reported for context) ----
     others = {}
-    for name in [t for t in args.others.split(",") if t]:
+    for name in [t for t in args.others.split(",") if t and t != args.workload]:
+        if time.perf_counter() - t_start > args.time_budget:
+            others.setdefault("skipped_for_time", []).append(name)
+            continue
         so = make_config(name)
         Ro = Runner(A, torch, so, dev, loop, spmv_kernel, vec_kernel=vec_kernel, fuse_vec=fuse)
         a_, _ = Ro.summary(args.policy, 2)

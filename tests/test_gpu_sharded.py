@@ -105,6 +105,25 @@ def test_sharded_solve_matches_oracle_and_unsharded(name, size, world):
         g.close()
 
 
+def test_sharded_solve_with_staged_vector_kernels():
+    """the bulk-copy staged z / x-r kernels post their partial sums to the mailboxes like the direct ones"""
+    s = make_config("c3", 18)
+    rp, ci, va, b = to_device(s)
+    g, parts = make_group(s, 3, vec_kernel=A.VEC_STAGED)
+    try:
+        assert all(h.format_info().vec_staged == 3 for h in g.handles)
+        for pname in ("amp_fp64_delay", "amp_fp64_delay_lagged", "pcg_fp64"):
+            spec = POLICY_SPECS[pname]
+            ref = O.amp_pcg(s.rowptr, s.colidx, s.vals, s.b, s.tol, s.maxit, oracle_policy(spec))
+            xs = [torch.zeros(bb - aa, dtype=torch.float64, device="cuda") for aa, bb in parts]
+            st = g.solve(split(b, parts), xs, s.tol, s.maxit, cuda_policy(spec, x0_zero=1))[0]
+            assert st.status == 0 and iters_close(st.iters, ref.iters) and st.relres_true <= 2 * s.tol
+            for key in ("it_ur32", "it_uz32", "it_uz16"):
+                assert switch_close(getattr(st, key), getattr(ref, key), 1)
+    finally:
+        g.close()
+
+
 def test_sharded_edge_cases():
     s = make_config("c3", 16)
     rp, ci, va, b = to_device(s)

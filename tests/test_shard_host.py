@@ -249,3 +249,21 @@ def test_sharded_run_over_gloo_reproduces_the_one_rank_oracle(A, tmp_path, name,
             assert set(o["halo_precs"].tolist()) == {2}            # AMP-PCG(FP16): FP16 halos throughout
         else:
             assert o["halo_precs"][-1] == 2 and o["halo_precs"][0] == 0
+
+
+@pytest.mark.parametrize("name", ["c2", "c5"])
+def test_plan_at_full_size_for_eight_ranks(A, name):
+    """the partition bench.py --shard would use on the real configs: 8 ranks, halo = one grid plane (c2) / the 50 000-row
+    band (c5), balanced to a few per cent"""
+    s = make_config(name)
+    plan = A.shard_plan(s.rowptr, s.colidx, 8)
+    rows = [sh.row1 - sh.row0 for sh in plan]
+    cost = [sh.nnz + 4 * r for sh, r in zip(plan, rows)]
+    assert max(cost) <= 1.03 * sum(cost) / 8
+    halo = max(max(sh.halo_lo, sh.halo_hi) for sh in plan)
+    if name == "c2":
+        assert halo == 128 * 128 and all(sh.halo_lo in (0, halo) and sh.halo_hi in (0, halo) for sh in plan)
+    else:
+        assert 49000 <= halo <= 50008 and halo < min(rows)
+    # bytes per iteration that cross ranks, FP16 phase: 2 B per halo entry (the 4x shrink against FP64 is AMP's)
+    assert sum(sh.halo_lo + sh.halo_hi for sh in plan) * 2 <= (2 * 7 * halo) * 2
