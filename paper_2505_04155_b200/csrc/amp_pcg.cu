@@ -649,6 +649,8 @@ extern "C" amp_pcg_t* amp_pcg_create_ex(int64_t n, int64_t nnz, const int32_t* r
   h->grid_cheb0 = vec_grid_for((const void*)k_cheb0);
   h->grid_cheb_step = vec_grid_for((const void*)k_cheb_step);
   h->vec_grid = vec_grid_for((const void*)k_setup);
+  c.spmv_grid_direct = h->spmv_grid;
+  c.spmv_grid_pipe = h->pipe_grid;
   // fused vector kernel (vec_fused.cuh): one cooperative kernel per iteration instead of k_xr, k_z, k_p
   {
     int occ = 0, coop = 0;
@@ -880,9 +882,11 @@ static cudaError_t launch_iteration_lagged(amp_pcg* h, const Ctx& c, cudaStream_
 
 // loop body with the fused vector kernel (vec_fused.cuh): the mat-vec of iteration k, then x/r of k and z, p of k + 1 in
 // one cooperative kernel (z_0, p_0 come from k_z, k_p before the loop)
-static cudaError_t launch_iteration_fused(amp_pcg* h, const Ctx& c, cudaStream_t s, bool pdl, bool lagged, int prof_iter = -1) {
+static cudaError_t launch_iteration_fused(amp_pcg* h, const Ctx& c0, cudaStream_t s, bool pdl, bool lagged, int prof_iter = -1) {
   const bool prof = prof_iter >= 0;
   if (prof) pdl = false;
+  Ctx c = c0;
+  c.defer_gamma = 1;  // the mat-vec publishes partial sums, k_vec_fused adds them and computes alpha
   cudaError_t e = cudaSuccess;
   if (prof) e = prof_mark(h, s, AMP_K_SPMV, prof_iter);
   if (e == cudaSuccess) e = launch_spmv_loop(h, s, c, pdl, 0, 0);

@@ -128,6 +128,10 @@ struct Ctx {
   // every row + offset (the handle's own p / z), so no clamp is needed either
   int32_t uni_w, uni_noclamp;
   int32_t uni_base[8];
+  // fused loop (vec_fused.cuh): the mat-vec only publishes its per-block partial sums of gamma; every block of
+  // k_vec_fused adds them in index order and computes alpha on its replica (no last-block tail in the mat-vec)
+  int32_t defer_gamma;
+  int32_t spmv_grid_direct, spmv_grid_pipe;  // blocks of k_spmv / k_spmv_uni and of k_spmv_pipe (how many partials there are)
   int64_t n_scale;                  // rows of the WHOLE system (= n unless sharded): the n of the RMS scale sqrt(n)/||r||
   const ShardCtx* sh;               // device pointer, nullptr unless attached to a group (amp_pcg_shard_attach*)
 };
@@ -355,6 +359,13 @@ __device__ __forceinline__ void grid_reduce(double v, double* partials, unsigned
       epi(tot);
     }
   }
+}
+
+// first half of grid_reduce only: publish this block's partial sum (the consumer kernel adds the partials itself)
+template <int NT>
+__device__ __forceinline__ void grid_publish(double v, double* partials, int bid, double* sm) {
+  const double bs = block_sum<NT>(v, sm);
+  if (threadIdx.x == 0) __stcg(partials + bid, bs);
 }
 
 // the same for two sums at once (partials interleaved: [2*bid], [2*bid+1])

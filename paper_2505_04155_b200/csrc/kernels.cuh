@@ -136,6 +136,7 @@ __global__ void __launch_bounds__(kSpmvThreads, kSpmvMinBlocks) k_spmv(const Ctx
   if (c.sh != nullptr) shard_wait_halo(c, (unsigned int)s->k + 1u);  // the neighbours' entries of p are in the halo bands
   const double v = dispatch_spmv<false, kSpmvThreads>(c, s->ur, s->uz, zmode, bid, nb, red);
   if (zmode) return;  // q = A z inside M^-1: no inner product
+  if (c.defer_gamma) { grid_publish<kSpmvThreads>(v, c.partials + 1 * kMaxGrid, bid, red); return; }
   grid_reduce<kSpmvThreads>(v, c.partials + 1 * kMaxGrid, &s->counter[1], bid, nb, red,
                             [&](double tot) { if (c.sh != nullptr) shard_reduce_point(c, kEpiGamma, tot, 0.0); else epi_gamma(epi_ctx(c), tot); });
 }
@@ -163,6 +164,7 @@ __global__ void __launch_bounds__(kSpmvThreads, kSpmvMinBlocks) k_spmv_uni(const
   const int bid = blockIdx.x, nb = gridDim.x;
   if (c.sh != nullptr) shard_wait_halo(c, (unsigned int)s->k + 1u);
   const double v = dispatch_spmv_uni<kSpmvThreads>(c, s->ur, s->uz, bid, nb);
+  if (c.defer_gamma) { grid_publish<kSpmvThreads>(v, c.partials + 1 * kMaxGrid, bid, red); return; }
   grid_reduce<kSpmvThreads>(v, c.partials + 1 * kMaxGrid, &s->counter[1], bid, nb, red,
                             [&](double tot) { if (c.sh != nullptr) shard_reduce_point(c, kEpiGamma, tot, 0.0); else epi_gamma(epi_ctx(c), tot); });
 }

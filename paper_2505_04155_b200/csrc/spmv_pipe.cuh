@@ -226,6 +226,7 @@ __global__ void __launch_bounds__(kPipeThreads, 1) k_spmv_pipe(const Ctx c, int 
   else if (uz == P32) v = pipe_body<P32>(c, c.p32, c.p32, c.q32, pipe_smem, hseq);
   else v = pipe_body<P32>(c, c.p32, c.p64, c.q32, pipe_smem, hseq);  // gathers the FP32 copy RN32(p) written by the p update
   pdl_wait();  // (the producer warp has not waited yet) before touching the reduction scratch shared with other kernels
+  if (c.defer_gamma) { grid_publish<kPipeThreads>(v, c.partials + 1 * kMaxGrid, blockIdx.x, red); return; }
   grid_reduce<kPipeThreads>(v, c.partials + 1 * kMaxGrid, &s->counter[1], blockIdx.x, gridDim.x, red,
                             [&](double tot) { if (c.sh != nullptr) shard_reduce_point(c, kEpiGamma, tot, 0.0); else epi_gamma(epi_ctx(c), tot); });
 }

@@ -43,9 +43,30 @@ __global__ void __launch_bounds__(kFusedThreads, kFusedMinBlocks) k_vec_fused(co
   EpiCtx ec = epi_ctx(c);
   ec.st = s;
   ec.use_cond = (bid == 0) ? c.use_cond : 0;  // one block speaks for the WHILE node
-  if (s->done) {  // breakdown in the mat-vec, or nothing to do
+  if (s->done) {  // nothing to do
     if (bid == 0 && threadIdx.x == 0) set_loop_cond(ec, 0);
     return;
+  }
+  if (c.defer_gamma) {
+    // gamma = q^T p: the mat-vec left one partial sum per block; every block adds them in index order and runs
+    // epi_gamma on its replica (alpha, breakdown test) — the same numbers in the same order everywhere
+    const int nbs = (c.use_pipe && s->ur == P32) ? c.spmv_grid_pipe : c.spmv_grid_direct;
+    double a = 0.0;
+    for (int i = threadIdx.x; i < nbs; i += kFusedThreads) a += __ldcg(c.partials + 1 * kMaxGrid + i);
+    const double t = block_sum<kFusedThreads>(a, red);
+    if (threadIdx.x == 0) epi_gamma(ec, t);
+    __syncthreads();
+    if (s->done) {  // breakdown: block 0 publishes status and stops the loop (epi_gamma has set the condition)
+      if (bid == 0) {
+        int* dst = reinterpret_cast<int*>(c.st);
+        const int* src = reinterpret_cast<const int*>(&ls);
+        const int skip0 = (int)(offsetof(DevState, fp16_subnormal) / sizeof(int));
+        const int skip1 = (int)((offsetof(DevState, bar_pad) + sizeof(unsigned int)) / sizeof(int));
+        for (int i = threadIdx.x; i < (int)(sizeof(DevState) / sizeof(int)); i += kFusedThreads)
+          if (i < skip0 || i >= skip1) dst[i] = src[i];
+      }
+      return;
+    }
   }
   // arrivals count up over the whole solve: this is launch number k, every earlier launch made `per` barriers
   constexpr unsigned int per = LAGGED ? 1u : 2u;
