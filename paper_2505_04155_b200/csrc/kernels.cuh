@@ -154,7 +154,10 @@ __device__ __forceinline__ double dispatch_spmv_uni(const Ctx& c, int ur, int uz
   return phase_spmv_uni<P32, NT>(c, c.p16, c.p16, c.q32, bid, nb);
 }
 
-__global__ void __launch_bounds__(kSpmvThreads, kSpmvMinBlocks) k_spmv_uni(const Ctx c) {
+#ifndef AMP_SPMV_UNI_BLOCKS
+#define AMP_SPMV_UNI_BLOCKS AMP_SPMV_MINBLOCKS
+#endif
+__global__ void __launch_bounds__(kSpmvThreads, AMP_SPMV_UNI_BLOCKS) k_spmv_uni(const Ctx c) {
   __shared__ double red[32];
   DevState* s = c.st;
   pdl_launch_dependents();
