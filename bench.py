@@ -61,7 +61,7 @@ def parse_args():
     ap.add_argument("--others", default="c2,c3,c1,c5",
                     help="comma list of further workloads to report under 'other_workloads' (value / time_to_tol / speed-up "
                          "only; '' = none); a workload is skipped once --time-budget seconds have passed")
-    ap.add_argument("--time-budget", type=float, default=150.0,
+    ap.add_argument("--time-budget", type=float, default=100.0,
                     help="seconds after which the optional legs (other workloads) are skipped, so that the default run ends "
                          "within a few minutes")
     ap.add_argument("--cheb-degrees", default="2,3", help="degrees of the Chebyshev-Jacobi preconditioner to time beside "
