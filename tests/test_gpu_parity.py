@@ -318,4 +318,4 @@ def test_paper_examples_parity(ex, spec):
             assert lo <= st.it_uz32 <= hi, (st.it_uz32, lo, hi, ref.it_uz32)
         else:
             assert abs(st.iters - ref.iters) <= max(2, math.ceil(0.05 * ref.iters)), (st.iters, ref.iters)
-            assert switch_close(st.it_ur32, ref.it_ur32, 3) and switch_close(st.it_uz16, ref.it_uz16, 3)
+            assert switch_close(st.it_ur32, ref.it_ur32, 2) and switch_close(st.it_uz16, ref.it_uz16, 2)
