@@ -184,3 +184,32 @@ def test_export_blob_describes_the_rank():
         assert any(bytes(e.mem[0])) and any(bytes(e.mem[3]))
     finally:
         g.close()
+
+
+def test_attach_through_export_blobs_single_rank():
+    """amp_pcg_shard_export / amp_pcg_shard_attach with a group of one (no peer to open): the one-process-per-GPU wiring,
+    whose reducing kernels collect and step inline and whose loop is the WHILE-node graph"""
+    s = make_config("c3", 18)
+    rp, ci, va, b = to_device(s)
+    spec = POLICY_SPECS["amp_fp64_delay"]
+    ref = O.amp_pcg(s.rowptr, s.colidx, s.vals, s.b, s.tol, s.maxit, oracle_policy(spec))
+    h = A.AmpPcg(rp, ci, va)
+    g = A.ShardGroup.attach_ipc(h, 0, [A.ShardGroup.export(h)])
+    try:
+        for lm in (A.LOOP_AUTO, A.LOOP_STREAM):
+            x = torch.zeros(s.n, dtype=torch.float64, device="cuda")
+            st = g.solve([b], [x], s.tol, s.maxit, cuda_policy(spec, x0_zero=1, loop_mode=lm))[0]
+            assert st.status == 0 and st.loop_mode == (A.LOOP_GRAPH if lm == A.LOOP_AUTO else A.LOOP_STREAM)
+            assert iters_close(st.iters, ref.iters) and st.relres_true <= 2 * s.tol
+            for key in ("it_ur32", "it_uz32", "it_uz16"):
+                assert switch_close(getattr(st, key), getattr(ref, key), 1)
+            # inline scalar steps: no k_epi launches — 4 kernels per iteration + set-up, residual mat-vec (2), finalize
+            assert h.last_launch_count() == 4 * st.iters + 4
+        p = torch.rand(s.n, dtype=torch.float64, device="cuda")
+        q = g.spmv([p], A.FP64)[0]
+        assert np.array_equal(q.cpu().numpy(), O.spmv_fp64(s.rowptr, s.colidx, s.vals, p.cpu().numpy()))
+        with pytest.raises(A.AmpPcgError):   # a blob list that does not describe this handle
+            bad = A.ShardExport.from_buffer_copy(A.ShardGroup.export(h)); bad.n += 32
+            A.ShardGroup.attach_ipc(h, 0, [bytes(bad)])
+    finally:
+        g.close()
