@@ -108,7 +108,7 @@ struct amp_pcg {
 #ifndef AMP_GRAPH_UNROLL
 #define AMP_GRAPH_UNROLL 4
 #endif
-constexpr int kGraphUnroll = AMP_GRAPH_UNROLL;  // iterations per body of the fused graph loop (measured, us per iteration for 1 / 2 / 4:
+constexpr int kGraphUnroll = AMP_GRAPH_UNROLL;  // iterations per body of a graph loop (measured on the fused loop, us per iteration for 1 / 2 / 4:
                                                 // c2 47.1 / 45.0 / 44.4, c3 79.7 / 77.9 / 76.3, 262 K rows 23.9 / 21.9 / 20.9: the WHILE node costs
                                                 // about 2.7 us per evaluation)
 constexpr int64_t kVecStagedAutoMinRows = 4000000;  // AMP_VEC_AUTO stages the z and p updates from here on
@@ -927,9 +927,9 @@ static int build_graph_once(amp_pcg* h, bool pdl, bool lagged, int kind) {
   cudaError_t e = cudaStreamBeginCaptureToGraph(cap, body, nullptr, nullptr, 0, cudaStreamCaptureModeRelaxed);
   if (e == cudaSuccess) {
     cudaError_t el = cudaSuccess;
-    // the fused body may hold several iterations: its kernels return at once when the solve has ended, so the WHILE
+    // the body holds several iterations: the loop kernels return at once when the solve has ended, so the WHILE
     // condition is evaluated (and the body re-launched) once per kGraphUnroll iterations
-    for (int u = 0; u < (fused ? kGraphUnroll : 1) && el == cudaSuccess; ++u)
+    for (int u = 0; u < kGraphUnroll && el == cudaSuccess; ++u)
       el = fused     ? launch_iteration_fused(h, c, cap, pdl, lagged)
            : sharded ? launch_iteration_sharded(h, c, cap, pdl, lagged)
                      : (lagged ? launch_iteration_lagged(h, c, cap, pdl) : launch_iteration(h, c, cap, pdl));
@@ -1165,8 +1165,8 @@ static int solve_impl(amp_pcg* h, const double* b, double* x, double tol, int32_
   {
     const int spmv_k = h->use_pipe ? 2 : 1, sweeps = std::max(h->cheb_s, 1);
     const int per_it = fused ? 1 + spmv_k : (lagged ? 2 : 3) + spmv_k + (sweeps - 1) * (spmv_k + 1);  // vector kernels + a4 + extra sweeps
-    // the fused graph body holds kGraphUnroll iterations: the ones after the last are launched too (and return at once)
-    const int64_t its_launched = (fused && mode == AMP_LOOP_GRAPH) ? (int64_t)(iters + kGraphUnroll - 1) / kGraphUnroll * kGraphUnroll : iters;
+    // a graph body holds kGraphUnroll iterations: the ones after the last are launched too (and return at once)
+    const int64_t its_launched = (mode == AMP_LOOP_GRAPH) ? (int64_t)(iters + kGraphUnroll - 1) / kGraphUnroll * kGraphUnroll : iters;
     h->launches += (mode == AMP_LOOP_PERSISTENT) ? 1 : (int64_t)per_it * its_launched;
   }
   if (stats) fill_stats(h, hs, mode, lagged, ms, stats);

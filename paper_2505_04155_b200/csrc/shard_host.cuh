@@ -407,8 +407,9 @@ extern "C" int amp_pcg_solve_sharded(amp_pcg_t* const* handles, int32_t nlocal, 
     h->last_iters = hs->k;
     const int spmv_k = h->use_pipe ? 2 : 1;
     const int epi = split_epi ? 1 : 0;  // k_epi launches per reduction point
+    const int64_t its = (mode == AMP_LOOP_GRAPH) ? (int64_t)(hs->k + kGraphUnroll - 1) / kGraphUnroll * kGraphUnroll : hs->k;
     h->launches = 1 + epi + (pol.x0_zero ? 0 : 2) + (lagged ? 1 + epi : 0) + (pol.true_residual ? 3 + epi : 1) +
-                  (int64_t)hs->k * ((lagged ? 2 : 3) + spmv_k + (lagged ? 2 : 3) * epi);
+                  its * ((lagged ? 2 : 3) + spmv_k + (lagged ? 2 : 3) * epi);
     if (stats) fill_stats(h, hs, mode, lagged, ms, stats + i);
     if (i == 0) status = hs->status;
     else if (hs->status != status || hs->k != handles[0]->h_state->k) {

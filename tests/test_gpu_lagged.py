@@ -41,8 +41,8 @@ def test_lagged_parity(name, size, pname):
                 if st.loop_mode != A.LOOP_PERSISTENT:
                     # unfused: 3 kernels per iteration + setup, first k_z, residual SpMV, finalize;
                     # fused: mat-vec + k_vec_fused per iteration + setup, first k_z and k_p, residual SpMV, finalize
-                    # (the fused GRAPH body holds 4 iterations: the launches after the last one return at once but count)
-                    its = st.iters if (fuse == A.FUSE_OFF or st.loop_mode != A.LOOP_GRAPH) else (st.iters + 3) // 4 * 4
+                    # (a GRAPH body holds 4 iterations: the launches after the last one return at once but count)
+                    its = st.iters if st.loop_mode != A.LOOP_GRAPH else (st.iters + 3) // 4 * 4
                     assert h.last_launch_count() == (3 * its + 4 if fuse == A.FUSE_OFF else 2 * its + 5)
 
 
