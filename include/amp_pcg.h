@@ -398,6 +398,32 @@ typedef struct {
  * Synchronises the stream.  Returns AMP_OK, AMP_ERR_INVALID or AMP_ERR_CUDA. */
 int amp_pcg_debug_step(amp_pcg_t *h, amp_debug_step_t *io, double *x);
 
+/* ---- step a5 without any device allocation ------------------------------------------------------------------------
+ * x += alpha p,  r -= alpha q,  *delta_out = ||r||_2   (Algorithm 4.1 lines 15-17), all FP64, in one
+ * kernel, for callers that can't let this library allocate: every other entry point works on a handle, and
+ * amp_pcg_create() calls cudaMalloc.  That is no option for a process that gave the whole device memory to its own pool
+ * at start-up (a later cudaMalloc fails there, or takes memory the pool's owner counted on), nor for a loop with a
+ * latency bound (cudaMalloc and cudaFree may synchronise the device and have no time bound).  This call needs no handle
+ * and makes no cudaMalloc, cudaFree or other allocating call: the scratch memory of its grid reduction is a static
+ * device array of 131 328 bytes inside the library image, which every GPU that loads the library holds until exit.
+ *   n          elements, 0 < n <= AMP_XR_STATIC_MAX_N (what the fixed array serves; beyond it: AMP_ERR_INVALID, nothing runs)
+ *   alpha      step length (HOST value)
+ *   p, q       float64[n] DEVICE, read-only, 16-byte aligned
+ *   x, r       float64[n] DEVICE, updated in place, 16-byte aligned
+ *   delta_out  float64[1] DEVICE: ||r||_2 after the update, written by the kernel (no host synchronisation)
+ *   cuda_stream  cudaStream_t the work is queued on (NULL = legacy default stream); the call is asynchronous
+ * The arrays must live on the device that is current at the call.  x and r come out bit-identical to the handle path's
+ * FP64 x / r update (k_xr); the norm is added in another fixed order (agreement to n 2^-53 relative).
+ * Sharing: all calls on a device use the one array, which keeps the previous call's contents; the call clears what has
+ * to start at zero itself, in stream order.  Calls that can overlap on one GPU (different streams without an order
+ * between them) race on the array: order them.
+ * Set-up: the first call on each device looks up the array's device address (cudaGetSymbolAddress, once per device,
+ * thread-safe); make that first call before beginning any stream capture.
+ * Returns AMP_OK, AMP_ERR_INVALID (size, null or misaligned pointer) or AMP_ERR_CUDA; amp_pcg_last_error() says why. */
+#define AMP_XR_STATIC_MAX_N 67108864
+int amp_xr_update_static(int64_t n, double alpha, const double *p, const double *q, double *x, double *r,
+                         double *delta_out, void *cuda_stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -15,6 +15,7 @@ from .binding import (  # noqa: F401
     DebugStep,
     AmpPcgError,
     bytes_per_row,
+    xr_update_static, XR_STATIC_MAX_N,
     load_library,
     library_path,
     FP64, FP32, FP16,

@@ -35,8 +35,9 @@ EXPORTED_SYMBOLS = (
     "amp_pcg_eta_posteriori", "amp_pcg_kernel_times",
     "amp_pcg_debug_set_vector", "amp_pcg_debug_get_vector", "amp_pcg_debug_step",
     "amp_pcg_format_info", "amp_shard_plan", "amp_shard_extract", "amp_pcg_shard_export", "amp_pcg_shard_attach", "amp_pcg_shard_attach_local",
-    "amp_pcg_solve_sharded", "amp_spmv_sharded",
+    "amp_pcg_solve_sharded", "amp_spmv_sharded", "amp_xr_update_static",
 )
+XR_STATIC_MAX_N = 67108864  # AMP_XR_STATIC_MAX_N
 SHARD_MAX_WORLD = 16
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
@@ -220,6 +221,8 @@ def load_library(variant: str = ""):
                                         C.POINTER(Stats)]
     L.amp_spmv_sharded.restype = C.c_int
     L.amp_spmv_sharded.argtypes = [C.POINTER(vp), i32, C.c_int, C.c_int, C.POINTER(vp), C.POINTER(vp)]
+    L.amp_xr_update_static.restype = C.c_int
+    L.amp_xr_update_static.argtypes = [i64, dbl, vp, vp, vp, vp, vp, vp]
     _libs[variant] = L
     return L
 
@@ -230,6 +233,28 @@ def bytes_per_row(m: float, uz: int, ur: int) -> float:
 
 def _last_error(L=None) -> str:
     return (L or load_library()).amp_pcg_last_error().decode("utf-8", "replace")
+
+
+def xr_update_static(alpha: float, p, q, x, r, delta_out, n: Optional[int] = None) -> None:
+    """amp_xr_update_static: x += alpha p, r -= alpha q, delta_out[0] = ||r|| (FP64 torch CUDA tensors, x and r updated
+    in place) on torch's current stream, without a handle and without any device allocation by the library — for
+    callers whose process can't cudaMalloc any more (all device memory already in their own pool) or can't afford its
+    device-wide synchronisation.  n <= XR_STATIC_MAX_N; calls that may overlap on one GPU must be ordered by the caller
+    (they share one static scratch array); make the first call on a device outside stream capture.  Asynchronous."""
+    import torch
+
+    L = load_library()
+    n = int(p.numel() if n is None else n)
+    for t in (p, q, x, r, delta_out):
+        if not (t.is_cuda and t.dtype == torch.float64 and t.is_contiguous() and t.device == x.device):
+            raise AmpPcgError("xr_update_static: contiguous float64 CUDA tensors on one device expected")
+    if min(p.numel(), q.numel(), x.numel(), r.numel()) < n or delta_out.numel() < 1:
+        raise AmpPcgError("xr_update_static: a tensor is shorter than n")
+    with torch.cuda.device(x.device):
+        rc = L.amp_xr_update_static(n, float(alpha), p.data_ptr(), q.data_ptr(), x.data_ptr(), r.data_ptr(),
+                                    delta_out.data_ptr(), torch.cuda.current_stream().cuda_stream)
+    if rc != 0:
+        raise AmpPcgError(f"amp_xr_update_static failed ({rc}): {_last_error(L)}")
 
 
 class AmpPcg:

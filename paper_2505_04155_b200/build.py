@@ -12,7 +12,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libamp_pcg.so")
-SOURCES = ["amp_pcg.cu"]
+SOURCES = ["amp_pcg.cu", "xr_static.cu"]
 HEADERS = ["common.cuh", "phases.cuh", "spmv.cuh", "spmv_pipe.cuh", "kernels.cuh", "persistent.cuh", "shard.cuh", "shard_host.cuh", "vec_pipe.cuh", "vec_fused.cuh", "async_copy.cuh"]
 
 NVCC_FLAGS = [

@@ -30,6 +30,9 @@ static void set_error(const char* fmt, ...) {
   va_end(ap);
   g_last_error = buf;
 }
+namespace amp {
+void set_error_text(const char* msg) { g_last_error = msg; }  // for the library's other translation units (xr_static.cu)
+}
 
 #define CU_TRY(call, onfail)                                                                  \
   do {                                                                                        \
