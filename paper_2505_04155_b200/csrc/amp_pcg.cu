@@ -102,6 +102,8 @@ struct amp_pcg {
   cudaGraphConditionalHandle cond_fu[2] = {};
   int use_vstage = 0;                    // bit 0: k_z and k_p, bit 1: k_xr and k_xrz are the bulk-copy staged kernels (vec_pipe.cuh)
   int shard_inline = 0;                  // the reducing kernels also collect and step (ranks run concurrently): no k_epi launches
+  bool h_state_upload_queued = false;    // an asynchronous upload of h_state may still be queued (amp_spmv_sharded returns without
+                                         // synchronising): staging_ready() waits for it before the pinned buffer is rewritten
   unsigned int shard_epoch = 0;          // sharded solves / mat-vecs made so far (identical on all ranks of the group)
   std::vector<void*> ipc_opened;         // peer allocations opened with cudaIpcOpenMemHandle
   cudaGraph_t graph_sh[2] = {nullptr, nullptr};          // [lagged] graph loops of the sharded solve
@@ -116,6 +118,15 @@ constexpr int kGraphUnroll = AMP_GRAPH_UNROLL;  // iterations per body of a grap
                                                 // about 2.7 us per evaluation)
 constexpr int64_t kVecStagedAutoMinRows = 4000000;  // AMP_VEC_AUTO stages the z and p updates from here on
 constexpr size_t kXchgBytes = sizeof(Mail) * kMailEntries + 64;
+
+// The pinned staging copy of the device state is rewritten by every solve / step / sharded mat-vec.  A call that queued an
+// upload from it and returned without synchronising must be waited for first, else the next call's host writes race with
+// the copy engine (ranks would upload different epochs and wait 10 s for halo tags that never come).
+static cudaError_t staging_ready(amp_pcg* h) {
+  if (!h->h_state_upload_queued) return cudaSuccess;
+  h->h_state_upload_queued = false;
+  return cudaStreamSynchronize(h->stream);
+}
 
 template <class T> static T* dev_alloc(amp_pcg* h, size_t count, bool zero) {
   void* p = nullptr;
@@ -524,6 +535,8 @@ extern "C" amp_pcg_t* amp_pcg_create_ex(int64_t n, int64_t nnz, const int32_t* r
       if (o.spmv_kernel == AMP_SPMV_AUTO && (double)wsum < 12.0 * (double)nsl) eligible = false;
       if (eligible) {
         cudaError_t ea = cudaFuncSetAttribute((const void*)k_spmv_pipe, cudaFuncAttributeMaxDynamicSharedMemorySize, kPipeSmemBytes);
+        if (ea == cudaSuccess)
+          ea = cudaFuncSetAttribute((const void*)k_spmv_pipe_sh, cudaFuncAttributeMaxDynamicSharedMemorySize, kPipeSmemBytes);
         if (ea != cudaSuccess) { cudaGetLastError(); eligible = false; }
       }
       if (!eligible && o.spmv_kernel == AMP_SPMV_PIPELINED) {
@@ -726,8 +739,12 @@ static void launch_spmv_any(amp_pcg* h, const void* p, void* q, unsigned int hal
     c.col_max = (int32_t)(h->n - 1);
     c.uni_noclamp = 0;
   }
-  k_spmv_any<UR, PT><<<h->spmv_grid, kSpmvThreads, 0, h->stream>>>(
-      c, static_cast<const PT*>(p), static_cast<typename Store<UR>::T*>(q), halo_seq);
+  if (halo_seq == 0u)
+    k_spmv_any<UR, PT, false><<<h->spmv_grid, kSpmvThreads, 0, h->stream>>>(
+        c, static_cast<const PT*>(p), static_cast<typename Store<UR>::T*>(q), halo_seq);
+  else  // peers store into the halo bands while the kernel may already run: coherent gathers
+    k_spmv_any<UR, PT, true><<<h->spmv_grid, kSpmvThreads, 0, h->stream>>>(
+        c, static_cast<const PT*>(p), static_cast<typename Store<UR>::T*>(q), halo_seq);
 }
 
 // halo_seq != 0 (row-sharded solve): p is the handle's own extended p vector; wait for the neighbours' push first
@@ -819,10 +836,12 @@ static cudaError_t launch_vec(amp_pcg* h, int which, cudaStream_t s, const Ctx& 
 // pdl_first: whether the first of the (up to) two kernels may start early (false when the mat-vec opens an iteration)
 static cudaError_t launch_spmv_loop(amp_pcg* h, cudaStream_t s, const Ctx& c, bool pdl, int zmode = 0, int pdl_first = -1) {
   const bool p1 = pdl_first < 0 ? pdl : pdl_first != 0;
-  cudaError_t e = (h->use_uni_kernel && zmode == 0) ? launch_loop_kernel_ex(k_spmv_uni, h->spmv_grid, kSpmvThreads, s, p1, 0, c)
-                                                    : launch_loop_kernel_ex(k_spmv, h->spmv_grid, kSpmvThreads, s, p1, 0, c, zmode);
+  const bool sh = c.sh != nullptr;  // attached to a shard group: the twins whose gathers of p are coherent loads (kernels.cuh)
+  cudaError_t e = (h->use_uni_kernel && zmode == 0)
+                      ? launch_loop_kernel_ex(sh ? k_spmv_uni_sh : k_spmv_uni, h->spmv_grid, kSpmvThreads, s, p1, 0, c)
+                      : launch_loop_kernel_ex(sh ? k_spmv_sh : k_spmv, h->spmv_grid, kSpmvThreads, s, p1, 0, c, zmode);
   if (e == cudaSuccess && h->use_pipe)
-    e = launch_loop_kernel_ex(k_spmv_pipe, h->pipe_grid, kPipeThreads, s, pdl, (size_t)kPipeSmemBytes, c, zmode);
+    e = launch_loop_kernel_ex(sh ? k_spmv_pipe_sh : k_spmv_pipe, h->pipe_grid, kPipeThreads, s, pdl, (size_t)kPipeSmemBytes, c, zmode);
   return e;
 }
 
@@ -1308,6 +1327,7 @@ extern "C" int amp_pcg_debug_step(amp_pcg_t* h, amp_debug_step_t* io, double* x)
     h->hist_cap = 64;
   }
   CU_TRY(cudaMemsetAsync(h->hist, 0, sizeof(double) * 64, st), return AMP_ERR_CUDA);
+  CU_TRY(staging_ready(h), return AMP_ERR_CUDA);
   DevState* hs = h->h_state;
   std::memset(hs, 0, sizeof(DevState));
   hs->x = x; hs->hist = h->hist;

@@ -125,8 +125,8 @@ __global__ void __launch_bounds__(kVecThreads, 2) k_p_sh(const Ctx c) {
   shard_signal_halo(c, (unsigned int)k + 1u, &s->counter[3], (int)gridDim.x);
 }
 
-__global__ void __launch_bounds__(kSpmvThreads, kSpmvMinBlocks) k_spmv(const Ctx c, int zmode) {
-  __shared__ double red[32];
+template <bool COH>
+__device__ __forceinline__ void spmv_kernel(const Ctx& c, int zmode, double* red) {
   DevState* s = c.st;
   pdl_launch_dependents();
   pdl_wait();
@@ -134,31 +134,44 @@ __global__ void __launch_bounds__(kSpmvThreads, kSpmvMinBlocks) k_spmv(const Ctx
   if (c.use_pipe && s->ur == P32) return;  // this iteration's mat-vec is k_spmv_pipe's (next in the chain)
   const int bid = blockIdx.x, nb = gridDim.x;
   if (c.sh != nullptr) shard_wait_halo(c, (unsigned int)s->k + 1u);  // the neighbours' entries of p are in the halo bands
-  const double v = dispatch_spmv<false, kSpmvThreads>(c, s->ur, s->uz, zmode, bid, nb, red);
+  const double v = dispatch_spmv<COH, kSpmvThreads>(c, s->ur, s->uz, zmode, bid, nb, red);
   if (zmode) return;  // q = A z inside M^-1: no inner product
   if (c.defer_gamma) { grid_publish<kSpmvThreads>(v, c.partials + 1 * kMaxGrid, bid, red); return; }
   grid_reduce<kSpmvThreads>(v, c.partials + 1 * kMaxGrid, &s->counter[1], bid, nb, red,
                             [&](double tot) { if (c.sh != nullptr) shard_reduce_point(c, kEpiGamma, tot, 0.0); else epi_gamma(epi_ctx(c), tot); });
 }
 
+__global__ void __launch_bounds__(kSpmvThreads, kSpmvMinBlocks) k_spmv(const Ctx c, int zmode) {
+  __shared__ double red[32];
+  spmv_kernel<false>(c, zmode, red);
+}
+// Handles attached to a shard group run the _sh twins of the three mat-vec kernels: the halo bands of p are stored by peer
+// GPUs while the kernel may already be running (it waits for their flags with ld.acquire.sys), and the PTX memory model
+// does not order a non-coherent load (ld.global.nc, __ldg) behind an acquire made by another thread: every gather of p
+// is a plain coherent load there.  Same arithmetic, same bits.
+__global__ void __launch_bounds__(kSpmvThreads, kSpmvMinBlocks) k_spmv_sh(const Ctx c, int zmode) {
+  __shared__ double red[32];
+  spmv_kernel<true>(c, zmode, red);
+}
+
 // step a4 for uniform-stencil matrices (phase_spmv_uni); takes k_spmv's place in the loop when the handle qualifies
-template <int NT>
+template <int NT, bool COH = false>
 __device__ __forceinline__ double dispatch_spmv_uni(const Ctx& c, int ur, int uz, int bid, int nb) {
   if (ur == P64) {
-    if (uz == P64) return phase_spmv_uni<P64, NT>(c, c.p64, c.p64, c.q64, bid, nb);
-    if (uz == P32) return phase_spmv_uni<P64, NT>(c, c.p32, c.p32, c.q64, bid, nb);
-    return phase_spmv_uni<P64, NT>(c, c.p16, c.p16, c.q64, bid, nb);
+    if (uz == P64) return phase_spmv_uni<P64, NT, COH>(c, c.p64, c.p64, c.q64, bid, nb);
+    if (uz == P32) return phase_spmv_uni<P64, NT, COH>(c, c.p32, c.p32, c.q64, bid, nb);
+    return phase_spmv_uni<P64, NT, COH>(c, c.p16, c.p16, c.q64, bid, nb);
   }
-  if (uz == P64) return phase_spmv_uni<P32, NT>(c, c.p32, c.p64, c.q32, bid, nb);  // gathers RN32(p) (phase_p, shadow32)
-  if (uz == P32) return phase_spmv_uni<P32, NT>(c, c.p32, c.p32, c.q32, bid, nb);
-  return phase_spmv_uni<P32, NT>(c, c.p16, c.p16, c.q32, bid, nb);
+  if (uz == P64) return phase_spmv_uni<P32, NT, COH>(c, c.p32, c.p64, c.q32, bid, nb);  // gathers RN32(p) (phase_p, shadow32)
+  if (uz == P32) return phase_spmv_uni<P32, NT, COH>(c, c.p32, c.p32, c.q32, bid, nb);
+  return phase_spmv_uni<P32, NT, COH>(c, c.p16, c.p16, c.q32, bid, nb);
 }
 
 #ifndef AMP_SPMV_UNI_BLOCKS
 #define AMP_SPMV_UNI_BLOCKS AMP_SPMV_MINBLOCKS
 #endif
-__global__ void __launch_bounds__(kSpmvThreads, AMP_SPMV_UNI_BLOCKS) k_spmv_uni(const Ctx c) {
-  __shared__ double red[32];
+template <bool COH>
+__device__ __forceinline__ void spmv_uni_kernel(const Ctx& c, double* red) {
   DevState* s = c.st;
   pdl_launch_dependents();
   pdl_wait();
@@ -166,10 +179,19 @@ __global__ void __launch_bounds__(kSpmvThreads, AMP_SPMV_UNI_BLOCKS) k_spmv_uni(
   if (c.use_pipe && s->ur == P32) return;  // this iteration's mat-vec is k_spmv_pipe's (next in the chain)
   const int bid = blockIdx.x, nb = gridDim.x;
   if (c.sh != nullptr) shard_wait_halo(c, (unsigned int)s->k + 1u);
-  const double v = dispatch_spmv_uni<kSpmvThreads>(c, s->ur, s->uz, bid, nb);
+  const double v = dispatch_spmv_uni<kSpmvThreads, COH>(c, s->ur, s->uz, bid, nb);
   if (c.defer_gamma) { grid_publish<kSpmvThreads>(v, c.partials + 1 * kMaxGrid, bid, red); return; }
   grid_reduce<kSpmvThreads>(v, c.partials + 1 * kMaxGrid, &s->counter[1], bid, nb, red,
                             [&](double tot) { if (c.sh != nullptr) shard_reduce_point(c, kEpiGamma, tot, 0.0); else epi_gamma(epi_ctx(c), tot); });
+}
+
+__global__ void __launch_bounds__(kSpmvThreads, AMP_SPMV_UNI_BLOCKS) k_spmv_uni(const Ctx c) {
+  __shared__ double red[32];
+  spmv_uni_kernel<false>(c, red);
+}
+__global__ void __launch_bounds__(kSpmvThreads, AMP_SPMV_UNI_BLOCKS) k_spmv_uni_sh(const Ctx c) {  // see k_spmv_sh
+  __shared__ double red[32];
+  spmv_uni_kernel<true>(c, red);
 }
 
 __global__ void __launch_bounds__(kVecThreads, AMP_KXR_BLOCKS) k_xr(const Ctx c) {
@@ -291,12 +313,13 @@ __global__ void __launch_bounds__(kVecThreads, 2) k_xrz(const Ctx c) {
 
 // ------------------------------------------------------------------ stand-alone SpMV --------
 // halo_seq != 0 (row-sharded solve): wait for the neighbours' halo push with that sequence number first
-template <int UR, class PT>
+// COH = true whenever a halo is waited for: the gathers are then plain coherent loads (see k_spmv_sh)
+template <int UR, class PT, bool COH = false>
 __global__ void __launch_bounds__(kSpmvThreads, kSpmvMinBlocks) k_spmv_any(const Ctx c, const PT* p, typename Store<UR>::T* q,
                                                                            unsigned int halo_seq) {
   __shared__ double red[32];
   if (halo_seq != 0u && c.sh != nullptr) shard_wait_halo(c, halo_seq);
-  (void)phase_spmv<UR, false, kSpmvThreads>(c, p, p, q, blockIdx.x, gridDim.x, red);
+  (void)phase_spmv<UR, COH, kSpmvThreads>(c, p, p, q, blockIdx.x, gridDim.x, red);
 }
 
 // ------------------------------------------------------------------ set-up / finalise -------

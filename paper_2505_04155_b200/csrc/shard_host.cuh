@@ -44,8 +44,12 @@ extern "C" int amp_shard_plan(int64_t n, const int32_t* rowptr, const int32_t* c
     out[r].halo_hi = ((cmax - (end - 1)) + 7) / 8 * 8;
     row = end;
   }
-  for (int32_t r = 0; r < world; ++r) {  // a halo must lie inside the adjacent rank (rounding may not leave the matrix either)
-    const int64_t below = r > 0 ? out[r - 1].row1 - out[r - 1].row0 : 0, above = r + 1 < world ? out[r + 1].row1 - out[r + 1].row0 : 0;
+  // a halo must lie inside the adjacent rank.  The widths are rounded up to 8 and a rank's p is zero-padded to a multiple of 8
+  // (the pushed chunks may cover the padding), so the bound is the neighbour's PADDED row count: only the last rank's can
+  // differ from its row count (the other boundaries are multiples of 32)
+  for (int32_t r = 0; r < world; ++r) {
+    const int64_t below = r > 0 ? out[r - 1].row1 - out[r - 1].row0 : 0;
+    const int64_t above = r + 1 < world ? (out[r + 1].row1 - out[r + 1].row0 + 7) / 8 * 8 : 0;
     if (r == 0) out[r].halo_lo = 0;
     if (r == world - 1) out[r].halo_hi = 0;
     if (out[r].halo_lo > below || out[r].halo_hi > above) {
@@ -114,7 +118,7 @@ static int shard_wire(amp_pcg* h, int rank, int world, const ShardPeer* peers, b
   if (rank == world - 1 && h->halo_hi != 0) { set_error("shard attach: the last rank must have halo_hi = 0"); return AMP_ERR_INVALID; }
   if (rank > 0) {  // rank-1 needs my first halo_hi(rank-1) entries in its upper band
     const ShardPeer& nb = peers[rank - 1];
-    if (nb.halo_hi > h->n || h->halo_lo > nb.n || nb.halo_hi > nb.guard || (nb.n & 31)) {
+    if (nb.halo_hi > h->npad || h->halo_lo > nb.n || nb.halo_hi > nb.guard || (nb.n & 31)) {  // npad: see amp_shard_plan
       set_error("shard attach: halo of rank %d / %d does not fit its neighbour (or %d's rows are not a multiple of 32)", rank - 1, rank, rank - 1);
       return AMP_ERR_INVALID;
     }
@@ -125,7 +129,7 @@ static int shard_wire(amp_pcg* h, int rank, int world, const ShardPeer* peers, b
   }
   if (rank + 1 < world) {  // rank+1 needs my last halo_lo(rank+1) entries in its lower band
     const ShardPeer& nb = peers[rank + 1];
-    if (nb.halo_lo > h->n || h->halo_hi > nb.n || nb.halo_lo > nb.guard || (h->n & 31)) {
+    if (nb.halo_lo > h->n || h->halo_hi > (nb.n + 7) / 8 * 8 || nb.halo_lo > nb.guard || (h->n & 31)) {
       set_error("shard attach: halo of rank %d / %d does not fit its neighbour (or %d's rows are not a multiple of 32)", rank, rank + 1, rank);
       return AMP_ERR_INVALID;
     }
@@ -331,6 +335,7 @@ extern "C" int amp_pcg_solve_sharded(amp_pcg_t* const* handles, int32_t nlocal, 
     rc = ensure_hist(h, maxit);
     if (rc != AMP_OK) return rc;
     if (mode == AMP_LOOP_GRAPH) { rc = build_graph(h, lagged, true); if (rc != AMP_OK) return rc; }
+    CU_TRY(staging_ready(h), return AMP_ERR_CUDA);
     h->shard_epoch += 1;
     fill_state(h->h_state, h, b[i], x[i], tol, maxit, pol);
     h->h_state->epoch = h->shard_epoch;
@@ -435,10 +440,12 @@ extern "C" int amp_spmv_sharded(amp_pcg_t* const* handles, int32_t nlocal, int m
     amp_pcg* h = handles[i];
     if (!p[i] || !q[i]) { set_error("amp_spmv_sharded: null vector"); return AMP_ERR_INVALID; }
     CU_TRY(cudaSetDevice(h->device), return AMP_ERR_CUDA);
+    CU_TRY(staging_ready(h), return AMP_ERR_CUDA);
     h->shard_epoch += 1;
     std::memset(h->h_state, 0, sizeof(DevState));
     h->h_state->epoch = h->shard_epoch;
     CU_TRY(cudaMemcpyAsync(h->ctx.st, h->h_state, sizeof(DevState), cudaMemcpyHostToDevice, h->stream), return AMP_ERR_CUDA);
+    h->h_state_upload_queued = true;  // this call returns without synchronising
     h->launches = 2;
   }
   FOR_RANKS(k_shard_load_p<<<h->vec_grid, kVecThreads, 0, h->stream>>>(h->ctx, p[i_], vec_prec, kHaloTagSpmv));

@@ -532,7 +532,9 @@ __device__ __forceinline__ double phase_spmv_fmt(const Ctx& c, const PT* p, cons
 // prefetch and three index formats through every pass: at 7 entries per row that bookkeeping was more than half of the
 // 267 instructions of a pass and spilled loop-carried values at the 64-register budget (ncu source page, c2).
 // Slices that are not flagged uniform (grid boundaries) take the aligned slice_sum.  Same fma chains: same bits.
-template <int UR, int NT, class PT, class PG>
+// COH: as in phase_spmv (true: p holds entries a peer GPU stored while this kernel was already running — the halo bands of a
+// sharded solve — so every gather is a plain coherent load, never ld.global.nc)
+template <int UR, int NT, bool COH = false, class PT, class PG>
 __device__ __forceinline__ double phase_spmv_uni(const Ctx& c, const PT* p, const PG* pg, typename Store<UR>::T* q, int bid, int nb) {
   using A = typename SpmvT<UR>::A;
   constexpr int G = SpmvGroup<UR>::G;
@@ -567,15 +569,15 @@ __device__ __forceinline__ double phase_spmv_uni(const Ctx& c, const PT* p, cons
     for (int g = 0; g < G; ++g) {
       const int row = (gi * G + g) * 32 + lane;
       rows[g] = (gi * G + g < nslices && row < n) ? row : -1;
-      pi[g] = gather64<false>(pg, rows[g] < 0 ? 0 : rows[g]);  // the stored p_i for gamma
+      pi[g] = gather64<COH>(pg, rows[g] < 0 ? 0 : rows[g]);  // the stored p_i for gamma
     }
     A acc[G];
     if (all_uni) {
-      if (c.uni_noclamp) narrow_uniform_sum<UR, false, G, false>(c, p, wp, lane, rows, acc);
-      else narrow_uniform_sum<UR, false, G, true>(c, p, wp, lane, rows, acc);
+      if (c.uni_noclamp) narrow_uniform_sum<UR, COH, G, false>(c, p, wp, lane, rows, acc);
+      else narrow_uniform_sum<UR, COH, G, true>(c, p, wp, lane, rows, acc);
     } else {
 #pragma unroll
-      for (int g = 0; g < G; ++g) acc[g] = slice_sum<UR, false, 2>(c, p, wp[g], wp[g + 1] - wp[g], lane, rows[g]);
+      for (int g = 0; g < G; ++g) acc[g] = slice_sum<UR, COH, 2>(c, p, wp[g], wp[g + 1] - wp[g], lane, rows[g]);
     }
 #pragma unroll
     for (int g = 0; g < G; ++g) {

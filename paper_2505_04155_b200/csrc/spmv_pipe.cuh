@@ -42,7 +42,8 @@ constexpr int kPipeSmemBytes = kPipeValueBytes + kPipeMaxStages * 4 * (kPipeBase
 constexpr int kPipeMaxGuard = 1 << 22;                       // elements of zero guard band per side we are willing to pay
 
 // gather of p[j] converted to the working type; j may be negative or >= n (guard band)
-template <class A, class PT> __device__ __forceinline__ A pipe_gather(const PT* pl, int off) { return gatherA<false>(A(0), pl, off); }
+// COH = true (sharded solve): plain coherent loads, the halo entries were stored by a peer GPU while this kernel ran
+template <bool COH, class A, class PT> __device__ __forceinline__ A pipe_gather(const PT* pl, int off) { return gatherA<COH>(A(0), pl, off); }
 
 // one slice from shared memory: this lane's row sum, ONE fma chain in stored order.
 // The quads of a slice are taken in trips of up to QT; a trip of NQ quads is straight-line code (template), so only
@@ -64,14 +65,14 @@ template <> __device__ __forceinline__ void pipe_ld_quad<double>(const double* s
   v[0] = t0.x; v[1] = t0.y; v[2] = t1.x; v[3] = t1.y;
 }
 
-template <int NQ, class A, class PT>
+template <bool COH, int NQ, class A, class PT>
 __device__ __forceinline__ A pipe_trip(const A* sv, const int* sb, int cq, int lane, const PT* pl, A acc) {
   A v[NQ][4], x[NQ][4];
 #pragma unroll
   for (int t = 0; t < NQ; ++t) {
     pipe_ld_quad<A>(sv, cq + t, lane, v[t]);
 #pragma unroll
-    for (int u = 0; u < 4; ++u) x[t][u] = pipe_gather<A>(pl, sb[4 * (cq + t) + u]);
+    for (int u = 0; u < 4; ++u) x[t][u] = pipe_gather<COH, A>(pl, sb[4 * (cq + t) + u]);
   }
 #pragma unroll
   for (int t = 0; t < NQ; ++t) {
@@ -81,13 +82,13 @@ __device__ __forceinline__ A pipe_trip(const A* sv, const int* sb, int cq, int l
   return acc;
 }
 
-template <class A, class PT>
+template <bool COH, class A, class PT>
 __device__ __forceinline__ A pipe_slice_sum(const A* sv, const int* sb, int w, int lane, const PT* pl) {
   constexpr int QT = PipeTrip<A>::QT;
   const int a = w >> 2;
   A acc = 0;
   int cq = 0;
-  for (; cq + QT <= a; cq += QT) acc = pipe_trip<QT, A, PT>(sv, sb, cq, lane, pl, acc);
+  for (; cq + QT <= a; cq += QT) acc = pipe_trip<COH, QT, A, PT>(sv, sb, cq, lane, pl, acc);
   // the last trip: fewer than QT quads, then the pair and the single of the 4a + 2b + c cut
   const bool hp = (w & 2) != 0, hs = (w & 1) != 0;
   A vp[2], xp[2], vs, xs;
@@ -99,20 +100,20 @@ __device__ __forceinline__ A pipe_slice_sum(const A* sv, const int* sb, int w, i
       const double2 t = *reinterpret_cast<const double2*>(sv + a * 128 + lane * 2);
       vp[0] = t.x; vp[1] = t.y;
     }
-    xp[0] = pipe_gather<A>(pl, sb[4 * a]);
-    xp[1] = pipe_gather<A>(pl, sb[4 * a + 1]);
+    xp[0] = pipe_gather<COH, A>(pl, sb[4 * a]);
+    xp[1] = pipe_gather<COH, A>(pl, sb[4 * a + 1]);
   }
   if (hs) {
     vs = sv[a * 128 + (hp ? 64 : 0) + lane];
-    xs = pipe_gather<A>(pl, sb[w - 1]);
+    xs = pipe_gather<COH, A>(pl, sb[w - 1]);
   }
   const int rem = a - cq;
   if constexpr (QT >= 4) {
-    if (rem == 3) acc = pipe_trip<3, A, PT>(sv, sb, cq, lane, pl, acc);
-    else if (rem == 2) acc = pipe_trip<2, A, PT>(sv, sb, cq, lane, pl, acc);
-    else if (rem == 1) acc = pipe_trip<1, A, PT>(sv, sb, cq, lane, pl, acc);
+    if (rem == 3) acc = pipe_trip<COH, 3, A, PT>(sv, sb, cq, lane, pl, acc);
+    else if (rem == 2) acc = pipe_trip<COH, 2, A, PT>(sv, sb, cq, lane, pl, acc);
+    else if (rem == 1) acc = pipe_trip<COH, 1, A, PT>(sv, sb, cq, lane, pl, acc);
   } else {
-    if (rem == 1) acc = pipe_trip<1, A, PT>(sv, sb, cq, lane, pl, acc);
+    if (rem == 1) acc = pipe_trip<COH, 1, A, PT>(sv, sb, cq, lane, pl, acc);
   }
   if (hp) { acc = fma(vp[0], xp[0], acc); acc = fma(vp[1], xp[1], acc); }
   if (hs) acc = fma(vs, xs, acc);
@@ -123,7 +124,7 @@ __device__ __forceinline__ A pipe_slice_sum(const A* sv, const int* sb, int w, i
 // entry nchunks closes the list
 struct PipeChunk { int32_t s0, w0; };
 
-template <int UR, class PT, class PG>
+template <int UR, bool COH = false, class PT, class PG>
 __device__ __forceinline__ double pipe_body(const Ctx& c, const PT* p, const PG* pg, typename Store<UR>::T* q, unsigned char* smem,
                                             unsigned int halo_seq) {
   using A = typename SpmvT<UR>::A;
@@ -185,9 +186,9 @@ __device__ __forceinline__ double pipe_body(const Ctx& c, const PT* p, const PG*
         const int w0 = sw0[sl] & ~kWptrFlags, w = (sw0[sl + 1] & ~kWptrFlags) - w0;
         const int row = sl * 32 + lane;
         const PT* pl = p + row;
-        const double pi = gather64<false>(pg, row);  // the stored p_i (u_z precision) for gamma
+        const double pi = gather64<COH>(pg, row);  // the stored p_i (u_z precision) for gamma
         A acc = 0;
-        if (w > 0) acc = pipe_slice_sum<A, PT>(sv0 + (size_t)(w0 - hd.z) * 32, sb0 + w0, w, lane, pl);
+        if (w > 0) acc = pipe_slice_sum<COH, A, PT>(sv0 + (size_t)(w0 - hd.z) * 32, sb0 + w0, w, lane, pl);
         if (row < n) {
           q[row] = acc;
           gsum = fma(pi, (double)acc, gsum);
@@ -204,31 +205,48 @@ __device__ __forceinline__ double pipe_body(const Ctx& c, const PT* p, const PG*
 // (The u_r = FP64 phases stay with the direct kernel, which already streams at the copy rate there: measured on c4,
 // 303 us direct against 327-349 us pipelined, profiles/r02.md.  Both kernels sit in the loop; the one whose phase it
 // is not returns at once.)
-__global__ void __launch_bounds__(kPipeThreads, 1) k_spmv_pipe(const Ctx c, int zmode) {
-  extern __shared__ __align__(128) unsigned char pipe_smem[];
-  __shared__ double red[32];
+template <bool COH>
+__device__ __forceinline__ void spmv_pipe_kernel(const Ctx& c, int zmode, unsigned char* pipe_smem, double* red) {
   DevState* s = c.st;
   pdl_launch_dependents();
-  // done, ur, uz were last written by the final kernel of the PREVIOUS iteration (epi_delta), which had completed
-  // before the first kernel of this iteration started (plain dependency): safe to read before the wait
+  // Single-GPU loop: done, ur, uz, k were last written by the final kernel of the PREVIOUS iteration (epi_delta), which had
+  // completed before the first kernel of this iteration started (plain dependency), and NOTHING between that kernel and
+  // this one writes them (epi_rho writes rho / beta only) — an invariant this early read rests on: safe before the wait,
+  // so the producer warp streams the matrix while the p update is still finishing.
+  // Sharded loop (COH): the block that completes a cross-rank reduction inside k_z / k_p_sh may set done and status
+  // (a peer timed out, breakdown on another rank), so there the state is read only after the predecessors have finished.
+  if (COH) pdl_wait();
   const int ur = s->ur, uz = s->uz;
   if (s->done || ur != P32) { pdl_wait(); return; }
   const unsigned int hseq = (unsigned int)s->k + 1u;
   double v;
   if (zmode) {  // q = A z inside the Chebyshev-Jacobi preconditioner
-    if (uz == P16) v = pipe_body<P32>(c, c.z16, c.z16, c.q32, pipe_smem, hseq);
-    else if (uz == P32) v = pipe_body<P32>(c, c.z32, c.z32, c.q32, pipe_smem, hseq);
-    else v = pipe_body<P32>(c, c.z64, c.z64, c.q32, pipe_smem, hseq);  // RN32(z_j) per gathered entry
+    if (uz == P16) v = pipe_body<P32, COH>(c, c.z16, c.z16, c.q32, pipe_smem, hseq);
+    else if (uz == P32) v = pipe_body<P32, COH>(c, c.z32, c.z32, c.q32, pipe_smem, hseq);
+    else v = pipe_body<P32, COH>(c, c.z64, c.z64, c.q32, pipe_smem, hseq);  // RN32(z_j) per gathered entry
     pdl_wait();
     return;
   }
-  if (uz == P16) v = pipe_body<P32>(c, c.p16, c.p16, c.q32, pipe_smem, hseq);
-  else if (uz == P32) v = pipe_body<P32>(c, c.p32, c.p32, c.q32, pipe_smem, hseq);
-  else v = pipe_body<P32>(c, c.p32, c.p64, c.q32, pipe_smem, hseq);  // gathers the FP32 copy RN32(p) written by the p update
+  if (uz == P16) v = pipe_body<P32, COH>(c, c.p16, c.p16, c.q32, pipe_smem, hseq);
+  else if (uz == P32) v = pipe_body<P32, COH>(c, c.p32, c.p32, c.q32, pipe_smem, hseq);
+  else v = pipe_body<P32, COH>(c, c.p32, c.p64, c.q32, pipe_smem, hseq);  // gathers the FP32 copy RN32(p) written by the p update
   pdl_wait();  // (the producer warp has not waited yet) before touching the reduction scratch shared with other kernels
   if (c.defer_gamma) { grid_publish<kPipeThreads>(v, c.partials + 1 * kMaxGrid, blockIdx.x, red); return; }
   grid_reduce<kPipeThreads>(v, c.partials + 1 * kMaxGrid, &s->counter[1], blockIdx.x, gridDim.x, red,
                             [&](double tot) { if (c.sh != nullptr) shard_reduce_point(c, kEpiGamma, tot, 0.0); else epi_gamma(epi_ctx(c), tot); });
+}
+
+__global__ void __launch_bounds__(kPipeThreads, 1) k_spmv_pipe(const Ctx c, int zmode) {
+  extern __shared__ __align__(128) unsigned char pipe_smem[];
+  __shared__ double red[32];
+  spmv_pipe_kernel<false>(c, zmode, pipe_smem, red);
+}
+// the same kernel for a handle attached to a shard group (c.sh != nullptr): the halo bands of p are filled by peer GPUs
+// while this kernel may already be running, and ld.global.nc is not ordered behind the acquire of the halo flag
+__global__ void __launch_bounds__(kPipeThreads, 1) k_spmv_pipe_sh(const Ctx c, int zmode) {
+  extern __shared__ __align__(128) unsigned char pipe_smem[];
+  __shared__ double red[32];
+  spmv_pipe_kernel<true>(c, zmode, pipe_smem, red);
 }
 
 }  // namespace amp

@@ -214,3 +214,46 @@ def test_attach_through_export_blobs_single_rank():
             A.ShardGroup.attach_ipc(h, 0, [bytes(bad)])
     finally:
         g.close()
+
+
+@pytest.mark.parametrize("n", [70, 67, 203])
+def test_sharded_halo_wider_than_the_last_rank(n):
+    """n not a multiple of 8 and a coupling that reaches the last row: the rounded halo of rank 0 is wider than rank 1's
+    row count (n = 70: 6 rows, halo 8), so the push covers rank 1's zero padding.  Two mat-vecs in a row (the second call
+    re-uses the pinned state staging while the first one's upload may still be queued), then a solve, then a mat-vec."""
+    import types
+
+    sp = pytest.importorskip("scipy.sparse")
+    rng = np.random.default_rng(5)
+    M = sp.random(n, n, density=0.08, random_state=rng, format="lil")
+    for bnd in range(32, n, 32):
+        M[bnd - 1, n - 1] = 0.25
+        M[bnd, 0] = 0.25
+    M = (M + M.T).tocsr()
+    M = (M + sp.diags(np.asarray(abs(M).sum(axis=1)).ravel() + 1.0)).tocsr()
+    M.sort_indices()
+    s = types.SimpleNamespace(n=n, rowptr=M.indptr.astype(np.int32), colidx=M.indices.astype(np.int32),
+                              vals=M.data.astype(np.float64), b=rng.uniform(-1, 1, n))
+    g, parts = make_group(s, 2)
+    try:
+        rows1 = parts[1][1] - parts[1][0]
+        assert rows1 % 8 != 0 and A.shard_plan(s.rowptr, s.colidx, 2)[0].halo_hi > rows1
+        rp, ci, va = (torch.from_numpy(a).cuda() for a in (s.rowptr, s.colidx, s.vals))
+        b = torch.from_numpy(s.b).cuda()
+        with A.AmpPcg(rp, ci, va) as whole:
+            for rep in range(2):
+                p64 = torch.from_numpy(rng.uniform(-1, 1, n)).cuda()
+                for vec_dt in (torch.float64, torch.float32):
+                    p = p64.to(vec_dt)
+                    for mat in (A.FP64, A.FP32):
+                        q1 = g.spmv(split(p, parts), mat)       # back to back, no synchronisation in between
+                        q2 = g.spmv(split(p, parts), mat)
+                        assert torch.equal(torch.cat(q1), whole.spmv(p, mat)) and torch.equal(torch.cat(q2), torch.cat(q1))
+                spec = POLICY_SPECS["amp_fp64_delay"]
+                ref = O.amp_pcg(s.rowptr, s.colidx, s.vals, s.b, 1e-10, 500, oracle_policy(spec))
+                xs = [torch.zeros(bb - aa, dtype=torch.float64, device="cuda") for aa, bb in parts]
+                st = g.solve(split(b, parts), xs, 1e-10, 500, cuda_policy(spec, x0_zero=1))[0]
+                assert st.status == ref.status == 0 and abs(st.iters - ref.iters) <= 1, (st.status, st.iters, ref.iters)
+                assert st.relres_true <= 2e-10
+    finally:
+        g.close()

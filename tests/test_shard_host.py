@@ -87,6 +87,39 @@ def test_plan_refuses_a_coupling_that_is_not_banded(A):
         A.shard_plan(Amat.indptr.astype(np.int32), Amat.indices.astype(np.int32), 9)
 
 
+def _full_reach_band(n, seed=5):
+    """SPD test matrix whose rows around the rank boundary reach every row of the neighbour rank (a halo as wide as the rank)"""
+    rng = np.random.default_rng(seed)
+    M = sp.random(n, n, density=0.08, random_state=rng, format="lil")
+    for b in range(32, n, 32):   # wherever the planner puts the rank boundary (a multiple of 32):
+        M[b - 1, n - 1] = 0.25   # the last row below it reaches the LAST row of the matrix
+        M[b, 0] = 0.25           # and the first row above it reaches row 0
+    M = (M + M.T).tocsr()
+    M = (M + sp.diags(np.asarray(abs(M).sum(axis=1)).ravel() + 1.0)).tocsr()
+    M.sort_indices()
+    return M
+
+
+@pytest.mark.parametrize("n", [70, 67, 100])
+def test_plan_accepts_a_rounded_halo_inside_the_padded_last_rank(A, n):
+    """n not a multiple of 8 with a coupling that reaches the last row: the halo width rounded up to 8 exceeds the last rank's
+    row count but not its zero-padded length, which is what the exchange pushes (n = 70: rank 1 has 38 rows, halo 40)"""
+    M = _full_reach_band(n)
+    rp, ci = M.indptr.astype(np.int32), M.indices.astype(np.int32)
+    plan = A.shard_plan(rp, ci, 2)
+    assert plan[0].row1 % 32 == 0 and plan[1].row1 == n
+    rows0, rows1 = plan[0].row1, n - plan[0].row1
+    assert rows1 % 8 != 0
+    assert plan[0].halo_hi == (rows1 + 7) // 8 * 8 and plan[0].halo_hi > rows1     # wider than the neighbour's row count
+    assert plan[1].halo_lo == rows0 and plan[0].halo_lo == 0 and plan[1].halo_hi == 0
+    blocks = []
+    for sh in plan:
+        r_, c_, v_ = A.shard_extract(rp, ci, M.data, sh)
+        assert c_.min() >= 0 and c_.max() < sh.halo_lo + (sh.row1 - sh.row0) + sh.halo_hi
+        blocks.append(sp.csr_matrix((v_, c_.astype(np.int64) - sh.halo_lo + sh.row0, r_), shape=(sh.row1 - sh.row0, n)))
+    assert (sp.vstack(blocks).tocsr() != M).nnz == 0
+
+
 # ------------------------------------------------------------------ the sharded loop over gloo, oracle arithmetic ----
 def _free_port() -> int:
     with socket.socket() as s:
