@@ -30,6 +30,12 @@ POLICIES = {
     "amp_fp64_delay": dict(amp=1, u0=O.FP64, eta_rule=O.ETA_DELAY),
     "amp_fp16_linear": dict(amp=1, u0=O.FP16, eta_rule=O.ETA_LINEAR),
     "amp_fp64_delay_strict": dict(amp=1, u0=O.FP64, eta_rule=O.ETA_DELAY, eta_safety=0.1, stop_safety=0.9),
+    # the (3.10) split "switch at eta <= theta tol ||b||, stop at ||r|| <= (1 - theta) tol ||b||" for
+    # other theta: the sweep behind bench.py's choice of the headline policy (rule: true relres <= tol on c2-c4, then the
+    # fewest iterations with the FP64 matrix + extra iterations at the end; reading R12)
+    "amp_fp64_delay_strict_t02": dict(amp=1, u0=O.FP64, eta_rule=O.ETA_DELAY, eta_safety=0.2, stop_safety=0.8),
+    "amp_fp64_delay_strict_t03": dict(amp=1, u0=O.FP64, eta_rule=O.ETA_DELAY, eta_safety=0.3, stop_safety=0.7),
+    "amp_fp64_delay_strict_t05": dict(amp=1, u0=O.FP64, eta_rule=O.ETA_DELAY, eta_safety=0.5, stop_safety=0.5),
     "amp_fp64_delay_lagged": dict(amp=1, u0=O.FP64, eta_rule=O.ETA_DELAY, scale_mode=O.SCALE_LAGGED),
     # omega = sqrt(n)/||r_k|| ("other scaling factors can be used"): the evidence for the scaling
     # decision of DESIGN.md section 2 (reading R10) — FP16 subnormal exposure and iteration counts at full size

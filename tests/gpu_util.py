@@ -12,6 +12,9 @@ POLICY_SPECS = {
     "amp_fp64_delay": dict(amp=1, u0=0, eta_rule=0),
     "amp_fp16_linear": dict(amp=1, u0=2, eta_rule=1),
     "amp_fp64_delay_strict": dict(amp=1, u0=0, eta_rule=0, eta_safety=0.1, stop_safety=0.9),
+    "amp_fp64_delay_strict_t02": dict(amp=1, u0=0, eta_rule=0, eta_safety=0.2, stop_safety=0.8),
+    "amp_fp64_delay_strict_t03": dict(amp=1, u0=0, eta_rule=0, eta_safety=0.3, stop_safety=0.7),  # bench.py's headline policy
+    "amp_fp64_delay_strict_t05": dict(amp=1, u0=0, eta_rule=0, eta_safety=0.5, stop_safety=0.5),
     "amp_fp32_never": dict(amp=1, u0=1, eta_rule=2),
     "amp_fp64_rms": dict(amp=1, u0=0, eta_rule=0, scale_mode=1),
     "amp_fp64_pow2": dict(amp=1, u0=0, eta_rule=0, scale_mode=2),

@@ -54,6 +54,22 @@ def test_full_size_against_oracle_golden(name):
         q32 = h.spmv(p16, A.FP32).cpu().numpy()
         q32_ref = O.spmv_fp32(s.rowptr, s.colidx, s.vals, p16[:s.n].cpu().numpy().astype(np.float64))
         assert np.array_equal(q32.astype(np.float64), q32_ref)
+        # the IN-LOOP mat-vec kernels (k_spmv / k_spmv_uni / k_spmv_pipe through amp_pcg_debug_step, not the stand-alone
+        # k_spmv_any above) over the whole vector at full size — the full grid of k_spmv_uni, every round of k_spmv_pipe's
+        # stage ring (31 on c4): q bit for bit, gamma = q^T p to reduction accuracy (Alg 4.1 lines 11-13)
+        if name in ("c2", "c3", "c4"):
+            rnd = {0: lambda a: a, 2: lambda a: a.astype(np.float16).astype(np.float64)}
+            tdt = {0: torch.float64, 1: torch.float32, 2: torch.float16}
+            for ur, uz in ((0, 0), (1, 0), (1, 2)):
+                pz = rnd[uz](p)
+                q_ref = O.spmv_fp64(s.rowptr, s.colidx, s.vals, pz) if ur == 0 else O.spmv_fp32(s.rowptr, s.colidx, s.vals, pz)
+                h.debug_set_vector(A.VEC_P, torch.from_numpy(pz).cuda().to(tdt[uz]))
+                h.debug_set_vector(A.VEC_Q, torch.full((s.n,), 7.0, dtype=tdt[ur], device="cuda"))
+                io = h.debug_step(A.STEP_SPMV, rs=ur, ur=ur, uz=uz, ps=uz, ur_n=ur, uz_n=uz)
+                q_in = h.debug_get_vector(A.VEC_Q, ur).cpu().numpy().astype(np.float64)
+                assert np.array_equal(q_in, q_ref), (name, ur, uz, int((q_in != q_ref).sum()))
+                bound = s.n * 2.0 ** -53 * float(np.abs(q_ref * pz).sum())
+                assert abs(io.sum0 - O.dot(q_ref, pz)) <= bound, (name, ur, uz, io.sum0)
         # independent FP64 mat-vec for the true residual
         crow = rp.to(torch.int64)
         At = torch.sparse_csr_tensor(crow, ci.to(torch.int64), va, size=(s.n, s.n))
